@@ -1,0 +1,551 @@
+// tpc_oracle.cpp -- plain single-threaded CPU ORACLE of the TPC sector tracker (test infrastructure).
+//
+// Follows DESIGN.md section 3 (formula sheet = SURVEY.md 8(c) readings R0..R27 of BASELINE.json
+// north_star; PAPER.md itself gives no algorithmic detail, see tpc_oracle.h) step by step:
+//   O1 grid, O2 neighbour finder, O3 cleaner + start hits, O4 tracklet constructor, O5 selector.
+// No blocking, fusion or reordering.  Shares no code with the CUDA path.
+//
+// Build: g++ -O2 -ffp-contract=off -fno-fast-math -shared -fPIC tpc_oracle.cpp -o libtpcoracle.so
+// (R0: one IEEE rounding per written operation, no FMA contraction, no reassociation.)
+#include "tpc_oracle.h"
+
+#include <cmath>
+#include <cstring>
+#include <vector>
+
+namespace {
+
+inline int tri(int i, int j) { return i * (i + 1) / 2 + j; }   // i >= j, order 00,10,11,20,21,22,...
+
+template <typename Real>
+struct State {
+  Real x, y, z, s, t, q;   // p = (y, z, sin(phi), dz/ds, q/pT) at plane x          (O4 "State")
+  Real C[15];
+  Real chi2;
+};
+
+// ---- O4 Propagate(dx): exact circle in the bend plane, series arc length; C <- F C F^T ------------
+template <typename Real>
+bool propagate(State<Real>& st, Real xnew, Real b, Real max_sinphi) {
+  const Real dx = xnew - st.x;
+  const Real s = st.s, t = st.t;
+  const Real k = st.q * b;
+  const Real s1 = s + dx * k;
+  if (!(std::fabs(s) < max_sinphi) || !(std::fabs(s1) < max_sinphi)) return false;
+  const Real one = 1;
+  const Real c0 = std::sqrt(one - s * s);
+  const Real c1 = std::sqrt(one - s1 * s1);
+  const Real T = (s + s1) / (c0 + c1);
+  const Real y1 = st.y + dx * T;
+  const Real dl = dx * std::sqrt(one + T * T);
+  const Real kd = k * dl;
+  const Real a2 = kd * kd;
+  const Real c24 = (Real)(1.0 / 24.0), c640 = (Real)(3.0 / 640.0), c6 = (Real)(1.0 / 6.0);
+  const Real dS = dl * (one + a2 * c24 + a2 * a2 * c640);
+  const Real z1 = st.z + t * dS;
+  const Real cc = one + s * s1 + c0 * c1;
+  const Real csum = c0 + c1;
+  const Real c0c1 = c0 * c1;
+  const Real Fys = dx * cc / (c0c1 * csum);
+  const Real Fyq = dx * dx * b * cc / (c1 * csum * csum);
+  const Real Fsq = dx * b;
+  const Real Fzt = dS;
+  const Real Fzs = t * dx * T / c0c1;
+  const Real sm = (Real)0.5 * (s + s1);
+  const Real cm = std::sqrt(one - sm * sm);
+  const Real Fzq = t * b * dx * dx * c6 * ((Real)2 * sm / (cm * cm * cm) + s1 / (c1 * c1 * c1));
+  // M = F C (full 5x5), F = I + {Fys(0,2), Fyq(0,4), Fzs(1,2), Fzt(1,3), Fzq(1,4), Fsq(2,4)}
+  Real Cf[5][5], M[5][5];
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j < 5; ++j) Cf[i][j] = st.C[i >= j ? tri(i, j) : tri(j, i)];
+  for (int j = 0; j < 5; ++j) {
+    M[0][j] = Cf[0][j] + Fys * Cf[2][j] + Fyq * Cf[4][j];
+    M[1][j] = Cf[1][j] + Fzs * Cf[2][j] + Fzt * Cf[3][j] + Fzq * Cf[4][j];
+    M[2][j] = Cf[2][j] + Fsq * Cf[4][j];
+    M[3][j] = Cf[3][j];
+    M[4][j] = Cf[4][j];
+  }
+  // C' = M F^T, lower triangle
+  for (int i = 0; i < 5; ++i) {
+    st.C[tri(i, 0)] = M[i][0] + M[i][2] * Fys + M[i][4] * Fyq;
+    if (i >= 1) st.C[tri(i, 1)] = M[i][1] + M[i][2] * Fzs + M[i][3] * Fzt + M[i][4] * Fzq;
+    if (i >= 2) st.C[tri(i, 2)] = M[i][2] + M[i][4] * Fsq;
+    if (i >= 3) st.C[tri(i, 3)] = M[i][3];
+    if (i >= 4) st.C[tri(i, 4)] = M[i][4];
+  }
+  st.x = xnew; st.y = y1; st.z = z1; st.s = s1;
+  return true;
+}
+
+// ---- O4 Update: sequential scalar updates, y (m=0) then z (m=1); guards R12 ------------------------
+template <typename Real>
+bool update(State<Real>& st, Real ym, Real zm, Real err2_y, Real err2_z) {
+  Real p[5] = {st.y, st.z, st.s, st.t, st.q};
+  Real C[15];
+  for (int i = 0; i < 15; ++i) C[i] = st.C[i];
+  Real chi2 = st.chi2;
+  for (int m = 0; m < 2; ++m) {
+    const Real v = m == 0 ? ym : zm;
+    const Real r = m == 0 ? err2_y : err2_z;
+    Real Cm[5], K[5];
+    for (int j = 0; j < 5; ++j) Cm[j] = C[j >= m ? tri(j, m) : tri(m, j)];
+    const Real S = Cm[m] + r;
+    for (int i = 0; i < 5; ++i) K[i] = Cm[i] / S;
+    const Real rho = v - p[m];
+    for (int i = 0; i < 5; ++i) p[i] = p[i] + K[i] * rho;
+    for (int i = 0; i < 5; ++i)
+      for (int j = 0; j <= i; ++j) C[tri(i, j)] = C[tri(i, j)] - K[i] * Cm[j];
+    chi2 = chi2 + rho * rho / S;
+  }
+  for (int i = 0; i < 5; ++i)
+    if (!(C[tri(i, i)] > (Real)0)) return false;
+  for (int i = 0; i < 5; ++i)
+    if (!std::isfinite(p[i])) return false;
+  for (int i = 0; i < 15; ++i)
+    if (!std::isfinite(C[i])) return false;
+  if (!std::isfinite(chi2)) return false;
+  st.y = p[0]; st.z = p[1]; st.s = p[2]; st.t = p[3]; st.q = p[4];
+  for (int i = 0; i < 15; ++i) st.C[i] = C[i];
+  st.chi2 = chi2;
+  return true;
+}
+
+template <typename Real>
+struct Tracklet {
+  int status = 0;   // 0 discarded in chain fit, 1 rejected, 2 accepted
+  int nhits = 0, first_row = -1, last_row = -1;
+  State<Real> st{};
+  std::vector<int32_t> rowhit;
+};
+
+struct Grid {   // O1, one per (sector,row) bucket
+  float y0 = 0, z0 = 0, inv_e = 0;
+  int ny = 0, nz = 0;
+  std::vector<uint32_t> cell_start;   // [ny*nz+1], positions into sorted (bucket-local)
+};
+
+}  // namespace
+
+struct orcResult {
+  int64_t n = 0;
+  int n_sectors = 0, n_rows = 0;
+  bool fp64 = false, brute = false;
+  std::vector<uint32_t> sorted_to_orig;
+  std::vector<int32_t> cell_of_sorted, n_cells;
+  std::vector<int32_t> up_raw, dn_raw, up, dn;
+  std::vector<uint32_t> start_hits;
+  // tracklets (stored as double regardless of Real)
+  std::vector<int32_t> tl_status, tl_nhits, tl_first, tl_last, tl_rowhit;
+  std::vector<double> tl_x, tl_par, tl_cov, tl_chi2;
+  // tracks
+  std::vector<int32_t> tr_id, tr_sector, tr_first, tr_last, tr_ncl;
+  std::vector<double> tr_x, tr_par, tr_cov, tr_chi2;
+  std::vector<uint32_t> tr_cl_offset, tr_cl_index;
+};
+
+namespace {
+
+template <typename Real>
+struct Tracker {
+  const orcGeometry& g;
+  const orcParams& P;
+  const int64_t N;
+  const uint32_t* off;
+  const bool brute;
+  const int R, S;
+  std::vector<Real> Y, Z, X;           // cluster coords; row x
+  std::vector<int32_t> rowOf, secOf;   // per cluster (R26: recovered from row_offset)
+  std::vector<int> upRow, dnRow;       // R2
+  std::vector<Grid> grids;
+  std::vector<uint32_t> sorted;        // sorted_to_orig
+  orcResult& res;
+
+  Tracker(const orcGeometry& g_, const orcParams& p_, int64_t n, const uint32_t* off_, const float* y, const float* z,
+          bool brute_, orcResult& r)
+      : g(g_), P(p_), N(n), off(off_), brute(brute_), R(g_.n_rows), S(g_.n_sectors), res(r) {
+    Y.resize(N); Z.resize(N); rowOf.resize(N); secOf.resize(N);
+    for (int64_t i = 0; i < N; ++i) { Y[i] = (Real)y[i]; Z[i] = (Real)z[i]; }
+    for (int s = 0; s < S; ++s)
+      for (int r = 0; r < R; ++r)
+        for (uint32_t i = off[s * R + r]; i < off[s * R + r + 1]; ++i) { rowOf[i] = r; secOf[i] = s; }
+    X.resize(R);
+    for (int r = 0; r < R; ++r) X[r] = (Real)g.row_x[r];
+    // R2: up(r) = first live row among (r+1, r+2); dn(r) = first live row among (r-1, r-2)
+    upRow.assign(R, -1); dnRow.assign(R, -1);
+    for (int r = 0; r < R; ++r) {
+      if (dead(r)) continue;
+      for (int k = 1; k <= 2; ++k) if (r + k < R && !dead(r + k)) { upRow[r] = r + k; break; }
+      for (int k = 1; k <= 2; ++k) if (r - k >= 0 && !dead(r - k)) { dnRow[r] = r - k; break; }
+    }
+  }
+  bool dead(int r) const { return g.row_dead && g.row_dead[r]; }
+
+  // ---- O1 ----------------------------------------------------------------------------------------
+  int cellCoord(float v, float v0, float inv_e, int n) const {
+    float f = std::floor((v - v0) * inv_e);
+    if (!(f >= 0.0f)) return 0;
+    if (f > (float)(n - 1)) return n - 1;
+    return (int)f;
+  }
+  void buildGrid() {
+    grids.resize((size_t)S * R);
+    sorted.resize(N);
+    res.cell_of_sorted.assign(N, 0);
+    res.n_cells.assign((size_t)S * R, 0);
+    for (int b = 0; b < S * R; ++b) {
+      const int r = b % R;
+      const uint32_t lo = off[b], hi = off[b + 1], n = hi - lo;
+      Grid& G = grids[b];
+      const float hw = g.row_x[r] * g.tan_half_sector;
+      const float Wy = 2.0f * hw, Wz = g.z_max - g.z_min;
+      float e = n > 0 ? std::sqrt(Wy * Wz / (float)n) : P.cell_max;
+      if (e < P.cell_min) e = P.cell_min;
+      if (e > P.cell_max) e = P.cell_max;
+      G.y0 = -hw; G.z0 = g.z_min; G.inv_e = 1.0f / e;
+      G.ny = (int)std::ceil(Wy / e); G.nz = (int)std::ceil(Wz / e);
+      if (G.ny < 1) G.ny = 1;
+      if (G.nz < 1) G.nz = 1;
+      const int nc = G.ny * G.nz;
+      res.n_cells[b] = nc;
+      G.cell_start.assign(nc + 1, 0);
+      std::vector<int> cell(n);
+      for (uint32_t i = 0; i < n; ++i) {
+        int by = cellCoord((float)Y[lo + i], G.y0, G.inv_e, G.ny);
+        int bz = cellCoord((float)Z[lo + i], G.z0, G.inv_e, G.nz);
+        cell[i] = bz * G.ny + by;
+        G.cell_start[cell[i] + 1]++;
+      }
+      for (int c = 0; c < nc; ++c) G.cell_start[c + 1] += G.cell_start[c];
+      std::vector<uint32_t> cur(G.cell_start.begin(), G.cell_start.end() - 1);
+      for (uint32_t i = 0; i < n; ++i) {   // stable counting sort
+        uint32_t pos = lo + cur[cell[i]]++;
+        sorted[pos] = lo + i;
+        res.cell_of_sorted[pos] = cell[i];
+      }
+    }
+    res.sorted_to_orig = sorted;
+  }
+
+  // R3: a search is DEFINED as the predicate over all clusters of the bucket; the grid only enumerates a superset.
+  template <typename F>
+  void forWindow(int b, Real yc, Real zc, Real wy, Real wz, F&& f) const {
+    const uint32_t lo = off[b], hi = off[b + 1];
+    if (brute) {
+      for (uint32_t i = lo; i < hi; ++i)
+        if (std::fabs(Y[i] - yc) <= wy && std::fabs(Z[i] - zc) <= wz) f((int32_t)i);
+      return;
+    }
+    if (hi == lo) return;
+    const Grid& G = grids[b];
+    // slack covers the rounding of the predicate's subtraction (superset only; predicate decides)
+    const float sy = 1e-5f * ((float)std::fabs(yc) + (float)wy) + 1e-6f;
+    const float sz = 1e-5f * ((float)std::fabs(zc) + (float)wz) + 1e-6f;
+    const int by0 = cellCoord((float)(yc - wy) - sy, G.y0, G.inv_e, G.ny);
+    const int by1 = cellCoord((float)(yc + wy) + sy, G.y0, G.inv_e, G.ny);
+    const int bz0 = cellCoord((float)(zc - wz) - sz, G.z0, G.inv_e, G.nz);
+    const int bz1 = cellCoord((float)(zc + wz) + sz, G.z0, G.inv_e, G.nz);
+    for (int bz = bz0; bz <= bz1; ++bz)
+      for (uint32_t k = G.cell_start[bz * G.ny + by0]; k < G.cell_start[bz * G.ny + by1 + 1]; ++k) {
+        const uint32_t i = sorted[lo + k];
+        if (std::fabs(Y[i] - yc) <= wy && std::fabs(Z[i] - zc) <= wz) f((int32_t)i);
+      }
+  }
+
+  // ---- O2 ----------------------------------------------------------------------------------------
+  void findNeighbours() {
+    res.up_raw.assign(N, -1); res.dn_raw.assign(N, -1);
+    std::vector<int32_t> U, D;
+    std::vector<Real> tyu, tzu, tyd, tzd;
+    for (int64_t h = 0; h < N; ++h) {
+      const int r = rowOf[h], s = secOf[h];
+      if (dead(r)) continue;
+      const int ru = upRow[r], rd = dnRow[r];
+      if (ru < 0 || rd < 0) continue;
+      const Real dxu = X[ru] - X[r], dxd = X[r] - X[rd];
+      const Real iu = (Real)1 / dxu, id = (Real)1 / dxd;
+      const Real wyu = (Real)P.area_y * dxu, wzu = (Real)P.area_z * dxu;
+      const Real wyd = (Real)P.area_y * dxd, wzd = (Real)P.area_z * dxd;
+      U.clear(); D.clear(); tyu.clear(); tzu.clear(); tyd.clear(); tzd.clear();
+      forWindow(s * R + ru, Y[h], Z[h], wyu, wzu, [&](int32_t u) { U.push_back(u); });
+      forWindow(s * R + rd, Y[h], Z[h], wyd, wzd, [&](int32_t d) { D.push_back(d); });
+      if (U.empty() || D.empty()) continue;
+      for (int32_t u : U) { tyu.push_back((Y[u] - Y[h]) * iu); tzu.push_back((Z[u] - Z[h]) * iu); }
+      for (int32_t d : D) { tyd.push_back((Y[h] - Y[d]) * id); tzd.push_back((Z[h] - Z[d]) * id); }
+      bool have = false;
+      Real best = 0; int32_t bu = -1, bd = -1;
+      for (size_t a = 0; a < U.size(); ++a)
+        for (size_t c = 0; c < D.size(); ++c) {
+          const Real ey = tyu[a] - tyd[c], ez = tzu[a] - tzd[c];
+          const Real dev = ey * ey + ez * ez;
+          // R6: lexicographic key (Dev, orig(u), orig(d))
+          bool better = !have || dev < best ||
+                        (dev == best && (U[a] < bu || (U[a] == bu && D[c] < bd)));
+          if (better) { have = true; best = dev; bu = U[a]; bd = D[c]; }
+        }
+      if (have && best <= (Real)P.link_dev2_max) { res.up_raw[h] = bu; res.dn_raw[h] = bd; }
+    }
+  }
+
+  // ---- O3 ----------------------------------------------------------------------------------------
+  void cleanAndStart() {
+    res.up.assign(N, -1); res.dn.assign(N, -1);
+    for (int64_t h = 0; h < N; ++h) {
+      const int32_t u = res.up_raw[h], d = res.dn_raw[h];
+      res.up[h] = (u >= 0 && res.dn_raw[u] == (int32_t)h) ? u : -1;
+      res.dn[h] = (d >= 0 && res.up_raw[d] == (int32_t)h) ? d : -1;
+    }
+    res.start_hits.clear();
+    for (int64_t h = 0; h < N; ++h)
+      if (res.dn[h] == -1 && res.up[h] != -1) res.start_hits.push_back((uint32_t)h);
+  }
+
+  // ---- O4 ----------------------------------------------------------------------------------------
+  int32_t search(int b, const State<Real>& st) const {
+    Real ry = (Real)P.road_sigma * std::sqrt(st.C[0] + (Real)P.err2_y);
+    Real rz = (Real)P.road_sigma * std::sqrt(st.C[2] + (Real)P.err2_z);
+    if (!(ry >= (Real)P.road_min)) ry = (Real)P.road_min;
+    if (ry > (Real)P.road_max) ry = (Real)P.road_max;
+    if (!(rz >= (Real)P.road_min)) rz = (Real)P.road_min;
+    if (rz > (Real)P.road_max) rz = (Real)P.road_max;
+    int32_t best = -1; Real bestd = 0;
+    forWindow(b, st.y, st.z, ry, rz, [&](int32_t c) {
+      const Real dy = Y[c] - st.y, dz = Z[c] - st.z;
+      const Real d2 = dy * dy + dz * dz;
+      if (best < 0 || d2 < bestd || (d2 == bestd && c < best)) { best = c; bestd = d2; }
+    });
+    return best;
+  }
+
+  void setDiag(State<Real>& st, Real vy, Real vz) const {
+    for (int i = 0; i < 15; ++i) st.C[i] = 0;
+    st.C[tri(0, 0)] = vy; st.C[tri(1, 1)] = vz;
+    st.C[tri(2, 2)] = (Real)P.init_var_s; st.C[tri(3, 3)] = (Real)P.init_var_t; st.C[tri(4, 4)] = (Real)P.init_var_q;
+  }
+
+  void construct(uint32_t h0, Tracklet<Real>& T) const {
+    const Real b = (Real)(0.00299792458 * (double)g.bz_tesla);
+    const Real msp = (Real)P.max_sinphi, e2y = (Real)P.err2_y, e2z = (Real)P.err2_z;
+    const int s = secOf[h0], r0 = rowOf[h0];
+    const int32_t h1 = res.up[h0];
+    const int r1 = rowOf[h1];
+    T.rowhit.assign(R, -1);
+    State<Real>& st = T.st;
+    // 1. init from the first link
+    st.x = X[r0]; st.y = Y[h0]; st.z = Z[h0];
+    {
+      const Real dx = X[r1] - X[r0], dy = Y[h1] - Y[h0], dz = Z[h1] - Z[h0];
+      const Real L = std::sqrt(dx * dx + dy * dy);
+      st.s = dy / L; st.t = dz / L; st.q = 0;
+    }
+    setDiag(st, e2y, e2z);
+    st.chi2 = 0;
+    T.rowhit[r0] = (int32_t)h0;
+    int nhits = 1, rc = r0;
+    // 2. chain fit
+    for (int32_t h = h1; h != -1;) {
+      const int r = rowOf[h];
+      if (!propagate(st, X[r], b, msp)) break;
+      rc = r;
+      if (!update(st, Y[h], Z[h], e2y, e2z)) break;
+      T.rowhit[r] = h; ++nhits;
+      h = res.up[h];
+    }
+    if (nhits < P.min_chain_hits) { T.status = 0; T.nhits = nhits; return; }
+    // 3. up-extrapolation
+    int miss = 0;
+    for (int r = rc + 1; r < R; ++r) {
+      if (dead(r)) continue;                       // R23
+      if (!propagate(st, X[r], b, msp)) break;
+      const int32_t c = search(s * R + r, st);
+      if (c >= 0) {
+        if (!update(st, Y[c], Z[c], e2y, e2z)) break;
+        T.rowhit[r] = c; ++nhits; miss = 0;
+      } else if (++miss > P.max_row_gap) break;
+    }
+    // 4. turn (R17)
+    setDiag(st, (Real)P.turn_var_scale * e2y, (Real)P.turn_var_scale * e2z);
+    st.chi2 = 0;
+    int rtop = -1;
+    for (int r = R - 1; r >= 0; --r) if (T.rowhit[r] != -1) { rtop = r; break; }
+    // 5. down pass
+    int nh = 0, snap_row = -1, snap_nh = 0;
+    State<Real> snap{};
+    miss = 0;
+    for (int r = rtop; r >= 0; --r) {
+      if (dead(r)) continue;
+      if (!propagate(st, X[r], b, msp)) break;
+      int32_t c = T.rowhit[r];
+      const bool known = c != -1;
+      if (!known) c = search(s * R + r, st);
+      if (c >= 0) {
+        if (!update(st, Y[c], Z[c], e2y, e2z)) break;
+        if (!known) T.rowhit[r] = c;
+        ++nh; snap = st; snap_row = r; snap_nh = nh;
+        if (r < r0) miss = 0;
+      } else if (r < r0) {
+        if (++miss > P.max_row_gap) break;
+      }
+    }
+    // 6. output = last snapshot
+    if (snap_row < 0) { T.status = 1; T.nhits = 0; for (auto& v : T.rowhit) v = -1; return; }
+    for (int r = 0; r < snap_row; ++r) T.rowhit[r] = -1;
+    T.st = snap; T.nhits = snap_nh; T.first_row = snap_row; T.last_row = rtop;
+    T.status = snap_nh >= P.min_tracklet_hits ? 2 : 1;
+  }
+
+  void run() {
+    if (!brute) buildGrid();
+    findNeighbours();
+    cleanAndStart();
+    const int64_t ns = (int64_t)res.start_hits.size();
+    res.tl_status.assign(ns, 0); res.tl_nhits.assign(ns, 0); res.tl_first.assign(ns, -1); res.tl_last.assign(ns, -1);
+    res.tl_rowhit.assign((size_t)ns * R, -1);
+    res.tl_x.assign(ns, 0); res.tl_par.assign((size_t)ns * 5, 0); res.tl_cov.assign((size_t)ns * 15, 0);
+    res.tl_chi2.assign(ns, 0);
+    std::vector<Real> chi2r(ns, 0);
+    for (int64_t t = 0; t < ns; ++t) {
+      Tracklet<Real> T;
+      construct(res.start_hits[t], T);
+      res.tl_status[t] = T.status; res.tl_nhits[t] = T.nhits; res.tl_first[t] = T.first_row; res.tl_last[t] = T.last_row;
+      if (T.status == 0) continue;
+      for (int r = 0; r < R; ++r) res.tl_rowhit[(size_t)t * R + r] = T.rowhit[r];
+      res.tl_x[t] = (double)T.st.x;
+      const Real p[5] = {T.st.y, T.st.z, T.st.s, T.st.t, T.st.q};
+      for (int i = 0; i < 5; ++i) res.tl_par[(size_t)t * 5 + i] = (double)p[i];
+      for (int i = 0; i < 15; ++i) res.tl_cov[(size_t)t * 15 + i] = (double)T.st.C[i];
+      res.tl_chi2[t] = (double)T.st.chi2;
+      chi2r[t] = T.st.chi2;
+    }
+    // ---- O5 selector: owner(c) = best-priority accepted tracklet containing c -----------------------
+    std::vector<int32_t> owner(N, -1);
+    auto better = [&](int32_t a, int32_t bb) {   // is tracklet a of higher priority than bb ? (R19)
+      if (bb < 0) return true;
+      if (res.tl_nhits[a] != res.tl_nhits[bb]) return res.tl_nhits[a] > res.tl_nhits[bb];
+      if (chi2r[a] != chi2r[bb]) return chi2r[a] < chi2r[bb];
+      return a < bb;
+    };
+    for (int64_t t = 0; t < ns; ++t) {
+      if (res.tl_status[t] != 2) continue;
+      for (int r = 0; r < R; ++r) {
+        const int32_t c = res.tl_rowhit[(size_t)t * R + r];
+        if (c >= 0 && better((int32_t)t, owner[c])) owner[c] = (int32_t)t;
+      }
+    }
+    res.tr_cl_offset.assign(1, 0);
+    for (int64_t t = 0; t < ns; ++t) {
+      if (res.tl_status[t] != 2) continue;
+      int kept = 0, first = -1, last = -1;
+      for (int r = 0; r < R; ++r) {
+        const int32_t c = res.tl_rowhit[(size_t)t * R + r];
+        if (c >= 0 && owner[c] == (int32_t)t) { ++kept; if (first < 0) first = r; last = r; }
+      }
+      if (kept < P.min_track_hits) continue;     // R20, R21: its clusters stay claimed
+      for (int r = 0; r < R; ++r) {
+        const int32_t c = res.tl_rowhit[(size_t)t * R + r];
+        if (c >= 0 && owner[c] == (int32_t)t) res.tr_cl_index.push_back((uint32_t)c);
+      }
+      res.tr_cl_offset.push_back((uint32_t)res.tr_cl_index.size());
+      res.tr_id.push_back((int32_t)t); res.tr_sector.push_back(secOf[res.start_hits[t]]);
+      res.tr_first.push_back(first); res.tr_last.push_back(last); res.tr_ncl.push_back(kept);
+      res.tr_x.push_back(res.tl_x[t]); res.tr_chi2.push_back(res.tl_chi2[t]);     // R22: not refitted
+      for (int i = 0; i < 5; ++i) res.tr_par.push_back(res.tl_par[(size_t)t * 5 + i]);
+      for (int i = 0; i < 15; ++i) res.tr_cov.push_back(res.tl_cov[(size_t)t * 15 + i]);
+    }
+  }
+};
+
+template <typename T>
+void copyOut(T* dst, const std::vector<T>& v) { if (dst && !v.empty()) std::memcpy(dst, v.data(), v.size() * sizeof(T)); }
+
+}  // namespace
+
+extern "C" {
+
+void orcDefaultParams(orcParams* p) {
+  p->area_y = 1.5f; p->area_z = 1.5f; p->link_dev2_max = 0.64f;
+  p->err2_y = 0.01f; p->err2_z = 0.01f; p->init_var_s = 1.0f; p->init_var_t = 1.0f; p->init_var_q = 100.0f;
+  p->turn_var_scale = 100.0f; p->max_sinphi = 0.98f; p->road_sigma = 4.0f; p->road_min = 0.3f; p->road_max = 2.0f;
+  p->max_row_gap = 4; p->min_chain_hits = 3; p->min_tracklet_hits = 10; p->min_track_hits = 10;
+  p->cell_min = 0.5f; p->cell_max = 8.0f;
+}
+
+int orcRun(const orcGeometry* g, const orcParams* p, int64_t n, const uint32_t* off, const float* y, const float* z,
+           int flags, orcResult** out) {
+  if (!g || !p || !out || n < 0 || !off || g->n_sectors < 1 || g->n_rows < 3 || !g->row_x || (n > 0 && (!y || !z)))
+    return ORC_ERR_INVALID_ARG;
+  if (n > 0x7fffffffll) return ORC_ERR_INVALID_ARG;
+  for (int r = 1; r < g->n_rows; ++r) if (!(g->row_x[r] > g->row_x[r - 1])) return ORC_ERR_INVALID_ARG;
+  const int nb = g->n_sectors * g->n_rows;
+  if (off[0] != 0 || (int64_t)off[nb] != n) return ORC_ERR_UNSORTED_OFFSETS;
+  for (int b = 0; b < nb; ++b) if (off[b + 1] < off[b]) return ORC_ERR_UNSORTED_OFFSETS;
+  for (int64_t i = 0; i < n; ++i) if (!std::isfinite(y[i]) || !std::isfinite(z[i])) return ORC_ERR_INVALID_ARG;  // R25
+  orcResult* r = new orcResult();
+  r->n = n; r->n_sectors = g->n_sectors; r->n_rows = g->n_rows;
+  r->fp64 = (flags & ORC_FP64) != 0; r->brute = (flags & ORC_BRUTE_FORCE) != 0;
+  if (r->fp64) { Tracker<double> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); }
+  else { Tracker<float> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); }
+  *out = r;
+  return ORC_OK;
+}
+void orcFree(orcResult* r) { delete r; }
+
+int64_t orcNumClusters(const orcResult* r) { return r->n; }
+int64_t orcNumStartHits(const orcResult* r) { return (int64_t)r->start_hits.size(); }
+int64_t orcNumTracks(const orcResult* r) { return (int64_t)r->tr_id.size(); }
+int64_t orcNumTrackClusters(const orcResult* r) { return (int64_t)r->tr_cl_index.size(); }
+
+void orcGetGrid(const orcResult* r, uint32_t* s2o, int32_t* cell, int32_t* ncells) {
+  copyOut(s2o, r->sorted_to_orig); copyOut(cell, r->cell_of_sorted); copyOut(ncells, r->n_cells);
+}
+void orcGetLinks(const orcResult* r, int32_t* ur, int32_t* dr, int32_t* u, int32_t* d) {
+  copyOut(ur, r->up_raw); copyOut(dr, r->dn_raw); copyOut(u, r->up); copyOut(d, r->dn);
+}
+void orcGetStartHits(const orcResult* r, uint32_t* sh) { copyOut(sh, r->start_hits); }
+void orcGetTracklets(const orcResult* r, int32_t* status, int32_t* nhits, int32_t* first, int32_t* last, int32_t* rowhit,
+                     double* x, double* par, double* cov, double* chi2) {
+  copyOut(status, r->tl_status); copyOut(nhits, r->tl_nhits); copyOut(first, r->tl_first); copyOut(last, r->tl_last);
+  copyOut(rowhit, r->tl_rowhit); copyOut(x, r->tl_x); copyOut(par, r->tl_par); copyOut(cov, r->tl_cov);
+  copyOut(chi2, r->tl_chi2);
+}
+void orcGetTracks(const orcResult* r, int32_t* id, int32_t* sector, int32_t* first, int32_t* last, int32_t* ncl, double* x,
+                  double* par, double* cov, double* chi2, uint32_t* off, uint32_t* idx) {
+  copyOut(id, r->tr_id); copyOut(sector, r->tr_sector); copyOut(first, r->tr_first); copyOut(last, r->tr_last);
+  copyOut(ncl, r->tr_ncl); copyOut(x, r->tr_x); copyOut(par, r->tr_par); copyOut(cov, r->tr_cov);
+  copyOut(chi2, r->tr_chi2); copyOut(off, r->tr_cl_offset); copyOut(idx, r->tr_cl_index);
+}
+
+int orcPropagate(double* state, double* cov, double x_new, double bz, double max_sinphi, int fp64) {
+  if (fp64) {
+    State<double> st{state[0], state[1], state[2], state[3], state[4], state[5], {}, 0};
+    for (int i = 0; i < 15; ++i) st.C[i] = cov[i];
+    if (!propagate<double>(st, x_new, 0.00299792458 * bz, max_sinphi)) return 0;
+    state[0] = st.x; state[1] = st.y; state[2] = st.z; state[3] = st.s; state[4] = st.t; state[5] = st.q;
+    for (int i = 0; i < 15; ++i) cov[i] = st.C[i];
+  } else {
+    State<float> st{(float)state[0], (float)state[1], (float)state[2], (float)state[3], (float)state[4], (float)state[5], {}, 0};
+    for (int i = 0; i < 15; ++i) st.C[i] = (float)cov[i];
+    if (!propagate<float>(st, (float)x_new, (float)(0.00299792458 * (double)(float)bz), (float)max_sinphi)) return 0;
+    state[0] = st.x; state[1] = st.y; state[2] = st.z; state[3] = st.s; state[4] = st.t; state[5] = st.q;
+    for (int i = 0; i < 15; ++i) cov[i] = st.C[i];
+  }
+  return 1;
+}
+
+int orcUpdate(double* state, double* cov, double* chi2, double ym, double zm, double e2y, double e2z, int fp64) {
+  if (fp64) {
+    State<double> st{state[0], state[1], state[2], state[3], state[4], state[5], {}, *chi2};
+    for (int i = 0; i < 15; ++i) st.C[i] = cov[i];
+    if (!update<double>(st, ym, zm, e2y, e2z)) return 0;
+    state[1] = st.y; state[2] = st.z; state[3] = st.s; state[4] = st.t; state[5] = st.q; *chi2 = st.chi2;
+    for (int i = 0; i < 15; ++i) cov[i] = st.C[i];
+  } else {
+    State<float> st{(float)state[0], (float)state[1], (float)state[2], (float)state[3], (float)state[4], (float)state[5], {}, (float)*chi2};
+    for (int i = 0; i < 15; ++i) st.C[i] = (float)cov[i];
+    if (!update<float>(st, (float)ym, (float)zm, (float)e2y, (float)e2z)) return 0;
+    state[1] = st.y; state[2] = st.z; state[3] = st.s; state[4] = st.t; state[5] = st.q; *chi2 = st.chi2;
+    for (int i = 0; i < 15; ++i) cov[i] = st.C[i];
+  }
+  return 1;
+}
+
+}  // extern "C"

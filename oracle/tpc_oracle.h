@@ -1,0 +1,89 @@
+/* tpc_oracle.h -- C interface of the CPU ORACLE of the TPC sector tracker.
+ *
+ * TEST INFRASTRUCTURE, NOT THE PRODUCT.  Only tests/, __graft_entry__.smoke() and bench.py's
+ * cpu_baseline / --impl reference legs may load this library.  It shares no code, header, table or
+ * constant with the CUDA path (paper_1910_12214_b200/csrc, include/tpc_abi.h); the structs below are
+ * the oracle's own.
+ *
+ * What it computes: the five steps O1..O5 of DESIGN.md section 3 (formula sheet), which restates
+ * the reading of BASELINE.json north_star adopted because PAPER.md gives
+ * no algorithmic detail for the tracker ("derived from the Run 2 HLT GPU
+ * tracker", nothing more).  Single thread, plain loops, one rounding per written operation, no FMA
+ * contraction (build with -ffp-contract=off -fno-fast-math), binary32 (the parity reference) or
+ * binary64 (algebra checks).
+ *
+ * Pins (tests/test_oracle_*.py): grid search == brute-force search; collinear / hand-built link
+ * cases; reciprocity and path invariants; Propagate vs the closed-form asin helix and vs finite
+ * differences; Update / fit vs numpy least squares; exact helix recovery; unit pulls; full
+ * attachment of noise-free high-pT helices; selector vs sorted greedy.
+ * Parity unpinned: physics efficiency / fake rate on configs 1-4 (no reference numbers exist).
+ */
+#ifndef TPC_ORACLE_H
+#define TPC_ORACLE_H
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct {
+  int32_t n_sectors, n_rows;
+  const float* row_x;        /* [n_rows] */
+  const uint8_t* row_dead;   /* [n_rows] or NULL */
+  float bz_tesla, tan_half_sector, z_min, z_max;
+} orcGeometry;
+
+/* Table P of SURVEY.md 8(c) / DESIGN.md 3; orcDefaultParams fills the defaults */
+typedef struct {
+  float area_y, area_z, link_dev2_max;
+  float err2_y, err2_z, init_var_s, init_var_t, init_var_q, turn_var_scale;
+  float max_sinphi, road_sigma, road_min, road_max;
+  int32_t max_row_gap, min_chain_hits, min_tracklet_hits, min_track_hits;
+  float cell_min, cell_max;
+} orcParams;
+
+typedef struct orcResult orcResult;
+
+enum { ORC_OK = 0, ORC_ERR_INVALID_ARG = -1, ORC_ERR_UNSORTED_OFFSETS = -2 };
+enum { ORC_BRUTE_FORCE = 1, ORC_FP64 = 2 };
+
+void orcDefaultParams(orcParams* p);
+
+/* Runs O1..O5 on host arrays.  flags: ORC_BRUTE_FORCE = every search loops over all clusters of the
+ * row instead of the grid; ORC_FP64 = all arithmetic in binary64.  On success *out owns the result. */
+int orcRun(const orcGeometry* g, const orcParams* p, int64_t n_clusters, const uint32_t* row_offset,
+           const float* y, const float* z, int flags, orcResult** out);
+void orcFree(orcResult* r);
+
+/* sizes */
+int64_t orcNumClusters(const orcResult*);
+int64_t orcNumStartHits(const orcResult*);   /* == number of tracklet ids */
+int64_t orcNumTracks(const orcResult*);
+int64_t orcNumTrackClusters(const orcResult*);
+
+/* O1: grid invariants. sorted_to_orig [n]; cell_of_sorted [n] (cell id inside the bucket);
+ * n_cells [n_sectors*n_rows]. NULL-able. Empty when ORC_BRUTE_FORCE. */
+void orcGetGrid(const orcResult*, uint32_t* sorted_to_orig, int32_t* cell_of_sorted, int32_t* n_cells);
+/* O2/O3: links, global original indices, -1 none */
+void orcGetLinks(const orcResult*, int32_t* up_raw, int32_t* dn_raw, int32_t* up, int32_t* dn);
+void orcGetStartHits(const orcResult*, uint32_t* start_hits);
+/* O4: one entry per start hit (tracklet id = rank).  status: 0 discarded in the chain fit,
+ * 1 built but rejected (nhits < min_tracklet_hits or no snapshot), 2 accepted.
+ * rowhit [n_start*n_rows] global indices / -1; x [n_start]; par [n_start*5]; cov [n_start*15]. */
+void orcGetTracklets(const orcResult*, int32_t* status, int32_t* nhits, int32_t* first_row, int32_t* last_row,
+                     int32_t* rowhit, double* x, double* par, double* cov, double* chi2);
+/* O5: tracks in ascending tracklet id; par [n_tracks*5], cov [n_tracks*15] (track-major);
+ * cl_offset [n_tracks+1]; cl_index [n_track_clusters] ascending row. */
+void orcGetTracks(const orcResult*, int32_t* tracklet_id, int32_t* sector, int32_t* first_row, int32_t* last_row,
+                  int32_t* ncl, double* x, double* par, double* cov, double* chi2, uint32_t* cl_offset,
+                  uint32_t* cl_index);
+
+/* Single KF steps for the pins.  state = {x, y, z, s, t, q}, cov = 15 lower-triangle elements
+ * (00,10,11,20,21,22,30,...,44), both in/out as doubles (rounded to binary32 first unless fp64).
+ * Return 1 on success, 0 on failure (state untouched). */
+int orcPropagate(double* state, double* cov, double x_new, double bz_tesla, double max_sinphi, int fp64);
+int orcUpdate(double* state, double* cov, double* chi2, double ym, double zm, double err2_y, double err2_z, int fp64);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

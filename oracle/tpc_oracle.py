@@ -1,0 +1,189 @@
+"""ctypes wrapper of the CPU oracle (oracle/tpc_oracle.cpp).  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may import
+this module.  It does not import the CUDA package (only plain numpy arrays come in).
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from dataclasses import dataclass
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "tpc_oracle.cpp")
+_HDR = os.path.join(_HERE, "tpc_oracle.h")
+_LIB = os.path.join(_HERE, "libtpcoracle.so")
+
+BRUTE_FORCE = 1
+FP64 = 2
+
+
+def build(force: bool = False) -> str:
+    """g++ -O2 -ffp-contract=off -fno-fast-math (R0: no FMA contraction, no reassociation)."""
+    newest = max(os.path.getmtime(_SRC), os.path.getmtime(_HDR))
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < newest:
+        subprocess.check_call(["g++", "-O2", "-ffp-contract=off", "-fno-fast-math", "-shared", "-fPIC", _SRC, "-o", _LIB])
+    return _LIB
+
+
+class Geometry(ctypes.Structure):
+    _fields_ = [("n_sectors", ctypes.c_int32), ("n_rows", ctypes.c_int32), ("row_x", ctypes.c_void_p),
+                ("row_dead", ctypes.c_void_p), ("bz_tesla", ctypes.c_float), ("tan_half_sector", ctypes.c_float),
+                ("z_min", ctypes.c_float), ("z_max", ctypes.c_float)]
+
+
+class Params(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_float) for n in
+                ("area_y", "area_z", "link_dev2_max", "err2_y", "err2_z", "init_var_s", "init_var_t", "init_var_q",
+                 "turn_var_scale", "max_sinphi", "road_sigma", "road_min", "road_max")] + \
+               [(n, ctypes.c_int32) for n in ("max_row_gap", "min_chain_hits", "min_tracklet_hits", "min_track_hits")] + \
+               [("cell_min", ctypes.c_float), ("cell_max", ctypes.c_float)]
+
+
+_lib = None
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        L = ctypes.CDLL(_LIB)
+        vp, i64, dbl, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int
+        L.orcDefaultParams.argtypes = [ctypes.POINTER(Params)]
+        L.orcDefaultParams.restype = None
+        L.orcRun.argtypes = [ctypes.POINTER(Geometry), ctypes.POINTER(Params), i64, vp, vp, vp, ci, ctypes.POINTER(vp)]
+        L.orcRun.restype = ci
+        L.orcFree.argtypes = [vp]
+        L.orcFree.restype = None
+        for f in ("orcNumClusters", "orcNumStartHits", "orcNumTracks", "orcNumTrackClusters"):
+            getattr(L, f).argtypes = [vp]
+            getattr(L, f).restype = i64
+        L.orcGetGrid.argtypes = [vp] * 4
+        L.orcGetLinks.argtypes = [vp] * 5
+        L.orcGetStartHits.argtypes = [vp] * 2
+        L.orcGetTracklets.argtypes = [vp] * 10
+        L.orcGetTracks.argtypes = [vp] * 12
+        for f in ("orcGetGrid", "orcGetLinks", "orcGetStartHits", "orcGetTracklets", "orcGetTracks"):
+            getattr(L, f).restype = None
+        L.orcPropagate.argtypes = [vp, vp, dbl, dbl, dbl, ci]
+        L.orcPropagate.restype = ci
+        L.orcUpdate.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, ci]
+        L.orcUpdate.restype = ci
+        _lib = L
+    return _lib
+
+
+def default_params() -> Params:
+    p = Params()
+    _load().orcDefaultParams(ctypes.byref(p))
+    return p
+
+
+@dataclass
+class OracleResult:
+    n_clusters: int
+    sorted_to_orig: np.ndarray
+    cell_of_sorted: np.ndarray
+    n_cells: np.ndarray
+    link_up_raw: np.ndarray
+    link_dn_raw: np.ndarray
+    link_up: np.ndarray
+    link_dn: np.ndarray
+    start_hits: np.ndarray
+    tl_status: np.ndarray
+    tl_nhits: np.ndarray
+    tl_first_row: np.ndarray
+    tl_last_row: np.ndarray
+    tl_rowhit: np.ndarray      # [n_start, n_rows]
+    tl_x: np.ndarray
+    tl_par: np.ndarray         # [n_start, 5]
+    tl_cov: np.ndarray         # [n_start, 15]
+    tl_chi2: np.ndarray
+    trk_tracklet: np.ndarray
+    trk_sector: np.ndarray
+    trk_first_row: np.ndarray
+    trk_last_row: np.ndarray
+    trk_ncl: np.ndarray
+    trk_x: np.ndarray
+    trk_par: np.ndarray        # [n_tracks, 5]
+    trk_cov: np.ndarray        # [n_tracks, 15]
+    trk_chi2: np.ndarray
+    trk_cl_offset: np.ndarray
+    trk_cl_index: np.ndarray
+
+    @property
+    def n_tracks(self) -> int:
+        return int(self.trk_ncl.shape[0])
+
+
+def _ptr(a):
+    return a.ctypes.data if a is not None and a.size else None
+
+
+def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool = False,
+        stages_only: bool = False) -> OracleResult:
+    """Run O1..O5 on an Event-like object (fields n_sectors, n_rows, row_x, row_dead, bz_tesla,
+    tan_half_sector, z_min, z_max, row_offset, y, z; numpy arrays)."""
+    L = _load()
+    p = params if params is not None else default_params()
+    row_x = np.ascontiguousarray(ev.row_x, np.float32)
+    dead = np.ascontiguousarray(ev.row_dead, np.uint8)
+    g = Geometry(ev.n_sectors, ev.n_rows, row_x.ctypes.data, dead.ctypes.data if dead.any() else None, ev.bz_tesla,
+                 ev.tan_half_sector, ev.z_min, ev.z_max)
+    off = np.ascontiguousarray(ev.row_offset, np.uint32)
+    y = np.ascontiguousarray(ev.y, np.float32)
+    z = np.ascontiguousarray(ev.z, np.float32)
+    n = int(y.shape[0])
+    h = ctypes.c_void_p()
+    rc = L.orcRun(ctypes.byref(g), ctypes.byref(p), n, off.ctypes.data, _ptr(y), _ptr(z),
+                  (BRUTE_FORCE if brute_force else 0) | (FP64 if fp64 else 0), ctypes.byref(h))
+    if rc != 0:
+        raise ValueError(f"orcRun failed with {rc}")
+    try:
+        R = ev.n_rows
+        ns, nt, ntc = L.orcNumStartHits(h), L.orcNumTracks(h), L.orcNumTrackClusters(h)
+        ng = 0 if brute_force else n
+        s2o, cell = np.zeros(ng, np.uint32), np.zeros(ng, np.int32)
+        ncell = np.zeros(ev.n_sectors * R if not brute_force else 0, np.int32)
+        L.orcGetGrid(h, _ptr(s2o), _ptr(cell), _ptr(ncell))
+        ur, dr, u, d = (np.full(n, -1, np.int32) for _ in range(4))
+        L.orcGetLinks(h, _ptr(ur), _ptr(dr), _ptr(u), _ptr(d))
+        sh = np.zeros(ns, np.uint32)
+        L.orcGetStartHits(h, _ptr(sh))
+        st, nh, fr, lr = (np.zeros(ns, np.int32) for _ in range(4))
+        rh = np.full((ns, R), -1, np.int32)
+        tx, tchi = np.zeros(ns), np.zeros(ns)
+        tpar, tcov = np.zeros((ns, 5)), np.zeros((ns, 15))
+        L.orcGetTracklets(h, _ptr(st), _ptr(nh), _ptr(fr), _ptr(lr), _ptr(rh), _ptr(tx), _ptr(tpar), _ptr(tcov),
+                          _ptr(tchi))
+        kid, ks, kf, kl, kn = (np.zeros(nt, np.int32) for _ in range(5))
+        kx, kchi = np.zeros(nt), np.zeros(nt)
+        kpar, kcov = np.zeros((nt, 5)), np.zeros((nt, 15))
+        koff, kidx = np.zeros(nt + 1, np.uint32), np.zeros(ntc, np.uint32)
+        L.orcGetTracks(h, _ptr(kid), _ptr(ks), _ptr(kf), _ptr(kl), _ptr(kn), _ptr(kx), _ptr(kpar), _ptr(kcov),
+                       _ptr(kchi), _ptr(koff), _ptr(kidx))
+    finally:
+        L.orcFree(h)
+    return OracleResult(n, s2o, cell, ncell, ur, dr, u, d, sh, st, nh, fr, lr, rh, tx, tpar, tcov, tchi, kid, ks, kf, kl,
+                        kn, kx, kpar, kcov, kchi, koff, kidx)
+
+
+def propagate(state, cov, x_new, bz_tesla=0.5, max_sinphi=0.98, fp64=True):
+    """One Propagate step.  state = (x, y, z, s, t, q); cov = 15 lower-triangle elements.  Returns (ok, state, cov)."""
+    s = np.array(state, np.float64)
+    c = np.array(cov, np.float64)
+    ok = _load().orcPropagate(s.ctypes.data, c.ctypes.data, float(x_new), float(bz_tesla), float(max_sinphi), int(fp64))
+    return bool(ok), s, c
+
+
+def update(state, cov, chi2, ym, zm, err2_y=0.01, err2_z=0.01, fp64=True):
+    """One Update step (y then z).  Returns (ok, state, cov, chi2)."""
+    s = np.array(state, np.float64)
+    c = np.array(cov, np.float64)
+    x2 = np.array([chi2], np.float64)
+    ok = _load().orcUpdate(s.ctypes.data, c.ctypes.data, x2.ctypes.data, float(ym), float(zm), float(err2_y),
+                           float(err2_z), int(fp64))
+    return bool(ok), s, c, float(x2[0])
