@@ -1,0 +1,168 @@
+/* tpc_abi.h -- C ABI of libtpcgpu.so, the B200 (sm_100a) TPC sector tracker.
+ *
+ * What the library computes (BASELINE.json north_star; "TPC track finding ... derived
+ * from the Run 2 HLT TPC tracking on GPUs"; clusters with single-precision properties in, PAPER.md
+ * L69-L70; tracks and the cluster-to-track attachment out):
+ *   a1 grid build          per (sector,row) counting sort of the clusters over a (y,z) grid
+ *   a2 neighbour finder    best (up,down) pair per cluster against a straight line
+ *   a3 cleaner/start hits  reciprocal links only; heads of link chains
+ *   a4 tracklet constructor link-chain fit + row-by-row helix Kalman extrapolation (5 params, 15 cov, fp32)
+ *   a5 tracklet selector   shared clusters go to the longest / lowest-chi2 tracklet
+ * The formulas, constants and tie-breaks are DESIGN.md section 3 (readings R0..R27 of SURVEY.md 8(c)).
+ *
+ * Conventions
+ *   - every call returns an int status: TPC_OK (0) or a negative TPC_ERR_*; no exceptions, no global state;
+ *   - "DEVICE" pointers are CUDA device pointers of the handle's device, "HOST" pointers are host memory;
+ *   - the caller owns every buffer it passes (inputs, outputs, workspace); inputs are never written;
+ *   - tpcRun only enqueues work on the given stream and returns; results and the status are valid after
+ *     the stream has been synchronised (tpcGetRunStatus does that itself);
+ *   - a handle is not thread-safe; distinct handles are independent;
+ *   - there is no CPU fallback: without a CUDA device tpcCreate fails with TPC_ERR_CUDA.
+ */
+#ifndef TPC_ABI_H
+#define TPC_ABI_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+  TPC_OK = 0,
+  TPC_ERR_INVALID_ARG = -1,         /* NULL / negative / inconsistent argument */
+  TPC_ERR_UNSORTED_OFFSETS = -2,    /* row_offset not monotone or its ends != 0 / n_clusters (found on the device) */
+  TPC_ERR_WORKSPACE_TOO_SMALL = -3,
+  TPC_ERR_CAPACITY = -4,            /* an output capacity was exceeded: outputs truncated, nothing written out of
+                                       bounds, required sizes are in tpcRunStatus */
+  TPC_ERR_CUDA = -5,                /* a CUDA runtime call failed (tpcErrorString gives the last message) */
+  TPC_ERR_NONFINITE_INPUT = -6      /* validate_input was set and a cluster coordinate is NaN/Inf (R25) */
+};
+
+typedef struct tpcHandle tpcHandle;
+
+/* Detector description (R1, R2).  All pointers HOST, copied by tpcCreate. */
+typedef struct {
+  int32_t n_sectors;            /* 36 (config 0: 1) */
+  int32_t n_rows;               /* 152; 3 <= n_rows <= 255 */
+  const float* row_x;           /* [n_rows] local x of the pad-row planes, cm, strictly increasing */
+  const float* row_pitch;       /* [n_rows] pad pitch, cm; carried only (may be NULL) */
+  const uint8_t* row_dead;      /* [n_rows] 1 = dead row, or NULL */
+  float bz_tesla;               /* uniform field, 0.5 */
+  float tan_half_sector;        /* tan(10 deg): row half width = row_x * tan_half_sector */
+  float z_min, z_max;           /* grid z range, cm; clusters outside are clamped into edge cells */
+} tpcGeometry;
+
+/* Table P of DESIGN.md section 3.  tpcDefaultParams fills the defaults given in the comments. */
+typedef struct {
+  float area_y, area_z;         /* 1.5, 1.5   neighbour window = area * |dx| (O2) */
+  float link_dev2_max;          /* 0.64       max squared slope mismatch of a link (O2) */
+  float err2_y, err2_z;         /* 0.01, 0.01 measurement variances, cm^2 (O4 Update) */
+  float init_var_s, init_var_t, init_var_q;   /* 1, 1, 100  prior variances (O4 step 1) */
+  float turn_var_scale;         /* 100        y,z variance scale at the turn (O4 step 4) */
+  float max_sinphi;             /* 0.98 */
+  float road_sigma, road_min, road_max;       /* 4, 0.3, 2.0  search road (O4 Search) */
+  int32_t max_row_gap;          /* 4 */
+  int32_t min_chain_hits;       /* 3 */
+  int32_t min_tracklet_hits;    /* 10 */
+  int32_t min_track_hits;       /* 10 */
+  float cell_min, cell_max;     /* 0.5, 8.0   grid cell edge limits, cm (O1; do not change results, R3) */
+  float clusters_per_cell;      /* 1.0        target occupancy of a grid cell (implementation choice, R3) */
+  int32_t validate_input;       /* 0          1 = scan y,z for NaN/Inf and fail with TPC_ERR_NONFINITE_INPUT */
+  int32_t force_wide_keys;      /* 0          1 = use the two-pass selector keys even when the packed 64-bit key
+                                              fits (R27; results are identical, for tests) */
+} tpcParams;
+
+/* Input clusters: CSR by (sector,row), fp32 SoA (single-precision cluster properties). */
+typedef struct {
+  int64_t n_clusters;           /* 0 <= n_clusters < 2^31 */
+  const uint32_t* row_offset;   /* DEVICE [n_sectors*n_rows+1]; clusters of (s,r) = [off[s*n_rows+r], off[s*n_rows+r+1]) */
+  const float* x;               /* DEVICE [n_clusters] or NULL; not read: a cluster's x is row_x[r] */
+  const float* y;               /* DEVICE [n_clusters] local y (pad direction), cm */
+  const float* z;               /* DEVICE [n_clusters] z (drift/time direction), cm */
+  const float* q;               /* DEVICE [n_clusters] charge or NULL; not read by this path */
+} tpcClusters;
+
+/* Outputs.  All pointers DEVICE.  Tracks are emitted in ascending tracklet id (= rank of the start hit in
+ * ascending global cluster index); a track's clusters in ascending row. */
+typedef struct {
+  int64_t cap_tracks;           /* capacity of the trk_* arrays */
+  int64_t cap_track_clusters;   /* capacity of trk_cl_index */
+  int32_t* trk_tracklet;        /* [cap_tracks] tracklet id of the track */
+  int32_t* trk_sector;          /* [cap_tracks] */
+  int32_t* trk_first_row;       /* [cap_tracks] first / last row with a kept cluster */
+  int32_t* trk_last_row;
+  int32_t* trk_ncl;             /* [cap_tracks] kept clusters */
+  float* trk_x;                 /* [cap_tracks] x of the reference plane (innermost attached row of the tracklet) */
+  float* trk_par;               /* [5][cap_tracks] SoA: y, z, sin(phi), dz/ds, q/pT */
+  float* trk_cov;               /* [15][cap_tracks] SoA: lower triangle 00,10,11,20,21,22,30,...,44 */
+  float* trk_chi2;              /* [cap_tracks] chi2 of the constructor's down pass (R22: not refitted) */
+  uint32_t* trk_cl_offset;      /* [cap_tracks+1] CSR offsets into trk_cl_index */
+  uint32_t* trk_cl_index;       /* [cap_track_clusters] global (input) cluster indices */
+  /* optional per-stage outputs for parity tests; any may be NULL */
+  int32_t* link_up_raw;         /* [n_clusters] O2 links as global input indices, -1 = none */
+  int32_t* link_dn_raw;
+  int32_t* link_up;             /* [n_clusters] O3 cleaned links */
+  int32_t* link_dn;
+  uint32_t* start_hits;         /* [cap_tracklets] O3 start hits, ascending global index */
+  int32_t* tl_status;           /* [cap_tracklets] 0 discarded in the chain fit, 1 rejected, 2 accepted */
+  int32_t* tl_nhits;            /* [cap_tracklets] */
+  int32_t* tl_first_row;        /* [cap_tracklets] */
+  int32_t* tl_last_row;
+  int32_t* tl_rowhit;           /* [cap_tracklets][n_rows] global input indices / -1 (tracklet-major) */
+  float* tl_x;                  /* [cap_tracklets] */
+  float* tl_par;                /* [cap_tracklets][5] (tracklet-major) */
+  float* tl_cov;                /* [cap_tracklets][15] */
+  float* tl_chi2;               /* [cap_tracklets] */
+} tpcTracks;
+
+/* Filled by tpcGetRunStatus after the stream has drained. */
+typedef struct {
+  int32_t status;               /* TPC_OK, TPC_ERR_CAPACITY, TPC_ERR_UNSORTED_OFFSETS, TPC_ERR_NONFINITE_INPUT */
+  int32_t kernel_launches;      /* kernels + memsets enqueued by the last tpcRun */
+  int64_t n_clusters;
+  int64_t n_start_hits;         /* = tracklet ids; required cap_tracklets */
+  int64_t n_tracklets;          /* accepted tracklets (status 2) */
+  int64_t n_tracklet_hits;      /* H: hits summed over accepted tracklets */
+  int64_t n_tracks;             /* required cap_tracks */
+  int64_t n_track_clusters;     /* required cap_track_clusters */
+  int64_t n_cells;              /* grid cells over all (sector,row) */
+  float stage_ms[8];            /* per-stage device times of the last run when profiling is on (else 0):
+                                   0 grid, 1 neighbour finder, 2 cleaner+start hits, 3 constructor, 4 selector,
+                                   5 optional exports, 6 total, 7 unused */
+} tpcRunStatus;
+
+int tpcDefaultParams(tpcParams* p);
+
+/* Creates a tracker on CUDA device `cuda_device`; copies geometry and parameters.  HOST pointers. */
+int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cuda_device);
+int tpcDestroy(tpcHandle* h);
+
+/* Bytes of DEVICE workspace tpcRun needs for up to n_clusters clusters and cap_tracklets start hits. */
+int tpcWorkspaceBytes(const tpcHandle* h, int64_t n_clusters, int64_t cap_tracklets, size_t* bytes);
+
+/* Enqueues a1..a5 on `cuda_stream` (a cudaStream_t, NULL = default stream) and returns without synchronising.
+ * `workspace` is DEVICE memory of at least tpcWorkspaceBytes(n_clusters, cap_tracklets), 256-byte aligned.
+ * Argument errors are returned here; data-dependent errors (capacity, offsets) by tpcGetRunStatus. */
+int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_tracklets, void* workspace,
+           size_t workspace_bytes, void* cuda_stream);
+
+/* Synchronises with the last tpcRun and reports counts, required capacities and the data-dependent status. */
+int tpcGetRunStatus(tpcHandle* h, tpcRunStatus* out);
+
+/* 1 = record CUDA events between the stages of every tpcRun (stage_ms); 0 = off (default). */
+int tpcSetProfiling(tpcHandle* h, int on);
+
+/* Host-buffer convenience call (the end-to-end path a host application uses): copies row_offset, y, z
+ * (HOST, pageable or pinned) to device memory owned by the handle (grown on demand), runs a1..a5, copies
+ * the tracks back into the HOST arrays of `out_host` (same layout as tpcTracks but HOST pointers; the
+ * optional per-stage pointers must be NULL) and synchronises.  *status receives the run status. */
+int tpcRunHost(tpcHandle* h, int64_t n_clusters, const uint32_t* row_offset, const float* y, const float* z,
+               tpcTracks* out_host, tpcRunStatus* status, void* cuda_stream);
+
+const char* tpcErrorString(int code);
+const char* tpcLastCudaError(const tpcHandle* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TPC_ABI_H */

@@ -1,0 +1,485 @@
+// tpc_api.cu -- host side of libtpcgpu.so: the C ABI of include/tpc_abi.h, workspace layout and the launch
+// sequence a1..a5 on one stream (no host round trip inside tpcRun).
+//
+// Build (see paper_1910_12214_b200/build.py):
+//   nvcc -gencode arch=compute_100a,code=sm_100a -O3 -lineinfo --fmad=false -prec-div=true -prec-sqrt=true
+//        -ftz=false -shared -Xcompiler -fPIC tpc_api.cu -o libtpcgpu.so
+#include "../../include/tpc_abi.h"
+
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "tpc_common.cuh"
+#include "tpc_scan.cuh"
+#include "tpc_grid.cuh"
+#include "tpc_links.cuh"
+#include "tpc_kalman.cuh"
+#include "tpc_tracklet.cuh"
+#include "tpc_select.cuh"
+
+using namespace tpc;
+
+namespace {
+
+constexpr size_t ALIGN = 256;
+inline size_t alignUp(size_t v) { return (v + ALIGN - 1) / ALIGN * ALIGN; }
+inline int64_t ceilDiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
+
+struct Workspace {
+  GridDesc* desc;
+  uint32_t* cell_start;
+  uint32_t* rank;            // aliases spos_by_orig (a1 only)
+  float2* syz;
+  uint32_t* s2o;
+  int32_t *lup, *ldn, *cup, *cdn;
+  int32_t* spos_by_orig;
+  uint32_t* tiles32;         // tile sums: cells scan / start compaction
+  unsigned long long* tiles64;
+  uint32_t *start_orig, *start_pos;
+  TrackletStore tl;
+  unsigned long long *tsel, *tscan;
+  int32_t *kept_first, *kept_last;
+  unsigned long long* owner_key;
+  uint32_t* owner_id;
+  size_t bytes;
+};
+
+}  // namespace
+
+struct tpcHandle {
+  int device = 0;
+  tpcParams params{};
+  DevParams P{};
+  std::vector<float> row_x;
+  float* d_row_x = nullptr;
+  int16_t *d_up = nullptr, *d_dn = nullptr;
+  uint8_t* d_dead = nullptr;
+  int64_t* d_cnt = nullptr;        // CNT_COUNT counters + 1 slot for the packed selector total
+  int64_t* h_cnt = nullptr;        // pinned copy
+  cudaEvent_t ev_done = nullptr;
+  cudaEvent_t ev_stage[7] = {};
+  int profiling = 0;
+  int launches = 0;
+  bool pending = false;
+  int64_t last_n = 0;
+  double cells_per_bucket_bound = 0;   // sum over buckets of the n-independent part of the cell bound
+  char cuda_msg[256] = {0};
+  // pools of tpcRunHost
+  void* pool[16] = {};
+  size_t pool_bytes[16] = {};
+};
+
+namespace {
+
+int cudaFail(tpcHandle* h, cudaError_t e, const char* what) {
+  if (h) snprintf(h->cuda_msg, sizeof(h->cuda_msg), "%s: %s", what, cudaGetErrorString(e));
+  return TPC_ERR_CUDA;
+}
+#define TPC_CUDA(h, call)                                   \
+  do {                                                      \
+    cudaError_t e_ = (call);                                \
+    if (e_ != cudaSuccess) return cudaFail(h, e_, #call);   \
+  } while (0)
+
+int64_t capCells(const tpcHandle* h, int64_t n) {
+  const double cpc = h->params.clusters_per_cell;
+  return (int64_t)((double)n / cpc * 1.01 + h->cells_per_bucket_bound * 1.01) + 4 * h->P.n_buckets + 1024;
+}
+
+// carve the workspace; base may be NULL (size query)
+Workspace layout(const tpcHandle* h, int64_t N, int64_t capT, char* base) {
+  Workspace w{};
+  size_t o = 0;
+  auto take = [&](size_t bytes) { char* p = base ? base + o : nullptr; o += alignUp(bytes); return (void*)p; };
+  const int nb = h->P.n_buckets, R = h->P.n_rows;
+  const int64_t cc = capCells(h, N);
+  const int64_t Nn = N > 0 ? N : 1, Tn = capT > 0 ? capT : 1;
+  w.desc = (GridDesc*)take(sizeof(GridDesc) * nb);
+  w.cell_start = (uint32_t*)take(4 * (size_t)(cc + 1));
+  w.spos_by_orig = (int32_t*)take(4 * (size_t)Nn);
+  w.rank = (uint32_t*)w.spos_by_orig;
+  w.syz = (float2*)take(8 * (size_t)Nn);
+  w.s2o = (uint32_t*)take(4 * (size_t)Nn);
+  w.lup = (int32_t*)take(4 * (size_t)Nn);
+  w.ldn = (int32_t*)take(4 * (size_t)Nn);
+  w.cup = (int32_t*)take(4 * (size_t)Nn);
+  w.cdn = (int32_t*)take(4 * (size_t)Nn);
+  const int64_t t32 = ceilDiv(cc + 1, SCAN_TILE) + ceilDiv(Nn, CP_TILE) + 2;
+  w.tiles32 = (uint32_t*)take(4 * (size_t)t32);
+  w.tiles64 = (unsigned long long*)take(8 * (size_t)(ceilDiv(Tn, SCAN_TILE) + 2));
+  w.start_orig = (uint32_t*)take(4 * (size_t)Tn);
+  w.start_pos = (uint32_t*)take(4 * (size_t)Tn);
+  w.tl.capT = capT;
+  w.tl.status = (int32_t*)take(4 * (size_t)Tn);
+  w.tl.nhits = (int32_t*)take(4 * (size_t)Tn);
+  w.tl.first_row = (int32_t*)take(4 * (size_t)Tn);
+  w.tl.last_row = (int32_t*)take(4 * (size_t)Tn);
+  w.tl.sector = (int32_t*)take(4 * (size_t)Tn);
+  w.tl.x = (float*)take(4 * (size_t)Tn);
+  w.tl.chi2 = (float*)take(4 * (size_t)Tn);
+  w.tl.par = (float*)take(4 * 5 * (size_t)Tn);
+  w.tl.cov = (float*)take(4 * 15 * (size_t)Tn);
+  w.tl.rowhit = (int32_t*)take(4 * (size_t)R * (size_t)Tn);
+  w.tsel = (unsigned long long*)take(8 * (size_t)(Tn + 1));
+  w.tscan = (unsigned long long*)take(8 * (size_t)(Tn + 1));
+  w.kept_first = (int32_t*)take(4 * (size_t)Tn);
+  w.kept_last = (int32_t*)take(4 * (size_t)Tn);
+  w.owner_key = (unsigned long long*)take(8 * (size_t)Nn);
+  w.owner_id = (uint32_t*)take(4 * (size_t)Nn);
+  w.bytes = o;
+  return w;
+}
+
+}  // namespace
+
+extern "C" {
+
+int tpcDefaultParams(tpcParams* p) {
+  if (!p) return TPC_ERR_INVALID_ARG;
+  p->area_y = 1.5f; p->area_z = 1.5f; p->link_dev2_max = 0.64f;
+  p->err2_y = 0.01f; p->err2_z = 0.01f;
+  p->init_var_s = 1.0f; p->init_var_t = 1.0f; p->init_var_q = 100.0f;
+  p->turn_var_scale = 100.0f; p->max_sinphi = 0.98f;
+  p->road_sigma = 4.0f; p->road_min = 0.3f; p->road_max = 2.0f;
+  p->max_row_gap = 4; p->min_chain_hits = 3; p->min_tracklet_hits = 10; p->min_track_hits = 10;
+  p->cell_min = 0.5f; p->cell_max = 8.0f; p->clusters_per_cell = 1.0f;
+  p->validate_input = 0; p->force_wide_keys = 0;
+  return TPC_OK;
+}
+
+int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cuda_device) {
+  if (!out || !g || !p || !g->row_x) return TPC_ERR_INVALID_ARG;
+  *out = nullptr;
+  const int R = g->n_rows, S = g->n_sectors;
+  if (R < 3 || R >= MAX_ROWS || S < 1 || (int64_t)R * S > (1 << 24)) return TPC_ERR_INVALID_ARG;
+  for (int r = 1; r < R; ++r)
+    if (!(g->row_x[r] > g->row_x[r - 1])) return TPC_ERR_INVALID_ARG;
+  if (!(g->z_max > g->z_min) || !(g->tan_half_sector > 0) || !(g->row_x[0] > 0)) return TPC_ERR_INVALID_ARG;
+  if (!(p->cell_min > 0) || !(p->cell_max >= p->cell_min) || !(p->clusters_per_cell > 0)) return TPC_ERR_INVALID_ARG;
+  if (p->min_chain_hits < 2 || p->max_row_gap < 0) return TPC_ERR_INVALID_ARG;
+  tpcHandle* h = new (std::nothrow) tpcHandle();
+  if (!h) return TPC_ERR_INVALID_ARG;
+  h->device = cuda_device;
+  h->params = *p;
+  DevParams& P = h->P;
+  P.area_y = p->area_y; P.area_z = p->area_z; P.link_dev2_max = p->link_dev2_max;
+  P.err2_y = p->err2_y; P.err2_z = p->err2_z; P.init_var_s = p->init_var_s; P.init_var_t = p->init_var_t;
+  P.init_var_q = p->init_var_q; P.turn_var_scale = p->turn_var_scale; P.max_sinphi = p->max_sinphi;
+  P.road_sigma = p->road_sigma; P.road_min = p->road_min; P.road_max = p->road_max;
+  P.max_row_gap = p->max_row_gap; P.min_chain_hits = p->min_chain_hits; P.min_tracklet_hits = p->min_tracklet_hits;
+  P.min_track_hits = p->min_track_hits; P.cell_min = p->cell_min; P.cell_max = p->cell_max;
+  P.clusters_per_cell = p->clusters_per_cell;
+  P.b = (float)(0.00299792458 * (double)g->bz_tesla);     // curvature constant, O4
+  P.tan_half_sector = g->tan_half_sector; P.z_min = g->z_min; P.z_max = g->z_max;
+  P.n_rows = R; P.n_sectors = S; P.n_buckets = R * S;
+  P.max_cells_per_bucket = 1 << 24;
+  h->row_x.assign(g->row_x, g->row_x + R);
+  // R2: up(r) = first live row among r+1, r+2; dn(r) = first live row among r-1, r-2; none for dead rows
+  std::vector<int16_t> up(R, -1), dn(R, -1);
+  std::vector<uint8_t> dead(R, 0);
+  for (int r = 0; r < R; ++r) dead[r] = (g->row_dead && g->row_dead[r]) ? 1 : 0;
+  for (int r = 0; r < R; ++r) {
+    if (dead[r]) continue;
+    for (int k = 1; k <= 2; ++k) if (r + k < R && !dead[r + k]) { up[r] = (int16_t)(r + k); break; }
+    for (int k = 1; k <= 2; ++k) if (r - k >= 0 && !dead[r - k]) { dn[r] = (int16_t)(r - k); break; }
+  }
+  double bound = 0;
+  const double Wz = (double)g->z_max - (double)g->z_min;
+  for (int r = 0; r < R; ++r) {
+    const double Wy = 2.0 * g->row_x[r] * g->tan_half_sector;
+    bound += Wy * Wz / ((double)p->cell_max * p->cell_max) + (Wy + Wz) / p->cell_min + 2.0;
+  }
+  h->cells_per_bucket_bound = bound * S;
+  cudaError_t e = cudaSetDevice(cuda_device);
+  if (e != cudaSuccess) { delete h; return TPC_ERR_CUDA; }
+  bool ok = cudaMalloc(&h->d_row_x, 4 * R) == cudaSuccess && cudaMalloc(&h->d_up, 2 * R) == cudaSuccess &&
+            cudaMalloc(&h->d_dn, 2 * R) == cudaSuccess && cudaMalloc(&h->d_dead, R) == cudaSuccess &&
+            cudaMalloc(&h->d_cnt, 8 * (CNT_COUNT + 1)) == cudaSuccess &&
+            cudaMallocHost(&h->h_cnt, 8 * (CNT_COUNT + 1)) == cudaSuccess &&
+            cudaEventCreate(&h->ev_done) == cudaSuccess;
+  for (int i = 0; ok && i < 7; ++i) ok = cudaEventCreate(&h->ev_stage[i]) == cudaSuccess;
+  ok = ok && cudaMemcpy(h->d_row_x, g->row_x, 4 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
+       cudaMemcpy(h->d_up, up.data(), 2 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
+       cudaMemcpy(h->d_dn, dn.data(), 2 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
+       cudaMemcpy(h->d_dead, dead.data(), R, cudaMemcpyHostToDevice) == cudaSuccess;
+  if (!ok) { tpcDestroy(h); return TPC_ERR_CUDA; }
+  memset(h->h_cnt, 0, 8 * (CNT_COUNT + 1));
+  *out = h;
+  return TPC_OK;
+}
+
+int tpcDestroy(tpcHandle* h) {
+  if (!h) return TPC_ERR_INVALID_ARG;
+  cudaSetDevice(h->device);
+  cudaDeviceSynchronize();
+  cudaFree(h->d_row_x); cudaFree(h->d_up); cudaFree(h->d_dn); cudaFree(h->d_dead); cudaFree(h->d_cnt);
+  if (h->h_cnt) cudaFreeHost(h->h_cnt);
+  if (h->ev_done) cudaEventDestroy(h->ev_done);
+  for (int i = 0; i < 7; ++i) if (h->ev_stage[i]) cudaEventDestroy(h->ev_stage[i]);
+  for (int i = 0; i < 16; ++i) if (h->pool[i]) cudaFree(h->pool[i]);
+  delete h;
+  return TPC_OK;
+}
+
+int tpcWorkspaceBytes(const tpcHandle* h, int64_t n_clusters, int64_t cap_tracklets, size_t* bytes) {
+  if (!h || !bytes || n_clusters < 0 || n_clusters >= (1ll << 31) || cap_tracklets < 0 || cap_tracklets >= (1ll << 31))
+    return TPC_ERR_INVALID_ARG;
+  *bytes = layout(h, n_clusters, cap_tracklets, nullptr).bytes;
+  return TPC_OK;
+}
+
+int tpcSetProfiling(tpcHandle* h, int on) {
+  if (!h) return TPC_ERR_INVALID_ARG;
+  h->profiling = on ? 1 : 0;
+  return TPC_OK;
+}
+
+int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_tracklets, void* workspace,
+           size_t workspace_bytes, void* cuda_stream) {
+  if (!h || !in || !out) return TPC_ERR_INVALID_ARG;
+  const int64_t N = in->n_clusters, capT = cap_tracklets;
+  if (N < 0 || N >= (1ll << 31) || capT < 0 || capT >= (1ll << 31) || !in->row_offset) return TPC_ERR_INVALID_ARG;
+  if (N > 0 && (!in->y || !in->z)) return TPC_ERR_INVALID_ARG;
+  if (out->cap_tracks < 0 || out->cap_track_clusters < 0 || out->cap_tracks >= (1ll << 31) ||
+      out->cap_track_clusters >= (1ll << 32))
+    return TPC_ERR_INVALID_ARG;
+  if (!out->trk_cl_offset) return TPC_ERR_INVALID_ARG;
+  if (out->cap_tracks > 0 && (!out->trk_tracklet || !out->trk_sector || !out->trk_first_row || !out->trk_last_row ||
+                              !out->trk_ncl || !out->trk_x || !out->trk_par || !out->trk_cov || !out->trk_chi2))
+    return TPC_ERR_INVALID_ARG;
+  if (out->cap_track_clusters > 0 && !out->trk_cl_index) return TPC_ERR_INVALID_ARG;
+  if (!workspace || ((uintptr_t)workspace % ALIGN) != 0) return TPC_ERR_INVALID_ARG;
+  const Workspace w = layout(h, N, capT, (char*)workspace);
+  if (workspace_bytes < w.bytes) return TPC_ERR_WORKSPACE_TOO_SMALL;
+  TPC_CUDA(h, cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const DevParams& P = h->P;
+  const int nb = P.n_buckets;
+  const RowTables T{h->d_row_x, h->d_up, h->d_dn, h->d_dead};
+  int64_t* cnt = h->d_cnt;
+  const int wide = (h->params.force_wide_keys || capT >= (1ll << 24)) ? 1 : 0;
+  int L = 0;
+  auto stage = [&](int i) { if (h->profiling) cudaEventRecord(h->ev_stage[i], st); };
+  const unsigned gN256 = (unsigned)ceilDiv(N, 256);
+  const int64_t cc = capCells(h, N);
+
+  stage(0);
+  TPC_CUDA(h, cudaMemsetAsync(cnt, 0, 8 * (CNT_COUNT + 1), st)); ++L;
+  // ---- a1 grid ----------------------------------------------------------------------------------
+  gridSetup<<<1, 1024, 0, st>>>(in->row_offset, N, P, h->d_row_x, w.desc, cnt, cc); ++L;
+  if (N > 0) {
+    TPC_CUDA(h, cudaMemsetAsync(w.cell_start, 0, 4 * (size_t)(cc + 1), st)); ++L;
+    gridCount<<<gN256, 256, 0, st>>>(in->row_offset, in->y, in->z, N, nb, w.desc, w.cell_start, w.rank, cnt,
+                                     h->params.validate_input); ++L;
+    const unsigned tiles = (unsigned)ceilDiv(cc, SCAN_TILE);
+    scanTileSums<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.cell_start, cnt + CNT_N_CELLS, cc, w.tiles32); ++L;
+    scanTileOffsets<uint32_t><<<1, 1024, 0, st>>>(w.tiles32, cnt + CNT_N_CELLS, cc, nullptr); ++L;
+    scanApply<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.cell_start, w.cell_start, cnt + CNT_N_CELLS, cc, w.tiles32); ++L;
+    gridScatter<<<gN256, 256, 0, st>>>(in->row_offset, in->y, in->z, N, nb, w.desc, w.cell_start, w.rank, w.syz, w.s2o,
+                                       cnt); ++L;
+  }
+  stage(1);
+  // ---- a2 neighbour finder ------------------------------------------------------------------------
+  if (N > 0) {
+    neighbourFinder<<<(unsigned)ceilDiv(N, NF_THREADS), NF_THREADS, 0, st>>>(in->row_offset, N, P, T, w.desc, w.cell_start,
+                                                                             w.syz, w.s2o, w.lup, w.ldn, cnt); ++L;
+  }
+  stage(2);
+  // ---- a3 cleaner + start hits --------------------------------------------------------------------
+  const int64_t cpTiles = N > 0 ? ceilDiv(N, CP_TILE) : 0;
+  uint32_t* cpTile = w.tiles32 + ceilDiv(cc + 1, SCAN_TILE) + 1;
+  if (N > 0) {
+    TPC_CUDA(h, cudaMemsetAsync(w.spos_by_orig, 0xFF, 4 * (size_t)N, st)); ++L;
+    cleanLinks<<<gN256, 256, 0, st>>>(N, w.lup, w.ldn, w.s2o, w.cup, w.cdn, w.spos_by_orig, cnt); ++L;
+    startCount<<<(unsigned)cpTiles, CP_THREADS, 0, st>>>(N, w.spos_by_orig, cpTile); ++L;
+  }
+  scanArrayInPlace<uint32_t><<<1, 1024, 0, st>>>(cpTile, cpTiles, cnt + CNT_N_START); ++L;
+  if (N > 0 && capT > 0) {
+    startWrite<<<(unsigned)cpTiles, CP_THREADS, 0, st>>>(N, w.spos_by_orig, cpTile, capT, w.start_orig, w.start_pos); ++L;
+  }
+  stage(3);
+  // ---- a4 tracklet constructor --------------------------------------------------------------------
+  if (N > 0 && capT > 0) {
+    const unsigned grid = (unsigned)std::min<int64_t>(ceilDiv(capT, TC_THREADS), 148 * 64);
+    trackletConstructor<<<grid, TC_THREADS, 0, st>>>(in->row_offset, P, T, w.desc, w.cell_start, w.syz, w.s2o, w.cup,
+                                                     w.start_pos, w.tl, cnt); ++L;
+  }
+  stage(4);
+  // ---- a5 selector ----------------------------------------------------------------------------------
+  const TrackOut to{out->cap_tracks, out->cap_track_clusters, out->trk_tracklet, out->trk_sector, out->trk_first_row,
+                    out->trk_last_row, out->trk_ncl, out->trk_x, out->trk_par, out->trk_cov, out->trk_chi2,
+                    out->trk_cl_offset, out->trk_cl_index};
+  unsigned long long* sel_total = (unsigned long long*)(cnt + CNT_COUNT);
+  if (N > 0 && capT > 0) {
+    const unsigned gT = (unsigned)ceilDiv(capT, 128);
+    TPC_CUDA(h, cudaMemsetAsync(w.owner_key, 0, 8 * (size_t)N, st)); ++L;
+    selectClaim<<<gT, 128, 0, st>>>(w.tl, w.owner_key, wide, cnt); ++L;
+    if (wide) {
+      TPC_CUDA(h, cudaMemsetAsync(w.owner_id, 0xFF, 4 * (size_t)N, st)); ++L;
+      selectClaimId<<<gT, 128, 0, st>>>(w.tl, w.owner_key, w.owner_id, cnt); ++L;
+    }
+    selectCount<<<gT, 128, 0, st>>>(w.tl, w.owner_key, w.owner_id, wide, P.min_track_hits, w.tsel, w.kept_first,
+                                    w.kept_last, cnt); ++L;
+    const unsigned tiles = (unsigned)ceilDiv(capT, SCAN_TILE);
+    scanTileSums<unsigned long long><<<tiles, SCAN_THREADS, 0, st>>>(w.tsel, cnt + CNT_N_START, capT, w.tiles64); ++L;
+    scanTileOffsets<unsigned long long><<<1, 1024, 0, st>>>(w.tiles64, cnt + CNT_N_START, capT, sel_total); ++L;
+    scanApply<unsigned long long><<<tiles, SCAN_THREADS, 0, st>>>(w.tsel, w.tscan, cnt + CNT_N_START, capT, w.tiles64); ++L;
+    selectEmit<<<gT, 128, 0, st>>>(w.tl, w.owner_key, w.owner_id, wide, w.tsel, w.tscan, w.kept_first, w.kept_last,
+                                   w.s2o, to, cnt); ++L;
+  }
+  finalize<<<1, 32, 0, st>>>(sel_total, to, capT, cnt); ++L;
+  stage(5);
+  // ---- optional per-stage exports -----------------------------------------------------------------
+  if (N > 0 && (out->link_up_raw || out->link_dn_raw || out->link_up || out->link_dn)) {
+    exportLinks<<<gN256, 256, 0, st>>>(N, w.s2o, w.lup, w.ldn, w.cup, w.cdn, out->link_up_raw, out->link_dn_raw,
+                                       out->link_up, out->link_dn, cnt); ++L;
+  }
+  if (N > 0 && capT > 0 && (out->start_hits || out->tl_status || out->tl_nhits || out->tl_first_row || out->tl_last_row ||
+                            out->tl_rowhit || out->tl_x || out->tl_par || out->tl_cov || out->tl_chi2)) {
+    const TrackletOut xo{out->start_hits, out->tl_status, out->tl_nhits, out->tl_first_row, out->tl_last_row,
+                         out->tl_rowhit, out->tl_x, out->tl_par, out->tl_cov, out->tl_chi2};
+    exportTracklets<<<(unsigned)ceilDiv(capT, 128), 128, 0, st>>>(w.tl, w.start_orig, w.s2o, P.n_rows, xo, cnt); ++L;
+  }
+  stage(6);
+  TPC_CUDA(h, cudaGetLastError());
+  TPC_CUDA(h, cudaMemcpyAsync(h->h_cnt, cnt, 8 * (CNT_COUNT + 1), cudaMemcpyDeviceToHost, st));
+  TPC_CUDA(h, cudaEventRecord(h->ev_done, st));
+  h->launches = L;
+  h->pending = true;
+  h->last_n = N;
+  return TPC_OK;
+}
+
+int tpcGetRunStatus(tpcHandle* h, tpcRunStatus* out) {
+  if (!h || !out) return TPC_ERR_INVALID_ARG;
+  if (!h->pending) return TPC_ERR_INVALID_ARG;
+  TPC_CUDA(h, cudaEventSynchronize(h->ev_done));
+  memset(out, 0, sizeof(*out));
+  const int64_t* c = h->h_cnt;
+  out->status = (int32_t)c[CNT_ERROR];
+  out->kernel_launches = h->launches;
+  out->n_clusters = h->last_n;
+  out->n_start_hits = c[CNT_N_START];
+  out->n_tracklets = c[CNT_N_TRACKLETS];
+  out->n_tracklet_hits = c[CNT_N_TL_HITS];
+  out->n_tracks = c[CNT_N_TRACKS];
+  out->n_track_clusters = c[CNT_N_TRK_CL];
+  out->n_cells = c[CNT_N_CELLS];
+  if (h->profiling) {
+    for (int i = 0; i < 6; ++i) {
+      float ms = 0;
+      if (cudaEventElapsedTime(&ms, h->ev_stage[i], h->ev_stage[i + 1]) == cudaSuccess) out->stage_ms[i] = ms;
+    }
+    float ms = 0;
+    if (cudaEventElapsedTime(&ms, h->ev_stage[0], h->ev_stage[6]) == cudaSuccess) out->stage_ms[6] = ms;
+  }
+  return TPC_OK;
+}
+
+const char* tpcErrorString(int code) {
+  switch (code) {
+    case TPC_OK: return "ok";
+    case TPC_ERR_INVALID_ARG: return "invalid argument";
+    case TPC_ERR_UNSORTED_OFFSETS: return "row_offset is not a monotone CSR offset array ending at n_clusters";
+    case TPC_ERR_WORKSPACE_TOO_SMALL: return "workspace too small";
+    case TPC_ERR_CAPACITY: return "output capacity exceeded (outputs truncated; see tpcRunStatus for required sizes)";
+    case TPC_ERR_CUDA: return "CUDA runtime error";
+    case TPC_ERR_NONFINITE_INPUT: return "non-finite cluster coordinate";
+    default: return "unknown error";
+  }
+}
+
+const char* tpcLastCudaError(const tpcHandle* h) { return h ? h->cuda_msg : ""; }
+
+}  // extern "C"
+
+// ---- host-buffer convenience path ---------------------------------------------------------------------------
+namespace {
+int poolGet(tpcHandle* h, int idx, size_t bytes, void** p) {
+  if (bytes == 0) bytes = ALIGN;
+  if (h->pool_bytes[idx] < bytes) {
+    if (h->pool[idx]) cudaFree(h->pool[idx]);
+    h->pool[idx] = nullptr; h->pool_bytes[idx] = 0;
+    const size_t want = bytes + bytes / 8;   // head-room so that slowly growing inputs do not reallocate every call
+    TPC_CUDA(h, cudaMalloc(&h->pool[idx], want));
+    h->pool_bytes[idx] = want;
+  }
+  *p = h->pool[idx];
+  return TPC_OK;
+}
+}  // namespace
+
+extern "C" int tpcRunHost(tpcHandle* h, int64_t N, const uint32_t* row_offset, const float* y, const float* z,
+                          tpcTracks* oh, tpcRunStatus* status, void* cuda_stream) {
+  if (!h || !row_offset || !oh || !status || N < 0 || N >= (1ll << 31) || (N > 0 && (!y || !z))) return TPC_ERR_INVALID_ARG;
+  if (oh->link_up_raw || oh->link_dn_raw || oh->link_up || oh->link_dn || oh->start_hits || oh->tl_status || oh->tl_nhits ||
+      oh->tl_first_row || oh->tl_last_row || oh->tl_rowhit || oh->tl_x || oh->tl_par || oh->tl_cov || oh->tl_chi2)
+    return TPC_ERR_INVALID_ARG;
+  if (!oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0) return TPC_ERR_INVALID_ARG;
+  TPC_CUDA(h, cudaSetDevice(h->device));
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const int nb = h->P.n_buckets;
+  int64_t capT = std::max<int64_t>(4096, N / 8), capK = capT, capC = std::max<int64_t>(N, 1);
+  void *d_off, *d_y, *d_z;
+  int rc;
+  if ((rc = poolGet(h, 0, 4 * (size_t)(nb + 1), &d_off)) || (rc = poolGet(h, 1, 4 * (size_t)N, &d_y)) ||
+      (rc = poolGet(h, 2, 4 * (size_t)N, &d_z)))
+    return rc;
+  TPC_CUDA(h, cudaMemcpyAsync(d_off, row_offset, 4 * (size_t)(nb + 1), cudaMemcpyHostToDevice, st));
+  if (N > 0) {
+    TPC_CUDA(h, cudaMemcpyAsync(d_y, y, 4 * (size_t)N, cudaMemcpyHostToDevice, st));
+    TPC_CUDA(h, cudaMemcpyAsync(d_z, z, 4 * (size_t)N, cudaMemcpyHostToDevice, st));
+  }
+  tpcTracks od{};
+  for (int attempt = 0;; ++attempt) {
+    size_t wsb = 0;
+    if ((rc = tpcWorkspaceBytes(h, N, capT, &wsb))) return rc;
+    void* ws;
+    if ((rc = poolGet(h, 3, wsb, &ws))) return rc;
+    void* p[11];
+    const size_t K = (size_t)capK;
+    const size_t sz[11] = {4 * K, 4 * K, 4 * K, 4 * K, 4 * K, 4 * K, 20 * K, 60 * K, 4 * K, 4 * (K + 1), 4 * (size_t)capC};
+    for (int i = 0; i < 11; ++i)
+      if ((rc = poolGet(h, 4 + i, sz[i], &p[i]))) return rc;
+    od = tpcTracks{};
+    od.cap_tracks = capK; od.cap_track_clusters = capC;
+    od.trk_tracklet = (int32_t*)p[0]; od.trk_sector = (int32_t*)p[1]; od.trk_first_row = (int32_t*)p[2];
+    od.trk_last_row = (int32_t*)p[3]; od.trk_ncl = (int32_t*)p[4]; od.trk_x = (float*)p[5]; od.trk_par = (float*)p[6];
+    od.trk_cov = (float*)p[7]; od.trk_chi2 = (float*)p[8]; od.trk_cl_offset = (uint32_t*)p[9];
+    od.trk_cl_index = (uint32_t*)p[10];
+    const tpcClusters in{N, (const uint32_t*)d_off, nullptr, (const float*)d_y, (const float*)d_z, nullptr};
+    if ((rc = tpcRun(h, &in, &od, capT, ws, h->pool_bytes[3], st))) return rc;
+    if ((rc = tpcGetRunStatus(h, status))) return rc;
+    if (status->status != TPC_ERR_CAPACITY || attempt >= 2) break;
+    capT = std::max(capT, status->n_start_hits);
+    capK = std::max(capK, status->n_tracks);
+    capC = std::max(capC, status->n_track_clusters);
+  }
+  if (status->status != TPC_OK) return TPC_OK;   // data-dependent error: reported through *status
+  const int64_t nt = std::min<int64_t>(status->n_tracks, oh->cap_tracks);
+  const int64_t nc = status->n_track_clusters;
+  if (status->n_tracks > oh->cap_tracks || nc > oh->cap_track_clusters) status->status = TPC_ERR_CAPACITY;
+  auto back = [&](void* dst, const void* src, size_t bytes) {
+    return (dst && bytes) ? cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st) : cudaSuccess;
+  };
+  const size_t n4 = 4 * (size_t)nt;
+  TPC_CUDA(h, back(oh->trk_tracklet, od.trk_tracklet, n4));
+  TPC_CUDA(h, back(oh->trk_sector, od.trk_sector, n4));
+  TPC_CUDA(h, back(oh->trk_first_row, od.trk_first_row, n4));
+  TPC_CUDA(h, back(oh->trk_last_row, od.trk_last_row, n4));
+  TPC_CUDA(h, back(oh->trk_ncl, od.trk_ncl, n4));
+  TPC_CUDA(h, back(oh->trk_x, od.trk_x, n4));
+  TPC_CUDA(h, back(oh->trk_chi2, od.trk_chi2, n4));
+  if (nt > 0 && oh->trk_par)
+    TPC_CUDA(h, cudaMemcpy2DAsync(oh->trk_par, 4 * (size_t)oh->cap_tracks, od.trk_par, 4 * (size_t)od.cap_tracks, n4, 5,
+                                  cudaMemcpyDeviceToHost, st));
+  if (nt > 0 && oh->trk_cov)
+    TPC_CUDA(h, cudaMemcpy2DAsync(oh->trk_cov, 4 * (size_t)oh->cap_tracks, od.trk_cov, 4 * (size_t)od.cap_tracks, n4, 15,
+                                  cudaMemcpyDeviceToHost, st));
+  TPC_CUDA(h, back(oh->trk_cl_offset, od.trk_cl_offset, 4 * (size_t)(nt + 1)));
+  if (status->status == TPC_OK) TPC_CUDA(h, back(oh->trk_cl_index, od.trk_cl_index, 4 * (size_t)nc));
+  TPC_CUDA(h, cudaStreamSynchronize(st));
+  return TPC_OK;
+}

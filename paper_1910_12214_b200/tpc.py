@@ -1,0 +1,336 @@
+"""Thin binding of libtpcgpu.so (include/tpc_abi.h): same names, argument marshalling only.
+
+PyTorch is used for device memory and the stream, nothing else: every step of the path (grid, neighbour
+finder, cleaner, tracklet constructor, selector) runs in the library's CUDA kernels.  There is no CPU
+fallback: loading fails loudly when the library cannot be built or loaded.
+"""
+from __future__ import annotations
+
+import ctypes
+from ctypes import POINTER, byref, c_char_p, c_float, c_int, c_int32, c_int64, c_size_t, c_void_p
+from dataclasses import dataclass
+
+import numpy as np
+
+from . import build as _build
+
+TPC_OK = 0
+TPC_ERR_INVALID_ARG = -1
+TPC_ERR_UNSORTED_OFFSETS = -2
+TPC_ERR_WORKSPACE_TOO_SMALL = -3
+TPC_ERR_CAPACITY = -4
+TPC_ERR_CUDA = -5
+TPC_ERR_NONFINITE_INPUT = -6
+
+
+class tpcGeometry(ctypes.Structure):
+    _fields_ = [("n_sectors", c_int32), ("n_rows", c_int32), ("row_x", c_void_p), ("row_pitch", c_void_p),
+                ("row_dead", c_void_p), ("bz_tesla", c_float), ("tan_half_sector", c_float), ("z_min", c_float),
+                ("z_max", c_float)]
+
+
+class tpcParams(ctypes.Structure):
+    _fields_ = [(n, c_float) for n in ("area_y", "area_z", "link_dev2_max", "err2_y", "err2_z", "init_var_s",
+                                       "init_var_t", "init_var_q", "turn_var_scale", "max_sinphi", "road_sigma",
+                                       "road_min", "road_max")] + \
+               [(n, c_int32) for n in ("max_row_gap", "min_chain_hits", "min_tracklet_hits", "min_track_hits")] + \
+               [("cell_min", c_float), ("cell_max", c_float), ("clusters_per_cell", c_float),
+                ("validate_input", c_int32), ("force_wide_keys", c_int32)]
+
+
+class tpcClusters(ctypes.Structure):
+    _fields_ = [("n_clusters", c_int64), ("row_offset", c_void_p), ("x", c_void_p), ("y", c_void_p), ("z", c_void_p),
+                ("q", c_void_p)]
+
+
+_TRK_PTRS = ("trk_tracklet", "trk_sector", "trk_first_row", "trk_last_row", "trk_ncl", "trk_x", "trk_par", "trk_cov",
+             "trk_chi2", "trk_cl_offset", "trk_cl_index")
+_STAGE_PTRS = ("link_up_raw", "link_dn_raw", "link_up", "link_dn", "start_hits", "tl_status", "tl_nhits",
+               "tl_first_row", "tl_last_row", "tl_rowhit", "tl_x", "tl_par", "tl_cov", "tl_chi2")
+
+
+class tpcTracks(ctypes.Structure):
+    _fields_ = [("cap_tracks", c_int64), ("cap_track_clusters", c_int64)] + \
+               [(n, c_void_p) for n in _TRK_PTRS + _STAGE_PTRS]
+
+
+class tpcRunStatus(ctypes.Structure):
+    _fields_ = [("status", c_int32), ("kernel_launches", c_int32), ("n_clusters", c_int64), ("n_start_hits", c_int64),
+                ("n_tracklets", c_int64), ("n_tracklet_hits", c_int64), ("n_tracks", c_int64),
+                ("n_track_clusters", c_int64), ("n_cells", c_int64), ("stage_ms", c_float * 8)]
+
+
+ABI_SYMBOLS = ("tpcDefaultParams", "tpcCreate", "tpcDestroy", "tpcWorkspaceBytes", "tpcRun", "tpcGetRunStatus",
+               "tpcSetProfiling", "tpcRunHost", "tpcErrorString", "tpcLastCudaError")
+
+_lib = None
+
+
+def load_library(build_if_stale: bool = True) -> ctypes.CDLL:
+    """dlopen libtpcgpu.so (building it with nvcc when missing or older than its sources)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if build_if_stale:
+        _build.build_cuda()
+    try:
+        L = ctypes.CDLL(_build.LIB)
+    except OSError as e:   # no fallback: the product path needs the CUDA library
+        raise RuntimeError(f"libtpcgpu.so could not be loaded ({e}); the TPC tracker has no CPU fallback") from e
+    vp = c_void_p
+    L.tpcDefaultParams.argtypes = [POINTER(tpcParams)]
+    L.tpcCreate.argtypes = [POINTER(vp), POINTER(tpcGeometry), POINTER(tpcParams), c_int]
+    L.tpcDestroy.argtypes = [vp]
+    L.tpcWorkspaceBytes.argtypes = [vp, c_int64, c_int64, POINTER(c_size_t)]
+    L.tpcRun.argtypes = [vp, POINTER(tpcClusters), POINTER(tpcTracks), c_int64, vp, c_size_t, vp]
+    L.tpcGetRunStatus.argtypes = [vp, POINTER(tpcRunStatus)]
+    L.tpcSetProfiling.argtypes = [vp, c_int]
+    L.tpcRunHost.argtypes = [vp, c_int64, vp, vp, vp, POINTER(tpcTracks), POINTER(tpcRunStatus), vp]
+    for f in ABI_SYMBOLS[:8]:
+        getattr(L, f).restype = c_int
+    L.tpcErrorString.argtypes = [c_int]
+    L.tpcErrorString.restype = c_char_p
+    L.tpcLastCudaError.argtypes = [vp]
+    L.tpcLastCudaError.restype = c_char_p
+    _lib = L
+    return L
+
+
+class TpcError(RuntimeError):
+    def __init__(self, code: int, where: str, detail: str = ""):
+        self.code = code
+        msg = load_library().tpcErrorString(code).decode()
+        super().__init__(f"{where}: {msg} ({code})" + (f": {detail}" if detail else ""))
+
+
+# ---- the ABI calls under their own names -------------------------------------------------------------------
+def tpcDefaultParams() -> tpcParams:
+    p = tpcParams()
+    rc = load_library().tpcDefaultParams(byref(p))
+    if rc != TPC_OK:
+        raise TpcError(rc, "tpcDefaultParams")
+    return p
+
+
+def tpcCreate(geometry: tpcGeometry, params: tpcParams, cuda_device: int = 0) -> c_void_p:
+    h = c_void_p()
+    rc = load_library().tpcCreate(byref(h), byref(geometry), byref(params), cuda_device)
+    if rc != TPC_OK:
+        raise TpcError(rc, "tpcCreate")
+    return h
+
+
+def tpcDestroy(handle) -> None:
+    load_library().tpcDestroy(handle)
+
+
+def tpcWorkspaceBytes(handle, n_clusters: int, cap_tracklets: int) -> int:
+    b = c_size_t()
+    rc = load_library().tpcWorkspaceBytes(handle, n_clusters, cap_tracklets, byref(b))
+    if rc != TPC_OK:
+        raise TpcError(rc, "tpcWorkspaceBytes")
+    return b.value
+
+
+def tpcRun(handle, clusters: tpcClusters, tracks: tpcTracks, cap_tracklets: int, workspace_ptr: int,
+           workspace_bytes: int, cuda_stream: int = 0) -> None:
+    L = load_library()
+    rc = L.tpcRun(handle, byref(clusters), byref(tracks), cap_tracklets, workspace_ptr, workspace_bytes, cuda_stream)
+    if rc != TPC_OK:
+        raise TpcError(rc, "tpcRun", L.tpcLastCudaError(handle).decode())
+
+
+def tpcGetRunStatus(handle) -> tpcRunStatus:
+    L = load_library()
+    s = tpcRunStatus()
+    rc = L.tpcGetRunStatus(handle, byref(s))
+    if rc != TPC_OK:
+        raise TpcError(rc, "tpcGetRunStatus", L.tpcLastCudaError(handle).decode())
+    return s
+
+
+def tpcSetProfiling(handle, on: bool) -> None:
+    load_library().tpcSetProfiling(handle, int(on))
+
+
+# ---- convenience wrapper: allocation of device tensors with torch, nothing else ---------------------------
+@dataclass
+class TrackResult:
+    """Device tensors (torch) of one tpcRun, trimmed to the counts of the run status."""
+    status: tpcRunStatus
+    n_tracks: int
+    n_track_clusters: int
+    trk: dict          # name -> torch tensor (device); trk_par [5,n], trk_cov [15,n]
+    stages: dict       # optional per-stage outputs (device tensors), empty unless requested
+
+    def numpy(self) -> dict:
+        out = {k: v.cpu().numpy() for k, v in self.trk.items()}
+        out.update({k: v.cpu().numpy() for k, v in self.stages.items()})
+        return out
+
+
+class TpcTracker:
+    """Owns a tpcHandle plus torch-allocated workspace and output buffers (grown on demand)."""
+
+    def __init__(self, n_sectors, n_rows, row_x, row_dead=None, row_pitch=None, bz_tesla=0.5,
+                 tan_half_sector=0.17632698070846498, z_min=-250.0, z_max=250.0, params: tpcParams | None = None,
+                 device: int = 0):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("TpcTracker needs a CUDA device (there is no CPU fallback)")
+        self.torch = torch
+        self.device = torch.device("cuda", device)
+        self.n_sectors, self.n_rows = int(n_sectors), int(n_rows)
+        self._row_x = np.ascontiguousarray(row_x, np.float32)
+        self._row_dead = None if row_dead is None else np.ascontiguousarray(row_dead, np.uint8)
+        self._row_pitch = None if row_pitch is None else np.ascontiguousarray(row_pitch, np.float32)
+        self.params = params if params is not None else tpcDefaultParams()
+        g = tpcGeometry(self.n_sectors, self.n_rows, self._row_x.ctypes.data,
+                        None if self._row_pitch is None else self._row_pitch.ctypes.data,
+                        None if self._row_dead is None else self._row_dead.ctypes.data, bz_tesla, tan_half_sector,
+                        z_min, z_max)
+        self.handle = tpcCreate(g, self.params, device)
+        self._ws = None
+        self._out = {}
+        self._caps = (0, 0, 0)
+
+    @classmethod
+    def from_event(cls, ev, params: tpcParams | None = None, device: int = 0) -> "TpcTracker":
+        return cls(ev.n_sectors, ev.n_rows, ev.row_x, ev.row_dead if np.any(ev.row_dead) else None, ev.row_pitch,
+                   ev.bz_tesla, ev.tan_half_sector, ev.z_min, ev.z_max, params, device)
+
+    def close(self):
+        if getattr(self, "handle", None):
+            tpcDestroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def set_profiling(self, on: bool):
+        tpcSetProfiling(self.handle, on)
+
+    def upload(self, ev):
+        """Copy an Event's row_offset / y / z to the device (torch tensors; int32 view of the uint32 offsets)."""
+        t = self.torch
+        off = t.from_numpy(np.ascontiguousarray(ev.row_offset, np.uint32).view(np.int32)).to(self.device)
+        y = t.from_numpy(np.ascontiguousarray(ev.y, np.float32)).to(self.device)
+        z = t.from_numpy(np.ascontiguousarray(ev.z, np.float32)).to(self.device)
+        return off, y, z
+
+    def _ensure(self, n, capT, capK, capC, stages):
+        t = self.torch
+        need = tpcWorkspaceBytes(self.handle, n, capT)
+        if self._ws is None or self._ws.numel() < need:
+            self._ws = None
+            self._ws = t.empty(need, dtype=t.uint8, device=self.device)
+        i32, f32 = t.int32, t.float32
+        spec = {"trk_tracklet": ((capK,), i32), "trk_sector": ((capK,), i32), "trk_first_row": ((capK,), i32),
+                "trk_last_row": ((capK,), i32), "trk_ncl": ((capK,), i32), "trk_x": ((capK,), f32),
+                "trk_par": ((5, capK), f32), "trk_cov": ((15, capK), f32), "trk_chi2": ((capK,), f32),
+                "trk_cl_offset": ((capK + 1,), i32), "trk_cl_index": ((max(capC, 1),), i32)}
+        if stages:
+            R = self.n_rows
+            spec.update({"link_up_raw": ((max(n, 1),), i32), "link_dn_raw": ((max(n, 1),), i32),
+                         "link_up": ((max(n, 1),), i32), "link_dn": ((max(n, 1),), i32),
+                         "start_hits": ((capT,), i32), "tl_status": ((capT,), i32), "tl_nhits": ((capT,), i32),
+                         "tl_first_row": ((capT,), i32), "tl_last_row": ((capT,), i32), "tl_rowhit": ((capT, R), i32),
+                         "tl_x": ((capT,), f32), "tl_par": ((capT, 5), f32), "tl_cov": ((capT, 15), f32),
+                         "tl_chi2": ((capT,), f32)})
+        for k, (shape, dt) in spec.items():
+            cur = self._out.get(k)
+            if cur is None or tuple(cur.shape) != shape:
+                self._out[k] = t.empty(shape, dtype=dt, device=self.device)
+        for k in list(self._out):
+            if k not in spec:
+                del self._out[k]
+
+    def run(self, row_offset, y, z, cap_tracklets: int | None = None, cap_tracks: int | None = None,
+            cap_track_clusters: int | None = None, stages: bool = False, stream=None, sync: bool = True,
+            grow: bool = True):
+        """One tpcRun on device tensors.  Returns a TrackResult (after synchronising) or None when sync=False."""
+        t = self.torch
+        n = int(y.shape[0])
+        capT = int(cap_tracklets) if cap_tracklets is not None else max(4096, n // 8)
+        capK = int(cap_tracks) if cap_tracks is not None else capT
+        capC = int(cap_track_clusters) if cap_track_clusters is not None else max(n, 1)
+        attempts = 3 if grow else 0     # a too-small cap_tracklets hides the true track counts: up to 3 rounds
+        while True:
+            self._ensure(n, capT, capK, capC, stages)
+            cl = tpcClusters(n, row_offset.data_ptr(), None, y.data_ptr() if n else None, z.data_ptr() if n else None,
+                             None)
+            tr = tpcTracks()
+            tr.cap_tracks, tr.cap_track_clusters = capK, capC
+            for k, v in self._out.items():
+                setattr(tr, k, v.data_ptr())
+            s = stream if stream is not None else t.cuda.current_stream(self.device)
+            tpcRun(self.handle, cl, tr, capT, self._ws.data_ptr(), self._ws.numel(), s.cuda_stream)
+            if not sync:
+                return None
+            st = tpcGetRunStatus(self.handle)
+            if st.status == TPC_ERR_CAPACITY and attempts > 0:
+                capT = max(capT, st.n_start_hits)
+                capK = max(capK, st.n_tracks)
+                capC = max(capC, st.n_track_clusters)
+                attempts -= 1
+                continue
+            break
+        if st.status not in (TPC_OK, TPC_ERR_CAPACITY):
+            raise TpcError(st.status, "tpcRun (device status)")
+        nt = min(int(st.n_tracks), capK)
+        nc = min(int(st.n_track_clusters), capC)
+        ns = min(int(st.n_start_hits), capT)
+        o = self._out
+        trk = {k: (o[k][:, :nt] if o[k].dim() == 2 else o[k][:nt]) for k in _TRK_PTRS[:9]}
+        trk["trk_cl_offset"] = o["trk_cl_offset"][:nt + 1]
+        trk["trk_cl_index"] = o["trk_cl_index"][:nc]
+        stg = {}
+        if stages:
+            for k in _STAGE_PTRS:
+                stg[k] = o[k][:n] if k.startswith("link_") else o[k][:ns]
+        return TrackResult(st, nt, nc, trk, stg)
+
+    def status(self) -> tpcRunStatus:
+        return tpcGetRunStatus(self.handle)
+
+    def run_host(self, row_offset: np.ndarray, y: np.ndarray, z: np.ndarray, cap_tracks: int | None = None,
+                 cap_track_clusters: int | None = None):
+        """tpcRunHost: host (numpy) buffers in, host buffers out; copies are part of the call."""
+        L = load_library()
+        n = int(y.shape[0])
+        capK = int(cap_tracks) if cap_tracks is not None else max(4096, n // 8)
+        capC = int(cap_track_clusters) if cap_track_clusters is not None else max(n, 1)
+        key = (capK, capC)
+        if getattr(self, "_host_key", None) != key:
+            self._host = {"trk_tracklet": np.empty(capK, np.int32), "trk_sector": np.empty(capK, np.int32),
+                          "trk_first_row": np.empty(capK, np.int32), "trk_last_row": np.empty(capK, np.int32),
+                          "trk_ncl": np.empty(capK, np.int32), "trk_x": np.empty(capK, np.float32),
+                          "trk_par": np.empty((5, capK), np.float32), "trk_cov": np.empty((15, capK), np.float32),
+                          "trk_chi2": np.empty(capK, np.float32), "trk_cl_offset": np.empty(capK + 1, np.uint32),
+                          "trk_cl_index": np.empty(capC, np.uint32)}
+            self._host_key = key
+        tr = tpcTracks()
+        tr.cap_tracks, tr.cap_track_clusters = capK, capC
+        for k, v in self._host.items():
+            setattr(tr, k, v.ctypes.data)
+        st = tpcRunStatus()
+        off = np.ascontiguousarray(row_offset, np.uint32)
+        y = np.ascontiguousarray(y, np.float32)
+        z = np.ascontiguousarray(z, np.float32)
+        s = self.torch.cuda.current_stream(self.device).cuda_stream
+        rc = L.tpcRunHost(self.handle, n, off.ctypes.data, y.ctypes.data if n else None, z.ctypes.data if n else None,
+                          byref(tr), byref(st), s)
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpcRunHost", L.tpcLastCudaError(self.handle).decode())
+        if st.status not in (TPC_OK, TPC_ERR_CAPACITY):
+            raise TpcError(st.status, "tpcRunHost (device status)")
+        nt = min(int(st.n_tracks), capK)
+        nc = min(int(st.n_track_clusters), capC)
+        h = self._host
+        out = {k: (h[k][:, :nt] if h[k].ndim == 2 else h[k][:nt]) for k in _TRK_PTRS[:9]}
+        out["trk_cl_offset"] = h["trk_cl_offset"][:nt + 1]
+        out["trk_cl_index"] = h["trk_cl_index"][:nc]
+        return st, out

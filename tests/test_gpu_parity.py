@@ -1,0 +1,210 @@
+"""-m gpu: the CUDA path (through the C ABI) against the CPU oracle, element by element.
+
+Sizes: the oracle finishes each case in seconds; the cases span many grid cells, several thread blocks
+and ragged tails.  Full-size configs are covered by tests/test_gpu_full.py.
+"""
+import numpy as np
+import pytest
+
+from oracle import tpc_oracle as orc
+from paper_1910_12214_b200 import datagen
+from tests.parity import compare
+
+pytestmark = pytest.mark.gpu
+
+R = 152
+
+
+def _tracker(ev, **par):
+    from paper_1910_12214_b200 import tpc
+    p = tpc.tpcDefaultParams()
+    for k, v in par.items():
+        setattr(p, k, v)
+    return tpc.TpcTracker.from_event(ev, params=p)
+
+
+def _oracle_params(**par):
+    p = orc.default_params()
+    for k, v in par.items():
+        if hasattr(p, k):
+            setattr(p, k, v)
+    return p
+
+
+def _run_both(ev, stages=True, **par):
+    trk = _tracker(ev, **par)
+    off, y, z = trk.upload(ev)
+    res = trk.run(off, y, z, stages=stages)
+    assert res.status.status == 0
+    g = res.numpy()
+    o = orc.run(ev, _oracle_params(**par))
+    rep = compare(g, o, ev.n_rows, check_stages=stages)
+    trk.close()
+    return rep, res, o
+
+
+@pytest.mark.parametrize("idx,scale", [(0, 1.0), (1, 0.1), (2, 0.1), (3, 0.06), (4, 0.02)])
+def test_parity_configs_scaled(idx, scale):
+    ev = datagen.make_event(idx, scale=scale)
+    rep, res, o = _run_both(ev)
+    assert o.n_tracks > 0
+    print(ev.name, ev.n_clusters, "tracks", o.n_tracks, rep)
+
+
+def test_parity_config1_full():
+    """BASELINE.json configs[1] at full size (1.46 M clusters; the oracle needs ~2 s)."""
+    ev = datagen.make_event(1)
+    rep, res, o = _run_both(ev)
+    assert o.n_tracks > 10000
+    print(rep)
+
+
+def test_parity_config2_full():
+    ev = datagen.make_event(2)
+    rep, res, o = _run_both(ev)
+    print(rep)
+
+
+def test_parity_dense_window_overflows_the_candidate_stash():
+    """More than NF_STASH (12) down candidates per window: the re-enumeration path of the neighbour finder."""
+    rng = np.random.default_rng(3)
+    counts = np.zeros(R, np.int64)
+    ys, zs = [], []
+    for r in range(30, 60):
+        k = 1500
+        counts[r] = k
+        ys.append(rng.uniform(-6, 6, k))
+        zs.append(rng.uniform(-6, 6, k))      # ~10 clusters / cm^2 -> ~100 candidates per 3.2 x 3.2 cm window
+    off = np.concatenate([[0], np.cumsum(counts)])
+    ev = datagen.event_from_arrays(off, np.concatenate(ys), np.concatenate(zs), 1, R)
+    rep, res, o = _run_both(ev)
+    assert (o.link_up_raw >= 0).sum() > 1000
+
+
+def test_parity_exact_ties_use_the_original_index():
+    """Duplicated clusters (exact ties in Dev and in the search distance), shuffled input order."""
+    ev0 = datagen.make_event(1, scale=0.02)
+    rng = np.random.default_rng(11)
+    counts = np.diff(ev0.row_offset.astype(np.int64))
+    ys, zs, newc = [], [], []
+    for b in range(len(counts)):
+        lo, hi = ev0.row_offset[b], ev0.row_offset[b + 1]
+        y = np.concatenate([ev0.y[lo:hi], ev0.y[lo:hi]])      # every cluster twice
+        z = np.concatenate([ev0.z[lo:hi], ev0.z[lo:hi]])
+        p = rng.permutation(len(y))
+        ys.append(y[p])
+        zs.append(z[p])
+        newc.append(len(y))
+    off = np.concatenate([[0], np.cumsum(newc)])
+    ev = datagen.event_from_arrays(off, np.concatenate(ys), np.concatenate(zs), ev0.n_sectors, R)
+    rep, res, o = _run_both(ev)
+    assert o.n_tracks > 0
+
+
+def test_parity_dead_rows():
+    ev = datagen.make_event(0, dead_rows=(40, 97))
+    rep, res, o = _run_both(ev)
+    assert o.n_tracks > 50
+    ev = datagen.make_event(1, scale=0.05, dead_rows=(1, 40, 41, 97, 150))
+    _run_both(ev)
+
+
+def test_parity_wide_selector_keys():
+    """R27: the two-pass (wide) selector keys give the same tracks as the packed 64-bit key."""
+    ev = datagen.make_event(2, scale=0.1)
+    _run_both(ev, force_wide_keys=1)
+
+
+def test_parity_other_parameters():
+    ev = datagen.make_event(1, scale=0.05)
+    _run_both(ev, road_sigma=3.0, max_row_gap=2, min_track_hits=20, min_tracklet_hits=15, link_dev2_max=0.3,
+              clusters_per_cell=3.0)
+    _run_both(ev, clusters_per_cell=0.25, cell_min=0.3)
+
+
+def test_determinism_two_runs_identical_bytes():
+    ev = datagen.make_event(3, scale=0.06)
+    trk = _tracker(ev)
+    off, y, z = trk.upload(ev)
+    a = trk.run(off, y, z, stages=True).numpy()
+    a = {k: v.copy() for k, v in a.items()}
+    b = trk.run(off, y, z, stages=True).numpy()
+    for k in a:
+        assert np.array_equal(a[k], b[k]), k
+    trk.close()
+
+
+def test_empty_and_tiny_inputs():
+    from paper_1910_12214_b200 import tpc
+    ev = datagen.event_from_arrays(np.zeros(R + 1, np.uint32), [], [], 1, R)
+    trk = _tracker(ev)
+    off, y, z = trk.upload(ev)
+    res = trk.run(off, y, z, stages=True)
+    assert res.status.status == 0 and res.n_tracks == 0 and res.status.n_start_hits == 0
+    assert int(res.trk["trk_cl_offset"][0]) == 0
+    trk.close()
+    counts = np.zeros(R, np.int64)
+    counts[10] = 1
+    ev = datagen.event_from_arrays(np.concatenate([[0], np.cumsum(counts)]), [0.0], [0.0], 1, R)
+    _run_both(ev)
+    assert tpc.TPC_OK == 0
+
+
+def test_capacity_overflow_is_reported_and_nothing_is_written_out_of_bounds():
+    from paper_1910_12214_b200 import tpc
+    ev = datagen.make_event(1, scale=0.1)
+    trk = _tracker(ev)
+    off, y, z = trk.upload(ev)
+    full = trk.run(off, y, z)
+    assert full.status.status == 0
+    nt, nc, ns = full.n_tracks, full.n_track_clusters, int(full.status.n_start_hits)
+    ref = {k: v.clone() for k, v in full.trk.items()}
+    # tracks capacity too small: status CAPACITY, required sizes reported, the first cap tracks are intact
+    res = trk.run(off, y, z, cap_tracks=nt // 2, grow=False)
+    assert res.status.status == tpc.TPC_ERR_CAPACITY
+    assert res.status.n_tracks == nt and res.status.n_track_clusters == nc
+    assert np.array_equal(res.trk["trk_tracklet"].cpu().numpy(), ref["trk_tracklet"][:nt // 2].cpu().numpy())
+    # cluster-index capacity too small
+    res = trk.run(off, y, z, cap_track_clusters=nc // 3, grow=False)
+    assert res.status.status == tpc.TPC_ERR_CAPACITY and res.status.n_track_clusters == nc
+    # tracklet capacity too small: required cap_tracklets reported
+    res = trk.run(off, y, z, cap_tracklets=ns // 2, grow=False)
+    assert res.status.status == tpc.TPC_ERR_CAPACITY and res.status.n_start_hits == ns
+    # and the automatic growth path recovers the full result
+    res = trk.run(off, y, z, cap_tracklets=ns // 2, cap_tracks=nt // 2, cap_track_clusters=nc // 3)
+    assert res.status.status == 0 and res.n_tracks == nt
+    for k in ref:
+        assert np.array_equal(res.trk[k].cpu().numpy(), ref[k].cpu().numpy()), k
+    trk.close()
+
+
+def test_bad_offsets_and_non_finite_input_are_reported():
+    from paper_1910_12214_b200 import tpc
+    ev = datagen.make_event(0)
+    trk = _tracker(ev, validate_input=1)
+    off, y, z = trk.upload(ev)
+    bad = off.clone()
+    bad[3] = bad[4] + 5            # off[4] < off[3]: not monotone
+    with pytest.raises(tpc.TpcError) as e:
+        trk.run(bad, y, z)
+    assert e.value.code == tpc.TPC_ERR_UNSORTED_OFFSETS
+    y2 = y.clone()
+    y2[100] = float("nan")
+    with pytest.raises(tpc.TpcError) as e:
+        trk.run(off, y2, z)
+    assert e.value.code == tpc.TPC_ERR_NONFINITE_INPUT
+    res = trk.run(off, y, z)      # the handle is still usable
+    assert res.status.status == 0 and res.n_tracks > 0
+    trk.close()
+
+
+def test_run_host_matches_device_path():
+    ev = datagen.make_event(1, scale=0.1)
+    trk = _tracker(ev)
+    off, y, z = trk.upload(ev)
+    dev = trk.run(off, y, z).numpy()
+    st, host = trk.run_host(ev.row_offset, ev.y, ev.z)
+    assert st.status == 0
+    for k in host:
+        assert np.array_equal(np.asarray(host[k]).view(np.int32) if host[k].dtype == np.uint32 else host[k], dev[k]), k
+    trk.close()
