@@ -1,0 +1,299 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the TPC sector tracker (a1..a5 in one tpcRun) on synthetic time frames.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config 4] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (grid, neighbour finder, cleaner + start hits, tracklet
+constructor, selector) over one synthetic event.  At N=1 the workload is BASELINE.json configs[4] (the
+200-collision time frame the north_star quotes its target on); with N>1 every rank tracks its own
+time frame (different seed), no data-path collective ("replicas only") -> weak scaling.
+Prints ONE JSON line (rank 0).  See DESIGN.md section 8 for the roofline accounting.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "tpc_clusters_per_s_tracked"
+UNIT = "clusters/s"
+WORKLOADS = {0: "config0 single sector, 200 primaries", 1: "config1 central Pb-Pb-like event, 8000 primaries",
+             2: "config2 loopers + primaries", 3: "config3 time slice, 50 collisions",
+             4: "config4 time frame, 200 collisions"}
+
+
+def _peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 100 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows = []
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms",
+                                          "100", "-i", str(index)], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL,
+                                         text=True)
+            self.th = threading.Thread(target=self._read, daemon=True)
+            self.th.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append((time.time(), line.strip()))
+
+    def stop(self, t0: float, t1: float) -> dict:
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        rows = [r for (t, r) in self.rows if t0 <= t <= t1 + 0.1] or [r for (_, r) in self.rows]
+        for r in rows:
+            f = [x.strip() for x in r.split(",")]
+            try:
+                sm.append(float(f[0]))
+                mx.append(float(f[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, f[2:6]):
+                if v == "Active":
+                    reasons.add(n)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": sorted(reasons), "samples": len(sm)}
+
+
+def _sector_sample(ev, n_keep_sectors=1, z_frac=1.0):
+    """Bounded sample of the workload for the CPU oracle: the first sector(s), optionally a z slab of it."""
+    from paper_1910_12214_b200 import datagen
+    R = ev.n_rows
+    hi = int(ev.row_offset[n_keep_sectors * R])
+    off = ev.row_offset[:n_keep_sectors * R + 1].astype(np.int64)
+    y, z = ev.y[:hi], ev.z[:hi]
+    if z_frac < 1.0:
+        zc = 0.5 * (ev.z_min + ev.z_max) + 0.25 * (ev.z_max - ev.z_min)     # slab inside the z > 0 drift volume
+        hw = 0.25 * (ev.z_max - ev.z_min) * z_frac
+        keep = np.abs(z - zc) <= hw
+        bucket = np.repeat(np.arange(n_keep_sectors * R), np.diff(off))
+        counts = np.bincount(bucket[keep], minlength=n_keep_sectors * R)
+        off = np.concatenate([[0], np.cumsum(counts)])
+        y, z = y[keep], z[keep]
+    return datagen.event_from_arrays(off, y, z, n_keep_sectors, R, row_x=ev.row_x, z_min=ev.z_min, z_max=ev.z_max,
+                                     bz_tesla=ev.bz_tesla)
+
+
+def _time_oracle(sample, repeats=1):
+    from oracle import tpc_oracle as orc
+    best = None
+    for _ in range(repeats):
+        t = time.perf_counter()
+        res = orc.run(sample)
+        dt = time.perf_counter() - t
+        best = dt if best is None else min(best, dt)
+    return best, res
+
+
+def run_reference(args, rank):
+    """--impl reference: the CPU oracle as it stands, single thread, on a bounded sample of the same workload."""
+    if rank != 0:
+        return
+    from paper_1910_12214_b200 import datagen
+    ev = datagen.make_event(args.config)
+    total = args.steps + args.warmup
+    # one sector of config 4 costs ~15 s on one core; keep the whole run within ~150 s
+    z_frac = 1.0
+    if ev.n_sectors > 1 and ev.n_clusters > 5e6:
+        z_frac = min(1.0, max(0.02, 150.0 / (15.0 * max(total, 1))))
+    sample = _sector_sample(ev, 1, z_frac) if ev.n_sectors > 1 and ev.n_clusters > 2e6 else ev
+    times = []
+    for i in range(total):
+        dt, _ = _time_oracle(sample)
+        if i >= args.warmup:
+            times.append(dt)
+    ms = 1e3 * float(np.mean(times)) if times else 0.0
+    value = sample.n_clusters / (ms * 1e-3) if ms > 0 else 0.0
+    desc = (f"sector 0 of {WORKLOADS[args.config]}" + (f", z slab of {z_frac:.2f} of the drift length" if z_frac < 1 else "")
+            + f" ({sample.n_clusters} clusters per step)") if sample is not ev else f"whole event ({ev.n_clusters} clusters)"
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": WORKLOADS[args.config], "n_clusters_per_step": int(sample.n_clusters), "sample": desc},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": desc},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line), flush=True)
+
+
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_1910_12214_b200 import datagen, tpc
+
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the tracker has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    # every rank tracks its own time frame (replicas: independent data per GPU)
+    ev = datagen.generate(datagen.config(args.config, seed=args.config + 1 + 100 * rank), name=f"config{args.config}")
+    N = ev.n_clusters
+    trk = tpc.TpcTracker.from_event(ev, device=local_rank)
+    off, y, z = trk.upload(ev)
+    first = trk.run(off, y, z)                     # discovers the capacities (grows once if needed)
+    st0 = first.status
+    assert st0.status == 0, st0.status
+    capT = int(st0.n_start_hits * 1.05) + 1024
+    capK = int(st0.n_tracks * 1.05) + 1024
+    capC = int(st0.n_track_clusters * 1.05) + 1024
+    trk.set_profiling(True)
+    stream = torch.cuda.current_stream()
+
+    def step():
+        trk.run(off, y, z, cap_tracklets=capT, cap_tracks=capK, cap_track_clusters=capC, sync=False)
+
+    for _ in range(max(args.warmup, 3)):
+        step()
+    st = trk.status()
+    assert st.status == 0
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    t0 = time.time()
+    stage = np.zeros(8)
+    e0.record(stream)
+    for _ in range(args.steps):
+        step()
+        s = trk.status()                            # waits for the step; per-stage CUDA-event times of this step
+        stage += np.array(list(s.stage_ms))
+    e1.record(stream)
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t1 = time.time()
+    ms_total = e0.elapsed_time(e1)
+    clusters = torch.tensor([float(N)], device="cuda")
+    tmax = torch.tensor([ms_total], device="cuda")
+    if world > 1:
+        dist.all_reduce(clusters, op=dist.ReduceOp.SUM)
+        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
+    ms_step = float(tmax.item()) / args.steps
+    value = float(clusters.item()) / (ms_step * 1e-3)
+    clocks = sampler.stop(t0, t1) if sampler else None
+    stage /= args.steps
+
+    # ---- end to end through the host-buffer ABI call (pinned host memory; copies inside the timed region) ----
+    hy = torch.from_numpy(ev.y).pin_memory()
+    hz = torch.from_numpy(ev.z).pin_memory()
+    hoff = torch.from_numpy(ev.row_offset.view(np.int32)).pin_memory()
+    ny, nz, noff = hy.numpy(), hz.numpy(), hoff.numpy().view(np.uint32)
+    e2e_steps = max(1, min(args.steps, 5))
+    sth, outh = trk.run_host(noff, ny, nz, cap_tracks=capK, cap_track_clusters=capC)     # warm-up: pools grow here
+    assert sth.status == 0
+    if world > 1:
+        dist.barrier()
+    torch.cuda.synchronize()
+    e0.record(stream)
+    for _ in range(e2e_steps):
+        sth, outh = trk.run_host(noff, ny, nz, cap_tracks=capK, cap_track_clusters=capC)
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms_e2e = torch.tensor([e0.elapsed_time(e1) / e2e_steps], device="cuda")
+    if world > 1:
+        dist.all_reduce(ms_e2e, op=dist.ReduceOp.MAX)
+    e2e_value = float(clusters.item()) / (float(ms_e2e.item()) * 1e-3)
+    nt, nc = int(sth.n_tracks), int(sth.n_track_clusters)
+    h2d = 4 * (len(ev.row_offset)) + 8 * N
+    d2h = nt * (5 * 4 + 4 + 20 + 60 + 4) + 4 * (nt + 1) + 4 * nc + 8 * 9
+
+    if rank != 0:
+        return
+    # ---- roofline of the dominant kernel (algorithmic bytes per stage) -------------------
+    peak, peak_src = _peaks()
+    H = int(st.n_tracklet_hits)
+    nT = int(st.n_tracklets)
+    alg = {"a1_grid": 24 * N, "a2_neighbours": 20 * N, "a3_cleaner_start": 24 * N, "a4_constructor": 40 * H + 100 * nT,
+           "a5_selector": 32 * H}
+    names = list(alg)
+    stages = {}
+    for i, k in enumerate(names):
+        ms = float(stage[i])
+        stages[k] = {"ms": round(ms, 4), "alg_bytes": int(alg[k]),
+                     "gbs": round(alg[k] / (ms * 1e-3) / 1e9, 1) if ms > 0 else None}
+    dom = max(names, key=lambda k: stages[k]["ms"])
+    dom_ms = stages[dom]["ms"]
+    achieved = alg[dom] / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0
+    total_alg = sum(alg.values())
+    roofline = {"bound": "hbm", "kernel": {"a4_constructor": "trackletConstructor", "a2_neighbours": "neighbourFinder"}.get(dom, dom),
+                "achieved": round(achieved, 2), "peak": peak, "unit": "GB/s", "frac": round(achieved / peak, 5),
+                "traffic": None, "peak_source": peak_src,
+                "whole_path": {"alg_bytes": int(total_alg), "gbs": round(total_alg / (ms_step * 1e-3) / 1e9, 1),
+                               "frac": round(total_alg / (ms_step * 1e-3) / 1e9 / peak, 5)},
+                "share_of_step": round(dom_ms / max(float(stage[6]), 1e-9), 4)}
+    # ---- CPU baseline: the oracle on one sector of this event (rank 0, N = 1 only) ----------------------------
+    cpu = None
+    if world == 1 and not args.no_cpu_baseline:
+        sample = _sector_sample(ev, 1) if ev.n_sectors > 1 and N > 2e6 else ev
+        dt, ores = _time_oracle(sample)
+        cpu = {"value": sample.n_clusters / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
+               "sample": (f"sector 0 of the event ({sample.n_clusters} clusters, 1/{ev.n_sectors} of the step), {dt:.1f} s"
+                          if sample is not ev else f"whole event ({N} clusters), {dt:.2f} s"),
+               "host_cores_available": os.cpu_count()}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic",
+            "config": {"workload": WORKLOADS[args.config], "n_clusters_per_gpu": N, "n_sectors": ev.n_sectors,
+                       "n_rows": ev.n_rows, "cache": "inputs_larger_than_L2" if 8 * N > 126e6 else "working set may fit L2",
+                       "parallelism": f"replicas x{world}", "tracks_per_step": int(st.n_tracks),
+                       "tracklets_per_step": nT, "start_hits_per_step": int(st.n_start_hits), "tracklet_hits": H},
+            "tracks_per_s": float(st.n_tracks) * world / (ms_step * 1e-3),
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                    "ms_per_step": float(ms_e2e.item()), "steps": e2e_steps},
+            "gpu_launches": int(st.kernel_launches) * args.steps,
+            "clocks": clocks, "roofline": roofline, "stages": stages, "cpu_baseline": cpu}
+    print(json.dumps(line), flush=True)
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=4, choices=sorted(WORKLOADS))
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+        return
+    run_ours(args, rank, world, local_rank)
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

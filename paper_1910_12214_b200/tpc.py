@@ -305,12 +305,17 @@ class TpcTracker:
         capC = int(cap_track_clusters) if cap_track_clusters is not None else max(n, 1)
         key = (capK, capC)
         if getattr(self, "_host_key", None) != key:
-            self._host = {"trk_tracklet": np.empty(capK, np.int32), "trk_sector": np.empty(capK, np.int32),
-                          "trk_first_row": np.empty(capK, np.int32), "trk_last_row": np.empty(capK, np.int32),
-                          "trk_ncl": np.empty(capK, np.int32), "trk_x": np.empty(capK, np.float32),
-                          "trk_par": np.empty((5, capK), np.float32), "trk_cov": np.empty((15, capK), np.float32),
-                          "trk_chi2": np.empty(capK, np.float32), "trk_cl_offset": np.empty(capK + 1, np.uint32),
-                          "trk_cl_index": np.empty(capC, np.uint32)}
+            t = self.torch
+
+            def pinned(shape, dt, view=None):     # pinned host memory: D2H copies run at full PCIe/C2C speed
+                a = t.empty(shape, dtype=dt, pin_memory=True).numpy()
+                return a.view(view) if view is not None else a
+            i32, f32 = t.int32, t.float32
+            self._host = {"trk_tracklet": pinned(capK, i32), "trk_sector": pinned(capK, i32),
+                          "trk_first_row": pinned(capK, i32), "trk_last_row": pinned(capK, i32),
+                          "trk_ncl": pinned(capK, i32), "trk_x": pinned(capK, f32), "trk_par": pinned((5, capK), f32),
+                          "trk_cov": pinned((15, capK), f32), "trk_chi2": pinned(capK, f32),
+                          "trk_cl_offset": pinned(capK + 1, i32, np.uint32), "trk_cl_index": pinned(capC, i32, np.uint32)}
             self._host_key = key
         tr = tpcTracks()
         tr.cap_tracks, tr.cap_track_clusters = capK, capC
