@@ -62,6 +62,7 @@ struct tpcHandle {
   cudaEvent_t ev_stage[7] = {};
   int profiling = 0;
   int launches = 0;
+  int tc_grid = 148;               // persistent grid of the tracklet constructor: SMs x resident blocks
   bool pending = false;
   int64_t last_n = 0;
   double cells_per_bucket_bound = 0;   // sum over buckets of the n-independent part of the cell bound
@@ -112,6 +113,7 @@ Workspace layout(const tpcHandle* h, int64_t N, int64_t capT, char* base) {
   w.start_orig = (uint32_t*)take(4 * (size_t)Tn);
   w.start_pos = (uint32_t*)take(4 * (size_t)Tn);
   w.tl.capT = capT;
+  w.tl.n_rows = R;
   w.tl.status = (int32_t*)take(4 * (size_t)Tn);
   w.tl.nhits = (int32_t*)take(4 * (size_t)Tn);
   w.tl.first_row = (int32_t*)take(4 * (size_t)Tn);
@@ -205,6 +207,13 @@ int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cud
        cudaMemcpy(h->d_dn, dn.data(), 2 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
        cudaMemcpy(h->d_dead, dead.data(), R, cudaMemcpyHostToDevice) == cudaSuccess;
   if (!ok) { tpcDestroy(h); return TPC_ERR_CUDA; }
+  {
+    int sms = 148, per_sm = 1;
+    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, cuda_device);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trackletConstructor, TC_THREADS, 0) != cudaSuccess || per_sm < 1)
+      per_sm = 1;
+    h->tc_grid = sms * per_sm;
+  }
   memset(h->h_cnt, 0, 8 * (CNT_COUNT + 1));
   *out = h;
   return TPC_OK;
@@ -302,7 +311,7 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   stage(3);
   // ---- a4 tracklet constructor --------------------------------------------------------------------
   if (N > 0 && capT > 0) {
-    const unsigned grid = (unsigned)std::min<int64_t>(ceilDiv(capT, TC_THREADS), 148 * 64);
+    const unsigned grid = (unsigned)std::min<int64_t>(ceilDiv(capT, TC_THREADS), h->tc_grid);
     trackletConstructor<<<grid, TC_THREADS, 0, st>>>(in->row_offset, P, T, w.desc, w.cell_start, w.syz, w.s2o, w.cup,
                                                      w.start_pos, w.tl, cnt); ++L;
   }

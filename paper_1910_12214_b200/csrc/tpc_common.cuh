@@ -55,8 +55,9 @@ struct TrackletStore {
   float* par;           // [5][capT]
   float* cov;           // [15][capT]
   float* chi2;          // [capT]
-  int32_t* rowhit;      // [n_rows][capT] sorted positions, valid for first_row..last_row only
+  int32_t* rowhit;      // [capT][n_rows] sorted positions, valid for first_row..last_row only
   int64_t capT;
+  int32_t n_rows;
 };
 
 __device__ __forceinline__ int cellCoord(float v, float v0, float inv_e, int n) {
@@ -82,6 +83,8 @@ __device__ __forceinline__ bool finitef(float v) { return (__float_as_uint(v) & 
 // Enumerate the clusters of one bucket inside the closed window [yc-wy, yc+wy] x [zc-wz, zc+wz].
 // The grid gives a superset (whole cells, with slack for the rounding of the predicate's subtraction);
 // the exact fp32 predicate of DESIGN.md O2/O4 decides.  f(pos, y, z) is called for every accepted cluster.
+// One flat loop: an iteration either tests one candidate or advances to the next cell row, so that the lanes
+// of a warp stay together whatever the lengths of their cell ranges are.
 template <typename F>
 __device__ __forceinline__ void forWindow(const GridDesc& G, const uint32_t* __restrict__ cell_start,
                                           const float2* __restrict__ syz, float yc, float zc, float wy, float wz, F&& f) {
@@ -90,15 +93,20 @@ __device__ __forceinline__ void forWindow(const GridDesc& G, const uint32_t* __r
   const float sz = 1e-5f * (fabsf(zc) + wz) + 1e-6f;
   const int by0 = cellCoord((yc - wy) - sy, G.y0, G.inv_e, G.ny);
   const int by1 = cellCoord((yc + wy) + sy, G.y0, G.inv_e, G.ny);
-  const int bz0 = cellCoord((zc - wz) - sz, G.z0, G.inv_e, G.nz);
+  int bz = cellCoord((zc - wz) - sz, G.z0, G.inv_e, G.nz);
   const int bz1 = cellCoord((zc + wz) + sz, G.z0, G.inv_e, G.nz);
-  const uint32_t* cs = cell_start + G.cell_base;
-  for (int bz = bz0; bz <= bz1; ++bz) {
-    const uint32_t k0 = __ldg(cs + bz * G.ny + by0);
-    const uint32_t k1 = __ldg(cs + bz * G.ny + by1 + 1);
-    for (uint32_t k = k0; k < k1; ++k) {
+  const uint32_t* cs = cell_start + G.cell_base + by0;
+  const int span = by1 - by0 + 1;
+  uint32_t k = __ldg(cs + bz * G.ny), kend = __ldg(cs + bz * G.ny + span);
+  for (;;) {
+    if (k < kend) {
       const float2 c = __ldg(syz + k);
       if (fabsf(c.x - yc) <= wy && fabsf(c.y - zc) <= wz) f(k, c.x, c.y);
+      ++k;
+    } else {
+      if (++bz > bz1) break;
+      k = __ldg(cs + bz * G.ny);
+      kend = __ldg(cs + bz * G.ny + span);
     }
   }
 }

@@ -25,7 +25,7 @@ __global__ void __launch_bounds__(128) selectClaim(TrackletStore tl, unsigned lo
   const unsigned long long key = selKey(tl.nhits[t], tl.chi2[t], (uint32_t)t, wide != 0);
   const int r1 = tl.last_row[t];
   for (int r = tl.first_row[t]; r <= r1; ++r) {
-    const int32_t c = tl.rowhit[(int64_t)r * tl.capT + t];
+    const int32_t c = tl.rowhit[t * tl.n_rows + r];
     if (c >= 0) atomicMax(owner_key + c, key);
   }
 }
@@ -40,7 +40,7 @@ __global__ void __launch_bounds__(128) selectClaimId(TrackletStore tl, const uns
   const unsigned long long key = selKey(tl.nhits[t], tl.chi2[t], (uint32_t)t, true);
   const int r1 = tl.last_row[t];
   for (int r = tl.first_row[t]; r <= r1; ++r) {
-    const int32_t c = tl.rowhit[(int64_t)r * tl.capT + t];
+    const int32_t c = tl.rowhit[t * tl.n_rows + r];
     if (c >= 0 && owner_key[c] == key) atomicMin(owner_id + c, (uint32_t)t);
   }
 }
@@ -71,7 +71,7 @@ __global__ void __launch_bounds__(128) selectCount(TrackletStore tl, const unsig
       int kept = 0, first = -1, last = -1;
       const int r1 = tl.last_row[t];
       for (int r = tl.first_row[t]; r <= r1; ++r) {
-        const int32_t c = tl.rowhit[(int64_t)r * tl.capT + t];
+        const int32_t c = tl.rowhit[t * tl.n_rows + r];
         if (c >= 0 && owns(c, key, (uint32_t)t, wide, owner_key, owner_id)) { ++kept; if (first < 0) first = r; last = r; }
       }
       if (kept >= min_track_hits) {
@@ -134,7 +134,7 @@ __global__ void __launch_bounds__(128) selectEmit(TrackletStore tl, const unsign
   int64_t w = off;
   const int r1 = tl.last_row[t];
   for (int r = tl.first_row[t]; r <= r1; ++r) {
-    const int32_t c = tl.rowhit[(int64_t)r * capT + t];
+    const int32_t c = tl.rowhit[t * tl.n_rows + r];
     if (c >= 0 && owns(c, key, (uint32_t)t, wide, owner_key, owner_id)) {
       if (w < o.cap_cl) o.cl_index[w] = s2o[c];
       ++w;
@@ -197,7 +197,7 @@ __global__ void __launch_bounds__(128) exportTracklets(TrackletStore tl, const u
   const bool has = st != 0 && f >= 0;
   if (o.rowhit)
     for (int r = 0; r < n_rows; ++r) {
-      int32_t c = (has && r >= f && r <= l) ? tl.rowhit[(int64_t)r * capT + t] : -1;
+      int32_t c = (has && r >= f && r <= l) ? tl.rowhit[t * tl.n_rows + r] : -1;
       o.rowhit[t * n_rows + r] = c >= 0 ? (int32_t)s2o[c] : -1;
     }
   if (o.x) o.x[t] = has ? tl.x[t] : 0.0f;

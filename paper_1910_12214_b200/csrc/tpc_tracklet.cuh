@@ -1,9 +1,9 @@
 // tpc_tracklet.cuh -- a4 tracklet constructor (O4, steps 1-6; R9..R18, R23).
 //
-// One thread per start hit.  The thread keeps the Kalman state, the snapshot of the down pass and its
-// bookkeeping in registers; rowhit[row][tracklet] lives in global memory (tracklet fastest, so threads of a
-// warp that advance row by row together write coalesced).  Only rows first_row..last_row of a tracklet are
-// ever read back, and every one of them is written here.
+// One lane per start hit at a time.  The lane keeps the Kalman state and its bookkeeping in registers, the
+// snapshot of the down pass in shared memory; rowhit[tracklet][row] lives in global memory (row fastest: a
+// lane walks its own 32-byte sectors row by row, so L2 merges its writes).  Only rows first_row..last_row of
+// a tracklet are ever read back, and every one of them is written here.
 #pragma once
 #include "tpc_kalman.cuh"
 #include "tpc_links.cuh"
@@ -34,115 +34,164 @@ __device__ __forceinline__ int32_t kfSearch(const KFState& S, const GridDesc& G,
   return best;
 }
 
+// Persistent warps; every lane owns one seed at a time and fetches the next one from a global counter as soon
+// as its seed is finished ("lane refill"), so a warp stays full although seeds need between 1 and ~300 steps.
+// The three passes of O4 (chain fit, up extrapolation, down pass) are folded into ONE step body
+//     Propagate -> candidate (link | known hit | Search) -> Update -> bookkeeping
+// driven by a per-lane phase, so that all lanes execute the expensive Kalman arithmetic together.  The order
+// of floating-point operations of a seed is exactly the sequential algorithm's.
 __global__ void __launch_bounds__(TC_THREADS) trackletConstructor(
     const uint32_t* __restrict__ off, DevParams P, RowTables T, const GridDesc* __restrict__ desc,
     const uint32_t* __restrict__ cell_start, const float2* __restrict__ syz, const uint32_t* __restrict__ s2o,
-    const int32_t* __restrict__ cup, const uint32_t* __restrict__ start_pos, TrackletStore out,
-    const int64_t* __restrict__ cnt) {
+    const int32_t* __restrict__ cup, const uint32_t* __restrict__ start_pos, TrackletStore out, int64_t* __restrict__ cnt) {
   __shared__ float sx[MAX_ROWS];
   __shared__ int16_t sup[MAX_ROWS];
   __shared__ uint8_t sdead[MAX_ROWS];
+  __shared__ float snap[22][TC_THREADS];     // state after the last Update of the down pass (O4 step 5)
   if (cnt[CNT_ERROR] != 0) return;
   const int R = P.n_rows;
-  for (int i = threadIdx.x; i < R; i += blockDim.x) { sx[i] = T.row_x[i]; sup[i] = T.up_row[i]; sdead[i] = T.dead[i]; }
+  const int tid = threadIdx.x;
+  for (int i = tid; i < R; i += blockDim.x) { sx[i] = T.row_x[i]; sup[i] = T.up_row[i]; sdead[i] = T.dead[i]; }
   __syncthreads();
   const int64_t nT = min(cnt[CNT_N_START], out.capT);
   const int64_t capT = out.capT;
-  for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < nT; t += (int64_t)gridDim.x * blockDim.x) {
-    const uint32_t h0 = start_pos[t];
-    const int b0 = bucketOf(off, P.n_buckets, h0);
-    const int r0 = b0 % R;
-    const int bsec = b0 - r0;                 // bucket of row 0 of this sector
-    int32_t* rowhit = out.rowhit + t;         // row stride capT
-    KFState S;
-    // 1. initialise from the first link
-    const int32_t h1 = cup[h0];
-    int r = sup[r0];
-    {
-      const float2 a = syz[h0], c = syz[h1];
-      S.x = sx[r0]; S.y = a.x; S.z = a.y;
-      const float dx = sx[r] - sx[r0], dy = c.x - a.x, dz = c.y - a.y;
-      const float L = sqrtf(dx * dx + dy * dy);
-      S.s = dy / L; S.t = dz / L; S.q = 0.0f;
-    }
-    kfSetDiag(S, P.err2_y, P.err2_z, P);
-    S.chi2 = 0.0f;
-    rowhit[(int64_t)r0 * capT] = (int32_t)h0;
-    int nhits = 1, rc = r0, lastw = r0;
-    // 2. fit along the link chain
-    for (int32_t h = h1; h != -1;) {
-      if (!kfPropagate(S, sx[r], P)) break;
-      rc = r;
-      const float2 c = syz[h];
-      if (!kfUpdate(S, c.x, c.y, P)) break;
-      for (int g = lastw + 1; g < r; ++g) rowhit[(int64_t)g * capT] = -1;
-      rowhit[(int64_t)r * capT] = h;
-      lastw = r; ++nhits;
-      h = cup[h];
-      r = sup[r];
-    }
-    out.sector[t] = bsec / R;
-    if (nhits < P.min_chain_hits) {
-      out.status[t] = 0; out.nhits[t] = nhits; out.first_row[t] = -1; out.last_row[t] = -1;
-      continue;
-    }
-    // 3. extrapolate upwards, picking up clusters through the grid
-    int miss = 0;
-    for (r = rc + 1; r < R; ++r) {
-      if (sdead[r]) continue;
-      if (!kfPropagate(S, sx[r], P)) break;
-      const int32_t c = kfSearch(S, desc[bsec + r], cell_start, syz, s2o, P);
-      if (c >= 0) {
-        const float2 m = syz[c];
-        if (!kfUpdate(S, m.x, m.y, P)) break;
-        for (int g = lastw + 1; g < r; ++g) rowhit[(int64_t)g * capT] = -1;
-        rowhit[(int64_t)r * capT] = c;
-        lastw = r; ++nhits; miss = 0;
-      } else if (++miss > P.max_row_gap) break;
-    }
-    // 4. turn: diffuse covariance, parameters kept as the linearisation point (R17)
-    kfSetDiag(S, P.turn_var_scale * P.err2_y, P.turn_var_scale * P.err2_z, P);
-    S.chi2 = 0.0f;
-    const int rtop = lastw;
-    // 5. down pass over all collected hits, filling gaps and extending below the start row
-    KFState snap = S;
-    int snap_row = -1, nh = 0;
-    miss = 0;
-    for (r = rtop; r >= 0; --r) {
-      if (sdead[r]) { if (r < r0) rowhit[(int64_t)r * capT] = -1; continue; }
-      if (!kfPropagate(S, sx[r], P)) break;
-      int32_t c = (r >= r0) ? rowhit[(int64_t)r * capT] : -1;
-      const bool known = c != -1;
-      if (!known) c = kfSearch(S, desc[bsec + r], cell_start, syz, s2o, P);
-      bool ok = false;
-      if (c >= 0) {
-        const float2 m = syz[c];
-        if (!kfUpdate(S, m.x, m.y, P)) break;
-        ok = true;
-      }
-      if (!known && (ok || r < r0)) rowhit[(int64_t)r * capT] = ok ? c : -1;
-      if (ok) {
-        ++nh; snap = S; snap_row = r;
-        if (r < r0) miss = 0;
-      } else if (r < r0) {
-        if (++miss > P.max_row_gap) break;
+  unsigned long long* work = (unsigned long long*)(cnt + CNT_WORK);
+
+  KFState S;
+  int phase = -1;                 // -1 wants a seed, -2 no seeds left, 0 chain fit, 1 up extrapolation, 2 down pass
+  int64_t t = 0;
+  int32_t* rowhit = nullptr;      // this tracklet's [n_rows] slice
+  int r0 = 0, bsec = 0, rn = 0, rc = 0, lastw = 0, nhits = 0, miss = 0, snap_row = -1, rtop = 0;
+  int32_t hlink = -1;
+
+  for (;;) {
+    if (phase == -1) {            // ---- fetch and initialise the next seed (O4 step 1) ----
+      t = (int64_t)atomicAdd(work, 1ull);
+      if (t >= nT) {
+        phase = -2;
+      } else {
+        const uint32_t h0 = start_pos[t];
+        const int b0 = bucketOf(off, P.n_buckets, h0);
+        r0 = b0 % R;
+        bsec = b0 - r0;
+        rowhit = out.rowhit + t * R;
+        hlink = cup[h0];
+        rn = sup[r0];
+        const float2 a = syz[h0], c = syz[hlink];
+        S.x = sx[r0]; S.y = a.x; S.z = a.y;
+        const float dx = sx[rn] - sx[r0], dy = c.x - a.x, dz = c.y - a.y;
+        const float L = sqrtf(dx * dx + dy * dy);
+        S.s = dy / L; S.t = dz / L; S.q = 0.0f;
+        kfSetDiag(S, P.err2_y, P.err2_z, P);
+        S.chi2 = 0.0f;
+        rowhit[r0] = (int32_t)h0;
+        nhits = 1; rc = r0; lastw = r0; miss = 0; snap_row = -1;
+        out.sector[t] = bsec / R;
+        phase = 0;
       }
     }
-    // 6. output = last snapshot (state at the innermost attached row)
-    if (snap_row < 0) {
-      out.status[t] = 1; out.nhits[t] = 0; out.first_row[t] = -1; out.last_row[t] = -1;
-      continue;
+    __syncwarp();
+    if (__all_sync(0xffffffffu, phase == -2)) break;
+
+    // ---- one step: Propagate -> candidate -> Update ----
+    const bool act = phase >= 0;
+    const bool okp = act && kfPropagate(S, sx[act ? rn : 0], P);
+    int32_t c = -1;
+    bool known = false;
+    if (okp) {
+      if (phase == 0) { c = hlink; rc = rn; }
+      else if (phase == 2 && rn >= r0) { c = rowhit[rn]; known = c != -1; }
     }
-    out.status[t] = nh >= P.min_tracklet_hits ? 2 : 1;
-    out.nhits[t] = nh; out.first_row[t] = snap_row; out.last_row[t] = rtop;
-    out.x[t] = snap.x; out.chi2[t] = snap.chi2;
-    out.par[0 * capT + t] = snap.y; out.par[1 * capT + t] = snap.z; out.par[2 * capT + t] = snap.s;
-    out.par[3 * capT + t] = snap.t; out.par[4 * capT + t] = snap.q;
-    float* cv = out.cov + t;
-    cv[0 * capT] = snap.c00; cv[1 * capT] = snap.c10; cv[2 * capT] = snap.c11; cv[3 * capT] = snap.c20;
-    cv[4 * capT] = snap.c21; cv[5 * capT] = snap.c22; cv[6 * capT] = snap.c30; cv[7 * capT] = snap.c31;
-    cv[8 * capT] = snap.c32; cv[9 * capT] = snap.c33; cv[10 * capT] = snap.c40; cv[11 * capT] = snap.c41;
-    cv[12 * capT] = snap.c42; cv[13 * capT] = snap.c43; cv[14 * capT] = snap.c44;
+    const bool need_search = okp && c < 0;
+    __syncwarp();
+    if (need_search) c = kfSearch(S, desc[bsec + rn], cell_start, syz, s2o, P);
+    __syncwarp();
+    bool oku = false;
+    if (okp && c >= 0) {
+      const float2 m = syz[c];
+      oku = kfUpdate(S, m.x, m.y, P);
+    }
+    __syncwarp();
+    if (!act) continue;
+
+    // ---- bookkeeping and phase transitions ----
+    bool end_phase = !okp || (c >= 0 && !oku);       // Propagate or Update refused: the pass ends here
+    bool turn = false;
+    if (phase == 0) {
+      if (oku) {
+        for (int g = lastw + 1; g < rn; ++g) rowhit[g] = -1;
+        rowhit[rn] = c;
+        lastw = rn; ++nhits;
+        hlink = cup[c];
+        rn = sup[rn];
+        if (hlink == -1) end_phase = true;
+      }
+      if (end_phase) {
+        if (nhits < P.min_chain_hits) {
+          out.status[t] = 0; out.nhits[t] = nhits; out.first_row[t] = -1; out.last_row[t] = -1;
+          phase = -1;
+        } else {
+          phase = 1; miss = 0;
+          rn = rc + 1;
+          while (rn < R && sdead[rn]) ++rn;
+          if (rn >= R) turn = true;
+        }
+      }
+    } else if (phase == 1) {
+      if (oku) {
+        for (int g = lastw + 1; g < rn; ++g) rowhit[g] = -1;
+        rowhit[rn] = c;
+        lastw = rn; ++nhits; miss = 0;
+      } else if (!end_phase) {
+        if (++miss > P.max_row_gap) end_phase = true;
+      }
+      if (!end_phase) {
+        ++rn;
+        while (rn < R && sdead[rn]) ++rn;
+        if (rn >= R) end_phase = true;
+      }
+      if (end_phase) turn = true;
+    } else {
+      if (!end_phase) {
+        if (!known && (oku || rn < r0)) rowhit[rn] = oku ? c : -1;
+        if (oku) {
+          ++nhits; snap_row = rn;
+          snap[0][tid] = S.x; snap[1][tid] = S.y; snap[2][tid] = S.z; snap[3][tid] = S.s; snap[4][tid] = S.t;
+          snap[5][tid] = S.q; snap[6][tid] = S.chi2; snap[7][tid] = S.c00; snap[8][tid] = S.c10; snap[9][tid] = S.c11;
+          snap[10][tid] = S.c20; snap[11][tid] = S.c21; snap[12][tid] = S.c22; snap[13][tid] = S.c30;
+          snap[14][tid] = S.c31; snap[15][tid] = S.c32; snap[16][tid] = S.c33; snap[17][tid] = S.c40;
+          snap[18][tid] = S.c41; snap[19][tid] = S.c42; snap[20][tid] = S.c43; snap[21][tid] = S.c44;
+          if (rn < r0) miss = 0;
+        } else if (rn < r0) {
+          if (++miss > P.max_row_gap) end_phase = true;
+        }
+      }
+      if (!end_phase) {
+        --rn;
+        while (rn >= 0 && sdead[rn]) { if (rn < r0) rowhit[rn] = -1; --rn; }
+        if (rn < 0) end_phase = true;
+      }
+      if (end_phase) {            // O4 step 6: output = last snapshot
+        if (snap_row < 0) {
+          out.status[t] = 1; out.nhits[t] = 0; out.first_row[t] = -1; out.last_row[t] = -1;
+        } else {
+          out.status[t] = nhits >= P.min_tracklet_hits ? 2 : 1;
+          out.nhits[t] = nhits; out.first_row[t] = snap_row; out.last_row[t] = rtop;
+          out.x[t] = snap[0][tid]; out.chi2[t] = snap[6][tid];
+#pragma unroll
+          for (int i = 0; i < 5; ++i) out.par[i * capT + t] = snap[1 + i][tid];
+#pragma unroll
+          for (int i = 0; i < 15; ++i) out.cov[i * capT + t] = snap[7 + i][tid];
+        }
+        phase = -1;
+      }
+    }
+    if (turn) {                   // O4 step 4: diffuse covariance, parameters kept (R17); down pass starts at rtop
+      kfSetDiag(S, P.turn_var_scale * P.err2_y, P.turn_var_scale * P.err2_z, P);
+      S.chi2 = 0.0f;
+      rtop = lastw; rn = rtop;
+      phase = 2; miss = 0; nhits = 0; snap_row = -1;
+    }
   }
 }
 
