@@ -31,8 +31,17 @@ def is_stale() -> bool:
     return any(os.path.getmtime(s) > t for s in _sources())
 
 
-def build_cuda(force: bool = False, verbose: bool = False) -> str:
-    """Compile csrc/tpc_api.cu (which includes every kernel header) into libtpcgpu.so."""
+def build_cuda(force: bool = False, verbose: bool = False, defines=(), out: str | None = None) -> str:
+    """Compile csrc/tpc_api.cu (which includes every kernel header) into libtpcgpu.so.
+
+    ``defines`` / ``out`` build a tuning variant (-DNAME=VALUE ...) under another file name; the product is
+    always the default build.
+    """
+    if out is not None:
+        nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+        subprocess.check_call([nvcc] + NVCC_FLAGS + [f"-D{d}" for d in defines] +
+                              [os.path.join(CSRC, "tpc_api.cu"), "-o", out])
+        return out
     if not force and not is_stale():
         return LIB
     nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"

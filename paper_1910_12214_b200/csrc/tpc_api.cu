@@ -29,6 +29,7 @@ inline int64_t ceilDiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
 
 struct Workspace {
   GridDesc* desc;
+  uint32_t* chunk_base;      // [nb+1] first neighbour-finder CTA of every bucket
   uint32_t* cell_start;
   uint32_t* rank;            // aliases spos_by_orig (a1 only)
   float2* syz;
@@ -98,6 +99,7 @@ Workspace layout(const tpcHandle* h, int64_t N, int64_t capT, char* base) {
   const int64_t cc = capCells(h, N);
   const int64_t Nn = N > 0 ? N : 1, Tn = capT > 0 ? capT : 1;
   w.desc = (GridDesc*)take(sizeof(GridDesc) * nb);
+  w.chunk_base = (uint32_t*)take(4 * (size_t)(nb + 1));
   w.cell_start = (uint32_t*)take(4 * (size_t)(cc + 1));
   w.spos_by_orig = (int32_t*)take(4 * (size_t)Nn);
   w.rank = (uint32_t*)w.spos_by_orig;
@@ -277,7 +279,7 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   stage(0);
   TPC_CUDA(h, cudaMemsetAsync(cnt, 0, 8 * (CNT_COUNT + 1), st)); ++L;
   // ---- a1 grid ----------------------------------------------------------------------------------
-  gridSetup<<<1, 1024, 0, st>>>(in->row_offset, N, P, h->d_row_x, w.desc, cnt, cc); ++L;
+  gridSetup<<<1, 1024, 0, st>>>(in->row_offset, N, P, h->d_row_x, w.desc, w.chunk_base, NF_THREADS, cnt, cc); ++L;
   if (N > 0) {
     TPC_CUDA(h, cudaMemsetAsync(w.cell_start, 0, 4 * (size_t)(cc + 1), st)); ++L;
     gridCount<<<gN256, 256, 0, st>>>(in->row_offset, in->y, in->z, N, nb, w.desc, w.cell_start, w.rank, cnt,
@@ -292,8 +294,9 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   stage(1);
   // ---- a2 neighbour finder ------------------------------------------------------------------------
   if (N > 0) {
-    neighbourFinder<<<(unsigned)ceilDiv(N, NF_THREADS), NF_THREADS, 0, st>>>(in->row_offset, N, P, T, w.desc, w.cell_start,
-                                                                             w.syz, w.s2o, w.lup, w.ldn, cnt); ++L;
+    // one CTA per chunk of NF_THREADS clusters of one bucket; the exact CTA count is on the device (chunk_base[nb])
+    neighbourFinder<<<(unsigned)(ceilDiv(N, NF_THREADS) + nb), NF_THREADS, 0, st>>>(w.chunk_base, P, T, w.desc, w.cell_start,
+                                                                                    w.syz, w.s2o, w.lup, w.ldn, cnt); ++L;
   }
   stage(2);
   // ---- a3 cleaner + start hits --------------------------------------------------------------------

@@ -12,7 +12,8 @@ namespace tpc {
 // One block.  Validates row_offset, sizes every bucket's grid and lays the cell tables out back to back.
 __global__ void __launch_bounds__(1024) gridSetup(const uint32_t* __restrict__ off, int64_t N, DevParams P,
                                                   const float* __restrict__ row_x, GridDesc* __restrict__ desc,
-                                                  int64_t* __restrict__ cnt, int64_t cap_cells) {
+                                                  uint32_t* __restrict__ chunk_base, int chunk, int64_t* __restrict__ cnt,
+                                                  int64_t cap_cells) {
   __shared__ uint32_t sm[33];
   __shared__ int bad;
   const int nb = P.n_buckets;
@@ -22,16 +23,16 @@ __global__ void __launch_bounds__(1024) gridSetup(const uint32_t* __restrict__ o
     if (off[b + 1] < off[b]) bad = 1;
   __syncthreads();
   if (bad) {
-    for (int b = threadIdx.x; b < nb; b += blockDim.x) desc[b] = GridDesc{0.f, 0.f, 1.f, 1, 1, 0u, 0u, 0u};
-    if (threadIdx.x == 0) { cnt[CNT_ERROR] = -2; cnt[CNT_N_CELLS] = 0; }
+    for (int b = threadIdx.x; b < nb; b += blockDim.x) { desc[b] = GridDesc{0.f, 0.f, 1.f, 1, 1, 0u, 0u, 0u}; chunk_base[b] = 0; }
+    if (threadIdx.x == 0) { cnt[CNT_ERROR] = -2; cnt[CNT_N_CELLS] = 0; chunk_base[nb] = 0; }
     return;
   }
-  uint32_t carry = 0;
+  uint32_t carry = 0, ccarry = 0;      // running cell / chunk totals
   const float Wz = P.z_max - P.z_min;
   for (int base = 0; base < nb; base += blockDim.x) {
     const int b = base + threadIdx.x;
     GridDesc g{0.f, 0.f, 1.f, 1, 1, 0u, 0u, 0u};
-    uint32_t nc = 0;
+    uint32_t nc = 0, nch = 0;
     if (b < nb) {
       const int r = b % P.n_rows;
       const uint32_t lo = off[b], n = off[b + 1] - lo;
@@ -48,13 +49,18 @@ __global__ void __launch_bounds__(1024) gridSetup(const uint32_t* __restrict__ o
       }
       g.y0 = -hw; g.z0 = P.z_min; g.inv_e = 1.0f / e; g.ny = ny; g.nz = nz; g.lo = lo; g.n = n;
       nc = (uint32_t)(ny * nz);
+      nch = (n + chunk - 1) / chunk;      // CTAs of the neighbour finder: `chunk` clusters of one bucket each
     }
     uint32_t total;
     const uint32_t ex = blockExclusiveScan(nc, sm, &total);
     if (b < nb) { g.cell_base = carry + ex; desc[b] = g; }
     carry += total;
+    const uint32_t cex = blockExclusiveScan(nch, sm, &total);
+    if (b < nb) chunk_base[b] = ccarry + cex;
+    ccarry += total;
   }
   if (threadIdx.x == 0) {
+    chunk_base[nb] = ccarry;
     cnt[CNT_N_CELLS] = carry;
     if ((int64_t)carry > cap_cells) cnt[CNT_ERROR] = -3;
   }

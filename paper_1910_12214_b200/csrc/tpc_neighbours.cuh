@@ -1,0 +1,242 @@
+// tpc_neighbours.cuh -- a2 neighbour finder (O2; R2, R4..R7).
+//
+// For every cluster h on row r:  U = clusters of row up(r) with |y_u-y_h| <= area_y*dxu and |z_u-z_h| <= area_z*dxu,
+// D likewise on row dn(r);  tyu=(y_u-y_h)*iu, tzu=(z_u-z_h)*iu, tyd=(y_h-y_d)*id, tzd=(z_h-z_d)*id;
+// Dev(u,d) = (tyu-tyd)^2 + (tzu-tzd)^2;  best = argmin of (Dev, orig(u), orig(d));  link both iff Dev <= link_dev2_max.
+//
+// Organisation (one CTA = up to 128 consecutive sorted clusters of ONE (sector,row) bucket):
+//   1. the clusters of a CTA are neighbours in z (the grid order is z-major), so all their up / down candidates
+//      lie in two CONTIGUOUS ranges of the sorted array: both are staged in shared memory with coalesced loads;
+//   2. each thread walks the grid cells of its own windows and keeps the 16-bit region indices of the clusters
+//      that pass the exact predicate (its U and D lists);
+//   3. the nU x nD pair loop is NOT run per cluster (nU*nD varies from 1 to >500 inside a warp): the (h,u)
+//      combinations of the whole CTA become a flat item list and every lane takes items, looping over the D
+//      list of the item's h -- lanes of a warp mostly share h, so the loop lengths agree and reads broadcast;
+//   4. each thread reduces the results of its own items with the full lexicographic key.
+// Anything that does not fit the fixed shared-memory budget (huge regions, > NF_LIST candidates in a window,
+// > NF_ITEMS items) takes a per-thread slow path with the same predicate, arithmetic and key.
+#pragma once
+#include "tpc_common.cuh"
+
+namespace tpc {
+
+constexpr int NF_THREADS = 128;
+constexpr int NF_REGION = 768;     // staged candidates per side
+constexpr int NF_LIST = 24;        // window candidates kept per thread and side (<= 32: packed item code)
+constexpr int NF_ITEMS = 2048;     // (h,u) items per CTA
+
+struct RowTables {
+  const float* row_x;     // [R]
+  const int16_t* up_row;  // [R] first live row among r+1, r+2 or -1 (R2); -1 for dead rows
+  const int16_t* dn_row;  // [R]
+  const uint8_t* dead;    // [R]
+};
+
+// lexicographic (Dev, orig(u), orig(d)) "is the new pair better" (R6)
+__device__ __forceinline__ bool pairBetter(bool have, float dev, float best, uint32_t u, uint32_t d, uint32_t bu,
+                                           uint32_t bd, const uint32_t* __restrict__ s2o) {
+  if (!have || dev < best) return true;
+  if (dev != best) return false;
+  if (u != bu) return __ldg(s2o + u) < __ldg(s2o + bu);
+  return __ldg(s2o + d) < __ldg(s2o + bd);
+}
+
+// per-thread reference path: nested enumeration of both windows straight from global memory
+__device__ __noinline__ void neighbourSlow(uint32_t p, float2 h, const GridDesc& Gu, const GridDesc& Gd,
+                                           const uint32_t* __restrict__ cell_start, const float2* __restrict__ syz,
+                                           const uint32_t* __restrict__ s2o, float iu, float id, float wyu, float wzu,
+                                           float wyd, float wzd, float dev_max, int32_t* __restrict__ lup,
+                                           int32_t* __restrict__ ldn) {
+  bool have = false;
+  float best = 0.0f;
+  uint32_t bu = 0, bd = 0;
+  forWindow(Gu, cell_start, syz, h.x, h.y, wyu, wzu, [&](uint32_t u, float yu, float zu) {
+    const float tyu = (yu - h.x) * iu, tzu = (zu - h.y) * iu;
+    forWindow(Gd, cell_start, syz, h.x, h.y, wyd, wzd, [&](uint32_t d, float yd, float zd) {
+      const float tyd = (h.x - yd) * id, tzd = (h.y - zd) * id;
+      const float ey = tyu - tyd, ez = tzu - tzd;
+      const float dev = ey * ey + ez * ez;
+      if (pairBetter(have, dev, best, u, d, bu, bd, s2o)) { have = true; best = dev; bu = u; bd = d; }
+    });
+  });
+  const bool link = have && best <= dev_max;
+  lup[p] = link ? (int32_t)bu : -1;
+  ldn[p] = link ? (int32_t)bd : -1;
+}
+
+// window walk over a region staged in shared memory: the cell ranges come from the global cell table, the
+// coordinates from `reg` (region index = sorted position - k0).  Appends the indices passing the predicate.
+__device__ __forceinline__ int gatherWindow(const GridDesc& G, const uint32_t* __restrict__ cell_start, const float2* reg,
+                                            uint32_t k0, float yc, float zc, float wy, float wz, uint16_t* list, int tid) {
+  if (G.n == 0) return 0;
+  const float sy = 1e-5f * (fabsf(yc) + wy) + 1e-6f;
+  const float sz = 1e-5f * (fabsf(zc) + wz) + 1e-6f;
+  const int by0 = cellCoord((yc - wy) - sy, G.y0, G.inv_e, G.ny);
+  const int by1 = cellCoord((yc + wy) + sy, G.y0, G.inv_e, G.ny);
+  int bz = cellCoord((zc - wz) - sz, G.z0, G.inv_e, G.nz);
+  const int bz1 = cellCoord((zc + wz) + sz, G.z0, G.inv_e, G.nz);
+  const uint32_t* cs = cell_start + G.cell_base + by0;
+  const int span = by1 - by0 + 1;
+  uint32_t k = __ldg(cs + bz * G.ny), kend = __ldg(cs + bz * G.ny + span);
+  int n = 0;
+  for (;;) {
+    if (k < kend) {
+      const float2 c = reg[k - k0];
+      if (fabsf(c.x - yc) <= wy && fabsf(c.y - zc) <= wz) {
+        if (n < NF_LIST) list[n * NF_THREADS + tid] = (uint16_t)(k - k0);
+        ++n;
+      }
+      ++k;
+    } else {
+      if (++bz > bz1) break;
+      k = __ldg(cs + bz * G.ny);
+      kend = __ldg(cs + bz * G.ny + span);
+    }
+  }
+  return n;
+}
+
+__global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __restrict__ chunk_base, DevParams P, RowTables T,
+                                                              const GridDesc* __restrict__ desc,
+                                                              const uint32_t* __restrict__ cell_start,
+                                                              const float2* __restrict__ syz,
+                                                              const uint32_t* __restrict__ s2o, int32_t* __restrict__ lup,
+                                                              int32_t* __restrict__ ldn, const int64_t* __restrict__ cnt) {
+  __shared__ float2 sD[NF_REGION], sU[NF_REGION], sH[NF_THREADS];
+  __shared__ uint16_t dl[NF_LIST * NF_THREADS], ul[NF_LIST * NF_THREADS];
+  __shared__ uint16_t it[NF_ITEMS], it_d[NF_ITEMS];
+  __shared__ float it_dev[NF_ITEMS];
+  __shared__ uint8_t snD[NF_THREADS];
+  __shared__ float red[2][NF_THREADS / 32];
+  __shared__ uint32_t sscan[33];
+  __shared__ int sm_b;
+  __shared__ uint32_t sm_T;
+  if (cnt[CNT_ERROR] != 0) return;
+  const int tid = threadIdx.x;
+  const int nb = P.n_buckets;
+  if (blockIdx.x >= __ldg(chunk_base + nb)) return;
+  if (tid == 0) {   // bucket of this chunk: largest b with chunk_base[b] <= blockIdx.x
+    int lo = 0, hi = nb;
+    while (hi - lo > 1) {
+      const int mid = (lo + hi) >> 1;
+      if (__ldg(chunk_base + mid) <= blockIdx.x) lo = mid; else hi = mid;
+    }
+    sm_b = lo;
+    sm_T = 0;
+  }
+  __syncthreads();
+  const int b = sm_b;
+  const GridDesc Gh = desc[b];
+  const uint32_t p = Gh.lo + (blockIdx.x - __ldg(chunk_base + b)) * NF_THREADS + tid;
+  const bool valid = p < Gh.lo + Gh.n;
+  const int r = b % P.n_rows;
+  const int ru = T.up_row[r], rd = T.dn_row[r];
+  if (ru < 0 || rd < 0) {   // no row pair (first / last rows, dead rows): no links (uniform branch)
+    if (valid) { lup[p] = -1; ldn[p] = -1; }
+    return;
+  }
+  const float xr = T.row_x[r];
+  const float dxu = T.row_x[ru] - xr, dxd = xr - T.row_x[rd];
+  const float iu = 1.0f / dxu, id = 1.0f / dxd;
+  const float wyu = P.area_y * dxu, wzu = P.area_z * dxu;
+  const float wyd = P.area_y * dxd, wzd = P.area_z * dxd;
+  const GridDesc Gu = desc[b - r + ru], Gd = desc[b - r + rd];
+  const float2 h = valid ? syz[p] : make_float2(0.0f, 0.0f);
+
+  // ---- z extent of the chunk -> contiguous candidate regions ----
+  float zlo = valid ? h.y : 3.0e38f, zhi = valid ? h.y : -3.0e38f;
+  for (int d = 16; d > 0; d >>= 1) {
+    zlo = fminf(zlo, __shfl_xor_sync(0xffffffffu, zlo, d));
+    zhi = fmaxf(zhi, __shfl_xor_sync(0xffffffffu, zhi, d));
+  }
+  if ((tid & 31) == 0) { red[0][tid >> 5] = zlo; red[1][tid >> 5] = zhi; }
+  __syncthreads();
+  zlo = fminf(fminf(red[0][0], red[0][1]), fminf(red[0][2], red[0][3]));
+  zhi = fmaxf(fmaxf(red[1][0], red[1][1]), fmaxf(red[1][2], red[1][3]));
+  uint32_t kD0 = 0, kD1 = 0, kU0 = 0, kU1 = 0;
+  {
+    const float s = 1e-5f * (fmaxf(fabsf(zlo), fabsf(zhi)) + wzu + wzd) + 1e-6f;
+    if (Gd.n) {
+      const int a = cellCoord((zlo - wzd) - s, Gd.z0, Gd.inv_e, Gd.nz), e = cellCoord((zhi + wzd) + s, Gd.z0, Gd.inv_e, Gd.nz);
+      kD0 = __ldg(cell_start + Gd.cell_base + a * Gd.ny);
+      kD1 = __ldg(cell_start + Gd.cell_base + (e + 1) * Gd.ny);
+    }
+    if (Gu.n) {
+      const int a = cellCoord((zlo - wzu) - s, Gu.z0, Gu.inv_e, Gu.nz), e = cellCoord((zhi + wzu) + s, Gu.z0, Gu.inv_e, Gu.nz);
+      kU0 = __ldg(cell_start + Gu.cell_base + a * Gu.ny);
+      kU1 = __ldg(cell_start + Gu.cell_base + (e + 1) * Gu.ny);
+    }
+  }
+  if (kD1 - kD0 > NF_REGION || kU1 - kU0 > NF_REGION) {     // regions too large for shared memory (uniform branch)
+    if (valid) neighbourSlow(p, h, Gu, Gd, cell_start, syz, s2o, iu, id, wyu, wzu, wyd, wzd, P.link_dev2_max, lup, ldn);
+    return;
+  }
+  for (uint32_t i = tid; i < kD1 - kD0; i += NF_THREADS) sD[i] = __ldg(syz + kD0 + i);
+  for (uint32_t i = tid; i < kU1 - kU0; i += NF_THREADS) sU[i] = __ldg(syz + kU0 + i);
+  sH[tid] = h;
+  __syncthreads();
+
+  // ---- per-thread window lists ----
+  int nD = 0, nU = 0;
+  if (valid) {
+    nD = gatherWindow(Gd, cell_start, sD, kD0, h.x, h.y, wyd, wzd, dl, tid);
+    if (nD > 0) nU = gatherWindow(Gu, cell_start, sU, kU0, h.x, h.y, wyu, wzu, ul, tid);
+  }
+  bool slow = nD > NF_LIST || nU > NF_LIST;
+  uint32_t cntU = (nD > 0 && !slow) ? (uint32_t)nU : 0u;
+  uint32_t total;
+  const uint32_t base = blockExclusiveScan(cntU, sscan, &total);
+  if (cntU > 0 && base + cntU > NF_ITEMS) { slow = true; cntU = 0; }     // item list full: this and all later threads
+  if (cntU > 0) {
+    atomicMax(&sm_T, base + cntU);
+    for (uint32_t a = 0; a < cntU; ++a) it[base + a] = (uint16_t)(tid * 32 + a);
+  }
+  snD[tid] = (uint8_t)min(nD, NF_LIST);
+  __syncthreads();
+
+  // ---- pair phase: one item = (h, u); loop over the D list of h ----
+  const uint32_t Tn = sm_T;
+  for (uint32_t i = tid; i < Tn; i += NF_THREADS) {
+    const uint32_t e = it[i];
+    const int hl = e >> 5, a = e & 31;
+    const float2 hh = sH[hl];
+    const float2 uu = sU[ul[a * NF_THREADS + hl]];
+    const float tyu = (uu.x - hh.x) * iu, tzu = (uu.y - hh.y) * iu;
+    const int n = snD[hl];
+    float best = 0.0f;
+    uint32_t bd = 0;
+    for (int j = 0; j < n; ++j) {
+      const uint32_t di = dl[j * NF_THREADS + hl];
+      const float2 dd = sD[di];
+      const float tyd = (hh.x - dd.x) * id, tzd = (hh.y - dd.y) * id;
+      const float ey = tyu - tyd, ez = tzu - tzd;
+      const float dev = ey * ey + ez * ez;
+      if (j == 0 || dev < best || (dev == best && __ldg(s2o + kD0 + di) < __ldg(s2o + kD0 + bd))) { best = dev; bd = di; }
+    }
+    it_dev[i] = best;
+    it_d[i] = (uint16_t)bd;
+  }
+  __syncthreads();
+
+  // ---- per-cluster reduction over its own items, full key (Dev, orig u, orig d) ----
+  if (!valid) return;
+  if (slow) {
+    neighbourSlow(p, h, Gu, Gd, cell_start, syz, s2o, iu, id, wyu, wzu, wyd, wzd, P.link_dev2_max, lup, ldn);
+    return;
+  }
+  bool have = false;
+  float best = 0.0f;
+  uint32_t bu = 0, bd = 0;
+  for (uint32_t a = 0; a < cntU; ++a) {
+    const float dev = it_dev[base + a];
+    if (!have || dev <= best) {
+      const uint32_t u = kU0 + ul[a * NF_THREADS + tid], d = kD0 + it_d[base + a];
+      if (pairBetter(have, dev, best, u, d, bu, bd, s2o)) { have = true; best = dev; bu = u; bd = d; }
+    }
+  }
+  const bool link = have && best <= P.link_dev2_max;
+  lup[p] = link ? (int32_t)bu : -1;
+  ldn[p] = link ? (int32_t)bd : -1;
+}
+
+}  // namespace tpc

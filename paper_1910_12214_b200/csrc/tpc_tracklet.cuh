@@ -11,26 +11,74 @@
 namespace tpc {
 
 constexpr int TC_THREADS = 128;
+#ifndef TC_MIN_BLOCKS
+#define TC_MIN_BLOCKS 5
+#endif
 constexpr int MAX_ROWS = 256;
 
 // Search (O4): nearest cluster of the bucket inside the road around the predicted (y,z); key (d2, orig index).
-__device__ __forceinline__ int32_t kfSearch(const KFState& S, const GridDesc& G, const uint32_t* __restrict__ cell_start,
-                                            const float2* __restrict__ syz, const uint32_t* __restrict__ s2o,
-                                            const DevParams& P) {
-  float ry = P.road_sigma * sqrtf(S.c00 + P.err2_y);
-  float rz = P.road_sigma * sqrtf(S.c11 + P.err2_z);
+// Split in two so that the first grid loads are in flight while Propagate finishes the covariance transport:
+// searchBegin (called from Propagate's hook) computes the road and the cell window and loads the cell ranges
+// of the first two cell rows; searchFinish scans the candidates.
+struct SearchPre {
+  float yp, zp, ry, rz;
+  int bz0, bz1, ny, span;
+  const uint32_t* cs;        // cell_start + cell_base + by0
+  uint32_t kA0, kA1, kB0, kB1;
+};
+
+__device__ __forceinline__ void searchBegin(SearchPre& sp, float yp, float zp, float c00, float c11, const GridDesc& G,
+                                            const uint32_t* __restrict__ cell_start, const DevParams& P) {
+  float ry = P.road_sigma * sqrtf(c00 + P.err2_y);
+  float rz = P.road_sigma * sqrtf(c11 + P.err2_z);
   if (!(ry >= P.road_min)) ry = P.road_min;
   if (ry > P.road_max) ry = P.road_max;
   if (!(rz >= P.road_min)) rz = P.road_min;
   if (rz > P.road_max) rz = P.road_max;
+  const float sy = 1e-5f * (fabsf(yp) + ry) + 1e-6f;      // superset slack, see forWindow
+  const float sz = 1e-5f * (fabsf(zp) + rz) + 1e-6f;
+  const int by0 = cellCoord((yp - ry) - sy, G.y0, G.inv_e, G.ny);
+  const int by1 = cellCoord((yp + ry) + sy, G.y0, G.inv_e, G.ny);
+  sp.bz0 = cellCoord((zp - rz) - sz, G.z0, G.inv_e, G.nz);
+  sp.bz1 = cellCoord((zp + rz) + sz, G.z0, G.inv_e, G.nz);
+  sp.yp = yp; sp.zp = zp; sp.ry = ry; sp.rz = rz;
+  sp.ny = G.ny; sp.span = by1 - by0 + 1;
+  sp.cs = cell_start + G.cell_base + by0;
+  const uint32_t* rA = sp.cs + sp.bz0 * G.ny;
+  const uint32_t* rB = sp.cs + min(sp.bz0 + 1, sp.bz1) * G.ny;
+  sp.kA0 = __ldg(rA); sp.kA1 = __ldg(rA + sp.span);
+  sp.kB0 = __ldg(rB); sp.kB1 = __ldg(rB + sp.span);
+}
+
+// returns the sorted position of the best cluster or -1; its coordinates in (ym, zm)
+__device__ __forceinline__ int32_t searchFinish(const SearchPre& sp, const float2* __restrict__ syz,
+                                                const uint32_t* __restrict__ s2o, float& ym, float& zm) {
   int32_t best = -1;
   float bestd = 0.0f;
-  const float yp = S.y, zp = S.z;
-  forWindow(G, cell_start, syz, yp, zp, ry, rz, [&](uint32_t c, float yc, float zc) {
-    const float dy = yc - yp, dz = zc - zp;
-    const float d2 = dy * dy + dz * dz;
-    if (best < 0 || d2 < bestd || (d2 == bestd && __ldg(s2o + c) < __ldg(s2o + best))) { best = (int32_t)c; bestd = d2; }
-  });
+  auto test = [&](uint32_t k, const float2 c) {
+    if (fabsf(c.x - sp.yp) <= sp.ry && fabsf(c.y - sp.zp) <= sp.rz) {
+      const float dy = c.x - sp.yp, dz = c.y - sp.zp;
+      const float d2 = dy * dy + dz * dz;
+      if (best < 0 || d2 < bestd || (d2 == bestd && __ldg(s2o + k) < __ldg(s2o + best))) {
+        best = (int32_t)k; bestd = d2; ym = c.x; zm = c.y;
+      }
+    }
+  };
+  auto scan = [&](uint32_t k0, uint32_t k1) {      // two independent loads per trip
+    for (uint32_t k = k0; k < k1; k += 2) {
+      const bool two = k + 1 < k1;
+      const float2 a = __ldg(syz + k);
+      const float2 c = __ldg(syz + (two ? k + 1 : k));
+      test(k, a);
+      if (two) test(k + 1, c);
+    }
+  };
+  scan(sp.kA0, sp.kA1);
+  if (sp.bz1 > sp.bz0) scan(sp.kB0, sp.kB1);
+  for (int bz = sp.bz0 + 2; bz <= sp.bz1; ++bz) {   // roads wider than two cell rows: rare
+    const uint32_t* r = sp.cs + bz * sp.ny;
+    scan(__ldg(r), __ldg(r + sp.span));
+  }
   return best;
 }
 
@@ -38,9 +86,12 @@ __device__ __forceinline__ int32_t kfSearch(const KFState& S, const GridDesc& G,
 // as its seed is finished ("lane refill"), so a warp stays full although seeds need between 1 and ~300 steps.
 // The three passes of O4 (chain fit, up extrapolation, down pass) are folded into ONE step body
 //     Propagate -> candidate (link | known hit | Search) -> Update -> bookkeeping
-// driven by a per-lane phase, so that all lanes execute the expensive Kalman arithmetic together.  The order
-// of floating-point operations of a seed is exactly the sequential algorithm's.
-__global__ void __launch_bounds__(TC_THREADS) trackletConstructor(
+// driven by a per-lane phase, so that all lanes execute the expensive Kalman arithmetic together.  Loads are
+// software-pipelined around the arithmetic: the hit of a step (link or known row hit) is fetched one step
+// ahead, its coordinates and the row's grid descriptor are requested before Propagate, the cell ranges of a
+// search from inside Propagate.  The order of floating-point operations of a seed is exactly the sequential
+// algorithm's.
+__global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor(
     const uint32_t* __restrict__ off, DevParams P, RowTables T, const GridDesc* __restrict__ desc,
     const uint32_t* __restrict__ cell_start, const float2* __restrict__ syz, const uint32_t* __restrict__ s2o,
     const int32_t* __restrict__ cup, const uint32_t* __restrict__ start_pos, TrackletStore out, int64_t* __restrict__ cnt) {
@@ -62,7 +113,9 @@ __global__ void __launch_bounds__(TC_THREADS) trackletConstructor(
   int64_t t = 0;
   int32_t* rowhit = nullptr;      // this tracklet's [n_rows] slice
   int r0 = 0, bsec = 0, rn = 0, rc = 0, lastw = 0, nhits = 0, miss = 0, snap_row = -1, rtop = 0;
-  int32_t hlink = -1;
+  int32_t c_cur = -1;             // hit of the coming step if known (link / row hit), else -1 = search
+  int32_t c_nxt = -1;             // down pass: row hit of the step after (loaded one step ahead)
+  int32_t last_c = -1;            // last recorded hit (the hit on row lastw)
 
   for (;;) {
     if (phase == -1) {            // ---- fetch and initialise the next seed (O4 step 1) ----
@@ -75,9 +128,9 @@ __global__ void __launch_bounds__(TC_THREADS) trackletConstructor(
         r0 = b0 % R;
         bsec = b0 - r0;
         rowhit = out.rowhit + t * R;
-        hlink = cup[h0];
+        c_cur = cup[h0];
         rn = sup[r0];
-        const float2 a = syz[h0], c = syz[hlink];
+        const float2 a = syz[h0], c = syz[c_cur];
         S.x = sx[r0]; S.y = a.x; S.z = a.y;
         const float dx = sx[rn] - sx[r0], dy = c.x - a.x, dz = c.y - a.y;
         const float L = sqrtf(dx * dx + dy * dy);
@@ -85,6 +138,7 @@ __global__ void __launch_bounds__(TC_THREADS) trackletConstructor(
         kfSetDiag(S, P.err2_y, P.err2_z, P);
         S.chi2 = 0.0f;
         rowhit[r0] = (int32_t)h0;
+        last_c = (int32_t)h0;
         nhits = 1; rc = r0; lastw = r0; miss = 0; snap_row = -1;
         out.sector[t] = bsec / R;
         phase = 0;
@@ -93,24 +147,33 @@ __global__ void __launch_bounds__(TC_THREADS) trackletConstructor(
     __syncwarp();
     if (__all_sync(0xffffffffu, phase == -2)) break;
 
-    // ---- one step: Propagate -> candidate -> Update ----
+    // ---- one step: early loads -> Propagate (search loads issued inside) -> candidate -> Update ----
     const bool act = phase >= 0;
-    const bool okp = act && kfPropagate(S, sx[act ? rn : 0], P);
-    int32_t c = -1;
-    bool known = false;
-    if (okp) {
-      if (phase == 0) { c = hlink; rc = rn; }
-      else if (phase == 2 && rn >= r0) { c = rowhit[rn]; known = c != -1; }
+    float ym = 0.0f, zm = 0.0f;
+    int32_t hnext = -1;
+    GridDesc G;
+    if (act) {
+      if (c_cur >= 0) {
+        const float2 m = __ldg(syz + c_cur);
+        ym = m.x; zm = m.y;
+        if (phase == 0) hnext = __ldg(cup + c_cur);
+      } else {
+        G = desc[bsec + rn];
+      }
     }
-    const bool need_search = okp && c < 0;
+    SearchPre sp;
+    const bool want_search = act && c_cur < 0;
+    const bool okp = act && kfPropagate(S, sx[act ? rn : 0], P, [&](float y1, float z1, float c00, float c11) {
+      if (want_search) searchBegin(sp, y1, z1, c00, c11, G, cell_start, P);
+    });
+    int32_t c = c_cur;
+    const bool known = okp && c >= 0 && phase == 2;
+    if (okp && phase == 0) rc = rn;
     __syncwarp();
-    if (need_search) c = kfSearch(S, desc[bsec + rn], cell_start, syz, s2o, P);
+    if (okp && c < 0) c = searchFinish(sp, syz, s2o, ym, zm);
     __syncwarp();
     bool oku = false;
-    if (okp && c >= 0) {
-      const float2 m = syz[c];
-      oku = kfUpdate(S, m.x, m.y, P);
-    }
+    if (okp && c >= 0) oku = kfUpdate(S, ym, zm, P);
     __syncwarp();
     if (!act) continue;
 
@@ -121,17 +184,17 @@ __global__ void __launch_bounds__(TC_THREADS) trackletConstructor(
       if (oku) {
         for (int g = lastw + 1; g < rn; ++g) rowhit[g] = -1;
         rowhit[rn] = c;
-        lastw = rn; ++nhits;
-        hlink = cup[c];
+        lastw = rn; last_c = c; ++nhits;
+        c_cur = hnext;
         rn = sup[rn];
-        if (hlink == -1) end_phase = true;
+        if (hnext == -1) end_phase = true;
       }
       if (end_phase) {
         if (nhits < P.min_chain_hits) {
           out.status[t] = 0; out.nhits[t] = nhits; out.first_row[t] = -1; out.last_row[t] = -1;
           phase = -1;
         } else {
-          phase = 1; miss = 0;
+          phase = 1; miss = 0; c_cur = -1;
           rn = rc + 1;
           while (rn < R && sdead[rn]) ++rn;
           if (rn >= R) turn = true;
@@ -141,7 +204,7 @@ __global__ void __launch_bounds__(TC_THREADS) trackletConstructor(
       if (oku) {
         for (int g = lastw + 1; g < rn; ++g) rowhit[g] = -1;
         rowhit[rn] = c;
-        lastw = rn; ++nhits; miss = 0;
+        lastw = rn; last_c = c; ++nhits; miss = 0;
       } else if (!end_phase) {
         if (++miss > P.max_row_gap) end_phase = true;
       }
@@ -171,7 +234,12 @@ __global__ void __launch_bounds__(TC_THREADS) trackletConstructor(
         while (rn >= 0 && sdead[rn]) { if (rn < r0) rowhit[rn] = -1; --rn; }
         if (rn < 0) end_phase = true;
       }
-      if (end_phase) {            // O4 step 6: output = last snapshot
+      if (!end_phase) {           // pipeline: this step's hit was loaded a step ago; request the one after
+        c_cur = c_nxt;
+        int r2 = rn - 1;
+        while (r2 >= 0 && sdead[r2]) --r2;
+        c_nxt = (r2 >= r0) ? rowhit[r2] : -1;
+      } else {                    // O4 step 6: output = last snapshot
         if (snap_row < 0) {
           out.status[t] = 1; out.nhits[t] = 0; out.first_row[t] = -1; out.last_row[t] = -1;
         } else {
@@ -191,6 +259,10 @@ __global__ void __launch_bounds__(TC_THREADS) trackletConstructor(
       S.chi2 = 0.0f;
       rtop = lastw; rn = rtop;
       phase = 2; miss = 0; nhits = 0; snap_row = -1;
+      c_cur = last_c;             // the hit on row rtop
+      int r2 = rn - 1;
+      while (r2 >= 0 && sdead[r2]) --r2;
+      c_nxt = (r2 >= r0) ? rowhit[r2] : -1;
     }
   }
 }

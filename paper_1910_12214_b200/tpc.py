@@ -71,10 +71,14 @@ def load_library(build_if_stale: bool = True) -> ctypes.CDLL:
     global _lib
     if _lib is not None:
         return _lib
-    if build_if_stale:
-        _build.build_cuda()
+    import os
+    path = os.environ.get("TPCGPU_LIB")          # tuning variants (build.build_cuda(out=...)); default: the product
+    if not path:
+        path = _build.LIB
+        if build_if_stale:
+            _build.build_cuda()
     try:
-        L = ctypes.CDLL(_build.LIB)
+        L = ctypes.CDLL(path)
     except OSError as e:   # no fallback: the product path needs the CUDA library
         raise RuntimeError(f"libtpcgpu.so could not be loaded ({e}); the TPC tracker has no CPU fallback") from e
     vp = c_void_p
