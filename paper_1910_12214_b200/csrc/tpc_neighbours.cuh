@@ -21,9 +21,9 @@
 namespace tpc {
 
 constexpr int NF_THREADS = 128;
-constexpr int NF_REGION = 768;     // staged candidates per side
-constexpr int NF_LIST = 24;        // window candidates kept per thread and side (<= 32: packed item code)
-constexpr int NF_ITEMS = 2048;     // (h,u) items per CTA
+constexpr int NF_REGION = 640;     // staged candidates per side
+constexpr int NF_LIST = 32;        // window candidates kept per thread and side (<= 32: packed item code)
+constexpr int NF_ITEMS = 1536;     // (h,u) items per CTA
 
 struct RowTables {
   const float* row_x;     // [R]
@@ -122,7 +122,6 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
       if (__ldg(chunk_base + mid) <= blockIdx.x) lo = mid; else hi = mid;
     }
     sm_b = lo;
-    sm_T = 0;
   }
   __syncthreads();
   const int b = sm_b;
@@ -182,57 +181,65 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
     nD = gatherWindow(Gd, cell_start, sD, kD0, h.x, h.y, wyd, wzd, dl, tid);
     if (nD > 0) nU = gatherWindow(Gu, cell_start, sU, kU0, h.x, h.y, wyu, wzu, ul, tid);
   }
-  bool slow = nD > NF_LIST || nU > NF_LIST;
-  uint32_t cntU = (nD > 0 && !slow) ? (uint32_t)nU : 0u;
-  uint32_t total;
-  const uint32_t base = blockExclusiveScan(cntU, sscan, &total);
-  if (cntU > 0 && base + cntU > NF_ITEMS) { slow = true; cntU = 0; }     // item list full: this and all later threads
-  if (cntU > 0) {
-    atomicMax(&sm_T, base + cntU);
-    for (uint32_t a = 0; a < cntU; ++a) it[base + a] = (uint16_t)(tid * 32 + a);
-  }
+  const bool slow = nD > NF_LIST || nU > NF_LIST;
   snD[tid] = (uint8_t)min(nD, NF_LIST);
-  __syncthreads();
-
-  // ---- pair phase: one item = (h, u); loop over the D list of h ----
-  const uint32_t Tn = sm_T;
-  for (uint32_t i = tid; i < Tn; i += NF_THREADS) {
-    const uint32_t e = it[i];
-    const int hl = e >> 5, a = e & 31;
-    const float2 hh = sH[hl];
-    const float2 uu = sU[ul[a * NF_THREADS + hl]];
-    const float tyu = (uu.x - hh.x) * iu, tzu = (uu.y - hh.y) * iu;
-    const int n = snD[hl];
-    float best = 0.0f;
-    uint32_t bd = 0;
-    for (int j = 0; j < n; ++j) {
-      const uint32_t di = dl[j * NF_THREADS + hl];
-      const float2 dd = sD[di];
-      const float tyd = (hh.x - dd.x) * id, tzd = (hh.y - dd.y) * id;
-      const float ey = tyu - tyd, ez = tzu - tzd;
-      const float dev = ey * ey + ez * ez;
-      if (j == 0 || dev < best || (dev == best && __ldg(s2o + kD0 + di) < __ldg(s2o + kD0 + bd))) { best = dev; bd = di; }
+  bool pending = nD > 0 && nU > 0 && !slow;        // still has to put its nU items through the pair phase
+  bool have = false;
+  float best = 0.0f;
+  uint32_t bu = 0, bd = 0;
+  // The item list holds NF_ITEMS (h,u) items; CTAs with more run the pair phase in several rounds.
+  for (;;) {
+    uint32_t total;
+    const uint32_t mine = pending ? (uint32_t)nU : 0u;
+    if (tid == 0) sm_T = 0;
+    const uint32_t base = blockExclusiveScan(mine, sscan, &total);
+    if (total == 0) break;                          // uniform
+    const bool now = pending && base + mine <= NF_ITEMS;
+    if (now) {
+      for (uint32_t a = 0; a < mine; ++a) it[base + a] = (uint16_t)(tid * 32 + a);
+      atomicMax(&sm_T, base + mine);
     }
-    it_dev[i] = best;
-    it_d[i] = (uint16_t)bd;
+    __syncthreads();
+    const uint32_t Tn = sm_T;                       // end of the last thread that fitted this round
+    // ---- pair phase: one item = (h, u); loop over the D list of h ----
+    for (uint32_t i = tid; i < Tn; i += NF_THREADS) {
+      const uint32_t e = it[i];
+      const int hl = e >> 5, a = e & 31;
+      const float2 hh = sH[hl];
+      const float2 uu = sU[ul[a * NF_THREADS + hl]];
+      const float tyu = (uu.x - hh.x) * iu, tzu = (uu.y - hh.y) * iu;
+      const int n = snD[hl];
+      float bdev = 0.0f;
+      uint32_t bdi = 0;
+      for (int j = 0; j < n; ++j) {
+        const uint32_t di = dl[j * NF_THREADS + hl];
+        const float2 dd = sD[di];
+        const float tyd = (hh.x - dd.x) * id, tzd = (hh.y - dd.y) * id;
+        const float ey = tyu - tyd, ez = tzu - tzd;
+        const float dev = ey * ey + ez * ez;
+        if (j == 0 || dev < bdev || (dev == bdev && __ldg(s2o + kD0 + di) < __ldg(s2o + kD0 + bdi))) { bdev = dev; bdi = di; }
+      }
+      it_dev[i] = bdev;
+      it_d[i] = (uint16_t)bdi;
+    }
+    __syncthreads();
+    // ---- per-cluster reduction over its own items, full key (Dev, orig u, orig d) ----
+    if (now) {
+      for (uint32_t a = 0; a < mine; ++a) {
+        const float dev = it_dev[base + a];
+        if (!have || dev <= best) {
+          const uint32_t u = kU0 + ul[a * NF_THREADS + tid], d = kD0 + it_d[base + a];
+          if (pairBetter(have, dev, best, u, d, bu, bd, s2o)) { have = true; best = dev; bu = u; bd = d; }
+        }
+      }
+      pending = false;
+    }
+    __syncthreads();                                // the item arrays are rewritten in the next round
   }
-  __syncthreads();
-
-  // ---- per-cluster reduction over its own items, full key (Dev, orig u, orig d) ----
   if (!valid) return;
   if (slow) {
     neighbourSlow(p, h, Gu, Gd, cell_start, syz, s2o, iu, id, wyu, wzu, wyd, wzd, P.link_dev2_max, lup, ldn);
     return;
-  }
-  bool have = false;
-  float best = 0.0f;
-  uint32_t bu = 0, bd = 0;
-  for (uint32_t a = 0; a < cntU; ++a) {
-    const float dev = it_dev[base + a];
-    if (!have || dev <= best) {
-      const uint32_t u = kU0 + ul[a * NF_THREADS + tid], d = kD0 + it_d[base + a];
-      if (pairBetter(have, dev, best, u, d, bu, bd, s2o)) { have = true; best = dev; bu = u; bd = d; }
-    }
   }
   const bool link = have && best <= P.link_dev2_max;
   lup[p] = link ? (int32_t)bu : -1;
