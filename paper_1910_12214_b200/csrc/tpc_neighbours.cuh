@@ -23,7 +23,8 @@ namespace tpc {
 constexpr int NF_THREADS = 128;
 constexpr int NF_REGION = 640;     // staged candidates per side
 constexpr int NF_LIST = 32;        // window candidates kept per thread and side (<= 32: packed item code)
-constexpr int NF_ITEMS = 1536;     // (h,u) items per CTA
+constexpr int NF_UB = 4;          // u's per item (register blocking of the pair loop)
+constexpr int NF_ITEMS = 512;      // items per CTA and round
 
 struct RowTables {
   const float* row_x;     // [R]
@@ -82,10 +83,9 @@ __device__ __forceinline__ int gatherWindow(const GridDesc& G, const uint32_t* _
   for (;;) {
     if (k < kend) {
       const float2 c = reg[k - k0];
-      if (fabsf(c.x - yc) <= wy && fabsf(c.y - zc) <= wz) {
-        if (n < NF_LIST) list[n * NF_THREADS + tid] = (uint16_t)(k - k0);
-        ++n;
-      }
+      const bool pass = fabsf(c.x - yc) <= wy && fabsf(c.y - zc) <= wz;
+      list[min(n, NF_LIST) * NF_THREADS + tid] = (uint16_t)(k - k0);     // row NF_LIST is a spare: no branch needed
+      n += pass ? 1 : 0;
       ++k;
     } else {
       if (++bz > bz1) break;
@@ -103,10 +103,10 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
                                                               const uint32_t* __restrict__ s2o, int32_t* __restrict__ lup,
                                                               int32_t* __restrict__ ldn, const int64_t* __restrict__ cnt) {
   __shared__ float2 sD[NF_REGION], sU[NF_REGION], sH[NF_THREADS];
-  __shared__ uint16_t dl[NF_LIST * NF_THREADS], ul[NF_LIST * NF_THREADS];
-  __shared__ uint16_t it[NF_ITEMS], it_d[NF_ITEMS];
-  __shared__ float it_dev[NF_ITEMS];
-  __shared__ uint8_t snD[NF_THREADS];
+  __shared__ uint16_t dl[(NF_LIST + 1) * NF_THREADS], ul[(NF_LIST + 1) * NF_THREADS];
+  __shared__ uint16_t it[NF_ITEMS], it_d[NF_ITEMS * NF_UB];
+  __shared__ float it_dev[NF_ITEMS * NF_UB];
+  __shared__ uint8_t snD[NF_THREADS], snU[NF_THREADS];
   __shared__ float red[2][NF_THREADS / 32];
   __shared__ uint32_t sscan[33];
   __shared__ int sm_b;
@@ -183,6 +183,7 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
   }
   const bool slow = nD > NF_LIST || nU > NF_LIST;
   snD[tid] = (uint8_t)min(nD, NF_LIST);
+  snU[tid] = (uint8_t)min(nU, NF_LIST);
   bool pending = nD > 0 && nU > 0 && !slow;        // still has to put its nU items through the pair phase
   bool have = false;
   float best = 0.0f;
@@ -190,45 +191,59 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
   // The item list holds NF_ITEMS (h,u) items; CTAs with more run the pair phase in several rounds.
   for (;;) {
     uint32_t total;
-    const uint32_t mine = pending ? (uint32_t)nU : 0u;
+    const uint32_t mine = pending ? (uint32_t)((nU + NF_UB - 1) / NF_UB) : 0u;     // items: groups of NF_UB u's
     if (tid == 0) sm_T = 0;
     const uint32_t base = blockExclusiveScan(mine, sscan, &total);
     if (total == 0) break;                          // uniform
     const bool now = pending && base + mine <= NF_ITEMS;
     if (now) {
-      for (uint32_t a = 0; a < mine; ++a) it[base + a] = (uint16_t)(tid * 32 + a);
+      for (uint32_t a = 0; a < mine; ++a) it[base + a] = (uint16_t)(tid * 32 + a * NF_UB);
       atomicMax(&sm_T, base + mine);
     }
     __syncthreads();
     const uint32_t Tn = sm_T;                       // end of the last thread that fitted this round
-    // ---- pair phase: one item = (h, u); loop over the D list of h ----
+    // ---- pair phase: one item = (h, NF_UB consecutive u's of its list); loop over the D list of h.
+    //      The down slopes are computed once per d and used for all u's of the item (register blocking).
     for (uint32_t i = tid; i < Tn; i += NF_THREADS) {
       const uint32_t e = it[i];
-      const int hl = e >> 5, a = e & 31;
+      const int hl = e >> 5, a0 = e & 31;
       const float2 hh = sH[hl];
-      const float2 uu = sU[ul[a * NF_THREADS + hl]];
-      const float tyu = (uu.x - hh.x) * iu, tzu = (uu.y - hh.y) * iu;
+      const int nu = snU[hl];
+      float tyu[NF_UB], tzu[NF_UB], bdev[NF_UB];
+      uint32_t bdi[NF_UB];
+#pragma unroll
+      for (int q = 0; q < NF_UB; ++q) {
+        const float2 uu = sU[ul[min(a0 + q, nu - 1) * NF_THREADS + hl]];     // a short last group repeats its last u
+        tyu[q] = (uu.x - hh.x) * iu; tzu[q] = (uu.y - hh.y) * iu;
+        bdev[q] = __int_as_float(0x7f800000); bdi[q] = 0;
+      }
       const int n = snD[hl];
-      float bdev = 0.0f;
-      uint32_t bdi = 0;
       for (int j = 0; j < n; ++j) {
         const uint32_t di = dl[j * NF_THREADS + hl];
         const float2 dd = sD[di];
         const float tyd = (hh.x - dd.x) * id, tzd = (hh.y - dd.y) * id;
-        const float ey = tyu - tyd, ez = tzu - tzd;
-        const float dev = ey * ey + ez * ez;
-        if (j == 0 || dev < bdev || (dev == bdev && __ldg(s2o + kD0 + di) < __ldg(s2o + kD0 + bdi))) { bdev = dev; bdi = di; }
+#pragma unroll
+        for (int q = 0; q < NF_UB; ++q) {
+          const float ey = tyu[q] - tyd, ez = tzu[q] - tzd;
+          const float dev = ey * ey + ez * ez;
+          // Window slopes are bounded by area_y/area_z, so dev is finite: +inf is a safe "none yet".  The minimum
+          // is tracked with selects (no branch); exact ties (duplicated clusters) are rare and resolved apart.
+          if (dev == bdev[q] && __ldg(s2o + kD0 + di) < __ldg(s2o + kD0 + bdi[q])) bdi[q] = di;
+          const bool better = dev < bdev[q];
+          bdi[q] = better ? di : bdi[q];
+          bdev[q] = better ? dev : bdev[q];
+        }
       }
-      it_dev[i] = bdev;
-      it_d[i] = (uint16_t)bdi;
+#pragma unroll
+      for (int q = 0; q < NF_UB; ++q) { it_dev[i * NF_UB + q] = bdev[q]; it_d[i * NF_UB + q] = (uint16_t)bdi[q]; }
     }
     __syncthreads();
     // ---- per-cluster reduction over its own items, full key (Dev, orig u, orig d) ----
     if (now) {
-      for (uint32_t a = 0; a < mine; ++a) {
-        const float dev = it_dev[base + a];
+      for (int a = 0; a < nU; ++a) {
+        const float dev = it_dev[base * NF_UB + a];
         if (!have || dev <= best) {
-          const uint32_t u = kU0 + ul[a * NF_THREADS + tid], d = kD0 + it_d[base + a];
+          const uint32_t u = kU0 + ul[a * NF_THREADS + tid], d = kD0 + it_d[base * NF_UB + a];
           if (pairBetter(have, dev, best, u, d, bu, bd, s2o)) { have = true; best = dev; bu = u; bd = d; }
         }
       }
