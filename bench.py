@@ -143,6 +143,18 @@ def run_reference(args, rank):
     print(json.dumps(line), flush=True)
 
 
+def aggregate(units: float, ms: float, device, world: int):
+    """Whole-job figures of a replicated (weak-scaling) run: units summed over ranks, time = max over ranks."""
+    import torch
+    import torch.distributed as dist
+    u = torch.tensor([units], dtype=torch.float64, device=device)
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    if world > 1:
+        dist.all_reduce(u, op=dist.ReduceOp.SUM)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(u.item()), float(t.item())
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
@@ -192,13 +204,9 @@ def run_ours(args, rank, world, local_rank):
         dist.barrier()
     t1 = time.time()
     ms_total = e0.elapsed_time(e1)
-    clusters = torch.tensor([float(N)], device="cuda")
-    tmax = torch.tensor([ms_total], device="cuda")
-    if world > 1:
-        dist.all_reduce(clusters, op=dist.ReduceOp.SUM)
-        dist.all_reduce(tmax, op=dist.ReduceOp.MAX)
-    ms_step = float(tmax.item()) / args.steps
-    value = float(clusters.item()) / (ms_step * 1e-3)
+    total_clusters, ms_max = aggregate(float(N), ms_total, torch.device("cuda", local_rank), world)
+    ms_step = ms_max / args.steps
+    value = total_clusters / (ms_step * 1e-3)
     clocks = sampler.stop(t0, t1) if sampler else None
     stage /= args.steps
 
@@ -218,10 +226,8 @@ def run_ours(args, rank, world, local_rank):
         sth, outh = trk.run_host(noff, ny, nz, cap_tracks=capK, cap_track_clusters=capC)
     e1.record(stream)
     torch.cuda.synchronize()
-    ms_e2e = torch.tensor([e0.elapsed_time(e1) / e2e_steps], device="cuda")
-    if world > 1:
-        dist.all_reduce(ms_e2e, op=dist.ReduceOp.MAX)
-    e2e_value = float(clusters.item()) / (float(ms_e2e.item()) * 1e-3)
+    _, ms_e2e = aggregate(float(N), e0.elapsed_time(e1) / e2e_steps, torch.device("cuda", local_rank), world)
+    e2e_value = total_clusters / (ms_e2e * 1e-3)
     nt, nc = int(sth.n_tracks), int(sth.n_track_clusters)
     h2d = 4 * (len(ev.row_offset)) + 8 * N
     d2h = nt * (5 * 4 + 4 + 20 + 60 + 4) + 4 * (nt + 1) + 4 * nc + 8 * 9
@@ -268,7 +274,7 @@ def run_ours(args, rank, world, local_rank):
                        "tracklets_per_step": nT, "start_hits_per_step": int(st.n_start_hits), "tracklet_hits": H},
             "tracks_per_s": float(st.n_tracks) * world / (ms_step * 1e-3),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                    "ms_per_step": float(ms_e2e.item()), "steps": e2e_steps},
+                    "ms_per_step": ms_e2e, "steps": e2e_steps},
             "gpu_launches": int(st.kernel_launches) * args.steps,
             "clocks": clocks, "roofline": roofline, "stages": stages, "cpu_baseline": cpu}
     print(json.dumps(line), flush=True)

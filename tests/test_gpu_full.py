@@ -1,0 +1,86 @@
+"""-m gpu: parity at BASELINE.json's full sizes, in the launch configuration bench.py times.
+
+Configs 3 and 4 (15-75 M clusters) are too large for the oracle as a whole, but sectors are independent
+(DESIGN.md section 9): the GPU result restricted to sector 0 of the full event must equal, bit for bit, the
+oracle's result on sector 0 alone (its clusters and start hits come first in the CSR order, so cluster indices
+and tracklet ids coincide).  Properties that hold at any size are checked on the whole event.
+"""
+import numpy as np
+import pytest
+
+from oracle import tpc_oracle as orc
+from paper_1910_12214_b200 import datagen
+from tests.parity import compare
+
+pytestmark = pytest.mark.gpu
+R = 152
+
+
+def _sector0(ev):
+    hi = int(ev.row_offset[R])
+    return datagen.event_from_arrays(ev.row_offset[:R + 1], ev.y[:hi], ev.z[:hi], 1, R, row_x=ev.row_x, z_min=ev.z_min,
+                                     z_max=ev.z_max, bz_tesla=ev.bz_tesla)
+
+
+@pytest.mark.parametrize("idx", [3, 4])
+def test_full_size_sector0_equals_oracle_and_global_invariants(idx):
+    import torch
+    from paper_1910_12214_b200 import tpc
+    ev = datagen.make_event(idx)
+    trk = tpc.TpcTracker.from_event(ev)
+    off, y, z = trk.upload(ev)
+    first = trk.run(off, y, z)
+    st = first.status
+    assert st.status == 0
+    # same capacities as bench.py; per-stage link outputs requested for the invariants
+    capT = int(st.n_start_hits * 1.05) + 1024
+    capK = int(st.n_tracks * 1.05) + 1024
+    capC = int(st.n_track_clusters * 1.05) + 1024
+    res = trk.run(off, y, z, cap_tracklets=capT, cap_tracks=capK, cap_track_clusters=capC, stages=True)
+    assert res.status.status == 0
+    n0 = int(ev.row_offset[R])
+    o = orc.run(_sector0(ev))
+    ns0 = len(o.start_hits)
+    g = {}
+    for k in ("link_up_raw", "link_dn_raw", "link_up", "link_dn"):
+        g[k] = res.stages[k][:n0].cpu().numpy()
+    for k in ("start_hits", "tl_status", "tl_nhits", "tl_first_row", "tl_last_row", "tl_rowhit", "tl_x", "tl_par", "tl_cov",
+              "tl_chi2"):
+        g[k] = res.stages[k][:ns0].cpu().numpy()
+    sec = res.trk["trk_sector"]
+    nt0 = int((sec == 0).sum().item())
+    assert bool((sec[:nt0] == 0).all().item())                 # ascending tracklet id = ascending sector
+    offs = res.trk["trk_cl_offset"].cpu().numpy().view(np.uint32)
+    for k in ("trk_tracklet", "trk_sector", "trk_first_row", "trk_last_row", "trk_ncl", "trk_x", "trk_chi2"):
+        g[k] = res.trk[k][:nt0].cpu().numpy()
+    g["trk_par"] = res.trk["trk_par"][:, :nt0].cpu().numpy()
+    g["trk_cov"] = res.trk["trk_cov"][:, :nt0].cpu().numpy()
+    g["trk_cl_offset"] = offs[:nt0 + 1].view(np.int32)
+    g["trk_cl_index"] = res.trk["trk_cl_index"][:int(offs[nt0])].cpu().numpy()
+    # start hits of sector 0 are exactly the first ns0 of the list
+    sh = res.stages["start_hits"].cpu().numpy().view(np.uint32)
+    assert ns0 == int((sh < n0).sum()) and np.all(sh[:ns0] < n0)
+    rep = compare(g, o, R)
+    print(ev.name, ev.n_clusters, "sector-0 tracks", nt0, rep)
+    # ---- whole event: invariants that hold at any size ----
+    up, dn = res.stages["link_up"].long(), res.stages["link_dn"].long()
+    n = ev.n_clusters
+    ar = torch.arange(n, device=up.device)
+    hu = up >= 0
+    assert bool((dn[up[hu]] == ar[hu]).all().item())           # reciprocity (north_star check 5)
+    hd = dn >= 0
+    assert bool((up[dn[hd]] == ar[hd]).all().item())
+    idx_all = res.trk["trk_cl_index"].long()
+    assert int(torch.unique(idx_all).numel()) == idx_all.numel()                      # a cluster is in <= 1 track
+    ncl = res.trk["trk_ncl"].long()
+    o64 = torch.from_numpy(offs.astype(np.int64)).to(ncl.device)
+    assert bool(((o64[1:] - o64[:-1]) == ncl).all().item()) and int(ncl.sum().item()) == idx_all.numel()
+    assert int(ncl.min().item()) >= 10
+    t = res.trk["trk_tracklet"].long()
+    assert bool((t[1:] > t[:-1]).all().item())                                        # ascending tracklet id
+    # clusters of a track lie in its sector
+    bucket_sector = torch.from_numpy(np.repeat(np.arange(ev.n_sectors * R) // R, np.diff(ev.row_offset.astype(np.int64)))).to(ncl.device)
+    trk_of_cl = torch.repeat_interleave(torch.arange(res.n_tracks, device=ncl.device), ncl)
+    assert bool((bucket_sector[idx_all] == res.trk["trk_sector"].long()[trk_of_cl]).all().item())
+    assert bool(torch.isfinite(res.trk["trk_par"]).all().item()) and bool(torch.isfinite(res.trk["trk_cov"]).all().item())
+    trk.close()
