@@ -41,7 +41,8 @@ enum Counter {
   CNT_N_TRK_CL = 5,     // track clusters (may exceed cap)
   CNT_N_CELLS = 6,
   CNT_WORK = 7,         // dynamic work counter of the constructor
-  CNT_COUNT = 8
+  CNT_N_LONG = 8,       // seeds whose link chain is long enough to survive the chain fit (the constructor's work list)
+  CNT_COUNT = 9
 };
 
 // Tracklet SoA in the workspace (capT = capacity in tracklets).

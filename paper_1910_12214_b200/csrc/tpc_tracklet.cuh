@@ -73,13 +73,76 @@ __device__ __forceinline__ int32_t searchFinish(const SearchPre& sp, const float
       if (two) test(k + 1, c);
     }
   };
-  scan(sp.kA0, sp.kA1);
-  if (sp.bz1 > sp.bz0) scan(sp.kB0, sp.kB1);
+  // first the heads of the two prefetched cell rows: up to 4 + 4 candidates, every load in flight before the
+  // first test (one memory latency per search instead of one per candidate)
+  const uint32_t nA = sp.kA1 - sp.kA0;
+  const uint32_t nB = sp.bz1 > sp.bz0 ? sp.kB1 - sp.kB0 : 0u;
+  float2 ca[4], cb[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) ca[i] = i < nA ? __ldg(syz + sp.kA0 + i) : make_float2(0.0f, 0.0f);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) cb[i] = i < nB ? __ldg(syz + sp.kB0 + i) : make_float2(0.0f, 0.0f);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) if (i < nA) test(sp.kA0 + i, ca[i]);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) if (i < nB) test(sp.kB0 + i, cb[i]);
+  if (nA > 4) scan(sp.kA0 + 4, sp.kA1);
+  if (nB > 4) scan(sp.kB0 + 4, sp.kB1);
   for (int bz = sp.bz0 + 2; bz <= sp.bz1; ++bz) {   // roads wider than two cell rows: rare
     const uint32_t* r = sp.cs + bz * sp.ny;
     scan(__ldg(r), __ldg(r + sp.span));
   }
   return best;
+}
+
+// One thread per start hit, before the constructor: bucket of the seed, length of its link chain.  Chains shorter
+// than min_chain_hits can only end as "discarded in the chain fit" (O4 step 2): they are fitted right here (the
+// hit count of a discarded tracklet is part of the per-stage output) and never reach the persistent kernel;
+// the others are appended to the constructor's work list.  At high occupancy most start hits are such stubs.
+__global__ void __launch_bounds__(128) seedPrepare(const uint32_t* __restrict__ off, DevParams P, RowTables T,
+                                                   const float2* __restrict__ syz, const int32_t* __restrict__ cup,
+                                                   const uint32_t* __restrict__ start_pos, uint32_t* __restrict__ start_bucket,
+                                                   uint32_t* __restrict__ work, TrackletStore out, int64_t* __restrict__ cnt) {
+  if (cnt[CNT_ERROR] != 0) return;
+  const int64_t nT = min(cnt[CNT_N_START], out.capT);
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nT) return;
+  const uint32_t h0 = start_pos[t];
+  const int b0 = bucketOf(off, P.n_buckets, h0);
+  start_bucket[t] = (uint32_t)b0;
+  int len = 1;
+  for (int32_t h = cup[h0]; h != -1 && len < P.min_chain_hits; h = cup[h]) ++len;
+  if (len >= P.min_chain_hits) {
+    const unsigned long long j = atomicAdd((unsigned long long*)(cnt + CNT_N_LONG), 1ull);
+    work[j] = (uint32_t)t;
+    return;
+  }
+  // short chain: O4 steps 1-2 on its len-1 links; the result is always status 0, nhits = hits fitted
+  const int R = P.n_rows;
+  const int r0 = b0 % R;
+  int r = T.up_row[r0];
+  int32_t h = cup[h0];
+  KFState S;
+  {
+    const float2 a = syz[h0], c = syz[h];
+    S.x = T.row_x[r0]; S.y = a.x; S.z = a.y;
+    const float dx = T.row_x[r] - T.row_x[r0], dy = c.x - a.x, dz = c.y - a.y;
+    const float L = sqrtf(dx * dx + dy * dy);
+    S.s = dy / L; S.t = dz / L; S.q = 0.0f;
+  }
+  kfSetDiag(S, P.err2_y, P.err2_z, P);
+  S.chi2 = 0.0f;
+  int nhits = 1;
+  while (h != -1) {
+    if (!kfPropagate(S, T.row_x[r], P, [](float, float, float, float) {})) break;
+    const float2 c = syz[h];
+    if (!kfUpdate(S, c.x, c.y, P)) break;
+    ++nhits;
+    h = cup[h];
+    r = T.up_row[r];
+  }
+  out.sector[t] = b0 / R;
+  out.status[t] = 0; out.nhits[t] = nhits; out.first_row[t] = -1; out.last_row[t] = -1;
 }
 
 // Persistent warps; every lane owns one seed at a time and fetches the next one from a global counter as soon
@@ -92,9 +155,10 @@ __device__ __forceinline__ int32_t searchFinish(const SearchPre& sp, const float
 // search from inside Propagate.  The order of floating-point operations of a seed is exactly the sequential
 // algorithm's.
 __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor(
-    const uint32_t* __restrict__ off, DevParams P, RowTables T, const GridDesc* __restrict__ desc,
-    const uint32_t* __restrict__ cell_start, const float2* __restrict__ syz, const uint32_t* __restrict__ s2o,
-    const int32_t* __restrict__ cup, const uint32_t* __restrict__ start_pos, TrackletStore out, int64_t* __restrict__ cnt) {
+    DevParams P, RowTables T, const GridDesc* __restrict__ desc, const uint32_t* __restrict__ cell_start,
+    const float2* __restrict__ syz, const uint32_t* __restrict__ s2o, const int32_t* __restrict__ cup,
+    const uint32_t* __restrict__ start_pos, const uint32_t* __restrict__ start_bucket, const uint32_t* __restrict__ work_list,
+    TrackletStore out, int64_t* __restrict__ cnt) {
   __shared__ float sx[MAX_ROWS];
   __shared__ int16_t sup[MAX_ROWS];
   __shared__ uint8_t sdead[MAX_ROWS];
@@ -104,7 +168,7 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
   const int tid = threadIdx.x;
   for (int i = tid; i < R; i += blockDim.x) { sx[i] = T.row_x[i]; sup[i] = T.up_row[i]; sdead[i] = T.dead[i]; }
   __syncthreads();
-  const int64_t nT = min(cnt[CNT_N_START], out.capT);
+  const int64_t nW = cnt[CNT_N_LONG];            // seeds on the work list (seedPrepare)
   const int64_t capT = out.capT;
   unsigned long long* work = (unsigned long long*)(cnt + CNT_WORK);
 
@@ -119,12 +183,13 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
 
   for (;;) {
     if (phase == -1) {            // ---- fetch and initialise the next seed (O4 step 1) ----
-      t = (int64_t)atomicAdd(work, 1ull);
-      if (t >= nT) {
+      const int64_t j = (int64_t)atomicAdd(work, 1ull);
+      if (j >= nW) {
         phase = -2;
       } else {
+        t = work_list[j];
         const uint32_t h0 = start_pos[t];
-        const int b0 = bucketOf(off, P.n_buckets, h0);
+        const int b0 = (int)start_bucket[t];
         r0 = b0 % R;
         bsec = b0 - r0;
         rowhit = out.rowhit + t * R;
