@@ -185,7 +185,7 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
   snD[tid] = (uint8_t)min(nD, NF_LIST);
   snU[tid] = (uint8_t)min(nU, NF_LIST);
   bool pending = nD > 0 && nU > 0 && !slow;        // still has to put its nU items through the pair phase
-  bool have = false;
+  bool have = false, tied = false;
   float best = 0.0f;
   uint32_t bu = 0, bd = 0;
   // The item list holds NF_ITEMS (h,u) items; CTAs with more run the pair phase in several rounds.
@@ -211,11 +211,12 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
       const int nu = snU[hl];
       float tyu[NF_UB], tzu[NF_UB], bdev[NF_UB];
       uint32_t bdi[NF_UB];
+      bool tie[NF_UB];
 #pragma unroll
       for (int q = 0; q < NF_UB; ++q) {
         const float2 uu = sU[ul[min(a0 + q, nu - 1) * NF_THREADS + hl]];     // a short last group repeats its last u
         tyu[q] = (uu.x - hh.x) * iu; tzu[q] = (uu.y - hh.y) * iu;
-        bdev[q] = __int_as_float(0x7f800000); bdi[q] = 0;
+        bdev[q] = __int_as_float(0x7f800000); bdi[q] = 0; tie[q] = false;
       }
       const int n = snD[hl];
       for (int j = 0; j < n; ++j) {
@@ -227,15 +228,19 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
           const float ey = tyu[q] - tyd, ez = tzu[q] - tzd;
           const float dev = ey * ey + ez * ez;
           // Window slopes are bounded by area_y/area_z, so dev is finite: +inf is a safe "none yet".  The minimum
-          // is tracked with selects (no branch); exact ties (duplicated clusters) are rare and resolved apart.
-          if (dev == bdev[q] && __ldg(s2o + kD0 + di) < __ldg(s2o + kD0 + bdi[q])) bdi[q] = di;
+          // is tracked with selects (no branch).  An exact tie with the running minimum (duplicated clusters) is
+          // only flagged: such a cluster is redone by neighbourSlow with the full key (R6).
+          tie[q] = tie[q] || dev == bdev[q];
           const bool better = dev < bdev[q];
           bdi[q] = better ? di : bdi[q];
           bdev[q] = better ? dev : bdev[q];
         }
       }
 #pragma unroll
-      for (int q = 0; q < NF_UB; ++q) { it_dev[i * NF_UB + q] = bdev[q]; it_d[i * NF_UB + q] = (uint16_t)bdi[q]; }
+      for (int q = 0; q < NF_UB; ++q) {
+        it_dev[i * NF_UB + q] = bdev[q];
+        it_d[i * NF_UB + q] = (uint16_t)(bdi[q] | (tie[q] ? 0x8000u : 0u));
+      }
     }
     __syncthreads();
     // ---- per-cluster reduction over its own items, full key (Dev, orig u, orig d) ----
@@ -243,7 +248,9 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
       for (int a = 0; a < nU; ++a) {
         const float dev = it_dev[base * NF_UB + a];
         if (!have || dev <= best) {
-          const uint32_t u = kU0 + ul[a * NF_THREADS + tid], d = kD0 + it_d[base * NF_UB + a];
+          const uint32_t dcode = it_d[base * NF_UB + a];
+          tied = tied || (dcode & 0x8000u) != 0u;
+          const uint32_t u = kU0 + ul[a * NF_THREADS + tid], d = kD0 + (dcode & 0x7fffu);
           if (pairBetter(have, dev, best, u, d, bu, bd, s2o)) { have = true; best = dev; bu = u; bd = d; }
         }
       }
@@ -252,7 +259,7 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
     __syncthreads();                                // the item arrays are rewritten in the next round
   }
   if (!valid) return;
-  if (slow) {
+  if (slow || tied) {
     neighbourSlow(p, h, Gu, Gd, cell_start, syz, s2o, iu, id, wyu, wzu, wyd, wzd, P.link_dev2_max, lup, ldn);
     return;
   }
