@@ -25,6 +25,7 @@ constexpr int NF_REGION = 640;     // staged candidates per side
 constexpr int NF_LIST = 32;        // window candidates kept per thread and side (<= 32: packed item code)
 constexpr int NF_UB = 4;          // u's per item (register blocking of the pair loop)
 constexpr int NF_ITEMS = 512;      // items per CTA and round
+constexpr int NF_ROWS = 6;         // cell rows of a window whose ranges are staged (more: slow path)
 
 struct RowTables {
   const float* row_x;     // [R]
@@ -65,32 +66,44 @@ __device__ __noinline__ void neighbourSlow(uint32_t p, float2 h, const GridDesc&
   ldn[p] = link ? (int32_t)bd : -1;
 }
 
-// window walk over a region staged in shared memory: the cell ranges come from the global cell table, the
-// coordinates from `reg` (region index = sorted position - k0).  Appends the indices passing the predicate.
+// window walk over a region staged in shared memory: the cluster ranges of the window's cell rows come from the
+// global cell table (all requested at once, kept as 16-bit region offsets in `rows`), the coordinates from `reg`
+// (region index = sorted position - k0).  Appends the indices passing the predicate; returns their number, or
+// NF_LIST + 1 when the window spans more than NF_ROWS cell rows (the caller then takes the slow path).
 __device__ __forceinline__ int gatherWindow(const GridDesc& G, const uint32_t* __restrict__ cell_start, const float2* reg,
-                                            uint32_t k0, float yc, float zc, float wy, float wz, uint16_t* list, int tid) {
+                                            uint32_t k0, float yc, float zc, float wy, float wz, uint16_t* list,
+                                            ushort2* rows, int tid) {
   if (G.n == 0) return 0;
   const float sy = 1e-5f * (fabsf(yc) + wy) + 1e-6f;
   const float sz = 1e-5f * (fabsf(zc) + wz) + 1e-6f;
   const int by0 = cellCoord((yc - wy) - sy, G.y0, G.inv_e, G.ny);
   const int by1 = cellCoord((yc + wy) + sy, G.y0, G.inv_e, G.ny);
-  int bz = cellCoord((zc - wz) - sz, G.z0, G.inv_e, G.nz);
-  const int bz1 = cellCoord((zc + wz) + sz, G.z0, G.inv_e, G.nz);
-  const uint32_t* cs = cell_start + G.cell_base + by0;
+  const int bz0 = cellCoord((zc - wz) - sz, G.z0, G.inv_e, G.nz);
+  const int nr = cellCoord((zc + wz) + sz, G.z0, G.inv_e, G.nz) - bz0 + 1;
+  if (nr > NF_ROWS) return NF_LIST + 1;
+  const uint32_t* cs = cell_start + G.cell_base + by0 + bz0 * G.ny;
   const int span = by1 - by0 + 1;
-  uint32_t k = __ldg(cs + bz * G.ny), kend = __ldg(cs + bz * G.ny + span);
-  int n = 0;
+  uint32_t ra[NF_ROWS], rb[NF_ROWS];
+#pragma unroll
+  for (int r = 0; r < NF_ROWS; ++r) {
+    const uint32_t* c = cs + (r < nr ? r : 0) * G.ny;
+    ra[r] = __ldg(c); rb[r] = __ldg(c + span);
+  }
+#pragma unroll
+  for (int r = 0; r < NF_ROWS; ++r) rows[r * NF_THREADS + tid] = make_ushort2((uint16_t)(ra[r] - k0), (uint16_t)(rb[r] - k0));
+  uint32_t k = ra[0] - k0, kend = rb[0] - k0;
+  int n = 0, r = 0;
   for (;;) {
     if (k < kend) {
-      const float2 c = reg[k - k0];
+      const float2 c = reg[k];
       const bool pass = fabsf(c.x - yc) <= wy && fabsf(c.y - zc) <= wz;
-      list[min(n, NF_LIST) * NF_THREADS + tid] = (uint16_t)(k - k0);     // row NF_LIST is a spare: no branch needed
+      list[min(n, NF_LIST) * NF_THREADS + tid] = (uint16_t)k;     // row NF_LIST is a spare: no branch needed
       n += pass ? 1 : 0;
       ++k;
     } else {
-      if (++bz > bz1) break;
-      k = __ldg(cs + bz * G.ny);
-      kend = __ldg(cs + bz * G.ny + span);
+      if (++r >= nr) break;
+      const ushort2 v = rows[r * NF_THREADS + tid];
+      k = v.x; kend = v.y;
     }
   }
   return n;
@@ -107,6 +120,7 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
   __shared__ uint16_t it[NF_ITEMS], it_d[NF_ITEMS * NF_UB];
   __shared__ float it_dev[NF_ITEMS * NF_UB];
   __shared__ uint8_t snD[NF_THREADS], snU[NF_THREADS];
+  __shared__ ushort2 srow[NF_ROWS * NF_THREADS];
   __shared__ float red[2][NF_THREADS / 32];
   __shared__ uint32_t sscan[33];
   __shared__ int sm_b;
@@ -178,8 +192,8 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
   // ---- per-thread window lists ----
   int nD = 0, nU = 0;
   if (valid) {
-    nD = gatherWindow(Gd, cell_start, sD, kD0, h.x, h.y, wyd, wzd, dl, tid);
-    if (nD > 0) nU = gatherWindow(Gu, cell_start, sU, kU0, h.x, h.y, wyu, wzu, ul, tid);
+    nD = gatherWindow(Gd, cell_start, sD, kD0, h.x, h.y, wyd, wzd, dl, srow, tid);
+    if (nD > 0) nU = gatherWindow(Gu, cell_start, sU, kU0, h.x, h.y, wyu, wzu, ul, srow, tid);
   }
   const bool slow = nD > NF_LIST || nU > NF_LIST;
   snD[tid] = (uint8_t)min(nD, NF_LIST);
