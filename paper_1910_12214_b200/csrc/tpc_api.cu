@@ -38,7 +38,8 @@ struct Workspace {
   int32_t* spos_by_orig;
   uint32_t* tiles32;         // tile sums: cells scan / start compaction
   unsigned long long* tiles64;
-  uint32_t *start_orig, *start_pos, *start_bucket, *work_list;
+  uint32_t *start_orig, *start_pos;
+  SeedRec* work_list;        // long seeds, in the order the constructor takes them
   TrackletStore tl;
   unsigned long long *tsel, *tscan;
   int32_t *kept_first, *kept_last;
@@ -114,8 +115,7 @@ Workspace layout(const tpcHandle* h, int64_t N, int64_t capT, char* base) {
   w.tiles64 = (unsigned long long*)take(8 * (size_t)(ceilDiv(Tn, SCAN_TILE) + 2));
   w.start_orig = (uint32_t*)take(4 * (size_t)Tn);
   w.start_pos = (uint32_t*)take(4 * (size_t)Tn);
-  w.start_bucket = (uint32_t*)take(4 * (size_t)Tn);
-  w.work_list = (uint32_t*)take(4 * (size_t)Tn);
+  w.work_list = (SeedRec*)take(sizeof(SeedRec) * (size_t)Tn);
   w.tl.capT = capT;
   w.tl.n_rows = R;
   w.tl.status = (int32_t*)take(4 * (size_t)Tn);
@@ -317,10 +317,10 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   // ---- a4 tracklet constructor --------------------------------------------------------------------
   if (N > 0 && capT > 0) {
     const unsigned grid = (unsigned)std::min<int64_t>(ceilDiv(capT, TC_THREADS), h->tc_grid);
-    seedPrepare<<<(unsigned)ceilDiv(capT, 128), 128, 0, st>>>(in->row_offset, P, T, w.syz, w.cup, w.start_pos, w.start_bucket,
-                                                              w.work_list, w.tl, cnt); ++L;
-    trackletConstructor<<<grid, TC_THREADS, 0, st>>>(P, T, w.desc, w.cell_start, w.syz, w.s2o, w.cup, w.start_pos,
-                                                     w.start_bucket, w.work_list, w.tl, cnt); ++L;
+    seedPrepare<<<(unsigned)ceilDiv(capT, 128), 128, 0, st>>>(in->row_offset, P, T, w.syz, w.cup, w.start_pos, w.work_list,
+                                                              w.tl, cnt); ++L;
+    trackletConstructor<<<grid, TC_THREADS, 0, st>>>(P, T, w.desc, w.cell_start, w.syz, w.s2o, w.cup, w.work_list,
+                                                     w.tl, cnt); ++L;
   }
   stage(4);
   // ---- a5 selector ----------------------------------------------------------------------------------

@@ -50,50 +50,89 @@ __device__ __forceinline__ void searchBegin(SearchPre& sp, float yp, float zp, f
   sp.kB0 = __ldg(rB); sp.kB1 = __ldg(rB + sp.span);
 }
 
-// returns the sorted position of the best cluster or -1; its coordinates in (ym, zm)
-__device__ __forceinline__ int32_t searchFinish(const SearchPre& sp, const float2* __restrict__ syz,
-                                                const uint32_t* __restrict__ s2o, float& ym, float& zm) {
+// Exact re-scan of a window with the full key (d2, original index): only after the fast scan saw two candidates
+// at exactly the same distance (duplicated clusters, R6).
+__device__ __noinline__ int32_t searchExact(const SearchPre& sp, const float2* __restrict__ syz,
+                                            const uint32_t* __restrict__ s2o, float* ym, float* zm) {
   int32_t best = -1;
-  float bestd = 0.0f;
-  auto test = [&](uint32_t k, const float2 c) {
-    if (fabsf(c.x - sp.yp) <= sp.ry && fabsf(c.y - sp.zp) <= sp.rz) {
-      const float dy = c.x - sp.yp, dz = c.y - sp.zp;
-      const float d2 = dy * dy + dz * dz;
-      if (best < 0 || d2 < bestd || (d2 == bestd && __ldg(s2o + k) < __ldg(s2o + best))) {
-        best = (int32_t)k; bestd = d2; ym = c.x; zm = c.y;
+  float bestd = 0.0f, by = 0.0f, bz = 0.0f;
+  for (int r = sp.bz0; r <= sp.bz1; ++r) {
+    const uint32_t* row = sp.cs + r * sp.ny;
+    const uint32_t k1 = __ldg(row + sp.span);
+    for (uint32_t k = __ldg(row); k < k1; ++k) {
+      const float2 c = __ldg(syz + k);
+      if (fabsf(c.x - sp.yp) <= sp.ry && fabsf(c.y - sp.zp) <= sp.rz) {
+        const float dy = c.x - sp.yp, dz = c.y - sp.zp;
+        const float d2 = dy * dy + dz * dz;
+        if (best < 0 || d2 < bestd || (d2 == bestd && __ldg(s2o + k) < __ldg(s2o + best))) {
+          best = (int32_t)k; bestd = d2; by = c.x; bz = c.y;
+        }
       }
     }
+  }
+  *ym = by; *zm = bz;
+  return best;
+}
+
+// returns the sorted position of the best cluster or -1; its coordinates in (ym, zm).
+// The heads of the two prefetched cell rows (up to 4 + 4 candidates, every load in flight before the first test:
+// one memory latency per search instead of one per candidate) are evaluated without branches; unused slots hold
+// a point outside every window.  Longer rows and further cell rows are scanned by loops.
+__device__ __forceinline__ int32_t searchFinish(const SearchPre& sp, const float2* __restrict__ syz,
+                                                const uint32_t* __restrict__ s2o, float& ym, float& zm) {
+  const float yp = sp.yp, zp = sp.zp, ry = sp.ry, rz = sp.rz;
+  const uint32_t nA = sp.kA1 - sp.kA0;
+  const uint32_t nB = sp.bz1 > sp.bz0 ? sp.kB1 - sp.kB0 : 0u;
+  const float2 far = make_float2(3.0e38f, 3.0e38f);
+  float2 ca[4], cb[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) ca[i] = i < nA ? __ldg(syz + sp.kA0 + i) : far;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) cb[i] = i < nB ? __ldg(syz + sp.kB0 + i) : far;
+  float bestd = __int_as_float(0x7f800000);     // d2 of a candidate inside the road is finite
+  int32_t best = -1;
+  bool tie = false;
+  auto eval = [&](const float2 c, uint32_t k) {
+    const bool in = fabsf(c.x - yp) <= ry && fabsf(c.y - zp) <= rz;
+    const float dy = c.x - yp, dz = c.y - zp;
+    const float d2 = dy * dy + dz * dz;
+    tie = tie || (in && d2 == bestd);
+    const bool better = in && d2 < bestd;
+    best = better ? (int32_t)k : best;
+    bestd = better ? d2 : bestd;
+    ym = better ? c.x : ym;
+    zm = better ? c.y : zm;
   };
+#pragma unroll
+  for (int i = 0; i < 4; ++i) eval(ca[i], sp.kA0 + i);
+#pragma unroll
+  for (int i = 0; i < 4; ++i) eval(cb[i], sp.kB0 + i);
   auto scan = [&](uint32_t k0, uint32_t k1) {      // two independent loads per trip
     for (uint32_t k = k0; k < k1; k += 2) {
       const bool two = k + 1 < k1;
       const float2 a = __ldg(syz + k);
-      const float2 c = __ldg(syz + (two ? k + 1 : k));
-      test(k, a);
-      if (two) test(k + 1, c);
+      const float2 c = two ? __ldg(syz + k + 1) : far;
+      eval(a, k);
+      eval(c, k + 1);
     }
   };
-  // first the heads of the two prefetched cell rows: up to 4 + 4 candidates, every load in flight before the
-  // first test (one memory latency per search instead of one per candidate)
-  const uint32_t nA = sp.kA1 - sp.kA0;
-  const uint32_t nB = sp.bz1 > sp.bz0 ? sp.kB1 - sp.kB0 : 0u;
-  float2 ca[4], cb[4];
-#pragma unroll
-  for (int i = 0; i < 4; ++i) ca[i] = i < nA ? __ldg(syz + sp.kA0 + i) : make_float2(0.0f, 0.0f);
-#pragma unroll
-  for (int i = 0; i < 4; ++i) cb[i] = i < nB ? __ldg(syz + sp.kB0 + i) : make_float2(0.0f, 0.0f);
-#pragma unroll
-  for (int i = 0; i < 4; ++i) if (i < nA) test(sp.kA0 + i, ca[i]);
-#pragma unroll
-  for (int i = 0; i < 4; ++i) if (i < nB) test(sp.kB0 + i, cb[i]);
   if (nA > 4) scan(sp.kA0 + 4, sp.kA1);
   if (nB > 4) scan(sp.kB0 + 4, sp.kB1);
   for (int bz = sp.bz0 + 2; bz <= sp.bz1; ++bz) {   // roads wider than two cell rows: rare
     const uint32_t* r = sp.cs + bz * sp.ny;
     scan(__ldg(r), __ldg(r + sp.span));
   }
+  if (tie) best = searchExact(sp, syz, s2o, &ym, &zm);
   return best;
 }
+
+// One long seed in the constructor's work list (32 bytes, written by seedPrepare).
+struct SeedRec {
+  uint32_t t, h0;        // tracklet id, sorted position of the start hit
+  int32_t h1;            // first link
+  uint32_t b0r0;         // bucket << 8 | row of the start hit
+  float y0, z0, y1, z1;  // coordinates of h0 and h1
+};
 
 // One thread per start hit, before the constructor: bucket of the seed, length of its link chain.  Chains shorter
 // than min_chain_hits can only end as "discarded in the chain fit" (O4 step 2): they are fitted right here (the
@@ -101,25 +140,29 @@ __device__ __forceinline__ int32_t searchFinish(const SearchPre& sp, const float
 // the others are appended to the constructor's work list.  At high occupancy most start hits are such stubs.
 __global__ void __launch_bounds__(128) seedPrepare(const uint32_t* __restrict__ off, DevParams P, RowTables T,
                                                    const float2* __restrict__ syz, const int32_t* __restrict__ cup,
-                                                   const uint32_t* __restrict__ start_pos, uint32_t* __restrict__ start_bucket,
-                                                   uint32_t* __restrict__ work, TrackletStore out, int64_t* __restrict__ cnt) {
+                                                   const uint32_t* __restrict__ start_pos, SeedRec* __restrict__ work,
+                                                   TrackletStore out, int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
   const int64_t nT = min(cnt[CNT_N_START], out.capT);
   const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= nT) return;
   const uint32_t h0 = start_pos[t];
   const int b0 = bucketOf(off, P.n_buckets, h0);
-  start_bucket[t] = (uint32_t)b0;
+  const int R = P.n_rows;
+  const int r0 = b0 % R;
+  out.sector[t] = b0 / R;
   int len = 1;
   for (int32_t h = cup[h0]; h != -1 && len < P.min_chain_hits; h = cup[h]) ++len;
   if (len >= P.min_chain_hits) {
     const unsigned long long j = atomicAdd((unsigned long long*)(cnt + CNT_N_LONG), 1ull);
-    work[j] = (uint32_t)t;
+    const int32_t h1 = cup[h0];
+    const float2 a = syz[h0], c = syz[h1];
+    uint4* q = reinterpret_cast<uint4*>(work + j);
+    q[0] = make_uint4((uint32_t)t, h0, (uint32_t)h1, ((uint32_t)b0 << 8) | (uint32_t)r0);
+    q[1] = make_uint4(__float_as_uint(a.x), __float_as_uint(a.y), __float_as_uint(c.x), __float_as_uint(c.y));
     return;
   }
   // short chain: O4 steps 1-2 on its len-1 links; the result is always status 0, nhits = hits fitted
-  const int R = P.n_rows;
-  const int r0 = b0 % R;
   int r = T.up_row[r0];
   int32_t h = cup[h0];
   KFState S;
@@ -141,7 +184,6 @@ __global__ void __launch_bounds__(128) seedPrepare(const uint32_t* __restrict__ 
     h = cup[h];
     r = T.up_row[r];
   }
-  out.sector[t] = b0 / R;
   out.status[t] = 0; out.nhits[t] = nhits; out.first_row[t] = -1; out.last_row[t] = -1;
 }
 
@@ -157,16 +199,22 @@ __global__ void __launch_bounds__(128) seedPrepare(const uint32_t* __restrict__ 
 __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor(
     DevParams P, RowTables T, const GridDesc* __restrict__ desc, const uint32_t* __restrict__ cell_start,
     const float2* __restrict__ syz, const uint32_t* __restrict__ s2o, const int32_t* __restrict__ cup,
-    const uint32_t* __restrict__ start_pos, const uint32_t* __restrict__ start_bucket, const uint32_t* __restrict__ work_list,
-    TrackletStore out, int64_t* __restrict__ cnt) {
+    const SeedRec* __restrict__ work_list, TrackletStore out, int64_t* __restrict__ cnt) {
   __shared__ float sx[MAX_ROWS];
-  __shared__ int16_t sup[MAX_ROWS];
-  __shared__ uint8_t sdead[MAX_ROWS];
+  __shared__ int16_t sup[MAX_ROWS];          // up_row (R2)
+  __shared__ int16_t snu[MAX_ROWS];          // next live row above (n_rows if none)
+  __shared__ int16_t snd[MAX_ROWS];          // next live row below (-1 if none)
   __shared__ float snap[22][TC_THREADS];     // state after the last Update of the down pass (O4 step 5)
   if (cnt[CNT_ERROR] != 0) return;
   const int R = P.n_rows;
   const int tid = threadIdx.x;
-  for (int i = tid; i < R; i += blockDim.x) { sx[i] = T.row_x[i]; sup[i] = T.up_row[i]; sdead[i] = T.dead[i]; }
+  for (int i = tid; i < R; i += blockDim.x) {
+    sx[i] = T.row_x[i]; sup[i] = T.up_row[i];
+    int u = i + 1, d = i - 1;
+    while (u < R && T.dead[u]) ++u;
+    while (d >= 0 && T.dead[d]) --d;
+    snu[i] = (int16_t)u; snd[i] = (int16_t)d;
+  }
   __syncthreads();
   const int64_t nW = cnt[CNT_N_LONG];            // seeds on the work list (seedPrepare)
   const int64_t capT = out.capT;
@@ -174,7 +222,7 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
 
   KFState S;
   int phase = -1;                 // -1 wants a seed, -2 no seeds left, 0 chain fit, 1 up extrapolation, 2 down pass
-  int64_t t = 0;
+  uint32_t t = 0;
   int32_t* rowhit = nullptr;      // this tracklet's [n_rows] slice
   int r0 = 0, bsec = 0, rn = 0, rc = 0, lastw = 0, nhits = 0, miss = 0, snap_row = -1, rtop = 0;
   int32_t c_cur = -1;             // hit of the coming step if known (link / row hit), else -1 = search
@@ -187,17 +235,18 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
       if (j >= nW) {
         phase = -2;
       } else {
-        t = work_list[j];
-        const uint32_t h0 = start_pos[t];
-        const int b0 = (int)start_bucket[t];
-        r0 = b0 % R;
-        bsec = b0 - r0;
-        rowhit = out.rowhit + t * R;
-        c_cur = cup[h0];
+        const uint4* rp = reinterpret_cast<const uint4*>(work_list + j);
+        const uint4 a = __ldg(rp), b = __ldg(rp + 1);
+        t = a.x;
+        const uint32_t h0 = a.y;
+        c_cur = (int32_t)a.z;
+        r0 = (int)(a.w & 0xffu);
+        bsec = (int)(a.w >> 8) - r0;
+        rowhit = out.rowhit + (int64_t)t * R;
         rn = sup[r0];
-        const float2 a = syz[h0], c = syz[c_cur];
-        S.x = sx[r0]; S.y = a.x; S.z = a.y;
-        const float dx = sx[rn] - sx[r0], dy = c.x - a.x, dz = c.y - a.y;
+        const float y0 = __uint_as_float(b.x), z0 = __uint_as_float(b.y);
+        S.x = sx[r0]; S.y = y0; S.z = z0;
+        const float dx = sx[rn] - sx[r0], dy = __uint_as_float(b.z) - y0, dz = __uint_as_float(b.w) - z0;
         const float L = sqrtf(dx * dx + dy * dy);
         S.s = dy / L; S.t = dz / L; S.q = 0.0f;
         kfSetDiag(S, P.err2_y, P.err2_z, P);
@@ -205,22 +254,20 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
         rowhit[r0] = (int32_t)h0;
         last_c = (int32_t)h0;
         nhits = 1; rc = r0; lastw = r0; miss = 0; snap_row = -1;
-        out.sector[t] = bsec / R;
         phase = 0;
       }
     }
-    __syncwarp();
     if (__all_sync(0xffffffffu, phase == -2)) break;
 
     // ---- one step: early loads -> Propagate (search loads issued inside) -> candidate -> Update ----
     const bool act = phase >= 0;
     float ym = 0.0f, zm = 0.0f;
+    float2 mk = make_float2(0.0f, 0.0f);         // coordinates of the known hit: consumed only at the Update
     int32_t hnext = -1;
     GridDesc G;
     if (act) {
       if (c_cur >= 0) {
-        const float2 m = __ldg(syz + c_cur);
-        ym = m.x; zm = m.y;
+        mk = __ldg(syz + c_cur);
         if (phase == 0) hnext = __ldg(cup + c_cur);
       } else {
         G = desc[bsec + rn];
@@ -233,25 +280,23 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
     });
     int32_t c = c_cur;
     const bool known = okp && c >= 0 && phase == 2;
-    if (okp && phase == 0) rc = rn;
-    __syncwarp();
     if (okp && c < 0) c = searchFinish(sp, syz, s2o, ym, zm);
-    __syncwarp();
+    if (c_cur >= 0) { ym = mk.x; zm = mk.y; }
     bool oku = false;
     if (okp && c >= 0) oku = kfUpdate(S, ym, zm, P);
-    __syncwarp();
     if (!act) continue;
 
     // ---- bookkeeping and phase transitions ----
     bool end_phase = !okp || (c >= 0 && !oku);       // Propagate or Update refused: the pass ends here
     bool turn = false;
+    const int rb = rn;                               // the row of this step
+    if (okp && !known) rowhit[rb] = oku ? c : -1;    // rows beyond the final first/last row are never read
     if (phase == 0) {
+      if (okp) rc = rb;
       if (oku) {
-        for (int g = lastw + 1; g < rn; ++g) rowhit[g] = -1;
-        rowhit[rn] = c;
-        lastw = rn; last_c = c; ++nhits;
+        lastw = rb; last_c = c; ++nhits;
         c_cur = hnext;
-        rn = sup[rn];
+        rn = sup[rb];
         if (hnext == -1) end_phase = true;
       }
       if (end_phase) {
@@ -260,49 +305,42 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
           phase = -1;
         } else {
           phase = 1; miss = 0; c_cur = -1;
-          rn = rc + 1;
-          while (rn < R && sdead[rn]) ++rn;
+          rn = snu[rc];
           if (rn >= R) turn = true;
         }
       }
     } else if (phase == 1) {
       if (oku) {
-        for (int g = lastw + 1; g < rn; ++g) rowhit[g] = -1;
-        rowhit[rn] = c;
-        lastw = rn; last_c = c; ++nhits; miss = 0;
+        lastw = rb; last_c = c; ++nhits; miss = 0;
       } else if (!end_phase) {
         if (++miss > P.max_row_gap) end_phase = true;
       }
       if (!end_phase) {
-        ++rn;
-        while (rn < R && sdead[rn]) ++rn;
+        rn = snu[rb];
         if (rn >= R) end_phase = true;
       }
       if (end_phase) turn = true;
     } else {
       if (!end_phase) {
-        if (!known && (oku || rn < r0)) rowhit[rn] = oku ? c : -1;
         if (oku) {
-          ++nhits; snap_row = rn;
+          ++nhits; snap_row = rb;
           snap[0][tid] = S.x; snap[1][tid] = S.y; snap[2][tid] = S.z; snap[3][tid] = S.s; snap[4][tid] = S.t;
           snap[5][tid] = S.q; snap[6][tid] = S.chi2; snap[7][tid] = S.c00; snap[8][tid] = S.c10; snap[9][tid] = S.c11;
           snap[10][tid] = S.c20; snap[11][tid] = S.c21; snap[12][tid] = S.c22; snap[13][tid] = S.c30;
           snap[14][tid] = S.c31; snap[15][tid] = S.c32; snap[16][tid] = S.c33; snap[17][tid] = S.c40;
           snap[18][tid] = S.c41; snap[19][tid] = S.c42; snap[20][tid] = S.c43; snap[21][tid] = S.c44;
-          if (rn < r0) miss = 0;
-        } else if (rn < r0) {
+          if (rb < r0) miss = 0;
+        } else if (rb < r0) {
           if (++miss > P.max_row_gap) end_phase = true;
         }
       }
       if (!end_phase) {
-        --rn;
-        while (rn >= 0 && sdead[rn]) { if (rn < r0) rowhit[rn] = -1; --rn; }
+        rn = snd[rb];
         if (rn < 0) end_phase = true;
       }
       if (!end_phase) {           // pipeline: this step's hit was loaded a step ago; request the one after
         c_cur = c_nxt;
-        int r2 = rn - 1;
-        while (r2 >= 0 && sdead[r2]) --r2;
+        const int r2 = snd[rn];
         c_nxt = (r2 >= r0) ? rowhit[r2] : -1;
       } else {                    // O4 step 6: output = last snapshot
         if (snap_row < 0) {
@@ -325,9 +363,12 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
       rtop = lastw; rn = rtop;
       phase = 2; miss = 0; nhits = 0; snap_row = -1;
       c_cur = last_c;             // the hit on row rtop
-      int r2 = rn - 1;
-      while (r2 >= 0 && sdead[r2]) --r2;
+      const int r2 = snd[rn];
       c_nxt = (r2 >= r0) ? rowhit[r2] : -1;
+    } else if (phase >= 0) {      // dead rows stepped over (R23) hold no hit
+      const int lo = min(rb, rn), hi = max(rb, rn);
+      if (hi - lo > 1)
+        for (int g = lo + 1; g < hi; ++g) rowhit[g] = -1;
     }
   }
 }
