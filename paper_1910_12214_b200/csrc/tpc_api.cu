@@ -72,6 +72,7 @@ struct tpcHandle {
   // pools of tpcRunHost
   void* pool[16] = {};
   size_t pool_bytes[16] = {};
+  int64_t hint_T = 0, hint_K = 0, hint_C = 0;   // capacities the last tpcRunHost needed (+ head-room)
 };
 
 namespace {
@@ -437,7 +438,9 @@ extern "C" int tpcRunHost(tpcHandle* h, int64_t N, const uint32_t* row_offset, c
   TPC_CUDA(h, cudaSetDevice(h->device));
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const int nb = h->P.n_buckets;
-  int64_t capT = std::max<int64_t>(4096, N / 8), capK = capT, capC = std::max<int64_t>(N, 1);
+  int64_t capT = std::max<int64_t>(std::max<int64_t>(4096, N / 8), h->hint_T);
+  int64_t capK = std::max<int64_t>(std::max<int64_t>(4096, N / 64), h->hint_K);
+  int64_t capC = std::max<int64_t>(std::max<int64_t>(N / 2, 1), h->hint_C);
   void *d_off, *d_y, *d_z;
   int rc;
   if ((rc = poolGet(h, 0, 4 * (size_t)(nb + 1), &d_off)) || (rc = poolGet(h, 1, 4 * (size_t)N, &d_y)) ||
@@ -469,10 +472,14 @@ extern "C" int tpcRunHost(tpcHandle* h, int64_t N, const uint32_t* row_offset, c
     if ((rc = tpcRun(h, &in, &od, capT, ws, h->pool_bytes[3], st))) return rc;
     if ((rc = tpcGetRunStatus(h, status))) return rc;
     if (status->status != TPC_ERR_CAPACITY || attempt >= 2) break;
-    capT = std::max(capT, status->n_start_hits);
-    capK = std::max(capK, status->n_tracks);
-    capC = std::max(capC, status->n_track_clusters);
+    capT = std::max(capT, status->n_start_hits + status->n_start_hits / 16);
+    capK = std::max(capK, status->n_tracks + status->n_tracks / 16);
+    capC = std::max(capC, status->n_track_clusters + status->n_track_clusters / 16);
   }
+  // the next call on similar data gets it right the first time
+  h->hint_T = std::max(h->hint_T, status->n_start_hits + status->n_start_hits / 16);
+  h->hint_K = std::max(h->hint_K, status->n_tracks + status->n_tracks / 16);
+  h->hint_C = std::max(h->hint_C, status->n_track_clusters + status->n_track_clusters / 16);
   if (status->status != TPC_OK) return TPC_OK;   // data-dependent error: reported through *status
   const int64_t nt = std::min<int64_t>(status->n_tracks, oh->cap_tracks);
   const int64_t nc = status->n_track_clusters;
