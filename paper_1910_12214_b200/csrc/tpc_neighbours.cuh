@@ -22,9 +22,15 @@ namespace tpc {
 
 constexpr int NF_THREADS = 128;
 constexpr int NF_REGION = 640;     // staged candidates per side
-constexpr int NF_LIST = 32;        // window candidates kept per thread and side (<= 32: packed item code)
+#ifndef NF_LIST_
+#define NF_LIST_ 32
+#endif
+#ifndef NF_ITEMS_
+#define NF_ITEMS_ 512
+#endif
+constexpr int NF_LIST = NF_LIST_;  // window candidates kept per thread and side (<= 32: packed item code)
 constexpr int NF_UB = 4;          // u's per item (register blocking of the pair loop)
-constexpr int NF_ITEMS = 512;      // items per CTA and round
+constexpr int NF_ITEMS = NF_ITEMS_; // items per CTA and round
 constexpr int NF_ROWS = 6;         // cell rows of a window whose ranges are staged (more: slow path)
 
 struct RowTables {
@@ -120,7 +126,8 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
   __shared__ uint16_t it[NF_ITEMS], it_d[NF_ITEMS * NF_UB];
   __shared__ float it_dev[NF_ITEMS * NF_UB];
   __shared__ uint8_t snD[NF_THREADS], snU[NF_THREADS];
-  __shared__ ushort2 srow[NF_ROWS * NF_THREADS];
+  ushort2* srow = reinterpret_cast<ushort2*>(it_dev);   // cell-row ranges: only live while the lists are built
+  static_assert(sizeof(float) * NF_ITEMS * NF_UB >= sizeof(ushort2) * NF_ROWS * NF_THREADS, "srow aliases it_dev");
   __shared__ float red[2][NF_THREADS / 32];
   __shared__ uint32_t sscan[33];
   __shared__ int sm_b;

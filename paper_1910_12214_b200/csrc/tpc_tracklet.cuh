@@ -15,6 +15,9 @@ constexpr int TC_THREADS = 128;
 #define TC_MIN_BLOCKS 5
 #endif
 constexpr int MAX_ROWS = 256;
+#ifndef TC_HEADS
+#define TC_HEADS 6                  // candidates per cell row loaded and evaluated without a loop
+#endif
 
 // Search (O4): nearest cluster of the bucket inside the road around the predicted (y,z); key (d2, orig index).
 // Split in two so that the first grid loads are in flight while Propagate finishes the covariance transport:
@@ -75,7 +78,7 @@ __device__ __noinline__ int32_t searchExact(const SearchPre& sp, const float2* _
 }
 
 // returns the sorted position of the best cluster or -1; its coordinates in (ym, zm).
-// The heads of the two prefetched cell rows (up to 4 + 4 candidates, every load in flight before the first test:
+// The heads of the two prefetched cell rows (up to TC_HEADS + TC_HEADS candidates, every load in flight before the first test:
 // one memory latency per search instead of one per candidate) are evaluated without branches; unused slots hold
 // a point outside every window.  Longer rows and further cell rows are scanned by loops.
 __device__ __forceinline__ int32_t searchFinish(const SearchPre& sp, const float2* __restrict__ syz,
@@ -84,11 +87,11 @@ __device__ __forceinline__ int32_t searchFinish(const SearchPre& sp, const float
   const uint32_t nA = sp.kA1 - sp.kA0;
   const uint32_t nB = sp.bz1 > sp.bz0 ? sp.kB1 - sp.kB0 : 0u;
   const float2 far = make_float2(3.0e38f, 3.0e38f);
-  float2 ca[4], cb[4];
+  float2 ca[TC_HEADS], cb[TC_HEADS];
 #pragma unroll
-  for (int i = 0; i < 4; ++i) ca[i] = i < nA ? __ldg(syz + sp.kA0 + i) : far;
+  for (int i = 0; i < TC_HEADS; ++i) ca[i] = i < nA ? __ldg(syz + sp.kA0 + i) : far;
 #pragma unroll
-  for (int i = 0; i < 4; ++i) cb[i] = i < nB ? __ldg(syz + sp.kB0 + i) : far;
+  for (int i = 0; i < TC_HEADS; ++i) cb[i] = i < nB ? __ldg(syz + sp.kB0 + i) : far;
   float bestd = __int_as_float(0x7f800000);     // d2 of a candidate inside the road is finite
   int32_t best = -1;
   bool tie = false;
@@ -104,9 +107,9 @@ __device__ __forceinline__ int32_t searchFinish(const SearchPre& sp, const float
     zm = better ? c.y : zm;
   };
 #pragma unroll
-  for (int i = 0; i < 4; ++i) eval(ca[i], sp.kA0 + i);
+  for (int i = 0; i < TC_HEADS; ++i) eval(ca[i], sp.kA0 + i);
 #pragma unroll
-  for (int i = 0; i < 4; ++i) eval(cb[i], sp.kB0 + i);
+  for (int i = 0; i < TC_HEADS; ++i) eval(cb[i], sp.kB0 + i);
   auto scan = [&](uint32_t k0, uint32_t k1) {      // two independent loads per trip
     for (uint32_t k = k0; k < k1; k += 2) {
       const bool two = k + 1 < k1;
@@ -116,8 +119,8 @@ __device__ __forceinline__ int32_t searchFinish(const SearchPre& sp, const float
       eval(c, k + 1);
     }
   };
-  if (nA > 4) scan(sp.kA0 + 4, sp.kA1);
-  if (nB > 4) scan(sp.kB0 + 4, sp.kB1);
+  if (nA > TC_HEADS) scan(sp.kA0 + TC_HEADS, sp.kA1);
+  if (nB > TC_HEADS) scan(sp.kB0 + TC_HEADS, sp.kB1);
   for (int bz = sp.bz0 + 2; bz <= sp.bz1; ++bz) {   // roads wider than two cell rows: rare
     const uint32_t* r = sp.cs + bz * sp.ny;
     scan(__ldg(r), __ldg(r + sp.span));
