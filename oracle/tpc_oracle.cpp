@@ -141,6 +141,10 @@ struct orcResult {
   std::vector<int32_t> tr_id, tr_sector, tr_first, tr_last, tr_ncl;
   std::vector<double> tr_x, tr_par, tr_cov, tr_chi2;
   std::vector<uint32_t> tr_cl_offset, tr_cl_index;
+  // O6 refit (NEXT-2): status 1 = refitted, 0 = failed; inner = state at the first kept cluster (down pass),
+  // outer = state at the last kept cluster (up pass)
+  std::vector<int32_t> rf_status;
+  std::vector<double> rf_x_in, rf_par_in, rf_cov_in, rf_chi2, rf_x_out, rf_par_out, rf_cov_out;
 };
 
 namespace {
@@ -322,6 +326,56 @@ struct Tracker {
     st.C[tri(2, 2)] = (Real)P.init_var_s; st.C[tri(3, 3)] = (Real)P.init_var_t; st.C[tri(4, 4)] = (Real)P.init_var_q;
   }
 
+  // ---- O6 refit of a selected track over its kept clusters (O6; readings R28..R30) --------
+  // up pass: state from the first two kept clusters as in O4 step 1, Propagate + Update through the others in
+  // ascending row -> outer state; turn (R17); down pass over all kept clusters -> inner state, chi2.
+  bool refit(const uint32_t* cl, int n, State<Real>& inner, State<Real>& outer) const {
+    const Real b = (Real)(0.00299792458 * (double)g.bz_tesla);
+    const Real msp = (Real)P.max_sinphi, e2y = (Real)P.err2_y, e2z = (Real)P.err2_z;
+    if (n < 2) return false;
+    State<Real> st{};
+    const uint32_t c0 = cl[0], c1 = cl[1];
+    st.x = X[rowOf[c0]]; st.y = Y[c0]; st.z = Z[c0];
+    {
+      const Real dx = X[rowOf[c1]] - X[rowOf[c0]], dy = Y[c1] - Y[c0], dz = Z[c1] - Z[c0];
+      const Real L = std::sqrt(dx * dx + dy * dy);
+      st.s = dy / L; st.t = dz / L; st.q = 0;
+    }
+    setDiag(st, e2y, e2z);
+    st.chi2 = 0;
+    for (int i = 1; i < n; ++i) {
+      if (!propagate(st, X[rowOf[cl[i]]], b, msp)) return false;
+      if (!update(st, Y[cl[i]], Z[cl[i]], e2y, e2z)) return false;
+    }
+    outer = st;
+    setDiag(st, (Real)P.turn_var_scale * e2y, (Real)P.turn_var_scale * e2z);
+    st.chi2 = 0;
+    for (int i = n - 1; i >= 0; --i) {
+      if (!propagate(st, X[rowOf[cl[i]]], b, msp)) return false;
+      if (!update(st, Y[cl[i]], Z[cl[i]], e2y, e2z)) return false;
+    }
+    inner = st;
+    return true;
+  }
+
+  void refitAll() {
+    const int64_t nt = (int64_t)res.tr_id.size();
+    res.rf_status.assign(nt, 0);
+    res.rf_x_in.assign(nt, 0); res.rf_chi2.assign(nt, 0); res.rf_x_out.assign(nt, 0);
+    res.rf_par_in.assign((size_t)nt * 5, 0); res.rf_par_out.assign((size_t)nt * 5, 0);
+    res.rf_cov_in.assign((size_t)nt * 15, 0); res.rf_cov_out.assign((size_t)nt * 15, 0);
+    for (int64_t k = 0; k < nt; ++k) {
+      const uint32_t lo = res.tr_cl_offset[k], hi = res.tr_cl_offset[k + 1];
+      State<Real> in{}, out{};
+      if (!refit(res.tr_cl_index.data() + lo, (int)(hi - lo), in, out)) continue;
+      res.rf_status[k] = 1;
+      res.rf_x_in[k] = (double)in.x; res.rf_chi2[k] = (double)in.chi2; res.rf_x_out[k] = (double)out.x;
+      const Real pi[5] = {in.y, in.z, in.s, in.t, in.q}, po[5] = {out.y, out.z, out.s, out.t, out.q};
+      for (int i = 0; i < 5; ++i) { res.rf_par_in[(size_t)k * 5 + i] = (double)pi[i]; res.rf_par_out[(size_t)k * 5 + i] = (double)po[i]; }
+      for (int i = 0; i < 15; ++i) { res.rf_cov_in[(size_t)k * 15 + i] = (double)in.C[i]; res.rf_cov_out[(size_t)k * 15 + i] = (double)out.C[i]; }
+    }
+  }
+
   void construct(uint32_t h0, Tracklet<Real>& T) const {
     const Real b = (Real)(0.00299792458 * (double)g.bz_tesla);
     const Real msp = (Real)P.max_sinphi, e2y = (Real)P.err2_y, e2z = (Real)P.err2_z;
@@ -482,8 +536,9 @@ int orcRun(const orcGeometry* g, const orcParams* p, int64_t n, const uint32_t* 
   orcResult* r = new orcResult();
   r->n = n; r->n_sectors = g->n_sectors; r->n_rows = g->n_rows;
   r->fp64 = (flags & ORC_FP64) != 0; r->brute = (flags & ORC_BRUTE_FORCE) != 0;
-  if (r->fp64) { Tracker<double> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); }
-  else { Tracker<float> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); }
+  const bool rf = (flags & ORC_REFIT) != 0;
+  if (r->fp64) { Tracker<double> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); if (rf) T.refitAll(); }
+  else { Tracker<float> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); if (rf) T.refitAll(); }
   *out = r;
   return ORC_OK;
 }
@@ -501,6 +556,55 @@ void orcGetLinks(const orcResult* r, int32_t* ur, int32_t* dr, int32_t* u, int32
   copyOut(ur, r->up_raw); copyOut(dr, r->dn_raw); copyOut(u, r->up); copyOut(d, r->dn);
 }
 void orcGetStartHits(const orcResult* r, uint32_t* sh) { copyOut(sh, r->start_hits); }
+void orcGetRefit(const orcResult* r, int32_t* status, double* x_in, double* par_in, double* cov_in, double* chi2,
+                 double* x_out, double* par_out, double* cov_out) {
+  copyOut(status, r->rf_status); copyOut(x_in, r->rf_x_in); copyOut(par_in, r->rf_par_in); copyOut(cov_in, r->rf_cov_in);
+  copyOut(chi2, r->rf_chi2); copyOut(x_out, r->rf_x_out); copyOut(par_out, r->rf_par_out); copyOut(cov_out, r->rf_cov_out);
+}
+
+}  // extern "C"
+
+namespace {
+template <typename Real>
+int refitPoints(const orcGeometry* g, const orcParams* p, int n, const int32_t* rows, const double* y, const double* z,
+                double* in, double* out) {
+  // one sector, the given clusters (ascending rows, any number per row) as the only input
+  std::vector<uint32_t> off((size_t)g->n_rows + 1, 0);
+  for (int i = 0; i < n; ++i) off[rows[i] + 1]++;
+  for (int r = 0; r < g->n_rows; ++r) off[r + 1] += off[r];
+  std::vector<float> yf(n), zf(n);
+  for (int i = 0; i < n; ++i) { yf[i] = (float)y[i]; zf[i] = (float)z[i]; }
+  orcGeometry g1 = *g; g1.n_sectors = 1;
+  orcResult res;
+  Tracker<Real> T(g1, *p, n, off.data(), yf.data(), zf.data(), true, res);
+  for (int i = 0; i < n; ++i) { T.Y[i] = (Real)y[i]; T.Z[i] = (Real)z[i]; }     // binary64 inputs stay exact
+  std::vector<uint32_t> cl(n);
+  for (int i = 0; i < n; ++i) cl[i] = (uint32_t)i;
+  State<Real> si{}, so{};
+  if (!T.refit(cl.data(), n, si, so)) return 0;
+  const State<Real>* st[2] = {&si, &so};
+  double* dst[2] = {in, out};
+  for (int k = 0; k < 2; ++k) {     // 22 doubles: x, y, z, s, t, q, C[15], chi2
+    double* d = dst[k];
+    d[0] = (double)st[k]->x; d[1] = (double)st[k]->y; d[2] = (double)st[k]->z; d[3] = (double)st[k]->s;
+    d[4] = (double)st[k]->t; d[5] = (double)st[k]->q;
+    for (int i = 0; i < 15; ++i) d[6 + i] = (double)st[k]->C[i];
+    d[21] = (double)st[k]->chi2;
+  }
+  return 1;
+}
+}  // namespace
+
+extern "C" {
+
+int orcRefitPoints(const orcGeometry* g, const orcParams* p, int n, const int32_t* rows, const double* y, const double* z,
+                   int fp64, double* inner22, double* outer22) {
+  if (!g || !p || n < 2 || !rows || !y || !z || !inner22 || !outer22) return 0;
+  for (int i = 0; i < n; ++i)
+    if (rows[i] < 0 || rows[i] >= g->n_rows || (i > 0 && rows[i] < rows[i - 1])) return 0;
+  return fp64 ? refitPoints<double>(g, p, n, rows, y, z, inner22, outer22)
+              : refitPoints<float>(g, p, n, rows, y, z, inner22, outer22);
+}
 void orcGetTracklets(const orcResult* r, int32_t* status, int32_t* nhits, int32_t* first, int32_t* last, int32_t* rowhit,
                      double* x, double* par, double* cov, double* chi2) {
   copyOut(status, r->tl_status); copyOut(nhits, r->tl_nhits); copyOut(first, r->tl_first); copyOut(last, r->tl_last);

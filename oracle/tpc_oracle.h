@@ -44,7 +44,7 @@ typedef struct {
 typedef struct orcResult orcResult;
 
 enum { ORC_OK = 0, ORC_ERR_INVALID_ARG = -1, ORC_ERR_UNSORTED_OFFSETS = -2 };
-enum { ORC_BRUTE_FORCE = 1, ORC_FP64 = 2 };
+enum { ORC_BRUTE_FORCE = 1, ORC_FP64 = 2, ORC_REFIT = 4 };
 
 void orcDefaultParams(orcParams* p);
 
@@ -76,6 +76,17 @@ void orcGetTracklets(const orcResult*, int32_t* status, int32_t* nhits, int32_t*
 void orcGetTracks(const orcResult*, int32_t* tracklet_id, int32_t* sector, int32_t* first_row, int32_t* last_row,
                   int32_t* ncl, double* x, double* par, double* cov, double* chi2, uint32_t* cl_offset,
                   uint32_t* cl_index);
+
+/* O6 (NEXT-2 of SURVEY.md 8(f), DESIGN.md section 3 "O6"): refit of every selected track over its kept clusters,
+ * only when orcRun was called with ORC_REFIT.  status [n_tracks] 1 = refitted, 0 = Propagate / Update refused;
+ * *_in = state at the first kept cluster after the down pass (chi2 of that pass), *_out = state at the last kept
+ * cluster after the up pass.  par [n_tracks*5], cov [n_tracks*15] track-major.  Pins: tests/test_oracle_refit.py. */
+void orcGetRefit(const orcResult*, int32_t* status, double* x_in, double* par_in, double* cov_in, double* chi2,
+                 double* x_out, double* par_out, double* cov_out);
+/* The same refit on n given clusters of one sector (rows ascending, binary64 coordinates kept exact when fp64):
+ * inner22 / outer22 = x, y, z, s, t, q, C[15], chi2.  Returns 1 on success. */
+int orcRefitPoints(const orcGeometry* g, const orcParams* p, int n, const int32_t* rows, const double* y, const double* z,
+                   int fp64, double* inner22, double* outer22);
 
 /* Single KF steps for the pins.  state = {x, y, z, s, t, q}, cov = 15 lower-triangle elements
  * (00,10,11,20,21,22,30,...,44), both in/out as doubles (rounded to binary32 first unless fp64).

@@ -19,6 +19,7 @@ _LIB = os.path.join(_HERE, "libtpcoracle.so")
 
 BRUTE_FORCE = 1
 FP64 = 2
+REFIT = 4
 
 
 def build(force: bool = False) -> str:
@@ -68,6 +69,10 @@ def _load():
         L.orcGetTracks.argtypes = [vp] * 12
         for f in ("orcGetGrid", "orcGetLinks", "orcGetStartHits", "orcGetTracklets", "orcGetTracks"):
             getattr(L, f).restype = None
+        L.orcGetRefit.argtypes = [vp] * 9
+        L.orcGetRefit.restype = None
+        L.orcRefitPoints.argtypes = [ctypes.POINTER(Geometry), ctypes.POINTER(Params), ci, vp, vp, vp, ci, vp, vp]
+        L.orcRefitPoints.restype = ci
         L.orcPropagate.argtypes = [vp, vp, dbl, dbl, dbl, ci]
         L.orcPropagate.restype = ci
         L.orcUpdate.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, ci]
@@ -113,6 +118,15 @@ class OracleResult:
     trk_chi2: np.ndarray
     trk_cl_offset: np.ndarray
     trk_cl_index: np.ndarray
+    # O6 refit (only with refit=True): status, inner state (down pass), outer state (up pass)
+    rf_status: np.ndarray | None = None
+    rf_x_in: np.ndarray | None = None
+    rf_par_in: np.ndarray | None = None     # [n_tracks, 5]
+    rf_cov_in: np.ndarray | None = None     # [n_tracks, 15]
+    rf_chi2: np.ndarray | None = None
+    rf_x_out: np.ndarray | None = None
+    rf_par_out: np.ndarray | None = None
+    rf_cov_out: np.ndarray | None = None
 
     @property
     def n_tracks(self) -> int:
@@ -124,7 +138,7 @@ def _ptr(a):
 
 
 def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool = False,
-        stages_only: bool = False) -> OracleResult:
+        stages_only: bool = False, refit: bool = False) -> OracleResult:
     """Run O1..O5 on an Event-like object (fields n_sectors, n_rows, row_x, row_dead, bz_tesla,
     tan_half_sector, z_min, z_max, row_offset, y, z; numpy arrays)."""
     L = _load()
@@ -139,7 +153,8 @@ def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool 
     n = int(y.shape[0])
     h = ctypes.c_void_p()
     rc = L.orcRun(ctypes.byref(g), ctypes.byref(p), n, off.ctypes.data, _ptr(y), _ptr(z),
-                  (BRUTE_FORCE if brute_force else 0) | (FP64 if fp64 else 0), ctypes.byref(h))
+                  (BRUTE_FORCE if brute_force else 0) | (FP64 if fp64 else 0) | (REFIT if refit else 0),
+                  ctypes.byref(h))
     if rc != 0:
         raise ValueError(f"orcRun failed with {rc}")
     try:
@@ -165,10 +180,18 @@ def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool 
         koff, kidx = np.zeros(nt + 1, np.uint32), np.zeros(ntc, np.uint32)
         L.orcGetTracks(h, _ptr(kid), _ptr(ks), _ptr(kf), _ptr(kl), _ptr(kn), _ptr(kx), _ptr(kpar), _ptr(kcov),
                        _ptr(kchi), _ptr(koff), _ptr(kidx))
+        rf = {}
+        if refit:
+            rst = np.zeros(nt, np.int32)
+            rxi, rchi, rxo = np.zeros(nt), np.zeros(nt), np.zeros(nt)
+            rpi, rpo, rci, rco = np.zeros((nt, 5)), np.zeros((nt, 5)), np.zeros((nt, 15)), np.zeros((nt, 15))
+            L.orcGetRefit(h, _ptr(rst), _ptr(rxi), _ptr(rpi), _ptr(rci), _ptr(rchi), _ptr(rxo), _ptr(rpo), _ptr(rco))
+            rf = dict(rf_status=rst, rf_x_in=rxi, rf_par_in=rpi, rf_cov_in=rci, rf_chi2=rchi, rf_x_out=rxo, rf_par_out=rpo,
+                      rf_cov_out=rco)
     finally:
         L.orcFree(h)
     return OracleResult(n, s2o, cell, ncell, ur, dr, u, d, sh, st, nh, fr, lr, rh, tx, tpar, tcov, tchi, kid, ks, kf, kl,
-                        kn, kx, kpar, kcov, kchi, koff, kidx)
+                        kn, kx, kpar, kcov, kchi, koff, kidx, **rf)
 
 
 def propagate(state, cov, x_new, bz_tesla=0.5, max_sinphi=0.98, fp64=True):
@@ -187,3 +210,18 @@ def update(state, cov, chi2, ym, zm, err2_y=0.01, err2_z=0.01, fp64=True):
     ok = _load().orcUpdate(s.ctypes.data, c.ctypes.data, x2.ctypes.data, float(ym), float(zm), float(err2_y),
                            float(err2_z), int(fp64))
     return bool(ok), s, c, float(x2[0])
+
+
+def refit_points(rows, y, z, row_x, bz_tesla=0.5, params: Params | None = None, fp64=True):
+    """O6 refit of the given clusters (ascending rows) of one sector.  Returns (ok, inner, outer), each state an
+    array of 22 doubles: x, y, z, s, t, q, C[15], chi2."""
+    L = _load()
+    p = params if params is not None else default_params()
+    row_x = np.ascontiguousarray(row_x, np.float32)
+    g = Geometry(1, len(row_x), row_x.ctypes.data, None, bz_tesla, float(np.tan(np.radians(10.0))), -250.0, 250.0)
+    rows = np.ascontiguousarray(rows, np.int32)
+    yy, zz = np.ascontiguousarray(y, np.float64), np.ascontiguousarray(z, np.float64)
+    inner, outer = np.zeros(22), np.zeros(22)
+    ok = L.orcRefitPoints(ctypes.byref(g), ctypes.byref(p), len(rows), rows.ctypes.data, yy.ctypes.data, zz.ctypes.data,
+                          int(fp64), inner.ctypes.data, outer.ctypes.data)
+    return bool(ok), inner, outer
