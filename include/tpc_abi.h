@@ -8,6 +8,7 @@
  *   a3 cleaner/start hits  reciprocal links only; heads of link chains
  *   a4 tracklet constructor link-chain fit + row-by-row helix Kalman extrapolation (5 params, 15 cov, fp32)
  *   a5 tracklet selector   shared clusters go to the longest / lowest-chi2 tracklet
+ *   a6 refit (optional)    Kalman refit of every selected track over its kept clusters: inner and outer state
  * The formulas, constants and tie-breaks are DESIGN.md section 3 (readings R0..R27 of SURVEY.md 8(c)).
  *
  * Conventions
@@ -113,6 +114,16 @@ typedef struct {
   float* tl_par;                /* [cap_tracklets][5] (tracklet-major) */
   float* tl_cov;                /* [cap_tracklets][15] */
   float* tl_chi2;               /* [cap_tracklets] */
+  /* optional O6 refit of the selected tracks over their kept clusters (DESIGN.md section 3 "O6"; the paper names a
+   * track refit at PAPER.md L11 / L92).  All NULL = no refit; otherwise ALL eight must be given.  Never changes trk_*. */
+  int32_t* trk_rf_status;       /* [cap_tracks] 1 = refitted, 0 = a Propagate / Update was refused (outputs zero) */
+  float* trk_rf_x_in;           /* [cap_tracks] x of the first kept cluster: reference plane of the inner state */
+  float* trk_rf_par_in;         /* [5][cap_tracks] inner state (after the down pass) */
+  float* trk_rf_cov_in;         /* [15][cap_tracks] */
+  float* trk_rf_chi2;           /* [cap_tracks] chi2 of the down pass, ndf = 2 ncl - 5 */
+  float* trk_rf_x_out;          /* [cap_tracks] x of the last kept cluster: reference plane of the outer state */
+  float* trk_rf_par_out;        /* [5][cap_tracks] outer state (after the up pass) */
+  float* trk_rf_cov_out;        /* [15][cap_tracks] */
 } tpcTracks;
 
 /* Filled by tpcGetRunStatus after the stream has drained. */
@@ -128,7 +139,7 @@ typedef struct {
   int64_t n_cells;              /* grid cells over all (sector,row) */
   float stage_ms[8];            /* per-stage device times of the last run when profiling is on (else 0):
                                    0 grid, 1 neighbour finder, 2 cleaner+start hits, 3 constructor, 4 selector,
-                                   5 optional exports, 6 total, 7 unused */
+                                   5 optional exports and refit, 6 total, 7 refit alone */
 } tpcRunStatus;
 
 int tpcDefaultParams(tpcParams* p);

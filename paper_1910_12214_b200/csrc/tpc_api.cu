@@ -18,6 +18,7 @@
 #include "tpc_kalman.cuh"
 #include "tpc_tracklet.cuh"
 #include "tpc_select.cuh"
+#include "tpc_refit.cuh"
 
 using namespace tpc;
 
@@ -61,7 +62,7 @@ struct tpcHandle {
   int64_t* d_cnt = nullptr;        // CNT_COUNT counters + 1 slot for the packed selector total
   int64_t* h_cnt = nullptr;        // pinned copy
   cudaEvent_t ev_done = nullptr;
-  cudaEvent_t ev_stage[7] = {};
+  cudaEvent_t ev_stage[9] = {};    // 0..6 stage boundaries, 7/8 around the optional refit
   int profiling = 0;
   int launches = 0;
   int tc_grid = 148;               // persistent grid of the tracklet constructor: SMs x resident blocks
@@ -206,7 +207,7 @@ int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cud
             cudaMalloc(&h->d_cnt, 8 * (CNT_COUNT + 1)) == cudaSuccess &&
             cudaMallocHost(&h->h_cnt, 8 * (CNT_COUNT + 1)) == cudaSuccess &&
             cudaEventCreate(&h->ev_done) == cudaSuccess;
-  for (int i = 0; ok && i < 7; ++i) ok = cudaEventCreate(&h->ev_stage[i]) == cudaSuccess;
+  for (int i = 0; ok && i < 9; ++i) ok = cudaEventCreate(&h->ev_stage[i]) == cudaSuccess;
   ok = ok && cudaMemcpy(h->d_row_x, g->row_x, 4 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
        cudaMemcpy(h->d_up, up.data(), 2 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
        cudaMemcpy(h->d_dn, dn.data(), 2 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
@@ -231,7 +232,7 @@ int tpcDestroy(tpcHandle* h) {
   cudaFree(h->d_row_x); cudaFree(h->d_up); cudaFree(h->d_dn); cudaFree(h->d_dead); cudaFree(h->d_cnt);
   if (h->h_cnt) cudaFreeHost(h->h_cnt);
   if (h->ev_done) cudaEventDestroy(h->ev_done);
-  for (int i = 0; i < 7; ++i) if (h->ev_stage[i]) cudaEventDestroy(h->ev_stage[i]);
+  for (int i = 0; i < 9; ++i) if (h->ev_stage[i]) cudaEventDestroy(h->ev_stage[i]);
   for (int i = 0; i < 16; ++i) if (h->pool[i]) cudaFree(h->pool[i]);
   delete h;
   return TPC_OK;
@@ -264,6 +265,10 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
                               !out->trk_ncl || !out->trk_x || !out->trk_par || !out->trk_cov || !out->trk_chi2))
     return TPC_ERR_INVALID_ARG;
   if (out->cap_track_clusters > 0 && !out->trk_cl_index) return TPC_ERR_INVALID_ARG;
+  const int n_rf = (out->trk_rf_status != nullptr) + (out->trk_rf_x_in != nullptr) + (out->trk_rf_par_in != nullptr) +
+                   (out->trk_rf_cov_in != nullptr) + (out->trk_rf_chi2 != nullptr) + (out->trk_rf_x_out != nullptr) +
+                   (out->trk_rf_par_out != nullptr) + (out->trk_rf_cov_out != nullptr);
+  if (n_rf != 0 && n_rf != 8) return TPC_ERR_INVALID_ARG;      // the refit outputs come all or none
   if (!workspace || ((uintptr_t)workspace % ALIGN) != 0) return TPC_ERR_INVALID_ARG;
   const Workspace w = layout(h, N, capT, (char*)workspace);
   if (workspace_bytes < w.bytes) return TPC_ERR_WORKSPACE_TOO_SMALL;
@@ -348,6 +353,15 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   }
   finalize<<<1, 32, 0, st>>>(sel_total, to, capT, cnt); ++L;
   stage(5);
+  // ---- a6 optional refit of the selected tracks (O6) ------------------------------------------------
+  stage(7);
+  if (n_rf == 8 && N > 0 && out->cap_tracks > 0) {
+    const RefitOut rf{out->trk_rf_status, out->trk_rf_x_in, out->trk_rf_par_in, out->trk_rf_cov_in, out->trk_rf_chi2,
+                      out->trk_rf_x_out, out->trk_rf_par_out, out->trk_rf_cov_out};
+    const int64_t nk = std::min<int64_t>(out->cap_tracks, capT);
+    refitTracks<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(in->row_offset, in->y, in->z, P, T, to, rf, cnt); ++L;
+  }
+  stage(8);
   // ---- optional per-stage exports -----------------------------------------------------------------
   if (N > 0 && (out->link_up_raw || out->link_dn_raw || out->link_up || out->link_dn)) {
     exportLinks<<<gN256, 256, 0, st>>>(N, w.s2o, w.lup, w.ldn, w.cup, w.cdn, out->link_up_raw, out->link_dn_raw,
@@ -391,6 +405,7 @@ int tpcGetRunStatus(tpcHandle* h, tpcRunStatus* out) {
     }
     float ms = 0;
     if (cudaEventElapsedTime(&ms, h->ev_stage[0], h->ev_stage[6]) == cudaSuccess) out->stage_ms[6] = ms;
+    if (cudaEventElapsedTime(&ms, h->ev_stage[7], h->ev_stage[8]) == cudaSuccess) out->stage_ms[7] = ms;
   }
   return TPC_OK;
 }
@@ -432,7 +447,9 @@ extern "C" int tpcRunHost(tpcHandle* h, int64_t N, const uint32_t* row_offset, c
                           tpcTracks* oh, tpcRunStatus* status, void* cuda_stream) {
   if (!h || !row_offset || !oh || !status || N < 0 || N >= (1ll << 31) || (N > 0 && (!y || !z))) return TPC_ERR_INVALID_ARG;
   if (oh->link_up_raw || oh->link_dn_raw || oh->link_up || oh->link_dn || oh->start_hits || oh->tl_status || oh->tl_nhits ||
-      oh->tl_first_row || oh->tl_last_row || oh->tl_rowhit || oh->tl_x || oh->tl_par || oh->tl_cov || oh->tl_chi2)
+      oh->tl_first_row || oh->tl_last_row || oh->tl_rowhit || oh->tl_x || oh->tl_par || oh->tl_cov || oh->tl_chi2 ||
+      oh->trk_rf_status || oh->trk_rf_x_in || oh->trk_rf_par_in || oh->trk_rf_cov_in || oh->trk_rf_chi2 || oh->trk_rf_x_out ||
+      oh->trk_rf_par_out || oh->trk_rf_cov_out)
     return TPC_ERR_INVALID_ARG;
   if (!oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0) return TPC_ERR_INVALID_ARG;
   TPC_CUDA(h, cudaSetDevice(h->device));

@@ -47,11 +47,13 @@ _TRK_PTRS = ("trk_tracklet", "trk_sector", "trk_first_row", "trk_last_row", "trk
              "trk_chi2", "trk_cl_offset", "trk_cl_index")
 _STAGE_PTRS = ("link_up_raw", "link_dn_raw", "link_up", "link_dn", "start_hits", "tl_status", "tl_nhits",
                "tl_first_row", "tl_last_row", "tl_rowhit", "tl_x", "tl_par", "tl_cov", "tl_chi2")
+_REFIT_PTRS = ("trk_rf_status", "trk_rf_x_in", "trk_rf_par_in", "trk_rf_cov_in", "trk_rf_chi2", "trk_rf_x_out",
+               "trk_rf_par_out", "trk_rf_cov_out")
 
 
 class tpcTracks(ctypes.Structure):
     _fields_ = [("cap_tracks", c_int64), ("cap_track_clusters", c_int64)] + \
-               [(n, c_void_p) for n in _TRK_PTRS + _STAGE_PTRS]
+               [(n, c_void_p) for n in _TRK_PTRS + _STAGE_PTRS + _REFIT_PTRS]
 
 
 class tpcRunStatus(ctypes.Structure):
@@ -225,7 +227,7 @@ class TpcTracker:
         z = t.from_numpy(np.ascontiguousarray(ev.z, np.float32)).to(self.device)
         return off, y, z
 
-    def _ensure(self, n, capT, capK, capC, stages):
+    def _ensure(self, n, capT, capK, capC, stages, refit=False):
         t = self.torch
         need = tpcWorkspaceBytes(self.handle, n, capT)
         if self._ws is None or self._ws.numel() < need:
@@ -244,6 +246,10 @@ class TpcTracker:
                          "tl_first_row": ((capT,), i32), "tl_last_row": ((capT,), i32), "tl_rowhit": ((capT, R), i32),
                          "tl_x": ((capT,), f32), "tl_par": ((capT, 5), f32), "tl_cov": ((capT, 15), f32),
                          "tl_chi2": ((capT,), f32)})
+        if refit:
+            spec.update({"trk_rf_status": ((capK,), i32), "trk_rf_x_in": ((capK,), f32), "trk_rf_par_in": ((5, capK), f32),
+                         "trk_rf_cov_in": ((15, capK), f32), "trk_rf_chi2": ((capK,), f32), "trk_rf_x_out": ((capK,), f32),
+                         "trk_rf_par_out": ((5, capK), f32), "trk_rf_cov_out": ((15, capK), f32)})
         for k, (shape, dt) in spec.items():
             cur = self._out.get(k)
             if cur is None or tuple(cur.shape) != shape:
@@ -254,7 +260,7 @@ class TpcTracker:
 
     def run(self, row_offset, y, z, cap_tracklets: int | None = None, cap_tracks: int | None = None,
             cap_track_clusters: int | None = None, stages: bool = False, stream=None, sync: bool = True,
-            grow: bool = True):
+            grow: bool = True, refit: bool = False):
         """One tpcRun on device tensors.  Returns a TrackResult (after synchronising) or None when sync=False."""
         t = self.torch
         n = int(y.shape[0])
@@ -263,7 +269,7 @@ class TpcTracker:
         capC = int(cap_track_clusters) if cap_track_clusters is not None else max(n, 1)
         attempts = 3 if grow else 0     # a too-small cap_tracklets hides the true track counts: up to 3 rounds
         while True:
-            self._ensure(n, capT, capK, capC, stages)
+            self._ensure(n, capT, capK, capC, stages, refit)
             cl = tpcClusters(n, row_offset.data_ptr(), None, y.data_ptr() if n else None, z.data_ptr() if n else None,
                              None)
             tr = tpcTracks()
@@ -291,6 +297,9 @@ class TpcTracker:
         trk = {k: (o[k][:, :nt] if o[k].dim() == 2 else o[k][:nt]) for k in _TRK_PTRS[:9]}
         trk["trk_cl_offset"] = o["trk_cl_offset"][:nt + 1]
         trk["trk_cl_index"] = o["trk_cl_index"][:nc]
+        if refit:
+            for k in _REFIT_PTRS:
+                trk[k] = o[k][:, :nt] if o[k].dim() == 2 else o[k][:nt]
         stg = {}
         if stages:
             for k in _STAGE_PTRS:
