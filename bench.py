@@ -216,6 +216,17 @@ def run_ours(args, rank, world, local_rank):
     clocks = sampler.stop(t0, t1) if sampler else None
     stage /= args.steps
 
+    # ---- the NEXT-2 row (a6 refit of the selected tracks), timed apart: it is not part of the a1..a5 step ----------
+    refit_ms = None
+    if not args.no_refit:
+        acc = 0.0
+        for i in range(4):
+            trk.run(off, y, z, cap_tracklets=capT, cap_tracks=capK, cap_track_clusters=capC, sync=False, refit=True)
+            s = trk.status()
+            if i > 0:
+                acc += float(s.stage_ms[7])
+        refit_ms = acc / 3
+
     # ---- end to end through the host-buffer ABI call (pinned host memory; copies inside the timed region) ----
     hy = torch.from_numpy(ev.y).pin_memory()
     hz = torch.from_numpy(ev.z).pin_memory()
@@ -299,6 +310,12 @@ def run_ours(args, rank, world, local_rank):
                     "ms_per_step": ms_e2e, "steps": e2e_steps},
             "gpu_launches": int(st.kernel_launches) * args.steps,
             "clocks": clocks, "roofline": roofline, "stages": stages, "cpu_baseline": cpu}
+    if refit_ms is not None:
+        ncl = int(st.n_track_clusters)
+        rb = 2 * 12 * ncl + 2 * 88 * int(st.n_tracks)       # per pass: index 4 + y,z 8 per cluster; two 88-byte states out
+        line["next_refit"] = {"what": "a6 refit of the selected tracks (NEXT-2), not part of `value`", "ms": round(refit_ms, 4),
+                              "alg_bytes": rb, "gbs": round(rb / (refit_ms * 1e-3) / 1e9, 1) if refit_ms > 0 else None,
+                              "tracks": int(st.n_tracks), "track_clusters": ncl}
     print(json.dumps(line), flush=True)
 
 
@@ -310,6 +327,7 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-refit", action="store_true", help="skip the separate timing of the a6 refit (NEXT-2)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))

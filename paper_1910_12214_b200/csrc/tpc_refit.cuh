@@ -57,19 +57,28 @@ __global__ void __launch_bounds__(128) refitTracks(const uint32_t* __restrict__ 
     }
     kfSetDiag(S, P.err2_y, P.err2_z, P);
     S.chi2 = 0.0f;
+    // Both passes are software-pipelined: the index and the coordinates of the NEXT cluster are requested before the
+    // Kalman arithmetic of the current one (the input arrays are read at random: one DRAM latency per step otherwise).
+    uint32_t cn = c1;
+    float yn = y[c1], zn = z[c1];
     for (int i = 1; i < n && ok; ++i) {           // up pass
-      const uint32_t c = cl[i];
+      const uint32_t c = cn;
+      const float ym = yn, zm = zn;
+      if (i + 1 < n) { cn = cl[i + 1]; yn = y[cn]; zn = z[cn]; }
       while (__ldg(off + b + 1) <= c) ++b;
-      ok = kfPropagate(S, T.row_x[b - bsec], P, [](float, float, float, float) {}) && kfUpdate(S, y[c], z[c], P);
+      ok = kfPropagate(S, T.row_x[b - bsec], P, [](float, float, float, float) {}) && kfUpdate(S, ym, zm, P);
     }
     So = S;
     if (ok) {                                     // turn (R17) and down pass
       kfSetDiag(S, P.turn_var_scale * P.err2_y, P.turn_var_scale * P.err2_z, P);
       S.chi2 = 0.0f;
+      cn = cl[n - 1]; yn = y[cn]; zn = z[cn];
       for (int i = n - 1; i >= 0 && ok; --i) {
-        const uint32_t c = cl[i];
+        const uint32_t c = cn;
+        const float ym = yn, zm = zn;
+        if (i > 0) { cn = cl[i - 1]; yn = y[cn]; zn = z[cn]; }
         while (__ldg(off + b) > c) --b;
-        ok = kfPropagate(S, T.row_x[b - bsec], P, [](float, float, float, float) {}) && kfUpdate(S, y[c], z[c], P);
+        ok = kfPropagate(S, T.row_x[b - bsec], P, [](float, float, float, float) {}) && kfUpdate(S, ym, zm, P);
       }
     }
   }
