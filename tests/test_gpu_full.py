@@ -36,10 +36,10 @@ def test_full_size_sector0_equals_oracle_and_global_invariants(idx):
     capT = int(st.n_start_hits * 1.05) + 1024
     capK = int(st.n_tracks * 1.05) + 1024
     capC = int(st.n_track_clusters * 1.05) + 1024
-    res = trk.run(off, y, z, cap_tracklets=capT, cap_tracks=capK, cap_track_clusters=capC, stages=True)
+    res = trk.run(off, y, z, cap_tracklets=capT, cap_tracks=capK, cap_track_clusters=capC, stages=True, refit=True)
     assert res.status.status == 0
     n0 = int(ev.row_offset[R])
-    o = orc.run(_sector0(ev))
+    o = orc.run(_sector0(ev), refit=True)
     ns0 = len(o.start_hits)
     g = {}
     for k in ("link_up_raw", "link_dn_raw", "link_up", "link_dn"):
@@ -62,6 +62,16 @@ def test_full_size_sector0_equals_oracle_and_global_invariants(idx):
     assert ns0 == int((sh < n0).sum()) and np.all(sh[:ns0] < n0)
     rep = compare(g, o, R)
     print(ev.name, ev.n_clusters, "sector-0 tracks", nt0, rep)
+    # the optional a6 refit of sector 0's tracks: bit-identical to the oracle's O6
+    assert np.array_equal(res.trk["trk_rf_status"][:nt0].cpu().numpy(), o.rf_status)
+    for name, ref in (("trk_rf_x_in", o.rf_x_in), ("trk_rf_chi2", o.rf_chi2), ("trk_rf_x_out", o.rf_x_out)):
+        assert np.array_equal(res.trk[name][:nt0].cpu().numpy(), ref.astype(np.float32)), name
+    for name, ref in (("trk_rf_par_in", o.rf_par_in), ("trk_rf_cov_in", o.rf_cov_in), ("trk_rf_par_out", o.rf_par_out),
+                      ("trk_rf_cov_out", o.rf_cov_out)):
+        assert np.array_equal(res.trk[name][:, :nt0].cpu().numpy(), ref.T.astype(np.float32)), name
+    rfs = res.trk["trk_rf_status"]
+    assert float(rfs.float().mean().item()) > 0.95
+    assert bool(torch.isfinite(res.trk["trk_rf_par_in"]).all().item()) and bool(torch.isfinite(res.trk["trk_rf_cov_out"]).all().item())
     # ---- whole event: invariants that hold at any size ----
     up, dn = res.stages["link_up"].long(), res.stages["link_dn"].long()
     n = ev.n_clusters
