@@ -208,3 +208,25 @@ def test_run_host_matches_device_path():
     for k in host:
         assert np.array_equal(np.asarray(host[k]).view(np.int32) if host[k].dtype == np.uint32 else host[k], dev[k]), k
     trk.close()
+
+
+@pytest.mark.parametrize("seed", list(range(12)))
+def test_parity_fuzz_random_events_dead_rows_and_parameters(seed):
+    """Seeded random small events: workload, size, dead rows, coarsened coordinates (many exact ties) and the
+    parameters of Table P all vary; every stage must still be bit-identical to the oracle."""
+    rng = np.random.default_rng(1000 + seed)
+    idx = int(rng.integers(0, 5))
+    scale = float({0: 0.6, 1: 0.04, 2: 0.05, 3: 0.03, 4: 0.008}[idx] * rng.uniform(0.5, 1.5))
+    dead = tuple(int(r) for r in rng.choice(152, size=int(rng.integers(0, 6)), replace=False))
+    ev = datagen.make_event(idx, scale=scale, seed=100 + seed, dead_rows=dead)
+    if seed % 3 == 0:      # coordinates on a 1/8 cm lattice: exact ties in Dev and in the search distance
+        ev = datagen.event_from_arrays(ev.row_offset, np.round(ev.y * 8) / 8, np.round(ev.z * 8) / 8, ev.n_sectors, R,
+                                       row_dead=ev.row_dead)
+    par = dict(road_sigma=float(rng.uniform(2.5, 6.0)), road_min=float(rng.uniform(0.1, 0.5)),
+               road_max=float(rng.uniform(1.0, 3.0)), max_row_gap=int(rng.integers(1, 7)),
+               min_chain_hits=int(rng.integers(2, 6)), min_tracklet_hits=int(rng.integers(5, 25)),
+               min_track_hits=int(rng.integers(5, 25)), link_dev2_max=float(rng.uniform(0.1, 1.0)),
+               area_y=float(rng.uniform(0.8, 2.0)), area_z=float(rng.uniform(0.8, 2.0)),
+               max_sinphi=float(rng.uniform(0.8, 0.99)), clusters_per_cell=float(rng.uniform(0.2, 4.0)))
+    rep, res, o = _run_both(ev, **par)
+    assert len(o.start_hits) > 0
