@@ -110,6 +110,57 @@ bool update(State<Real>& st, Real ym, Real zm, Real err2_y, Real err2_z) {
   return true;
 }
 
+// ---- O7 Rotate(alpha): the same helix seen from a frame turned by alpha about z; C <- J C J^T -------------------
+template <typename Real>
+bool rotate(State<Real>& st, double alpha, Real b, Real max_sinphi) {
+  const Real ca = (Real)std::cos(alpha), sa = (Real)std::sin(alpha);
+  const Real s = st.s, t = st.t;
+  const Real c = std::sqrt((Real)1 - s * s);
+  const Real s1 = s * ca - c * sa;
+  if (!(std::fabs(s1) < max_sinphi)) return false;
+  const Real c1 = std::sqrt((Real)1 - s1 * s1);
+  const Real x1 = st.x * ca + st.y * sa;
+  const Real y1 = st.y * ca - st.x * sa;
+  const Real jy = c / c1, jz = -(sa * t) / c1, js = c1 / c, jq = -((st.q * b) * sa);   // jq = d s' / d y (curvature)
+  Real* C = st.C;
+  const Real C00 = C[0], C10 = C[1], C11 = C[2], C20 = C[3], C21 = C[4], C22 = C[5], C30 = C[6], C31 = C[7], C32 = C[8],
+             C40 = C[10], C41 = C[11], C42 = C[12];
+  C[0] = (jy * jy) * C00;
+  C[1] = jy * (jz * C00 + C10);
+  C[2] = ((jz * jz) * C00 + ((Real)2 * jz) * C10) + C11;
+  const Real m2 = jq * C00 + js * C20;
+  C[3] = jy * m2;
+  C[4] = jz * m2 + (jq * C10 + js * C21);
+  C[5] = ((jq * jq) * C00 + (((Real)2 * jq) * js) * C20) + (js * js) * C22;
+  C[6] = jy * C30;
+  C[7] = jz * C30 + C31;
+  C[8] = jq * C30 + js * C32;
+  C[10] = jy * C40;
+  C[11] = jz * C40 + C41;
+  C[12] = jq * C40 + js * C42;
+  st.x = x1; st.y = y1; st.s = s1;
+  return true;
+}
+
+// ---- O7 Match(a, b): outer state of a, rotated into b's sector if rel != 0, propagated to b's plane; diagonal chi2 ----
+template <typename Real>
+bool match(State<Real> a, int rel, const State<Real>& b, Real bfield, const orcParams& P, Real& chi2) {
+  const double a20 = 0.3490658503988659;   // 20 degrees
+  if (rel != 0 && !rotate(a, rel > 0 ? a20 : -a20, bfield, (Real)P.max_sinphi)) return false;
+  if (!propagate(a, b.x, bfield, (Real)P.max_sinphi)) return false;
+  const Real pa[5] = {a.y, a.z, a.s, a.t, a.q}, pb[5] = {b.y, b.z, b.s, b.t, b.q};
+  Real sum = 0;
+  for (int i = 0; i < 5; ++i) {
+    const Real den = a.C[tri(i, i)] + b.C[tri(i, i)];
+    if (!(den > (Real)0)) return false;
+    const Real d = pa[i] - pb[i];
+    sum = sum + (d * d) / den;
+  }
+  if (!(sum <= (Real)P.merge_chi2_max)) return false;
+  chi2 = sum;
+  return true;
+}
+
 template <typename Real>
 struct Tracklet {
   int status = 0;   // 0 discarded in chain fit, 1 rejected, 2 accepted
@@ -145,6 +196,9 @@ struct orcResult {
   // outer = state at the last kept cluster (up pass)
   std::vector<int32_t> rf_status;
   std::vector<double> rf_x_in, rf_par_in, rf_cov_in, rf_chi2, rf_x_out, rf_par_out, rf_cov_out;
+  // O7 merger (NEXT-1)
+  std::vector<int32_t> mg_next, mg_prev, mg_head;
+  std::vector<double> mg_chi2;
 };
 
 namespace {
@@ -376,6 +430,57 @@ struct Tracker {
     }
   }
 
+  // ---- O7 links between track segments (O7; readings R31..R33) ---------------------------
+  void mergeAll() {
+    const int64_t nt = (int64_t)res.tr_id.size();
+    res.mg_next.assign(nt, -1); res.mg_prev.assign(nt, -1); res.mg_head.assign(nt, -1); res.mg_chi2.assign(nt, 0);
+    const Real bf = (Real)(0.00299792458 * (double)g.bz_tesla);
+    auto stateOf = [&](int64_t k, bool outer) {
+      State<Real> st{};
+      const std::vector<double>& x = outer ? res.rf_x_out : res.rf_x_in;
+      const std::vector<double>& p = outer ? res.rf_par_out : res.rf_par_in;
+      const std::vector<double>& c = outer ? res.rf_cov_out : res.rf_cov_in;
+      st.x = (Real)x[k]; st.y = (Real)p[k * 5]; st.z = (Real)p[k * 5 + 1]; st.s = (Real)p[k * 5 + 2];
+      st.t = (Real)p[k * 5 + 3]; st.q = (Real)p[k * 5 + 4];
+      for (int i = 0; i < 15; ++i) st.C[i] = (Real)c[k * 15 + i];
+      return st;
+    };
+    auto relOf = [&](int sa, int sb) {          // 0 same sector, +1 / -1 azimuthal neighbour on the same side, 2 none
+      if (sa == sb) return 0;
+      if (S != 36 || sa / 18 != sb / 18) return 2;
+      const int ja = sa % 18, jb = sb % 18;
+      if (jb == (ja + 1) % 18) return 1;
+      if (jb == (ja + 17) % 18) return -1;
+      return 2;
+    };
+    std::vector<int32_t> bestB(nt, -1), bestA(nt, -1);
+    std::vector<Real> chiB(nt, 0), chiA(nt, 0);
+    for (int64_t a = 0; a < nt; ++a) {
+      if (!res.rf_status[a]) continue;
+      const State<Real> sa = stateOf(a, true);
+      for (int64_t b = 0; b < nt; ++b) {
+        if (b == a || !res.rf_status[b]) continue;
+        const int rel = relOf(res.tr_sector[a], res.tr_sector[b]);
+        if (rel == 2) continue;
+        const int gap = res.tr_first[b] - res.tr_last[a];
+        if (gap > P.merge_max_row_gap || gap < (rel == 0 ? 1 : -P.merge_back_rows)) continue;
+        Real chi2;
+        if (!match(sa, rel, stateOf(b, false), bf, P, chi2)) continue;
+        if (bestB[a] < 0 || chi2 < chiB[a]) { bestB[a] = (int32_t)b; chiB[a] = chi2; }          // ties: lowest b (loop order)
+        if (bestA[b] < 0 || chi2 < chiA[b]) { bestA[b] = (int32_t)a; chiA[b] = chi2; }          // ties: lowest a
+      }
+    }
+    for (int64_t a = 0; a < nt; ++a) {
+      const int32_t b = bestB[a];
+      if (b >= 0 && bestA[b] == (int32_t)a) { res.mg_next[a] = b; res.mg_prev[b] = (int32_t)a; res.mg_chi2[a] = (double)chiB[a]; }
+    }
+    for (int64_t k = 0; k < nt; ++k) {
+      int64_t h = k;
+      for (int64_t guard = 0; res.mg_prev[h] >= 0 && guard < nt; ++guard) h = res.mg_prev[h];
+      res.mg_head[k] = (int32_t)h;
+    }
+  }
+
   void construct(uint32_t h0, Tracklet<Real>& T) const {
     const Real b = (Real)(0.00299792458 * (double)g.bz_tesla);
     const Real msp = (Real)P.max_sinphi, e2y = (Real)P.err2_y, e2z = (Real)P.err2_z;
@@ -521,6 +626,7 @@ void orcDefaultParams(orcParams* p) {
   p->turn_var_scale = 100.0f; p->max_sinphi = 0.98f; p->road_sigma = 4.0f; p->road_min = 0.3f; p->road_max = 2.0f;
   p->max_row_gap = 4; p->min_chain_hits = 3; p->min_tracklet_hits = 10; p->min_track_hits = 10;
   p->cell_min = 0.5f; p->cell_max = 8.0f;
+  p->merge_max_row_gap = 40; p->merge_back_rows = 5; p->merge_chi2_max = 50.0f;
 }
 
 int orcRun(const orcGeometry* g, const orcParams* p, int64_t n, const uint32_t* off, const float* y, const float* z,
@@ -536,9 +642,10 @@ int orcRun(const orcGeometry* g, const orcParams* p, int64_t n, const uint32_t* 
   orcResult* r = new orcResult();
   r->n = n; r->n_sectors = g->n_sectors; r->n_rows = g->n_rows;
   r->fp64 = (flags & ORC_FP64) != 0; r->brute = (flags & ORC_BRUTE_FORCE) != 0;
-  const bool rf = (flags & ORC_REFIT) != 0;
-  if (r->fp64) { Tracker<double> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); if (rf) T.refitAll(); }
-  else { Tracker<float> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); if (rf) T.refitAll(); }
+  const bool mg = (flags & ORC_MERGE) != 0;
+  const bool rf = mg || (flags & ORC_REFIT) != 0;
+  if (r->fp64) { Tracker<double> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); if (rf) T.refitAll(); if (mg) T.mergeAll(); }
+  else { Tracker<float> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); if (rf) T.refitAll(); if (mg) T.mergeAll(); }
   *out = r;
   return ORC_OK;
 }
@@ -562,9 +669,36 @@ void orcGetRefit(const orcResult* r, int32_t* status, double* x_in, double* par_
   copyOut(chi2, r->rf_chi2); copyOut(x_out, r->rf_x_out); copyOut(par_out, r->rf_par_out); copyOut(cov_out, r->rf_cov_out);
 }
 
+void orcGetMerge(const orcResult* r, int32_t* next, int32_t* prev, int32_t* head, double* chi2) {
+  copyOut(next, r->mg_next); copyOut(prev, r->mg_prev); copyOut(head, r->mg_head); copyOut(chi2, r->mg_chi2);
+}
+
 }  // extern "C"
 
 namespace {
+template <typename Real>
+State<Real> stateFrom(const double* st, const double* cov) {
+  State<Real> s{};
+  s.x = (Real)st[0]; s.y = (Real)st[1]; s.z = (Real)st[2]; s.s = (Real)st[3]; s.t = (Real)st[4]; s.q = (Real)st[5];
+  for (int i = 0; i < 15; ++i) s.C[i] = (Real)cov[i];
+  return s;
+}
+template <typename Real>
+int rotateT(double* st, double* cov, double alpha, double bz, double msp) {
+  State<Real> s = stateFrom<Real>(st, cov);
+  if (!rotate(s, alpha, (Real)(0.00299792458 * bz), (Real)msp)) return 0;
+  st[0] = (double)s.x; st[1] = (double)s.y; st[2] = (double)s.z; st[3] = (double)s.s; st[4] = (double)s.t; st[5] = (double)s.q;
+  for (int i = 0; i < 15; ++i) cov[i] = (double)s.C[i];
+  return 1;
+}
+template <typename Real>
+int matchT(const orcParams* p, double bz, const double* as, const double* ac, int rel, const double* bs, const double* bc,
+           double* chi2) {
+  Real c2 = 0;
+  if (!match(stateFrom<Real>(as, ac), rel, stateFrom<Real>(bs, bc), (Real)(0.00299792458 * bz), *p, c2)) return 0;
+  *chi2 = (double)c2;
+  return 1;
+}
 template <typename Real>
 int refitPoints(const orcGeometry* g, const orcParams* p, int n, const int32_t* rows, const double* y, const double* z,
                 double* in, double* out) {
@@ -596,6 +730,15 @@ int refitPoints(const orcGeometry* g, const orcParams* p, int n, const int32_t* 
 }  // namespace
 
 extern "C" {
+
+int orcRotate(double* state, double* cov, double alpha, double bz_tesla, double max_sinphi, int fp64) {
+  return fp64 ? rotateT<double>(state, cov, alpha, bz_tesla, max_sinphi) : rotateT<float>(state, cov, alpha, bz_tesla, max_sinphi);
+}
+int orcMatch(const orcParams* p, double bz_tesla, const double* a_state, const double* a_cov, int rel, const double* b_state,
+             const double* b_cov, int fp64, double* chi2) {
+  return fp64 ? matchT<double>(p, bz_tesla, a_state, a_cov, rel, b_state, b_cov, chi2)
+              : matchT<float>(p, bz_tesla, a_state, a_cov, rel, b_state, b_cov, chi2);
+}
 
 int orcRefitPoints(const orcGeometry* g, const orcParams* p, int n, const int32_t* rows, const double* y, const double* z,
                    int fp64, double* inner22, double* outer22) {

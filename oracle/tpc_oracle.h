@@ -39,12 +39,14 @@ typedef struct {
   float max_sinphi, road_sigma, road_min, road_max;
   int32_t max_row_gap, min_chain_hits, min_tracklet_hits, min_track_hits;
   float cell_min, cell_max;
+  int32_t merge_max_row_gap, merge_back_rows;   /* O7: 40, 5 */
+  float merge_chi2_max;                         /* O7: 50 */
 } orcParams;
 
 typedef struct orcResult orcResult;
 
 enum { ORC_OK = 0, ORC_ERR_INVALID_ARG = -1, ORC_ERR_UNSORTED_OFFSETS = -2 };
-enum { ORC_BRUTE_FORCE = 1, ORC_FP64 = 2, ORC_REFIT = 4 };
+enum { ORC_BRUTE_FORCE = 1, ORC_FP64 = 2, ORC_REFIT = 4, ORC_MERGE = 8 /* implies ORC_REFIT */ };
 
 void orcDefaultParams(orcParams* p);
 
@@ -87,6 +89,18 @@ void orcGetRefit(const orcResult*, int32_t* status, double* x_in, double* par_in
  * inner22 / outer22 = x, y, z, s, t, q, C[15], chi2.  Returns 1 on success. */
 int orcRefitPoints(const orcGeometry* g, const orcParams* p, int n, const int32_t* rows, const double* y, const double* z,
                    int fp64, double* inner22, double* outer22);
+
+/* O7 (NEXT-1 of SURVEY.md 8(f), DESIGN.md section 3 "O7"): links between track segments, only with ORC_MERGE.
+ * next / prev / head [n_tracks] track indices (-1 none; head = first track of the chain), chi2 [n_tracks] of the link
+ * to next (0 if none).  Pins: tests/test_oracle_merge.py. */
+void orcGetMerge(const orcResult*, int32_t* next, int32_t* prev, int32_t* head, double* chi2);
+/* Pieces of O7 for the pins.  state = {x, y, z, s, t, q}, cov = 15 lower-triangle elements, in/out as doubles.
+ * orcRotate: frame turned by alpha (radians); returns 1 on success, 0 (untouched) on failure.
+ * orcMatch: chi2 of the match of outer state a to inner state b (b at plane b_state[0]); rel = 0 same sector,
+ * +1 / -1 b in the next / previous sector; returns 1 and *chi2 when admissible (chi2 <= merge_chi2_max), else 0. */
+int orcRotate(double* state, double* cov, double alpha, double bz_tesla, double max_sinphi, int fp64);
+int orcMatch(const orcParams* p, double bz_tesla, const double* a_state, const double* a_cov, int rel,
+             const double* b_state, const double* b_cov, int fp64, double* chi2);
 
 /* Single KF steps for the pins.  state = {x, y, z, s, t, q}, cov = 15 lower-triangle elements
  * (00,10,11,20,21,22,30,...,44), both in/out as doubles (rounded to binary32 first unless fp64).

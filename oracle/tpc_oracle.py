@@ -20,6 +20,7 @@ _LIB = os.path.join(_HERE, "libtpcoracle.so")
 BRUTE_FORCE = 1
 FP64 = 2
 REFIT = 4
+MERGE = 8
 
 
 def build(force: bool = False) -> str:
@@ -41,7 +42,8 @@ class Params(ctypes.Structure):
                 ("area_y", "area_z", "link_dev2_max", "err2_y", "err2_z", "init_var_s", "init_var_t", "init_var_q",
                  "turn_var_scale", "max_sinphi", "road_sigma", "road_min", "road_max")] + \
                [(n, ctypes.c_int32) for n in ("max_row_gap", "min_chain_hits", "min_tracklet_hits", "min_track_hits")] + \
-               [("cell_min", ctypes.c_float), ("cell_max", ctypes.c_float)]
+               [("cell_min", ctypes.c_float), ("cell_max", ctypes.c_float), ("merge_max_row_gap", ctypes.c_int32),
+                ("merge_back_rows", ctypes.c_int32), ("merge_chi2_max", ctypes.c_float)]
 
 
 _lib = None
@@ -69,6 +71,12 @@ def _load():
         L.orcGetTracks.argtypes = [vp] * 12
         for f in ("orcGetGrid", "orcGetLinks", "orcGetStartHits", "orcGetTracklets", "orcGetTracks"):
             getattr(L, f).restype = None
+        L.orcGetMerge.argtypes = [vp] * 5
+        L.orcGetMerge.restype = None
+        L.orcRotate.argtypes = [vp, vp, dbl, dbl, dbl, ci]
+        L.orcRotate.restype = ci
+        L.orcMatch.argtypes = [ctypes.POINTER(Params), dbl, vp, vp, ci, vp, vp, ci, vp]
+        L.orcMatch.restype = ci
         L.orcGetRefit.argtypes = [vp] * 9
         L.orcGetRefit.restype = None
         L.orcRefitPoints.argtypes = [ctypes.POINTER(Geometry), ctypes.POINTER(Params), ci, vp, vp, vp, ci, vp, vp]
@@ -127,6 +135,11 @@ class OracleResult:
     rf_x_out: np.ndarray | None = None
     rf_par_out: np.ndarray | None = None
     rf_cov_out: np.ndarray | None = None
+    # O7 merger (only with merge=True): links between track segments
+    mg_next: np.ndarray | None = None
+    mg_prev: np.ndarray | None = None
+    mg_head: np.ndarray | None = None
+    mg_chi2: np.ndarray | None = None
 
     @property
     def n_tracks(self) -> int:
@@ -138,7 +151,7 @@ def _ptr(a):
 
 
 def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool = False,
-        stages_only: bool = False, refit: bool = False) -> OracleResult:
+        stages_only: bool = False, refit: bool = False, merge: bool = False) -> OracleResult:
     """Run O1..O5 on an Event-like object (fields n_sectors, n_rows, row_x, row_dead, bz_tesla,
     tan_half_sector, z_min, z_max, row_offset, y, z; numpy arrays)."""
     L = _load()
@@ -153,7 +166,7 @@ def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool 
     n = int(y.shape[0])
     h = ctypes.c_void_p()
     rc = L.orcRun(ctypes.byref(g), ctypes.byref(p), n, off.ctypes.data, _ptr(y), _ptr(z),
-                  (BRUTE_FORCE if brute_force else 0) | (FP64 if fp64 else 0) | (REFIT if refit else 0),
+                  (BRUTE_FORCE if brute_force else 0) | (FP64 if fp64 else 0) | (REFIT if refit else 0) | (MERGE if merge else 0),
                   ctypes.byref(h))
     if rc != 0:
         raise ValueError(f"orcRun failed with {rc}")
@@ -181,6 +194,7 @@ def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool 
         L.orcGetTracks(h, _ptr(kid), _ptr(ks), _ptr(kf), _ptr(kl), _ptr(kn), _ptr(kx), _ptr(kpar), _ptr(kcov),
                        _ptr(kchi), _ptr(koff), _ptr(kidx))
         rf = {}
+        refit = refit or merge
         if refit:
             rst = np.zeros(nt, np.int32)
             rxi, rchi, rxo = np.zeros(nt), np.zeros(nt), np.zeros(nt)
@@ -188,6 +202,11 @@ def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool 
             L.orcGetRefit(h, _ptr(rst), _ptr(rxi), _ptr(rpi), _ptr(rci), _ptr(rchi), _ptr(rxo), _ptr(rpo), _ptr(rco))
             rf = dict(rf_status=rst, rf_x_in=rxi, rf_par_in=rpi, rf_cov_in=rci, rf_chi2=rchi, rf_x_out=rxo, rf_par_out=rpo,
                       rf_cov_out=rco)
+        if merge:
+            mn, mp, mh = (np.full(nt, -1, np.int32) for _ in range(3))
+            mc = np.zeros(nt)
+            L.orcGetMerge(h, _ptr(mn), _ptr(mp), _ptr(mh), _ptr(mc))
+            rf.update(mg_next=mn, mg_prev=mp, mg_head=mh, mg_chi2=mc)
     finally:
         L.orcFree(h)
     return OracleResult(n, s2o, cell, ncell, ur, dr, u, d, sh, st, nh, fr, lr, rh, tx, tpar, tcov, tchi, kid, ks, kf, kl,
@@ -225,3 +244,22 @@ def refit_points(rows, y, z, row_x, bz_tesla=0.5, params: Params | None = None, 
     ok = L.orcRefitPoints(ctypes.byref(g), ctypes.byref(p), len(rows), rows.ctypes.data, yy.ctypes.data, zz.ctypes.data,
                           int(fp64), inner.ctypes.data, outer.ctypes.data)
     return bool(ok), inner, outer
+
+
+def rotate(state, cov, alpha, bz_tesla=0.5, max_sinphi=0.98, fp64=True):
+    """O7 Rotate: the state seen from a frame turned by alpha (radians).  Returns (ok, state, cov)."""
+    s = np.array(state, np.float64)
+    c = np.array(cov, np.float64)
+    ok = _load().orcRotate(s.ctypes.data, c.ctypes.data, float(alpha), float(bz_tesla), float(max_sinphi), int(fp64))
+    return bool(ok), s, c
+
+
+def match(a_state, a_cov, rel, b_state, b_cov, bz_tesla=0.5, params: Params | None = None, fp64=True):
+    """O7 Match of outer state a to inner state b (rel = 0 same sector, +-1 neighbour).  Returns (ok, chi2)."""
+    p = params if params is not None else default_params()
+    a, ac = np.array(a_state, np.float64), np.array(a_cov, np.float64)
+    b, bc = np.array(b_state, np.float64), np.array(b_cov, np.float64)
+    chi2 = np.zeros(1)
+    ok = _load().orcMatch(ctypes.byref(p), float(bz_tesla), a.ctypes.data, ac.ctypes.data, int(rel), b.ctypes.data,
+                          bc.ctypes.data, int(fp64), chi2.ctypes.data)
+    return bool(ok), float(chi2[0])
