@@ -9,6 +9,7 @@
  *   a4 tracklet constructor link-chain fit + row-by-row helix Kalman extrapolation (5 params, 15 cov, fp32)
  *   a5 tracklet selector   shared clusters go to the longest / lowest-chi2 tracklet
  *   a6 refit (optional)    Kalman refit of every selected track over its kept clusters: inner and outer state
+ *   a7 merger (optional)   links between track segments across row gaps and sector borders
  * The formulas, constants and tie-breaks are DESIGN.md section 3 (readings R0..R27 of SURVEY.md 8(c)).
  *
  * Conventions
@@ -71,6 +72,9 @@ typedef struct {
   int32_t validate_input;       /* 0          1 = scan y,z for NaN/Inf and fail with TPC_ERR_NONFINITE_INPUT */
   int32_t force_wide_keys;      /* 0          1 = use the two-pass selector keys even when the packed 64-bit key
                                               fits (R27; results are identical, for tests) */
+  int32_t merge_max_row_gap;    /* 40         O7: rows between the end of a segment and the start of its continuation */
+  int32_t merge_back_rows;      /* 5          O7: a continuation in the neighbour sector may start this many rows lower */
+  float merge_chi2_max;         /* 50         O7: cut on the diagonal chi2 of a match */
 } tpcParams;
 
 /* Input clusters: CSR by (sector,row), fp32 SoA (single-precision cluster properties). */
@@ -124,6 +128,12 @@ typedef struct {
   float* trk_rf_x_out;          /* [cap_tracks] x of the last kept cluster: reference plane of the outer state */
   float* trk_rf_par_out;        /* [5][cap_tracks] outer state (after the up pass) */
   float* trk_rf_cov_out;        /* [15][cap_tracks] */
+  /* optional O7 links between track segments (DESIGN.md section 3 "O7").  All NULL = no merger; otherwise
+   * ALL four must be given together with the refit outputs (the merger works on the refitted states). */
+  int32_t* trk_mg_next;         /* [cap_tracks] track that continues this one, -1 none */
+  int32_t* trk_mg_prev;         /* [cap_tracks] track this one continues, -1 none */
+  int32_t* trk_mg_head;         /* [cap_tracks] first track of the chain (itself if unlinked) */
+  float* trk_mg_chi2;           /* [cap_tracks] chi2 of the link to trk_mg_next, 0 if none */
 } tpcTracks;
 
 /* Filled by tpcGetRunStatus after the stream has drained. */
@@ -139,7 +149,8 @@ typedef struct {
   int64_t n_cells;              /* grid cells over all (sector,row) */
   float stage_ms[8];            /* per-stage device times of the last run when profiling is on (else 0):
                                    0 grid, 1 neighbour finder, 2 cleaner+start hits, 3 constructor, 4 selector,
-                                   5 optional exports and refit, 6 total, 7 refit alone */
+                                   5 optional refit, merger and exports, 6 total, 7 refit alone */
+  float merge_ms;               /* the O7 merger alone (profiling on, merger requested) */
 } tpcRunStatus;
 
 int tpcDefaultParams(tpcParams* p);

@@ -19,6 +19,7 @@
 #include "tpc_tracklet.cuh"
 #include "tpc_select.cuh"
 #include "tpc_refit.cuh"
+#include "tpc_merge.cuh"
 
 using namespace tpc;
 
@@ -46,6 +47,10 @@ struct Workspace {
   int32_t *kept_first, *kept_last;
   unsigned long long* owner_key;
   uint32_t* owner_id;
+  uint32_t *mg_start, *mg_fill, *mg_list;   // merger: tracks bucketed by (sector, first row)
+  int32_t* mg_best_b;
+  float* mg_chi_b;
+  unsigned long long* mg_key_a;
   size_t bytes;
 };
 
@@ -62,7 +67,7 @@ struct tpcHandle {
   int64_t* d_cnt = nullptr;        // CNT_COUNT counters + 1 slot for the packed selector total
   int64_t* h_cnt = nullptr;        // pinned copy
   cudaEvent_t ev_done = nullptr;
-  cudaEvent_t ev_stage[9] = {};    // 0..6 stage boundaries, 7/8 around the optional refit
+  cudaEvent_t ev_stage[11] = {};   // 0..6 stage boundaries, 7/8 around the optional refit, 9/10 around the merger
   int profiling = 0;
   int launches = 0;
   int tc_grid = 148;               // persistent grid of the tracklet constructor: SMs x resident blocks
@@ -136,6 +141,12 @@ Workspace layout(const tpcHandle* h, int64_t N, int64_t capT, char* base) {
   w.kept_last = (int32_t*)take(4 * (size_t)Tn);
   w.owner_key = (unsigned long long*)take(8 * (size_t)Nn);
   w.owner_id = (uint32_t*)take(4 * (size_t)Nn);
+  w.mg_start = (uint32_t*)take(4 * (size_t)(nb + 1));
+  w.mg_fill = (uint32_t*)take(4 * (size_t)(nb + 1));
+  w.mg_list = (uint32_t*)take(4 * (size_t)Tn);
+  w.mg_best_b = (int32_t*)take(4 * (size_t)Tn);
+  w.mg_chi_b = (float*)take(4 * (size_t)Tn);
+  w.mg_key_a = (unsigned long long*)take(8 * (size_t)Tn);
   w.bytes = o;
   return w;
 }
@@ -154,6 +165,7 @@ int tpcDefaultParams(tpcParams* p) {
   p->max_row_gap = 4; p->min_chain_hits = 3; p->min_tracklet_hits = 10; p->min_track_hits = 10;
   p->cell_min = 0.5f; p->cell_max = 8.0f; p->clusters_per_cell = 1.0f;
   p->validate_input = 0; p->force_wide_keys = 0;
+  p->merge_max_row_gap = 40; p->merge_back_rows = 5; p->merge_chi2_max = 50.0f;
   return TPC_OK;
 }
 
@@ -167,6 +179,7 @@ int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cud
   if (!(g->z_max > g->z_min) || !(g->tan_half_sector > 0) || !(g->row_x[0] > 0)) return TPC_ERR_INVALID_ARG;
   if (!(p->cell_min > 0) || !(p->cell_max >= p->cell_min) || !(p->clusters_per_cell > 0)) return TPC_ERR_INVALID_ARG;
   if (p->min_chain_hits < 2 || p->max_row_gap < 0) return TPC_ERR_INVALID_ARG;
+  if (p->merge_max_row_gap < 0 || p->merge_back_rows < 0) return TPC_ERR_INVALID_ARG;
   tpcHandle* h = new (std::nothrow) tpcHandle();
   if (!h) return TPC_ERR_INVALID_ARG;
   h->device = cuda_device;
@@ -207,7 +220,7 @@ int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cud
             cudaMalloc(&h->d_cnt, 8 * (CNT_COUNT + 1)) == cudaSuccess &&
             cudaMallocHost(&h->h_cnt, 8 * (CNT_COUNT + 1)) == cudaSuccess &&
             cudaEventCreate(&h->ev_done) == cudaSuccess;
-  for (int i = 0; ok && i < 9; ++i) ok = cudaEventCreate(&h->ev_stage[i]) == cudaSuccess;
+  for (int i = 0; ok && i < 11; ++i) ok = cudaEventCreate(&h->ev_stage[i]) == cudaSuccess;
   ok = ok && cudaMemcpy(h->d_row_x, g->row_x, 4 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
        cudaMemcpy(h->d_up, up.data(), 2 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
        cudaMemcpy(h->d_dn, dn.data(), 2 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
@@ -232,7 +245,7 @@ int tpcDestroy(tpcHandle* h) {
   cudaFree(h->d_row_x); cudaFree(h->d_up); cudaFree(h->d_dn); cudaFree(h->d_dead); cudaFree(h->d_cnt);
   if (h->h_cnt) cudaFreeHost(h->h_cnt);
   if (h->ev_done) cudaEventDestroy(h->ev_done);
-  for (int i = 0; i < 9; ++i) if (h->ev_stage[i]) cudaEventDestroy(h->ev_stage[i]);
+  for (int i = 0; i < 11; ++i) if (h->ev_stage[i]) cudaEventDestroy(h->ev_stage[i]);
   for (int i = 0; i < 16; ++i) if (h->pool[i]) cudaFree(h->pool[i]);
   delete h;
   return TPC_OK;
@@ -269,6 +282,9 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
                    (out->trk_rf_cov_in != nullptr) + (out->trk_rf_chi2 != nullptr) + (out->trk_rf_x_out != nullptr) +
                    (out->trk_rf_par_out != nullptr) + (out->trk_rf_cov_out != nullptr);
   if (n_rf != 0 && n_rf != 8) return TPC_ERR_INVALID_ARG;      // the refit outputs come all or none
+  const int n_mg = (out->trk_mg_next != nullptr) + (out->trk_mg_prev != nullptr) + (out->trk_mg_head != nullptr) +
+                   (out->trk_mg_chi2 != nullptr);
+  if ((n_mg != 0 && n_mg != 4) || (n_mg == 4 && n_rf != 8)) return TPC_ERR_INVALID_ARG;   // the merger needs the refit
   if (!workspace || ((uintptr_t)workspace % ALIGN) != 0) return TPC_ERR_INVALID_ARG;
   const Workspace w = layout(h, N, capT, (char*)workspace);
   if (workspace_bytes < w.bytes) return TPC_ERR_WORKSPACE_TOO_SMALL;
@@ -362,6 +378,28 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
     refitTracks<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(in->row_offset, in->y, in->z, P, T, to, rf, cnt); ++L;
   }
   stage(8);
+  // ---- a7 optional links between track segments (O7) -------------------------------------------------
+  stage(9);
+  if (n_mg == 4 && N > 0 && out->cap_tracks > 0) {
+    const int64_t nk = std::min<int64_t>(out->cap_tracks, capT);     // tracks <= tracklets <= capT: the lists fit
+    const MergeIn mi{out->cap_tracks, out->trk_rf_status, out->trk_sector, out->trk_first_row, out->trk_last_row,
+                     out->trk_rf_x_in, out->trk_rf_par_in, out->trk_rf_cov_in, out->trk_rf_x_out, out->trk_rf_par_out,
+                     out->trk_rf_cov_out};
+    const MergeOut mo{out->trk_mg_next, out->trk_mg_prev, out->trk_mg_head, out->trk_mg_chi2};
+    const MergeParams mp{h->params.merge_max_row_gap, h->params.merge_back_rows, h->params.merge_chi2_max,
+                         (float)cos(0.3490658503988659), (float)sin(0.3490658503988659)};
+    const unsigned gK = (unsigned)ceilDiv(nk, 256);
+    TPC_CUDA(h, cudaMemsetAsync(w.mg_start, 0, 4 * (size_t)(nb + 1), st)); ++L;
+    TPC_CUDA(h, cudaMemsetAsync(w.mg_fill, 0, 4 * (size_t)(nb + 1), st)); ++L;
+    mergeCount<<<gK, 256, 0, st>>>(mi, mo, P.n_rows, w.mg_start, w.mg_best_b, w.mg_key_a, cnt); ++L;
+    scanArrayInPlace<uint32_t><<<1, 1024, 0, st>>>(w.mg_start, (int64_t)nb + 1, nullptr); ++L;
+    mergeFill<<<gK, 256, 0, st>>>(mi, P.n_rows, w.mg_start, w.mg_fill, w.mg_list, cnt); ++L;
+    mergeMatch<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(mi, P, T, mp, w.mg_start, w.mg_list, w.mg_best_b, w.mg_chi_b,
+                                                           w.mg_key_a, cnt); ++L;
+    mergeLink<<<gK, 256, 0, st>>>(mi, mo, w.mg_best_b, w.mg_chi_b, w.mg_key_a, cnt); ++L;
+    mergeHead<<<gK, 256, 0, st>>>(mi, mo, cnt); ++L;
+  }
+  stage(10);
   // ---- optional per-stage exports -----------------------------------------------------------------
   if (N > 0 && (out->link_up_raw || out->link_dn_raw || out->link_up || out->link_dn)) {
     exportLinks<<<gN256, 256, 0, st>>>(N, w.s2o, w.lup, w.ldn, w.cup, w.cdn, out->link_up_raw, out->link_dn_raw,
@@ -406,6 +444,7 @@ int tpcGetRunStatus(tpcHandle* h, tpcRunStatus* out) {
     float ms = 0;
     if (cudaEventElapsedTime(&ms, h->ev_stage[0], h->ev_stage[6]) == cudaSuccess) out->stage_ms[6] = ms;
     if (cudaEventElapsedTime(&ms, h->ev_stage[7], h->ev_stage[8]) == cudaSuccess) out->stage_ms[7] = ms;
+    if (cudaEventElapsedTime(&ms, h->ev_stage[9], h->ev_stage[10]) == cudaSuccess) out->merge_ms = ms;
   }
   return TPC_OK;
 }
@@ -449,7 +488,7 @@ extern "C" int tpcRunHost(tpcHandle* h, int64_t N, const uint32_t* row_offset, c
   if (oh->link_up_raw || oh->link_dn_raw || oh->link_up || oh->link_dn || oh->start_hits || oh->tl_status || oh->tl_nhits ||
       oh->tl_first_row || oh->tl_last_row || oh->tl_rowhit || oh->tl_x || oh->tl_par || oh->tl_cov || oh->tl_chi2 ||
       oh->trk_rf_status || oh->trk_rf_x_in || oh->trk_rf_par_in || oh->trk_rf_cov_in || oh->trk_rf_chi2 || oh->trk_rf_x_out ||
-      oh->trk_rf_par_out || oh->trk_rf_cov_out)
+      oh->trk_rf_par_out || oh->trk_rf_cov_out || oh->trk_mg_next || oh->trk_mg_prev || oh->trk_mg_head || oh->trk_mg_chi2)
     return TPC_ERR_INVALID_ARG;
   if (!oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0) return TPC_ERR_INVALID_ARG;
   TPC_CUDA(h, cudaSetDevice(h->device));

@@ -1,0 +1,186 @@
+// tpc_merge.cuh -- a7: optional links between track segments (DESIGN.md section 3 "O7", readings R31..R33; NEXT-1 of
+// SURVEY.md 8(f); PAPER.md L92 stresses the merging and gives no method).
+//
+// A refitted track a (outer state) may continue in a refitted track b (inner state) of the same sector further out, or
+// of the azimuthal neighbour sector.  chi2(a, b) = diagonal chi2 of a's outer state -- rotated into b's frame if
+// needed, propagated to b's reference plane -- against b's inner state.  next(a) = admissible b of minimal (chi2, id),
+// prev(b) = admissible a of minimal (chi2, id); a link is kept when both agree.
+//
+// Organisation: the tracks are bucketed by (sector, first kept row) -- all b of a bucket share their reference plane,
+// so a is propagated once per candidate ROW, not once per pair.  One thread per a walks the admissible rows of the
+// three sectors; a pair whose y term alone exceeds the cut is dropped after three loads (the terms are non-negative,
+// so the sum could only be larger: no result changes).  prev(b) is an atomicMin over (chi2 bits, a).
+#pragma once
+#include "tpc_kalman.cuh"
+#include "tpc_refit.cuh"
+
+namespace tpc {
+
+struct MergeIn {            // refit outputs and track bookkeeping (device, SoA with stride cap)
+  int64_t cap;
+  const int32_t *status, *sector, *first_row, *last_row;
+  const float *x_in, *par_in, *cov_in, *x_out, *par_out, *cov_out;
+};
+struct MergeOut {
+  int32_t *next, *prev, *head;
+  float* chi2;
+};
+struct MergeParams {
+  int32_t max_row_gap, back_rows;
+  float chi2_max, ca, sa;    // ca, sa = (float)cos / sin of 20 degrees
+};
+
+// per track: clear the outputs, count the refitted tracks per (sector, first row)
+__global__ void __launch_bounds__(256) mergeCount(MergeIn in, MergeOut out, int n_rows, uint32_t* __restrict__ bucket_cnt,
+                                                  int32_t* __restrict__ best_b, unsigned long long* __restrict__ key_a,
+                                                  const int64_t* __restrict__ cnt) {
+  if (cnt[CNT_ERROR] != 0) return;
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= cnt[CNT_N_TRACKS] || k >= in.cap) return;
+  out.next[k] = -1; out.prev[k] = -1; out.head[k] = (int32_t)k; out.chi2[k] = 0.0f;
+  best_b[k] = -1; key_a[k] = ~0ull;
+  if (in.status[k] == 1) atomicAdd(bucket_cnt + in.sector[k] * n_rows + in.first_row[k], 1u);
+}
+
+// per track: its slot in the bucket list (order inside a bucket is arbitrary: every argmin below breaks ties by id)
+__global__ void __launch_bounds__(256) mergeFill(MergeIn in, int n_rows, const uint32_t* __restrict__ bucket_start,
+                                                 uint32_t* __restrict__ bucket_fill, uint32_t* __restrict__ list,
+                                                 const int64_t* __restrict__ cnt) {
+  if (cnt[CNT_ERROR] != 0) return;
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= cnt[CNT_N_TRACKS] || k >= in.cap || in.status[k] != 1) return;
+  const int b = in.sector[k] * n_rows + in.first_row[k];
+  list[bucket_start[b] + atomicAdd(bucket_fill + b, 1u)] = (uint32_t)k;
+}
+
+// O7 Rotate(alpha) with (ca, sa); returns false (state untouched) if |sin phi'| would reach max_sinphi
+__device__ __forceinline__ bool kfRotate(KFState& S, float ca, float sa, const DevParams& P) {
+  const float s = S.s, t = S.t;
+  const float c = sqrtf(1.0f - s * s);
+  const float s1 = s * ca - c * sa;
+  if (!(fabsf(s1) < P.max_sinphi)) return false;
+  const float c1 = sqrtf(1.0f - s1 * s1);
+  const float x1 = S.x * ca + S.y * sa;
+  const float y1 = S.y * ca - S.x * sa;
+  const float jy = c / c1, jz = -(sa * t) / c1, js = c1 / c, jq = -((S.q * P.b) * sa);
+  const float C00 = S.c00, C10 = S.c10, C11 = S.c11, C20 = S.c20, C21 = S.c21, C22 = S.c22, C30 = S.c30, C31 = S.c31,
+              C32 = S.c32, C40 = S.c40, C41 = S.c41, C42 = S.c42;
+  const float m2 = jq * C00 + js * C20;
+  S.c00 = (jy * jy) * C00;
+  S.c10 = jy * (jz * C00 + C10);
+  S.c11 = ((jz * jz) * C00 + (2.0f * jz) * C10) + C11;
+  S.c20 = jy * m2;
+  S.c21 = jz * m2 + (jq * C10 + js * C21);
+  S.c22 = ((jq * jq) * C00 + ((2.0f * jq) * js) * C20) + (js * js) * C22;
+  S.c30 = jy * C30;
+  S.c31 = jz * C30 + C31;
+  S.c32 = jq * C30 + js * C32;
+  S.c40 = jy * C40;
+  S.c41 = jz * C40 + C41;
+  S.c42 = jq * C40 + js * C42;
+  S.x = x1; S.y = y1; S.s = s1;
+  return true;
+}
+
+__device__ __forceinline__ KFState mergeLoad(int64_t k, int64_t cap, const float* __restrict__ x,
+                                             const float* __restrict__ par, const float* __restrict__ cov) {
+  KFState S{};
+  S.x = x[k];
+  S.y = par[0 * cap + k]; S.z = par[1 * cap + k]; S.s = par[2 * cap + k]; S.t = par[3 * cap + k]; S.q = par[4 * cap + k];
+  S.c00 = cov[0 * cap + k]; S.c10 = cov[1 * cap + k]; S.c11 = cov[2 * cap + k]; S.c20 = cov[3 * cap + k];
+  S.c21 = cov[4 * cap + k]; S.c22 = cov[5 * cap + k]; S.c30 = cov[6 * cap + k]; S.c31 = cov[7 * cap + k];
+  S.c32 = cov[8 * cap + k]; S.c33 = cov[9 * cap + k]; S.c40 = cov[10 * cap + k]; S.c41 = cov[11 * cap + k];
+  S.c42 = cov[12 * cap + k]; S.c43 = cov[13 * cap + k]; S.c44 = cov[14 * cap + k];
+  return S;
+}
+
+// one thread per track a: best continuation b of a, and a's bid for every admissible b
+__global__ void __launch_bounds__(128) mergeMatch(MergeIn in, DevParams P, RowTables T, MergeParams M,
+                                                  const uint32_t* __restrict__ bucket_start,
+                                                  const uint32_t* __restrict__ list, int32_t* __restrict__ best_b,
+                                                  float* __restrict__ chi_b, unsigned long long* __restrict__ key_a,
+                                                  const int64_t* __restrict__ cnt) {
+  if (cnt[CNT_ERROR] != 0) return;
+  const int64_t a = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (a >= cnt[CNT_N_TRACKS] || a >= in.cap || in.status[a] != 1) return;
+  const int64_t cap = in.cap;
+  const int R = P.n_rows;
+  const int sa_sec = in.sector[a], la = in.last_row[a];
+  const KFState A0 = mergeLoad(a, cap, in.x_out, in.par_out, in.cov_out);
+  int32_t bb = -1;
+  float bchi = 0.0f;
+  for (int rel = 0; rel <= 2; ++rel) {           // 0 same sector, 1 next sector (+20 degrees), 2 previous sector
+    int sb = sa_sec;
+    KFState Ar = A0;
+    if (rel != 0) {
+      if (P.n_sectors != 36) break;
+      const int side = sa_sec / 18, j = sa_sec - side * 18;
+      sb = side * 18 + (rel == 1 ? (j + 1) % 18 : (j + 17) % 18);
+      if (!kfRotate(Ar, M.ca, rel == 1 ? M.sa : -M.sa, P)) continue;
+    }
+    const int r_lo = max(0, la + (rel == 0 ? 1 : -M.back_rows)), r_hi = min(R - 1, la + M.max_row_gap);
+    for (int r = r_lo; r <= r_hi; ++r) {
+      const uint32_t k0 = bucket_start[sb * R + r], k1 = bucket_start[sb * R + r + 1];
+      if (k0 == k1) continue;
+      KFState S = Ar;
+      if (!kfPropagate(S, T.row_x[r], P, [](float, float, float, float) {})) continue;
+      for (uint32_t i = k0; i < k1; ++i) {
+        const int64_t b = list[i];
+        if (b == a) continue;
+        // the y term first: it alone decides for almost every pair of the bucket
+        const float den0 = S.c00 + in.cov_in[0 * cap + b];
+        if (!(den0 > 0.0f)) continue;
+        const float d0 = S.y - in.par_in[0 * cap + b];
+        float sum = 0.0f + (d0 * d0) / den0;
+        if (!(sum <= M.chi2_max)) continue;
+        const float pa[4] = {S.z, S.s, S.t, S.q};
+        const float ca[4] = {S.c11, S.c22, S.c33, S.c44};
+        const int ci[4] = {2, 5, 9, 14};
+        bool ok = true;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+          const float den = ca[q] + in.cov_in[ci[q] * cap + b];
+          if (!(den > 0.0f)) { ok = false; break; }
+          const float d = pa[q] - in.par_in[(q + 1) * cap + b];
+          sum = sum + (d * d) / den;
+        }
+        if (!ok || !(sum <= M.chi2_max)) continue;
+        if (bb < 0 || sum < bchi || (sum == bchi && (int32_t)b < bb)) { bb = (int32_t)b; bchi = sum; }
+        atomicMin(key_a + b, ((unsigned long long)__float_as_uint(sum) << 32) | (unsigned long long)(uint32_t)a);
+      }
+    }
+  }
+  best_b[a] = bb;
+  chi_b[a] = bchi;
+}
+
+// a link is kept when next(a) = b and prev(b) = a (R33)
+__global__ void __launch_bounds__(256) mergeLink(MergeIn in, MergeOut out, const int32_t* __restrict__ best_b,
+                                                 const float* __restrict__ chi_b,
+                                                 const unsigned long long* __restrict__ key_a,
+                                                 const int64_t* __restrict__ cnt) {
+  if (cnt[CNT_ERROR] != 0) return;
+  const int64_t a = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (a >= cnt[CNT_N_TRACKS] || a >= in.cap) return;
+  const int32_t b = best_b[a];
+  if (b >= 0 && (uint32_t)(key_a[b] & 0xffffffffull) == (uint32_t)a) {
+    out.next[a] = b; out.prev[b] = (int32_t)a; out.chi2[a] = chi_b[a];
+  }
+}
+
+// head(k) = first track of k's chain (chains are a handful of segments long)
+__global__ void __launch_bounds__(256) mergeHead(MergeIn in, MergeOut out, const int64_t* __restrict__ cnt) {
+  if (cnt[CNT_ERROR] != 0) return;
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t nt = min(cnt[CNT_N_TRACKS], in.cap);
+  if (k >= nt) return;
+  int64_t h = k;
+  for (int64_t guard = 0; guard < nt; ++guard) {
+    const int32_t p = out.prev[h];
+    if (p < 0) break;
+    h = p;
+  }
+  out.head[k] = (int32_t)h;
+}
+
+}  // namespace tpc
