@@ -217,15 +217,18 @@ def run_ours(args, rank, world, local_rank):
     stage /= args.steps
 
     # ---- the NEXT-2 row (a6 refit of the selected tracks), timed apart: it is not part of the a1..a5 step ----------
-    refit_ms = None
+    refit_ms = merge_ms = None
+    n_links = 0
     if not args.no_refit:
-        acc = 0.0
+        acc = accm = 0.0
         for i in range(4):
-            trk.run(off, y, z, cap_tracklets=capT, cap_tracks=capK, cap_track_clusters=capC, sync=False, refit=True)
+            trk.run(off, y, z, cap_tracklets=capT, cap_tracks=capK, cap_track_clusters=capC, sync=False, merge=True)
             s = trk.status()
             if i > 0:
                 acc += float(s.stage_ms[7])
-        refit_ms = acc / 3
+                accm += float(s.merge_ms)
+        refit_ms, merge_ms = acc / 3, accm / 3
+        n_links = int((trk._out["trk_mg_next"][:int(s.n_tracks)] >= 0).sum().item())
 
     # ---- end to end through the host-buffer ABI call (pinned host memory; copies inside the timed region) ----
     hy = torch.from_numpy(ev.y).pin_memory()
@@ -316,6 +319,8 @@ def run_ours(args, rank, world, local_rank):
         line["next_refit"] = {"what": "a6 refit of the selected tracks (NEXT-2), not part of `value`", "ms": round(refit_ms, 4),
                               "alg_bytes": rb, "gbs": round(rb / (refit_ms * 1e-3) / 1e9, 1) if refit_ms > 0 else None,
                               "tracks": int(st.n_tracks), "track_clusters": ncl}
+        line["next_merge"] = {"what": "a7 segment merger (NEXT-1), not part of `value`", "ms": round(merge_ms, 4),
+                              "links": n_links}
     print(json.dumps(line), flush=True)
 
 

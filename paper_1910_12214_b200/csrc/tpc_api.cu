@@ -47,7 +47,8 @@ struct Workspace {
   int32_t *kept_first, *kept_last;
   unsigned long long* owner_key;
   uint32_t* owner_id;
-  uint32_t *mg_start, *mg_fill, *mg_list;   // merger: tracks bucketed by (sector, first row)
+  uint32_t *mg_start, *mg_fill, *mg_list;   // merger: tracks bucketed by (sector, first row, z bin, y bin)
+  uint32_t* mg_maxv;         // [2][n_buckets] largest inner variances of a (sector, row)
   int32_t* mg_best_b;
   float* mg_chi_b;
   unsigned long long* mg_key_a;
@@ -141,8 +142,10 @@ Workspace layout(const tpcHandle* h, int64_t N, int64_t capT, char* base) {
   w.kept_last = (int32_t*)take(4 * (size_t)Tn);
   w.owner_key = (unsigned long long*)take(8 * (size_t)Nn);
   w.owner_id = (uint32_t*)take(4 * (size_t)Nn);
-  w.mg_start = (uint32_t*)take(4 * (size_t)(nb + 1));
-  w.mg_fill = (uint32_t*)take(4 * (size_t)(nb + 1));
+  const size_t mgb = (size_t)nb * MG_NYB * MG_NZB + 1;
+  w.mg_start = (uint32_t*)take(4 * mgb);
+  w.mg_fill = (uint32_t*)take(4 * mgb);
+  w.mg_maxv = (uint32_t*)take(8 * (size_t)nb);
   w.mg_list = (uint32_t*)take(4 * (size_t)Tn);
   w.mg_best_b = (int32_t*)take(4 * (size_t)Tn);
   w.mg_chi_b = (float*)take(4 * (size_t)Tn);
@@ -389,13 +392,15 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
     const MergeParams mp{h->params.merge_max_row_gap, h->params.merge_back_rows, h->params.merge_chi2_max,
                          (float)cos(0.3490658503988659), (float)sin(0.3490658503988659)};
     const unsigned gK = (unsigned)ceilDiv(nk, 256);
-    TPC_CUDA(h, cudaMemsetAsync(w.mg_start, 0, 4 * (size_t)(nb + 1), st)); ++L;
-    TPC_CUDA(h, cudaMemsetAsync(w.mg_fill, 0, 4 * (size_t)(nb + 1), st)); ++L;
-    mergeCount<<<gK, 256, 0, st>>>(mi, mo, P.n_rows, w.mg_start, w.mg_best_b, w.mg_key_a, cnt); ++L;
-    scanArrayInPlace<uint32_t><<<1, 1024, 0, st>>>(w.mg_start, (int64_t)nb + 1, nullptr); ++L;
-    mergeFill<<<gK, 256, 0, st>>>(mi, P.n_rows, w.mg_start, w.mg_fill, w.mg_list, cnt); ++L;
-    mergeMatch<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(mi, P, T, mp, w.mg_start, w.mg_list, w.mg_best_b, w.mg_chi_b,
-                                                           w.mg_key_a, cnt); ++L;
+    const size_t mgb = (size_t)nb * MG_NYB * MG_NZB + 1;
+    TPC_CUDA(h, cudaMemsetAsync(w.mg_start, 0, 4 * mgb, st)); ++L;
+    TPC_CUDA(h, cudaMemsetAsync(w.mg_fill, 0, 4 * mgb, st)); ++L;
+    TPC_CUDA(h, cudaMemsetAsync(w.mg_maxv, 0, 8 * (size_t)nb, st)); ++L;
+    mergeCount<<<gK, 256, 0, st>>>(mi, mo, P, T, w.mg_start, w.mg_maxv, w.mg_best_b, w.mg_key_a, cnt); ++L;
+    scanArrayInPlace<uint32_t><<<1, 1024, 0, st>>>(w.mg_start, (int64_t)mgb, nullptr); ++L;
+    mergeFill<<<gK, 256, 0, st>>>(mi, P, T, w.mg_start, w.mg_fill, w.mg_list, cnt); ++L;
+    mergeMatch<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(mi, P, T, mp, w.mg_start, w.mg_maxv, w.mg_list, w.mg_best_b,
+                                                           w.mg_chi_b, w.mg_key_a, cnt); ++L;
     mergeLink<<<gK, 256, 0, st>>>(mi, mo, w.mg_best_b, w.mg_chi_b, w.mg_key_a, cnt); ++L;
     mergeHead<<<gK, 256, 0, st>>>(mi, mo, cnt); ++L;
   }

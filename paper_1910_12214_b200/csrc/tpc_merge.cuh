@@ -6,10 +6,11 @@
 // needed, propagated to b's reference plane -- against b's inner state.  next(a) = admissible b of minimal (chi2, id),
 // prev(b) = admissible a of minimal (chi2, id); a link is kept when both agree.
 //
-// Organisation: the tracks are bucketed by (sector, first kept row) -- all b of a bucket share their reference plane,
-// so a is propagated once per candidate ROW, not once per pair.  One thread per a walks the admissible rows of the
-// three sectors; a pair whose y term alone exceeds the cut is dropped after three loads (the terms are non-negative,
-// so the sum could only be larger: no result changes).  prev(b) is an atomicMin over (chi2 bits, a).
+// Organisation: the tracks are bucketed by (sector, first kept row, z bin, y bin of their inner state) -- all b of a
+// (sector, row) share their reference plane, so a is propagated once per candidate ROW, not once per pair, and only the
+// bins that can hold a b whose y or z term alone stays below the cut are visited: the terms are non-negative, so the
+// sum could only be larger, and the window uses the largest inner variances of the row (plus rounding slack), so it is a
+// superset of every admissible b -- no result changes (same argument as R3).  prev(b) is an atomicMin over (chi2 bits, a).
 #pragma once
 #include "tpc_kalman.cuh"
 #include "tpc_refit.cuh"
@@ -25,13 +26,23 @@ struct MergeOut {
   int32_t *next, *prev, *head;
   float* chi2;
 };
+constexpr int MG_NYB = 32, MG_NZB = 16;     // y / z bins of the inner states per (sector, row)
+
+__device__ __forceinline__ int mergeBucket(int sr, float y, float z, float x_row, const DevParams& P) {
+  const float hw = x_row * P.tan_half_sector;
+  const int by = cellCoord(y, -hw, (float)MG_NYB / (2.0f * hw), MG_NYB);
+  const int bz = cellCoord(z, P.z_min, (float)MG_NZB / (P.z_max - P.z_min), MG_NZB);
+  return (sr * MG_NZB + bz) * MG_NYB + by;
+}
+
 struct MergeParams {
   int32_t max_row_gap, back_rows;
   float chi2_max, ca, sa;    // ca, sa = (float)cos / sin of 20 degrees
 };
 
 // per track: clear the outputs, count the refitted tracks per (sector, first row)
-__global__ void __launch_bounds__(256) mergeCount(MergeIn in, MergeOut out, int n_rows, uint32_t* __restrict__ bucket_cnt,
+__global__ void __launch_bounds__(256) mergeCount(MergeIn in, MergeOut out, DevParams P, RowTables T,
+                                                  uint32_t* __restrict__ bucket_cnt, uint32_t* __restrict__ max_var,
                                                   int32_t* __restrict__ best_b, unsigned long long* __restrict__ key_a,
                                                   const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
@@ -39,17 +50,24 @@ __global__ void __launch_bounds__(256) mergeCount(MergeIn in, MergeOut out, int 
   if (k >= cnt[CNT_N_TRACKS] || k >= in.cap) return;
   out.next[k] = -1; out.prev[k] = -1; out.head[k] = (int32_t)k; out.chi2[k] = 0.0f;
   best_b[k] = -1; key_a[k] = ~0ull;
-  if (in.status[k] == 1) atomicAdd(bucket_cnt + in.sector[k] * n_rows + in.first_row[k], 1u);
+  if (in.status[k] == 1) {
+    const int r = in.first_row[k], sr = in.sector[k] * P.n_rows + r;
+    atomicAdd(bucket_cnt + mergeBucket(sr, in.par_in[k], in.par_in[in.cap + k], T.row_x[r], P), 1u);
+    // largest inner variances of the (sector, row): positive floats order like their bit patterns
+    atomicMax(max_var + 2 * sr, __float_as_uint(in.cov_in[k]));
+    atomicMax(max_var + 2 * sr + 1, __float_as_uint(in.cov_in[2 * in.cap + k]));
+  }
 }
 
 // per track: its slot in the bucket list (order inside a bucket is arbitrary: every argmin below breaks ties by id)
-__global__ void __launch_bounds__(256) mergeFill(MergeIn in, int n_rows, const uint32_t* __restrict__ bucket_start,
+__global__ void __launch_bounds__(256) mergeFill(MergeIn in, DevParams P, RowTables T, const uint32_t* __restrict__ bucket_start,
                                                  uint32_t* __restrict__ bucket_fill, uint32_t* __restrict__ list,
                                                  const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= cnt[CNT_N_TRACKS] || k >= in.cap || in.status[k] != 1) return;
-  const int b = in.sector[k] * n_rows + in.first_row[k];
+  const int r = in.first_row[k];
+  const int b = mergeBucket(in.sector[k] * P.n_rows + r, in.par_in[k], in.par_in[in.cap + k], T.row_x[r], P);
   list[bucket_start[b] + atomicAdd(bucket_fill + b, 1u)] = (uint32_t)k;
 }
 
@@ -97,6 +115,7 @@ __device__ __forceinline__ KFState mergeLoad(int64_t k, int64_t cap, const float
 // one thread per track a: best continuation b of a, and a's bid for every admissible b
 __global__ void __launch_bounds__(128) mergeMatch(MergeIn in, DevParams P, RowTables T, MergeParams M,
                                                   const uint32_t* __restrict__ bucket_start,
+                                                  const uint32_t* __restrict__ max_var,
                                                   const uint32_t* __restrict__ list, int32_t* __restrict__ best_b,
                                                   float* __restrict__ chi_b, unsigned long long* __restrict__ key_a,
                                                   const int64_t* __restrict__ cnt) {
@@ -120,10 +139,23 @@ __global__ void __launch_bounds__(128) mergeMatch(MergeIn in, DevParams P, RowTa
     }
     const int r_lo = max(0, la + (rel == 0 ? 1 : -M.back_rows)), r_hi = min(R - 1, la + M.max_row_gap);
     for (int r = r_lo; r <= r_hi; ++r) {
-      const uint32_t k0 = bucket_start[sb * R + r], k1 = bucket_start[sb * R + r + 1];
-      if (k0 == k1) continue;
+      const int sr = sb * R + r;
+      const float vy = __uint_as_float(max_var[2 * sr]);
+      if (vy == 0.0f) continue;                    // no refitted track starts on this (sector, row)
       KFState S = Ar;
-      if (!kfPropagate(S, T.row_x[r], P, [](float, float, float, float) {})) continue;
+      const float xr = T.row_x[r];
+      if (!kfPropagate(S, xr, P, [](float, float, float, float) {})) continue;
+      // bins that can hold an admissible b: |dy| <= sqrt(chi2_max * (C00 + max C00_b)), likewise z (with slack)
+      const float wy = sqrtf(M.chi2_max * (S.c00 + vy)) * 1.0001f + 1e-6f;
+      const float wz = sqrtf(M.chi2_max * (S.c11 + __uint_as_float(max_var[2 * sr + 1]))) * 1.0001f + 1e-6f;
+      if (!(wy >= 0.0f) || !(wz >= 0.0f)) continue;      // a non-positive variance of a: every denominator test fails below anyway
+      const float hw = xr * P.tan_half_sector;
+      const float iby = (float)MG_NYB / (2.0f * hw), ibz = (float)MG_NZB / (P.z_max - P.z_min);
+      const int by0 = cellCoord(S.y - wy, -hw, iby, MG_NYB), by1 = cellCoord(S.y + wy, -hw, iby, MG_NYB);
+      const int bz0 = cellCoord(S.z - wz, P.z_min, ibz, MG_NZB), bz1 = cellCoord(S.z + wz, P.z_min, ibz, MG_NZB);
+      for (int bz = bz0; bz <= bz1; ++bz) {
+      const uint32_t* row = bucket_start + (sr * MG_NZB + bz) * MG_NYB;
+      const uint32_t k0 = row[by0], k1 = row[by1 + 1];
       for (uint32_t i = k0; i < k1; ++i) {
         const int64_t b = list[i];
         if (b == a) continue;
@@ -147,6 +179,7 @@ __global__ void __launch_bounds__(128) mergeMatch(MergeIn in, DevParams P, RowTa
         if (!ok || !(sum <= M.chi2_max)) continue;
         if (bb < 0 || sum < bchi || (sum == bchi && (int32_t)b < bb)) { bb = (int32_t)b; bchi = sum; }
         atomicMin(key_a + b, ((unsigned long long)__float_as_uint(sum) << 32) | (unsigned long long)(uint32_t)a);
+      }
       }
     }
   }
