@@ -49,6 +49,8 @@ struct Workspace {
   uint32_t* owner_id;
   uint32_t *mg_start, *mg_fill, *mg_list;   // merger: tracks bucketed by (sector, first row, z bin, y bin)
   uint32_t* mg_maxv;         // [2][n_buckets] largest inner variances of a (sector, row)
+  uint32_t* mg_tiles;        // tile sums of the bucket scan
+  uint32_t *rf_hist, *rf_fill, *rf_order;   // refit: tracks ordered by length
   int32_t* mg_best_b;
   float* mg_chi_b;
   unsigned long long* mg_key_a;
@@ -146,7 +148,11 @@ Workspace layout(const tpcHandle* h, int64_t N, int64_t capT, char* base) {
   w.mg_start = (uint32_t*)take(4 * mgb);
   w.mg_fill = (uint32_t*)take(4 * mgb);
   w.mg_maxv = (uint32_t*)take(8 * (size_t)nb);
+  w.mg_tiles = (uint32_t*)take(4 * (size_t)(ceilDiv((int64_t)mgb, SCAN_TILE) + 2));
   w.mg_list = (uint32_t*)take(4 * (size_t)Tn);
+  w.rf_hist = (uint32_t*)take(4 * (size_t)(RF_BINS + 1));
+  w.rf_fill = (uint32_t*)take(4 * (size_t)(RF_BINS + 1));
+  w.rf_order = (uint32_t*)take(4 * (size_t)Tn);
   w.mg_best_b = (int32_t*)take(4 * (size_t)Tn);
   w.mg_chi_b = (float*)take(4 * (size_t)Tn);
   w.mg_key_a = (unsigned long long*)take(8 * (size_t)Tn);
@@ -378,7 +384,12 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
     const RefitOut rf{out->trk_rf_status, out->trk_rf_x_in, out->trk_rf_par_in, out->trk_rf_cov_in, out->trk_rf_chi2,
                       out->trk_rf_x_out, out->trk_rf_par_out, out->trk_rf_cov_out};
     const int64_t nk = std::min<int64_t>(out->cap_tracks, capT);
-    refitTracks<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(in->row_offset, in->y, in->z, P, T, to, rf, cnt); ++L;
+    TPC_CUDA(h, cudaMemsetAsync(w.rf_hist, 0, 4 * (size_t)(RF_BINS + 1), st)); ++L;
+    TPC_CUDA(h, cudaMemsetAsync(w.rf_fill, 0, 4 * (size_t)(RF_BINS + 1), st)); ++L;
+    refitCount<<<(unsigned)ceilDiv(nk, 256), 256, 0, st>>>(to, w.rf_hist, cnt); ++L;
+    scanArrayInPlace<uint32_t><<<1, 1024, 0, st>>>(w.rf_hist, (int64_t)RF_BINS + 1, nullptr); ++L;
+    refitFill<<<(unsigned)ceilDiv(nk, 256), 256, 0, st>>>(to, w.rf_hist, w.rf_fill, w.rf_order, cnt); ++L;
+    refitTracks<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(in->row_offset, w.rf_order, in->y, in->z, P, T, to, rf, cnt); ++L;
   }
   stage(8);
   // ---- a7 optional links between track segments (O7) -------------------------------------------------
@@ -397,7 +408,13 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
     TPC_CUDA(h, cudaMemsetAsync(w.mg_fill, 0, 4 * mgb, st)); ++L;
     TPC_CUDA(h, cudaMemsetAsync(w.mg_maxv, 0, 8 * (size_t)nb, st)); ++L;
     mergeCount<<<gK, 256, 0, st>>>(mi, mo, P, T, w.mg_start, w.mg_maxv, w.mg_best_b, w.mg_key_a, cnt); ++L;
-    scanArrayInPlace<uint32_t><<<1, 1024, 0, st>>>(w.mg_start, (int64_t)mgb, nullptr); ++L;
+    {   // exclusive scan of the bucket counts; the closing sentinel lands on the last (spare) entry
+      const int64_t nscan = (int64_t)mgb - 1;
+      const unsigned tiles = (unsigned)ceilDiv(nscan, SCAN_TILE);
+      scanTileSums<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.mg_start, cnt + CNT_INF, nscan, w.mg_tiles); ++L;
+      scanTileOffsets<uint32_t><<<1, 1024, 0, st>>>(w.mg_tiles, cnt + CNT_INF, nscan, nullptr); ++L;
+      scanApply<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.mg_start, w.mg_start, cnt + CNT_INF, nscan, w.mg_tiles); ++L;
+    }
     mergeFill<<<gK, 256, 0, st>>>(mi, P, T, w.mg_start, w.mg_fill, w.mg_list, cnt); ++L;
     mergeMatch<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(mi, P, T, mp, w.mg_start, w.mg_maxv, w.mg_list, w.mg_best_b,
                                                            w.mg_chi_b, w.mg_key_a, cnt); ++L;

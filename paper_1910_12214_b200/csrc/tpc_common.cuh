@@ -42,7 +42,8 @@ enum Counter {
   CNT_N_CELLS = 6,
   CNT_WORK = 7,         // dynamic work counter of the constructor
   CNT_N_LONG = 8,       // seeds whose link chain is long enough to survive the chain fit (the constructor's work list)
-  CNT_COUNT = 9
+  CNT_INF = 9,          // a count larger than any array: "scan everything" for the device-counted scan kernels
+  CNT_COUNT = 10
 };
 
 // Tracklet SoA in the workspace (capT = capacity in tracklets).

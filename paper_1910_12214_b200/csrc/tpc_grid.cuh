@@ -17,7 +17,7 @@ __global__ void __launch_bounds__(1024) gridSetup(const uint32_t* __restrict__ o
   __shared__ uint32_t sm[33];
   __shared__ int bad;
   const int nb = P.n_buckets;
-  if (threadIdx.x == 0) bad = (off[0] != 0u) || ((int64_t)off[nb] != N);
+  if (threadIdx.x == 0) { bad = (off[0] != 0u) || ((int64_t)off[nb] != N); cnt[CNT_INF] = (int64_t)1 << 62; }
   __syncthreads();
   for (int b = threadIdx.x; b < nb; b += blockDim.x)
     if (off[b + 1] < off[b]) bad = 1;

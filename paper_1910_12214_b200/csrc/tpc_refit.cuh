@@ -28,12 +28,34 @@ __device__ __forceinline__ void refitStore(const KFState& S, int64_t k, int64_t 
   cov[12 * cap + k] = S.c42; cov[13 * cap + k] = S.c43; cov[14 * cap + k] = S.c44;
 }
 
-__global__ void __launch_bounds__(128) refitTracks(const uint32_t* __restrict__ off, const float* __restrict__ y,
+// Tracks are refitted in the order of their length (longest first), so that the 32 tracks of a warp need about the same
+// number of steps: histogram of the lengths, exclusive scan (scanArrayInPlace), slots.  Order inside a length is arbitrary.
+constexpr int RF_BINS = 256;
+__device__ __forceinline__ int refitBin(uint32_t n) { return RF_BINS - 1 - (int)min(n, (uint32_t)(RF_BINS - 1)); }
+
+__global__ void __launch_bounds__(256) refitCount(TrackOut o, uint32_t* __restrict__ hist, const int64_t* __restrict__ cnt) {
+  if (cnt[CNT_ERROR] != 0) return;
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= cnt[CNT_N_TRACKS] || k >= o.cap_tracks) return;
+  atomicAdd(hist + refitBin(o.cl_offset[k + 1] - o.cl_offset[k]), 1u);
+}
+
+__global__ void __launch_bounds__(256) refitFill(TrackOut o, const uint32_t* __restrict__ start, uint32_t* __restrict__ fill,
+                                                 uint32_t* __restrict__ order, const int64_t* __restrict__ cnt) {
+  if (cnt[CNT_ERROR] != 0) return;
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= cnt[CNT_N_TRACKS] || k >= o.cap_tracks) return;
+  const int b = refitBin(o.cl_offset[k + 1] - o.cl_offset[k]);
+  order[start[b] + atomicAdd(fill + b, 1u)] = (uint32_t)k;
+}
+
+__global__ void __launch_bounds__(128) refitTracks(const uint32_t* __restrict__ off, const uint32_t* __restrict__ order, const float* __restrict__ y,
                                                    const float* __restrict__ z, DevParams P, RowTables T, TrackOut o,
                                                    RefitOut rf, const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;               // truncated cluster lists cannot be refitted
-  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (k >= cnt[CNT_N_TRACKS] || k >= o.cap_tracks) return;
+  const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= cnt[CNT_N_TRACKS] || j >= o.cap_tracks) return;
+  const int64_t k = order[j];
   const int64_t cap = o.cap_tracks;
   const uint32_t lo = o.cl_offset[k], hi = o.cl_offset[k + 1];
   const int n = (int)(hi - lo);
