@@ -112,6 +112,8 @@ __device__ __forceinline__ KFState mergeLoad(int64_t k, int64_t cap, const float
   return S;
 }
 
+__device__ __forceinline__ int64_t live_guard(int64_t a, int64_t cap) { return a < cap ? a : 0; }
+
 // one thread per track a: best continuation b of a, and a's bid for every admissible b
 __global__ void __launch_bounds__(128) mergeMatch(MergeIn in, DevParams P, RowTables T, MergeParams M,
                                                   const uint32_t* __restrict__ bucket_start,
@@ -121,30 +123,39 @@ __global__ void __launch_bounds__(128) mergeMatch(MergeIn in, DevParams P, RowTa
                                                   const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
   const int64_t a = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (a >= cnt[CNT_N_TRACKS] || a >= in.cap || in.status[a] != 1) return;
+  // Lanes without a track stay in the loops (predicated off): the row loop below has the same trip count for every
+  // lane and reconverges at __syncwarp(), so the 32 lanes run the Propagate of a row together.
+  const bool live = a < cnt[CNT_N_TRACKS] && a < in.cap && in.status[live_guard(a, in.cap)] == 1;
   const int64_t cap = in.cap;
   const int R = P.n_rows;
-  const int sa_sec = in.sector[a], la = in.last_row[a];
-  const KFState A0 = mergeLoad(a, cap, in.x_out, in.par_out, in.cov_out);
+  const int sa_sec = live ? in.sector[a] : 0, la = live ? in.last_row[a] : 0;
+  KFState A0{};
+  if (live) A0 = mergeLoad(a, cap, in.x_out, in.par_out, in.cov_out);
   int32_t bb = -1;
   float bchi = 0.0f;
+  const int n_it = M.back_rows + M.max_row_gap + 1;      // rows la - back_rows .. la + max_row_gap
   for (int rel = 0; rel <= 2; ++rel) {           // 0 same sector, 1 next sector (+20 degrees), 2 previous sector
+    if (rel != 0 && P.n_sectors != 36) break;    // uniform
     int sb = sa_sec;
     KFState Ar = A0;
+    bool rel_ok = live;
     if (rel != 0) {
-      if (P.n_sectors != 36) break;
       const int side = sa_sec / 18, j = sa_sec - side * 18;
       sb = side * 18 + (rel == 1 ? (j + 1) % 18 : (j + 17) % 18);
-      if (!kfRotate(Ar, M.ca, rel == 1 ? M.sa : -M.sa, P)) continue;
+      rel_ok = live && kfRotate(Ar, M.ca, rel == 1 ? M.sa : -M.sa, P);
     }
     const int r_lo = max(0, la + (rel == 0 ? 1 : -M.back_rows)), r_hi = min(R - 1, la + M.max_row_gap);
-    for (int r = r_lo; r <= r_hi; ++r) {
-      const int sr = sb * R + r;
-      const float vy = __uint_as_float(max_var[2 * sr]);
-      if (vy == 0.0f) continue;                    // no refitted track starts on this (sector, row)
+    for (int it = 0; it < n_it; ++it) {
+      __syncwarp();
+      const int r = la - M.back_rows + it;
+      bool act = rel_ok && r >= r_lo && r <= r_hi;
+      const int sr = act ? sb * R + r : 0;
+      const float vy = act ? __uint_as_float(max_var[2 * sr]) : 0.0f;
+      act = act && vy != 0.0f;                     // no refitted track starts on this (sector, row)
       KFState S = Ar;
-      const float xr = T.row_x[r];
-      if (!kfPropagate(S, xr, P, [](float, float, float, float) {})) continue;
+      const float xr = T.row_x[act ? r : 0];
+      const bool okp = kfPropagate(S, act ? xr : S.x, P, [](float, float, float, float) {});
+      if (!(act && okp)) continue;
       // bins that can hold an admissible b: |dy| <= sqrt(chi2_max * (C00 + max C00_b)), likewise z (with slack)
       const float wy = sqrtf(M.chi2_max * (S.c00 + vy)) * 1.0001f + 1e-6f;
       const float wz = sqrtf(M.chi2_max * (S.c11 + __uint_as_float(max_var[2 * sr + 1]))) * 1.0001f + 1e-6f;
@@ -183,8 +194,7 @@ __global__ void __launch_bounds__(128) mergeMatch(MergeIn in, DevParams P, RowTa
       }
     }
   }
-  best_b[a] = bb;
-  chi_b[a] = bchi;
+  if (live) { best_b[a] = bb; chi_b[a] = bchi; }
 }
 
 // a link is kept when next(a) = b and prev(b) = a (R33)
