@@ -235,18 +235,33 @@ def run_ours(args, rank, world, local_rank):
     hz = torch.from_numpy(ev.z).pin_memory()
     hoff = torch.from_numpy(ev.row_offset.view(np.int32)).pin_memory()
     ny, nz, noff = hy.numpy(), hz.numpy(), hoff.numpy().view(np.uint32)
-    e2e_steps = max(1, min(args.steps, 5))
-    sth, outh = trk.run_host(noff, ny, nz, cap_tracks=capK, cap_track_clusters=capC)     # warm-up: pools grow here
+    e2e_steps = max(2, min(args.steps, 10))
+    sth, outh = trk.run_host(noff, ny, nz, cap_tracks=capK, cap_track_clusters=capC)     # warm-up: pools and hints grow here
     assert sth.status == 0
+    # Double-buffered: the copies of one event overlap the kernels of the other (tpcSubmitHost / tpcCollectHost).  Every
+    # step still copies its inputs from pinned host memory and its tracks back to the host inside the timed region.
+    for w in range(2):
+        trk.submit_host(w, noff, ny, nz, capK, capC)
+    for w in range(2):
+        sth, outh = trk.collect_host(w)                # warm-up of both slots (their pools are allocated here)
+        assert sth.status == 0
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
+    t_e2e = time.perf_counter()
     e0.record(stream)
-    for _ in range(e2e_steps):
-        sth, outh = trk.run_host(noff, ny, nz, cap_tracks=capK, cap_track_clusters=capC)
+    trk.submit_host(0, noff, ny, nz, capK, capC)
+    for i in range(e2e_steps):
+        if i + 1 < e2e_steps:
+            trk.submit_host((i + 1) % 2, noff, ny, nz, capK, capC)
+        sth, outh = trk.collect_host(i % 2)
+        assert sth.status == 0
     e1.record(stream)
     torch.cuda.synchronize()
-    _, ms_e2e = aggregate(float(N), e0.elapsed_time(e1) / e2e_steps, torch.device("cuda", local_rank), world)
+    wall_e2e = (time.perf_counter() - t_e2e) * 1e3 / e2e_steps
+    # the slots run on the library's own streams: the host clock around submit ... collect is the measure (the events on
+    # torch's stream only bracket it); max over ranks as for `value`
+    _, ms_e2e = aggregate(float(N), max(wall_e2e, e0.elapsed_time(e1) / e2e_steps), torch.device("cuda", local_rank), world)
     e2e_value = total_clusters / (ms_e2e * 1e-3)
     nt, nc = int(sth.n_tracks), int(sth.n_track_clusters)
     h2d = 4 * (len(ev.row_offset)) + 8 * N
@@ -310,7 +325,7 @@ def run_ours(args, rank, world, local_rank):
                        "tracklets_per_step": nT, "start_hits_per_step": int(st.n_start_hits), "tracklet_hits": H},
             "tracks_per_s": float(st.n_tracks) * world / (ms_step * 1e-3),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
-                    "ms_per_step": ms_e2e, "steps": e2e_steps},
+                    "ms_per_step": ms_e2e, "steps": e2e_steps, "how": "tpcSubmitHost/tpcCollectHost, 2 slots, pinned host buffers"},
             "gpu_launches": int(st.kernel_launches) * args.steps,
             "clocks": clocks, "roofline": roofline, "stages": stages, "cpu_baseline": cpu}
     if refit_ms is not None:

@@ -181,6 +181,17 @@ int tpcSetProfiling(tpcHandle* h, int on);
 int tpcRunHost(tpcHandle* h, int64_t n_clusters, const uint32_t* row_offset, const float* y, const float* z,
                tpcTracks* out_host, tpcRunStatus* status, void* cuda_stream);
 
+/* Double-buffered form of tpcRunHost for a stream of events: tpcSubmitHost(slot) enqueues the copies in, a1..a5 and
+ * the copies out of one event on the slot's own stream and returns at once; tpcCollectHost(slot) waits for it and
+ * reports its status.  slot is 0 or 1, so that the copies of one event overlap the kernels of the other.  The HOST
+ * buffers (inputs and the arrays of `out_host`, pinned for real overlap) must stay valid and untouched until the
+ * collect.  The counts are not known at submit time: up to min(capacity of the handle's device buffers, capacity of
+ * out_host) entries are copied back and tpcRunStatus says how many are valid.  status TPC_ERR_CAPACITY = a capacity
+ * was too small (first events of a stream): run that event again with tpcRunHost, which grows the buffers. */
+int tpcSubmitHost(tpcHandle* h, int slot, int64_t n_clusters, const uint32_t* row_offset, const float* y, const float* z,
+                  const tpcTracks* out_host);
+int tpcCollectHost(tpcHandle* h, int slot, tpcRunStatus* status);
+
 const char* tpcErrorString(int code);
 const char* tpcLastCudaError(const tpcHandle* h);
 

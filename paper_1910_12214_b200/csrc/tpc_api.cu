@@ -82,6 +82,19 @@ struct tpcHandle {
   void* pool[16] = {};
   size_t pool_bytes[16] = {};
   int64_t hint_T = 0, hint_K = 0, hint_C = 0;   // capacities the last tpcRunHost needed (+ head-room)
+  // The per-run state above (d_cnt, h_cnt, ev_done, launches, pending, last_n, pool, pool_bytes) is the ACTIVE slot's;
+  // tpcSubmitHost / tpcCollectHost keep two more copies of it (double buffering) and swap them in and out.
+  struct Slot {
+    bool init = false;
+    int64_t* d_cnt = nullptr; int64_t* h_cnt = nullptr; cudaEvent_t ev_done = nullptr;
+    int launches = 0; bool pending = false; int64_t last_n = 0;
+    void* pool[16] = {}; size_t pool_bytes[16] = {};
+    cudaStream_t stream = nullptr;
+    bool submitted = false;
+    int64_t capK = 0, capC = 0;      // device capacities of the submitted run
+    tpcTracks oh{};                  // host outputs of the submitted run
+  } slots[3];
+  int cur_slot = 0;
 };
 
 namespace {
@@ -255,6 +268,14 @@ int tpcDestroy(tpcHandle* h) {
   if (h->h_cnt) cudaFreeHost(h->h_cnt);
   if (h->ev_done) cudaEventDestroy(h->ev_done);
   for (int i = 0; i < 11; ++i) if (h->ev_stage[i]) cudaEventDestroy(h->ev_stage[i]);
+  if (h->cur_slot != 0) {}   // the active state is freed below; the parked slots here
+  for (int k = 0; k < 3; ++k) {
+    if (k == h->cur_slot || !h->slots[k].init) continue;
+    tpcHandle::Slot& S = h->slots[k];
+    cudaFree(S.d_cnt); if (S.h_cnt) cudaFreeHost(S.h_cnt); if (S.ev_done) cudaEventDestroy(S.ev_done);
+    for (int i = 0; i < 16; ++i) if (S.pool[i]) cudaFree(S.pool[i]);
+  }
+  for (int k = 1; k < 3; ++k) if (h->slots[k].stream) cudaStreamDestroy(h->slots[k].stream);
   for (int i = 0; i < 16; ++i) if (h->pool[i]) cudaFree(h->pool[i]);
   delete h;
   return TPC_OK;
@@ -583,4 +604,118 @@ extern "C" int tpcRunHost(tpcHandle* h, int64_t N, const uint32_t* row_offset, c
   if (status->status == TPC_OK) TPC_CUDA(h, back(oh->trk_cl_index, od.trk_cl_index, 4 * (size_t)nc));
   TPC_CUDA(h, cudaStreamSynchronize(st));
   return TPC_OK;
+}
+
+// ---- double-buffered host path: tpcSubmitHost / tpcCollectHost -------------------------------------------------
+namespace {
+// make slot `s` the active per-run state of the handle (0 = the synchronous path, 1 / 2 = the two pipeline slots)
+int useSlot(tpcHandle* h, int s) {
+  if (s == h->cur_slot) return TPC_OK;
+  tpcHandle::Slot& o = h->slots[h->cur_slot];
+  o.init = true;
+  o.d_cnt = h->d_cnt; o.h_cnt = h->h_cnt; o.ev_done = h->ev_done; o.launches = h->launches; o.pending = h->pending;
+  o.last_n = h->last_n;
+  memcpy(o.pool, h->pool, sizeof(o.pool)); memcpy(o.pool_bytes, h->pool_bytes, sizeof(o.pool_bytes));
+  tpcHandle::Slot& n = h->slots[s];
+  if (!n.init) {
+    TPC_CUDA(h, cudaMalloc(&n.d_cnt, 8 * (CNT_COUNT + 1)));
+    TPC_CUDA(h, cudaMallocHost(&n.h_cnt, 8 * (CNT_COUNT + 1)));
+    TPC_CUDA(h, cudaEventCreate(&n.ev_done));
+    TPC_CUDA(h, cudaStreamCreateWithFlags(&n.stream, cudaStreamNonBlocking));
+    memset(n.h_cnt, 0, 8 * (CNT_COUNT + 1));
+    n.init = true;
+  }
+  h->d_cnt = n.d_cnt; h->h_cnt = n.h_cnt; h->ev_done = n.ev_done; h->launches = n.launches; h->pending = n.pending;
+  h->last_n = n.last_n;
+  memcpy(h->pool, n.pool, sizeof(n.pool)); memcpy(h->pool_bytes, n.pool_bytes, sizeof(n.pool_bytes));
+  h->cur_slot = s;
+  return TPC_OK;
+}
+}  // namespace
+
+extern "C" int tpcSubmitHost(tpcHandle* h, int slot, int64_t N, const uint32_t* row_offset, const float* y, const float* z,
+                             const tpcTracks* oh) {
+  if (!h || slot < 0 || slot > 1 || !row_offset || !oh || N < 0 || N >= (1ll << 31) || (N > 0 && (!y || !z)))
+    return TPC_ERR_INVALID_ARG;
+  if (oh->link_up_raw || oh->link_dn_raw || oh->link_up || oh->link_dn || oh->start_hits || oh->tl_status || oh->tl_nhits ||
+      oh->tl_first_row || oh->tl_last_row || oh->tl_rowhit || oh->tl_x || oh->tl_par || oh->tl_cov || oh->tl_chi2 ||
+      oh->trk_rf_status || oh->trk_mg_next || !oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0)
+    return TPC_ERR_INVALID_ARG;
+  TPC_CUDA(h, cudaSetDevice(h->device));
+  int rc;
+  if ((rc = useSlot(h, slot + 1))) return rc;
+  tpcHandle::Slot& S = h->slots[slot + 1];
+  if (S.submitted) { useSlot(h, 0); return TPC_ERR_INVALID_ARG; }      // collect first
+  cudaStream_t st = S.stream;
+  const int nb = h->P.n_buckets;
+  const int64_t capT = std::max<int64_t>(std::max<int64_t>(4096, N / 8), h->hint_T);
+  const int64_t capK = std::max<int64_t>(std::max<int64_t>(4096, N / 64), h->hint_K);
+  const int64_t capC = std::max<int64_t>(std::max<int64_t>(N / 2, 1), h->hint_C);
+  void *d_off, *d_y, *d_z, *ws;
+  size_t wsb = 0;
+  auto fail = [&](int code) { useSlot(h, 0); return code; };
+  if ((rc = poolGet(h, 0, 4 * (size_t)(nb + 1), &d_off)) || (rc = poolGet(h, 1, 4 * (size_t)N, &d_y)) ||
+      (rc = poolGet(h, 2, 4 * (size_t)N, &d_z)) || (rc = tpcWorkspaceBytes(h, N, capT, &wsb)) || (rc = poolGet(h, 3, wsb, &ws)))
+    return fail(rc);
+  void* p[11];
+  const size_t K = (size_t)capK;
+  const size_t sz[11] = {4 * K, 4 * K, 4 * K, 4 * K, 4 * K, 4 * K, 20 * K, 60 * K, 4 * K, 4 * (K + 1), 4 * (size_t)capC};
+  for (int i = 0; i < 11; ++i)
+    if ((rc = poolGet(h, 4 + i, sz[i], &p[i]))) return fail(rc);
+  if (cudaMemcpyAsync(d_off, row_offset, 4 * (size_t)(nb + 1), cudaMemcpyHostToDevice, st) != cudaSuccess ||
+      (N > 0 && (cudaMemcpyAsync(d_y, y, 4 * (size_t)N, cudaMemcpyHostToDevice, st) != cudaSuccess ||
+                 cudaMemcpyAsync(d_z, z, 4 * (size_t)N, cudaMemcpyHostToDevice, st) != cudaSuccess)))
+    return fail(TPC_ERR_CUDA);
+  tpcTracks od{};
+  od.cap_tracks = capK; od.cap_track_clusters = capC;
+  od.trk_tracklet = (int32_t*)p[0]; od.trk_sector = (int32_t*)p[1]; od.trk_first_row = (int32_t*)p[2];
+  od.trk_last_row = (int32_t*)p[3]; od.trk_ncl = (int32_t*)p[4]; od.trk_x = (float*)p[5]; od.trk_par = (float*)p[6];
+  od.trk_cov = (float*)p[7]; od.trk_chi2 = (float*)p[8]; od.trk_cl_offset = (uint32_t*)p[9];
+  od.trk_cl_index = (uint32_t*)p[10];
+  const tpcClusters in{N, (const uint32_t*)d_off, nullptr, (const float*)d_y, (const float*)d_z, nullptr};
+  if ((rc = tpcRun(h, &in, &od, capT, ws, h->pool_bytes[3], st))) return fail(rc);
+  // The counts are not known on the host yet: copy back up to the capacities (the hints sit a few percent above the
+  // last counts), tpcCollectHost trims.  tpcRun's own status copy and event come before these copies on the stream,
+  // so a second event closes the slot.
+  const int64_t nt = std::min<int64_t>(capK, oh->cap_tracks), nc = std::min<int64_t>(capC, oh->cap_track_clusters);
+  const size_t n4 = 4 * (size_t)nt;
+  auto back = [&](void* dst, const void* src, size_t bytes) {
+    return (dst && bytes) ? cudaMemcpyAsync(dst, src, bytes, cudaMemcpyDeviceToHost, st) : cudaSuccess;
+  };
+  bool ok = back(oh->trk_tracklet, od.trk_tracklet, n4) == cudaSuccess && back(oh->trk_sector, od.trk_sector, n4) == cudaSuccess &&
+            back(oh->trk_first_row, od.trk_first_row, n4) == cudaSuccess && back(oh->trk_last_row, od.trk_last_row, n4) == cudaSuccess &&
+            back(oh->trk_ncl, od.trk_ncl, n4) == cudaSuccess && back(oh->trk_x, od.trk_x, n4) == cudaSuccess &&
+            back(oh->trk_chi2, od.trk_chi2, n4) == cudaSuccess;
+  if (ok && nt > 0 && oh->trk_par)
+    ok = cudaMemcpy2DAsync(oh->trk_par, 4 * (size_t)oh->cap_tracks, od.trk_par, 4 * (size_t)capK, n4, 5, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+  if (ok && nt > 0 && oh->trk_cov)
+    ok = cudaMemcpy2DAsync(oh->trk_cov, 4 * (size_t)oh->cap_tracks, od.trk_cov, 4 * (size_t)capK, n4, 15, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+  ok = ok && back(oh->trk_cl_offset, od.trk_cl_offset, 4 * (size_t)(std::min<int64_t>(nt, oh->cap_tracks) + 1)) == cudaSuccess &&
+       back(oh->trk_cl_index, od.trk_cl_index, 4 * (size_t)nc) == cudaSuccess &&
+       cudaEventRecord(h->ev_done, st) == cudaSuccess;
+  if (!ok) return fail(TPC_ERR_CUDA);
+  S.submitted = true; S.capK = capK; S.capC = capC; S.oh = *oh;
+  return useSlot(h, 0);
+}
+
+extern "C" int tpcCollectHost(tpcHandle* h, int slot, tpcRunStatus* status) {
+  if (!h || slot < 0 || slot > 1 || !status) return TPC_ERR_INVALID_ARG;
+  tpcHandle::Slot& S = h->slots[slot + 1];
+  if (!S.submitted) return TPC_ERR_INVALID_ARG;
+  TPC_CUDA(h, cudaSetDevice(h->device));
+  int rc;
+  if ((rc = useSlot(h, slot + 1))) return rc;
+  rc = tpcGetRunStatus(h, status);            // waits for the slot's last event: run and copies are complete
+  S.submitted = false;
+  if (rc == TPC_OK) {
+    if (status->status == TPC_OK &&
+        (status->n_tracks > std::min(S.capK, S.oh.cap_tracks) || status->n_track_clusters > std::min(S.capC, S.oh.cap_track_clusters)))
+      status->status = TPC_ERR_CAPACITY;
+    // the next submission gets the capacities right (also after TPC_ERR_CAPACITY: the caller re-runs with tpcRunHost)
+    h->hint_T = std::max(h->hint_T, status->n_start_hits + status->n_start_hits / 16);
+    h->hint_K = std::max(h->hint_K, status->n_tracks + status->n_tracks / 16);
+    h->hint_C = std::max(h->hint_C, status->n_track_clusters + status->n_track_clusters / 16);
+  }
+  const int rc2 = useSlot(h, 0);
+  return rc ? rc : rc2;
 }

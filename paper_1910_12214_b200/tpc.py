@@ -65,7 +65,7 @@ class tpcRunStatus(ctypes.Structure):
 
 
 ABI_SYMBOLS = ("tpcDefaultParams", "tpcCreate", "tpcDestroy", "tpcWorkspaceBytes", "tpcRun", "tpcGetRunStatus",
-               "tpcSetProfiling", "tpcRunHost", "tpcErrorString", "tpcLastCudaError")
+               "tpcSetProfiling", "tpcRunHost", "tpcSubmitHost", "tpcCollectHost", "tpcErrorString", "tpcLastCudaError")
 
 _lib = None
 
@@ -94,7 +94,9 @@ def load_library(build_if_stale: bool = True) -> ctypes.CDLL:
     L.tpcGetRunStatus.argtypes = [vp, POINTER(tpcRunStatus)]
     L.tpcSetProfiling.argtypes = [vp, c_int]
     L.tpcRunHost.argtypes = [vp, c_int64, vp, vp, vp, POINTER(tpcTracks), POINTER(tpcRunStatus), vp]
-    for f in ABI_SYMBOLS[:8]:
+    L.tpcSubmitHost.argtypes = [vp, c_int, c_int64, vp, vp, vp, POINTER(tpcTracks)]
+    L.tpcCollectHost.argtypes = [vp, c_int, POINTER(tpcRunStatus)]
+    for f in ABI_SYMBOLS[:10]:
         getattr(L, f).restype = c_int
     L.tpcErrorString.argtypes = [c_int]
     L.tpcErrorString.restype = c_char_p
@@ -317,6 +319,61 @@ class TpcTracker:
 
     def status(self) -> tpcRunStatus:
         return tpcGetRunStatus(self.handle)
+
+    def _host_buffers(self, capK, capC, slot):
+        t = self.torch
+        key = (capK, capC)
+        bufs = getattr(self, "_host_slots", None)
+        if bufs is None:
+            bufs = self._host_slots = {}
+        if slot not in bufs or bufs[slot][0] != key:
+            def pinned(shape, dt, view=None):     # pinned host memory: the copies run asynchronously and at full speed
+                a = t.empty(shape, dtype=dt, pin_memory=True).numpy()
+                return a.view(view) if view is not None else a
+            i32, f32 = t.int32, t.float32
+            bufs[slot] = (key, {"trk_tracklet": pinned(capK, i32), "trk_sector": pinned(capK, i32),
+                                "trk_first_row": pinned(capK, i32), "trk_last_row": pinned(capK, i32),
+                                "trk_ncl": pinned(capK, i32), "trk_x": pinned(capK, f32), "trk_par": pinned((5, capK), f32),
+                                "trk_cov": pinned((15, capK), f32), "trk_chi2": pinned(capK, f32),
+                                "trk_cl_offset": pinned(capK + 1, i32, np.uint32),
+                                "trk_cl_index": pinned(capC, i32, np.uint32)})
+        return bufs[slot][1]
+
+    def submit_host(self, slot: int, row_offset: np.ndarray, y: np.ndarray, z: np.ndarray, cap_tracks: int,
+                    cap_track_clusters: int):
+        """tpcSubmitHost: enqueue one event (host buffers, ideally pinned) on pipeline slot 0 or 1 and return at once."""
+        L = load_library()
+        n = int(y.shape[0])
+        h = self._host_buffers(int(cap_tracks), int(cap_track_clusters), slot)
+        tr = tpcTracks()
+        tr.cap_tracks, tr.cap_track_clusters = int(cap_tracks), int(cap_track_clusters)
+        for k, v in h.items():
+            setattr(tr, k, v.ctypes.data)
+        assert row_offset.dtype == np.uint32 and y.dtype == np.float32 and z.dtype == np.float32
+        self._host_keep = getattr(self, "_host_keep", {})
+        self._host_keep[slot] = (row_offset, y, z)          # the inputs must outlive the asynchronous copies
+        rc = L.tpcSubmitHost(self.handle, slot, n, row_offset.ctypes.data, y.ctypes.data if n else None,
+                             z.ctypes.data if n else None, byref(tr))
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpcSubmitHost", L.tpcLastCudaError(self.handle).decode())
+
+    def collect_host(self, slot: int):
+        """tpcCollectHost: wait for the slot's event.  Returns (status, outputs); status.status may be TPC_ERR_CAPACITY
+        (run that event again with run_host)."""
+        L = load_library()
+        st = tpcRunStatus()
+        rc = L.tpcCollectHost(self.handle, slot, byref(st))
+        if rc != TPC_OK:
+            raise TpcError(rc, "tpcCollectHost", L.tpcLastCudaError(self.handle).decode())
+        if st.status not in (TPC_OK, TPC_ERR_CAPACITY):
+            raise TpcError(st.status, "tpcCollectHost (device status)")
+        h = self._host_slots[slot][1]
+        capK, capC = self._host_slots[slot][0]
+        nt, nc = min(int(st.n_tracks), capK), min(int(st.n_track_clusters), capC)
+        out = {k: (h[k][:, :nt] if h[k].ndim == 2 else h[k][:nt]) for k in _TRK_PTRS[:9]}
+        out["trk_cl_offset"] = h["trk_cl_offset"][:nt + 1]
+        out["trk_cl_index"] = h["trk_cl_index"][:nc]
+        return st, out
 
     def run_host(self, row_offset: np.ndarray, y: np.ndarray, z: np.ndarray, cap_tracks: int | None = None,
                  cap_track_clusters: int | None = None):

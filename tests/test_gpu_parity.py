@@ -230,3 +230,42 @@ def test_parity_fuzz_random_events_dead_rows_and_parameters(seed):
                max_sinphi=float(rng.uniform(0.8, 0.99)), clusters_per_cell=float(rng.uniform(0.2, 4.0)))
     rep, res, o = _run_both(ev, **par)
     assert len(o.start_hits) > 0
+
+
+def test_submit_collect_pipeline_matches_run_host():
+    """tpcSubmitHost / tpcCollectHost on two slots with different events in flight give, per event, exactly what the
+    synchronous tpcRunHost gives; a too small capacity is reported, not overrun."""
+    from paper_1910_12214_b200 import tpc
+    import torch
+    evs = [datagen.make_event(1, scale=0.05, seed=20 + i) for i in range(4)]
+    trk = _tracker(evs[0])
+    ref = []
+    for ev in evs:
+        st, out = trk.run_host(ev.row_offset, ev.y, ev.z)
+        assert st.status == 0
+        ref.append({k: v.copy() for k, v in out.items()})
+    capK = max(len(r["trk_ncl"]) for r in ref) + 64
+    capC = max(len(r["trk_cl_index"]) for r in ref) + 64
+
+    def pin(a):
+        return torch.from_numpy(np.ascontiguousarray(a)).pin_memory().numpy()
+    ins = [(pin(ev.row_offset.astype(np.uint32)), pin(ev.y), pin(ev.z)) for ev in evs]
+    trk.submit_host(0, *ins[0], capK, capC)
+    for i in range(len(evs)):
+        if i + 1 < len(evs):
+            trk.submit_host((i + 1) % 2, *ins[i + 1], capK, capC)
+        st, out = trk.collect_host(i % 2)
+        assert st.status == 0 and st.n_tracks == len(ref[i]["trk_ncl"])
+        for k in ref[i]:
+            assert np.array_equal(out[k], ref[i][k]), (i, k)
+    # capacity too small for the tracks: reported, the valid prefix only is exposed
+    trk.submit_host(0, *ins[0], 8, capC)
+    st, out = trk.collect_host(0)
+    assert st.status == tpc.TPC_ERR_CAPACITY and len(out["trk_ncl"]) == 8
+    # a slot must be collected before it is reused
+    trk.submit_host(1, *ins[1], capK, capC)
+    with pytest.raises(tpc.TpcError):
+        trk.submit_host(1, *ins[2], capK, capC)
+    st, out = trk.collect_host(1)
+    assert st.status == 0
+    trk.close()
