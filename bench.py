@@ -265,7 +265,8 @@ def run_ours(args, rank, world, local_rank):
     e2e_value = total_clusters / (ms_e2e * 1e-3)
     nt, nc = int(sth.n_tracks), int(sth.n_track_clusters)
     h2d = 4 * (len(ev.row_offset)) + 8 * N
-    d2h = nt * (5 * 4 + 4 + 20 + 60 + 4) + 4 * (nt + 1) + 4 * nc + 8 * 9
+    # tpcSubmitHost copies back up to the capacities (the counts are not known on the host at submit time)
+    d2h = capK * (5 * 4 + 4 + 20 + 60 + 4) + 4 * (capK + 1) + 4 * capC + 8 * 11
 
     if rank != 0:
         return

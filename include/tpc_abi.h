@@ -151,6 +151,8 @@ typedef struct {
                                    0 grid, 1 neighbour finder, 2 cleaner+start hits, 3 constructor, 4 selector,
                                    5 optional refit, merger and exports, 6 total, 7 refit alone */
   float merge_ms;               /* the O7 merger alone (profiling on, merger requested) */
+  float submit_ms[2];           /* tpcCollectHost only: device time of the slot from its first copy in to the end of its
+                                   kernels [0] and to the end of its copies out [1] (includes waiting for the other slot) */
 } tpcRunStatus;
 
 int tpcDefaultParams(tpcParams* p);

@@ -90,6 +90,7 @@ struct tpcHandle {
     int launches = 0; bool pending = false; int64_t last_n = 0;
     void* pool[16] = {}; size_t pool_bytes[16] = {};
     cudaStream_t stream = nullptr;
+    cudaEvent_t ev_begin = nullptr, ev_kernels = nullptr;   // first copy in / end of the kernels of the submitted run
     bool submitted = false;
     int64_t capK = 0, capC = 0;      // device capacities of the submitted run
     tpcTracks oh{};                  // host outputs of the submitted run
@@ -275,7 +276,11 @@ int tpcDestroy(tpcHandle* h) {
     cudaFree(S.d_cnt); if (S.h_cnt) cudaFreeHost(S.h_cnt); if (S.ev_done) cudaEventDestroy(S.ev_done);
     for (int i = 0; i < 16; ++i) if (S.pool[i]) cudaFree(S.pool[i]);
   }
-  for (int k = 1; k < 3; ++k) if (h->slots[k].stream) cudaStreamDestroy(h->slots[k].stream);
+  for (int k = 1; k < 3; ++k) {
+    if (h->slots[k].stream) cudaStreamDestroy(h->slots[k].stream);
+    if (h->slots[k].ev_begin) cudaEventDestroy(h->slots[k].ev_begin);
+    if (h->slots[k].ev_kernels) cudaEventDestroy(h->slots[k].ev_kernels);
+  }
   for (int i = 0; i < 16; ++i) if (h->pool[i]) cudaFree(h->pool[i]);
   delete h;
   return TPC_OK;
@@ -622,6 +627,8 @@ int useSlot(tpcHandle* h, int s) {
     TPC_CUDA(h, cudaMallocHost(&n.h_cnt, 8 * (CNT_COUNT + 1)));
     TPC_CUDA(h, cudaEventCreate(&n.ev_done));
     TPC_CUDA(h, cudaStreamCreateWithFlags(&n.stream, cudaStreamNonBlocking));
+    TPC_CUDA(h, cudaEventCreate(&n.ev_begin));
+    TPC_CUDA(h, cudaEventCreate(&n.ev_kernels));
     memset(n.h_cnt, 0, 8 * (CNT_COUNT + 1));
     n.init = true;
   }
@@ -662,10 +669,18 @@ extern "C" int tpcSubmitHost(tpcHandle* h, int slot, int64_t N, const uint32_t* 
   const size_t sz[11] = {4 * K, 4 * K, 4 * K, 4 * K, 4 * K, 4 * K, 20 * K, 60 * K, 4 * K, 4 * (K + 1), 4 * (size_t)capC};
   for (int i = 0; i < 11; ++i)
     if ((rc = poolGet(h, 4 + i, sz[i], &p[i]))) return fail(rc);
+  cudaEventRecord(S.ev_begin, st);
   if (cudaMemcpyAsync(d_off, row_offset, 4 * (size_t)(nb + 1), cudaMemcpyHostToDevice, st) != cudaSuccess ||
       (N > 0 && (cudaMemcpyAsync(d_y, y, 4 * (size_t)N, cudaMemcpyHostToDevice, st) != cudaSuccess ||
                  cudaMemcpyAsync(d_z, z, 4 * (size_t)N, cudaMemcpyHostToDevice, st) != cudaSuccess)))
     return fail(TPC_ERR_CUDA);
+  // The kernels of this event start when those of the other slot's event are done (its copies out then overlap these
+  // kernels, and the copies in above overlapped its kernels): without the order the two events would share the SMs
+  // and finish together, copies and kernels never overlapping.
+  {
+    tpcHandle::Slot& O = h->slots[2 - slot];
+    if (O.submitted && cudaStreamWaitEvent(st, O.ev_kernels, 0) != cudaSuccess) return fail(TPC_ERR_CUDA);
+  }
   tpcTracks od{};
   od.cap_tracks = capK; od.cap_track_clusters = capC;
   od.trk_tracklet = (int32_t*)p[0]; od.trk_sector = (int32_t*)p[1]; od.trk_first_row = (int32_t*)p[2];
@@ -674,6 +689,7 @@ extern "C" int tpcSubmitHost(tpcHandle* h, int slot, int64_t N, const uint32_t* 
   od.trk_cl_index = (uint32_t*)p[10];
   const tpcClusters in{N, (const uint32_t*)d_off, nullptr, (const float*)d_y, (const float*)d_z, nullptr};
   if ((rc = tpcRun(h, &in, &od, capT, ws, h->pool_bytes[3], st))) return fail(rc);
+  cudaEventRecord(S.ev_kernels, st);
   // The counts are not known on the host yet: copy back up to the capacities (the hints sit a few percent above the
   // last counts), tpcCollectHost trims.  tpcRun's own status copy and event come before these copies on the stream,
   // so a second event closes the slot.
@@ -708,6 +724,9 @@ extern "C" int tpcCollectHost(tpcHandle* h, int slot, tpcRunStatus* status) {
   rc = tpcGetRunStatus(h, status);            // waits for the slot's last event: run and copies are complete
   S.submitted = false;
   if (rc == TPC_OK) {
+    float ms = 0;
+    if (cudaEventElapsedTime(&ms, S.ev_begin, S.ev_kernels) == cudaSuccess) status->submit_ms[0] = ms;
+    if (cudaEventElapsedTime(&ms, S.ev_begin, h->ev_done) == cudaSuccess) status->submit_ms[1] = ms;
     if (status->status == TPC_OK &&
         (status->n_tracks > std::min(S.capK, S.oh.cap_tracks) || status->n_track_clusters > std::min(S.capC, S.oh.cap_track_clusters)))
       status->status = TPC_ERR_CAPACITY;

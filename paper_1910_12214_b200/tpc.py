@@ -61,7 +61,7 @@ class tpcTracks(ctypes.Structure):
 class tpcRunStatus(ctypes.Structure):
     _fields_ = [("status", c_int32), ("kernel_launches", c_int32), ("n_clusters", c_int64), ("n_start_hits", c_int64),
                 ("n_tracklets", c_int64), ("n_tracklet_hits", c_int64), ("n_tracks", c_int64),
-                ("n_track_clusters", c_int64), ("n_cells", c_int64), ("stage_ms", c_float * 8), ("merge_ms", c_float)]
+                ("n_track_clusters", c_int64), ("n_cells", c_int64), ("stage_ms", c_float * 8), ("merge_ms", c_float), ("submit_ms", c_float * 2)]
 
 
 ABI_SYMBOLS = ("tpcDefaultParams", "tpcCreate", "tpcDestroy", "tpcWorkspaceBytes", "tpcRun", "tpcGetRunStatus",
