@@ -199,6 +199,9 @@ struct orcResult {
   // O7 merger (NEXT-1)
   std::vector<int32_t> mg_next, mg_prev, mg_head;
   std::vector<double> mg_chi2;
+  // O8 cluster flags (NEXT-3)
+  std::vector<uint8_t> cf_flags;
+  std::vector<int32_t> cf_owner;
 };
 
 namespace {
@@ -481,6 +484,56 @@ struct Tracker {
     }
   }
 
+  // ---- O8 cluster flags (O8; readings R34..R37) ---------------------------
+  void flagAll() {
+    const int64_t nt = (int64_t)res.tr_id.size();
+    res.cf_flags.assign(N, 0); res.cf_owner.assign(N, -1);
+    const Real bf = (Real)(0.00299792458 * (double)g.bz_tesla);
+    const Real msp = (Real)P.max_sinphi, tube2 = (Real)P.tube_radius * (Real)P.tube_radius;
+    const Real sin70 = (Real)0.9396926207859084, qmax = (Real)P.inv_pt_protect;
+    std::vector<Real> ownerQ(N, 0);
+    std::vector<uint8_t> ownerBad(N, 0);         // owner is low or steep at the cluster's row
+    for (int64_t k = 0; k < nt; ++k) {
+      if (!res.rf_status[k]) continue;
+      State<Real> st{};
+      st.x = (Real)res.rf_x_in[k]; st.y = (Real)res.rf_par_in[k * 5]; st.z = (Real)res.rf_par_in[k * 5 + 1];
+      st.s = (Real)res.rf_par_in[k * 5 + 2]; st.t = (Real)res.rf_par_in[k * 5 + 3]; st.q = (Real)res.rf_par_in[k * 5 + 4];
+      for (int i = 0; i < 15; ++i) st.C[i] = (Real)res.rf_cov_in[k * 15 + i];
+      const Real aq = std::fabs(st.q);
+      const bool low = !(aq < qmax);
+      const int sec = res.tr_sector[k];
+      const uint32_t* cl = res.tr_cl_index.data() + res.tr_cl_offset[k];
+      const int ncl = (int)(res.tr_cl_offset[k + 1] - res.tr_cl_offset[k]);
+      int ic = 0;
+      for (int r = res.tr_first[k]; r <= res.tr_last[k]; ++r) {
+        if (dead(r)) continue;
+        if (r > res.tr_first[k] && !propagate(st, X[r], bf, msp)) break;
+        const bool bad = low || !(std::fabs(st.s) < sin70);
+        while (ic < ncl && rowOf[cl[ic]] < r) ++ic;
+        const int32_t own = (ic < ncl && rowOf[cl[ic]] == r) ? (int32_t)cl[ic] : -1;     // the attached cluster of this row
+        for (uint32_t c = off[sec * R + r]; c < off[sec * R + r + 1]; ++c) {
+          const Real dy = Y[c] - st.y, dz = Z[c] - st.z;
+          const Real d2 = dy * dy + dz * dz;
+          if (!(d2 <= tube2) && (int32_t)c != own) continue;
+          if (res.cf_owner[c] < 0 || aq < ownerQ[c]) {      // ties: the lower track index (loop order)
+            res.cf_owner[c] = (int32_t)k; ownerQ[c] = aq; ownerBad[c] = bad ? 1 : 0;
+          }
+        }
+      }
+    }
+    for (int64_t k = 0; k < nt; ++k)
+      for (uint32_t i = res.tr_cl_offset[k]; i < res.tr_cl_offset[k + 1]; ++i) res.cf_flags[res.tr_cl_index[i]] |= 1;
+    for (int64_t c = 0; c < N; ++c) {
+      uint8_t f = res.cf_flags[c];
+      const bool has = res.cf_owner[c] >= 0, prot = has && !ownerBad[c];
+      if (has) f |= 2;
+      if (prot) f |= 4;
+      if (has && !prot) f |= 8;
+      if (!prot) f |= 16;
+      res.cf_flags[c] = f;
+    }
+  }
+
   void construct(uint32_t h0, Tracklet<Real>& T) const {
     const Real b = (Real)(0.00299792458 * (double)g.bz_tesla);
     const Real msp = (Real)P.max_sinphi, e2y = (Real)P.err2_y, e2z = (Real)P.err2_z;
@@ -627,6 +680,7 @@ void orcDefaultParams(orcParams* p) {
   p->max_row_gap = 4; p->min_chain_hits = 3; p->min_tracklet_hits = 10; p->min_track_hits = 10;
   p->cell_min = 0.5f; p->cell_max = 8.0f;
   p->merge_max_row_gap = 40; p->merge_back_rows = 5; p->merge_chi2_max = 50.0f;
+  p->tube_radius = 1.5f; p->inv_pt_protect = 20.0f;
 }
 
 int orcRun(const orcGeometry* g, const orcParams* p, int64_t n, const uint32_t* off, const float* y, const float* z,
@@ -643,9 +697,10 @@ int orcRun(const orcGeometry* g, const orcParams* p, int64_t n, const uint32_t* 
   r->n = n; r->n_sectors = g->n_sectors; r->n_rows = g->n_rows;
   r->fp64 = (flags & ORC_FP64) != 0; r->brute = (flags & ORC_BRUTE_FORCE) != 0;
   const bool mg = (flags & ORC_MERGE) != 0;
-  const bool rf = mg || (flags & ORC_REFIT) != 0;
-  if (r->fp64) { Tracker<double> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); if (rf) T.refitAll(); if (mg) T.mergeAll(); }
-  else { Tracker<float> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); if (rf) T.refitAll(); if (mg) T.mergeAll(); }
+  const bool fg = (flags & ORC_FLAGS) != 0;
+  const bool rf = mg || fg || (flags & ORC_REFIT) != 0;
+  if (r->fp64) { Tracker<double> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); if (rf) T.refitAll(); if (mg) T.mergeAll(); if (fg) T.flagAll(); }
+  else { Tracker<float> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); if (rf) T.refitAll(); if (mg) T.mergeAll(); if (fg) T.flagAll(); }
   *out = r;
   return ORC_OK;
 }
@@ -669,6 +724,7 @@ void orcGetRefit(const orcResult* r, int32_t* status, double* x_in, double* par_
   copyOut(chi2, r->rf_chi2); copyOut(x_out, r->rf_x_out); copyOut(par_out, r->rf_par_out); copyOut(cov_out, r->rf_cov_out);
 }
 
+void orcGetClusterFlags(const orcResult* r, uint8_t* flags, int32_t* owner) { copyOut(flags, r->cf_flags); copyOut(owner, r->cf_owner); }
 void orcGetMerge(const orcResult* r, int32_t* next, int32_t* prev, int32_t* head, double* chi2) {
   copyOut(next, r->mg_next); copyOut(prev, r->mg_prev); copyOut(head, r->mg_head); copyOut(chi2, r->mg_chi2);
 }

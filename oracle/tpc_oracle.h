@@ -41,12 +41,14 @@ typedef struct {
   float cell_min, cell_max;
   int32_t merge_max_row_gap, merge_back_rows;   /* O7: 40, 5 */
   float merge_chi2_max;                         /* O7: 50 */
+  float tube_radius, inv_pt_protect;            /* O8: 1.5 cm, 20 c/GeV (pT = 50 MeV/c) */
 } orcParams;
 
 typedef struct orcResult orcResult;
 
 enum { ORC_OK = 0, ORC_ERR_INVALID_ARG = -1, ORC_ERR_UNSORTED_OFFSETS = -2 };
-enum { ORC_BRUTE_FORCE = 1, ORC_FP64 = 2, ORC_REFIT = 4, ORC_MERGE = 8 /* implies ORC_REFIT */ };
+enum { ORC_BRUTE_FORCE = 1, ORC_FP64 = 2, ORC_REFIT = 4, ORC_MERGE = 8 /* implies ORC_REFIT */,
+       ORC_FLAGS = 16 /* implies ORC_REFIT */ };
 
 void orcDefaultParams(orcParams* p);
 
@@ -94,6 +96,11 @@ int orcRefitPoints(const orcGeometry* g, const orcParams* p, int n, const int32_
  * next / prev / head [n_tracks] track indices (-1 none; head = first track of the chain), chi2 [n_tracks] of the link
  * to next (0 if none).  Pins: tests/test_oracle_merge.py. */
 void orcGetMerge(const orcResult*, int32_t* next, int32_t* prev, int32_t* head, double* chi2);
+/* O8 (NEXT-3 of SURVEY.md 8(f), DESIGN.md section 3 "O8"): per-cluster flags, only with ORC_FLAGS.
+ * flags [n_clusters] bit mask 1 attached, 2 adjacent, 4 protected, 8 removed by strategy A, 16 removed by strategy B;
+ * owner [n_clusters] track index of the highest-momentum track with the cluster in its tube, -1 none. */
+void orcGetClusterFlags(const orcResult*, uint8_t* flags, int32_t* owner);
+
 /* Pieces of O7 for the pins.  state = {x, y, z, s, t, q}, cov = 15 lower-triangle elements, in/out as doubles.
  * orcRotate: frame turned by alpha (radians); returns 1 on success, 0 (untouched) on failure.
  * orcMatch: chi2 of the match of outer state a to inner state b (b at plane b_state[0]); rel = 0 same sector,

@@ -21,6 +21,7 @@ BRUTE_FORCE = 1
 FP64 = 2
 REFIT = 4
 MERGE = 8
+FLAGS = 16
 
 
 def build(force: bool = False) -> str:
@@ -43,7 +44,8 @@ class Params(ctypes.Structure):
                  "turn_var_scale", "max_sinphi", "road_sigma", "road_min", "road_max")] + \
                [(n, ctypes.c_int32) for n in ("max_row_gap", "min_chain_hits", "min_tracklet_hits", "min_track_hits")] + \
                [("cell_min", ctypes.c_float), ("cell_max", ctypes.c_float), ("merge_max_row_gap", ctypes.c_int32),
-                ("merge_back_rows", ctypes.c_int32), ("merge_chi2_max", ctypes.c_float)]
+                ("merge_back_rows", ctypes.c_int32), ("merge_chi2_max", ctypes.c_float), ("tube_radius", ctypes.c_float),
+                ("inv_pt_protect", ctypes.c_float)]
 
 
 _lib = None
@@ -71,6 +73,8 @@ def _load():
         L.orcGetTracks.argtypes = [vp] * 12
         for f in ("orcGetGrid", "orcGetLinks", "orcGetStartHits", "orcGetTracklets", "orcGetTracks"):
             getattr(L, f).restype = None
+        L.orcGetClusterFlags.argtypes = [vp] * 3
+        L.orcGetClusterFlags.restype = None
         L.orcGetMerge.argtypes = [vp] * 5
         L.orcGetMerge.restype = None
         L.orcRotate.argtypes = [vp, vp, dbl, dbl, dbl, ci]
@@ -140,6 +144,9 @@ class OracleResult:
     mg_prev: np.ndarray | None = None
     mg_head: np.ndarray | None = None
     mg_chi2: np.ndarray | None = None
+    # O8 cluster flags (only with flags=True): bit mask per cluster and the owning track
+    cf_flags: np.ndarray | None = None
+    cf_owner: np.ndarray | None = None
 
     @property
     def n_tracks(self) -> int:
@@ -151,7 +158,7 @@ def _ptr(a):
 
 
 def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool = False,
-        stages_only: bool = False, refit: bool = False, merge: bool = False) -> OracleResult:
+        stages_only: bool = False, refit: bool = False, merge: bool = False, flags: bool = False) -> OracleResult:
     """Run O1..O5 on an Event-like object (fields n_sectors, n_rows, row_x, row_dead, bz_tesla,
     tan_half_sector, z_min, z_max, row_offset, y, z; numpy arrays)."""
     L = _load()
@@ -166,7 +173,7 @@ def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool 
     n = int(y.shape[0])
     h = ctypes.c_void_p()
     rc = L.orcRun(ctypes.byref(g), ctypes.byref(p), n, off.ctypes.data, _ptr(y), _ptr(z),
-                  (BRUTE_FORCE if brute_force else 0) | (FP64 if fp64 else 0) | (REFIT if refit else 0) | (MERGE if merge else 0),
+                  (BRUTE_FORCE if brute_force else 0) | (FP64 if fp64 else 0) | (REFIT if refit else 0) | (MERGE if merge else 0) | (FLAGS if flags else 0),
                   ctypes.byref(h))
     if rc != 0:
         raise ValueError(f"orcRun failed with {rc}")
@@ -194,7 +201,7 @@ def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool 
         L.orcGetTracks(h, _ptr(kid), _ptr(ks), _ptr(kf), _ptr(kl), _ptr(kn), _ptr(kx), _ptr(kpar), _ptr(kcov),
                        _ptr(kchi), _ptr(koff), _ptr(kidx))
         rf = {}
-        refit = refit or merge
+        refit = refit or merge or flags
         if refit:
             rst = np.zeros(nt, np.int32)
             rxi, rchi, rxo = np.zeros(nt), np.zeros(nt), np.zeros(nt)
@@ -207,6 +214,10 @@ def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool 
             mc = np.zeros(nt)
             L.orcGetMerge(h, _ptr(mn), _ptr(mp), _ptr(mh), _ptr(mc))
             rf.update(mg_next=mn, mg_prev=mp, mg_head=mh, mg_chi2=mc)
+        if flags:
+            cf, co = np.zeros(n, np.uint8), np.full(n, -1, np.int32)
+            L.orcGetClusterFlags(h, _ptr(cf), _ptr(co))
+            rf.update(cf_flags=cf, cf_owner=co)
     finally:
         L.orcFree(h)
     return OracleResult(n, s2o, cell, ncell, ur, dr, u, d, sh, st, nh, fr, lr, rh, tx, tpar, tcov, tchi, kid, ks, kf, kl,

@@ -1,0 +1,160 @@
+"""Pins of the oracle's O8 cluster flags (NEXT-3 of SURVEY.md 8(f); DESIGN.md section 3 "O8"; PAPER.md L77-L90:
+adjacent = within a tube of 1.5 cm, ambiguity to the higher-momentum track; protected = adjacent to a track with
+pT > 50 MeV/c and |phi| < 70 deg; strategy B removes everything unprotected, strategy A the unprotected clusters
+attached or adjacent to a low-pT / steep track).
+
+Hand-built cases with known distances and momenta, a numpy restatement of the rule on top of the pinned single
+Propagate step, the truth table of the flag bits, and set invariants.  CPU only.
+"""
+import math
+
+import numpy as np
+import pytest
+
+from oracle import tpc_oracle as orc
+from paper_1910_12214_b200 import datagen
+from tests.helpers import helix_step_closed_form
+
+BZ = 0.5
+R = 152
+ROW_X = (85.0 + np.arange(R) * (160.0 / 151.0)).astype(np.float32).astype(np.float64)
+ATT, ADJ, PROT, RMA, RMB = 1, 2, 4, 8, 16
+
+
+def _event(points):
+    """points: list of (row, y, z) -> one-sector Event; returns (event, index of every point in the CSR order)."""
+    pts = sorted(enumerate(points), key=lambda t: t[1][0])
+    rows = np.array([p[1][0] for p in pts])
+    counts = np.bincount(rows, minlength=R)
+    off = np.concatenate([[0], np.cumsum(counts)])
+    ev = datagen.event_from_arrays(off, np.array([p[1][1] for p in pts], np.float32), np.array([p[1][2] for p in pts], np.float32), 1, R)
+    where = np.empty(len(points), int)
+    for pos, (orig, _) in enumerate(pts):
+        where[orig] = pos
+    return ev, where
+
+
+def _helix_points(pt, charge, s0, t, y0, z0, rows):
+    st0 = np.array([ROW_X[rows[0]], y0, z0, s0, t, charge / pt])
+    return [helix_step_closed_form(st0, ROW_X[r] - ROW_X[rows[0]], BZ) for r in rows]
+
+
+def test_tube_radius_on_a_hand_built_track():
+    """Exact straight-ish track (pT = 20 GeV/c) plus four extra clusters on row 30 at known distances from it."""
+    rows = list(range(10, 70))
+    tr = _helix_points(20.0, 1, 0.1, 0.3, -3.0, 20.0, rows)
+    pts = [(r, p[1], p[2]) for r, p in zip(rows, tr)]
+    y30, z30 = tr[20][1], tr[20][2]
+    extra = [(30, y30 + 1.4, z30), (30, y30 - 1.6, z30), (30, y30 + 1.0, z30 - 1.0), (30, y30 - 1.1, z30 + 1.1)]
+    ev, where = _event(pts + extra)
+    res = orc.run(ev, flags=True)
+    assert res.n_tracks == 1 and res.trk_ncl[0] == len(rows)
+    f = res.cf_flags
+    assert np.all(f[where[:len(rows)]] == ATT | ADJ | PROT)
+    e = where[len(rows):]
+    assert f[e[0]] == ADJ | PROT and f[e[2]] == ADJ | PROT           # 1.4 cm and sqrt(2) cm: inside the tube
+    assert f[e[1]] == RMB and f[e[3]] == RMB                          # 1.6 cm and 1.1 * sqrt(2) cm: outside
+    assert np.all(res.cf_owner[where[:len(rows)]] == 0) and res.cf_owner[e[0]] == 0 and res.cf_owner[e[1]] == -1
+
+
+def test_ambiguity_goes_to_the_higher_momentum_track_and_low_momentum_tracks_do_not_protect():
+    rows = list(range(5, 45))         # short enough that the different curvatures keep the two tracks > 1.5 cm apart
+    a = _helix_points(2.0, 1, 0.0, 0.2, 0.0, 10.0, rows)            # 2 GeV/c
+    b = _helix_points(6.0, 1, 0.0, 0.2, 2.5, 10.0, rows)            # 6 GeV/c, 2.5 cm beside it
+    pts = [(r, p[1], p[2]) for r, p in zip(rows, a)] + [(r, p[1], p[2]) for r, p in zip(rows, b)]
+    mid = [(r, 0.5 * (a[i][1] + b[i][1]), a[i][2]) for i, r in enumerate(rows) if 8 <= r <= 12]      # in both tubes
+    ev, where = _event(pts + mid)
+    res = orc.run(ev, flags=True)
+    assert res.n_tracks == 2
+    pt = 1.0 / np.abs(res.rf_par_in[:, 4])
+    hi = int(np.argmax(pt))
+    assert pt[hi] == pytest.approx(6.0, rel=0.05) and pt[1 - hi] == pytest.approx(2.0, rel=0.05)
+    m = where[2 * len(rows):]
+    assert np.all(res.cf_owner[m] == hi) and np.all(res.cf_flags[m] == ADJ | PROT)
+    # the tracks own their clusters (2.5 cm apart: outside each other's tube)
+    assert np.all(res.cf_owner[where[:len(rows)]] == 1 - hi) and np.all(res.cf_owner[where[len(rows):2 * len(rows)]] == hi)
+    # protect only above 4 GeV/c: the 2 GeV/c track now marks its clusters for removal by strategy A
+    p = orc.default_params()
+    p.inv_pt_protect = 0.25
+    res = orc.run(ev, p, flags=True)
+    assert np.all(res.cf_flags[where[:len(rows)]] == ATT | ADJ | RMA | RMB)
+    assert np.all(res.cf_flags[where[len(rows):2 * len(rows)]] == ATT | ADJ | PROT)
+    assert np.all(res.cf_flags[m] == ADJ | PROT)                     # still owned by the 6 GeV/c track
+
+
+def _flags_numpy(ev, res, p):
+    """O8 restated: walk every refitted track with the pinned single Propagate step (binary32), tubes by numpy."""
+    n = ev.n_clusters
+    off = ev.row_offset.astype(np.int64)
+    rowof = np.repeat(np.arange(ev.n_rows * ev.n_sectors), np.diff(off)) % ev.n_rows
+    owner = np.full(n, -1, np.int64)
+    oq = np.zeros(n, np.float32)
+    bad = np.zeros(n, bool)
+    sin70 = np.float32(0.9396926207859084)
+    tube2 = np.float32(p.tube_radius) * np.float32(p.tube_radius)
+    y32, z32 = ev.y.astype(np.float32), ev.z.astype(np.float32)
+    row_x = np.asarray(ev.row_x, np.float32).astype(np.float64)
+    for k in range(res.n_tracks):
+        if not res.rf_status[k]:
+            continue
+        st = np.concatenate([[res.rf_x_in[k]], res.rf_par_in[k]])
+        cov = res.rf_cov_in[k].copy()
+        aq = np.float32(abs(st[5]))
+        low = not (aq < np.float32(p.inv_pt_protect))
+        cl = res.trk_cl_index[res.trk_cl_offset[k]:res.trk_cl_offset[k + 1]].astype(np.int64)
+        sec = int(res.trk_sector[k])
+        for r in range(int(res.trk_first_row[k]), int(res.trk_last_row[k]) + 1):
+            if ev.row_dead[r]:
+                continue
+            if r > res.trk_first_row[k]:
+                ok, st, cov = orc.propagate(st, cov, row_x[r], ev.bz_tesla, p.max_sinphi, fp64=False)
+                if not ok:
+                    break
+            lo, hi = off[sec * ev.n_rows + r], off[sec * ev.n_rows + r + 1]
+            dy = y32[lo:hi] - np.float32(st[1])
+            dz = z32[lo:hi] - np.float32(st[2])
+            inside = (dy * dy + dz * dz) <= tube2
+            own = cl[rowof[cl] == r]
+            inside[own - lo] = True
+            b = low or not (np.float32(abs(st[3])) < sin70)
+            for c in np.nonzero(inside)[0] + lo:
+                if owner[c] < 0 or aq < oq[c]:
+                    owner[c], oq[c], bad[c] = k, aq, b
+    f = np.zeros(n, np.uint8)
+    f[res.trk_cl_index] |= ATT
+    has = owner >= 0
+    prot = has & ~bad
+    f[has] |= ADJ
+    f[prot] |= PROT
+    f[has & ~prot] |= RMA
+    f[~prot] |= RMB
+    return f, owner
+
+
+@pytest.mark.parametrize("idx,scale,dead", [(2, 0.03, ()), (1, 0.02, (40, 97))])
+def test_flags_equal_the_numpy_restatement(idx, scale, dead):
+    ev = datagen.make_event(idx, scale=scale, dead_rows=dead)
+    p = orc.default_params()
+    res = orc.run(ev, p, flags=True)
+    f, owner = _flags_numpy(ev, res, p)
+    assert np.array_equal(owner, res.cf_owner)
+    assert np.array_equal(f, res.cf_flags)
+    if idx == 2:
+        assert ((res.cf_flags & RMA) != 0).sum() > 10            # steep looper segments are exercised
+
+
+def test_flag_invariants_and_what_the_strategies_remove():
+    ev = datagen.make_event(2, scale=0.05)
+    res = orc.run(ev, flags=True)
+    f = res.cf_flags
+    att, adj, prot, rma, rmb = ((f & b) != 0 for b in (ATT, ADJ, PROT, RMA, RMB))
+    assert np.array_equal(adj, res.cf_owner >= 0)
+    assert not np.any(prot & ~adj) and not np.any(rma & ~adj)
+    assert np.array_equal(rmb, ~prot) and np.array_equal(rma, adj & ~prot)
+    refitted = res.rf_status[np.repeat(np.arange(res.n_tracks), res.trk_ncl)] == 1
+    assert np.all(adj[res.trk_cl_index[refitted]])                  # attached clusters of refitted tracks count as adjacent
+    # strategy A never removes a cluster no track claims; strategy B removes all of those (noise included)
+    noise = ev.truth_track < 0
+    assert rmb[noise & ~adj].all() and not rma[~adj].any()
+    # most noise is far from any track and most track clusters are protected
+    assert prot[~noise].mean() > 0.7 and rmb[noise].mean() > 0.6
