@@ -10,6 +10,7 @@
  *   a5 tracklet selector   shared clusters go to the longest / lowest-chi2 tracklet
  *   a6 refit (optional)    Kalman refit of every selected track over its kept clusters: inner and outer state
  *   a7 merger (optional)   links between track segments across row gaps and sector borders
+ *   a8 flags (optional)    per cluster: attached / adjacent / protected, removed by rejection strategy A / B
  * The formulas, constants and tie-breaks are DESIGN.md section 3 (readings R0..R27 of SURVEY.md 8(c)).
  *
  * Conventions
@@ -75,6 +76,8 @@ typedef struct {
   int32_t merge_max_row_gap;    /* 40         O7: rows between the end of a segment and the start of its continuation */
   int32_t merge_back_rows;      /* 5          O7: a continuation in the neighbour sector may start this many rows lower */
   float merge_chi2_max;         /* 50         O7: cut on the diagonal chi2 of a match */
+  float tube_radius;            /* 1.5        O8: clusters within this distance of a track are adjacent, cm */
+  float inv_pt_protect;         /* 20         O8: tracks with |q/pT| below this (pT > 50 MeV/c) protect */
 } tpcParams;
 
 /* Input clusters: CSR by (sector,row), fp32 SoA (single-precision cluster properties). */
@@ -134,6 +137,10 @@ typedef struct {
   int32_t* trk_mg_prev;         /* [cap_tracks] track this one continues, -1 none */
   int32_t* trk_mg_head;         /* [cap_tracks] first track of the chain (itself if unlinked) */
   float* trk_mg_chi2;           /* [cap_tracks] chi2 of the link to trk_mg_next, 0 if none */
+  /* optional O8 per-cluster flags (DESIGN.md section 3 "O8").  Both NULL = none; otherwise both, together
+   * with the refit outputs.  Indexed by the INPUT cluster index. */
+  uint8_t* cl_flags;            /* [n_clusters] 1 attached, 2 adjacent, 4 protected, 8 removed by strategy A, 16 by strategy B */
+  int32_t* cl_owner;            /* [n_clusters] track with the cluster in its tube (highest momentum), -1 none */
 } tpcTracks;
 
 /* Filled by tpcGetRunStatus after the stream has drained. */
@@ -151,6 +158,7 @@ typedef struct {
                                    0 grid, 1 neighbour finder, 2 cleaner+start hits, 3 constructor, 4 selector,
                                    5 optional refit, merger and exports, 6 total, 7 refit alone */
   float merge_ms;               /* the O7 merger alone (profiling on, merger requested) */
+  float flags_ms;               /* the O8 cluster flags alone (profiling on, flags requested) */
   float submit_ms[2];           /* tpcCollectHost only: device time of the slot from its first copy in to the end of its
                                    kernels [0] and to the end of its copies out [1] (includes waiting for the other slot) */
 } tpcRunStatus;

@@ -1,0 +1,101 @@
+// tpc_flags.cuh -- a8: optional per-cluster flags attached / adjacent / protected and the rejection strategies A and B
+// (DESIGN.md section 3 "O8", readings R34..R37; NEXT-3 of SURVEY.md 8(f); tube of 1.5 cm, ambiguity
+// to the higher-momentum track, protected = adjacent to a track with pT > 50 MeV/c and |phi| < 70 degrees).
+//
+// One thread per refitted track walks its rows from the inner state by Propagate alone and bids for every cluster in
+// its tube (found through the a1 grid: cells of the box around the tube, exact circle predicate) and for its own
+// attached cluster of the row.  The bid is a 64-bit key  |q/pT| bits : track id : bad  taken with atomicMin, so the
+// owner is the track of minimal (|q/pT|, id) and the key carries whether that track is low-pT or steep at the
+// cluster's row (a track meets a cluster on one row only, so the last bit never decides).  A last pass per cluster
+// decodes the key into the flag byte.  Keys and flags are indexed by the ORIGINAL cluster index.
+#pragma once
+#include "tpc_kalman.cuh"
+#include "tpc_select.cuh"
+
+namespace tpc {
+
+struct FlagIn {             // refitted tracks (device, SoA with stride cap)
+  int64_t cap;
+  const int32_t *status, *sector, *first_row, *last_row;
+  const float *x_in, *par_in, *cov_in;
+  const uint32_t *cl_offset, *cl_index;
+};
+
+// thread per track-cluster entry: the attached bit
+__global__ void __launch_bounds__(256) flagAttach(const uint32_t* __restrict__ cl_index, uint8_t* __restrict__ flags,
+                                                  const int64_t* __restrict__ cnt) {
+  if (cnt[CNT_ERROR] != 0) return;
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= cnt[CNT_N_TRK_CL]) return;
+  flags[cl_index[i]] = 1;
+}
+
+__global__ void __launch_bounds__(128) flagBid(FlagIn in, const uint32_t* __restrict__ off, DevParams P, RowTables T,
+                                               float tube, float inv_pt_protect, const GridDesc* __restrict__ desc,
+                                               const uint32_t* __restrict__ cell_start, const float2* __restrict__ syz,
+                                               const uint32_t* __restrict__ s2o, unsigned long long* __restrict__ key,
+                                               const int64_t* __restrict__ cnt) {
+  if (cnt[CNT_ERROR] != 0) return;
+  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= cnt[CNT_N_TRACKS] || k >= in.cap || in.status[k] != 1) return;
+  const int64_t cap = in.cap;
+  const int R = P.n_rows;
+  KFState S{};
+  S.x = in.x_in[k];
+  S.y = in.par_in[0 * cap + k]; S.z = in.par_in[1 * cap + k]; S.s = in.par_in[2 * cap + k]; S.t = in.par_in[3 * cap + k];
+  S.q = in.par_in[4 * cap + k];
+  S.c00 = in.cov_in[0 * cap + k]; S.c10 = in.cov_in[1 * cap + k]; S.c11 = in.cov_in[2 * cap + k]; S.c20 = in.cov_in[3 * cap + k];
+  S.c21 = in.cov_in[4 * cap + k]; S.c22 = in.cov_in[5 * cap + k]; S.c30 = in.cov_in[6 * cap + k]; S.c31 = in.cov_in[7 * cap + k];
+  S.c32 = in.cov_in[8 * cap + k]; S.c33 = in.cov_in[9 * cap + k]; S.c40 = in.cov_in[10 * cap + k]; S.c41 = in.cov_in[11 * cap + k];
+  S.c42 = in.cov_in[12 * cap + k]; S.c43 = in.cov_in[13 * cap + k]; S.c44 = in.cov_in[14 * cap + k];
+  const float aq = fabsf(S.q);
+  const bool low = !(aq < inv_pt_protect);
+  const float sin70 = (float)0.9396926207859084;
+  const float tube2 = tube * tube;
+  const unsigned long long khi = ((unsigned long long)__float_as_uint(aq) << 32) | ((unsigned long long)(uint32_t)k << 1);
+  const int sec = in.sector[k], f = in.first_row[k], l = in.last_row[k];
+  const int bsec = sec * R;
+  const uint32_t* cl = in.cl_index + in.cl_offset[k];
+  const int ncl = (int)(in.cl_offset[k + 1] - in.cl_offset[k]);
+  int ic = 0;
+  for (int r = f; r <= l; ++r) {
+    if (T.dead[r]) continue;
+    if (r > f && !kfPropagate(S, T.row_x[r], P, [](float, float, float, float) {})) break;
+    const unsigned long long bid = khi | (unsigned long long)((low || !(fabsf(S.s) < sin70)) ? 1u : 0u);
+    // the attached cluster of this row (R35): the list is in ascending row, rows follow from row_offset (R26)
+    const uint32_t b_lo = __ldg(off + bsec + r), b_hi = __ldg(off + bsec + r + 1);
+    while (ic < ncl && cl[ic] < b_lo) ++ic;
+    if (ic < ncl && cl[ic] < b_hi) atomicMin(key + cl[ic], bid);
+    // the tube: cells of the box around it, exact circle predicate
+    const GridDesc G = desc[bsec + r];
+    if (G.n == 0) continue;
+    const float yc = S.y, zc = S.z;
+    // (box a hair wider than the tube: fl(dy*dy) <= fl(tube*tube) does not quite imply |dy| <= tube)
+    forWindow(G, cell_start, syz, yc, zc, tube * 1.000001f, tube * 1.000001f, [&](uint32_t pos, float cy, float cz) {
+      const float dy = cy - yc, dz = cz - zc;
+      const float d2 = dy * dy + dz * dz;
+      if (d2 <= tube2) atomicMin(key + __ldg(s2o + pos), bid);
+    });
+  }
+}
+
+// thread per cluster: key -> flag byte and owner
+__global__ void __launch_bounds__(256) flagFinish(int64_t N, const unsigned long long* __restrict__ key,
+                                                  uint8_t* __restrict__ flags, int32_t* __restrict__ owner,
+                                                  const int64_t* __restrict__ cnt) {
+  if (cnt[CNT_ERROR] != 0) return;
+  const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= N) return;
+  const unsigned long long kk = key[c];
+  const bool has = kk != ~0ull;
+  const bool prot = has && (kk & 1ull) == 0ull;
+  uint8_t fl = flags[c] & 1;
+  if (has) fl |= 2;
+  if (prot) fl |= 4;
+  if (has && !prot) fl |= 8;
+  if (!prot) fl |= 16;
+  flags[c] = fl;
+  owner[c] = has ? (int32_t)((kk >> 1) & 0x7fffffffull) : -1;
+}
+
+}  // namespace tpc

@@ -1,0 +1,59 @@
+"""-m gpu: the optional a8 cluster flags (through the C ABI) against the oracle's O8: flag bytes and owners bit-exact."""
+import numpy as np
+import pytest
+
+from oracle import tpc_oracle as orc
+from paper_1910_12214_b200 import datagen
+
+pytestmark = pytest.mark.gpu
+
+
+def _both(ev, **par):
+    from paper_1910_12214_b200 import tpc
+    p = tpc.tpcDefaultParams()
+    po = orc.default_params()
+    for k, v in par.items():
+        setattr(p, k, v)
+        if hasattr(po, k):
+            setattr(po, k, v)
+    trk = tpc.TpcTracker.from_event(ev, params=p)
+    off, y, z = trk.upload(ev)
+    res = trk.run(off, y, z, flags=True, merge=True)
+    assert res.status.status == 0
+    g = res.numpy()
+    trk.close()
+    o = orc.run(ev, po, flags=True, merge=True)
+    assert np.array_equal(g["trk_cl_index"].view(np.uint32), o.trk_cl_index)
+    assert np.array_equal(g["cl_owner"], o.cf_owner)
+    assert np.array_equal(g["cl_flags"], o.cf_flags)
+    assert np.array_equal(g["trk_mg_next"], o.mg_next)          # the three optional stages coexist
+    return g, o, res
+
+
+@pytest.mark.parametrize("idx,scale", [(0, 1.0), (1, 0.1), (2, 0.1), (3, 0.05), (4, 0.015)])
+def test_flags_parity(idx, scale):
+    ev = datagen.make_event(idx, scale=scale)
+    g, o, res = _both(ev)
+    f = o.cf_flags
+    assert ((f & 4) != 0).sum() > 0.5 * ev.n_clusters * (0.2 if idx == 4 else 1.0) or idx >= 3
+    assert res.status.flags_ms >= 0.0
+
+
+def test_flags_parity_dead_rows_lattice_ties_and_other_cuts():
+    ev = datagen.make_event(2, scale=0.06, dead_rows=(30, 31, 90))
+    _both(ev)
+    ev2 = datagen.event_from_arrays(ev.row_offset, np.round(ev.y * 4) / 4, np.round(ev.z * 4) / 4, ev.n_sectors, ev.n_rows,
+                                    row_dead=ev.row_dead)                    # clusters exactly on tube borders
+    _both(ev2, tube_radius=1.25)
+    _both(ev, tube_radius=3.0, inv_pt_protect=2.0, clusters_per_cell=0.3)
+    _both(ev, tube_radius=0.0)
+
+
+def test_flags_on_an_event_without_tracks():
+    rng = np.random.default_rng(1)
+    n = 3000
+    rows = np.sort(rng.integers(0, 152, n))
+    off = np.concatenate([[0], np.cumsum(np.bincount(rows, minlength=152))])
+    ev = datagen.event_from_arrays(off, rng.uniform(-10, 10, n), rng.uniform(-200, 200, n), 1, 152)
+    g, o, _ = _both(ev)
+    assert o.n_tracks == 0 and np.all(g["cl_flags"] == 16) and np.all(g["cl_owner"] == -1)
