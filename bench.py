@@ -217,17 +217,22 @@ def run_ours(args, rank, world, local_rank):
     stage /= args.steps
 
     # ---- the NEXT-2 row (a6 refit of the selected tracks), timed apart: it is not part of the a1..a5 step ----------
-    refit_ms = merge_ms = None
+    refit_ms = merge_ms = flags_ms = None
     n_links = 0
+    flag_frac = {}
     if not args.no_refit:
-        acc = accm = 0.0
+        acc = accm = accf = 0.0
         for i in range(4):
-            trk.run(off, y, z, cap_tracklets=capT, cap_tracks=capK, cap_track_clusters=capC, sync=False, merge=True)
+            trk.run(off, y, z, cap_tracklets=capT, cap_tracks=capK, cap_track_clusters=capC, sync=False, merge=True, flags=True)
             s = trk.status()
             if i > 0:
                 acc += float(s.stage_ms[7])
                 accm += float(s.merge_ms)
-        refit_ms, merge_ms = acc / 3, accm / 3
+                accf += float(s.flags_ms)
+        refit_ms, merge_ms, flags_ms = acc / 3, accm / 3, accf / 3
+        fl = trk._out["cl_flags"][:N]
+        flag_frac = {name: round(float(((fl & bit) != 0).float().mean().item()), 4)
+                     for name, bit in (("attached", 1), ("adjacent", 2), ("protected", 4), ("removed_A", 8), ("removed_B", 16))}
         n_links = int((trk._out["trk_mg_next"][:int(s.n_tracks)] >= 0).sum().item())
 
     # ---- end to end through the host-buffer ABI call (pinned host memory; copies inside the timed region) ----
@@ -337,6 +342,8 @@ def run_ours(args, rank, world, local_rank):
                               "tracks": int(st.n_tracks), "track_clusters": ncl}
         line["next_merge"] = {"what": "a7 segment merger (NEXT-1), not part of `value`", "ms": round(merge_ms, 4),
                               "links": n_links}
+        line["next_flags"] = {"what": "a8 cluster flags and rejection strategies A / B (NEXT-3), not part of `value`",
+                              "ms": round(flags_ms, 4), "fractions_of_clusters": flag_frac}
     print(json.dumps(line), flush=True)
 
 
