@@ -466,7 +466,7 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
       const int64_t nk = std::min<int64_t>(out->cap_tracks, capT);
       flagAttach<<<(unsigned)ceilDiv(std::min<int64_t>(out->cap_track_clusters, N), 256), 256, 0, st>>>(out->trk_cl_index,
                                                                                                        out->cl_flags, cnt); ++L;
-      flagBid<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(fi, in->row_offset, P, T, h->params.tube_radius,
+      flagBid<<<(unsigned)ceilDiv(nk * FLAG_GROUP, 128), 128, 0, st>>>(fi, in->row_offset, P, T, h->params.tube_radius,
                                                           h->params.inv_pt_protect, w.desc, w.cell_start, w.syz, w.s2o,
                                                           w.fl_key, cnt); ++L;
     }

@@ -2,7 +2,8 @@
 // (DESIGN.md section 3 "O8", readings R34..R37; NEXT-3 of SURVEY.md 8(f); tube of 1.5 cm, ambiguity
 // to the higher-momentum track, protected = adjacent to a track with pT > 50 MeV/c and |phi| < 70 degrees).
 //
-// One thread per refitted track walks its rows from the inner state by Propagate alone and bids for every cluster in
+// A group of FLAG_GROUP lanes per refitted track walks its rows (every lane of the group carries the same state: the
+// Propagate is redundant but uniform, the candidates of a tube are shared out among the lanes).  The track walks its rows from the inner state by Propagate alone and bids for every cluster in
 // its tube (found through the a1 grid: cells of the box around the tube, exact circle predicate) and for its own
 // attached cluster of the row.  The bid is a 64-bit key  |q/pT| bits : track id : bad  taken with atomicMin, so the
 // owner is the track of minimal (|q/pT|, id) and the key carries whether that track is low-pT or steep at the
@@ -30,13 +31,16 @@ __global__ void __launch_bounds__(256) flagAttach(const uint32_t* __restrict__ c
   flags[cl_index[i]] = 1;
 }
 
+constexpr int FLAG_GROUP = 8;      // lanes per track
+
 __global__ void __launch_bounds__(128) flagBid(FlagIn in, const uint32_t* __restrict__ off, DevParams P, RowTables T,
                                                float tube, float inv_pt_protect, const GridDesc* __restrict__ desc,
                                                const uint32_t* __restrict__ cell_start, const float2* __restrict__ syz,
                                                const uint32_t* __restrict__ s2o, unsigned long long* __restrict__ key,
                                                const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
-  const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const int64_t k = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / FLAG_GROUP;
+  const int sub = threadIdx.x % FLAG_GROUP;
   if (k >= cnt[CNT_N_TRACKS] || k >= in.cap || in.status[k] != 1) return;
   const int64_t cap = in.cap;
   const int R = P.n_rows;
@@ -65,17 +69,25 @@ __global__ void __launch_bounds__(128) flagBid(FlagIn in, const uint32_t* __rest
     // the attached cluster of this row (R35): the list is in ascending row, rows follow from row_offset (R26)
     const uint32_t b_lo = __ldg(off + bsec + r), b_hi = __ldg(off + bsec + r + 1);
     while (ic < ncl && cl[ic] < b_lo) ++ic;
-    if (ic < ncl && cl[ic] < b_hi) atomicMin(key + cl[ic], bid);
-    // the tube: cells of the box around it, exact circle predicate
+    if (sub == 0 && ic < ncl && cl[ic] < b_hi) atomicMin(key + cl[ic], bid);
+    // the tube: cells of the box around it (a hair wider than the tube: fl(dy*dy) <= fl(tube*tube) does not quite imply
+    // |dy| <= tube), exact circle predicate; the lanes of the group take the candidates of a cell row in turn
     const GridDesc G = desc[bsec + r];
     if (G.n == 0) continue;
-    const float yc = S.y, zc = S.z;
-    // (box a hair wider than the tube: fl(dy*dy) <= fl(tube*tube) does not quite imply |dy| <= tube)
-    forWindow(G, cell_start, syz, yc, zc, tube * 1.000001f, tube * 1.000001f, [&](uint32_t pos, float cy, float cz) {
-      const float dy = cy - yc, dz = cz - zc;
-      const float d2 = dy * dy + dz * dz;
-      if (d2 <= tube2) atomicMin(key + __ldg(s2o + pos), bid);
-    });
+    const float yc = S.y, zc = S.z, w = tube * 1.000001f;
+    const float sy = 1e-5f * (fabsf(yc) + w) + 1e-6f, sz = 1e-5f * (fabsf(zc) + w) + 1e-6f;     // superset slack (R3)
+    const int by0 = cellCoord((yc - w) - sy, G.y0, G.inv_e, G.ny), by1 = cellCoord((yc + w) + sy, G.y0, G.inv_e, G.ny);
+    const int bz0 = cellCoord((zc - w) - sz, G.z0, G.inv_e, G.nz), bz1 = cellCoord((zc + w) + sz, G.z0, G.inv_e, G.nz);
+    const uint32_t* cs = cell_start + G.cell_base + by0;
+    for (int bz = bz0; bz <= bz1; ++bz) {
+      const uint32_t k0 = __ldg(cs + bz * G.ny), k1 = __ldg(cs + bz * G.ny + (by1 - by0 + 1));
+      for (uint32_t i = k0 + sub; i < k1; i += FLAG_GROUP) {
+        const float2 c = __ldg(syz + i);
+        const float dy = c.x - yc, dz = c.y - zc;
+        const float d2 = dy * dy + dz * dz;
+        if (d2 <= tube2) atomicMin(key + __ldg(s2o + i), bid);
+      }
+    }
   }
 }
 
