@@ -449,7 +449,7 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
       scanApply<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.mg_start, w.mg_start, cnt + CNT_INF, nscan, w.mg_tiles); ++L;
     }
     mergeFill<<<gK, 256, 0, st>>>(mi, P, T, w.mg_start, w.mg_fill, w.mg_list, cnt); ++L;
-    mergeMatch<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(mi, P, T, mp, w.mg_start, w.mg_maxv, w.mg_list, w.mg_best_b,
+    mergeMatch<<<(unsigned)ceilDiv(nk * MG_GROUP, 128), 128, 0, st>>>(mi, P, T, mp, w.mg_start, w.mg_maxv, w.mg_list, w.mg_best_b,
                                                            w.mg_chi_b, w.mg_key_a, cnt); ++L;
     mergeLink<<<gK, 256, 0, st>>>(mi, mo, w.mg_best_b, w.mg_chi_b, w.mg_key_a, cnt); ++L;
     mergeHead<<<gK, 256, 0, st>>>(mi, mo, cnt); ++L;
