@@ -787,6 +787,26 @@ int refitPoints(const orcGeometry* g, const orcParams* p, int n, const int32_t* 
 
 extern "C" {
 
+int orcPackCharge(int64_t n, const float* q, int nb, uint16_t* code) {
+  if (n < 0 || (n > 0 && (!q || !code)) || nb < 0 || nb > 14) return 0;
+  for (int64_t i = 0; i < n; ++i) {
+    float r = std::rint(q[i]);                       // nearest integer, ties to even
+    if (!(r >= 0.0f)) r = 0.0f;                      // negative and NaN -> 0
+    if (r > 65535.0f) r = 65535.0f;
+    uint32_t v = (uint32_t)r;
+    int L = 0;
+    for (uint32_t t = v; t; t >>= 1) ++L;            // bit length
+    if (L > nb + 1) {
+      const int sh = L - (nb + 1);
+      v = ((v + (1u << (sh - 1))) >> sh) << sh;      // to nearest, ties up; may carry into the next power of two
+      const uint32_t vmax = ((1u << (nb + 1)) - 1u) << (15 - nb);
+      if (v > vmax) v = vmax;
+    }
+    code[i] = (uint16_t)v;
+  }
+  return 1;
+}
+
 int orcRotate(double* state, double* cov, double alpha, double bz_tesla, double max_sinphi, int fp64) {
   return fp64 ? rotateT<double>(state, cov, alpha, bz_tesla, max_sinphi) : rotateT<float>(state, cov, alpha, bz_tesla, max_sinphi);
 }

@@ -101,6 +101,10 @@ void orcGetMerge(const orcResult*, int32_t* next, int32_t* prev, int32_t* head, 
  * owner [n_clusters] track index of the highest-momentum track with the cluster in its tube, -1 none. */
 void orcGetClusterFlags(const orcResult*, uint8_t* flags, int32_t* owner);
 
+/* O9 (part of NEXT-4, DESIGN.md section 3 "O9"): dynamic-precision code of n_values charges: the integer
+ * nearest to q, with every bit more than trunc_bits after its first non-zero bit rounded away.  Returns 0 on bad arguments. */
+int orcPackCharge(int64_t n_values, const float* q, int trunc_bits, uint16_t* code);
+
 /* Pieces of O7 for the pins.  state = {x, y, z, s, t, q}, cov = 15 lower-triangle elements, in/out as doubles.
  * orcRotate: frame turned by alpha (radians); returns 1 on success, 0 (untouched) on failure.
  * orcMatch: chi2 of the match of outer state a to inner state b (b at plane b_state[0]); rel = 0 same sector,

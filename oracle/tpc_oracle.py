@@ -73,6 +73,8 @@ def _load():
         L.orcGetTracks.argtypes = [vp] * 12
         for f in ("orcGetGrid", "orcGetLinks", "orcGetStartHits", "orcGetTracklets", "orcGetTracks"):
             getattr(L, f).restype = None
+        L.orcPackCharge.argtypes = [i64, vp, ci, vp]
+        L.orcPackCharge.restype = ci
         L.orcGetClusterFlags.argtypes = [vp] * 3
         L.orcGetClusterFlags.restype = None
         L.orcGetMerge.argtypes = [vp] * 5
@@ -274,3 +276,12 @@ def match(a_state, a_cov, rel, b_state, b_cov, bz_tesla=0.5, params: Params | No
     ok = _load().orcMatch(ctypes.byref(p), float(bz_tesla), a.ctypes.data, ac.ctypes.data, int(rel), b.ctypes.data,
                           bc.ctypes.data, int(fp64), chi2.ctypes.data)
     return bool(ok), float(chi2[0])
+
+
+def pack_charge(q, trunc_bits=4):
+    """O9: dynamic-precision 16-bit code of the charges."""
+    q = np.ascontiguousarray(q, np.float32)
+    code = np.zeros(q.shape[0], np.uint16)
+    if not _load().orcPackCharge(q.shape[0], _ptr(q), int(trunc_bits), _ptr(code)):
+        raise ValueError("orcPackCharge: bad arguments")
+    return code
