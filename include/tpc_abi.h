@@ -78,6 +78,7 @@ typedef struct {
   float merge_chi2_max;         /* 50         O7: cut on the diagonal chi2 of a match */
   float tube_radius;            /* 1.5        O8: clusters within this distance of a track are adjacent, cm */
   float inv_pt_protect;         /* 20         O8: tracks with |q/pT| below this (pT > 50 MeV/c) protect */
+  int32_t charge_trunc_bits;    /* 4          O9: bits kept after the first non-zero bit of a charge */
 } tpcParams;
 
 /* Input clusters: CSR by (sector,row), fp32 SoA (single-precision cluster properties). */
@@ -87,7 +88,7 @@ typedef struct {
   const float* x;               /* DEVICE [n_clusters] or NULL; not read: a cluster's x is row_x[r] */
   const float* y;               /* DEVICE [n_clusters] local y (pad direction), cm */
   const float* z;               /* DEVICE [n_clusters] z (drift/time direction), cm */
-  const float* q;               /* DEVICE [n_clusters] charge or NULL; not read by this path */
+  const float* q;               /* DEVICE [n_clusters] charge or NULL; read only for the optional cl_qcode output */
 } tpcClusters;
 
 /* Outputs.  All pointers DEVICE.  Tracks are emitted in ascending tracklet id (= rank of the start hit in
@@ -141,6 +142,9 @@ typedef struct {
    * with the refit outputs.  Indexed by the INPUT cluster index. */
   uint8_t* cl_flags;            /* [n_clusters] 1 attached, 2 adjacent, 4 protected, 8 removed by strategy A, 16 by strategy B */
   int32_t* cl_owner;            /* [n_clusters] track with the cluster in its tube (highest momentum), -1 none */
+  /* optional O9 dynamic-precision charge code (DESIGN.md section 3 "O9"); needs tpcClusters.q */
+  uint16_t* cl_qcode;           /* [n_clusters] integer charge with all bits beyond charge_trunc_bits after the first
+                                   non-zero bit rounded away; NULL = not computed */
 } tpcTracks;
 
 /* Filled by tpcGetRunStatus after the stream has drained. */
@@ -158,6 +162,7 @@ typedef struct {
                                    0 grid, 1 neighbour finder, 2 cleaner+start hits, 3 constructor, 4 selector,
                                    5 optional refit, merger and exports, 6 total, 7 refit alone */
   float merge_ms;               /* the O7 merger alone (profiling on, merger requested) */
+  float pack_ms;                /* the O9 charge code alone (profiling on, cl_qcode requested) */
   float flags_ms;               /* the O8 cluster flags alone (profiling on, flags requested) */
   float submit_ms[2];           /* tpcCollectHost only: device time of the slot from its first copy in to the end of its
                                    kernels [0] and to the end of its copies out [1] (includes waiting for the other slot) */

@@ -72,7 +72,8 @@ struct tpcHandle {
   int64_t* d_cnt = nullptr;        // CNT_COUNT counters + 1 slot for the packed selector total
   int64_t* h_cnt = nullptr;        // pinned copy
   cudaEvent_t ev_done = nullptr;
-  cudaEvent_t ev_stage[13] = {};   // 0..6 stage boundaries, 7/8 around the optional refit, 9/10 merger, 11/12 flags
+  cudaEvent_t ev_stage[15] = {};   // ... 13/14 around the charge code
+  //   // 0..6 stage boundaries, 7/8 around the optional refit, 9/10 merger, 11/12 flags
   int profiling = 0;
   int launches = 0;
   int tc_grid = 148;               // persistent grid of the tracklet constructor: SMs x resident blocks
@@ -192,7 +193,7 @@ int tpcDefaultParams(tpcParams* p) {
   p->cell_min = 0.5f; p->cell_max = 8.0f; p->clusters_per_cell = 1.0f;
   p->validate_input = 0; p->force_wide_keys = 0;
   p->merge_max_row_gap = 40; p->merge_back_rows = 5; p->merge_chi2_max = 50.0f;
-  p->tube_radius = 1.5f; p->inv_pt_protect = 20.0f;
+  p->tube_radius = 1.5f; p->inv_pt_protect = 20.0f; p->charge_trunc_bits = 4;
   return TPC_OK;
 }
 
@@ -207,7 +208,7 @@ int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cud
   if (!(p->cell_min > 0) || !(p->cell_max >= p->cell_min) || !(p->clusters_per_cell > 0)) return TPC_ERR_INVALID_ARG;
   if (p->min_chain_hits < 2 || p->max_row_gap < 0) return TPC_ERR_INVALID_ARG;
   if (p->merge_max_row_gap < 0 || p->merge_back_rows < 0) return TPC_ERR_INVALID_ARG;
-  if (!(p->tube_radius >= 0)) return TPC_ERR_INVALID_ARG;
+  if (!(p->tube_radius >= 0) || p->charge_trunc_bits < 0 || p->charge_trunc_bits > 14) return TPC_ERR_INVALID_ARG;
   tpcHandle* h = new (std::nothrow) tpcHandle();
   if (!h) return TPC_ERR_INVALID_ARG;
   h->device = cuda_device;
@@ -248,7 +249,7 @@ int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cud
             cudaMalloc(&h->d_cnt, 8 * (CNT_COUNT + 1)) == cudaSuccess &&
             cudaMallocHost(&h->h_cnt, 8 * (CNT_COUNT + 1)) == cudaSuccess &&
             cudaEventCreate(&h->ev_done) == cudaSuccess;
-  for (int i = 0; ok && i < 13; ++i) ok = cudaEventCreate(&h->ev_stage[i]) == cudaSuccess;
+  for (int i = 0; ok && i < 15; ++i) ok = cudaEventCreate(&h->ev_stage[i]) == cudaSuccess;
   ok = ok && cudaMemcpy(h->d_row_x, g->row_x, 4 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
        cudaMemcpy(h->d_up, up.data(), 2 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
        cudaMemcpy(h->d_dn, dn.data(), 2 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
@@ -273,7 +274,7 @@ int tpcDestroy(tpcHandle* h) {
   cudaFree(h->d_row_x); cudaFree(h->d_up); cudaFree(h->d_dn); cudaFree(h->d_dead); cudaFree(h->d_cnt);
   if (h->h_cnt) cudaFreeHost(h->h_cnt);
   if (h->ev_done) cudaEventDestroy(h->ev_done);
-  for (int i = 0; i < 13; ++i) if (h->ev_stage[i]) cudaEventDestroy(h->ev_stage[i]);
+  for (int i = 0; i < 15; ++i) if (h->ev_stage[i]) cudaEventDestroy(h->ev_stage[i]);
   if (h->cur_slot != 0) {}   // the active state is freed below; the parked slots here
   for (int k = 0; k < 3; ++k) {
     if (k == h->cur_slot || !h->slots[k].init) continue;
@@ -325,6 +326,7 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   const int n_mg = (out->trk_mg_next != nullptr) + (out->trk_mg_prev != nullptr) + (out->trk_mg_head != nullptr) +
                    (out->trk_mg_chi2 != nullptr);
   if ((n_mg != 0 && n_mg != 4) || (n_mg == 4 && n_rf != 8)) return TPC_ERR_INVALID_ARG;   // the merger needs the refit
+  if (out->cl_qcode && N > 0 && !in->q) return TPC_ERR_INVALID_ARG;                      // the charge code needs the charges
   const int n_fl = (out->cl_flags != nullptr) + (out->cl_owner != nullptr);
   if ((n_fl != 0 && n_fl != 2) || (n_fl == 2 && n_rf != 8)) return TPC_ERR_INVALID_ARG;   // so do the cluster flags
   if (!workspace || ((uintptr_t)workspace % ALIGN) != 0) return TPC_ERR_INVALID_ARG;
@@ -473,6 +475,12 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
     flagFinish<<<gN256, 256, 0, st>>>(N, w.fl_key, out->cl_flags, out->cl_owner, cnt); ++L;
   }
   stage(12);
+  // ---- a9 optional dynamic-precision charge code (O9) ------------------------------------------------
+  stage(13);
+  if (out->cl_qcode && N > 0) {
+    packCharge<<<(unsigned)ceilDiv(ceilDiv(N, 4), 256), 256, 0, st>>>(N, in->q, h->params.charge_trunc_bits, out->cl_qcode); ++L;
+  }
+  stage(14);
   // ---- optional per-stage exports -----------------------------------------------------------------
   if (N > 0 && (out->link_up_raw || out->link_dn_raw || out->link_up || out->link_dn)) {
     exportLinks<<<gN256, 256, 0, st>>>(N, w.s2o, w.lup, w.ldn, w.cup, w.cdn, out->link_up_raw, out->link_dn_raw,
@@ -519,6 +527,7 @@ int tpcGetRunStatus(tpcHandle* h, tpcRunStatus* out) {
     if (cudaEventElapsedTime(&ms, h->ev_stage[7], h->ev_stage[8]) == cudaSuccess) out->stage_ms[7] = ms;
     if (cudaEventElapsedTime(&ms, h->ev_stage[9], h->ev_stage[10]) == cudaSuccess) out->merge_ms = ms;
     if (cudaEventElapsedTime(&ms, h->ev_stage[11], h->ev_stage[12]) == cudaSuccess) out->flags_ms = ms;
+    if (cudaEventElapsedTime(&ms, h->ev_stage[13], h->ev_stage[14]) == cudaSuccess) out->pack_ms = ms;
   }
   return TPC_OK;
 }
@@ -563,7 +572,7 @@ extern "C" int tpcRunHost(tpcHandle* h, int64_t N, const uint32_t* row_offset, c
       oh->tl_first_row || oh->tl_last_row || oh->tl_rowhit || oh->tl_x || oh->tl_par || oh->tl_cov || oh->tl_chi2 ||
       oh->trk_rf_status || oh->trk_rf_x_in || oh->trk_rf_par_in || oh->trk_rf_cov_in || oh->trk_rf_chi2 || oh->trk_rf_x_out ||
       oh->trk_rf_par_out || oh->trk_rf_cov_out || oh->trk_mg_next || oh->trk_mg_prev || oh->trk_mg_head || oh->trk_mg_chi2 ||
-      oh->cl_flags || oh->cl_owner)
+      oh->cl_flags || oh->cl_owner || oh->cl_qcode)
     return TPC_ERR_INVALID_ARG;
   if (!oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0) return TPC_ERR_INVALID_ARG;
   TPC_CUDA(h, cudaSetDevice(h->device));
@@ -673,7 +682,7 @@ extern "C" int tpcSubmitHost(tpcHandle* h, int slot, int64_t N, const uint32_t* 
     return TPC_ERR_INVALID_ARG;
   if (oh->link_up_raw || oh->link_dn_raw || oh->link_up || oh->link_dn || oh->start_hits || oh->tl_status || oh->tl_nhits ||
       oh->tl_first_row || oh->tl_last_row || oh->tl_rowhit || oh->tl_x || oh->tl_par || oh->tl_cov || oh->tl_chi2 ||
-      oh->trk_rf_status || oh->trk_mg_next || oh->cl_flags || oh->cl_owner || !oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0)
+      oh->trk_rf_status || oh->trk_mg_next || oh->cl_flags || oh->cl_owner || oh->cl_qcode || !oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0)
     return TPC_ERR_INVALID_ARG;
   TPC_CUDA(h, cudaSetDevice(h->device));
   int rc;

@@ -110,4 +110,32 @@ __global__ void __launch_bounds__(256) flagFinish(int64_t N, const unsigned long
   owner[c] = has ? (int32_t)((kk >> 1) & 0x7fffffffull) : -1;
 }
 
+// a9 (part of NEXT-4; DESIGN.md section 3 "O9"): dynamic-precision 16-bit code of the cluster charges.
+// Streaming: 4 bytes in, 2 bytes out per cluster; four clusters per thread (16-byte load, 8-byte store).
+__device__ __forceinline__ uint32_t packOne(float q, int nb) {
+  float r = rintf(q);                              // nearest integer, ties to even
+  if (!(r >= 0.0f)) r = 0.0f;                      // negative and NaN -> 0
+  if (r > 65535.0f) r = 65535.0f;
+  uint32_t v = (uint32_t)r;
+  const int L = 32 - __clz(v);                     // bit length (0 for v = 0)
+  if (L > nb + 1) {
+    const int sh = L - (nb + 1);
+    v = ((v + (1u << (sh - 1))) >> sh) << sh;      // to nearest, ties up
+    v = min(v, ((1u << (nb + 1)) - 1u) << (15 - nb));
+  }
+  return v;
+}
+
+__global__ void __launch_bounds__(256) packCharge(int64_t N, const float* __restrict__ q, int nb, uint16_t* __restrict__ code) {
+  const int64_t i4 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * 4;
+  if (i4 >= N) return;
+  if (i4 + 4 <= N && (((uintptr_t)q | ((uintptr_t)code << 1)) & 15) == 0) {
+    const float4 v = *reinterpret_cast<const float4*>(q + i4);
+    const uint32_t a = packOne(v.x, nb) | (packOne(v.y, nb) << 16), b = packOne(v.z, nb) | (packOne(v.w, nb) << 16);
+    *reinterpret_cast<uint2*>(code + i4) = make_uint2(a, b);
+  } else {
+    for (int64_t i = i4; i < min(i4 + 4, N); ++i) code[i] = (uint16_t)packOne(q[i], nb);
+  }
+}
+
 }  // namespace tpc

@@ -37,7 +37,7 @@ class tpcParams(ctypes.Structure):
                [("cell_min", c_float), ("cell_max", c_float), ("clusters_per_cell", c_float),
                 ("validate_input", c_int32), ("force_wide_keys", c_int32), ("merge_max_row_gap", c_int32),
                 ("merge_back_rows", c_int32), ("merge_chi2_max", c_float), ("tube_radius", c_float),
-                ("inv_pt_protect", c_float)]
+                ("inv_pt_protect", c_float), ("charge_trunc_bits", c_int32)]
 
 
 class tpcClusters(ctypes.Structure):
@@ -53,17 +53,18 @@ _REFIT_PTRS = ("trk_rf_status", "trk_rf_x_in", "trk_rf_par_in", "trk_rf_cov_in",
                "trk_rf_par_out", "trk_rf_cov_out")
 _MERGE_PTRS = ("trk_mg_next", "trk_mg_prev", "trk_mg_head", "trk_mg_chi2")
 _FLAG_PTRS = ("cl_flags", "cl_owner")
+_PACK_PTRS = ("cl_qcode",)
 
 
 class tpcTracks(ctypes.Structure):
     _fields_ = [("cap_tracks", c_int64), ("cap_track_clusters", c_int64)] + \
-               [(n, c_void_p) for n in _TRK_PTRS + _STAGE_PTRS + _REFIT_PTRS + _MERGE_PTRS + _FLAG_PTRS]
+               [(n, c_void_p) for n in _TRK_PTRS + _STAGE_PTRS + _REFIT_PTRS + _MERGE_PTRS + _FLAG_PTRS + _PACK_PTRS]
 
 
 class tpcRunStatus(ctypes.Structure):
     _fields_ = [("status", c_int32), ("kernel_launches", c_int32), ("n_clusters", c_int64), ("n_start_hits", c_int64),
                 ("n_tracklets", c_int64), ("n_tracklet_hits", c_int64), ("n_tracks", c_int64),
-                ("n_track_clusters", c_int64), ("n_cells", c_int64), ("stage_ms", c_float * 8), ("merge_ms", c_float), ("flags_ms", c_float), ("submit_ms", c_float * 2)]
+                ("n_track_clusters", c_int64), ("n_cells", c_int64), ("stage_ms", c_float * 8), ("merge_ms", c_float), ("pack_ms", c_float), ("flags_ms", c_float), ("submit_ms", c_float * 2)]
 
 
 ABI_SYMBOLS = ("tpcDefaultParams", "tpcCreate", "tpcDestroy", "tpcWorkspaceBytes", "tpcRun", "tpcGetRunStatus",
@@ -233,7 +234,7 @@ class TpcTracker:
         z = t.from_numpy(np.ascontiguousarray(ev.z, np.float32)).to(self.device)
         return off, y, z
 
-    def _ensure(self, n, capT, capK, capC, stages, refit=False, merge=False, flags=False):
+    def _ensure(self, n, capT, capK, capC, stages, refit=False, merge=False, flags=False, pack=False):
         t = self.torch
         need = tpcWorkspaceBytes(self.handle, n, capT)
         if self._ws is None or self._ws.numel() < need:
@@ -256,6 +257,8 @@ class TpcTracker:
             spec.update({"trk_rf_status": ((capK,), i32), "trk_rf_x_in": ((capK,), f32), "trk_rf_par_in": ((5, capK), f32),
                          "trk_rf_cov_in": ((15, capK), f32), "trk_rf_chi2": ((capK,), f32), "trk_rf_x_out": ((capK,), f32),
                          "trk_rf_par_out": ((5, capK), f32), "trk_rf_cov_out": ((15, capK), f32)})
+        if pack:
+            spec.update({"cl_qcode": ((max(n, 1),), t.int16)})
         if flags:
             spec.update({"cl_flags": ((max(n, 1),), t.uint8), "cl_owner": ((max(n, 1),), i32)})
         if merge:
@@ -271,8 +274,8 @@ class TpcTracker:
 
     def run(self, row_offset, y, z, cap_tracklets: int | None = None, cap_tracks: int | None = None,
             cap_track_clusters: int | None = None, stages: bool = False, stream=None, sync: bool = True,
-            grow: bool = True, refit: bool = False, merge: bool = False, flags: bool = False):
-        """One tpcRun on device tensors.  Returns a TrackResult (after synchronising) or None when sync=False."""
+            grow: bool = True, refit: bool = False, merge: bool = False, flags: bool = False, q=None):
+        """One tpcRun on device tensors (q: optional device tensor of charges -> cl_qcode, the O9 charge code).  Returns a TrackResult (after synchronising) or None when sync=False."""
         t = self.torch
         n = int(y.shape[0])
         refit = refit or merge or flags   # the merger and the cluster flags work on the refitted states
@@ -281,9 +284,9 @@ class TpcTracker:
         capC = int(cap_track_clusters) if cap_track_clusters is not None else max(n, 1)
         attempts = 3 if grow else 0     # a too-small cap_tracklets hides the true track counts: up to 3 rounds
         while True:
-            self._ensure(n, capT, capK, capC, stages, refit, merge, flags)
+            self._ensure(n, capT, capK, capC, stages, refit, merge, flags, q is not None)
             cl = tpcClusters(n, row_offset.data_ptr(), None, y.data_ptr() if n else None, z.data_ptr() if n else None,
-                             None)
+                             q.data_ptr() if (q is not None and n) else None)
             tr = tpcTracks()
             tr.cap_tracks, tr.cap_track_clusters = capK, capC
             for k, v in self._out.items():
@@ -318,6 +321,8 @@ class TpcTracker:
         if flags:
             for k in _FLAG_PTRS:
                 trk[k] = o[k][:n]
+        if q is not None:
+            trk["cl_qcode"] = o["cl_qcode"][:n]
         stg = {}
         if stages:
             for k in _STAGE_PTRS:

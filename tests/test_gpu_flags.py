@@ -57,3 +57,25 @@ def test_flags_on_an_event_without_tracks():
     ev = datagen.event_from_arrays(off, rng.uniform(-10, 10, n), rng.uniform(-200, 200, n), 1, 152)
     g, o, _ = _both(ev)
     assert o.n_tracks == 0 and np.all(g["cl_flags"] == 16) and np.all(g["cl_owner"] == -1)
+
+
+@pytest.mark.parametrize("nb", [4, 3, 0, 9])
+def test_charge_code_parity(nb):
+    """a9 (O9): the 16-bit dynamic-precision charge code, bit-exact; inputs cover the 16-bit range, halves
+    (ties), negatives, NaN, infinities and a ragged tail."""
+    import torch
+    from paper_1910_12214_b200 import tpc
+    ev = datagen.make_event(1, scale=0.03)
+    n = ev.n_clusters
+    rng = np.random.default_rng(5)
+    q = np.concatenate([ev.q[: n // 2], rng.uniform(0, 70000, n - n // 2 - 9).astype(np.float32),
+                        np.array([0.5, 1.5, 2.5, -1.0, np.nan, np.inf, -np.inf, 65535.4, 33.0], np.float32)]).astype(np.float32)
+    p = tpc.tpcDefaultParams()
+    p.charge_trunc_bits = nb
+    trk = tpc.TpcTracker.from_event(ev, params=p)
+    off, y, z = trk.upload(ev)
+    res = trk.run(off, y, z, q=torch.from_numpy(q).cuda())
+    assert res.status.status == 0
+    got = res.trk["cl_qcode"].cpu().numpy().view(np.uint16)
+    assert np.array_equal(got, orc.pack_charge(q, nb))
+    trk.close()
