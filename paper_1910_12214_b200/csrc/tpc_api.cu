@@ -478,7 +478,7 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   // ---- a9 optional dynamic-precision charge code (O9) ------------------------------------------------
   stage(13);
   if (out->cl_qcode && N > 0) {
-    packCharge<<<(unsigned)ceilDiv(ceilDiv(N, 4), 256), 256, 0, st>>>(N, in->q, h->params.charge_trunc_bits, out->cl_qcode); ++L;
+    packCharge<<<(unsigned)ceilDiv(ceilDiv(N, 8), 256), 256, 0, st>>>(N, in->q, h->params.charge_trunc_bits, out->cl_qcode); ++L;
   }
   stage(14);
   // ---- optional per-stage exports -----------------------------------------------------------------

@@ -111,7 +111,7 @@ __global__ void __launch_bounds__(256) flagFinish(int64_t N, const unsigned long
 }
 
 // a9 (part of NEXT-4; DESIGN.md section 3 "O9"): dynamic-precision 16-bit code of the cluster charges.
-// Streaming: 4 bytes in, 2 bytes out per cluster; four clusters per thread (16-byte load, 8-byte store).
+// Streaming: 4 bytes in, 2 bytes out per cluster; eight clusters per thread (two 16-byte loads, one 16-byte store).
 __device__ __forceinline__ uint32_t packOne(float q, int nb) {
   float r = rintf(q);                              // nearest integer, ties to even
   if (!(r >= 0.0f)) r = 0.0f;                      // negative and NaN -> 0
@@ -127,14 +127,17 @@ __device__ __forceinline__ uint32_t packOne(float q, int nb) {
 }
 
 __global__ void __launch_bounds__(256) packCharge(int64_t N, const float* __restrict__ q, int nb, uint16_t* __restrict__ code) {
-  const int64_t i4 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * 4;
-  if (i4 >= N) return;
-  if (i4 + 4 <= N && (((uintptr_t)q | ((uintptr_t)code << 1)) & 15) == 0) {
-    const float4 v = *reinterpret_cast<const float4*>(q + i4);
-    const uint32_t a = packOne(v.x, nb) | (packOne(v.y, nb) << 16), b = packOne(v.z, nb) | (packOne(v.w, nb) << 16);
-    *reinterpret_cast<uint2*>(code + i4) = make_uint2(a, b);
+  const int64_t i8 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * 8;
+  if (i8 >= N) return;
+  if (i8 + 8 <= N && (((uintptr_t)q | (uintptr_t)code) & 15) == 0) {     // eight clusters: 2 x 16 bytes in, 16 bytes out
+    const float4 v = __ldcs(reinterpret_cast<const float4*>(q + i8));
+    const float4 w = __ldcs(reinterpret_cast<const float4*>(q + i8) + 1);
+    uint4 o;
+    o.x = packOne(v.x, nb) | (packOne(v.y, nb) << 16); o.y = packOne(v.z, nb) | (packOne(v.w, nb) << 16);
+    o.z = packOne(w.x, nb) | (packOne(w.y, nb) << 16); o.w = packOne(w.z, nb) | (packOne(w.w, nb) << 16);
+    __stcs(reinterpret_cast<uint4*>(code + i8), o);
   } else {
-    for (int64_t i = i4; i < min(i4 + 4, N); ++i) code[i] = (uint16_t)packOne(q[i], nb);
+    for (int64_t i = i8; i < min(i8 + 8, N); ++i) code[i] = (uint16_t)packOne(q[i], nb);
   }
 }
 
