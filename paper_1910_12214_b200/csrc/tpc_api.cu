@@ -33,6 +33,7 @@ inline int64_t ceilDiv(int64_t a, int64_t b) { return (a + b - 1) / b; }
 struct Workspace {
   GridDesc* desc;
   uint32_t* chunk_base;      // [nb+1] first neighbour-finder CTA of every bucket
+  uint32_t* chunk_bucket;    // [ceil(N/128)+nb] bucket of every neighbour-finder CTA
   uint32_t* cell_start;
   uint32_t* rank;            // aliases spos_by_orig (a1 only)
   float2* syz;
@@ -128,6 +129,7 @@ Workspace layout(const tpcHandle* h, int64_t N, int64_t capT, char* base) {
   const int64_t Nn = N > 0 ? N : 1, Tn = capT > 0 ? capT : 1;
   w.desc = (GridDesc*)take(sizeof(GridDesc) * nb);
   w.chunk_base = (uint32_t*)take(4 * (size_t)(nb + 1));
+  w.chunk_bucket = (uint32_t*)take(4 * (size_t)(ceilDiv(Nn, NF_THREADS) + nb));
   w.cell_start = (uint32_t*)take(4 * (size_t)(cc + 1));
   w.spos_by_orig = (int32_t*)take(4 * (size_t)Nn);
   w.rank = (uint32_t*)w.spos_by_orig;
@@ -363,7 +365,9 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   // ---- a2 neighbour finder ------------------------------------------------------------------------
   if (N > 0) {
     // one CTA per chunk of NF_THREADS clusters of one bucket; the exact CTA count is on the device (chunk_base[nb])
-    neighbourFinder<<<(unsigned)(ceilDiv(N, NF_THREADS) + nb), NF_THREADS, 0, st>>>(w.chunk_base, P, T, w.desc, w.cell_start,
+    const int64_t max_chunks = ceilDiv(N, NF_THREADS) + nb;
+    chunkFill<<<(unsigned)ceilDiv(max_chunks, 256), 256, 0, st>>>(w.chunk_base, nb, max_chunks, w.chunk_bucket, cnt); ++L;
+    neighbourFinder<<<(unsigned)max_chunks, NF_THREADS, 0, st>>>(w.chunk_base, w.chunk_bucket, P, T, w.desc, w.cell_start,
                                                                                     w.syz, w.s2o, w.lup, w.ldn, cnt); ++L;
   }
   stage(2);

@@ -115,7 +115,23 @@ __device__ __forceinline__ int gatherWindow(const GridDesc& G, const uint32_t* _
   return n;
 }
 
-__global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __restrict__ chunk_base, DevParams P, RowTables T,
+// thread per neighbour-finder CTA: its bucket (largest b with chunk_base[b] <= cta), so that the CTAs themselves start
+// with one load instead of a dependent binary search by one thread while 127 wait
+__global__ void __launch_bounds__(256) chunkFill(const uint32_t* __restrict__ chunk_base, int nb, int64_t max_chunks,
+                                                 uint32_t* __restrict__ chunk_bucket, const int64_t* __restrict__ cnt) {
+  if (cnt[CNT_ERROR] != 0) return;
+  const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= max_chunks || c >= __ldg(chunk_base + nb)) return;
+  int lo = 0, hi = nb;
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (__ldg(chunk_base + mid) <= (uint32_t)c) lo = mid; else hi = mid;
+  }
+  chunk_bucket[c] = (uint32_t)lo;
+}
+
+__global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __restrict__ chunk_base,
+                                                              const uint32_t* __restrict__ chunk_bucket, DevParams P, RowTables T,
                                                               const GridDesc* __restrict__ desc,
                                                               const uint32_t* __restrict__ cell_start,
                                                               const float2* __restrict__ syz,
@@ -130,22 +146,12 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
   static_assert(sizeof(float) * NF_ITEMS * NF_UB >= sizeof(ushort2) * NF_ROWS * NF_THREADS, "srow aliases it_dev");
   __shared__ float red[2][NF_THREADS / 32];
   __shared__ uint32_t sscan[33];
-  __shared__ int sm_b;
   __shared__ uint32_t sm_T;
   if (cnt[CNT_ERROR] != 0) return;
   const int tid = threadIdx.x;
   const int nb = P.n_buckets;
   if (blockIdx.x >= __ldg(chunk_base + nb)) return;
-  if (tid == 0) {   // bucket of this chunk: largest b with chunk_base[b] <= blockIdx.x
-    int lo = 0, hi = nb;
-    while (hi - lo > 1) {
-      const int mid = (lo + hi) >> 1;
-      if (__ldg(chunk_base + mid) <= blockIdx.x) lo = mid; else hi = mid;
-    }
-    sm_b = lo;
-  }
-  __syncthreads();
-  const int b = sm_b;
+  const int b = (int)__ldg(chunk_bucket + blockIdx.x);
   const GridDesc Gh = desc[b];
   const uint32_t p = Gh.lo + (blockIdx.x - __ldg(chunk_base + b)) * NF_THREADS + tid;
   const bool valid = p < Gh.lo + Gh.n;
