@@ -26,10 +26,13 @@ constexpr int NF_REGION = 640;     // staged candidates per side
 #define NF_LIST_ 32
 #endif
 #ifndef NF_ITEMS_
-#define NF_ITEMS_ 512
+#define NF_ITEMS_ 640
 #endif
 constexpr int NF_LIST = NF_LIST_;  // window candidates kept per thread and side (<= 32: packed item code)
-constexpr int NF_UB = 4;          // u's per item (register blocking of the pair loop)
+#ifndef NF_UB_
+#define NF_UB_ 2
+#endif
+constexpr int NF_UB = NF_UB_;          // u's per item (register blocking of the pair loop)
 constexpr int NF_ITEMS = NF_ITEMS_; // items per CTA and round
 constexpr int NF_ROWS = 6;         // cell rows of a window whose ranges are staged (more: slow path)
 
