@@ -69,7 +69,7 @@ typedef struct {
   int32_t min_tracklet_hits;    /* 10 */
   int32_t min_track_hits;       /* 10 */
   float cell_min, cell_max;     /* 0.5, 8.0   grid cell edge limits, cm (O1; do not change results, R3) */
-  float clusters_per_cell;      /* 1.0        target occupancy of a grid cell (implementation choice, R3) */
+  float clusters_per_cell;      /* 0.7        target occupancy of a grid cell (implementation choice, R3) */
   int32_t validate_input;       /* 0          1 = scan y,z for NaN/Inf and fail with TPC_ERR_NONFINITE_INPUT */
   int32_t force_wide_keys;      /* 0          1 = use the two-pass selector keys even when the packed 64-bit key
                                               fits (R27; results are identical, for tests) */

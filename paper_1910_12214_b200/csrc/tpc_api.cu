@@ -192,7 +192,7 @@ int tpcDefaultParams(tpcParams* p) {
   p->turn_var_scale = 100.0f; p->max_sinphi = 0.98f;
   p->road_sigma = 4.0f; p->road_min = 0.3f; p->road_max = 2.0f;
   p->max_row_gap = 4; p->min_chain_hits = 3; p->min_tracklet_hits = 10; p->min_track_hits = 10;
-  p->cell_min = 0.5f; p->cell_max = 8.0f; p->clusters_per_cell = 1.0f;
+  p->cell_min = 0.5f; p->cell_max = 8.0f; p->clusters_per_cell = 0.7f;
   p->validate_input = 0; p->force_wide_keys = 0;
   p->merge_max_row_gap = 40; p->merge_back_rows = 5; p->merge_chi2_max = 50.0f;
   p->tube_radius = 1.5f; p->inv_pt_protect = 20.0f; p->charge_trunc_bits = 4;

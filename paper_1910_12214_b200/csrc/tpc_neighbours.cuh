@@ -21,7 +21,10 @@
 namespace tpc {
 
 constexpr int NF_THREADS = 128;
-constexpr int NF_REGION = 640;     // staged candidates per side
+#ifndef NF_REGION_
+#define NF_REGION_ 640
+#endif
+constexpr int NF_REGION = NF_REGION_;     // staged candidates per side
 #ifndef NF_LIST_
 #define NF_LIST_ 32
 #endif
