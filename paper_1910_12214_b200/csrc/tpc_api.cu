@@ -393,6 +393,13 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
                                                      w.tl, cnt); ++L;
   }
   stage(4);
+  // optional per-stage export of the tracklets: before the selector, which compacts the row-hit slices in place
+  if (N > 0 && capT > 0 && (out->start_hits || out->tl_status || out->tl_nhits || out->tl_first_row || out->tl_last_row ||
+                            out->tl_rowhit || out->tl_x || out->tl_par || out->tl_cov || out->tl_chi2)) {
+    const TrackletOut xo{out->start_hits, out->tl_status, out->tl_nhits, out->tl_first_row, out->tl_last_row,
+                         out->tl_rowhit, out->tl_x, out->tl_par, out->tl_cov, out->tl_chi2};
+    exportTracklets<<<(unsigned)ceilDiv(capT, 128), 128, 0, st>>>(w.tl, w.start_orig, w.s2o, P.n_rows, xo, cnt); ++L;
+  }
   // ---- a5 selector ----------------------------------------------------------------------------------
   const TrackOut to{out->cap_tracks, out->cap_track_clusters, out->trk_tracklet, out->trk_sector, out->trk_first_row,
                     out->trk_last_row, out->trk_ncl, out->trk_x, out->trk_par, out->trk_cov, out->trk_chi2,
@@ -489,12 +496,6 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   if (N > 0 && (out->link_up_raw || out->link_dn_raw || out->link_up || out->link_dn)) {
     exportLinks<<<gN256, 256, 0, st>>>(N, w.s2o, w.lup, w.ldn, w.cup, w.cdn, out->link_up_raw, out->link_dn_raw,
                                        out->link_up, out->link_dn, cnt); ++L;
-  }
-  if (N > 0 && capT > 0 && (out->start_hits || out->tl_status || out->tl_nhits || out->tl_first_row || out->tl_last_row ||
-                            out->tl_rowhit || out->tl_x || out->tl_par || out->tl_cov || out->tl_chi2)) {
-    const TrackletOut xo{out->start_hits, out->tl_status, out->tl_nhits, out->tl_first_row, out->tl_last_row,
-                         out->tl_rowhit, out->tl_x, out->tl_par, out->tl_cov, out->tl_chi2};
-    exportTracklets<<<(unsigned)ceilDiv(capT, 128), 128, 0, st>>>(w.tl, w.start_orig, w.s2o, P.n_rows, xo, cnt); ++L;
   }
   stage(6);
   TPC_CUDA(h, cudaGetLastError());

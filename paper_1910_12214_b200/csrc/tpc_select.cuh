@@ -54,6 +54,7 @@ __device__ __forceinline__ bool owns(int32_t c, unsigned long long key, uint32_t
 
 // per tracklet: kept = hits it owns; a track iff kept >= min_track_hits (single pass, R21).
 // tsel[t] = is_track | kept << 32 (0 when not a track).  Also counts accepted tracklets and their hits.
+// NOTE: rewrites the front of every accepted tracklet's row-hit slice (exports of the row hits run before this kernel).
 __global__ void __launch_bounds__(128) selectCount(TrackletStore tl, const unsigned long long* __restrict__ owner_key,
                                                    const uint32_t* __restrict__ owner_id, int wide, int min_track_hits,
                                                    unsigned long long* __restrict__ tsel, int32_t* __restrict__ kept_first,
@@ -69,10 +70,16 @@ __global__ void __launch_bounds__(128) selectCount(TrackletStore tl, const unsig
       acc = 1ull | ((unsigned long long)nh << 32);
       const unsigned long long key = selKey(nh, tl.chi2[t], (uint32_t)t, wide != 0);
       int kept = 0, first = -1, last = -1;
-      const int r1 = tl.last_row[t];
-      for (int r = tl.first_row[t]; r <= r1; ++r) {
-        const int32_t c = tl.rowhit[t * tl.n_rows + r];
-        if (c >= 0 && owns(c, key, (uint32_t)t, wide, owner_key, owner_id)) { ++kept; if (first < 0) first = r; last = r; }
+      const int f = tl.first_row[t], r1 = tl.last_row[t];
+      int32_t* row = tl.rowhit + t * tl.n_rows;
+      // the kept hits are compacted to the front of the tracklet's own row-hit slice (the write index never passes the
+      // read index), so that selectEmit copies `kept` entries instead of walking the rows and the owner keys again
+      for (int r = f; r <= r1; ++r) {
+        const int32_t c = row[r];
+        if (c >= 0 && owns(c, key, (uint32_t)t, wide, owner_key, owner_id)) {
+          row[f + kept] = c;
+          ++kept; if (first < 0) first = r; last = r;
+        }
       }
       if (kept >= min_track_hits) {
         sel = 1ull | ((unsigned long long)kept << 32);
@@ -130,16 +137,10 @@ __global__ void __launch_bounds__(128) selectEmit(TrackletStore tl, const unsign
 #pragma unroll
   for (int i = 0; i < 15; ++i) o.cov[i * capK + k] = tl.cov[i * capT + t];
   o.cl_offset[k] = (uint32_t)off;
-  const unsigned long long key = selKey(tl.nhits[t], tl.chi2[t], (uint32_t)t, wide != 0);
-  int64_t w = off;
-  const int r1 = tl.last_row[t];
-  for (int r = tl.first_row[t]; r <= r1; ++r) {
-    const int32_t c = tl.rowhit[t * tl.n_rows + r];
-    if (c >= 0 && owns(c, key, (uint32_t)t, wide, owner_key, owner_id)) {
-      if (w < o.cap_cl) o.cl_index[w] = s2o[c];
-      ++w;
-    }
-  }
+  const int kept = (int)(sel >> 32);
+  const int32_t* row = tl.rowhit + t * tl.n_rows + tl.first_row[t];      // compacted by selectCount
+  for (int i = 0; i < kept; ++i)
+    if (off + i < o.cap_cl) o.cl_index[off + i] = s2o[row[i]];
 }
 
 // one thread: totals, closing CSR offset, capacity status.
