@@ -20,7 +20,10 @@
 
 namespace tpc {
 
-constexpr int NF_THREADS = 128;
+#ifndef NF_THREADS_
+#define NF_THREADS_ 128
+#endif
+constexpr int NF_THREADS = NF_THREADS_;
 #ifndef NF_REGION_
 #define NF_REGION_ 640
 #endif
@@ -183,8 +186,9 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
   }
   if ((tid & 31) == 0) { red[0][tid >> 5] = zlo; red[1][tid >> 5] = zhi; }
   __syncthreads();
-  zlo = fminf(fminf(red[0][0], red[0][1]), fminf(red[0][2], red[0][3]));
-  zhi = fmaxf(fmaxf(red[1][0], red[1][1]), fmaxf(red[1][2], red[1][3]));
+  zlo = red[0][0]; zhi = red[1][0];
+#pragma unroll
+  for (int w = 1; w < NF_THREADS / 32; ++w) { zlo = fminf(zlo, red[0][w]); zhi = fmaxf(zhi, red[1][w]); }
   uint32_t kD0 = 0, kD1 = 0, kU0 = 0, kU1 = 0;
   {
     const float s = 1e-5f * (fmaxf(fabsf(zlo), fabsf(zhi)) + wzu + wzd) + 1e-6f;

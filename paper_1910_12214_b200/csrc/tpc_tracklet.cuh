@@ -10,7 +10,10 @@
 
 namespace tpc {
 
-constexpr int TC_THREADS = 128;
+#ifndef TC_THREADS_
+#define TC_THREADS_ 128
+#endif
+constexpr int TC_THREADS = TC_THREADS_;
 #ifndef TC_MIN_BLOCKS
 #define TC_MIN_BLOCKS 5
 #endif
