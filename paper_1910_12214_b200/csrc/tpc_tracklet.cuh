@@ -270,14 +270,12 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
     float ym = 0.0f, zm = 0.0f;
     float2 mk = make_float2(0.0f, 0.0f);         // coordinates of the known hit: consumed only at the Update
     int32_t hnext = -1;
-    GridDesc G;
-    if (act) {
-      if (c_cur >= 0) {
-        mk = __ldg(syz + c_cur);
-        if (phase == 0) hnext = __ldg(cup + c_cur);
-      } else {
-        G = desc[bsec + rn];
-      }
+    // the grid descriptor of the row is loaded by every lane (a conditional struct assignment would make the compiler
+    // wait for the load right here, to merge it with the "not loaded" value)
+    const GridDesc G = desc[act ? bsec + rn : 0];
+    if (act && c_cur >= 0) {
+      mk = __ldg(syz + c_cur);
+      if (phase == 0) hnext = __ldg(cup + c_cur);
     }
     SearchPre sp;
     const bool want_search = act && c_cur < 0;
