@@ -16,6 +16,21 @@ __device__ __forceinline__ unsigned long long selKey(int nhits, float chi2, uint
   return ((unsigned long long)(uint32_t)nhits << 56) | (inv << 24) | (unsigned long long)((~id) & 0xFFFFFFu);
 }
 
+// four consecutive row hits of a tracklet's slice starting at row rb (a multiple of 4): one 16-byte load when the slices
+// are 16-byte aligned (n_rows a multiple of 4), rows outside [f, r1] masked to -1
+__device__ __forceinline__ void rowHits4(const int32_t* __restrict__ row, int n_rows, int rb, int f, int r1, int32_t c4[4]) {
+  if ((n_rows & 3) == 0) {
+    const int4 v = *reinterpret_cast<const int4*>(row + rb);
+    c4[0] = v.x; c4[1] = v.y; c4[2] = v.z; c4[3] = v.w;
+  } else {
+#pragma unroll
+    for (int k = 0; k < 4; ++k) c4[k] = rb + k < n_rows ? row[rb + k] : -1;
+  }
+#pragma unroll
+  for (int k = 0; k < 4; ++k)
+    if (rb + k < f || rb + k > r1) c4[k] = -1;
+}
+
 __global__ void __launch_bounds__(128) selectClaim(TrackletStore tl, unsigned long long* __restrict__ owner_key,
                                                    int wide, const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
@@ -23,10 +38,14 @@ __global__ void __launch_bounds__(128) selectClaim(TrackletStore tl, unsigned lo
   const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= nT || tl.status[t] != 2) return;
   const unsigned long long key = selKey(tl.nhits[t], tl.chi2[t], (uint32_t)t, wide != 0);
-  const int r1 = tl.last_row[t];
-  for (int r = tl.first_row[t]; r <= r1; ++r) {
-    const int32_t c = tl.rowhit[t * tl.n_rows + r];
-    if (c >= 0) atomicMax(owner_key + c, key);
+  const int f = tl.first_row[t], r1 = tl.last_row[t];
+  const int32_t* row = tl.rowhit + t * tl.n_rows;
+  for (int rb = f & ~3; rb <= r1; rb += 4) {
+    int32_t c4[4];
+    rowHits4(row, tl.n_rows, rb, f, r1, c4);
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+      if (c4[k] >= 0) atomicMax(owner_key + c4[k], key);
   }
 }
 
@@ -74,12 +93,18 @@ __global__ void __launch_bounds__(128) selectCount(TrackletStore tl, const unsig
       int32_t* row = tl.rowhit + t * tl.n_rows;
       // the kept hits are compacted to the front of the tracklet's own row-hit slice (the write index never passes the
       // read index), so that selectEmit copies `kept` entries instead of walking the rows and the owner keys again
-      for (int r = f; r <= r1; ++r) {
-        const int32_t c = row[r];
-        if (c >= 0 && owns(c, key, (uint32_t)t, wide, owner_key, owner_id)) {
-          row[f + kept] = c;
-          ++kept; if (first < 0) first = r; last = r;
-        }
+      for (int rb = f & ~3; rb <= r1; rb += 4) {       // four rows at a time: their owner keys are gathered together
+        int32_t c4[4];
+        rowHits4(row, tl.n_rows, rb, f, r1, c4);
+        bool own[4];
+#pragma unroll
+        for (int k = 0; k < 4; ++k) own[k] = c4[k] >= 0 && owns(c4[k], key, (uint32_t)t, wide, owner_key, owner_id);
+#pragma unroll
+        for (int k = 0; k < 4; ++k)
+          if (own[k]) {
+            row[f + kept] = c4[k];
+            ++kept; if (first < 0) first = rb + k; last = rb + k;
+          }
       }
       if (kept >= min_track_hits) {
         sel = 1ull | ((unsigned long long)kept << 32);
