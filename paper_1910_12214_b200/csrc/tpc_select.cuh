@@ -93,16 +93,18 @@ __global__ void __launch_bounds__(128) selectCount(TrackletStore tl, const unsig
       int32_t* row = tl.rowhit + t * tl.n_rows;
       // the kept hits are compacted to the front of the tracklet's own row-hit slice (the write index never passes the
       // read index), so that selectEmit copies `kept` entries instead of walking the rows and the owner keys again
-      for (int rb = f & ~3; rb <= r1; rb += 4) {       // four rows at a time: their owner keys are gathered together
-        int32_t c4[4];
-        rowHits4(row, tl.n_rows, rb, f, r1, c4);
-        bool own[4];
+      for (int rb = f & ~3; rb <= r1; rb += 8) {       // eight rows at a time: their owner keys are gathered together
+        int32_t c8[8];
+        rowHits4(row, tl.n_rows, rb, f, r1, c8);
+        if (rb + 4 <= r1) rowHits4(row, tl.n_rows, rb + 4, f, r1, c8 + 4);
+        else { c8[4] = c8[5] = c8[6] = c8[7] = -1; }
+        bool own[8];
 #pragma unroll
-        for (int k = 0; k < 4; ++k) own[k] = c4[k] >= 0 && owns(c4[k], key, (uint32_t)t, wide, owner_key, owner_id);
+        for (int k = 0; k < 8; ++k) own[k] = c8[k] >= 0 && owns(c8[k], key, (uint32_t)t, wide, owner_key, owner_id);
 #pragma unroll
-        for (int k = 0; k < 4; ++k)
+        for (int k = 0; k < 8; ++k)
           if (own[k]) {
-            row[f + kept] = c4[k];
+            row[f + kept] = c8[k];
             ++kept; if (first < 0) first = rb + k; last = rb + k;
           }
       }
