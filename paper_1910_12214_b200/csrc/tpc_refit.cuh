@@ -86,7 +86,7 @@ __global__ void __launch_bounds__(128) refitTracks(const uint32_t* __restrict__ 
     for (int i = 1; i < n && ok; ++i) {           // up pass
       const uint32_t c = cn;
       const float ym = yn, zm = zn;
-      if (i + 1 < n) { cn = cl[i + 1]; yn = y[cn]; zn = z[cn]; }
+      cn = cl[min(i + 1, n - 1)]; yn = y[cn]; zn = z[cn];      // unconditional: a conditional load would be waited for here
       while (__ldg(off + b + 1) <= c) ++b;
       ok = kfPropagate(S, T.row_x[b - bsec], P, [](float, float, float, float) {}) && kfUpdate(S, ym, zm, P);
     }
@@ -98,7 +98,7 @@ __global__ void __launch_bounds__(128) refitTracks(const uint32_t* __restrict__ 
       for (int i = n - 1; i >= 0 && ok; --i) {
         const uint32_t c = cn;
         const float ym = yn, zm = zn;
-        if (i > 0) { cn = cl[i - 1]; yn = y[cn]; zn = z[cn]; }
+        cn = cl[max(i - 1, 0)]; yn = y[cn]; zn = z[cn];
         while (__ldg(off + b) > c) --b;
         ok = kfPropagate(S, T.row_x[b - bsec], P, [](float, float, float, float) {}) && kfUpdate(S, ym, zm, P);
       }
