@@ -79,3 +79,24 @@ def test_charge_code_parity(nb):
     got = res.trk["cl_qcode"].cpu().numpy().view(np.uint16)
     assert np.array_equal(got, orc.pack_charge(q, nb))
     trk.close()
+
+
+def test_charge_code_golden_fixture():
+    """tests/golden/charge_codes.txt (written from oracle/ only) through the CUDA path."""
+    import os
+    import torch
+    from paper_1910_12214_b200 import tpc
+    rows = [l.split() for l in open(os.path.join(os.path.dirname(__file__), "golden", "charge_codes.txt")) if l[0] != "#"]
+    a = np.array(rows, np.float64)
+    ev = datagen.make_event(0, scale=0.2)
+    n = ev.n_clusters
+    q = np.resize(a[:, 0].astype(np.float32), n)
+    for nb, col in ((4, 1), (3, 2)):
+        p = tpc.tpcDefaultParams()
+        p.charge_trunc_bits = nb
+        trk = tpc.TpcTracker.from_event(ev, params=p)
+        off, y, z = trk.upload(ev)
+        res = trk.run(off, y, z, q=torch.from_numpy(q).cuda())
+        got = res.trk["cl_qcode"].cpu().numpy().view(np.uint16)
+        assert np.array_equal(got, np.resize(a[:, col].astype(np.uint16), n))
+        trk.close()

@@ -48,3 +48,19 @@ def test_float_inputs_round_to_the_nearest_integer_first_and_bad_values_are_clam
     assert code[7] == 34 and code[8] == 100          # 33 = 100001b -> 6 bits, keep 5: 34 (tie up); 100 = 1100100b -> 100
     assert code[9] == 0 and code[10] == 0 and code[11] == 63488 and code[12] == 63488
     assert list(orc.pack_charge(np.array([33.0, 100.0, 1000.0], np.float32), 3)) == [32, 104, 1024]
+
+
+def _golden():
+    import os
+    rows = [l.split() for l in open(os.path.join(os.path.dirname(__file__), "golden", "charge_codes.txt")) if l[0] != "#"]
+    a = np.array(rows, np.float64)
+    return a[:, 0].astype(np.float32), a[:, 1].astype(np.uint16), a[:, 2].astype(np.uint16)
+
+
+def test_golden_charge_codes_and_a_few_values_worked_by_hand():
+    q, c4, c3 = _golden()
+    assert np.array_equal(orc.pack_charge(q, 4), c4) and np.array_equal(orc.pack_charge(q, 3), c3)
+    # worked by hand from the sentence of PAPER.md L70: 67 = 1000011b, n = 4 keeps 10000|11 -> rounds up to 1000100b = 68;
+    # 1000 = 1111101000b, n = 4 keeps 11111|01000 -> 1111100000b = 992;  n = 3 keeps 1111|101000 -> rounds up to 1024
+    d = {float(v): (int(a), int(b)) for v, a, b in zip(q, c4, c3)}
+    assert d[67.0] == (68, 64) and d[1000.0] == (992, 1024) and d[35.0] == (36, 36) and d[17.0] == (17, 18)
