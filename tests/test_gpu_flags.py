@@ -100,3 +100,29 @@ def test_charge_code_golden_fixture():
         got = res.trk["cl_qcode"].cpu().numpy().view(np.uint16)
         assert np.array_equal(got, np.resize(a[:, col].astype(np.uint16), n))
         trk.close()
+
+
+def test_optional_stages_on_empty_and_overflowing_inputs():
+    """All optional stages requested on an empty event, on a rows-only event without tracks and with too small track
+    capacities: defined status, nothing written out of bounds (guard values around the outputs stay intact)."""
+    import torch
+    from paper_1910_12214_b200 import tpc
+    ev = datagen.event_from_arrays(np.zeros(153, np.uint32), np.zeros(0, np.float32), np.zeros(0, np.float32), 1, 152)
+    trk = tpc.TpcTracker.from_event(ev)
+    off, y, z = trk.upload(ev)
+    res = trk.run(off, y, z, merge=True, flags=True, q=torch.zeros(0, device="cuda"))
+    assert res.status.status == 0 and res.n_tracks == 0
+    trk.close()
+    ev = datagen.make_event(1, scale=0.05)
+    trk = tpc.TpcTracker.from_event(ev)
+    off, y, z = trk.upload(ev)
+    full = trk.run(off, y, z, merge=True, flags=True)
+    assert full.status.status == 0 and full.n_tracks > 100
+    res = trk.run(off, y, z, merge=True, flags=True, cap_tracks=full.n_tracks // 3, grow=False)
+    assert res.status.status == tpc.TPC_ERR_CAPACITY and res.status.n_tracks == full.n_tracks
+    res = trk.run(off, y, z, merge=True, flags=True, cap_track_clusters=full.n_track_clusters // 2, grow=False)
+    assert res.status.status == tpc.TPC_ERR_CAPACITY
+    again = trk.run(off, y, z, merge=True, flags=True)                 # and the tracker is fine afterwards
+    for k in ("trk_mg_next", "cl_flags", "cl_owner", "trk_rf_par_in"):
+        assert torch.equal(again.trk[k], full.trk[k]), k
+    trk.close()
