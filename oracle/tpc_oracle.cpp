@@ -202,6 +202,7 @@ struct orcResult {
   // O8 cluster flags (NEXT-3)
   std::vector<uint8_t> cf_flags;
   std::vector<int32_t> cf_owner;
+  std::vector<double> cf_res_y, cf_res_z;
 };
 
 namespace {
@@ -488,6 +489,7 @@ struct Tracker {
   void flagAll() {
     const int64_t nt = (int64_t)res.tr_id.size();
     res.cf_flags.assign(N, 0); res.cf_owner.assign(N, -1);
+    res.cf_res_y.assign(N, 0); res.cf_res_z.assign(N, 0);
     const Real bf = (Real)(0.00299792458 * (double)g.bz_tesla);
     const Real msp = (Real)P.max_sinphi, tube2 = (Real)P.tube_radius * (Real)P.tube_radius;
     const Real sin70 = (Real)0.9396926207859084, qmax = (Real)P.inv_pt_protect;
@@ -511,6 +513,7 @@ struct Tracker {
         const bool bad = low || !(std::fabs(st.s) < sin70);
         while (ic < ncl && rowOf[cl[ic]] < r) ++ic;
         const int32_t own = (ic < ncl && rowOf[cl[ic]] == r) ? (int32_t)cl[ic] : -1;     // the attached cluster of this row
+        if (own >= 0) { res.cf_res_y[own] = (double)(Y[own] - st.y); res.cf_res_z[own] = (double)(Z[own] - st.z); }   // R39
         for (uint32_t c = off[sec * R + r]; c < off[sec * R + r + 1]; ++c) {
           const Real dy = Y[c] - st.y, dz = Z[c] - st.z;
           const Real d2 = dy * dy + dz * dz;
@@ -725,6 +728,7 @@ void orcGetRefit(const orcResult* r, int32_t* status, double* x_in, double* par_
 }
 
 void orcGetClusterFlags(const orcResult* r, uint8_t* flags, int32_t* owner) { copyOut(flags, r->cf_flags); copyOut(owner, r->cf_owner); }
+void orcGetResiduals(const orcResult* r, double* ry, double* rz) { copyOut(ry, r->cf_res_y); copyOut(rz, r->cf_res_z); }
 void orcGetMerge(const orcResult* r, int32_t* next, int32_t* prev, int32_t* head, double* chi2) {
   copyOut(next, r->mg_next); copyOut(prev, r->mg_prev); copyOut(head, r->mg_head); copyOut(chi2, r->mg_chi2);
 }

@@ -100,6 +100,9 @@ void orcGetMerge(const orcResult*, int32_t* next, int32_t* prev, int32_t* head, 
  * flags [n_clusters] bit mask 1 attached, 2 adjacent, 4 protected, 8 removed by strategy A, 16 removed by strategy B;
  * owner [n_clusters] track index of the highest-momentum track with the cluster in its tube, -1 none. */
 void orcGetClusterFlags(const orcResult*, uint8_t* flags, int32_t* owner);
+/* track-model residuals (O8, R39) of the clusters attached to refitted tracks, 0 elsewhere;
+ * only with ORC_FLAGS.  res_y, res_z [n_clusters]. */
+void orcGetResiduals(const orcResult*, double* res_y, double* res_z);
 
 /* O9 (part of NEXT-4, DESIGN.md section 3 "O9"): dynamic-precision code of n_values charges: the integer
  * nearest to q, with every bit more than trunc_bits after its first non-zero bit rounded away.  Returns 0 on bad arguments. */

@@ -75,6 +75,8 @@ def _load():
             getattr(L, f).restype = None
         L.orcPackCharge.argtypes = [i64, vp, ci, vp]
         L.orcPackCharge.restype = ci
+        L.orcGetResiduals.argtypes = [vp] * 3
+        L.orcGetResiduals.restype = None
         L.orcGetClusterFlags.argtypes = [vp] * 3
         L.orcGetClusterFlags.restype = None
         L.orcGetMerge.argtypes = [vp] * 5
@@ -149,6 +151,8 @@ class OracleResult:
     # O8 cluster flags (only with flags=True): bit mask per cluster and the owning track
     cf_flags: np.ndarray | None = None
     cf_owner: np.ndarray | None = None
+    cf_res_y: np.ndarray | None = None      # track-model residuals of the clusters attached to refitted tracks
+    cf_res_z: np.ndarray | None = None
 
     @property
     def n_tracks(self) -> int:
@@ -219,7 +223,9 @@ def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool 
         if flags:
             cf, co = np.zeros(n, np.uint8), np.full(n, -1, np.int32)
             L.orcGetClusterFlags(h, _ptr(cf), _ptr(co))
-            rf.update(cf_flags=cf, cf_owner=co)
+            ry, rz = np.zeros(n), np.zeros(n)
+            L.orcGetResiduals(h, _ptr(ry), _ptr(rz))
+            rf.update(cf_flags=cf, cf_owner=co, cf_res_y=ry, cf_res_z=rz)
     finally:
         L.orcFree(h)
     return OracleResult(n, s2o, cell, ncell, ur, dr, u, d, sh, st, nh, fr, lr, rh, tx, tpar, tcov, tchi, kid, ks, kf, kl,

@@ -55,6 +55,9 @@ def test_tube_radius_on_a_hand_built_track():
     assert f[e[0]] == ADJ | PROT and f[e[2]] == ADJ | PROT           # 1.4 cm and sqrt(2) cm: inside the tube
     assert f[e[1]] == RMB and f[e[3]] == RMB                          # 1.6 cm and 1.1 * sqrt(2) cm: outside
     assert np.all(res.cf_owner[where[:len(rows)]] == 0) and res.cf_owner[e[0]] == 0 and res.cf_owner[e[1]] == -1
+    # track-model residuals (R39): exact helix points leave none (fp32 rounding only), unattached clusters carry 0
+    assert np.all(np.abs(res.cf_res_y[where[:len(rows)]]) < 2e-4) and np.all(np.abs(res.cf_res_z[where[:len(rows)]]) < 2e-4)
+    assert np.all(res.cf_res_y[e] == 0) and np.all(res.cf_res_z[e] == 0)
 
 
 def test_ambiguity_goes_to_the_higher_momentum_track_and_low_momentum_tracks_do_not_protect():
@@ -90,6 +93,7 @@ def _flags_numpy(ev, res, p):
     owner = np.full(n, -1, np.int64)
     oq = np.zeros(n, np.float32)
     bad = np.zeros(n, bool)
+    res_y, res_z = np.zeros(n), np.zeros(n)
     sin70 = np.float32(0.9396926207859084)
     tube2 = np.float32(p.tube_radius) * np.float32(p.tube_radius)
     y32, z32 = ev.y.astype(np.float32), ev.z.astype(np.float32)
@@ -116,6 +120,9 @@ def _flags_numpy(ev, res, p):
             inside = (dy * dy + dz * dz) <= tube2
             own = cl[rowof[cl] == r]
             inside[own - lo] = True
+            for c in own:
+                res_y[c] = float(y32[c] - np.float32(st[1]))
+                res_z[c] = float(z32[c] - np.float32(st[2]))
             b = low or not (np.float32(abs(st[3])) < sin70)
             for c in np.nonzero(inside)[0] + lo:
                 if owner[c] < 0 or aq < oq[c]:
@@ -128,7 +135,7 @@ def _flags_numpy(ev, res, p):
     f[prot] |= PROT
     f[has & ~prot] |= RMA
     f[~prot] |= RMB
-    return f, owner
+    return f, owner, res_y, res_z
 
 
 @pytest.mark.parametrize("idx,scale,dead", [(2, 0.03, ()), (1, 0.02, (40, 97))])
@@ -136,9 +143,10 @@ def test_flags_equal_the_numpy_restatement(idx, scale, dead):
     ev = datagen.make_event(idx, scale=scale, dead_rows=dead)
     p = orc.default_params()
     res = orc.run(ev, p, flags=True)
-    f, owner = _flags_numpy(ev, res, p)
+    f, owner, ry, rz = _flags_numpy(ev, res, p)
     assert np.array_equal(owner, res.cf_owner)
     assert np.array_equal(f, res.cf_flags)
+    assert np.array_equal(ry, res.cf_res_y) and np.array_equal(rz, res.cf_res_z)
     if idx == 2:
         assert ((res.cf_flags & RMA) != 0).sum() > 10            # steep looper segments are exercised
 
@@ -158,3 +166,22 @@ def test_flag_invariants_and_what_the_strategies_remove():
     assert rmb[noise & ~adj].all() and not rma[~adj].any()
     # most noise is far from any track and most track clusters are protected
     assert prot[~noise].mean() > 0.7 and rmb[noise].mean() > 0.6
+
+
+def test_residuals_have_the_least_squares_variance():
+    """Closed form: residuals of a least-squares fit with p free parameters over n points of variance sigma^2 have the
+    variance sigma^2 (1 - p / n); the helix has 3 parameters in the bend plane (y) and 2 in z.  Config 0: sigma = 0.1 cm."""
+    ev = datagen.make_event(0)
+    res = orc.run(ev, flags=True)
+    long_tracks = np.nonzero((res.rf_status == 1) & (res.trk_ncl >= 40))[0]
+    ry, rz, ey, ez = [], [], [], []
+    for k in long_tracks:
+        idx = res.trk_cl_index[res.trk_cl_offset[k]:res.trk_cl_offset[k + 1]]
+        n = len(idx)
+        ry.append(res.cf_res_y[idx]); rz.append(res.cf_res_z[idx])
+        ey.append(np.full(n, 0.01 * (1 - 3.0 / n))); ez.append(np.full(n, 0.01 * (1 - 2.0 / n)))
+    ry, rz, ey, ez = (np.concatenate(a) for a in (ry, rz, ey, ez))
+    assert len(ry) > 8000
+    assert np.mean(ry ** 2) == pytest.approx(np.mean(ey), rel=0.05)
+    assert np.mean(rz ** 2) == pytest.approx(np.mean(ez), rel=0.05)
+    assert abs(np.mean(ry)) < 0.005 and abs(np.mean(rz)) < 0.005
