@@ -142,6 +142,8 @@ typedef struct {
    * with the refit outputs.  Indexed by the INPUT cluster index. */
   uint8_t* cl_flags;            /* [n_clusters] 1 attached, 2 adjacent, 4 protected, 8 removed by strategy A, 16 by strategy B */
   int32_t* cl_owner;            /* [n_clusters] track with the cluster in its tube (highest momentum), -1 none */
+  float* cl_res_y;              /* [n_clusters] optional with the two above (both or none): track-model residuals */
+  float* cl_res_z;              /*   y_c - y_track, z_c - z_track of the clusters attached to refitted tracks, 0 elsewhere */
   /* optional O9 dynamic-precision charge code (DESIGN.md section 3 "O9"); needs tpcClusters.q */
   uint16_t* cl_qcode;           /* [n_clusters] integer charge with all bits beyond charge_trunc_bits after the first
                                    non-zero bit rounded away; NULL = not computed */

@@ -331,6 +331,7 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   if (out->cl_qcode && N > 0 && !in->q) return TPC_ERR_INVALID_ARG;                      // the charge code needs the charges
   const int n_fl = (out->cl_flags != nullptr) + (out->cl_owner != nullptr);
   if ((n_fl != 0 && n_fl != 2) || (n_fl == 2 && n_rf != 8)) return TPC_ERR_INVALID_ARG;   // so do the cluster flags
+  if ((out->cl_res_y != nullptr) != (out->cl_res_z != nullptr) || (out->cl_res_y && n_fl != 2)) return TPC_ERR_INVALID_ARG;
   if (!workspace || ((uintptr_t)workspace % ALIGN) != 0) return TPC_ERR_INVALID_ARG;
   const Workspace w = layout(h, N, capT, (char*)workspace);
   if (workspace_bytes < w.bytes) return TPC_ERR_WORKSPACE_TOO_SMALL;
@@ -473,6 +474,10 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   if (n_fl == 2 && N > 0) {
     TPC_CUDA(h, cudaMemsetAsync(w.fl_key, 0xFF, 8 * (size_t)N, st)); ++L;
     TPC_CUDA(h, cudaMemsetAsync(out->cl_flags, 0, (size_t)N, st)); ++L;
+    if (out->cl_res_y) {
+      TPC_CUDA(h, cudaMemsetAsync(out->cl_res_y, 0, 4 * (size_t)N, st)); ++L;
+      TPC_CUDA(h, cudaMemsetAsync(out->cl_res_z, 0, 4 * (size_t)N, st)); ++L;
+    }
     if (out->cap_tracks > 0 && out->cap_track_clusters > 0) {
       const FlagIn fi{out->cap_tracks, out->trk_rf_status, out->trk_sector, out->trk_first_row, out->trk_last_row,
                       out->trk_rf_x_in, out->trk_rf_par_in, out->trk_rf_cov_in, out->trk_cl_offset, out->trk_cl_index};
@@ -481,7 +486,7 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
                                                                                                        out->cl_flags, cnt); ++L;
       flagBid<<<(unsigned)ceilDiv(nk * FLAG_GROUP, 128), 128, 0, st>>>(fi, in->row_offset, P, T, h->params.tube_radius,
                                                           h->params.inv_pt_protect, w.desc, w.cell_start, w.syz, w.s2o,
-                                                          w.fl_key, cnt); ++L;
+                                                          w.fl_key, in->y, in->z, out->cl_res_y, out->cl_res_z, cnt); ++L;
     }
     flagFinish<<<gN256, 256, 0, st>>>(N, w.fl_key, out->cl_flags, out->cl_owner, cnt); ++L;
   }
@@ -577,7 +582,7 @@ extern "C" int tpcRunHost(tpcHandle* h, int64_t N, const uint32_t* row_offset, c
       oh->tl_first_row || oh->tl_last_row || oh->tl_rowhit || oh->tl_x || oh->tl_par || oh->tl_cov || oh->tl_chi2 ||
       oh->trk_rf_status || oh->trk_rf_x_in || oh->trk_rf_par_in || oh->trk_rf_cov_in || oh->trk_rf_chi2 || oh->trk_rf_x_out ||
       oh->trk_rf_par_out || oh->trk_rf_cov_out || oh->trk_mg_next || oh->trk_mg_prev || oh->trk_mg_head || oh->trk_mg_chi2 ||
-      oh->cl_flags || oh->cl_owner || oh->cl_qcode)
+      oh->cl_flags || oh->cl_owner || oh->cl_qcode || oh->cl_res_y || oh->cl_res_z)
     return TPC_ERR_INVALID_ARG;
   if (!oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0) return TPC_ERR_INVALID_ARG;
   TPC_CUDA(h, cudaSetDevice(h->device));
@@ -687,7 +692,7 @@ extern "C" int tpcSubmitHost(tpcHandle* h, int slot, int64_t N, const uint32_t* 
     return TPC_ERR_INVALID_ARG;
   if (oh->link_up_raw || oh->link_dn_raw || oh->link_up || oh->link_dn || oh->start_hits || oh->tl_status || oh->tl_nhits ||
       oh->tl_first_row || oh->tl_last_row || oh->tl_rowhit || oh->tl_x || oh->tl_par || oh->tl_cov || oh->tl_chi2 ||
-      oh->trk_rf_status || oh->trk_mg_next || oh->cl_flags || oh->cl_owner || oh->cl_qcode || !oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0)
+      oh->trk_rf_status || oh->trk_mg_next || oh->cl_flags || oh->cl_owner || oh->cl_qcode || oh->cl_res_y || oh->cl_res_z || !oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0)
     return TPC_ERR_INVALID_ARG;
   TPC_CUDA(h, cudaSetDevice(h->device));
   int rc;

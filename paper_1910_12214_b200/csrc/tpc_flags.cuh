@@ -37,6 +37,8 @@ __global__ void __launch_bounds__(128) flagBid(FlagIn in, const uint32_t* __rest
                                                float tube, float inv_pt_protect, const GridDesc* __restrict__ desc,
                                                const uint32_t* __restrict__ cell_start, const float2* __restrict__ syz,
                                                const uint32_t* __restrict__ s2o, unsigned long long* __restrict__ key,
+                                               const float* __restrict__ yin, const float* __restrict__ zin,
+                                               float* __restrict__ res_y, float* __restrict__ res_z,
                                                const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
   const int64_t k = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / FLAG_GROUP;
@@ -69,7 +71,11 @@ __global__ void __launch_bounds__(128) flagBid(FlagIn in, const uint32_t* __rest
     // the attached cluster of this row (R35): the list is in ascending row, rows follow from row_offset (R26)
     const uint32_t b_lo = __ldg(off + bsec + r), b_hi = __ldg(off + bsec + r + 1);
     while (ic < ncl && cl[ic] < b_lo) ++ic;
-    if (sub == 0 && ic < ncl && cl[ic] < b_hi) atomicMin(key + cl[ic], bid);
+    if (sub == 0 && ic < ncl && cl[ic] < b_hi) {
+      const uint32_t own = cl[ic];
+      atomicMin(key + own, bid);
+      if (res_y) { res_y[own] = yin[own] - S.y; res_z[own] = zin[own] - S.z; }     // track-model residuals (R39)
+    }
     // the tube: cells of the box around it (a hair wider than the tube: fl(dy*dy) <= fl(tube*tube) does not quite imply
     // |dy| <= tube), exact circle predicate; the lanes of the group take the candidates of a cell row in turn
     const GridDesc G = desc[bsec + r];

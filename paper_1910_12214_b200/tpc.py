@@ -52,7 +52,7 @@ _STAGE_PTRS = ("link_up_raw", "link_dn_raw", "link_up", "link_dn", "start_hits",
 _REFIT_PTRS = ("trk_rf_status", "trk_rf_x_in", "trk_rf_par_in", "trk_rf_cov_in", "trk_rf_chi2", "trk_rf_x_out",
                "trk_rf_par_out", "trk_rf_cov_out")
 _MERGE_PTRS = ("trk_mg_next", "trk_mg_prev", "trk_mg_head", "trk_mg_chi2")
-_FLAG_PTRS = ("cl_flags", "cl_owner")
+_FLAG_PTRS = ("cl_flags", "cl_owner", "cl_res_y", "cl_res_z")
 _PACK_PTRS = ("cl_qcode",)
 
 
@@ -260,7 +260,8 @@ class TpcTracker:
         if pack:
             spec.update({"cl_qcode": ((max(n, 1),), t.int16)})
         if flags:
-            spec.update({"cl_flags": ((max(n, 1),), t.uint8), "cl_owner": ((max(n, 1),), i32)})
+            spec.update({"cl_flags": ((max(n, 1),), t.uint8), "cl_owner": ((max(n, 1),), i32),
+                         "cl_res_y": ((max(n, 1),), f32), "cl_res_z": ((max(n, 1),), f32)})
         if merge:
             spec.update({"trk_mg_next": ((capK,), i32), "trk_mg_prev": ((capK,), i32), "trk_mg_head": ((capK,), i32),
                          "trk_mg_chi2": ((capK,), f32)})

@@ -26,6 +26,8 @@ def _both(ev, **par):
     assert np.array_equal(g["trk_cl_index"].view(np.uint32), o.trk_cl_index)
     assert np.array_equal(g["cl_owner"], o.cf_owner)
     assert np.array_equal(g["cl_flags"], o.cf_flags)
+    assert np.array_equal(g["cl_res_y"], o.cf_res_y.astype(np.float32))      # track-model residuals (R39), bit-exact
+    assert np.array_equal(g["cl_res_z"], o.cf_res_z.astype(np.float32))
     assert np.array_equal(g["trk_mg_next"], o.mg_next)          # the three optional stages coexist
     return g, o, res
 
