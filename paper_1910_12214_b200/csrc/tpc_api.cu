@@ -328,6 +328,7 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   const int n_mg = (out->trk_mg_next != nullptr) + (out->trk_mg_prev != nullptr) + (out->trk_mg_head != nullptr) +
                    (out->trk_mg_chi2 != nullptr);
   if ((n_mg != 0 && n_mg != 4) || (n_mg == 4 && n_rf != 8)) return TPC_ERR_INVALID_ARG;   // the merger needs the refit
+  if (n_mg == 4 && (int64_t)h->P.n_buckets * MG_NYB * MG_NZB >= (1ll << 31)) return TPC_ERR_INVALID_ARG;   // bucket ids are 32-bit
   if (out->cl_qcode && N > 0 && !in->q) return TPC_ERR_INVALID_ARG;                      // the charge code needs the charges
   const int n_fl = (out->cl_flags != nullptr) + (out->cl_owner != nullptr);
   if ((n_fl != 0 && n_fl != 2) || (n_fl == 2 && n_rf != 8)) return TPC_ERR_INVALID_ARG;   // so do the cluster flags
