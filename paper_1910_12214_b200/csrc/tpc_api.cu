@@ -163,7 +163,7 @@ Workspace layout(const tpcHandle* h, int64_t N, int64_t capT, char* base) {
   w.kept_last = (int32_t*)take(4 * (size_t)Tn);
   w.owner_key = (unsigned long long*)take(8 * (size_t)Nn);
   w.owner_id = (uint32_t*)take(4 * (size_t)Nn);
-  const size_t mgb = (size_t)nb * MG_NYB * MG_NZB + 1;
+  const size_t mgb = (int64_t)nb * MG_NYB * MG_NZB < (1ll << 31) ? (size_t)nb * MG_NYB * MG_NZB + 1 : 1;   // else: merger refused
   w.mg_start = (uint32_t*)take(4 * mgb);
   w.mg_fill = (uint32_t*)take(4 * mgb);
   w.mg_maxv = (uint32_t*)take(8 * (size_t)nb);
