@@ -49,6 +49,11 @@ struct RowTables {
   const uint8_t* dead;    // [R]
 };
 
+__device__ __forceinline__ void nfCpAsync8(void* smem, const void* gmem) {
+  const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(gmem) : "memory");
+}
+
 // lexicographic (Dev, orig(u), orig(d)) "is the new pair better" (R6)
 __device__ __forceinline__ bool pairBetter(bool have, float dev, float best, uint32_t u, uint32_t d, uint32_t bu,
                                            uint32_t bd, const uint32_t* __restrict__ s2o) {
@@ -207,8 +212,10 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
     if (valid) neighbourSlow(p, h, Gu, Gd, cell_start, syz, s2o, iu, id, wyu, wzu, wyd, wzd, P.link_dev2_max, lup, ldn);
     return;
   }
-  for (uint32_t i = tid; i < kD1 - kD0; i += NF_THREADS) sD[i] = __ldg(syz + kD0 + i);
-  for (uint32_t i = tid; i < kU1 - kU0; i += NF_THREADS) sU[i] = __ldg(syz + kU0 + i);
+  // both regions by asynchronous 8-byte copies: every load of the thread is in flight before the first one is waited for
+  for (uint32_t i = tid; i < kD1 - kD0; i += NF_THREADS) nfCpAsync8(sD + i, syz + kD0 + i);
+  for (uint32_t i = tid; i < kU1 - kU0; i += NF_THREADS) nfCpAsync8(sU + i, syz + kU0 + i);
+  asm volatile("cp.async.wait_all;\n" ::: "memory");
   sH[tid] = h;
   __syncthreads();
 
