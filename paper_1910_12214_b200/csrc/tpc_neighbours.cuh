@@ -111,19 +111,15 @@ __device__ __forceinline__ int gatherWindow(const GridDesc& G, const uint32_t* _
   }
 #pragma unroll
   for (int r = 0; r < NF_ROWS; ++r) rows[r * NF_THREADS + tid] = make_ushort2((uint16_t)(ra[r] - k0), (uint16_t)(rb[r] - k0));
-  uint32_t k = ra[0] - k0, kend = rb[0] - k0;
-  int n = 0, r = 0;
-  for (;;) {
-    if (k < kend) {
+  int n = 0;
+  for (int r = 0; r < nr; ++r) {
+    const ushort2 v = rows[r * NF_THREADS + tid];
+#pragma unroll 4
+    for (uint32_t k = v.x; k < v.y; ++k) {
       const float2 c = reg[k];
       const bool pass = fabsf(c.x - yc) <= wy && fabsf(c.y - zc) <= wz;
       list[min(n, NF_LIST) * NF_THREADS + tid] = (uint16_t)k;     // row NF_LIST is a spare: no branch needed
       n += pass ? 1 : 0;
-      ++k;
-    } else {
-      if (++r >= nr) break;
-      const ushort2 v = rows[r * NF_THREADS + tid];
-      k = v.x; kend = v.y;
     }
   }
   return n;
