@@ -40,6 +40,10 @@ constexpr int NF_LIST = NF_LIST_;  // window candidates kept per thread and side
 #endif
 constexpr int NF_UB = NF_UB_;          // u's per item (register blocking of the pair loop)
 constexpr int NF_ITEMS = NF_ITEMS_; // items per CTA and round
+#ifndef NF_GUNROLL_
+#define NF_GUNROLL_ 2
+#endif
+constexpr int NF_GUNROLL = NF_GUNROLL_;
 constexpr int NF_ROWS = 6;         // cell rows of a window whose ranges are staged (more: slow path)
 
 struct RowTables {
@@ -114,7 +118,7 @@ __device__ __forceinline__ int gatherWindow(const GridDesc& G, const uint32_t* _
   int n = 0;
   for (int r = 0; r < nr; ++r) {
     const ushort2 v = rows[r * NF_THREADS + tid];
-#pragma unroll 4
+#pragma unroll NF_GUNROLL
     for (uint32_t k = v.x; k < v.y; ++k) {
       const float2 c = reg[k];
       const bool pass = fabsf(c.x - yc) <= wy && fabsf(c.y - zc) <= wz;
