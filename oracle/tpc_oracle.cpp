@@ -161,6 +161,47 @@ bool match(State<Real> a, int rel, const State<Real>& b, Real bfield, const orcP
   return true;
 }
 
+// ---- O10 Mirror: the same helix seen from the frame turned by 180 degrees about z and walked backwards ------------
+// (x, y) -> (-x, -y); the direction turns with the frame and is reversed, so sin(phi) and cos(phi) > 0 stay; z stays;
+// dz/dl and the apparent charge change sign.  C <- J C J^T with J = diag(-1, +1, +1, -1, -1) over (y, z, s, t, q).
+template <typename Real>
+void mirror(State<Real>& st) {
+  st.x = -st.x; st.y = -st.y; st.t = -st.t; st.q = -st.q;
+  const int sg[5] = {-1, 1, 1, -1, -1};
+  for (int i = 0; i < 5; ++i)
+    for (int j = 0; j < i; ++j)
+      if (sg[i] * sg[j] < 0) st.C[tri(i, j)] = -st.C[tri(i, j)];
+}
+
+// ---- O10 LegMatch(a, b): outer states of two leg ends, b's sector d sectors after a's (d * sg >= 0) ---------------
+// a is turned by alpha = d*10 + sg*90 degrees (sg = sign of a's sin phi): the frame halfway between the two sectors,
+// with its x axis across the sectors in the direction a moves -- the symmetry axis of the turn, about which the two
+// sides mirror each other; b is turned by -alpha and mirrored into the same frame; then as Match.
+template <typename Real>
+bool legMatch(State<Real> a, int d, State<Real> b, Real bfield, const orcParams& P, Real& chi2) {
+  const double a10 = 0.17453292519943295, a90 = 1.5707963267948966;
+  const double sg = a.s > (Real)0 ? 1.0 : -1.0;
+  const double alpha = (double)d * a10 + sg * a90;
+  if (!rotate(a, alpha, bfield, (Real)P.max_sinphi)) return false;
+  if (!rotate(b, -alpha, bfield, (Real)P.max_sinphi)) return false;
+  mirror(b);
+  // R43: the arc of a turn is long (Propagate's arc-length series is made for row-to-row steps): eight equal steps
+  const Real x0 = a.x, step = (b.x - a.x) * (Real)0.125;
+  for (int i = 1; i <= 8; ++i)
+    if (!propagate(a, i < 8 ? x0 + (Real)i * step : b.x, bfield, (Real)P.max_sinphi)) return false;
+  const Real pa[5] = {a.y, a.z, a.s, a.t, a.q}, pb[5] = {b.y, b.z, b.s, b.t, b.q};
+  Real sum = 0;
+  for (int i = 0; i < 5; ++i) {
+    const Real den = a.C[tri(i, i)] + b.C[tri(i, i)];
+    if (!(den > (Real)0)) return false;
+    const Real dd = pa[i] - pb[i];
+    sum = sum + (dd * dd) / den;
+  }
+  if (!(sum <= (Real)P.leg_chi2_max)) return false;
+  chi2 = sum;
+  return true;
+}
+
 template <typename Real>
 struct Tracklet {
   int status = 0;   // 0 discarded in chain fit, 1 rejected, 2 accepted
@@ -199,6 +240,9 @@ struct orcResult {
   // O7 merger (NEXT-1)
   std::vector<int32_t> mg_next, mg_prev, mg_head;
   std::vector<double> mg_chi2;
+  // O10 looper legs (rest of NEXT-1)
+  std::vector<int32_t> lg_partner;
+  std::vector<double> lg_chi2;
   // O8 cluster flags (NEXT-3)
   std::vector<uint8_t> cf_flags;
   std::vector<int32_t> cf_owner;
@@ -485,6 +529,53 @@ struct Tracker {
     }
   }
 
+  // ---- O10 looper legs: the two sides of an outer turn (O10; readings R40..R43) ------------
+  void legAll() {
+    const int64_t nt = (int64_t)res.tr_id.size();
+    res.lg_partner.assign(nt, -1); res.lg_chi2.assign(nt, 0);
+    const Real bf = (Real)(0.00299792458 * (double)g.bz_tesla);
+    auto outer = [&](int64_t k) {
+      State<Real> st{};
+      st.x = (Real)res.rf_x_out[k]; st.y = (Real)res.rf_par_out[k * 5]; st.z = (Real)res.rf_par_out[k * 5 + 1];
+      st.s = (Real)res.rf_par_out[k * 5 + 2]; st.t = (Real)res.rf_par_out[k * 5 + 3]; st.q = (Real)res.rf_par_out[k * 5 + 4];
+      for (int i = 0; i < 15; ++i) st.C[i] = (Real)res.rf_cov_out[k * 15 + i];
+      return st;
+    };
+    auto isEnd = [&](int64_t k) {                // R40: a refitted track that ends steep
+      return res.rf_status[k] && !(std::fabs((Real)res.rf_par_out[k * 5 + 2]) < (Real)P.leg_min_sinphi);
+    };
+    auto dist = [&](int sa, int sb, int& d) {    // signed azimuthal distance a -> b on the same side
+      if (sa == sb) { d = 0; return true; }
+      if (S != 36 || sa / 18 != sb / 18) return false;
+      d = (sb % 18 - sa % 18 + 18) % 18;
+      if (d > 9) d -= 18;
+      return true;
+    };
+    std::vector<int32_t> best(nt, -1);
+    std::vector<Real> chi(nt, 0);
+    for (int64_t a = 0; a < nt; ++a) {
+      if (!isEnd(a)) continue;
+      const State<Real> sa = outer(a);
+      for (int64_t b = a + 1; b < nt; ++b) {     // R41: every pair once, the lower id is the one propagated
+        if (!isEnd(b)) continue;
+        int d;
+        if (!dist(res.tr_sector[a], res.tr_sector[b], d) || std::abs(d) > P.leg_max_sectors) continue;
+        if (std::abs(res.tr_last[a] - res.tr_last[b]) > P.leg_max_row_diff) continue;
+        const State<Real> sb = outer(b);
+        if (!(sa.s * sb.s < (Real)0)) continue;                  // opposite inclinations
+        if ((sa.s > (Real)0 && d < 0) || (sa.s < (Real)0 && d > 0)) continue;   // a moves towards b's sector
+        Real c2;
+        if (!legMatch(sa, d, sb, bf, P, c2)) continue;
+        if (best[a] < 0 || c2 < chi[a]) { best[a] = (int32_t)b; chi[a] = c2; }   // ties: lowest partner id (loop order:
+        if (best[b] < 0 || c2 < chi[b]) { best[b] = (int32_t)a; chi[b] = c2; }   // b's partners a come in ascending a too)
+      }
+    }
+    for (int64_t k = 0; k < nt; ++k) {            // R42: kept when reciprocal
+      const int32_t o = best[k];
+      if (o >= 0 && best[o] == (int32_t)k) { res.lg_partner[k] = o; res.lg_chi2[k] = (double)chi[k]; }
+    }
+  }
+
   // ---- O8 cluster flags (O8; readings R34..R37) ---------------------------
   void flagAll() {
     const int64_t nt = (int64_t)res.tr_id.size();
@@ -684,6 +775,7 @@ void orcDefaultParams(orcParams* p) {
   p->cell_min = 0.5f; p->cell_max = 8.0f;
   p->merge_max_row_gap = 40; p->merge_back_rows = 5; p->merge_chi2_max = 50.0f;
   p->tube_radius = 1.5f; p->inv_pt_protect = 20.0f;
+  p->leg_min_sinphi = 0.5f; p->leg_chi2_max = 50.0f; p->leg_max_sectors = 4; p->leg_max_row_diff = 12;
 }
 
 int orcRun(const orcGeometry* g, const orcParams* p, int64_t n, const uint32_t* off, const float* y, const float* z,
@@ -701,9 +793,10 @@ int orcRun(const orcGeometry* g, const orcParams* p, int64_t n, const uint32_t* 
   r->fp64 = (flags & ORC_FP64) != 0; r->brute = (flags & ORC_BRUTE_FORCE) != 0;
   const bool mg = (flags & ORC_MERGE) != 0;
   const bool fg = (flags & ORC_FLAGS) != 0;
-  const bool rf = mg || fg || (flags & ORC_REFIT) != 0;
-  if (r->fp64) { Tracker<double> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); if (rf) T.refitAll(); if (mg) T.mergeAll(); if (fg) T.flagAll(); }
-  else { Tracker<float> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); if (rf) T.refitAll(); if (mg) T.mergeAll(); if (fg) T.flagAll(); }
+  const bool lg = (flags & ORC_LEGS) != 0;
+  const bool rf = mg || fg || lg || (flags & ORC_REFIT) != 0;
+  if (r->fp64) { Tracker<double> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); if (rf) T.refitAll(); if (mg) T.mergeAll(); if (lg) T.legAll(); if (fg) T.flagAll(); }
+  else { Tracker<float> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); if (rf) T.refitAll(); if (mg) T.mergeAll(); if (lg) T.legAll(); if (fg) T.flagAll(); }
   *out = r;
   return ORC_OK;
 }
@@ -729,6 +822,7 @@ void orcGetRefit(const orcResult* r, int32_t* status, double* x_in, double* par_
 
 void orcGetClusterFlags(const orcResult* r, uint8_t* flags, int32_t* owner) { copyOut(flags, r->cf_flags); copyOut(owner, r->cf_owner); }
 void orcGetResiduals(const orcResult* r, double* ry, double* rz) { copyOut(ry, r->cf_res_y); copyOut(rz, r->cf_res_z); }
+void orcGetLegs(const orcResult* r, int32_t* partner, double* chi2) { copyOut(partner, r->lg_partner); copyOut(chi2, r->lg_chi2); }
 void orcGetMerge(const orcResult* r, int32_t* next, int32_t* prev, int32_t* head, double* chi2) {
   copyOut(next, r->mg_next); copyOut(prev, r->mg_prev); copyOut(head, r->mg_head); copyOut(chi2, r->mg_chi2);
 }
@@ -759,6 +853,23 @@ int matchT(const orcParams* p, double bz, const double* as, const double* ac, in
   *chi2 = (double)c2;
   return 1;
 }
+template <typename Real>
+void mirrorT(double* st, double* cov) {
+  State<Real> s = stateFrom<Real>(st, cov);
+  mirror(s);
+  st[0] = (double)s.x; st[1] = (double)s.y; st[2] = (double)s.z; st[3] = (double)s.s; st[4] = (double)s.t; st[5] = (double)s.q;
+  for (int i = 0; i < 15; ++i) cov[i] = (double)s.C[i];
+}
+
+template <typename Real>
+int legMatchT(const orcParams* p, double bz, const double* as, const double* ac, int d, const double* bs, const double* bc,
+              double* chi2) {
+  Real c2;
+  if (!legMatch(stateFrom<Real>(as, ac), d, stateFrom<Real>(bs, bc), (Real)(0.00299792458 * bz), *p, c2)) return 0;
+  *chi2 = (double)c2;
+  return 1;
+}
+
 template <typename Real>
 int refitPoints(const orcGeometry* g, const orcParams* p, int n, const int32_t* rows, const double* y, const double* z,
                 double* in, double* out) {
@@ -818,6 +929,13 @@ int orcMatch(const orcParams* p, double bz_tesla, const double* a_state, const d
              const double* b_cov, int fp64, double* chi2) {
   return fp64 ? matchT<double>(p, bz_tesla, a_state, a_cov, rel, b_state, b_cov, chi2)
               : matchT<float>(p, bz_tesla, a_state, a_cov, rel, b_state, b_cov, chi2);
+}
+
+void orcMirror(double* state, double* cov) { mirrorT<double>(state, cov); }
+int orcLegMatch(const orcParams* p, double bz_tesla, const double* a_state, const double* a_cov, int d, const double* b_state,
+                const double* b_cov, int fp64, double* chi2) {
+  return fp64 ? legMatchT<double>(p, bz_tesla, a_state, a_cov, d, b_state, b_cov, chi2)
+              : legMatchT<float>(p, bz_tesla, a_state, a_cov, d, b_state, b_cov, chi2);
 }
 
 int orcRefitPoints(const orcGeometry* g, const orcParams* p, int n, const int32_t* rows, const double* y, const double* z,

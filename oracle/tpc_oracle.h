@@ -15,7 +15,7 @@
  * Pins (tests/test_oracle_*.py): grid search == brute-force search; collinear / hand-built link
  * cases; reciprocity and path invariants; Propagate vs the closed-form asin helix and vs finite
  * differences; Update / fit vs numpy least squares; exact helix recovery; unit pulls; full
- * attachment of noise-free high-pT helices; selector vs sorted greedy.
+ * attachment of noise-free high-pT helices; selector vs sorted greedy; O6..O10: see DESIGN.md, pins table.
  * Parity unpinned: physics efficiency / fake rate on configs 1-4 (no reference numbers exist).
  */
 #ifndef TPC_ORACLE_H
@@ -42,13 +42,15 @@ typedef struct {
   int32_t merge_max_row_gap, merge_back_rows;   /* O7: 40, 5 */
   float merge_chi2_max;                         /* O7: 50 */
   float tube_radius, inv_pt_protect;            /* O8: 1.5 cm, 20 c/GeV (pT = 50 MeV/c) */
+  float leg_min_sinphi, leg_chi2_max;           /* O10: 0.5, 50 */
+  int32_t leg_max_sectors, leg_max_row_diff;    /* O10: 4, 12 */
 } orcParams;
 
 typedef struct orcResult orcResult;
 
 enum { ORC_OK = 0, ORC_ERR_INVALID_ARG = -1, ORC_ERR_UNSORTED_OFFSETS = -2 };
 enum { ORC_BRUTE_FORCE = 1, ORC_FP64 = 2, ORC_REFIT = 4, ORC_MERGE = 8 /* implies ORC_REFIT */,
-       ORC_FLAGS = 16 /* implies ORC_REFIT */ };
+       ORC_FLAGS = 16 /* implies ORC_REFIT */, ORC_LEGS = 32 /* implies ORC_REFIT */ };
 
 void orcDefaultParams(orcParams* p);
 
@@ -115,6 +117,16 @@ int orcPackCharge(int64_t n_values, const float* q, int trunc_bits, uint16_t* co
 int orcRotate(double* state, double* cov, double alpha, double bz_tesla, double max_sinphi, int fp64);
 int orcMatch(const orcParams* p, double bz_tesla, const double* a_state, const double* a_cov, int rel,
              const double* b_state, const double* b_cov, int fp64, double* chi2);
+
+/* O10 (rest of NEXT-1, DESIGN.md section 3 "O10"; legs of loopers): the two sides of a turn,
+ * only with ORC_LEGS.  partner [n_tracks] = the track whose outer end is the other side of this track's outer turn
+ * (-1 none; partner[partner[k]] == k), chi2 [n_tracks] of that pair (0 if none).  Pins: tests/test_oracle_legs.py. */
+void orcGetLegs(const orcResult*, int32_t* partner, double* chi2);
+/* Pieces of O10 for the pins.  orcMirror: the state seen from the frame turned by 180 degrees and walked backwards.
+ * orcLegMatch: chi2 of two outer states a, b (b's sector d sectors after a's); returns 1 and *chi2 when admissible. */
+void orcMirror(double* state, double* cov);
+int orcLegMatch(const orcParams* p, double bz_tesla, const double* a_state, const double* a_cov, int d,
+                const double* b_state, const double* b_cov, int fp64, double* chi2);
 
 /* Single KF steps for the pins.  state = {x, y, z, s, t, q}, cov = 15 lower-triangle elements
  * (00,10,11,20,21,22,30,...,44), both in/out as doubles (rounded to binary32 first unless fp64).

@@ -22,6 +22,7 @@ FP64 = 2
 REFIT = 4
 MERGE = 8
 FLAGS = 16
+LEGS = 32
 
 
 def build(force: bool = False) -> str:
@@ -45,7 +46,9 @@ class Params(ctypes.Structure):
                [(n, ctypes.c_int32) for n in ("max_row_gap", "min_chain_hits", "min_tracklet_hits", "min_track_hits")] + \
                [("cell_min", ctypes.c_float), ("cell_max", ctypes.c_float), ("merge_max_row_gap", ctypes.c_int32),
                 ("merge_back_rows", ctypes.c_int32), ("merge_chi2_max", ctypes.c_float), ("tube_radius", ctypes.c_float),
-                ("inv_pt_protect", ctypes.c_float)]
+                ("inv_pt_protect", ctypes.c_float),
+                ("leg_min_sinphi", ctypes.c_float), ("leg_chi2_max", ctypes.c_float), ("leg_max_sectors", ctypes.c_int32),
+                ("leg_max_row_diff", ctypes.c_int32)]
 
 
 _lib = None
@@ -85,6 +88,12 @@ def _load():
         L.orcRotate.restype = ci
         L.orcMatch.argtypes = [ctypes.POINTER(Params), dbl, vp, vp, ci, vp, vp, ci, vp]
         L.orcMatch.restype = ci
+        L.orcGetLegs.argtypes = [vp] * 3
+        L.orcGetLegs.restype = None
+        L.orcMirror.argtypes = [vp, vp]
+        L.orcMirror.restype = None
+        L.orcLegMatch.argtypes = [ctypes.POINTER(Params), dbl, vp, vp, ci, vp, vp, ci, vp]
+        L.orcLegMatch.restype = ci
         L.orcGetRefit.argtypes = [vp] * 9
         L.orcGetRefit.restype = None
         L.orcRefitPoints.argtypes = [ctypes.POINTER(Geometry), ctypes.POINTER(Params), ci, vp, vp, vp, ci, vp, vp]
@@ -148,6 +157,9 @@ class OracleResult:
     mg_prev: np.ndarray | None = None
     mg_head: np.ndarray | None = None
     mg_chi2: np.ndarray | None = None
+    # O10 looper legs (only with legs=True): the track on the other side of the outer turn, chi2 of the pair
+    lg_partner: np.ndarray | None = None
+    lg_chi2: np.ndarray | None = None
     # O8 cluster flags (only with flags=True): bit mask per cluster and the owning track
     cf_flags: np.ndarray | None = None
     cf_owner: np.ndarray | None = None
@@ -164,7 +176,8 @@ def _ptr(a):
 
 
 def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool = False,
-        stages_only: bool = False, refit: bool = False, merge: bool = False, flags: bool = False) -> OracleResult:
+        stages_only: bool = False, refit: bool = False, merge: bool = False, flags: bool = False,
+        legs: bool = False) -> OracleResult:
     """Run O1..O5 on an Event-like object (fields n_sectors, n_rows, row_x, row_dead, bz_tesla,
     tan_half_sector, z_min, z_max, row_offset, y, z; numpy arrays)."""
     L = _load()
@@ -179,7 +192,7 @@ def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool 
     n = int(y.shape[0])
     h = ctypes.c_void_p()
     rc = L.orcRun(ctypes.byref(g), ctypes.byref(p), n, off.ctypes.data, _ptr(y), _ptr(z),
-                  (BRUTE_FORCE if brute_force else 0) | (FP64 if fp64 else 0) | (REFIT if refit else 0) | (MERGE if merge else 0) | (FLAGS if flags else 0),
+                  (BRUTE_FORCE if brute_force else 0) | (FP64 if fp64 else 0) | (REFIT if refit else 0) | (MERGE if merge else 0) | (FLAGS if flags else 0) | (LEGS if legs else 0),
                   ctypes.byref(h))
     if rc != 0:
         raise ValueError(f"orcRun failed with {rc}")
@@ -207,7 +220,7 @@ def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool 
         L.orcGetTracks(h, _ptr(kid), _ptr(ks), _ptr(kf), _ptr(kl), _ptr(kn), _ptr(kx), _ptr(kpar), _ptr(kcov),
                        _ptr(kchi), _ptr(koff), _ptr(kidx))
         rf = {}
-        refit = refit or merge or flags
+        refit = refit or merge or flags or legs
         if refit:
             rst = np.zeros(nt, np.int32)
             rxi, rchi, rxo = np.zeros(nt), np.zeros(nt), np.zeros(nt)
@@ -220,6 +233,10 @@ def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool 
             mc = np.zeros(nt)
             L.orcGetMerge(h, _ptr(mn), _ptr(mp), _ptr(mh), _ptr(mc))
             rf.update(mg_next=mn, mg_prev=mp, mg_head=mh, mg_chi2=mc)
+        if legs:
+            lp, lc = np.full(nt, -1, np.int32), np.zeros(nt)
+            L.orcGetLegs(h, _ptr(lp), _ptr(lc))
+            rf.update(lg_partner=lp, lg_chi2=lc)
         if flags:
             cf, co = np.zeros(n, np.uint8), np.full(n, -1, np.int32)
             L.orcGetClusterFlags(h, _ptr(cf), _ptr(co))
@@ -281,6 +298,25 @@ def match(a_state, a_cov, rel, b_state, b_cov, bz_tesla=0.5, params: Params | No
     chi2 = np.zeros(1)
     ok = _load().orcMatch(ctypes.byref(p), float(bz_tesla), a.ctypes.data, ac.ctypes.data, int(rel), b.ctypes.data,
                           bc.ctypes.data, int(fp64), chi2.ctypes.data)
+    return bool(ok), float(chi2[0])
+
+
+def mirror(state, cov):
+    """O10 Mirror: the state seen from the frame turned by 180 degrees and walked backwards.  Returns (state, cov)."""
+    s = np.array(state, np.float64)
+    c = np.array(cov, np.float64)
+    _load().orcMirror(s.ctypes.data, c.ctypes.data)
+    return s, c
+
+
+def leg_match(a_state, a_cov, d, b_state, b_cov, bz_tesla=0.5, params: Params | None = None, fp64=True):
+    """O10 LegMatch of two outer states (b's sector d sectors after a's).  Returns (ok, chi2)."""
+    p = params if params is not None else default_params()
+    a, ac = np.array(a_state, np.float64), np.array(a_cov, np.float64)
+    b, bc = np.array(b_state, np.float64), np.array(b_cov, np.float64)
+    chi2 = np.zeros(1)
+    ok = _load().orcLegMatch(ctypes.byref(p), float(bz_tesla), a.ctypes.data, ac.ctypes.data, int(d), b.ctypes.data,
+                             bc.ctypes.data, int(fp64), chi2.ctypes.data)
     return bool(ok), float(chi2[0])
 
 
