@@ -32,9 +32,9 @@ WORKLOADS = {0: "config0 single sector, 200 primaries", 1: "config1 central Pb-P
 
 
 ALU_SMS = 148
-# ncu counts of one launch on the bench workload (config 4, seed 5), from the committed capture profiles/r1i_full_capture.md
-NCU_R1 = {(4, "a4_constructor"): {"kernel": "trackletConstructor", "warp_inst": 2.2821e10, "dram_bytes": 14120804000},
-          (4, "a2_neighbours"): {"kernel": "neighbourFinder", "warp_inst": 1.2086e10, "dram_bytes": 1604527000}}
+# ncu counts of one launch on the bench workload (config 4, seed 5), from the committed capture profiles/r1j_full_capture.md
+NCU_R1 = {(4, "a4_constructor"): {"kernel": "trackletConstructor", "warp_inst": 2.2818e10, "dram_bytes": 14122392000},
+          (4, "a2_neighbours"): {"kernel": "neighbourFinder", "warp_inst": 1.1833e10, "dram_bytes": 1607099000}}
 
 
 def _peaks():
@@ -298,7 +298,7 @@ def run_ours(args, rank, world, local_rank):
     share = round(dom_ms / max(float(stage[6]), 1e-9), 4)
     ncu = NCU_R1.get((args.config, dom))
     if ncu is not None:
-        # The dominant kernels are bound by instruction issue, not by HBM (profiles/r1i_full_capture.md):
+        # The dominant kernels are bound by instruction issue, not by HBM (profiles/r1j_full_capture.md):
         # achieved = warp instructions of one launch (ncu smsp__inst_executed.sum of the committed capture of this
         # workload) / the live CUDA-event time of the stage; peak = SMs x 4 schedulers x 1 instruction/clock x max SM clock.
         sm_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
@@ -309,7 +309,7 @@ def run_ours(args, rank, world, local_rank):
                     "peak_source": f"{ALU_SMS} SMs x 4 schedulers x {sm_mhz:.0f} MHz (B200_PROFILING.md unit counts and clocks)",
                     "alg_bytes": int(alg[dom]), "alg_gbs": round(alg[dom] / (dom_ms * 1e-3) / 1e9, 1),
                     "alg_frac_of_hbm_peak": round(alg[dom] / (dom_ms * 1e-3) / 1e9 / peak, 5),
-                    "counts_from": "profiles/r1i_full_capture.md", "whole_path": whole, "share_of_step": share}
+                    "counts_from": "profiles/r1j_full_capture.md", "whole_path": whole, "share_of_step": share}
     else:
         achieved = alg[dom] / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0
         roofline = {"bound": "hbm", "kernel": dom, "achieved": round(achieved, 2), "peak": peak, "unit": "GB/s",

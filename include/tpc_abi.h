@@ -10,6 +10,7 @@
  *   a5 tracklet selector   shared clusters go to the longest / lowest-chi2 tracklet
  *   a6 refit (optional)    Kalman refit of every selected track over its kept clusters: inner and outer state
  *   a7 merger (optional)   links between track segments across row gaps and sector borders
+ *   a10 legs (optional)    pairs of track ends that are the two sides of a looper's outer turn
  *   a8 flags (optional)    per cluster: attached / adjacent / protected, removed by rejection strategy A / B
  * The formulas, constants and tie-breaks are DESIGN.md section 3 (readings R0..R27 of SURVEY.md 8(c)).
  *
@@ -79,6 +80,10 @@ typedef struct {
   float tube_radius;            /* 1.5        O8: clusters within this distance of a track are adjacent, cm */
   float inv_pt_protect;         /* 20         O8: tracks with |q/pT| below this (pT > 50 MeV/c) protect */
   int32_t charge_trunc_bits;    /* 4          O9: bits kept after the first non-zero bit of a charge */
+  float leg_min_sinphi;         /* 0.5        O10: a refitted track that ends with |sin phi| not below this is a leg end */
+  float leg_chi2_max;           /* 50         O10: cut on the diagonal chi2 of the two sides of a turn */
+  int32_t leg_max_sectors;      /* 4          O10: the two ends of a turn are at most this many sectors apart (0..8) */
+  int32_t leg_max_row_diff;     /* 12         O10: and their last rows at most this many rows */
 } tpcParams;
 
 /* Input clusters: CSR by (sector,row), fp32 SoA (single-precision cluster properties). */
@@ -138,6 +143,11 @@ typedef struct {
   int32_t* trk_mg_prev;         /* [cap_tracks] track this one continues, -1 none */
   int32_t* trk_mg_head;         /* [cap_tracks] first track of the chain (itself if unlinked) */
   float* trk_mg_chi2;           /* [cap_tracks] chi2 of the link to trk_mg_next, 0 if none */
+  /* optional O10 pairs of looper legs (DESIGN.md section 3 "O10").  Both NULL = none; otherwise both,
+   * together with the refit outputs (the outer states are compared). */
+  int32_t* trk_leg_partner;     /* [cap_tracks] the track whose outer end is the other side of this track's outer turn, -1 none;
+                                   partner[partner[k]] == k */
+  float* trk_leg_chi2;          /* [cap_tracks] chi2 of that pair (the same on both), 0 if none */
   /* optional O8 per-cluster flags (DESIGN.md section 3 "O8").  Both NULL = none; otherwise both, together
    * with the refit outputs.  Indexed by the INPUT cluster index. */
   uint8_t* cl_flags;            /* [n_clusters] 1 attached, 2 adjacent, 4 protected, 8 removed by strategy A, 16 by strategy B */
@@ -166,6 +176,7 @@ typedef struct {
   float merge_ms;               /* the O7 merger alone (profiling on, merger requested) */
   float pack_ms;                /* the O9 charge code alone (profiling on, cl_qcode requested) */
   float flags_ms;               /* the O8 cluster flags alone (profiling on, flags requested) */
+  float legs_ms;                /* the O10 leg pairs alone (profiling on, legs requested) */
   float submit_ms[2];           /* tpcCollectHost only: device time of the slot from its first copy in to the end of its
                                    kernels [0] and to the end of its copies out [1] (includes waiting for the other slot) */
 } tpcRunStatus;

@@ -20,6 +20,7 @@
 #include "tpc_select.cuh"
 #include "tpc_refit.cuh"
 #include "tpc_merge.cuh"
+#include "tpc_legs.cuh"
 #include "tpc_flags.cuh"
 
 using namespace tpc;
@@ -57,6 +58,9 @@ struct Workspace {
   float* mg_chi_b;
   unsigned long long* mg_key_a;
   unsigned long long* fl_key;      // [N] bids of the cluster flags
+  uint32_t *lg_start, *lg_fill, *lg_list;   // leg pairs: leg ends bucketed by (sector, last row)
+  int32_t* lg_best;
+  float* lg_chi;
   size_t bytes;
 };
 
@@ -73,7 +77,7 @@ struct tpcHandle {
   int64_t* d_cnt = nullptr;        // CNT_COUNT counters + 1 slot for the packed selector total
   int64_t* h_cnt = nullptr;        // pinned copy
   cudaEvent_t ev_done = nullptr;
-  cudaEvent_t ev_stage[15] = {};   // ... 13/14 around the charge code
+  cudaEvent_t ev_stage[17] = {};   // ... 13/14 around the charge code, 15/16 leg pairs
   //   // 0..6 stage boundaries, 7/8 around the optional refit, 9/10 merger, 11/12 flags
   int profiling = 0;
   int launches = 0;
@@ -176,6 +180,11 @@ Workspace layout(const tpcHandle* h, int64_t N, int64_t capT, char* base) {
   w.mg_chi_b = (float*)take(4 * (size_t)Tn);
   w.mg_key_a = (unsigned long long*)take(8 * (size_t)Tn);
   w.fl_key = (unsigned long long*)take(8 * (size_t)Nn);
+  w.lg_start = (uint32_t*)take(4 * (size_t)(nb + 1));
+  w.lg_fill = (uint32_t*)take(4 * (size_t)(nb + 1));
+  w.lg_list = (uint32_t*)take(4 * (size_t)Tn);
+  w.lg_best = (int32_t*)take(4 * (size_t)Tn);
+  w.lg_chi = (float*)take(4 * (size_t)Tn);
   w.bytes = o;
   return w;
 }
@@ -196,6 +205,7 @@ int tpcDefaultParams(tpcParams* p) {
   p->validate_input = 0; p->force_wide_keys = 0;
   p->merge_max_row_gap = 40; p->merge_back_rows = 5; p->merge_chi2_max = 50.0f;
   p->tube_radius = 1.5f; p->inv_pt_protect = 20.0f; p->charge_trunc_bits = 4;
+  p->leg_min_sinphi = 0.5f; p->leg_chi2_max = 50.0f; p->leg_max_sectors = 4; p->leg_max_row_diff = 12;
   return TPC_OK;
 }
 
@@ -211,6 +221,7 @@ int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cud
   if (p->min_chain_hits < 2 || p->max_row_gap < 0) return TPC_ERR_INVALID_ARG;
   if (p->merge_max_row_gap < 0 || p->merge_back_rows < 0) return TPC_ERR_INVALID_ARG;
   if (!(p->tube_radius >= 0) || p->charge_trunc_bits < 0 || p->charge_trunc_bits > 14) return TPC_ERR_INVALID_ARG;
+  if (p->leg_max_sectors < 0 || p->leg_max_sectors > LEG_MAX_SECTORS || p->leg_max_row_diff < 0) return TPC_ERR_INVALID_ARG;
   tpcHandle* h = new (std::nothrow) tpcHandle();
   if (!h) return TPC_ERR_INVALID_ARG;
   h->device = cuda_device;
@@ -251,7 +262,7 @@ int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cud
             cudaMalloc(&h->d_cnt, 8 * (CNT_COUNT + 1)) == cudaSuccess &&
             cudaMallocHost(&h->h_cnt, 8 * (CNT_COUNT + 1)) == cudaSuccess &&
             cudaEventCreate(&h->ev_done) == cudaSuccess;
-  for (int i = 0; ok && i < 15; ++i) ok = cudaEventCreate(&h->ev_stage[i]) == cudaSuccess;
+  for (int i = 0; ok && i < 17; ++i) ok = cudaEventCreate(&h->ev_stage[i]) == cudaSuccess;
   ok = ok && cudaMemcpy(h->d_row_x, g->row_x, 4 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
        cudaMemcpy(h->d_up, up.data(), 2 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
        cudaMemcpy(h->d_dn, dn.data(), 2 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
@@ -276,7 +287,7 @@ int tpcDestroy(tpcHandle* h) {
   cudaFree(h->d_row_x); cudaFree(h->d_up); cudaFree(h->d_dn); cudaFree(h->d_dead); cudaFree(h->d_cnt);
   if (h->h_cnt) cudaFreeHost(h->h_cnt);
   if (h->ev_done) cudaEventDestroy(h->ev_done);
-  for (int i = 0; i < 15; ++i) if (h->ev_stage[i]) cudaEventDestroy(h->ev_stage[i]);
+  for (int i = 0; i < 17; ++i) if (h->ev_stage[i]) cudaEventDestroy(h->ev_stage[i]);
   if (h->cur_slot != 0) {}   // the active state is freed below; the parked slots here
   for (int k = 0; k < 3; ++k) {
     if (k == h->cur_slot || !h->slots[k].init) continue;
@@ -329,6 +340,8 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
                    (out->trk_mg_chi2 != nullptr);
   if ((n_mg != 0 && n_mg != 4) || (n_mg == 4 && n_rf != 8)) return TPC_ERR_INVALID_ARG;   // the merger needs the refit
   if (n_mg == 4 && (int64_t)h->P.n_buckets * MG_NYB * MG_NZB >= (1ll << 31)) return TPC_ERR_INVALID_ARG;   // bucket ids are 32-bit
+  const int n_lg = (out->trk_leg_partner != nullptr) + (out->trk_leg_chi2 != nullptr);
+  if ((n_lg != 0 && n_lg != 2) || (n_lg == 2 && n_rf != 8)) return TPC_ERR_INVALID_ARG;   // the leg pairs need the refit
   if (out->cl_qcode && N > 0 && !in->q) return TPC_ERR_INVALID_ARG;                      // the charge code needs the charges
   const int n_fl = (out->cl_flags != nullptr) + (out->cl_owner != nullptr);
   if ((n_fl != 0 && n_fl != 2) || (n_fl == 2 && n_rf != 8)) return TPC_ERR_INVALID_ARG;   // so do the cluster flags
@@ -470,6 +483,35 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
     mergeHead<<<gK, 256, 0, st>>>(mi, mo, cnt); ++L;
   }
   stage(10);
+  // ---- a10 optional pairs of looper legs (O10) -------------------------------------------------------
+  stage(15);
+  if (n_lg == 2 && N > 0 && out->cap_tracks > 0) {
+    const int64_t nk = std::min<int64_t>(out->cap_tracks, capT);
+    const LegIn li{out->cap_tracks, out->trk_rf_status, out->trk_sector, out->trk_last_row, out->trk_rf_x_out,
+                   out->trk_rf_par_out, out->trk_rf_cov_out};
+    const LegOut lo{out->trk_leg_partner, out->trk_leg_chi2};
+    LegParams lp{};
+    lp.min_sinphi = h->params.leg_min_sinphi; lp.chi2_max = h->params.leg_chi2_max;
+    lp.max_sectors = h->params.leg_max_sectors; lp.max_row_diff = h->params.leg_max_row_diff;
+    for (int d = -LEG_MAX_SECTORS; d <= LEG_MAX_SECTORS; ++d)
+      for (int sg = -1; sg <= 1; sg += 2) {
+        if (d * sg < 0) continue;                  // a moves towards b's sector
+        const double a10 = 0.17453292519943295, a90 = 1.5707963267948966;
+        const double alpha = (double)d * a10 + (double)sg * a90;
+        const int i = d + LEG_MAX_SECTORS + (sg > 0 ? 1 : 0);
+        lp.ca[i] = (float)cos(alpha); lp.sa[i] = (float)sin(alpha);
+        lp.cb[i] = (float)cos(-alpha); lp.sb[i] = (float)sin(-alpha);
+      }
+    const unsigned gK = (unsigned)ceilDiv(nk, 256);
+    TPC_CUDA(h, cudaMemsetAsync(w.lg_start, 0, 4 * (size_t)(nb + 1), st)); ++L;
+    TPC_CUDA(h, cudaMemsetAsync(w.lg_fill, 0, 4 * (size_t)(nb + 1), st)); ++L;
+    legCount<<<gK, 256, 0, st>>>(li, lo, P, lp, w.lg_start, w.lg_best, cnt); ++L;
+    scanArrayInPlace<uint32_t><<<1, 1024, 0, st>>>(w.lg_start, (int64_t)nb + 1, nullptr); ++L;
+    legFill<<<gK, 256, 0, st>>>(li, P, lp, w.lg_start, w.lg_fill, w.lg_list, cnt); ++L;
+    legMatch<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(li, P, lp, w.lg_start, w.lg_list, w.lg_best, w.lg_chi, cnt); ++L;
+    legLink<<<gK, 256, 0, st>>>(li, lo, w.lg_best, w.lg_chi, cnt); ++L;
+  }
+  stage(16);
   // ---- a8 optional per-cluster flags (O8) ------------------------------------------------------------
   stage(11);
   if (n_fl == 2 && N > 0) {
@@ -539,6 +581,7 @@ int tpcGetRunStatus(tpcHandle* h, tpcRunStatus* out) {
     if (cudaEventElapsedTime(&ms, h->ev_stage[9], h->ev_stage[10]) == cudaSuccess) out->merge_ms = ms;
     if (cudaEventElapsedTime(&ms, h->ev_stage[11], h->ev_stage[12]) == cudaSuccess) out->flags_ms = ms;
     if (cudaEventElapsedTime(&ms, h->ev_stage[13], h->ev_stage[14]) == cudaSuccess) out->pack_ms = ms;
+    if (cudaEventElapsedTime(&ms, h->ev_stage[15], h->ev_stage[16]) == cudaSuccess) out->legs_ms = ms;
   }
   return TPC_OK;
 }
@@ -583,7 +626,7 @@ extern "C" int tpcRunHost(tpcHandle* h, int64_t N, const uint32_t* row_offset, c
       oh->tl_first_row || oh->tl_last_row || oh->tl_rowhit || oh->tl_x || oh->tl_par || oh->tl_cov || oh->tl_chi2 ||
       oh->trk_rf_status || oh->trk_rf_x_in || oh->trk_rf_par_in || oh->trk_rf_cov_in || oh->trk_rf_chi2 || oh->trk_rf_x_out ||
       oh->trk_rf_par_out || oh->trk_rf_cov_out || oh->trk_mg_next || oh->trk_mg_prev || oh->trk_mg_head || oh->trk_mg_chi2 ||
-      oh->cl_flags || oh->cl_owner || oh->cl_qcode || oh->cl_res_y || oh->cl_res_z)
+      oh->trk_leg_partner || oh->trk_leg_chi2 || oh->cl_flags || oh->cl_owner || oh->cl_qcode || oh->cl_res_y || oh->cl_res_z)
     return TPC_ERR_INVALID_ARG;
   if (!oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0) return TPC_ERR_INVALID_ARG;
   TPC_CUDA(h, cudaSetDevice(h->device));
@@ -693,7 +736,7 @@ extern "C" int tpcSubmitHost(tpcHandle* h, int slot, int64_t N, const uint32_t* 
     return TPC_ERR_INVALID_ARG;
   if (oh->link_up_raw || oh->link_dn_raw || oh->link_up || oh->link_dn || oh->start_hits || oh->tl_status || oh->tl_nhits ||
       oh->tl_first_row || oh->tl_last_row || oh->tl_rowhit || oh->tl_x || oh->tl_par || oh->tl_cov || oh->tl_chi2 ||
-      oh->trk_rf_status || oh->trk_mg_next || oh->cl_flags || oh->cl_owner || oh->cl_qcode || oh->cl_res_y || oh->cl_res_z || !oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0)
+      oh->trk_rf_status || oh->trk_mg_next || oh->trk_leg_partner || oh->trk_leg_chi2 || oh->cl_flags || oh->cl_owner || oh->cl_qcode || oh->cl_res_y || oh->cl_res_z || !oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0)
     return TPC_ERR_INVALID_ARG;
   TPC_CUDA(h, cudaSetDevice(h->device));
   int rc;

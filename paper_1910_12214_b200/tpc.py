@@ -37,7 +37,8 @@ class tpcParams(ctypes.Structure):
                [("cell_min", c_float), ("cell_max", c_float), ("clusters_per_cell", c_float),
                 ("validate_input", c_int32), ("force_wide_keys", c_int32), ("merge_max_row_gap", c_int32),
                 ("merge_back_rows", c_int32), ("merge_chi2_max", c_float), ("tube_radius", c_float),
-                ("inv_pt_protect", c_float), ("charge_trunc_bits", c_int32)]
+                ("inv_pt_protect", c_float), ("charge_trunc_bits", c_int32), ("leg_min_sinphi", c_float),
+                ("leg_chi2_max", c_float), ("leg_max_sectors", c_int32), ("leg_max_row_diff", c_int32)]
 
 
 class tpcClusters(ctypes.Structure):
@@ -52,19 +53,21 @@ _STAGE_PTRS = ("link_up_raw", "link_dn_raw", "link_up", "link_dn", "start_hits",
 _REFIT_PTRS = ("trk_rf_status", "trk_rf_x_in", "trk_rf_par_in", "trk_rf_cov_in", "trk_rf_chi2", "trk_rf_x_out",
                "trk_rf_par_out", "trk_rf_cov_out")
 _MERGE_PTRS = ("trk_mg_next", "trk_mg_prev", "trk_mg_head", "trk_mg_chi2")
+_LEG_PTRS = ("trk_leg_partner", "trk_leg_chi2")
 _FLAG_PTRS = ("cl_flags", "cl_owner", "cl_res_y", "cl_res_z")
 _PACK_PTRS = ("cl_qcode",)
 
 
 class tpcTracks(ctypes.Structure):
     _fields_ = [("cap_tracks", c_int64), ("cap_track_clusters", c_int64)] + \
-               [(n, c_void_p) for n in _TRK_PTRS + _STAGE_PTRS + _REFIT_PTRS + _MERGE_PTRS + _FLAG_PTRS + _PACK_PTRS]
+               [(n, c_void_p) for n in _TRK_PTRS + _STAGE_PTRS + _REFIT_PTRS + _MERGE_PTRS + _LEG_PTRS + _FLAG_PTRS + _PACK_PTRS]
 
 
 class tpcRunStatus(ctypes.Structure):
     _fields_ = [("status", c_int32), ("kernel_launches", c_int32), ("n_clusters", c_int64), ("n_start_hits", c_int64),
                 ("n_tracklets", c_int64), ("n_tracklet_hits", c_int64), ("n_tracks", c_int64),
-                ("n_track_clusters", c_int64), ("n_cells", c_int64), ("stage_ms", c_float * 8), ("merge_ms", c_float), ("pack_ms", c_float), ("flags_ms", c_float), ("submit_ms", c_float * 2)]
+                ("n_track_clusters", c_int64), ("n_cells", c_int64), ("stage_ms", c_float * 8), ("merge_ms", c_float), ("pack_ms", c_float), ("flags_ms", c_float), ("legs_ms", c_float),
+                ("submit_ms", c_float * 2)]
 
 
 ABI_SYMBOLS = ("tpcDefaultParams", "tpcCreate", "tpcDestroy", "tpcWorkspaceBytes", "tpcRun", "tpcGetRunStatus",
@@ -234,7 +237,7 @@ class TpcTracker:
         z = t.from_numpy(np.ascontiguousarray(ev.z, np.float32)).to(self.device)
         return off, y, z
 
-    def _ensure(self, n, capT, capK, capC, stages, refit=False, merge=False, flags=False, pack=False):
+    def _ensure(self, n, capT, capK, capC, stages, refit=False, merge=False, flags=False, pack=False, legs=False):
         t = self.torch
         need = tpcWorkspaceBytes(self.handle, n, capT)
         if self._ws is None or self._ws.numel() < need:
@@ -265,6 +268,8 @@ class TpcTracker:
         if merge:
             spec.update({"trk_mg_next": ((capK,), i32), "trk_mg_prev": ((capK,), i32), "trk_mg_head": ((capK,), i32),
                          "trk_mg_chi2": ((capK,), f32)})
+        if legs:
+            spec.update({"trk_leg_partner": ((capK,), i32), "trk_leg_chi2": ((capK,), f32)})
         for k, (shape, dt) in spec.items():
             cur = self._out.get(k)
             if cur is None or tuple(cur.shape) != shape:
@@ -275,17 +280,18 @@ class TpcTracker:
 
     def run(self, row_offset, y, z, cap_tracklets: int | None = None, cap_tracks: int | None = None,
             cap_track_clusters: int | None = None, stages: bool = False, stream=None, sync: bool = True,
-            grow: bool = True, refit: bool = False, merge: bool = False, flags: bool = False, q=None):
+            grow: bool = True, refit: bool = False, merge: bool = False, flags: bool = False, q=None,
+            legs: bool = False):
         """One tpcRun on device tensors (q: optional device tensor of charges -> cl_qcode, the O9 charge code).  Returns a TrackResult (after synchronising) or None when sync=False."""
         t = self.torch
         n = int(y.shape[0])
-        refit = refit or merge or flags   # the merger and the cluster flags work on the refitted states
+        refit = refit or merge or flags or legs   # the merger, the leg pairs and the cluster flags work on the refitted states
         capT = int(cap_tracklets) if cap_tracklets is not None else max(4096, n // 8)
         capK = int(cap_tracks) if cap_tracks is not None else capT
         capC = int(cap_track_clusters) if cap_track_clusters is not None else max(n, 1)
         attempts = 3 if grow else 0     # a too-small cap_tracklets hides the true track counts: up to 3 rounds
         while True:
-            self._ensure(n, capT, capK, capC, stages, refit, merge, flags, q is not None)
+            self._ensure(n, capT, capK, capC, stages, refit, merge, flags, q is not None, legs)
             cl = tpcClusters(n, row_offset.data_ptr(), None, y.data_ptr() if n else None, z.data_ptr() if n else None,
                              q.data_ptr() if (q is not None and n) else None)
             tr = tpcTracks()
@@ -318,6 +324,9 @@ class TpcTracker:
                 trk[k] = o[k][:, :nt] if o[k].dim() == 2 else o[k][:nt]
         if merge:
             for k in _MERGE_PTRS:
+                trk[k] = o[k][:nt]
+        if legs:
+            for k in _LEG_PTRS:
                 trk[k] = o[k][:nt]
         if flags:
             for k in _FLAG_PTRS:

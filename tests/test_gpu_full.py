@@ -94,3 +94,64 @@ def test_full_size_sector0_equals_oracle_and_global_invariants(idx):
     assert bool((bucket_sector[idx_all] == res.trk["trk_sector"].long()[trk_of_cl]).all().item())
     assert bool(torch.isfinite(res.trk["trk_par"]).all().item()) and bool(torch.isfinite(res.trk["trk_cov"]).all().item())
     trk.close()
+
+
+def test_full_size_leg_pairs_sampled_against_the_oracle_pair_function():
+    """Config 4 with the a10 leg pairs: the pairing is a property of the refitted outer states (bit-identical to the oracle's,
+    see above), so sampled leg ends are re-paired from the GPU's own states with the oracle's LegMatch -- brute force over
+    every admissible end of the whole event -- and must give the GPU's partner and chi2 exactly; reciprocity and the
+    admission rules are checked on all pairs."""
+    from paper_1910_12214_b200 import tpc
+    ev = datagen.make_event(4)
+    trk = tpc.TpcTracker.from_event(ev)
+    off, y, z = trk.upload(ev)
+    st = trk.run(off, y, z).status
+    res = trk.run(off, y, z, cap_tracklets=int(st.n_start_hits * 1.05) + 1024, cap_tracks=int(st.n_tracks * 1.05) + 1024,
+                  cap_track_clusters=int(st.n_track_clusters * 1.05) + 1024, legs=True)
+    assert res.status.status == 0
+    g = res.numpy()
+    trk.close()
+    p = orc.default_params()
+    lp, lc = g["trk_leg_partner"], g["trk_leg_chi2"]
+    sec, last, ok = g["trk_sector"], g["trk_last_row"], g["trk_rf_status"] == 1
+    xo, po, co = g["trk_rf_x_out"], g["trk_rf_par_out"], g["trk_rf_cov_out"]          # [nt], [5, nt], [15, nt]
+    s_out = po[2]
+    linked = np.nonzero(lp >= 0)[0]
+    assert len(linked) > 1000
+    assert np.array_equal(lp[lp[linked]], linked) and np.array_equal(lc[lp[linked]], lc[linked])
+    assert np.all(ok[linked]) and np.all(np.abs(s_out[linked]) >= np.float32(p.leg_min_sinphi))
+    assert np.all(s_out[linked] * s_out[lp[linked]] < 0) and np.all(lc[linked] <= np.float32(p.leg_chi2_max))
+    assert np.all(np.abs(last[linked] - last[lp[linked]]) <= p.leg_max_row_diff) and np.all(sec[linked] // 18 == sec[lp[linked]] // 18)
+    assert np.all(lc[lp < 0] == 0)
+    ends = np.nonzero(ok & ~(np.abs(s_out) < np.float32(p.leg_min_sinphi)))[0]
+
+    def state(k):
+        return np.concatenate([[xo[k]], po[:, k]]).astype(np.float64), co[:, k].astype(np.float64)
+
+    def best_of(k):
+        d_all = (sec[ends] % 18 - sec[k] % 18) % 18
+        d_all = np.where(d_all > 9, d_all - 18, d_all)
+        sg = 1 if s_out[k] > 0 else -1
+        m = (sec[ends] // 18 == sec[k] // 18) & (np.abs(d_all) <= p.leg_max_sectors) & (d_all * sg >= 0) & (ends != k) & \
+            (np.abs(last[ends] - last[k]) <= p.leg_max_row_diff) & (s_out[ends] * s_out[k] < 0)
+        best = (np.inf, -1)
+        for b, d in zip(ends[m], d_all[m]):
+            lo, hi, dd = (k, b, int(d)) if k < b else (b, k, -int(d))
+            (sa, ca), (sb, cb) = state(lo), state(hi)
+            good, c2 = orc.leg_match(sa, ca, dd, sb, cb, ev.bz_tesla, p, fp64=False)
+            if good and (c2, b) < best:
+                best = (c2, int(b))
+        return best
+
+    rng = np.random.default_rng(7)
+    sample = np.concatenate([rng.choice(linked, 150, replace=False), rng.choice(ends, 150, replace=False)])
+    n_pairs = 0
+    for k in sample:
+        c2, b = best_of(int(k))
+        if b >= 0 and best_of(b)[1] == k:
+            assert lp[k] == b and lc[k] == np.float32(c2)
+            n_pairs += 1
+        else:
+            assert lp[k] == -1 and lc[k] == 0
+    assert n_pairs >= 150
+    print("config 4: leg ends", len(ends), "paired", len(linked), "legs_ms", res.status.legs_ms)
