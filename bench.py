@@ -217,25 +217,28 @@ def run_ours(args, rank, world, local_rank):
     stage /= args.steps
 
     # ---- the NEXT-2 row (a6 refit of the selected tracks), timed apart: it is not part of the a1..a5 step ----------
-    refit_ms = merge_ms = flags_ms = pack_ms = None
-    n_links = 0
+    refit_ms = merge_ms = flags_ms = pack_ms = legs_ms = None
+    n_links = n_legs = 0
     flag_frac = {}
     if not args.no_refit:
-        acc = accm = accf = accp = 0.0
+        acc = accm = accf = accp = accl = 0.0
         dq = torch.from_numpy(ev.q).to(y.device)
         for i in range(4):
-            trk.run(off, y, z, cap_tracklets=capT, cap_tracks=capK, cap_track_clusters=capC, sync=False, merge=True, flags=True, q=dq)
+            trk.run(off, y, z, cap_tracklets=capT, cap_tracks=capK, cap_track_clusters=capC, sync=False, merge=True, flags=True, q=dq,
+                    legs=True)
             s = trk.status()
             if i > 0:
                 acc += float(s.stage_ms[7])
                 accm += float(s.merge_ms)
                 accf += float(s.flags_ms)
                 accp += float(s.pack_ms)
-        refit_ms, merge_ms, flags_ms, pack_ms = acc / 3, accm / 3, accf / 3, accp / 3
+                accl += float(s.legs_ms)
+        refit_ms, merge_ms, flags_ms, pack_ms, legs_ms = acc / 3, accm / 3, accf / 3, accp / 3, accl / 3
         fl = trk._out["cl_flags"][:N]
         flag_frac = {name: round(float(((fl & bit) != 0).float().mean().item()), 4)
                      for name, bit in (("attached", 1), ("adjacent", 2), ("protected", 4), ("removed_A", 8), ("removed_B", 16))}
         n_links = int((trk._out["trk_mg_next"][:int(s.n_tracks)] >= 0).sum().item())
+        n_legs = int((trk._out["trk_leg_partner"][:int(s.n_tracks)] >= 0).sum().item()) // 2
 
     # ---- end to end through the host-buffer ABI call (pinned host memory; copies inside the timed region) ----
     hy = torch.from_numpy(ev.y).pin_memory()
@@ -363,6 +366,8 @@ def run_ours(args, rank, world, local_rank):
                               "tracks": int(st.n_tracks), "track_clusters": ncl}
         line["next_merge"] = {"what": "a7 segment merger (NEXT-1), not part of `value`", "ms": round(merge_ms, 4),
                               "links": n_links}
+        line["next_legs"] = {"what": "a10 pairs of looper legs (rest of NEXT-1), not part of `value`", "ms": round(legs_ms, 4),
+                             "pairs": n_legs}
         line["next_pack"] = {"what": "a9 dynamic-precision charge code (part of NEXT-4), not part of `value`",
                              "ms": round(pack_ms, 4), "alg_bytes": 6 * N, "bound": "hbm",
                              "gbs": round(6 * N / (pack_ms * 1e-3) / 1e9, 1) if pack_ms > 0 else None,

@@ -180,6 +180,15 @@ void mirror(State<Real>& st) {
 template <typename Real>
 bool legMatch(State<Real> a, int d, State<Real> b, Real bfield, const orcParams& P, Real& chi2) {
   const double a10 = 0.17453292519943295, a90 = 1.5707963267948966;
+  {   // R44: the two sides of a turn lie on one circle -- centres (a's frame; b's frame is turned by d * 20 degrees) close
+    const Real ka = a.q * bfield, kb = b.q * bfield;
+    const Real xa = a.x - a.s / ka, ya = a.y + std::sqrt((Real)1 - a.s * a.s) / ka;
+    const Real xb = b.x - b.s / kb, yb = b.y + std::sqrt((Real)1 - b.s * b.s) / kb;
+    const Real cd = (Real)std::cos((double)d * (2.0 * a10)), sd = (Real)std::sin((double)d * (2.0 * a10));
+    const Real ex = (xb * cd - yb * sd) - xa, ey = (xb * sd + yb * cd) - ya;
+    const Real md = (Real)P.leg_max_centre_dist;
+    if (!(ex * ex + ey * ey <= md * md)) return false;
+  }
   const double sg = a.s > (Real)0 ? 1.0 : -1.0;
   const double alpha = (double)d * a10 + sg * a90;
   if (!rotate(a, alpha, bfield, (Real)P.max_sinphi)) return false;
@@ -776,6 +785,7 @@ void orcDefaultParams(orcParams* p) {
   p->merge_max_row_gap = 40; p->merge_back_rows = 5; p->merge_chi2_max = 50.0f;
   p->tube_radius = 1.5f; p->inv_pt_protect = 20.0f;
   p->leg_min_sinphi = 0.5f; p->leg_chi2_max = 50.0f; p->leg_max_sectors = 4; p->leg_max_row_diff = 12;
+  p->leg_max_centre_dist = 10.0f;
 }
 
 int orcRun(const orcGeometry* g, const orcParams* p, int64_t n, const uint32_t* off, const float* y, const float* z,

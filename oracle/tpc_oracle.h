@@ -44,6 +44,7 @@ typedef struct {
   float tube_radius, inv_pt_protect;            /* O8: 1.5 cm, 20 c/GeV (pT = 50 MeV/c) */
   float leg_min_sinphi, leg_chi2_max;           /* O10: 0.5, 50 */
   int32_t leg_max_sectors, leg_max_row_diff;    /* O10: 4, 12 */
+  float leg_max_centre_dist;                    /* O10: 10 cm */
 } orcParams;
 
 typedef struct orcResult orcResult;

@@ -58,7 +58,8 @@ struct Workspace {
   float* mg_chi_b;
   unsigned long long* mg_key_a;
   unsigned long long* fl_key;      // [N] bids of the cluster flags
-  uint32_t *lg_start, *lg_fill, *lg_list;   // leg pairs: leg ends bucketed by (sector, last row)
+  uint32_t *lg_start, *lg_fill, *lg_list;   // leg pairs: leg ends bucketed by (sector, sign, last row, dip bin)
+  uint32_t *lg_maxv, *lg_tiles;             // largest dip variance per (sector, sign, row); tile sums of the bucket scan
   int32_t* lg_best;
   float* lg_chi;
   size_t bytes;
@@ -180,8 +181,11 @@ Workspace layout(const tpcHandle* h, int64_t N, int64_t capT, char* base) {
   w.mg_chi_b = (float*)take(4 * (size_t)Tn);
   w.mg_key_a = (unsigned long long*)take(8 * (size_t)Tn);
   w.fl_key = (unsigned long long*)take(8 * (size_t)Nn);
-  w.lg_start = (uint32_t*)take(4 * (size_t)(nb + 1));
-  w.lg_fill = (uint32_t*)take(4 * (size_t)(nb + 1));
+  const size_t lgb = (int64_t)nb * 2 * LEG_BINS < (1ll << 31) ? (size_t)nb * 2 * LEG_BINS + 1 : 1;   // else: leg pairs refused
+  w.lg_start = (uint32_t*)take(4 * lgb);
+  w.lg_fill = (uint32_t*)take(4 * lgb);
+  w.lg_maxv = (uint32_t*)take(4 * (size_t)nb * 2);
+  w.lg_tiles = (uint32_t*)take(4 * (size_t)(ceilDiv((int64_t)lgb, SCAN_TILE) + 2));
   w.lg_list = (uint32_t*)take(4 * (size_t)Tn);
   w.lg_best = (int32_t*)take(4 * (size_t)Tn);
   w.lg_chi = (float*)take(4 * (size_t)Tn);
@@ -342,6 +346,7 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   if (n_mg == 4 && (int64_t)h->P.n_buckets * MG_NYB * MG_NZB >= (1ll << 31)) return TPC_ERR_INVALID_ARG;   // bucket ids are 32-bit
   const int n_lg = (out->trk_leg_partner != nullptr) + (out->trk_leg_chi2 != nullptr);
   if ((n_lg != 0 && n_lg != 2) || (n_lg == 2 && n_rf != 8)) return TPC_ERR_INVALID_ARG;   // the leg pairs need the refit
+  if (n_lg == 2 && (int64_t)h->P.n_buckets * 2 * LEG_BINS >= (1ll << 31)) return TPC_ERR_INVALID_ARG;   // bucket ids are 32-bit
   if (out->cl_qcode && N > 0 && !in->q) return TPC_ERR_INVALID_ARG;                      // the charge code needs the charges
   const int n_fl = (out->cl_flags != nullptr) + (out->cl_owner != nullptr);
   if ((n_fl != 0 && n_fl != 2) || (n_fl == 2 && n_rf != 8)) return TPC_ERR_INVALID_ARG;   // so do the cluster flags
@@ -503,12 +508,20 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
         lp.cb[i] = (float)cos(-alpha); lp.sb[i] = (float)sin(-alpha);
       }
     const unsigned gK = (unsigned)ceilDiv(nk, 256);
-    TPC_CUDA(h, cudaMemsetAsync(w.lg_start, 0, 4 * (size_t)(nb + 1), st)); ++L;
-    TPC_CUDA(h, cudaMemsetAsync(w.lg_fill, 0, 4 * (size_t)(nb + 1), st)); ++L;
-    legCount<<<gK, 256, 0, st>>>(li, lo, P, lp, w.lg_start, w.lg_best, cnt); ++L;
-    scanArrayInPlace<uint32_t><<<1, 1024, 0, st>>>(w.lg_start, (int64_t)nb + 1, nullptr); ++L;
+    const size_t lgb = (size_t)nb * 2 * LEG_BINS + 1;
+    TPC_CUDA(h, cudaMemsetAsync(w.lg_start, 0, 4 * lgb, st)); ++L;
+    TPC_CUDA(h, cudaMemsetAsync(w.lg_fill, 0, 4 * lgb, st)); ++L;
+    TPC_CUDA(h, cudaMemsetAsync(w.lg_maxv, 0, 4 * (size_t)nb * 2, st)); ++L;
+    legCount<<<gK, 256, 0, st>>>(li, lo, P, lp, w.lg_start, w.lg_maxv, w.lg_best, cnt); ++L;
+    {   // exclusive scan of the bucket counts; the closing sentinel lands on the last (spare) entry
+      const int64_t nscan = (int64_t)lgb - 1;
+      const unsigned tiles = (unsigned)ceilDiv(nscan, SCAN_TILE);
+      scanTileSums<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.lg_start, cnt + CNT_INF, nscan, w.lg_tiles); ++L;
+      scanTileOffsets<uint32_t><<<1, 1024, 0, st>>>(w.lg_tiles, cnt + CNT_INF, nscan, nullptr); ++L;
+      scanApply<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.lg_start, w.lg_start, cnt + CNT_INF, nscan, w.lg_tiles); ++L;
+    }
     legFill<<<gK, 256, 0, st>>>(li, P, lp, w.lg_start, w.lg_fill, w.lg_list, cnt); ++L;
-    legMatch<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(li, P, lp, w.lg_start, w.lg_list, w.lg_best, w.lg_chi, cnt); ++L;
+    legMatch<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(li, P, lp, w.lg_start, w.lg_maxv, w.lg_list, w.lg_best, w.lg_chi, cnt); ++L;
     legLink<<<gK, 256, 0, st>>>(li, lo, w.lg_best, w.lg_chi, cnt); ++L;
   }
   stage(16);

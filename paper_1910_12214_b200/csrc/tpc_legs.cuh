@@ -7,10 +7,13 @@
 // and propagated (eight steps, R43) to the plane of the other, which is rotated by -alpha and mirrored; diagonal chi2.
 // partner(k) = the compared end of minimal (chi2, id), kept when reciprocal.
 //
-// Organisation: the leg ends are bucketed by (sector, last row); one thread per leg end visits the buckets of the
-// sectors it moves towards and of the rows around its own last row.  Every pair is evaluated by both of its ends with
-// the same operands in the same order, so both see the same chi2 and no atomics are needed; a last pass keeps the
-// reciprocal choices.
+// Organisation: the leg ends are bucketed by (sector, sign of sin phi, last row, bin of the dip t); one thread per leg
+// end visits the buckets of the sectors it moves towards, of the opposite inclination, of the rows around its own last
+// row and of the dip bins that can hold a partner: the dip term of the chi2 needs no transport (see legMatch), the terms
+// are non-negative, and the window uses the largest dip variance of the (sector, sign, row) plus rounding slack, so it
+// is a superset of every admissible partner -- no result changes (same argument as R3 and as the merger's bins).
+// Every pair is evaluated by both of its ends with the same operands in the same order, so both see the same chi2 and
+// no atomics are needed; a last pass keeps the reciprocal choices.
 #pragma once
 #include "tpc_kalman.cuh"
 #include "tpc_merge.cuh"
@@ -19,6 +22,15 @@ namespace tpc {
 
 constexpr int LEG_MAX_SECTORS = 8;          // d = 9 and d = -9 would be the same sector
 constexpr int LEG_ANGLES = 2 * LEG_MAX_SECTORS + 2;
+constexpr int LEG_NTB = 64;                 // dip bins over [-LEG_TMAX, LEG_TMAX] (clamped outside)
+constexpr float LEG_TMAX = 2.0f;
+constexpr float LEG_VWIDE = 2e-5f;          // ends with a larger dip variance go to one extra bin that is always visited,
+constexpr int LEG_BINS = LEG_NTB + 1;       // so that a few badly measured dips do not widen everybody's window
+
+// (sector, sign, row) index and the dip bin inside it
+__device__ __forceinline__ int legRowKey(int sector, bool positive, int row, int R) { return (sector * 2 + (positive ? 1 : 0)) * R + row; }
+__device__ __forceinline__ int legDipBin(float t) { return cellCoord(t, -LEG_TMAX, (float)LEG_NTB / (2.0f * LEG_TMAX), LEG_NTB); }
+__device__ __forceinline__ int legBin(float t, float var_t) { return var_t <= LEG_VWIDE ? legDipBin(t) : LEG_NTB; }
 
 struct LegParams {
   float min_sinphi, chi2_max;
@@ -40,14 +52,20 @@ __device__ __forceinline__ bool legIsEnd(const LegIn& in, int64_t k, const LegPa
   return in.status[k] == 1 && !(fabsf(in.par_out[2 * in.cap + k]) < L.min_sinphi);
 }
 
-// per track: clear the outputs, count the leg ends per (sector, last row)
+// per track: clear the outputs, count the leg ends per bucket, largest dip variance per (sector, sign, row)
 __global__ void __launch_bounds__(256) legCount(LegIn in, LegOut out, DevParams P, LegParams L, uint32_t* __restrict__ bucket_cnt,
-                                                int32_t* __restrict__ best, const int64_t* __restrict__ cnt) {
+                                                uint32_t* __restrict__ max_var, int32_t* __restrict__ best,
+                                                const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= cnt[CNT_N_TRACKS] || k >= in.cap) return;
   out.partner[k] = -1; out.chi2[k] = 0.0f; best[k] = -1;
-  if (legIsEnd(in, k, L)) atomicAdd(bucket_cnt + in.sector[k] * P.n_rows + in.last_row[k], 1u);
+  if (legIsEnd(in, k, L)) {
+    const int sr = legRowKey(in.sector[k], in.par_out[2 * in.cap + k] > 0.0f, in.last_row[k], P.n_rows);
+    const float vt = in.cov_out[9 * in.cap + k];
+    atomicAdd(bucket_cnt + sr * LEG_BINS + legBin(in.par_out[3 * in.cap + k], vt), 1u);
+    if (vt <= LEG_VWIDE) atomicMax(max_var + sr, __float_as_uint(vt));     // positive floats order like their bit patterns
+  }
 }
 
 // per leg end: its slot in the bucket list (the order inside a bucket is arbitrary: the argmin breaks ties by id)
@@ -57,7 +75,8 @@ __global__ void __launch_bounds__(256) legFill(LegIn in, DevParams P, LegParams 
   if (cnt[CNT_ERROR] != 0) return;
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= cnt[CNT_N_TRACKS] || k >= in.cap || !legIsEnd(in, k, L)) return;
-  const int b = in.sector[k] * P.n_rows + in.last_row[k];
+  const int b = legRowKey(in.sector[k], in.par_out[2 * in.cap + k] > 0.0f, in.last_row[k], P.n_rows) * LEG_BINS +
+                legBin(in.par_out[3 * in.cap + k], in.cov_out[9 * in.cap + k]);
   list[bucket_start[b] + atomicAdd(bucket_fill + b, 1u)] = (uint32_t)k;
 }
 
@@ -92,39 +111,72 @@ __device__ __forceinline__ bool legMatchPair(KFState A, KFState B, int d, const 
   return true;
 }
 
-// one thread per leg end a: the compared end of minimal (chi2, id)
+// one thread per leg end a: the compared end of minimal (chi2, id).
+// The candidates of a lane come in runs (one per sector and row); almost all of them fall to the cheap tests, and the
+// few that are left cost a LegMatch each (two Rotates, eight Propagates).  So the lanes of a warp look for their next
+// surviving candidate separately and then evaluate those together: the expensive part runs converged.
 __global__ void __launch_bounds__(128) legMatch(LegIn in, DevParams P, LegParams L, const uint32_t* __restrict__ bucket_start,
-                                                const uint32_t* __restrict__ list, int32_t* __restrict__ best,
-                                                float* __restrict__ best_chi, const int64_t* __restrict__ cnt) {
+                                                const uint32_t* __restrict__ max_var, const uint32_t* __restrict__ list,
+                                                int32_t* __restrict__ best, float* __restrict__ best_chi,
+                                                const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
   const int64_t a = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (a >= cnt[CNT_N_TRACKS] || a >= in.cap || !legIsEnd(in, a, L)) return;
+  const bool live = a < cnt[CNT_N_TRACKS] && a < in.cap && legIsEnd(in, live_guard(a, in.cap), L);
   const int64_t cap = in.cap;
   const int R = P.n_rows;
-  const KFState A0 = mergeLoad(a, cap, in.x_out, in.par_out, in.cov_out);
-  const int sec = in.sector[a], la = in.last_row[a];
+  KFState A0{};
+  if (live) A0 = mergeLoad(a, cap, in.x_out, in.par_out, in.cov_out);
+  const int sec = live ? in.sector[a] : 0, la = live ? in.last_row[a] : 0;
   const int sg = A0.s > 0.0f ? 1 : -1;
   const int side = sec / 18, j = sec - side * 18;
   const int r_lo = max(0, la - L.max_row_diff), r_hi = min(R - 1, la + L.max_row_diff);
+  const int n_rows = r_hi - r_lo + 1;
+  const int n_runs = live ? ((P.n_sectors == 36 ? L.max_sectors : 0) + 1) * n_rows : 0;
   int32_t bb = -1;
   float bchi = 0.0f;
-  const int dmax = P.n_sectors == 36 ? L.max_sectors : 0;
-  for (int dd = 0; dd <= dmax; ++dd) {
-    const int d = sg * dd;                                   // a moves towards the sectors on this side of it
-    const int sb = dd == 0 ? sec : side * 18 + (j + d + 18) % 18;
-    const uint32_t* bs = bucket_start + sb * R;
-    for (uint32_t i = bs[r_lo]; i < bs[r_hi + 1]; ++i) {       // the buckets of consecutive rows are contiguous
-      const int64_t b = list[i];
-      if (b == a) continue;
-      if (!(A0.s * in.par_out[2 * cap + b] < 0.0f)) continue;  // opposite inclinations
+  int m = -1, d = 0;                              // current run and its sector distance
+  uint32_t pos = 0, end = 0, wpos = 0, wend = 0;  // what is left of the run: binned ends, ends with a wide dip variance
+  for (;;) {
+    int64_t b = -1;
+    while (b < 0) {
+      uint32_t i;
+      if (pos < end) i = pos++;
+      else if (wpos < wend) i = wpos++;
+      else {
+        if (++m >= n_runs) break;
+        const int dd = m / n_rows, r = r_lo + (m - dd * n_rows);
+        d = sg * dd;                              // a moves towards the sectors on this side of it
+        const int sb = dd == 0 ? sec : side * 18 + (j + d + 18) % 18;
+        const int sr = legRowKey(sb, sg < 0, r, R);            // the other inclination
+        const uint32_t* bs = bucket_start + sr * LEG_BINS;
+        // dip bins that can hold a partner: |t_a + t_b| <= sqrt(chi2_max * (C33_a + max C33_b)), with slack; a window
+        // that is not >= 0 means no positive denominator is possible among the binned ends
+        const float w = sqrtf(L.chi2_max * (A0.c33 + __uint_as_float(max_var[sr]))) * 1.0001f + 1e-6f;
+        const bool any = w >= 0.0f;
+        pos = any ? bs[legDipBin(-A0.t - w)] : 0u; end = any ? bs[legDipBin(-A0.t + w) + 1] : 0u;
+        wpos = bs[LEG_NTB]; wend = bs[LEG_BINS];
+        continue;
+      }
+      const int64_t c = list[i];
+      if (c == a) continue;
+      if (!(A0.s * in.par_out[2 * cap + c] < 0.0f)) continue;  // opposite inclinations (sin phi = 0 is in the negative key)
+      // The dip and curvature terms of the chi2 need no transport: Rotate and Propagate leave t, q, C33 and C44 as they
+      // are and Mirror only changes the signs, so these are the very values LegMatch adds at the end; the terms are
+      // non-negative and rounding is monotone, so one of them above the cut means the sum is above it.
+      const float dt = A0.t + in.par_out[3 * cap + c], dq = A0.q + in.par_out[4 * cap + c];
+      const float t3 = (dt * dt) / (A0.c33 + in.cov_out[9 * cap + c]), t4 = (dq * dq) / (A0.c44 + in.cov_out[14 * cap + c]);
+      if (t3 > L.chi2_max || t4 > L.chi2_max) continue;
+      b = c;
+    }
+    if (!__any_sync(0xffffffffu, b >= 0)) break;
+    if (b >= 0) {
       const KFState B0 = mergeLoad(b, cap, in.x_out, in.par_out, in.cov_out);
       float c2;
       const bool ok = a < b ? legMatchPair(A0, B0, d, P, L, c2) : legMatchPair(B0, A0, -d, P, L, c2);
-      if (!ok) continue;
-      if (bb < 0 || c2 < bchi || (c2 == bchi && (int32_t)b < bb)) { bb = (int32_t)b; bchi = c2; }
+      if (ok && (bb < 0 || c2 < bchi || (c2 == bchi && (int32_t)b < bb))) { bb = (int32_t)b; bchi = c2; }
     }
   }
-  best[a] = bb; best_chi[a] = bchi;
+  if (live) { best[a] = bb; best_chi[a] = bchi; }
 }
 
 // a pair is kept when each is the other's choice (R42)

@@ -89,7 +89,7 @@ def test_leg_match_of_the_two_sides_of_an_exact_turn(h, d):
     cov = np.zeros(15)
     for i in range(5):
         cov[tri(i, i)] = 1e-4
-    found = 0
+    found = centre_cut_seen = 0
     # off_deg: where the circle starts, relative to sector sa
     for off_deg, xa, xb in itertools.product(range(-90, 91, 15), (100.0, 110.0, 120.0, 125.0), (100.0, 112.0, 124.0)):
         phi0 = sector_alpha(sa) + math.radians(off_deg)
@@ -123,12 +123,20 @@ def test_leg_match_of_the_two_sides_of_an_exact_turn(h, d):
         cy = cov.copy(); cy[tri(3, 3)] = 0.0                          # no dip variance: C11_a' = C11_a + jz^2 C00 >= 1e-4
         ok6, c6 = orc.leg_match(a, cy, dsec, b3, cov, BZ, p, fp64=True)
         assert ok6 and c6 >= c4
+        # R44: the circle centres of the two sides must be close: b moved sideways by 3 cm moves its centre by 3 cm
+        b4 = b.copy(); b4[1] += 3.0
+        verdict = {}
+        for cut in (2.9, 3.1, 1e9):
+            p4 = orc.default_params(); p4.leg_chi2_max = 1e30; p4.leg_max_centre_dist = cut
+            verdict[cut] = orc.leg_match(a, cov, dsec, b4, cov, BZ, p4, fp64=True)[0]
+        assert not verdict[2.9] and verdict[3.1] == verdict[1e9]
+        centre_cut_seen += verdict[3.1]
         # wrong charge or wrong dip on one side (what a missing sign in Mirror would look like)
         for idx in (4, 5):
             bw = b.copy(); bw[idx] = -bw[idx]
             okw, cw = orc.leg_match(a, cov, dsec, bw, cov, BZ, p, fp64=True)
             assert (not okw) or cw > 100.0
-    assert found >= 2
+    assert found >= 2 and centre_cut_seen >= 1
 
 
 def _legs_numpy(ev, res, p):
@@ -140,8 +148,20 @@ def _legs_numpy(ev, res, p):
     def outer(k):
         return np.concatenate([[res.rf_x_out[k]], res.rf_par_out[k]]), res.rf_cov_out[k].copy()
 
+    def centre(st):                                  # circle centre of a state in its own frame, binary32 step by step
+        x, y, s, q = f32(st[0]), f32(st[1]), f32(st[3]), f32(st[5])
+        k = q * f32(KAPPA * ev.bz_tesla)
+        return x - s / k, y + np.sqrt(f32(1) - s * s) / k
+
     def chi2_of(a, b, d):
         (A, CA), (B, CB) = outer(a), outer(b)
+        with np.errstate(all="ignore"):
+            (xa, ya), (xb, yb) = centre(A), centre(B)
+            cd, sd = f32(math.cos(d * 2.0 * 0.17453292519943295)), f32(math.sin(d * 2.0 * 0.17453292519943295))
+            ex, ey = (xb * cd - yb * sd) - xa, (xb * sd + yb * cd) - ya
+            md = f32(p.leg_max_centre_dist)
+            if not ex * ex + ey * ey <= md * md:
+                return None
         sg = 1.0 if A[3] > 0 else -1.0
         alpha = d * math.radians(10.0) + sg * A90
         oka, A, CA = orc.rotate(A, CA, alpha, ev.bz_tesla, msp, fp64=False)
@@ -193,13 +213,16 @@ def _legs_numpy(ev, res, p):
     return partner, chi2
 
 
-@pytest.mark.parametrize("scale,dead", [(0.05, ()), (0.04, (30, 31, 90))])
-def test_legs_equal_the_numpy_restatement(scale, dead):
+@pytest.mark.parametrize("scale,dead,centre,least", [(0.05, (), 10.0, 20), (0.04, (30, 31, 90), 10.0, 20), (0.05, (), 0.7, 4)])
+def test_legs_equal_the_numpy_restatement(scale, dead, centre, least):
     ev = datagen.make_event(2, scale=scale, dead_rows=dead)
     p = orc.default_params()
+    p.leg_max_centre_dist = centre
     res = orc.run(ev, p, legs=True)
     partner, chi2 = _legs_numpy(ev, res, p)
-    assert (partner >= 0).sum() >= 20
+    assert (partner >= 0).sum() >= least
+    if centre < 1.0:                                 # the tight cut really bites: fewer pairs than with the default
+        assert (partner >= 0).sum() < 0.8 * (orc.run(ev, legs=True).lg_partner >= 0).sum()
     assert np.array_equal(partner, res.lg_partner)
     assert np.array_equal(chi2, res.lg_chi2)
 
