@@ -84,6 +84,7 @@ typedef struct {
   float leg_chi2_max;           /* 50         O10: cut on the diagonal chi2 of the two sides of a turn */
   int32_t leg_max_sectors;      /* 4          O10: the two ends of a turn are at most this many sectors apart (0..8) */
   int32_t leg_max_row_diff;     /* 12         O10: and their last rows at most this many rows */
+  float leg_max_centre_dist;    /* 10         O10: and the centres of their circles at most this far apart, cm */
 } tpcParams;
 
 /* Input clusters: CSR by (sector,row), fp32 SoA (single-precision cluster properties). */

@@ -59,6 +59,7 @@ struct Workspace {
   unsigned long long* mg_key_a;
   unsigned long long* fl_key;      // [N] bids of the cluster flags
   uint32_t *lg_start, *lg_fill, *lg_list;   // leg pairs: leg ends bucketed by (sector, sign, last row, dip bin)
+  float4* lg_rec;                           // [capT] dip, curvature and their variances of the leg ends, in list order
   uint32_t *lg_maxv, *lg_tiles;             // largest dip variance per (sector, sign, row); tile sums of the bucket scan
   int32_t* lg_best;
   float* lg_chi;
@@ -187,6 +188,7 @@ Workspace layout(const tpcHandle* h, int64_t N, int64_t capT, char* base) {
   w.lg_maxv = (uint32_t*)take(4 * (size_t)nb * 2);
   w.lg_tiles = (uint32_t*)take(4 * (size_t)(ceilDiv((int64_t)lgb, SCAN_TILE) + 2));
   w.lg_list = (uint32_t*)take(4 * (size_t)Tn);
+  w.lg_rec = (float4*)take(16 * (size_t)Tn);
   w.lg_best = (int32_t*)take(4 * (size_t)Tn);
   w.lg_chi = (float*)take(4 * (size_t)Tn);
   w.bytes = o;
@@ -210,6 +212,7 @@ int tpcDefaultParams(tpcParams* p) {
   p->merge_max_row_gap = 40; p->merge_back_rows = 5; p->merge_chi2_max = 50.0f;
   p->tube_radius = 1.5f; p->inv_pt_protect = 20.0f; p->charge_trunc_bits = 4;
   p->leg_min_sinphi = 0.5f; p->leg_chi2_max = 50.0f; p->leg_max_sectors = 4; p->leg_max_row_diff = 12;
+  p->leg_max_centre_dist = 10.0f;
   return TPC_OK;
 }
 
@@ -498,6 +501,7 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
     LegParams lp{};
     lp.min_sinphi = h->params.leg_min_sinphi; lp.chi2_max = h->params.leg_chi2_max;
     lp.max_sectors = h->params.leg_max_sectors; lp.max_row_diff = h->params.leg_max_row_diff;
+    lp.max_centre_dist = h->params.leg_max_centre_dist;
     for (int d = -LEG_MAX_SECTORS; d <= LEG_MAX_SECTORS; ++d)
       for (int sg = -1; sg <= 1; sg += 2) {
         if (d * sg < 0) continue;                  // a moves towards b's sector
@@ -507,6 +511,10 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
         lp.ca[i] = (float)cos(alpha); lp.sa[i] = (float)sin(alpha);
         lp.cb[i] = (float)cos(-alpha); lp.sb[i] = (float)sin(-alpha);
       }
+    for (int d = -LEG_MAX_SECTORS; d <= LEG_MAX_SECTORS; ++d) {
+      const double a10 = 0.17453292519943295;
+      lp.cd[d + LEG_MAX_SECTORS] = (float)cos((double)d * (2.0 * a10)); lp.sd[d + LEG_MAX_SECTORS] = (float)sin((double)d * (2.0 * a10));
+    }
     const unsigned gK = (unsigned)ceilDiv(nk, 256);
     const size_t lgb = (size_t)nb * 2 * LEG_BINS + 1;
     TPC_CUDA(h, cudaMemsetAsync(w.lg_start, 0, 4 * lgb, st)); ++L;
@@ -520,8 +528,9 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
       scanTileOffsets<uint32_t><<<1, 1024, 0, st>>>(w.lg_tiles, cnt + CNT_INF, nscan, nullptr); ++L;
       scanApply<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.lg_start, w.lg_start, cnt + CNT_INF, nscan, w.lg_tiles); ++L;
     }
-    legFill<<<gK, 256, 0, st>>>(li, P, lp, w.lg_start, w.lg_fill, w.lg_list, cnt); ++L;
-    legMatch<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(li, P, lp, w.lg_start, w.lg_maxv, w.lg_list, w.lg_best, w.lg_chi, cnt); ++L;
+    legFill<<<gK, 256, 0, st>>>(li, P, lp, w.lg_start, w.lg_fill, w.lg_list, w.lg_rec, cnt); ++L;
+    legMatch<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(li, P, lp, w.lg_start, w.lg_maxv, w.lg_list, w.lg_rec, w.lg_best,
+                                                         w.lg_chi, cnt); ++L;
     legLink<<<gK, 256, 0, st>>>(li, lo, w.lg_best, w.lg_chi, cnt); ++L;
   }
   stage(16);

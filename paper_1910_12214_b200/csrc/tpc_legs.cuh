@@ -33,10 +33,11 @@ __device__ __forceinline__ int legDipBin(float t) { return cellCoord(t, -LEG_TMA
 __device__ __forceinline__ int legBin(float t, float var_t) { return var_t <= LEG_VWIDE ? legDipBin(t) : LEG_NTB; }
 
 struct LegParams {
-  float min_sinphi, chi2_max;
+  float min_sinphi, chi2_max, max_centre_dist;
   int32_t max_sectors, max_row_diff;
   // (float)cos / sin of alpha = d*10 + sg*90 degrees and of -alpha, index d + LEG_MAX_SECTORS + (sg > 0)
   float ca[LEG_ANGLES], sa[LEG_ANGLES], cb[LEG_ANGLES], sb[LEG_ANGLES];
+  float cd[2 * LEG_MAX_SECTORS + 1], sd[2 * LEG_MAX_SECTORS + 1];   // (float)cos / sin of d*20 degrees, index d + LEG_MAX_SECTORS
 };
 struct LegIn {
   int64_t cap;
@@ -71,13 +72,16 @@ __global__ void __launch_bounds__(256) legCount(LegIn in, LegOut out, DevParams 
 // per leg end: its slot in the bucket list (the order inside a bucket is arbitrary: the argmin breaks ties by id)
 __global__ void __launch_bounds__(256) legFill(LegIn in, DevParams P, LegParams L, const uint32_t* __restrict__ bucket_start,
                                                uint32_t* __restrict__ bucket_fill, uint32_t* __restrict__ list,
-                                               const int64_t* __restrict__ cnt) {
+                                               float4* __restrict__ rec, const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= cnt[CNT_N_TRACKS] || k >= in.cap || !legIsEnd(in, k, L)) return;
   const int b = legRowKey(in.sector[k], in.par_out[2 * in.cap + k] > 0.0f, in.last_row[k], P.n_rows) * LEG_BINS +
                 legBin(in.par_out[3 * in.cap + k], in.cov_out[9 * in.cap + k]);
-  list[bucket_start[b] + atomicAdd(bucket_fill + b, 1u)] = (uint32_t)k;
+  const uint32_t slot = bucket_start[b] + atomicAdd(bucket_fill + b, 1u);
+  list[slot] = (uint32_t)k;
+  // what the cheap tests of legMatch read, in list order: the candidates of a lane are a few contiguous runs
+  rec[slot] = make_float4(in.par_out[3 * in.cap + k], in.par_out[4 * in.cap + k], in.cov_out[9 * in.cap + k], in.cov_out[14 * in.cap + k]);
 }
 
 // O10 Mirror: frame turned by 180 degrees, helix walked backwards; C <- J C J^T, J = diag(-1, +1, +1, -1, -1)
@@ -86,7 +90,7 @@ __device__ __forceinline__ void kfMirror(KFState& S) {
   S.c10 = -S.c10; S.c20 = -S.c20; S.c31 = -S.c31; S.c32 = -S.c32; S.c41 = -S.c41; S.c42 = -S.c42;
 }
 
-// O10 LegMatch(a, b, d): a = the lower id; false when refused
+// O10 LegMatch(a, b, d) after its first step (legCentresClose): a = the lower id; false when refused
 __device__ __forceinline__ bool legMatchPair(KFState A, KFState B, int d, const DevParams& P, const LegParams& L, float& chi2) {
   const int ia = d + LEG_MAX_SECTORS + (A.s > 0.0f ? 1 : 0);
   if (!kfRotate(A, L.ca[ia], L.sa[ia], P)) return false;
@@ -111,72 +115,75 @@ __device__ __forceinline__ bool legMatchPair(KFState A, KFState B, int d, const 
   return true;
 }
 
-// one thread per leg end a: the compared end of minimal (chi2, id).
-// The candidates of a lane come in runs (one per sector and row); almost all of them fall to the cheap tests, and the
-// few that are left cost a LegMatch each (two Rotates, eight Propagates).  So the lanes of a warp look for their next
-// surviving candidate separately and then evaluate those together: the expensive part runs converged.
+// R44, the first step of LegMatch(a, b, d): the circle centres of the two outer states, each in its own frame (b's is
+// turned by d * 20 degrees), lie within max_centre_dist
+__device__ __forceinline__ bool legCentresClose(float xa, float ya, float sa, float qa, float xb, float yb, float sb, float qb,
+                                                int d, const DevParams& P, const LegParams& L) {
+  const float ka = qa * P.b, kb = qb * P.b;
+  const float xca = xa - sa / ka, yca = ya + sqrtf(1.0f - sa * sa) / ka;
+  const float xcb = xb - sb / kb, ycb = yb + sqrtf(1.0f - sb * sb) / kb;
+  const float cd = L.cd[d + LEG_MAX_SECTORS], sd = L.sd[d + LEG_MAX_SECTORS];
+  const float ex = (xcb * cd - ycb * sd) - xca, ey = (xcb * sd + ycb * cd) - yca;
+  return ex * ex + ey * ey <= L.max_centre_dist * L.max_centre_dist;
+}
+
+// one thread per leg end a: the compared end of minimal (chi2, id)
 __global__ void __launch_bounds__(128) legMatch(LegIn in, DevParams P, LegParams L, const uint32_t* __restrict__ bucket_start,
                                                 const uint32_t* __restrict__ max_var, const uint32_t* __restrict__ list,
-                                                int32_t* __restrict__ best, float* __restrict__ best_chi,
+                                                const float4* __restrict__ rec, int32_t* __restrict__ best,
+                                                float* __restrict__ best_chi,
                                                 const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
   const int64_t a = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const bool live = a < cnt[CNT_N_TRACKS] && a < in.cap && legIsEnd(in, live_guard(a, in.cap), L);
+  if (a >= cnt[CNT_N_TRACKS] || a >= in.cap || !legIsEnd(in, a, L)) return;
   const int64_t cap = in.cap;
   const int R = P.n_rows;
-  KFState A0{};
-  if (live) A0 = mergeLoad(a, cap, in.x_out, in.par_out, in.cov_out);
-  const int sec = live ? in.sector[a] : 0, la = live ? in.last_row[a] : 0;
+  const KFState A0 = mergeLoad(a, cap, in.x_out, in.par_out, in.cov_out);
+  const int sec = in.sector[a], la = in.last_row[a];
   const int sg = A0.s > 0.0f ? 1 : -1;
   const int side = sec / 18, j = sec - side * 18;
   const int r_lo = max(0, la - L.max_row_diff), r_hi = min(R - 1, la + L.max_row_diff);
-  const int n_rows = r_hi - r_lo + 1;
-  const int n_runs = live ? ((P.n_sectors == 36 ? L.max_sectors : 0) + 1) * n_rows : 0;
   int32_t bb = -1;
   float bchi = 0.0f;
-  int m = -1, d = 0;                              // current run and its sector distance
-  uint32_t pos = 0, end = 0, wpos = 0, wend = 0;  // what is left of the run: binned ends, ends with a wide dip variance
-  for (;;) {
-    int64_t b = -1;
-    while (b < 0) {
-      uint32_t i;
-      if (pos < end) i = pos++;
-      else if (wpos < wend) i = wpos++;
-      else {
-        if (++m >= n_runs) break;
-        const int dd = m / n_rows, r = r_lo + (m - dd * n_rows);
-        d = sg * dd;                              // a moves towards the sectors on this side of it
-        const int sb = dd == 0 ? sec : side * 18 + (j + d + 18) % 18;
-        const int sr = legRowKey(sb, sg < 0, r, R);            // the other inclination
-        const uint32_t* bs = bucket_start + sr * LEG_BINS;
-        // dip bins that can hold a partner: |t_a + t_b| <= sqrt(chi2_max * (C33_a + max C33_b)), with slack; a window
-        // that is not >= 0 means no positive denominator is possible among the binned ends
-        const float w = sqrtf(L.chi2_max * (A0.c33 + __uint_as_float(max_var[sr]))) * 1.0001f + 1e-6f;
-        const bool any = w >= 0.0f;
-        pos = any ? bs[legDipBin(-A0.t - w)] : 0u; end = any ? bs[legDipBin(-A0.t + w) + 1] : 0u;
-        wpos = bs[LEG_NTB]; wend = bs[LEG_BINS];
-        continue;
+  const int dmax = P.n_sectors == 36 ? L.max_sectors : 0;
+  for (int dd = 0; dd <= dmax; ++dd) {
+    const int d = sg * dd;                                     // a moves towards the sectors on this side of it
+    const int sb = dd == 0 ? sec : side * 18 + (j + d + 18) % 18;
+    for (int r = r_lo; r <= r_hi; ++r) {
+      const int sr = legRowKey(sb, sg < 0, r, R);              // the other inclination
+      const uint32_t* bs = bucket_start + sr * LEG_BINS;
+      // dip bins that can hold a partner: |t_a + t_b| <= sqrt(chi2_max * (C33_a + max C33_b)), with slack; a window
+      // that is not >= 0 means no positive denominator is possible among the binned ends
+      const float w = sqrtf(L.chi2_max * (A0.c33 + __uint_as_float(max_var[sr]))) * 1.0001f + 1e-6f;
+      const bool any = w >= 0.0f;
+      const uint32_t j0 = bs[LEG_NTB], j1 = bs[LEG_BINS];      // the ends with a wide dip variance: always visited
+      const uint32_t i0 = any ? bs[legDipBin(-A0.t - w)] : j0, i1 = any ? bs[legDipBin(-A0.t + w) + 1] : j0;
+      for (uint32_t ii = i0; ii < i1 + (j1 - j0); ++ii) {
+        const uint32_t i = ii < i1 ? ii : j0 + (ii - i1);
+        // The dip and curvature terms of the chi2 need no transport: Rotate and Propagate leave t, q, C33 and C44 as
+        // they are and Mirror only changes the signs, so these are the very values LegMatch adds at the end; the terms
+        // are non-negative and rounding is monotone, so one of them above the cut means the sum is above it.
+        const float4 rc = __ldg(rec + i);                      // t, q, C33, C44 of the candidate
+        const float q_b = rc.y;
+        const float dt = A0.t + rc.x, dq = A0.q + q_b;
+        const float t3 = (dt * dt) / (A0.c33 + rc.z), t4 = (dq * dq) / (A0.c44 + rc.w);
+        if (t3 > L.chi2_max || t4 > L.chi2_max) continue;
+        const int64_t b = list[i];
+        if (b == a) continue;
+        const float s_b = in.par_out[2 * cap + b];
+        if (!(A0.s * s_b < 0.0f)) continue;                    // opposite inclinations (sin phi = 0 is in the negative key)
+        const float x_b = in.x_out[b], y_b = in.par_out[b];
+        if (!(a < b ? legCentresClose(A0.x, A0.y, A0.s, A0.q, x_b, y_b, s_b, q_b, d, P, L)
+                    : legCentresClose(x_b, y_b, s_b, q_b, A0.x, A0.y, A0.s, A0.q, -d, P, L))) continue;
+        const KFState B0 = mergeLoad(b, cap, in.x_out, in.par_out, in.cov_out);
+        float c2;
+        const bool ok = a < b ? legMatchPair(A0, B0, d, P, L, c2) : legMatchPair(B0, A0, -d, P, L, c2);
+        if (!ok) continue;
+        if (bb < 0 || c2 < bchi || (c2 == bchi && (int32_t)b < bb)) { bb = (int32_t)b; bchi = c2; }
       }
-      const int64_t c = list[i];
-      if (c == a) continue;
-      if (!(A0.s * in.par_out[2 * cap + c] < 0.0f)) continue;  // opposite inclinations (sin phi = 0 is in the negative key)
-      // The dip and curvature terms of the chi2 need no transport: Rotate and Propagate leave t, q, C33 and C44 as they
-      // are and Mirror only changes the signs, so these are the very values LegMatch adds at the end; the terms are
-      // non-negative and rounding is monotone, so one of them above the cut means the sum is above it.
-      const float dt = A0.t + in.par_out[3 * cap + c], dq = A0.q + in.par_out[4 * cap + c];
-      const float t3 = (dt * dt) / (A0.c33 + in.cov_out[9 * cap + c]), t4 = (dq * dq) / (A0.c44 + in.cov_out[14 * cap + c]);
-      if (t3 > L.chi2_max || t4 > L.chi2_max) continue;
-      b = c;
-    }
-    if (!__any_sync(0xffffffffu, b >= 0)) break;
-    if (b >= 0) {
-      const KFState B0 = mergeLoad(b, cap, in.x_out, in.par_out, in.cov_out);
-      float c2;
-      const bool ok = a < b ? legMatchPair(A0, B0, d, P, L, c2) : legMatchPair(B0, A0, -d, P, L, c2);
-      if (ok && (bb < 0 || c2 < bchi || (c2 == bchi && (int32_t)b < bb))) { bb = (int32_t)b; bchi = c2; }
     }
   }
-  if (live) { best[a] = bb; best_chi[a] = bchi; }
+  best[a] = bb; best_chi[a] = bchi;
 }
 
 // a pair is kept when each is the other's choice (R42)

@@ -38,7 +38,8 @@ class tpcParams(ctypes.Structure):
                 ("validate_input", c_int32), ("force_wide_keys", c_int32), ("merge_max_row_gap", c_int32),
                 ("merge_back_rows", c_int32), ("merge_chi2_max", c_float), ("tube_radius", c_float),
                 ("inv_pt_protect", c_float), ("charge_trunc_bits", c_int32), ("leg_min_sinphi", c_float),
-                ("leg_chi2_max", c_float), ("leg_max_sectors", c_int32), ("leg_max_row_diff", c_int32)]
+                ("leg_chi2_max", c_float), ("leg_max_sectors", c_int32), ("leg_max_row_diff", c_int32),
+                ("leg_max_centre_dist", c_float)]
 
 
 class tpcClusters(ctypes.Structure):

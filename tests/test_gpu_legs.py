@@ -45,14 +45,15 @@ def test_legs_parity_with_other_cuts_dead_rows_and_the_merger_beside_it():
     ev = datagen.make_event(2, scale=0.1, dead_rows=(30, 31, 90))
     g, o, _ = _both(ev, merge=True)
     assert (o.lg_partner >= 0).sum() > 100
-    _both(ev, leg_min_sinphi=0.2, leg_chi2_max=500.0, leg_max_sectors=8, leg_max_row_diff=40)
+    _both(ev, leg_min_sinphi=0.2, leg_chi2_max=500.0, leg_max_sectors=8, leg_max_row_diff=40, leg_max_centre_dist=60.0)
+    _both(ev, leg_max_centre_dist=0.7)
     _both(ev, leg_min_sinphi=0.8, leg_chi2_max=5.0, leg_max_sectors=0, leg_max_row_diff=0)
     _both(ev, leg_max_sectors=2, max_sinphi=0.9)
 
 
 def test_legs_parity_single_sector_geometry():
     ev = datagen.make_event(0)                     # one sector: only d = 0 is compared
-    g, o, _ = _both(ev, leg_min_sinphi=0.05, leg_chi2_max=1e6, leg_max_row_diff=151)
+    g, o, _ = _both(ev, leg_min_sinphi=0.05, leg_chi2_max=1e6, leg_max_row_diff=151, leg_max_centre_dist=1e4)
     assert g["trk_leg_partner"].shape[0] > 100
 
 
