@@ -50,8 +50,10 @@ struct Workspace {
   int32_t *kept_first, *kept_last;
   unsigned long long* owner_key;
   uint32_t* owner_id;
-  uint32_t *mg_start, *mg_fill, *mg_list;   // merger: tracks bucketed by (sector, first row, z bin, y bin)
-  uint32_t* mg_maxv;         // [2][n_buckets] largest inner variances of a (sector, row)
+  uint32_t *mg_start, *mg_fill, *mg_list;   // merger: tracks bucketed by (sector, first row, dip bin)
+  uint32_t *mg_ostart, *mg_ofill, *mg_order;   // the same buckets over the outer states: the order mergeMatch works in
+  float4* mg_rec;            // [capT] dip, curvature and their variances of the inner states, in list order
+  uint32_t* mg_maxv;         // [n_buckets] largest binned dip variance of a (sector, row)
   uint32_t* mg_tiles;        // tile sums of the bucket scan
   uint32_t *rf_hist, *rf_fill, *rf_order;   // refit: tracks ordered by length
   int32_t* mg_best_b;
@@ -169,12 +171,16 @@ Workspace layout(const tpcHandle* h, int64_t N, int64_t capT, char* base) {
   w.kept_last = (int32_t*)take(4 * (size_t)Tn);
   w.owner_key = (unsigned long long*)take(8 * (size_t)Nn);
   w.owner_id = (uint32_t*)take(4 * (size_t)Nn);
-  const size_t mgb = (int64_t)nb * MG_NYB * MG_NZB < (1ll << 31) ? (size_t)nb * MG_NYB * MG_NZB + 1 : 1;   // else: merger refused
+  const size_t mgb = (int64_t)nb * MG_BINS < (1ll << 31) ? (size_t)nb * MG_BINS + 1 : 1;   // else: merger refused
   w.mg_start = (uint32_t*)take(4 * mgb);
   w.mg_fill = (uint32_t*)take(4 * mgb);
-  w.mg_maxv = (uint32_t*)take(8 * (size_t)nb);
+  w.mg_maxv = (uint32_t*)take(4 * (size_t)nb);
   w.mg_tiles = (uint32_t*)take(4 * (size_t)(ceilDiv((int64_t)mgb, SCAN_TILE) + 2));
   w.mg_list = (uint32_t*)take(4 * (size_t)Tn);
+  w.mg_rec = (float4*)take(16 * (size_t)Tn);
+  w.mg_ostart = (uint32_t*)take(4 * mgb);
+  w.mg_ofill = (uint32_t*)take(4 * mgb);
+  w.mg_order = (uint32_t*)take(4 * (size_t)Tn);
   w.rf_hist = (uint32_t*)take(4 * (size_t)(RF_BINS + 1));
   w.rf_fill = (uint32_t*)take(4 * (size_t)(RF_BINS + 1));
   w.rf_order = (uint32_t*)take(4 * (size_t)Tn);
@@ -346,7 +352,7 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   const int n_mg = (out->trk_mg_next != nullptr) + (out->trk_mg_prev != nullptr) + (out->trk_mg_head != nullptr) +
                    (out->trk_mg_chi2 != nullptr);
   if ((n_mg != 0 && n_mg != 4) || (n_mg == 4 && n_rf != 8)) return TPC_ERR_INVALID_ARG;   // the merger needs the refit
-  if (n_mg == 4 && (int64_t)h->P.n_buckets * MG_NYB * MG_NZB >= (1ll << 31)) return TPC_ERR_INVALID_ARG;   // bucket ids are 32-bit
+  if (n_mg == 4 && (int64_t)h->P.n_buckets * MG_BINS >= (1ll << 31)) return TPC_ERR_INVALID_ARG;   // bucket ids are 32-bit
   const int n_lg = (out->trk_leg_partner != nullptr) + (out->trk_leg_chi2 != nullptr);
   if ((n_lg != 0 && n_lg != 2) || (n_lg == 2 && n_rf != 8)) return TPC_ERR_INVALID_ARG;   // the leg pairs need the refit
   if (n_lg == 2 && (int64_t)h->P.n_buckets * 2 * LEG_BINS >= (1ll << 31)) return TPC_ERR_INVALID_ARG;   // bucket ids are 32-bit
@@ -472,21 +478,26 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
     const MergeParams mp{h->params.merge_max_row_gap, h->params.merge_back_rows, h->params.merge_chi2_max,
                          (float)cos(0.3490658503988659), (float)sin(0.3490658503988659)};
     const unsigned gK = (unsigned)ceilDiv(nk, 256);
-    const size_t mgb = (size_t)nb * MG_NYB * MG_NZB + 1;
+    const size_t mgb = (size_t)nb * MG_BINS + 1;
     TPC_CUDA(h, cudaMemsetAsync(w.mg_start, 0, 4 * mgb, st)); ++L;
     TPC_CUDA(h, cudaMemsetAsync(w.mg_fill, 0, 4 * mgb, st)); ++L;
-    TPC_CUDA(h, cudaMemsetAsync(w.mg_maxv, 0, 8 * (size_t)nb, st)); ++L;
-    mergeCount<<<gK, 256, 0, st>>>(mi, mo, P, T, w.mg_start, w.mg_maxv, w.mg_best_b, w.mg_key_a, cnt); ++L;
+    TPC_CUDA(h, cudaMemsetAsync(w.mg_ostart, 0, 4 * mgb, st)); ++L;
+    TPC_CUDA(h, cudaMemsetAsync(w.mg_ofill, 0, 4 * mgb, st)); ++L;
+    TPC_CUDA(h, cudaMemsetAsync(w.mg_maxv, 0, 4 * (size_t)nb, st)); ++L;
+    mergeCount<<<gK, 256, 0, st>>>(mi, mo, P, T, w.mg_start, w.mg_ostart, w.mg_maxv, w.mg_best_b, w.mg_key_a, cnt); ++L;
     {   // exclusive scan of the bucket counts; the closing sentinel lands on the last (spare) entry
       const int64_t nscan = (int64_t)mgb - 1;
       const unsigned tiles = (unsigned)ceilDiv(nscan, SCAN_TILE);
       scanTileSums<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.mg_start, cnt + CNT_INF, nscan, w.mg_tiles); ++L;
       scanTileOffsets<uint32_t><<<1, 1024, 0, st>>>(w.mg_tiles, cnt + CNT_INF, nscan, nullptr); ++L;
       scanApply<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.mg_start, w.mg_start, cnt + CNT_INF, nscan, w.mg_tiles); ++L;
+      scanTileSums<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.mg_ostart, cnt + CNT_INF, nscan, w.mg_tiles); ++L;
+      scanTileOffsets<uint32_t><<<1, 1024, 0, st>>>(w.mg_tiles, cnt + CNT_INF, nscan, nullptr); ++L;
+      scanApply<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.mg_ostart, w.mg_ostart, cnt + CNT_INF, nscan, w.mg_tiles); ++L;
     }
-    mergeFill<<<gK, 256, 0, st>>>(mi, P, T, w.mg_start, w.mg_fill, w.mg_list, cnt); ++L;
-    mergeMatch<<<(unsigned)ceilDiv(nk * MG_GROUP, 128), 128, 0, st>>>(mi, P, T, mp, w.mg_start, w.mg_maxv, w.mg_list, w.mg_best_b,
-                                                           w.mg_chi_b, w.mg_key_a, cnt); ++L;
+    mergeFill<<<gK, 256, 0, st>>>(mi, P, T, w.mg_start, w.mg_fill, w.mg_list, w.mg_rec, w.mg_ostart, w.mg_ofill, w.mg_order, cnt); ++L;
+    mergeMatch<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(mi, P, T, mp, w.mg_start, w.mg_maxv, w.mg_list, w.mg_rec, w.mg_ostart, w.mg_order, w.mg_best_b,
+                                                         w.mg_chi_b, w.mg_key_a, cnt); ++L;
     mergeLink<<<gK, 256, 0, st>>>(mi, mo, w.mg_best_b, w.mg_chi_b, w.mg_key_a, cnt); ++L;
     mergeHead<<<gK, 256, 0, st>>>(mi, mo, cnt); ++L;
   }

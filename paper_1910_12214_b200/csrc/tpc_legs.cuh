@@ -134,10 +134,13 @@ __global__ void __launch_bounds__(128) legMatch(LegIn in, DevParams P, LegParams
                                                 float* __restrict__ best_chi,
                                                 const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
-  const int64_t a = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (a >= cnt[CNT_N_TRACKS] || a >= in.cap || !legIsEnd(in, a, L)) return;
-  const int64_t cap = in.cap;
+  // the leg ends are taken in list order: the lanes of a warp hold ends of one (sector, sign, row, dip bin) or of its
+  // neighbours, so they walk nearly the same runs of candidates
+  const int64_t slot = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int R = P.n_rows;
+  if (slot >= bucket_start[(int64_t)P.n_buckets * 2 * LEG_BINS]) return;
+  const int64_t a = list[slot];
+  const int64_t cap = in.cap;
   const KFState A0 = mergeLoad(a, cap, in.x_out, in.par_out, in.cov_out);
   const int sec = in.sector[a], la = in.last_row[a];
   const int sg = A0.s > 0.0f ? 1 : -1;

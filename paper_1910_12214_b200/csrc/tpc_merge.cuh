@@ -6,11 +6,14 @@
 // needed, propagated to b's reference plane -- against b's inner state.  next(a) = admissible b of minimal (chi2, id),
 // prev(b) = admissible a of minimal (chi2, id); a link is kept when both agree.
 //
-// Organisation: the tracks are bucketed by (sector, first kept row, z bin, y bin of their inner state) -- all b of a
-// (sector, row) share their reference plane, so a is propagated once per candidate ROW, not once per pair, and only the
-// bins that can hold a b whose y or z term alone stays below the cut are visited: the terms are non-negative, so the
-// sum could only be larger, and the window uses the largest inner variances of the row (plus rounding slack), so it is a
-// superset of every admissible b -- no result changes (same argument as R3).  prev(b) is an atomicMin over (chi2 bits, a).
+// Organisation: the tracks are bucketed by (sector, first kept row, bin of the dip t of their inner state).  The dip and
+// curvature terms of the chi2 need no transport -- Rotate and Propagate leave t, q, C33 and C44 as they are -- so they are
+// tested first, on 16-byte records packed in list order, and only the dip bins that can hold a b whose dip term alone
+// stays below the cut are visited: the terms are non-negative and rounding is monotone, so the sum could only be larger,
+// and the window uses the largest dip variance of the (sector, row) (plus rounding slack; badly measured dips sit in one
+// extra bin that is always visited), so it is a superset of every admissible b -- no result changes (same argument as
+// R3).  All b of a (sector, row) share their reference plane: a is propagated once per ROW that has a surviving candidate,
+// which is a handful of the 132 rows in reach.  prev(b) is an atomicMin over (chi2 bits, a).
 #pragma once
 #include "tpc_kalman.cuh"
 #include "tpc_refit.cuh"
@@ -26,14 +29,14 @@ struct MergeOut {
   int32_t *next, *prev, *head;
   float* chi2;
 };
-constexpr int MG_NYB = 32, MG_NZB = 16;     // y / z bins of the inner states per (sector, row)
-constexpr int MG_GROUP = 1;                  // lanes per track in mergeMatch (more lanes only repeat the 132 Propagates: 4 -> 14.2 ms against 13.2)
+constexpr int MG_NTB = 64;                   // dip bins over [-MG_TMAX, MG_TMAX] (clamped outside)
+constexpr float MG_TMAX = 2.0f;
+constexpr float MG_VWIDE = 2e-5f;            // inner states with a larger dip variance go to one extra bin, always visited
+constexpr int MG_BINS = MG_NTB + 1;
 
-__device__ __forceinline__ int mergeBucket(int sr, float y, float z, float x_row, const DevParams& P) {
-  const float hw = x_row * P.tan_half_sector;
-  const int by = cellCoord(y, -hw, (float)MG_NYB / (2.0f * hw), MG_NYB);
-  const int bz = cellCoord(z, P.z_min, (float)MG_NZB / (P.z_max - P.z_min), MG_NZB);
-  return (sr * MG_NZB + bz) * MG_NYB + by;
+__device__ __forceinline__ int mergeDipBin(float t) { return cellCoord(t, -MG_TMAX, (float)MG_NTB / (2.0f * MG_TMAX), MG_NTB); }
+__device__ __forceinline__ int mergeBucket(int sr, float t, float var_t) {
+  return sr * MG_BINS + (var_t <= MG_VWIDE ? mergeDipBin(t) : MG_NTB);
 }
 
 struct MergeParams {
@@ -43,8 +46,8 @@ struct MergeParams {
 
 // per track: clear the outputs, count the refitted tracks per (sector, first row)
 __global__ void __launch_bounds__(256) mergeCount(MergeIn in, MergeOut out, DevParams P, RowTables T,
-                                                  uint32_t* __restrict__ bucket_cnt, uint32_t* __restrict__ max_var,
-                                                  int32_t* __restrict__ best_b, unsigned long long* __restrict__ key_a,
+                                                  uint32_t* __restrict__ bucket_cnt, uint32_t* __restrict__ order_cnt,
+                                                  uint32_t* __restrict__ max_var, int32_t* __restrict__ best_b, unsigned long long* __restrict__ key_a,
                                                   const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -52,24 +55,34 @@ __global__ void __launch_bounds__(256) mergeCount(MergeIn in, MergeOut out, DevP
   out.next[k] = -1; out.prev[k] = -1; out.head[k] = (int32_t)k; out.chi2[k] = 0.0f;
   best_b[k] = -1; key_a[k] = ~0ull;
   if (in.status[k] == 1) {
-    const int r = in.first_row[k], sr = in.sector[k] * P.n_rows + r;
-    atomicAdd(bucket_cnt + mergeBucket(sr, in.par_in[k], in.par_in[in.cap + k], T.row_x[r], P), 1u);
-    // largest inner variances of the (sector, row): positive floats order like their bit patterns
-    atomicMax(max_var + 2 * sr, __float_as_uint(in.cov_in[k]));
-    atomicMax(max_var + 2 * sr + 1, __float_as_uint(in.cov_in[2 * in.cap + k]));
+    const int sr = in.sector[k] * P.n_rows + in.first_row[k];
+    const float vt = in.cov_in[9 * in.cap + k];
+    atomicAdd(bucket_cnt + mergeBucket(sr, in.par_in[3 * in.cap + k], vt), 1u);
+    // largest binned dip variance of the (sector, row): positive floats order like their bit patterns
+    if (vt <= MG_VWIDE) atomicMax(max_var + sr, __float_as_uint(vt));
+    // the order in which mergeMatch takes the tracks a: by (sector, last row, dip bin) of the OUTER state
+    atomicAdd(order_cnt + mergeBucket(in.sector[k] * P.n_rows + in.last_row[k], in.par_out[3 * in.cap + k], in.cov_out[9 * in.cap + k]), 1u);
   }
 }
 
 // per track: its slot in the bucket list (order inside a bucket is arbitrary: every argmin below breaks ties by id)
 __global__ void __launch_bounds__(256) mergeFill(MergeIn in, DevParams P, RowTables T, const uint32_t* __restrict__ bucket_start,
                                                  uint32_t* __restrict__ bucket_fill, uint32_t* __restrict__ list,
+                                                 float4* __restrict__ rec, const uint32_t* __restrict__ order_start,
+                                                 uint32_t* __restrict__ order_fill, uint32_t* __restrict__ order,
                                                  const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= cnt[CNT_N_TRACKS] || k >= in.cap || in.status[k] != 1) return;
-  const int r = in.first_row[k];
-  const int b = mergeBucket(in.sector[k] * P.n_rows + r, in.par_in[k], in.par_in[in.cap + k], T.row_x[r], P);
-  list[bucket_start[b] + atomicAdd(bucket_fill + b, 1u)] = (uint32_t)k;
+  {
+    const int o = mergeBucket(in.sector[k] * P.n_rows + in.last_row[k], in.par_out[3 * in.cap + k], in.cov_out[9 * in.cap + k]);
+    order[order_start[o] + atomicAdd(order_fill + o, 1u)] = (uint32_t)k;
+  }
+  const float t = in.par_in[3 * in.cap + k], vt = in.cov_in[9 * in.cap + k];
+  const int b = mergeBucket(in.sector[k] * P.n_rows + in.first_row[k], t, vt);
+  const uint32_t slot = bucket_start[b] + atomicAdd(bucket_fill + b, 1u);
+  list[slot] = (uint32_t)k;
+  rec[slot] = make_float4(t, in.par_in[4 * in.cap + k], vt, in.cov_in[14 * in.cap + k]);   // what the first tests read
 }
 
 // O7 Rotate(alpha) with (ca, sa); returns false (state untouched) if |sin phi'| would reach max_sinphi
@@ -119,93 +132,79 @@ __device__ __forceinline__ int64_t live_guard(int64_t a, int64_t cap) { return a
 __global__ void __launch_bounds__(128) mergeMatch(MergeIn in, DevParams P, RowTables T, MergeParams M,
                                                   const uint32_t* __restrict__ bucket_start,
                                                   const uint32_t* __restrict__ max_var,
-                                                  const uint32_t* __restrict__ list, int32_t* __restrict__ best_b,
-                                                  float* __restrict__ chi_b, unsigned long long* __restrict__ key_a,
-                                                  const int64_t* __restrict__ cnt) {
+                                                  const uint32_t* __restrict__ list, const float4* __restrict__ rec,
+                                                  const uint32_t* __restrict__ order_start, const uint32_t* __restrict__ order,
+                                                  int32_t* __restrict__ best_b, float* __restrict__ chi_b,
+                                                  unsigned long long* __restrict__ key_a, const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
-  // MG_GROUP lanes per track: they carry the same state (the Propagate of a row is redundant but uniform) and share the
-  // candidates of the bins; their best continuations are merged by shuffles at the end.
-  const int64_t a = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / MG_GROUP;
-  const int sub = threadIdx.x % MG_GROUP;
-  // Lanes without a track stay in the loops (predicated off): the row loop below has the same trip count for every
-  // lane and reconverges at __syncwarp(), so the 32 lanes run the Propagate of a row together.
-  const bool live = a < cnt[CNT_N_TRACKS] && a < in.cap && in.status[live_guard(a, in.cap)] == 1;
+  // the tracks a are taken by (sector, last row, dip bin) of their outer state: the lanes of a warp walk nearly the
+  // same rows and the same runs of candidates
+  const int64_t slot = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (slot >= order_start[(int64_t)P.n_buckets * MG_BINS]) return;
+  const int64_t a = order[slot];
   const int64_t cap = in.cap;
   const int R = P.n_rows;
-  const int sa_sec = live ? in.sector[a] : 0, la = live ? in.last_row[a] : 0;
-  KFState A0{};
-  if (live) A0 = mergeLoad(a, cap, in.x_out, in.par_out, in.cov_out);
+  const int sa_sec = in.sector[a], la = in.last_row[a];
+  const KFState A0 = mergeLoad(a, cap, in.x_out, in.par_out, in.cov_out);
   int32_t bb = -1;
   float bchi = 0.0f;
-  const int n_it = M.back_rows + M.max_row_gap + 1;      // rows la - back_rows .. la + max_row_gap
   for (int rel = 0; rel <= 2; ++rel) {           // 0 same sector, 1 next sector (+20 degrees), 2 previous sector
-    if (rel != 0 && P.n_sectors != 36) break;    // uniform
+    if (rel != 0 && P.n_sectors != 36) break;
     int sb = sa_sec;
     KFState Ar = A0;
-    bool rel_ok = live;
     if (rel != 0) {
       const int side = sa_sec / 18, j = sa_sec - side * 18;
       sb = side * 18 + (rel == 1 ? (j + 1) % 18 : (j + 17) % 18);
-      rel_ok = live && kfRotate(Ar, M.ca, rel == 1 ? M.sa : -M.sa, P);
+      if (!kfRotate(Ar, M.ca, rel == 1 ? M.sa : -M.sa, P)) continue;
     }
     const int r_lo = max(0, la + (rel == 0 ? 1 : -M.back_rows)), r_hi = min(R - 1, la + M.max_row_gap);
-    for (int it = 0; it < n_it; ++it) {
-      __syncwarp();
-      const int r = la - M.back_rows + it;
-      bool act = rel_ok && r >= r_lo && r <= r_hi;
-      const int sr = act ? sb * R + r : 0;
-      const float vy = act ? __uint_as_float(max_var[2 * sr]) : 0.0f;
-      act = act && vy != 0.0f;                     // no refitted track starts on this (sector, row)
+    for (int r = r_lo; r <= r_hi; ++r) {
+      const int sr = sb * R + r;
+      const uint32_t* bs = bucket_start + sr * MG_BINS;
+      // dip bins that can hold an admissible b: |t_a - t_b| <= sqrt(chi2_max * (C33_a + max C33_b)), with slack; a window
+      // that is not >= 0 means no positive denominator is possible among the binned b
+      const float w = sqrtf(M.chi2_max * (Ar.c33 + __uint_as_float(max_var[sr]))) * 1.0001f + 1e-6f;
+      const bool any = w >= 0.0f;
+      const uint32_t j0 = bs[MG_NTB], j1 = bs[MG_BINS];        // the b with a wide dip variance: always visited
+      const uint32_t i0 = any ? bs[mergeDipBin(Ar.t - w)] : j0, i1 = any ? bs[mergeDipBin(Ar.t + w) + 1] : j0;
       KFState S = Ar;
-      const float xr = T.row_x[act ? r : 0];
-      const bool okp = kfPropagate(S, act ? xr : S.x, P, [](float, float, float, float) {});
-      if (!(act && okp)) continue;
-      // bins that can hold an admissible b: |dy| <= sqrt(chi2_max * (C00 + max C00_b)), likewise z (with slack)
-      const float wy = sqrtf(M.chi2_max * (S.c00 + vy)) * 1.0001f + 1e-6f;
-      const float wz = sqrtf(M.chi2_max * (S.c11 + __uint_as_float(max_var[2 * sr + 1]))) * 1.0001f + 1e-6f;
-      if (!(wy >= 0.0f) || !(wz >= 0.0f)) continue;      // a non-positive variance of a: every denominator test fails below anyway
-      const float hw = xr * P.tan_half_sector;
-      const float iby = (float)MG_NYB / (2.0f * hw), ibz = (float)MG_NZB / (P.z_max - P.z_min);
-      const int by0 = cellCoord(S.y - wy, -hw, iby, MG_NYB), by1 = cellCoord(S.y + wy, -hw, iby, MG_NYB);
-      const int bz0 = cellCoord(S.z - wz, P.z_min, ibz, MG_NZB), bz1 = cellCoord(S.z + wz, P.z_min, ibz, MG_NZB);
-      for (int bz = bz0; bz <= bz1; ++bz) {
-      const uint32_t* row = bucket_start + (sr * MG_NZB + bz) * MG_NYB;
-      const uint32_t k0 = row[by0], k1 = row[by1 + 1];
-      for (uint32_t i = k0 + sub; i < k1; i += MG_GROUP) {
+      int state = 0;                               // 0 not propagated to this row yet, 1 done, 2 refused
+      for (uint32_t ii = i0; ii < i1 + (j1 - j0) && state != 2; ++ii) {
+        const uint32_t i = ii < i1 ? ii : j0 + (ii - i1);
+        // The dip and curvature terms need no transport (see the header); one of them above the cut decides.
+        const float4 rc = __ldg(rec + i);          // t, q, C33, C44 of the candidate
+        const float den3 = Ar.c33 + rc.z, den4 = Ar.c44 + rc.w;
+        const float d3 = Ar.t - rc.x, d4 = Ar.q - rc.y;
+        const float t3 = (d3 * d3) / den3, t4 = (d4 * d4) / den4;
+        if (t3 > M.chi2_max || t4 > M.chi2_max) continue;
         const int64_t b = list[i];
         if (b == a) continue;
-        // the y term first: it alone decides for almost every pair of the bucket
-        const float den0 = S.c00 + in.cov_in[0 * cap + b];
-        if (!(den0 > 0.0f)) continue;
-        const float d0 = S.y - in.par_in[0 * cap + b];
-        float sum = 0.0f + (d0 * d0) / den0;
-        if (!(sum <= M.chi2_max)) continue;
-        const float pa[4] = {S.z, S.s, S.t, S.q};
-        const float ca[4] = {S.c11, S.c22, S.c33, S.c44};
-        const int ci[4] = {2, 5, 9, 14};
+        if (state == 0) state = kfPropagate(S, T.row_x[r], P, [](float, float, float, float) {}) ? 1 : 2;
+        if (state == 2) break;
+        // the five terms in the order of Match: y, z, s, t, q
+        const float pa[3] = {S.y, S.z, S.s};
+        const float ca[3] = {S.c00, S.c11, S.c22};
+        const int ci[3] = {0, 2, 5};
         bool ok = true;
+        float sum = 0.0f;
 #pragma unroll
-        for (int q = 0; q < 4; ++q) {
+        for (int q = 0; q < 3; ++q) {
           const float den = ca[q] + in.cov_in[ci[q] * cap + b];
           if (!(den > 0.0f)) { ok = false; break; }
-          const float d = pa[q] - in.par_in[(q + 1) * cap + b];
+          const float d = pa[q] - in.par_in[q * cap + b];
           sum = sum + (d * d) / den;
+          if (!(sum <= M.chi2_max)) { ok = false; break; }       // the terms are non-negative: it can only grow
         }
-        if (!ok || !(sum <= M.chi2_max)) continue;
+        if (!ok || !(den3 > 0.0f) || !(den4 > 0.0f)) continue;
+        sum = sum + t3;
+        sum = sum + t4;
+        if (!(sum <= M.chi2_max)) continue;
         if (bb < 0 || sum < bchi || (sum == bchi && (int32_t)b < bb)) { bb = (int32_t)b; bchi = sum; }
         atomicMin(key_a + b, ((unsigned long long)__float_as_uint(sum) << 32) | (unsigned long long)(uint32_t)a);
       }
-      }
     }
   }
-  __syncwarp();
-#pragma unroll
-  for (int d = 1; d < MG_GROUP; d <<= 1) {         // minimal (chi2, id) over the lanes of the group
-    const int32_t ob = __shfl_xor_sync(0xffffffffu, bb, d);
-    const float oc = __shfl_xor_sync(0xffffffffu, bchi, d);
-    if (ob >= 0 && (bb < 0 || oc < bchi || (oc == bchi && ob < bb))) { bb = ob; bchi = oc; }
-  }
-  if (live && sub == 0) { best_b[a] = bb; chi_b[a] = bchi; }
+  best_b[a] = bb; chi_b[a] = bchi;
 }
 
 // a link is kept when next(a) = b and prev(b) = a (R33)
