@@ -138,11 +138,14 @@ __global__ void __launch_bounds__(128) legMatch(LegIn in, DevParams P, LegParams
   // neighbours, so they walk nearly the same runs of candidates
   const int64_t slot = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   const int R = P.n_rows;
-  if (slot >= bucket_start[(int64_t)P.n_buckets * 2 * LEG_BINS]) return;
-  const int64_t a = list[slot];
+  // Lanes without an end stay in the loops (predicated off): the row loop has the same trip count for every lane and
+  // reconverges at __syncwarp().
+  const bool live = slot < bucket_start[(int64_t)P.n_buckets * 2 * LEG_BINS];
+  const int64_t a = live ? list[slot] : 0;
   const int64_t cap = in.cap;
-  const KFState A0 = mergeLoad(a, cap, in.x_out, in.par_out, in.cov_out);
-  const int sec = in.sector[a], la = in.last_row[a];
+  KFState A0{};
+  if (live) A0 = mergeLoad(a, cap, in.x_out, in.par_out, in.cov_out);
+  const int sec = live ? in.sector[a] : 0, la = live ? in.last_row[a] : 0;
   const int sg = A0.s > 0.0f ? 1 : -1;
   const int side = sec / 18, j = sec - side * 18;
   const int r_lo = max(0, la - L.max_row_diff), r_hi = min(R - 1, la + L.max_row_diff);
@@ -152,7 +155,10 @@ __global__ void __launch_bounds__(128) legMatch(LegIn in, DevParams P, LegParams
   for (int dd = 0; dd <= dmax; ++dd) {
     const int d = sg * dd;                                     // a moves towards the sectors on this side of it
     const int sb = dd == 0 ? sec : side * 18 + (j + d + 18) % 18;
-    for (int r = r_lo; r <= r_hi; ++r) {
+    for (int it = 0; it <= 2 * L.max_row_diff; ++it) {
+      __syncwarp();
+      const int r = la - L.max_row_diff + it;
+      if (!(live && r >= r_lo && r <= r_hi)) continue;
       const int sr = legRowKey(sb, sg < 0, r, R);              // the other inclination
       const uint32_t* bs = bucket_start + sr * LEG_BINS;
       // dip bins that can hold a partner: |t_a + t_b| <= sqrt(chi2_max * (C33_a + max C33_b)), with slack; a window
@@ -186,7 +192,7 @@ __global__ void __launch_bounds__(128) legMatch(LegIn in, DevParams P, LegParams
       }
     }
   }
-  best[a] = bb; best_chi[a] = bchi;
+  if (live) { best[a] = bb; best_chi[a] = bchi; }
 }
 
 // a pair is kept when each is the other's choice (R42)

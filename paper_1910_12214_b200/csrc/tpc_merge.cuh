@@ -139,26 +139,34 @@ __global__ void __launch_bounds__(128) mergeMatch(MergeIn in, DevParams P, RowTa
   if (cnt[CNT_ERROR] != 0) return;
   // the tracks a are taken by (sector, last row, dip bin) of their outer state: the lanes of a warp walk nearly the
   // same rows and the same runs of candidates
+  // Lanes without a track stay in the loops (predicated off): the row loop has the same trip count for every lane and
+  // reconverges at __syncwarp(), so the lanes set up a row together however many candidates each had on the last one.
   const int64_t slot = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (slot >= order_start[(int64_t)P.n_buckets * MG_BINS]) return;
-  const int64_t a = order[slot];
+  const bool live = slot < order_start[(int64_t)P.n_buckets * MG_BINS];
+  const int64_t a = live ? order[slot] : 0;
   const int64_t cap = in.cap;
   const int R = P.n_rows;
-  const int sa_sec = in.sector[a], la = in.last_row[a];
-  const KFState A0 = mergeLoad(a, cap, in.x_out, in.par_out, in.cov_out);
+  const int sa_sec = live ? in.sector[a] : 0, la = live ? in.last_row[a] : 0;
+  KFState A0{};
+  if (live) A0 = mergeLoad(a, cap, in.x_out, in.par_out, in.cov_out);
   int32_t bb = -1;
   float bchi = 0.0f;
+  const int n_it = M.back_rows + M.max_row_gap + 1;      // rows la - back_rows .. la + max_row_gap
   for (int rel = 0; rel <= 2; ++rel) {           // 0 same sector, 1 next sector (+20 degrees), 2 previous sector
-    if (rel != 0 && P.n_sectors != 36) break;
+    if (rel != 0 && P.n_sectors != 36) break;    // uniform
     int sb = sa_sec;
     KFState Ar = A0;
+    bool rel_ok = live;
     if (rel != 0) {
       const int side = sa_sec / 18, j = sa_sec - side * 18;
       sb = side * 18 + (rel == 1 ? (j + 1) % 18 : (j + 17) % 18);
-      if (!kfRotate(Ar, M.ca, rel == 1 ? M.sa : -M.sa, P)) continue;
+      rel_ok = live && kfRotate(Ar, M.ca, rel == 1 ? M.sa : -M.sa, P);
     }
     const int r_lo = max(0, la + (rel == 0 ? 1 : -M.back_rows)), r_hi = min(R - 1, la + M.max_row_gap);
-    for (int r = r_lo; r <= r_hi; ++r) {
+    for (int it = 0; it < n_it; ++it) {
+      __syncwarp();
+      const int r = la - M.back_rows + it;
+      if (!(rel_ok && r >= r_lo && r <= r_hi)) continue;
       const int sr = sb * R + r;
       const uint32_t* bs = bucket_start + sr * MG_BINS;
       // dip bins that can hold an admissible b: |t_a - t_b| <= sqrt(chi2_max * (C33_a + max C33_b)), with slack; a window
@@ -204,7 +212,7 @@ __global__ void __launch_bounds__(128) mergeMatch(MergeIn in, DevParams P, RowTa
       }
     }
   }
-  best_b[a] = bb; chi_b[a] = bchi;
+  if (live) { best_b[a] = bb; chi_b[a] = bchi; }
 }
 
 // a link is kept when next(a) = b and prev(b) = a (R33)
