@@ -181,8 +181,9 @@ Workspace layout(const tpcHandle* h, int64_t N, int64_t capT, char* base) {
   w.mg_ostart = (uint32_t*)take(4 * mgb);
   w.mg_ofill = (uint32_t*)take(4 * mgb);
   w.mg_order = (uint32_t*)take(4 * (size_t)Tn);
-  w.rf_hist = (uint32_t*)take(4 * (size_t)(RF_BINS + 1));
-  w.rf_fill = (uint32_t*)take(4 * (size_t)(RF_BINS + 1));
+  const size_t rfb = (size_t)(Tn / RF_CHUNK + 1) * RF_BINS + 1;
+  w.rf_hist = (uint32_t*)take(4 * rfb);
+  w.rf_fill = (uint32_t*)take(4 * rfb);
   w.rf_order = (uint32_t*)take(4 * (size_t)Tn);
   w.mg_best_b = (int32_t*)take(4 * (size_t)Tn);
   w.mg_chi_b = (float*)take(4 * (size_t)Tn);
@@ -459,10 +460,11 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
     const RefitOut rf{out->trk_rf_status, out->trk_rf_x_in, out->trk_rf_par_in, out->trk_rf_cov_in, out->trk_rf_chi2,
                       out->trk_rf_x_out, out->trk_rf_par_out, out->trk_rf_cov_out};
     const int64_t nk = std::min<int64_t>(out->cap_tracks, capT);
-    TPC_CUDA(h, cudaMemsetAsync(w.rf_hist, 0, 4 * (size_t)(RF_BINS + 1), st)); ++L;
-    TPC_CUDA(h, cudaMemsetAsync(w.rf_fill, 0, 4 * (size_t)(RF_BINS + 1), st)); ++L;
+    const size_t rfb = (size_t)(nk / RF_CHUNK + 1) * RF_BINS + 1;
+    TPC_CUDA(h, cudaMemsetAsync(w.rf_hist, 0, 4 * rfb, st)); ++L;
+    TPC_CUDA(h, cudaMemsetAsync(w.rf_fill, 0, 4 * rfb, st)); ++L;
     refitCount<<<(unsigned)ceilDiv(nk, 256), 256, 0, st>>>(to, w.rf_hist, cnt); ++L;
-    scanArrayInPlace<uint32_t><<<1, 1024, 0, st>>>(w.rf_hist, (int64_t)RF_BINS + 1, nullptr); ++L;
+    scanArrayInPlace<uint32_t><<<1, 1024, 0, st>>>(w.rf_hist, (int64_t)rfb, nullptr); ++L;
     refitFill<<<(unsigned)ceilDiv(nk, 256), 256, 0, st>>>(to, w.rf_hist, w.rf_fill, w.rf_order, cnt); ++L;
     refitTracks<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(in->row_offset, w.rf_order, in->y, in->z, P, T, to, rf, cnt); ++L;
   }

@@ -28,16 +28,24 @@ __device__ __forceinline__ void refitStore(const KFState& S, int64_t k, int64_t 
   cov[12 * cap + k] = S.c42; cov[13 * cap + k] = S.c43; cov[14 * cap + k] = S.c44;
 }
 
-// Tracks are refitted in the order of their length (longest first), so that the 32 tracks of a warp need about the same
-// number of steps: histogram of the lengths, exclusive scan (scanArrayInPlace), slots.  Order inside a length is arbitrary.
+// Tracks are refitted in the order of their length (longest first) inside chunks of RF_CHUNK consecutive tracks, so that
+// the 32 tracks of a warp need about the same number of steps AND the tracks in flight lie in a few sectors (the track
+// order is the sector order): their cluster reads, random inside a sector, then stay in the L2.  Histogram of (chunk,
+// length), exclusive scan (scanArrayInPlace), slots.  Order inside a bin is arbitrary.
 constexpr int RF_BINS = 256;
-__device__ __forceinline__ int refitBin(uint32_t n) { return RF_BINS - 1 - (int)min(n, (uint32_t)(RF_BINS - 1)); }
+#ifndef RF_CHUNK_
+#define RF_CHUNK_ 32768
+#endif
+constexpr int RF_CHUNK = RF_CHUNK_;
+__device__ __forceinline__ int64_t refitBin(int64_t k, uint32_t n) {
+  return (k / RF_CHUNK) * RF_BINS + (RF_BINS - 1 - (int)min(n, (uint32_t)(RF_BINS - 1)));
+}
 
 __global__ void __launch_bounds__(256) refitCount(TrackOut o, uint32_t* __restrict__ hist, const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= cnt[CNT_N_TRACKS] || k >= o.cap_tracks) return;
-  atomicAdd(hist + refitBin(o.cl_offset[k + 1] - o.cl_offset[k]), 1u);
+  atomicAdd(hist + refitBin(k, o.cl_offset[k + 1] - o.cl_offset[k]), 1u);
 }
 
 __global__ void __launch_bounds__(256) refitFill(TrackOut o, const uint32_t* __restrict__ start, uint32_t* __restrict__ fill,
@@ -45,7 +53,7 @@ __global__ void __launch_bounds__(256) refitFill(TrackOut o, const uint32_t* __r
   if (cnt[CNT_ERROR] != 0) return;
   const int64_t k = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (k >= cnt[CNT_N_TRACKS] || k >= o.cap_tracks) return;
-  const int b = refitBin(o.cl_offset[k + 1] - o.cl_offset[k]);
+  const int64_t b = refitBin(k, o.cl_offset[k + 1] - o.cl_offset[k]);
   order[start[b] + atomicAdd(fill + b, 1u)] = (uint32_t)k;
 }
 
