@@ -560,11 +560,20 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
       const FlagIn fi{out->cap_tracks, out->trk_rf_status, out->trk_sector, out->trk_first_row, out->trk_last_row,
                       out->trk_rf_x_in, out->trk_rf_par_in, out->trk_rf_cov_in, out->trk_cl_offset, out->trk_cl_index};
       const int64_t nk = std::min<int64_t>(out->cap_tracks, capT);
+      // the walking states of the attached clusters, one float2 per track-cluster entry: the selector's owner keys
+      // (8 bytes per cluster, dead since selectEmit) are the buffer
+      float2* walk_yz = out->cl_res_y ? reinterpret_cast<float2*>(w.owner_key) : nullptr;
+      const int64_t n_ent = std::min<int64_t>(out->cap_track_clusters, N);
+      if (walk_yz) { TPC_CUDA(h, cudaMemsetAsync(walk_yz, 0xFF, 8 * (size_t)n_ent, st)); ++L; }
       flagAttach<<<(unsigned)ceilDiv(std::min<int64_t>(out->cap_track_clusters, N), 256), 256, 0, st>>>(out->trk_cl_index,
                                                                                                        out->cl_flags, cnt); ++L;
       flagBid<<<(unsigned)ceilDiv(nk * FLAG_GROUP, 128), 128, 0, st>>>(fi, in->row_offset, P, T, h->params.tube_radius,
                                                           h->params.inv_pt_protect, w.desc, w.cell_start, w.syz, w.s2o,
-                                                          w.fl_key, in->y, in->z, out->cl_res_y, out->cl_res_z, cnt); ++L;
+                                                          w.fl_key, walk_yz, cnt); ++L;
+      if (walk_yz) {
+        flagResiduals<<<(unsigned)ceilDiv(n_ent, 256), 256, 0, st>>>(out->trk_cl_index, walk_yz, in->y, in->z, out->cl_res_y,
+                                                                    out->cl_res_z, cnt); ++L;
+      }
     }
     flagFinish<<<gN256, 256, 0, st>>>(N, w.fl_key, out->cl_flags, out->cl_owner, cnt); ++L;
   }

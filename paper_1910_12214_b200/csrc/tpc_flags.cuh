@@ -37,9 +37,7 @@ __global__ void __launch_bounds__(128) flagBid(FlagIn in, const uint32_t* __rest
                                                float tube, float inv_pt_protect, const GridDesc* __restrict__ desc,
                                                const uint32_t* __restrict__ cell_start, const float2* __restrict__ syz,
                                                const uint32_t* __restrict__ s2o, unsigned long long* __restrict__ key,
-                                               const float* __restrict__ yin, const float* __restrict__ zin,
-                                               float* __restrict__ res_y, float* __restrict__ res_z,
-                                               const int64_t* __restrict__ cnt) {
+                                               float2* __restrict__ walk_yz, const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
   const int64_t k = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / FLAG_GROUP;
   const int sub = threadIdx.x % FLAG_GROUP;
@@ -74,7 +72,9 @@ __global__ void __launch_bounds__(128) flagBid(FlagIn in, const uint32_t* __rest
     if (sub == 0 && ic < ncl && cl[ic] < b_hi) {
       const uint32_t own = cl[ic];
       atomicMin(key + own, bid);
-      if (res_y) { res_y[own] = yin[own] - S.y; res_z[own] = zin[own] - S.z; }     // track-model residuals (R39)
+      // for the track-model residuals (R39): the walking state at the attached cluster, in the order of the track's
+      // cluster list (consecutive writes); flagResiduals turns them into residuals in one pass over all lists
+      if (walk_yz) walk_yz[in.cl_offset[k] + ic] = make_float2(S.y, S.z);
     }
     // the tube: cells of the box around it (a hair wider than the tube: fl(dy*dy) <= fl(tube*tube) does not quite imply
     // |dy| <= tube), exact circle predicate; the lanes of the group take the candidates of a cell row in turn
@@ -95,6 +95,21 @@ __global__ void __launch_bounds__(128) flagBid(FlagIn in, const uint32_t* __rest
       }
     }
   }
+}
+
+// thread per track-cluster entry: res = cluster - walking state of its track on its row (R39); entries the walk did not
+// reach (refused Propagate, track not refitted) still hold the NaN pattern the buffer was filled with
+__global__ void __launch_bounds__(256) flagResiduals(const uint32_t* __restrict__ cl_index, const float2* __restrict__ walk_yz,
+                                                     const float* __restrict__ yin, const float* __restrict__ zin,
+                                                     float* __restrict__ res_y, float* __restrict__ res_z,
+                                                     const int64_t* __restrict__ cnt) {
+  if (cnt[CNT_ERROR] != 0) return;
+  const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= cnt[CNT_N_TRK_CL]) return;
+  const float2 w = walk_yz[i];
+  if (!(w.x == w.x)) return;
+  const uint32_t c = cl_index[i];
+  res_y[c] = yin[c] - w.x; res_z[c] = zin[c] - w.y;
 }
 
 // thread per cluster: key -> flag byte and owner
