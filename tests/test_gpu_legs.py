@@ -77,3 +77,40 @@ def test_legs_need_the_refit_outputs_and_both_pointers():
     with pytest.raises(tpc.TpcError):
         tpc.TpcTracker.from_event(ev, params=p)
     trk.close()
+
+
+@pytest.mark.parametrize("seed", list(range(8)))
+def test_fuzz_all_optional_stages_together(seed):
+    """Seeded random small events and parameters with the refit, the merger, the leg pairs and the cluster flags all
+    switched on in one tpcRun: every optional output must still be bit-identical to the oracle's."""
+    from paper_1910_12214_b200 import tpc
+    rng = np.random.default_rng(4000 + seed)
+    idx = int(rng.integers(1, 5))
+    scale = float({1: 0.04, 2: 0.06, 3: 0.03, 4: 0.008}[idx] * rng.uniform(0.6, 1.4))
+    dead = tuple(int(r) for r in rng.choice(152, size=int(rng.integers(0, 5)), replace=False))
+    ev = datagen.make_event(idx, scale=scale, seed=300 + seed, dead_rows=dead)
+    par = dict(max_sinphi=float(rng.uniform(0.85, 0.99)), min_track_hits=int(rng.integers(6, 20)),
+               merge_max_row_gap=int(rng.integers(5, 80)), merge_back_rows=int(rng.integers(0, 10)),
+               merge_chi2_max=float(rng.uniform(5.0, 200.0)), tube_radius=float(rng.uniform(0.5, 3.0)),
+               inv_pt_protect=float(rng.uniform(2.0, 30.0)), leg_min_sinphi=float(rng.uniform(0.1, 0.9)),
+               leg_chi2_max=float(rng.uniform(5.0, 300.0)), leg_max_sectors=int(rng.integers(0, 9)),
+               leg_max_row_diff=int(rng.integers(0, 40)), leg_max_centre_dist=float(rng.uniform(0.5, 50.0)))
+    p, po = tpc.tpcDefaultParams(), orc.default_params()
+    for k, v in par.items():
+        setattr(p, k, v)
+        setattr(po, k, v)
+    trk = tpc.TpcTracker.from_event(ev, params=p)
+    off, y, z = trk.upload(ev)
+    res = trk.run(off, y, z, legs=True, merge=True, flags=True)
+    assert res.status.status == 0
+    g = res.numpy()
+    trk.close()
+    o = orc.run(ev, po, legs=True, merge=True, flags=True)
+    assert np.array_equal(g["trk_cl_index"].view(np.uint32), o.trk_cl_index)
+    assert np.array_equal(g["trk_rf_status"], o.rf_status)
+    assert np.array_equal(g["trk_rf_par_out"], o.rf_par_out.T.astype(np.float32))
+    assert np.array_equal(g["trk_leg_partner"], o.lg_partner) and np.array_equal(g["trk_leg_chi2"], o.lg_chi2.astype(np.float32))
+    assert np.array_equal(g["trk_mg_next"], o.mg_next) and np.array_equal(g["trk_mg_prev"], o.mg_prev)
+    assert np.array_equal(g["trk_mg_head"], o.mg_head) and np.array_equal(g["trk_mg_chi2"], o.mg_chi2.astype(np.float32))
+    assert np.array_equal(g["cl_flags"], o.cf_flags) and np.array_equal(g["cl_owner"], o.cf_owner)
+    assert np.array_equal(g["cl_res_y"], o.cf_res_y.astype(np.float32)) and np.array_equal(g["cl_res_z"], o.cf_res_z.astype(np.float32))
