@@ -932,6 +932,26 @@ int orcPackCharge(int64_t n, const float* q, int nb, uint16_t* code) {
   return 1;
 }
 
+// O11 (rest of NEXT-4; DESIGN.md section 3 "O11", reading R45): positions -- absolute, or residuals to
+// the track model -- as 16-bit integers in units of 2^-bits cm: nearest integer (ties to even), saturated; NaN -> 0.
+int orcPackPositions(int64_t n, const float* y, const float* z, int bits, uint32_t* code) {
+  if (n < 0 || (n > 0 && (!y || !z || !code)) || bits < 0 || bits > 15) return 0;
+  const float scale = (float)(1 << bits);
+  for (int64_t i = 0; i < n; ++i) {
+    const float v[2] = {y[i], z[i]};
+    uint32_t w = 0;
+    for (int k = 0; k < 2; ++k) {
+      float r = std::rint(v[k] * scale);               // a power of two: the product is exact (short of overflow)
+      if (!(r == r)) r = 0.0f;
+      if (r < -32768.0f) r = -32768.0f;
+      if (r > 32767.0f) r = 32767.0f;
+      w |= (uint32_t)(uint16_t)(int16_t)(int32_t)r << (16 * k);
+    }
+    code[i] = w;
+  }
+  return 1;
+}
+
 int orcRotate(double* state, double* cov, double alpha, double bz_tesla, double max_sinphi, int fp64) {
   return fp64 ? rotateT<double>(state, cov, alpha, bz_tesla, max_sinphi) : rotateT<float>(state, cov, alpha, bz_tesla, max_sinphi);
 }

@@ -111,6 +111,11 @@ void orcGetResiduals(const orcResult*, double* res_y, double* res_z);
  * nearest to q, with every bit more than trunc_bits after its first non-zero bit rounded away.  Returns 0 on bad arguments. */
 int orcPackCharge(int64_t n_values, const float* q, int trunc_bits, uint16_t* code);
 
+/* O11 (rest of NEXT-4, DESIGN.md section 3 "O11"): 16-bit integer format of positions (absolute, or
+ * residuals to the track model): code[i] = y16 | z16 << 16 with v16 = the integer nearest to v * 2^bits (ties to even),
+ * saturated to [-32768, 32767], NaN -> 0.  Returns 0 on bad arguments. */
+int orcPackPositions(int64_t n_values, const float* y, const float* z, int bits, uint32_t* code);
+
 /* Pieces of O7 for the pins.  state = {x, y, z, s, t, q}, cov = 15 lower-triangle elements, in/out as doubles.
  * orcRotate: frame turned by alpha (radians); returns 1 on success, 0 (untouched) on failure.
  * orcMatch: chi2 of the match of outer state a to inner state b (b at plane b_state[0]); rel = 0 same sector,

@@ -78,6 +78,8 @@ def _load():
             getattr(L, f).restype = None
         L.orcPackCharge.argtypes = [i64, vp, ci, vp]
         L.orcPackCharge.restype = ci
+        L.orcPackPositions.argtypes = [i64, vp, vp, ci, vp]
+        L.orcPackPositions.restype = ci
         L.orcGetResiduals.argtypes = [vp] * 3
         L.orcGetResiduals.restype = None
         L.orcGetClusterFlags.argtypes = [vp] * 3
@@ -165,6 +167,7 @@ class OracleResult:
     cf_owner: np.ndarray | None = None
     cf_res_y: np.ndarray | None = None      # track-model residuals of the clusters attached to refitted tracks
     cf_res_z: np.ndarray | None = None
+    cf_res_code: np.ndarray | None = None   # O11: the residuals as 16-bit integers (y16 | z16 << 16), pos_bits of the call
 
     @property
     def n_tracks(self) -> int:
@@ -177,7 +180,7 @@ def _ptr(a):
 
 def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool = False,
         stages_only: bool = False, refit: bool = False, merge: bool = False, flags: bool = False,
-        legs: bool = False) -> OracleResult:
+        legs: bool = False, pos_bits: int = 6) -> OracleResult:
     """Run O1..O5 on an Event-like object (fields n_sectors, n_rows, row_x, row_dead, bz_tesla,
     tan_half_sector, z_min, z_max, row_offset, y, z; numpy arrays)."""
     L = _load()
@@ -245,6 +248,8 @@ def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool 
             rf.update(cf_flags=cf, cf_owner=co, cf_res_y=ry, cf_res_z=rz)
     finally:
         L.orcFree(h)
+    if flags:        # O11: the residuals in the 16-bit integer format
+        rf["cf_res_code"] = pack_positions(rf["cf_res_y"].astype(np.float32), rf["cf_res_z"].astype(np.float32), pos_bits)
     return OracleResult(n, s2o, cell, ncell, ur, dr, u, d, sh, st, nh, fr, lr, rh, tx, tpar, tcov, tchi, kid, ks, kf, kl,
                         kn, kx, kpar, kcov, kchi, koff, kidx, **rf)
 
@@ -318,6 +323,16 @@ def leg_match(a_state, a_cov, d, b_state, b_cov, bz_tesla=0.5, params: Params | 
     ok = _load().orcLegMatch(ctypes.byref(p), float(bz_tesla), a.ctypes.data, ac.ctypes.data, int(d), b.ctypes.data,
                              bc.ctypes.data, int(fp64), chi2.ctypes.data)
     return bool(ok), float(chi2[0])
+
+
+def pack_positions(y, z, bits=6):
+    """O11: positions (or residuals) as 16-bit integers in units of 2^-bits cm; returns uint32 = y16 | z16 << 16."""
+    y = np.ascontiguousarray(y, np.float32)
+    z = np.ascontiguousarray(z, np.float32)
+    code = np.zeros(y.shape[0], np.uint32)
+    if y.shape != z.shape or not _load().orcPackPositions(y.shape[0], _ptr(y), _ptr(z), int(bits), _ptr(code)):
+        raise ValueError("orcPackPositions: bad arguments")
+    return code
 
 
 def pack_charge(q, trunc_bits=4):
