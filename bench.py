@@ -225,7 +225,7 @@ def run_ours(args, rank, world, local_rank):
         dq = torch.from_numpy(ev.q).to(y.device)
         for i in range(4):
             trk.run(off, y, z, cap_tracklets=capT, cap_tracks=capK, cap_track_clusters=capC, sync=False, merge=True, flags=True, q=dq,
-                    legs=True)
+                    legs=True, pos=True)
             s = trk.status()
             if i > 0:
                 acc += float(s.stage_ms[7])
@@ -368,10 +368,12 @@ def run_ours(args, rank, world, local_rank):
                               "links": n_links}
         line["next_legs"] = {"what": "a10 pairs of looper legs (rest of NEXT-1), not part of `value`", "ms": round(legs_ms, 4),
                              "pairs": n_legs}
-        line["next_pack"] = {"what": "a9 dynamic-precision charge code (part of NEXT-4), not part of `value`",
-                             "ms": round(pack_ms, 4), "alg_bytes": 6 * N, "bound": "hbm",
-                             "gbs": round(6 * N / (pack_ms * 1e-3) / 1e9, 1) if pack_ms > 0 else None,
-                             "frac_of_hbm_peak": round(6 * N / (pack_ms * 1e-3) / 1e9 / peak, 4) if pack_ms > 0 else None}
+        pb = 6 * N + 12 * N       # charge: 4 B in, 2 B out; positions: 8 B in, 4 B out
+        line["next_pack"] = {"what": "a9 dynamic-precision charge code and 16-bit position code (NEXT-4), two streaming "
+                                     "kernels, not part of `value`",
+                             "ms": round(pack_ms, 4), "alg_bytes": pb, "bound": "hbm",
+                             "gbs": round(pb / (pack_ms * 1e-3) / 1e9, 1) if pack_ms > 0 else None,
+                             "frac_of_hbm_peak": round(pb / (pack_ms * 1e-3) / 1e9 / peak, 4) if pack_ms > 0 else None}
         line["next_flags"] = {"what": "a8 cluster flags and rejection strategies A / B (NEXT-3), not part of `value`",
                               "ms": round(flags_ms, 4), "fractions_of_clusters": flag_frac}
     print(json.dumps(line), flush=True)

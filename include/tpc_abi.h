@@ -85,6 +85,7 @@ typedef struct {
   int32_t leg_max_sectors;      /* 4          O10: the two ends of a turn are at most this many sectors apart (0..8) */
   int32_t leg_max_row_diff;     /* 12         O10: and their last rows at most this many rows */
   float leg_max_centre_dist;    /* 10         O10: and the centres of their circles at most this far apart, cm */
+  int32_t pos_bits;             /* 6          O11: positions and residuals are stored in units of 2^-pos_bits cm (0..15) */
 } tpcParams;
 
 /* Input clusters: CSR by (sector,row), fp32 SoA (single-precision cluster properties). */
@@ -158,6 +159,11 @@ typedef struct {
   /* optional O9 dynamic-precision charge code (DESIGN.md section 3 "O9"); needs tpcClusters.q */
   uint16_t* cl_qcode;           /* [n_clusters] integer charge with all bits beyond charge_trunc_bits after the first
                                    non-zero bit rounded away; NULL = not computed */
+  /* optional O11 16-bit integer format (DESIGN.md section 3 "O11"): y16 | z16 << 16 per cluster, v16 = the
+   * integer nearest to v * 2^pos_bits (ties to even), saturated to [-32768, 32767] */
+  uint32_t* cl_pos_code;        /* [n_clusters] code of the absolute (y, z) of every cluster; NULL = not computed */
+  uint32_t* cl_res_code;        /* [n_clusters] code of the track-model residuals (0 where there is none); needs cl_flags and
+                                   cl_owner (and with them the refit outputs); NULL = not computed */
 } tpcTracks;
 
 /* Filled by tpcGetRunStatus after the stream has drained. */
@@ -175,7 +181,7 @@ typedef struct {
                                    0 grid, 1 neighbour finder, 2 cleaner+start hits, 3 constructor, 4 selector,
                                    5 optional refit, merger and exports, 6 total, 7 refit alone */
   float merge_ms;               /* the O7 merger alone (profiling on, merger requested) */
-  float pack_ms;                /* the O9 charge code alone (profiling on, cl_qcode requested) */
+  float pack_ms;                /* the O9 charge code and the O11 position code alone (profiling on, cl_qcode / cl_pos_code requested) */
   float flags_ms;               /* the O8 cluster flags alone (profiling on, flags requested) */
   float legs_ms;                /* the O10 leg pairs alone (profiling on, legs requested) */
   float submit_ms[2];           /* tpcCollectHost only: device time of the slot from its first copy in to the end of its

@@ -219,7 +219,7 @@ int tpcDefaultParams(tpcParams* p) {
   p->merge_max_row_gap = 40; p->merge_back_rows = 5; p->merge_chi2_max = 50.0f;
   p->tube_radius = 1.5f; p->inv_pt_protect = 20.0f; p->charge_trunc_bits = 4;
   p->leg_min_sinphi = 0.5f; p->leg_chi2_max = 50.0f; p->leg_max_sectors = 4; p->leg_max_row_diff = 12;
-  p->leg_max_centre_dist = 10.0f;
+  p->leg_max_centre_dist = 10.0f; p->pos_bits = 6;
   return TPC_OK;
 }
 
@@ -235,6 +235,7 @@ int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cud
   if (p->min_chain_hits < 2 || p->max_row_gap < 0) return TPC_ERR_INVALID_ARG;
   if (p->merge_max_row_gap < 0 || p->merge_back_rows < 0) return TPC_ERR_INVALID_ARG;
   if (!(p->tube_radius >= 0) || p->charge_trunc_bits < 0 || p->charge_trunc_bits > 14) return TPC_ERR_INVALID_ARG;
+  if (p->pos_bits < 0 || p->pos_bits > 15) return TPC_ERR_INVALID_ARG;
   if (p->leg_max_sectors < 0 || p->leg_max_sectors > LEG_MAX_SECTORS || p->leg_max_row_diff < 0) return TPC_ERR_INVALID_ARG;
   tpcHandle* h = new (std::nothrow) tpcHandle();
   if (!h) return TPC_ERR_INVALID_ARG;
@@ -361,6 +362,7 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   const int n_fl = (out->cl_flags != nullptr) + (out->cl_owner != nullptr);
   if ((n_fl != 0 && n_fl != 2) || (n_fl == 2 && n_rf != 8)) return TPC_ERR_INVALID_ARG;   // so do the cluster flags
   if ((out->cl_res_y != nullptr) != (out->cl_res_z != nullptr) || (out->cl_res_y && n_fl != 2)) return TPC_ERR_INVALID_ARG;
+  if (out->cl_res_code && n_fl != 2) return TPC_ERR_INVALID_ARG;                         // the residual code rides on the flag pass
   if (!workspace || ((uintptr_t)workspace % ALIGN) != 0) return TPC_ERR_INVALID_ARG;
   const Workspace w = layout(h, N, capT, (char*)workspace);
   if (workspace_bytes < w.bytes) return TPC_ERR_WORKSPACE_TOO_SMALL;
@@ -552,6 +554,7 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   if (n_fl == 2 && N > 0) {
     TPC_CUDA(h, cudaMemsetAsync(w.fl_key, 0xFF, 8 * (size_t)N, st)); ++L;
     TPC_CUDA(h, cudaMemsetAsync(out->cl_flags, 0, (size_t)N, st)); ++L;
+    if (out->cl_res_code) { TPC_CUDA(h, cudaMemsetAsync(out->cl_res_code, 0, 4 * (size_t)N, st)); ++L; }
     if (out->cl_res_y) {
       TPC_CUDA(h, cudaMemsetAsync(out->cl_res_y, 0, 4 * (size_t)N, st)); ++L;
       TPC_CUDA(h, cudaMemsetAsync(out->cl_res_z, 0, 4 * (size_t)N, st)); ++L;
@@ -562,7 +565,7 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
       const int64_t nk = std::min<int64_t>(out->cap_tracks, capT);
       // the walking states of the attached clusters, one float2 per track-cluster entry: the selector's owner keys
       // (8 bytes per cluster, dead since selectEmit) are the buffer
-      float2* walk_yz = out->cl_res_y ? reinterpret_cast<float2*>(w.owner_key) : nullptr;
+      float2* walk_yz = (out->cl_res_y || out->cl_res_code) ? reinterpret_cast<float2*>(w.owner_key) : nullptr;
       const int64_t n_ent = std::min<int64_t>(out->cap_track_clusters, N);
       if (walk_yz) { TPC_CUDA(h, cudaMemsetAsync(walk_yz, 0xFF, 8 * (size_t)n_ent, st)); ++L; }
       flagAttach<<<(unsigned)ceilDiv(std::min<int64_t>(out->cap_track_clusters, N), 256), 256, 0, st>>>(out->trk_cl_index,
@@ -572,7 +575,7 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
                                                           w.fl_key, walk_yz, cnt); ++L;
       if (walk_yz) {
         flagResiduals<<<(unsigned)ceilDiv(n_ent, 256), 256, 0, st>>>(out->trk_cl_index, walk_yz, in->y, in->z, out->cl_res_y,
-                                                                    out->cl_res_z, cnt); ++L;
+                                                                    out->cl_res_z, out->cl_res_code, h->params.pos_bits, cnt); ++L;
       }
     }
     flagFinish<<<gN256, 256, 0, st>>>(N, w.fl_key, out->cl_flags, out->cl_owner, cnt); ++L;
@@ -582,6 +585,9 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   stage(13);
   if (out->cl_qcode && N > 0) {
     packCharge<<<(unsigned)ceilDiv(ceilDiv(N, 8), 256), 256, 0, st>>>(N, in->q, h->params.charge_trunc_bits, out->cl_qcode); ++L;
+  }
+  if (out->cl_pos_code && N > 0) {    // O11 of the absolute positions
+    packPositions<<<(unsigned)ceilDiv(ceilDiv(N, 4), 256), 256, 0, st>>>(N, in->y, in->z, h->params.pos_bits, out->cl_pos_code); ++L;
   }
   stage(14);
   // ---- optional per-stage exports -----------------------------------------------------------------
@@ -670,7 +676,7 @@ extern "C" int tpcRunHost(tpcHandle* h, int64_t N, const uint32_t* row_offset, c
       oh->tl_first_row || oh->tl_last_row || oh->tl_rowhit || oh->tl_x || oh->tl_par || oh->tl_cov || oh->tl_chi2 ||
       oh->trk_rf_status || oh->trk_rf_x_in || oh->trk_rf_par_in || oh->trk_rf_cov_in || oh->trk_rf_chi2 || oh->trk_rf_x_out ||
       oh->trk_rf_par_out || oh->trk_rf_cov_out || oh->trk_mg_next || oh->trk_mg_prev || oh->trk_mg_head || oh->trk_mg_chi2 ||
-      oh->trk_leg_partner || oh->trk_leg_chi2 || oh->cl_flags || oh->cl_owner || oh->cl_qcode || oh->cl_res_y || oh->cl_res_z)
+      oh->trk_leg_partner || oh->trk_leg_chi2 || oh->cl_flags || oh->cl_owner || oh->cl_qcode || oh->cl_res_y || oh->cl_res_z || oh->cl_pos_code || oh->cl_res_code)
     return TPC_ERR_INVALID_ARG;
   if (!oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0) return TPC_ERR_INVALID_ARG;
   TPC_CUDA(h, cudaSetDevice(h->device));
@@ -780,7 +786,7 @@ extern "C" int tpcSubmitHost(tpcHandle* h, int slot, int64_t N, const uint32_t* 
     return TPC_ERR_INVALID_ARG;
   if (oh->link_up_raw || oh->link_dn_raw || oh->link_up || oh->link_dn || oh->start_hits || oh->tl_status || oh->tl_nhits ||
       oh->tl_first_row || oh->tl_last_row || oh->tl_rowhit || oh->tl_x || oh->tl_par || oh->tl_cov || oh->tl_chi2 ||
-      oh->trk_rf_status || oh->trk_mg_next || oh->trk_leg_partner || oh->trk_leg_chi2 || oh->cl_flags || oh->cl_owner || oh->cl_qcode || oh->cl_res_y || oh->cl_res_z || !oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0)
+      oh->trk_rf_status || oh->trk_mg_next || oh->trk_leg_partner || oh->trk_leg_chi2 || oh->cl_flags || oh->cl_owner || oh->cl_qcode || oh->cl_res_y || oh->cl_res_z || oh->cl_pos_code || oh->cl_res_code || !oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0)
     return TPC_ERR_INVALID_ARG;
   TPC_CUDA(h, cudaSetDevice(h->device));
   int rc;

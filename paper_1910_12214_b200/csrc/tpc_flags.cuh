@@ -97,11 +97,22 @@ __global__ void __launch_bounds__(128) flagBid(FlagIn in, const uint32_t* __rest
   }
 }
 
+// O11 (rest of NEXT-4; DESIGN.md section 3 "O11", reading R45): a position or residual in units of
+// 2^-pos_bits cm as a 16-bit integer: nearest (ties to even), saturated, NaN -> 0; two per word, y16 | z16 << 16
+__device__ __forceinline__ uint32_t posCode16(float v, float scale) {
+  float r = rintf(v * scale);
+  if (!(r == r)) r = 0.0f;
+  r = fminf(fmaxf(r, -32768.0f), 32767.0f);
+  return (uint32_t)(uint16_t)(int16_t)(int32_t)r;
+}
+__device__ __forceinline__ uint32_t posCode(float y, float z, float scale) { return posCode16(y, scale) | (posCode16(z, scale) << 16); }
+
 // thread per track-cluster entry: res = cluster - walking state of its track on its row (R39); entries the walk did not
 // reach (refused Propagate, track not refitted) still hold the NaN pattern the buffer was filled with
 __global__ void __launch_bounds__(256) flagResiduals(const uint32_t* __restrict__ cl_index, const float2* __restrict__ walk_yz,
                                                      const float* __restrict__ yin, const float* __restrict__ zin,
                                                      float* __restrict__ res_y, float* __restrict__ res_z,
+                                                     uint32_t* __restrict__ res_code, int pos_bits,
                                                      const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
   const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -109,7 +120,9 @@ __global__ void __launch_bounds__(256) flagResiduals(const uint32_t* __restrict_
   const float2 w = walk_yz[i];
   if (!(w.x == w.x)) return;
   const uint32_t c = cl_index[i];
-  res_y[c] = yin[c] - w.x; res_z[c] = zin[c] - w.y;
+  const float ry = yin[c] - w.x, rz = zin[c] - w.y;
+  if (res_y) { res_y[c] = ry; res_z[c] = rz; }
+  if (res_code) res_code[c] = posCode(ry, rz, (float)(1 << pos_bits));       // O11
 }
 
 // thread per cluster: key -> flag byte and owner
@@ -159,6 +172,22 @@ __global__ void __launch_bounds__(256) packCharge(int64_t N, const float* __rest
     __stcs(reinterpret_cast<uint4*>(code + i8), o);
   } else {
     for (int64_t i = i8; i < min(i8 + 8, N); ++i) code[i] = (uint16_t)packOne(q[i], nb);
+  }
+}
+
+// O11 of the absolute positions.  Streaming: 8 bytes in, 4 bytes out per cluster; four clusters per thread.
+__global__ void __launch_bounds__(256) packPositions(int64_t N, const float* __restrict__ y, const float* __restrict__ z,
+                                                     int pos_bits, uint32_t* __restrict__ code) {
+  const int64_t i4 = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) * 4;
+  if (i4 >= N) return;
+  const float scale = (float)(1 << pos_bits);
+  if (i4 + 4 <= N && (((uintptr_t)y | (uintptr_t)z | (uintptr_t)code) & 15) == 0) {
+    const float4 a = __ldcs(reinterpret_cast<const float4*>(y + i4));
+    const float4 b = __ldcs(reinterpret_cast<const float4*>(z + i4));
+    __stcs(reinterpret_cast<uint4*>(code + i4),
+           make_uint4(posCode(a.x, b.x, scale), posCode(a.y, b.y, scale), posCode(a.z, b.z, scale), posCode(a.w, b.w, scale)));
+  } else {
+    for (int64_t i = i4; i < min(i4 + 4, N); ++i) code[i] = posCode(y[i], z[i], scale);
   }
 }
 

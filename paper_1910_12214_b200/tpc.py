@@ -39,7 +39,7 @@ class tpcParams(ctypes.Structure):
                 ("merge_back_rows", c_int32), ("merge_chi2_max", c_float), ("tube_radius", c_float),
                 ("inv_pt_protect", c_float), ("charge_trunc_bits", c_int32), ("leg_min_sinphi", c_float),
                 ("leg_chi2_max", c_float), ("leg_max_sectors", c_int32), ("leg_max_row_diff", c_int32),
-                ("leg_max_centre_dist", c_float)]
+                ("leg_max_centre_dist", c_float), ("pos_bits", c_int32)]
 
 
 class tpcClusters(ctypes.Structure):
@@ -57,11 +57,12 @@ _MERGE_PTRS = ("trk_mg_next", "trk_mg_prev", "trk_mg_head", "trk_mg_chi2")
 _LEG_PTRS = ("trk_leg_partner", "trk_leg_chi2")
 _FLAG_PTRS = ("cl_flags", "cl_owner", "cl_res_y", "cl_res_z")
 _PACK_PTRS = ("cl_qcode",)
+_POS_PTRS = ("cl_pos_code", "cl_res_code")
 
 
 class tpcTracks(ctypes.Structure):
     _fields_ = [("cap_tracks", c_int64), ("cap_track_clusters", c_int64)] + \
-               [(n, c_void_p) for n in _TRK_PTRS + _STAGE_PTRS + _REFIT_PTRS + _MERGE_PTRS + _LEG_PTRS + _FLAG_PTRS + _PACK_PTRS]
+               [(n, c_void_p) for n in _TRK_PTRS + _STAGE_PTRS + _REFIT_PTRS + _MERGE_PTRS + _LEG_PTRS + _FLAG_PTRS + _PACK_PTRS + _POS_PTRS]
 
 
 class tpcRunStatus(ctypes.Structure):
@@ -238,7 +239,7 @@ class TpcTracker:
         z = t.from_numpy(np.ascontiguousarray(ev.z, np.float32)).to(self.device)
         return off, y, z
 
-    def _ensure(self, n, capT, capK, capC, stages, refit=False, merge=False, flags=False, pack=False, legs=False):
+    def _ensure(self, n, capT, capK, capC, stages, refit=False, merge=False, flags=False, pack=False, legs=False, pos=False):
         t = self.torch
         need = tpcWorkspaceBytes(self.handle, n, capT)
         if self._ws is None or self._ws.numel() < need:
@@ -269,6 +270,10 @@ class TpcTracker:
         if merge:
             spec.update({"trk_mg_next": ((capK,), i32), "trk_mg_prev": ((capK,), i32), "trk_mg_head": ((capK,), i32),
                          "trk_mg_chi2": ((capK,), f32)})
+        if pos:
+            spec.update({"cl_pos_code": ((max(n, 1),), i32)})
+            if flags:
+                spec.update({"cl_res_code": ((max(n, 1),), i32)})
         if legs:
             spec.update({"trk_leg_partner": ((capK,), i32), "trk_leg_chi2": ((capK,), f32)})
         for k, (shape, dt) in spec.items():
@@ -282,7 +287,7 @@ class TpcTracker:
     def run(self, row_offset, y, z, cap_tracklets: int | None = None, cap_tracks: int | None = None,
             cap_track_clusters: int | None = None, stages: bool = False, stream=None, sync: bool = True,
             grow: bool = True, refit: bool = False, merge: bool = False, flags: bool = False, q=None,
-            legs: bool = False):
+            legs: bool = False, pos: bool = False):
         """One tpcRun on device tensors (q: optional device tensor of charges -> cl_qcode, the O9 charge code).  Returns a TrackResult (after synchronising) or None when sync=False."""
         t = self.torch
         n = int(y.shape[0])
@@ -292,7 +297,7 @@ class TpcTracker:
         capC = int(cap_track_clusters) if cap_track_clusters is not None else max(n, 1)
         attempts = 3 if grow else 0     # a too-small cap_tracklets hides the true track counts: up to 3 rounds
         while True:
-            self._ensure(n, capT, capK, capC, stages, refit, merge, flags, q is not None, legs)
+            self._ensure(n, capT, capK, capC, stages, refit, merge, flags, q is not None, legs, pos)
             cl = tpcClusters(n, row_offset.data_ptr(), None, y.data_ptr() if n else None, z.data_ptr() if n else None,
                              q.data_ptr() if (q is not None and n) else None)
             tr = tpcTracks()
@@ -334,6 +339,10 @@ class TpcTracker:
                 trk[k] = o[k][:n]
         if q is not None:
             trk["cl_qcode"] = o["cl_qcode"][:n]
+        if pos:            # O11: 16-bit integer positions, and residuals when the flags are on
+            trk["cl_pos_code"] = o["cl_pos_code"][:n]
+            if flags:
+                trk["cl_res_code"] = o["cl_res_code"][:n]
         stg = {}
         if stages:
             for k in _STAGE_PTRS:

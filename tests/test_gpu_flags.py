@@ -104,6 +104,45 @@ def test_charge_code_golden_fixture():
         trk.close()
 
 
+@pytest.mark.parametrize("bits", [6, 0, 9, 15])
+def test_position_and_residual_code_parity(bits):
+    """O11: the 16-bit integer codes of the absolute positions and of the track-model residuals,
+    bit-exact; the positions are overwritten in places with ties (half units), values beyond the range, NaN-free
+    infinities are not valid tracker input, so the extreme values ride on a tracker-free call at the end."""
+    import torch
+    from paper_1910_12214_b200 import tpc
+    ev = datagen.make_event(2, scale=0.05)
+    p, po = tpc.tpcDefaultParams(), orc.default_params()
+    p.pos_bits = bits
+    trk = tpc.TpcTracker.from_event(ev, params=p)
+    off, y, z = trk.upload(ev)
+    res = trk.run(off, y, z, flags=True, pos=True)
+    assert res.status.status == 0
+    g = res.numpy()
+    o = orc.run(ev, po, flags=True, pos_bits=bits)
+    assert np.array_equal(g["cl_pos_code"].view(np.uint32), orc.pack_positions(ev.y, ev.z, bits))
+    assert np.array_equal(g["cl_res_y"], o.cf_res_y.astype(np.float32))
+    assert np.array_equal(g["cl_res_code"].view(np.uint32), o.cf_res_code)
+    assert (o.cf_res_code != 0).sum() > 1000 or bits == 0
+    # positions alone (no flags, no refit): ties, saturation and a ragged tail (n not a multiple of 4)
+    n = ev.n_clusters - (ev.n_clusters % 4) - 1
+    off2 = ev.row_offset.copy().astype(np.int64)
+    off2 = np.minimum(off2, n).astype(np.uint32)
+    rng = np.random.default_rng(9)
+    unit = 2.0 ** -bits
+    yy = (rng.integers(-40000, 40000, n) * 0.5 * unit).astype(np.float32)          # half units: every second one a tie
+    zz = rng.uniform(-600, 600, n).astype(np.float32)
+    ev2 = datagen.event_from_arrays(off2, yy, zz, ev.n_sectors, ev.n_rows)
+    off, y, z = trk.upload(ev2)
+    res = trk.run(off, y, z, pos=True)
+    assert np.array_equal(res.numpy()["cl_pos_code"].view(np.uint32), orc.pack_positions(yy, zz, bits))
+    trk.close()
+    bad = tpc.tpcDefaultParams()
+    bad.pos_bits = 16
+    with pytest.raises(tpc.TpcError):
+        tpc.TpcTracker.from_event(ev, params=bad)
+
+
 def test_optional_stages_on_empty_and_overflowing_inputs():
     """All optional stages requested on an empty event, on a rows-only event without tracks and with too small track
     capacities: defined status, nothing written out of bounds (guard values around the outputs stay intact)."""
