@@ -31,7 +31,10 @@ __global__ void __launch_bounds__(256) flagAttach(const uint32_t* __restrict__ c
   flags[cl_index[i]] = 1;
 }
 
-constexpr int FLAG_GROUP = 8;      // lanes per track
+#ifndef FLAG_GROUP_
+#define FLAG_GROUP_ 4
+#endif
+constexpr int FLAG_GROUP = FLAG_GROUP_;      // lanes per track
 
 __global__ void __launch_bounds__(128) flagBid(FlagIn in, const uint32_t* __restrict__ off, DevParams P, RowTables T,
                                                float tube, float inv_pt_protect, const GridDesc* __restrict__ desc,
