@@ -37,6 +37,13 @@ NCU_R1 = {(4, "a4_constructor"): {"kernel": "trackletConstructor", "warp_inst": 
           (4, "a2_neighbours"): {"kernel": "neighbourFinder", "warp_inst": 1.1833e10, "dram_bytes": 1607099000}}
 
 
+# O4 operations per hit of the accepted tracklets on config 4 (oracle/count_o4_ops.py, sectors 0 / 7 / 20 agree to 0.5 %):
+# Propagate, Update, Search, clusters inside the roads; and the fp32 operations of each as DESIGN.md section 3 writes them
+# (adds, multiplies, divisions, square roots each counted once; R0: nothing is fused): DESIGN.md section 8.
+O4_OPS_PER_HIT = {4: (1.515, 1.443, 1.020, 1.444)}
+O4_FLOPS = (176, 100, 6, 5)
+
+
 def _peaks():
     p = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(p):
@@ -305,14 +312,30 @@ def run_ours(args, rank, world, local_rank):
         # achieved = warp instructions of one launch (ncu smsp__inst_executed.sum of the committed capture of this
         # workload) / the live CUDA-event time of the stage; peak = SMs x 4 schedulers x 1 instruction/clock x max SM clock.
         sm_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
-        alu_peak = ALU_SMS * 4 * sm_mhz * 1e6 / 1e9
-        achieved = ncu["warp_inst"] / (dom_ms * 1e-3) / 1e9
-        roofline = {"bound": "alu", "kernel": ncu["kernel"], "achieved": round(achieved, 2), "peak": round(alu_peak, 1),
-                    "unit": "Gwarp-inst/s", "frac": round(achieved / alu_peak, 5), "traffic": ncu["dram_bytes"],
-                    "peak_source": f"{ALU_SMS} SMs x 4 schedulers x {sm_mhz:.0f} MHz (B200_PROFILING.md unit counts and clocks)",
-                    "alg_bytes": int(alg[dom]), "alg_gbs": round(alg[dom] / (dom_ms * 1e-3) / 1e9, 1),
-                    "alg_frac_of_hbm_peak": round(alg[dom] / (dom_ms * 1e-3) / 1e9 / peak, 5),
-                    "counts_from": "profiles/r1j_full_capture.md", "whole_path": whole, "share_of_step": share}
+        issue_peak = ALU_SMS * 4 * sm_mhz * 1e6 / 1e9
+        issued = ncu["warp_inst"] / (dom_ms * 1e-3) / 1e9
+        issue = {"achieved": round(issued, 2), "peak": round(issue_peak, 1), "unit": "Gwarp-inst/s",
+                 "frac": round(issued / issue_peak, 5), "counts_from": "profiles/r1j_full_capture.md",
+                 "peak_source": f"{ALU_SMS} SMs x 4 schedulers x {sm_mhz:.0f} MHz"}
+        common = {"traffic": ncu["dram_bytes"], "alg_bytes": int(alg[dom]),
+                  "alg_gbs": round(alg[dom] / (dom_ms * 1e-3) / 1e9, 1),
+                  "alg_frac_of_hbm_peak": round(alg[dom] / (dom_ms * 1e-3) / 1e9 / peak, 5),
+                  "issue": issue, "whole_path": whole, "share_of_step": share}
+        per_hit = O4_OPS_PER_HIT.get(args.config) if dom == "a4_constructor" else None
+        if per_hit is not None:
+            # algorithmic fp32 operations of one launch = tracklet hits x (O4 operations per hit x operations each), against
+            # the non-fused fp32 peak: SMs x 128 lanes x 1 operation / clock (R0 forbids the FMA that doubles it)
+            flops = H * sum(a * b for a, b in zip(per_hit, O4_FLOPS))
+            alu_peak = ALU_SMS * 128 * sm_mhz * 1e6 / 1e12
+            achieved = flops / (dom_ms * 1e-3) / 1e12
+            roofline = {"bound": "alu", "kernel": ncu["kernel"], "achieved": round(achieved, 3), "peak": round(alu_peak, 2),
+                        "unit": "TFLOP/s", "frac": round(achieved / alu_peak, 5), "alg_flops": int(flops),
+                        "flops_per_tracklet_hit": round(flops / max(H, 1), 1),
+                        "peak_source": f"{ALU_SMS} SMs x 128 fp32 lanes x {sm_mhz:.0f} MHz, no FMA (B200_PROFILING.md unit "
+                                       "counts and clocks; DESIGN.md section 8)", **common}
+        else:
+            roofline = {"bound": "alu", "kernel": ncu["kernel"], "achieved": issue["achieved"], "peak": issue["peak"],
+                        "unit": issue["unit"], "frac": issue["frac"], "peak_source": issue["peak_source"], **common}
     else:
         achieved = alg[dom] / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0
         roofline = {"bound": "hbm", "kernel": dom, "achieved": round(achieved, 2), "peak": peak, "unit": "GB/s",

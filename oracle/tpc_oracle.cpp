@@ -246,6 +246,7 @@ struct orcResult {
   // outer = state at the last kept cluster (up pass)
   std::vector<int32_t> rf_status;
   std::vector<double> rf_x_in, rf_par_in, rf_cov_in, rf_chi2, rf_x_out, rf_par_out, rf_cov_out;
+  int64_t o4_ops[4] = {0, 0, 0, 0};   // Propagates, Updates, Searches, clusters inside the roads (O4)
   // O7 merger (NEXT-1)
   std::vector<int32_t> mg_next, mg_prev, mg_head;
   std::vector<double> mg_chi2;
@@ -415,7 +416,11 @@ struct Tracker {
   }
 
   // ---- O4 ----------------------------------------------------------------------------------------
+  // ops: how often O4 ran a Propagate, an Update, a Search, and how many clusters the Searches found inside their roads
+  // (plain counters for the measurement's algorithmic operation count; no arithmetic depends on them)
+  mutable int64_t ops[4] = {0, 0, 0, 0};
   int32_t search(int b, const State<Real>& st) const {
+    ++ops[2];
     Real ry = (Real)P.road_sigma * std::sqrt(st.C[0] + (Real)P.err2_y);
     Real rz = (Real)P.road_sigma * std::sqrt(st.C[2] + (Real)P.err2_z);
     if (!(ry >= (Real)P.road_min)) ry = (Real)P.road_min;
@@ -424,6 +429,7 @@ struct Tracker {
     if (rz > (Real)P.road_max) rz = (Real)P.road_max;
     int32_t best = -1; Real bestd = 0;
     forWindow(b, st.y, st.z, ry, rz, [&](int32_t c) {
+      ++ops[3];
       const Real dy = Y[c] - st.y, dz = Z[c] - st.z;
       const Real d2 = dy * dy + dz * dz;
       if (best < 0 || d2 < bestd || (d2 == bestd && c < best)) { best = c; bestd = d2; }
@@ -659,9 +665,9 @@ struct Tracker {
     // 2. chain fit
     for (int32_t h = h1; h != -1;) {
       const int r = rowOf[h];
-      if (!propagate(st, X[r], b, msp)) break;
+      ++ops[0]; if (!propagate(st, X[r], b, msp)) break;
       rc = r;
-      if (!update(st, Y[h], Z[h], e2y, e2z)) break;
+      ++ops[1]; if (!update(st, Y[h], Z[h], e2y, e2z)) break;
       T.rowhit[r] = h; ++nhits;
       h = res.up[h];
     }
@@ -670,10 +676,10 @@ struct Tracker {
     int miss = 0;
     for (int r = rc + 1; r < R; ++r) {
       if (dead(r)) continue;                       // R23
-      if (!propagate(st, X[r], b, msp)) break;
+      ++ops[0]; if (!propagate(st, X[r], b, msp)) break;
       const int32_t c = search(s * R + r, st);
       if (c >= 0) {
-        if (!update(st, Y[c], Z[c], e2y, e2z)) break;
+        ++ops[1]; if (!update(st, Y[c], Z[c], e2y, e2z)) break;
         T.rowhit[r] = c; ++nhits; miss = 0;
       } else if (++miss > P.max_row_gap) break;
     }
@@ -688,12 +694,12 @@ struct Tracker {
     miss = 0;
     for (int r = rtop; r >= 0; --r) {
       if (dead(r)) continue;
-      if (!propagate(st, X[r], b, msp)) break;
+      ++ops[0]; if (!propagate(st, X[r], b, msp)) break;
       int32_t c = T.rowhit[r];
       const bool known = c != -1;
       if (!known) c = search(s * R + r, st);
       if (c >= 0) {
-        if (!update(st, Y[c], Z[c], e2y, e2z)) break;
+        ++ops[1]; if (!update(st, Y[c], Z[c], e2y, e2z)) break;
         if (!known) T.rowhit[r] = c;
         ++nh; snap = st; snap_row = r; snap_nh = nh;
         if (r < r0) miss = 0;
@@ -731,6 +737,7 @@ struct Tracker {
       res.tl_chi2[t] = (double)T.st.chi2;
       chi2r[t] = T.st.chi2;
     }
+    for (int i = 0; i < 4; ++i) res.o4_ops[i] = ops[i];
     // ---- O5 selector: owner(c) = best-priority accepted tracklet containing c -----------------------
     std::vector<int32_t> owner(N, -1);
     auto better = [&](int32_t a, int32_t bb) {   // is tracklet a of higher priority than bb ? (R19)
@@ -823,6 +830,7 @@ void orcGetGrid(const orcResult* r, uint32_t* s2o, int32_t* cell, int32_t* ncell
 void orcGetLinks(const orcResult* r, int32_t* ur, int32_t* dr, int32_t* u, int32_t* d) {
   copyOut(ur, r->up_raw); copyOut(dr, r->dn_raw); copyOut(u, r->up); copyOut(d, r->dn);
 }
+void orcGetO4Counts(const orcResult* r, int64_t* four) { for (int i = 0; i < 4; ++i) four[i] = r->o4_ops[i]; }
 void orcGetStartHits(const orcResult* r, uint32_t* sh) { copyOut(sh, r->start_hits); }
 void orcGetRefit(const orcResult* r, int32_t* status, double* x_in, double* par_in, double* cov_in, double* chi2,
                  double* x_out, double* par_out, double* cov_out) {

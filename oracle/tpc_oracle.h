@@ -73,6 +73,9 @@ void orcGetGrid(const orcResult*, uint32_t* sorted_to_orig, int32_t* cell_of_sor
 /* O2/O3: links, global original indices, -1 none */
 void orcGetLinks(const orcResult*, int32_t* up_raw, int32_t* dn_raw, int32_t* up, int32_t* dn);
 void orcGetStartHits(const orcResult*, uint32_t* start_hits);
+/* How often O4 ran Propagate, Update, Search, and how many clusters its Searches found inside their roads (four counts):
+ * the algorithmic operation count of the measurement. */
+void orcGetO4Counts(const orcResult*, int64_t* four);
 /* O4: one entry per start hit (tracklet id = rank).  status: 0 discarded in the chain fit,
  * 1 built but rejected (nhits < min_tracklet_hits or no snapshot), 2 accepted.
  * rowhit [n_start*n_rows] global indices / -1; x [n_start]; par [n_start*5]; cov [n_start*15]. */

@@ -71,6 +71,8 @@ def _load():
             getattr(L, f).restype = i64
         L.orcGetGrid.argtypes = [vp] * 4
         L.orcGetLinks.argtypes = [vp] * 5
+        L.orcGetO4Counts.argtypes = [vp] * 2
+        L.orcGetO4Counts.restype = None
         L.orcGetStartHits.argtypes = [vp] * 2
         L.orcGetTracklets.argtypes = [vp] * 10
         L.orcGetTracks.argtypes = [vp] * 12
@@ -168,6 +170,7 @@ class OracleResult:
     cf_res_y: np.ndarray | None = None      # track-model residuals of the clusters attached to refitted tracks
     cf_res_z: np.ndarray | None = None
     cf_res_code: np.ndarray | None = None   # O11: the residuals as 16-bit integers (y16 | z16 << 16), pos_bits of the call
+    o4_ops: np.ndarray | None = None        # O4: Propagates, Updates, Searches, clusters inside the roads (counters only)
 
     @property
     def n_tracks(self) -> int:
@@ -223,6 +226,9 @@ def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool 
         L.orcGetTracks(h, _ptr(kid), _ptr(ks), _ptr(kf), _ptr(kl), _ptr(kn), _ptr(kx), _ptr(kpar), _ptr(kcov),
                        _ptr(kchi), _ptr(koff), _ptr(kidx))
         rf = {}
+        ops = np.zeros(4, np.int64)
+        L.orcGetO4Counts(h, _ptr(ops))
+        rf["o4_ops"] = ops
         refit = refit or merge or flags or legs
         if refit:
             rst = np.zeros(nt, np.int32)

@@ -40,6 +40,22 @@ def test_noise_free_high_pt_helices_are_fully_found():
     assert n_found >= 35
 
 
+def test_o4_operation_counters_of_one_full_length_track():
+    """The O4 counters behind bench.py's algorithmic operation count, on a case the algorithm fixes:
+    one noise-free track with a cluster on each of the n = 152 rows.  The end rows have no (up, down) pair, so the chain
+    runs over rows 1..n-2: n-3 Propagate + Update in the chain fit, one Propagate + Search + Update for row n-1 going up,
+    then n Propagates and n Updates going down with one Search (row 0): 2n-2, 2n-2, 2 Searches, 2 clusters inside the roads."""
+    n_checked = 0
+    for seed in range(1, 21):
+        ev = datagen.generate(_single_sector_cfg(seed, 1, 1.0, 10.0, 0.0))
+        if ev.n_clusters != R or np.any(np.diff(ev.row_offset.astype(np.int64)) != 1):
+            continue
+        res = orc.run(ev)
+        assert res.o4_ops.tolist() == [2 * R - 2, 2 * R - 2, 2, 2], seed
+        n_checked += 1
+    assert n_checked >= 10
+
+
 def test_exact_helix_through_the_whole_pipeline_fp64():
     """north_star check 3 through orcRun (fp64 arithmetic on fp32-rounded coordinates)."""
     checked = 0
