@@ -95,18 +95,42 @@ __global__ void __launch_bounds__(SCAN_THREADS) scanApply(const T* in, T* out, c
   T v[SCAN_ITEMS];
   T s = 0;
   const int64_t first = base + (int64_t)threadIdx.x * SCAN_ITEMS;
+  // a thread's items are SCAN_ITEMS * sizeof(T) consecutive bytes: 16-byte loads and stores wherever the whole run is
+  // inside the array and the arrays are 16-byte aligned (always, for the workspace arrays of this library)
+  constexpr int VEC = 16 / sizeof(T);
+  const bool whole = first + SCAN_ITEMS <= n && ((reinterpret_cast<uintptr_t>(in) | reinterpret_cast<uintptr_t>(out)) & 15) == 0;
+  if (whole) {
 #pragma unroll
-  for (int k = 0; k < SCAN_ITEMS; ++k) {
-    v[k] = (first + k < n) ? in[first + k] : T(0);
-    s += v[k];
+    for (int k = 0; k < SCAN_ITEMS; k += VEC) {
+      const uint4 q = *reinterpret_cast<const uint4*>(in + first + k);
+      memcpy(&v[k], &q, 16);
+    }
+  } else {
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) v[k] = (first + k < n) ? in[first + k] : T(0);
   }
+#pragma unroll
+  for (int k = 0; k < SCAN_ITEMS; ++k) s += v[k];
   T total;
   T ex = blockExclusiveScan(s, sm, &total) + tile_off[blockIdx.x];
+  if (whole) {
+    T o[SCAN_ITEMS];
 #pragma unroll
-  for (int k = 0; k < SCAN_ITEMS; ++k) {
-    if (first + k < n) out[first + k] = ex;
-    ex += v[k];
-    if (first + k == n - 1) out[n] = ex;
+    for (int k = 0; k < SCAN_ITEMS; ++k) { o[k] = ex; ex += v[k]; }
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; k += VEC) {
+      uint4 q;
+      memcpy(&q, &o[k], 16);
+      *reinterpret_cast<uint4*>(out + first + k) = q;
+    }
+    if (first + SCAN_ITEMS == n) out[n] = ex;
+  } else {
+#pragma unroll
+    for (int k = 0; k < SCAN_ITEMS; ++k) {
+      if (first + k < n) out[first + k] = ex;
+      ex += v[k];
+      if (first + k == n - 1) out[n] = ex;
+    }
   }
 }
 
