@@ -128,7 +128,13 @@ __device__ __forceinline__ int32_t searchFinish(const SearchPre& sp, const float
     const uint32_t* r = sp.cs + bz * sp.ny;
     scan(__ldg(r), __ldg(r + sp.span));
   }
-  if (tie) best = searchExact(sp, syz, s2o, &ym, &zm);
+  if (tie) {     // the out-of-line re-scan gets copies: `sp`, `ym`, `zm` themselves must never have their address taken,
+                 // or they live in local memory and the store of the cell ranges waits for their loads right in searchBegin
+    const SearchPre cp = sp;
+    float ey = 0.0f, ez = 0.0f;
+    best = searchExact(cp, syz, s2o, &ey, &ez);
+    ym = ey; zm = ez;
+  }
   return best;
 }
 
@@ -232,7 +238,10 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
   int32_t* rowhit = nullptr;      // this tracklet's [n_rows] slice
   int r0 = 0, bsec = 0, rn = 0, rc = 0, lastw = 0, nhits = 0, miss = 0, snap_row = -1, rtop = 0;
   int32_t c_cur = -1;             // hit of the coming step if known (link / row hit), else -1 = search
-  int32_t c_nxt = -1;             // down pass: row hit of the step after (loaded one step ahead)
+  // down pass: row hit of the step after, loaded one step ahead.  Kept as (raw value, valid) and merged with -1 only
+  // when it becomes c_cur: a select right behind the load would wait for the load and undo the pipelining.
+  int32_t nx_raw = -1;
+  bool nx_ok = false;
   int32_t last_c = -1;            // last recorded hit (the hit on row lastw)
 
   for (;;) {
@@ -343,9 +352,10 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
         if (rn < 0) end_phase = true;
       }
       if (!end_phase) {           // pipeline: this step's hit was loaded a step ago; request the one after
-        c_cur = c_nxt;
+        c_cur = nx_ok ? nx_raw : -1;
         const int r2 = snd[rn];
-        c_nxt = (r2 >= r0) ? rowhit[r2] : -1;
+        nx_ok = r2 >= r0;
+        if (nx_ok) nx_raw = rowhit[r2];
       } else {                    // O4 step 6: output = last snapshot
         if (snap_row < 0) {
           out.status[t] = 1; out.nhits[t] = 0; out.first_row[t] = -1; out.last_row[t] = -1;
@@ -368,7 +378,8 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
       phase = 2; miss = 0; nhits = 0; snap_row = -1;
       c_cur = last_c;             // the hit on row rtop
       const int r2 = snd[rn];
-      c_nxt = (r2 >= r0) ? rowhit[r2] : -1;
+      nx_ok = r2 >= r0;
+      if (nx_ok) nx_raw = rowhit[r2];
     } else if (phase >= 0) {      // dead rows stepped over (R23) hold no hit
       const int lo = min(rb, rn), hi = max(rb, rn);
       if (hi - lo > 1)
