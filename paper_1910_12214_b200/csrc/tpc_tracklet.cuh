@@ -208,7 +208,11 @@ __global__ void __launch_bounds__(128) seedPrepare(const uint32_t* __restrict__ 
 // ahead, its coordinates and the row's grid descriptor are requested before Propagate, the cell ranges of a
 // search from inside Propagate.  The order of floating-point operations of a seed is exactly the sequential
 // algorithm's.
+#ifdef TC_MAXNREG
+__global__ void __maxnreg__(TC_MAXNREG) trackletConstructor(
+#else
 __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor(
+#endif
     DevParams P, RowTables T, const GridDesc* __restrict__ desc, const uint32_t* __restrict__ cell_start,
     const float2* __restrict__ syz, const uint32_t* __restrict__ s2o, const int32_t* __restrict__ cup,
     const SeedRec* __restrict__ work_list, TrackletStore out, int64_t* __restrict__ cnt) {
@@ -217,6 +221,12 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
   __shared__ int16_t snu[MAX_ROWS];          // next live row above (n_rows if none)
   __shared__ int16_t snd[MAX_ROWS];          // next live row below (-1 if none)
   __shared__ float snap[22][TC_THREADS];     // state after the last Update of the down pass (O4 step 5)
+  // per-lane bookkeeping that is read once per step or less lives in shared memory (volatile: re-read where used):
+  // in registers it pushed the kernel over 96 and the spilled bucket base sat on the path to every grid load
+  __shared__ volatile uint32_t s_t[TC_THREADS];       // tracklet id
+  __shared__ volatile int s_bsec[TC_THREADS];         // first bucket of the seed's sector
+  __shared__ volatile int16_t s_rtop[TC_THREADS];     // top row of the down pass
+  __shared__ volatile int16_t s_rc[TC_THREADS];       // chain fit: row of the last Propagate
   if (cnt[CNT_ERROR] != 0) return;
   const int R = P.n_rows;
   const int tid = threadIdx.x;
@@ -234,9 +244,8 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
 
   KFState S;
   int phase = -1;                 // -1 wants a seed, -2 no seeds left, 0 chain fit, 1 up extrapolation, 2 down pass
-  uint32_t t = 0;
   int32_t* rowhit = nullptr;      // this tracklet's [n_rows] slice
-  int r0 = 0, bsec = 0, rn = 0, rc = 0, lastw = 0, nhits = 0, miss = 0, snap_row = -1, rtop = 0;
+  int r0 = 0, rn = 0, lastw = 0, nhits = 0, miss = 0, snap_row = -1;
   int32_t c_cur = -1;             // hit of the coming step if known (link / row hit), else -1 = search
   // down pass: row hit of the step after, loaded one step ahead.  Kept as (raw value, valid) and merged with -1 only
   // when it becomes c_cur: a select right behind the load would wait for the load and undo the pipelining.
@@ -252,11 +261,12 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
       } else {
         const uint4* rp = reinterpret_cast<const uint4*>(work_list + j);
         const uint4 a = __ldg(rp), b = __ldg(rp + 1);
-        t = a.x;
+        const uint32_t t = a.x;
+        s_t[tid] = t;
         const uint32_t h0 = a.y;
         c_cur = (int32_t)a.z;
         r0 = (int)(a.w & 0xffu);
-        bsec = (int)(a.w >> 8) - r0;
+        s_bsec[tid] = (int)(a.w >> 8) - r0;
         rowhit = out.rowhit + (int64_t)t * R;
         rn = sup[r0];
         const float y0 = __uint_as_float(b.x), z0 = __uint_as_float(b.y);
@@ -268,7 +278,7 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
         S.chi2 = 0.0f;
         rowhit[r0] = (int32_t)h0;
         last_c = (int32_t)h0;
-        nhits = 1; rc = r0; lastw = r0; miss = 0; snap_row = -1;
+        nhits = 1; s_rc[tid] = (int16_t)r0; lastw = r0; miss = 0; snap_row = -1;
         phase = 0;
       }
     }
@@ -281,7 +291,7 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
     int32_t hnext = -1;
     // the grid descriptor of the row is loaded by every lane (a conditional struct assignment would make the compiler
     // wait for the load right here, to merge it with the "not loaded" value)
-    const GridDesc G = desc[act ? bsec + rn : 0];
+    const GridDesc G = desc[act ? s_bsec[tid] + rn : 0];
     if (act && c_cur >= 0) {
       mk = __ldg(syz + c_cur);
       if (phase == 0) hnext = __ldg(cup + c_cur);
@@ -305,7 +315,7 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
     const int rb = rn;                               // the row of this step
     if (okp && !known) rowhit[rb] = oku ? c : -1;    // rows beyond the final first/last row are never read
     if (phase == 0) {
-      if (okp) rc = rb;
+      if (okp) s_rc[tid] = (int16_t)rb;
       if (oku) {
         lastw = rb; last_c = c; ++nhits;
         c_cur = hnext;
@@ -314,11 +324,12 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
       }
       if (end_phase) {
         if (nhits < P.min_chain_hits) {
+          const uint32_t t = s_t[tid];
           out.status[t] = 0; out.nhits[t] = nhits; out.first_row[t] = -1; out.last_row[t] = -1;
           phase = -1;
         } else {
           phase = 1; miss = 0; c_cur = -1;
-          rn = snu[rc];
+          rn = snu[s_rc[tid]];
           if (rn >= R) turn = true;
         }
       }
@@ -357,11 +368,12 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
         nx_ok = r2 >= r0;
         if (nx_ok) nx_raw = rowhit[r2];
       } else {                    // O4 step 6: output = last snapshot
+        const uint32_t t = s_t[tid];
         if (snap_row < 0) {
           out.status[t] = 1; out.nhits[t] = 0; out.first_row[t] = -1; out.last_row[t] = -1;
         } else {
           out.status[t] = nhits >= P.min_tracklet_hits ? 2 : 1;
-          out.nhits[t] = nhits; out.first_row[t] = snap_row; out.last_row[t] = rtop;
+          out.nhits[t] = nhits; out.first_row[t] = snap_row; out.last_row[t] = s_rtop[tid];
           out.x[t] = snap[0][tid]; out.chi2[t] = snap[6][tid];
 #pragma unroll
           for (int i = 0; i < 5; ++i) out.par[i * capT + t] = snap[1 + i][tid];
@@ -374,7 +386,7 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
     if (turn) {                   // O4 step 4: diffuse covariance, parameters kept (R17); down pass starts at rtop
       kfSetDiag(S, P.turn_var_scale * P.err2_y, P.turn_var_scale * P.err2_z, P);
       S.chi2 = 0.0f;
-      rtop = lastw; rn = rtop;
+      s_rtop[tid] = (int16_t)lastw; rn = lastw;
       phase = 2; miss = 0; nhits = 0; snap_row = -1;
       c_cur = last_c;             // the hit on row rtop
       const int r2 = snd[rn];
