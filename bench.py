@@ -32,9 +32,9 @@ WORKLOADS = {0: "config0 single sector, 200 primaries", 1: "config1 central Pb-P
 
 
 ALU_SMS = 148
-# ncu counts of one launch on the bench workload (config 4, seed 5), from the committed capture profiles/r1l_full_capture.md
-NCU_R1 = {(4, "a4_constructor"): {"kernel": "trackletConstructor", "warp_inst": 2.2829e10, "dram_bytes": 14507216000},
-          (4, "a2_neighbours"): {"kernel": "neighbourFinder", "warp_inst": 1.1833e10, "dram_bytes": 1603174000}}
+# ncu counts of one launch on the bench workload (config 4, seed 5), from the committed capture profiles/r1m_full_capture.md
+NCU_R1 = {(4, "a4_constructor"): {"kernel": "trackletConstructor", "warp_inst": 2.2849e10, "dram_bytes": 13136154000},
+          (4, "a2_neighbours"): {"kernel": "neighbourFinder", "warp_inst": 1.1833e10, "dram_bytes": 1605503999}}
 
 
 # O4 operations per hit of the accepted tracklets on config 4 (oracle/count_o4_ops.py, sectors 0 / 7 / 20 agree to 0.5 %):
@@ -308,14 +308,14 @@ def run_ours(args, rank, world, local_rank):
     share = round(dom_ms / max(float(stage[6]), 1e-9), 4)
     ncu = NCU_R1.get((args.config, dom))
     if ncu is not None:
-        # The dominant kernels are bound by instruction issue, not by HBM (profiles/r1l_full_capture.md):
+        # The dominant kernels are bound by instruction issue, not by HBM (profiles/r1m_full_capture.md):
         # achieved = warp instructions of one launch (ncu smsp__inst_executed.sum of the committed capture of this
         # workload) / the live CUDA-event time of the stage; peak = SMs x 4 schedulers x 1 instruction/clock x max SM clock.
         sm_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
         issue_peak = ALU_SMS * 4 * sm_mhz * 1e6 / 1e9
         issued = ncu["warp_inst"] / (dom_ms * 1e-3) / 1e9
         issue = {"achieved": round(issued, 2), "peak": round(issue_peak, 1), "unit": "Gwarp-inst/s",
-                 "frac": round(issued / issue_peak, 5), "counts_from": "profiles/r1l_full_capture.md",
+                 "frac": round(issued / issue_peak, 5), "counts_from": "profiles/r1m_full_capture.md",
                  "peak_source": f"{ALU_SMS} SMs x 4 schedulers x {sm_mhz:.0f} MHz"}
         common = {"traffic": ncu["dram_bytes"], "alg_bytes": int(alg[dom]),
                   "alg_gbs": round(alg[dom] / (dom_ms * 1e-3) / 1e9, 1),
