@@ -98,9 +98,14 @@ __global__ void __launch_bounds__(128) selectCount(TrackletStore tl, const unsig
         rowHits4(row, tl.n_rows, rb, f, r1, c8);
         if (rb + 4 <= r1) rowHits4(row, tl.n_rows, rb + 4, f, r1, c8 + 4);
         else { c8[4] = c8[5] = c8[6] = c8[7] = -1; }
+        // all eight gathers are requested before the first compare (rows without a hit read entry 0 and are masked):
+        // behind `c >= 0 &&` each load sat in its own branch and the eight latencies came one after the other
+        unsigned long long kk[8];
+#pragma unroll
+        for (int k = 0; k < 8; ++k) kk[k] = owner_key[c8[k] >= 0 ? c8[k] : 0];
         bool own[8];
 #pragma unroll
-        for (int k = 0; k < 8; ++k) own[k] = c8[k] >= 0 && owns(c8[k], key, (uint32_t)t, wide, owner_key, owner_id);
+        for (int k = 0; k < 8; ++k) own[k] = c8[k] >= 0 && kk[k] == key && (!wide || owner_id[c8[k]] == (uint32_t)t);
 #pragma unroll
         for (int k = 0; k < 8; ++k)
           if (own[k]) {
