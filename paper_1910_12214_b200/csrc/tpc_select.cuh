@@ -173,10 +173,15 @@ __global__ void __launch_bounds__(128) selectEmit(TrackletStore tl, const unsign
   const int32_t* row = tl.rowhit + t * tl.n_rows + tl.first_row[t];      // compacted by selectCount
   const int nk = (int)max((int64_t)0, min((int64_t)kept, o.cap_cl - off));      // entries that fit the output
   int i = 0;
-  for (; i + 4 <= nk; i += 4) {       // four independent row -> index gathers in flight
-    const int32_t c0 = row[i], c1 = row[i + 1], c2 = row[i + 2], c3 = row[i + 3];
-    const uint32_t g0 = s2o[c0], g1 = s2o[c1], g2 = s2o[c2], g3 = s2o[c3];
-    o.cl_index[off + i] = g0; o.cl_index[off + i + 1] = g1; o.cl_index[off + i + 2] = g2; o.cl_index[off + i + 3] = g3;
+  for (; i + 8 <= nk; i += 8) {       // eight independent row -> index gathers in flight
+    int32_t c[8];
+    uint32_t g[8];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) c[q] = row[i + q];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) g[q] = s2o[c[q]];
+#pragma unroll
+    for (int q = 0; q < 8; ++q) o.cl_index[off + i + q] = g[q];
   }
   for (; i < nk; ++i) o.cl_index[off + i] = s2o[row[i]];
 }
