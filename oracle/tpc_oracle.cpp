@@ -916,6 +916,21 @@ int refitPoints(const orcGeometry* g, const orcParams* p, int n, const int32_t* 
   }
   return 1;
 }
+
+// One Search (O4, R13) of the clusters of one sector for the pins: the given clusters are the only input, the grid is
+// built as in a run unless brute.
+template <typename Real>
+int searchPoints(const orcGeometry* g, const orcParams* p, int n, const int32_t* rows, const float* y, const float* z,
+                 int row, const double* st, const double* cov, int brute) {
+  std::vector<uint32_t> off((size_t)g->n_rows + 1, 0);
+  for (int i = 0; i < n; ++i) off[rows[i] + 1]++;
+  for (int r = 0; r < g->n_rows; ++r) off[r + 1] += off[r];
+  orcGeometry g1 = *g; g1.n_sectors = 1;
+  orcResult res;
+  Tracker<Real> T(g1, *p, n, off.data(), y, z, brute != 0, res);
+  if (!brute) T.buildGrid();
+  return (int)T.search(row, stateFrom<Real>(st, cov));
+}
 }  // namespace
 
 extern "C" {
@@ -995,6 +1010,15 @@ void orcGetTracks(const orcResult* r, int32_t* id, int32_t* sector, int32_t* fir
   copyOut(id, r->tr_id); copyOut(sector, r->tr_sector); copyOut(first, r->tr_first); copyOut(last, r->tr_last);
   copyOut(ncl, r->tr_ncl); copyOut(x, r->tr_x); copyOut(par, r->tr_par); copyOut(cov, r->tr_cov);
   copyOut(chi2, r->tr_chi2); copyOut(off, r->tr_cl_offset); copyOut(idx, r->tr_cl_index);
+}
+
+int orcSearch(const orcGeometry* g, const orcParams* p, int n, const int32_t* rows, const float* y, const float* z, int row,
+              const double* state, const double* cov, int fp64, int brute) {
+  if (!g || !p || n < 0 || (n > 0 && (!rows || !y || !z)) || !state || !cov || row < 0 || row >= g->n_rows) return -2;
+  for (int i = 0; i < n; ++i)
+    if (rows[i] < 0 || rows[i] >= g->n_rows || (i > 0 && rows[i] < rows[i - 1])) return -2;
+  return fp64 ? searchPoints<double>(g, p, n, rows, y, z, row, state, cov, brute)
+              : searchPoints<float>(g, p, n, rows, y, z, row, state, cov, brute);
 }
 
 int orcPropagate(double* state, double* cov, double x_new, double bz, double max_sinphi, int fp64) {

@@ -15,7 +15,8 @@
  * Pins (tests/test_oracle_*.py): grid search == brute-force search; collinear / hand-built link
  * cases; reciprocity and path invariants; Propagate vs the closed-form asin helix and vs finite
  * differences; Update / fit vs numpy least squares; exact helix recovery; unit pulls; full
- * attachment of noise-free high-pT helices; selector vs sorted greedy; O6..O10: see DESIGN.md, pins table.
+ * attachment of noise-free high-pT helices; Search (road widths, clamps, nearest, ties) and the gap / length rules of
+ * O4 / O5 on hand-worked cases; selector vs sorted greedy; O6..O10: see DESIGN.md, pins table.
  * Parity unpinned: physics efficiency / fake rate on configs 1-4 (no reference numbers exist).
  */
 #ifndef TPC_ORACLE_H
@@ -141,6 +142,13 @@ int orcLegMatch(const orcParams* p, double bz_tesla, const double* a_state, cons
  * (00,10,11,20,21,22,30,...,44), both in/out as doubles (rounded to binary32 first unless fp64).
  * Return 1 on success, 0 on failure (state untouched). */
 int orcPropagate(double* state, double* cov, double x_new, double bz_tesla, double max_sinphi, int fp64);
+/* One Search of O4 (DESIGN.md section 3 "Search", reading R13) for the pins: the n given clusters of one sector
+ * (rows ascending, index = position in the arrays) are the whole input; the road is taken from the state
+ * {x, y, z, s, t, q} and its covariance, on pad row `row`.  Returns the index of the picked cluster, -1 when the
+ * road is empty, -2 on bad arguments.  brute = 1: every cluster of the row is tested, no grid. */
+int orcSearch(const orcGeometry* g, const orcParams* p, int n, const int32_t* rows, const float* y, const float* z, int row,
+              const double* state, const double* cov, int fp64, int brute);
+
 int orcUpdate(double* state, double* cov, double* chi2, double ym, double zm, double err2_y, double err2_z, int fp64);
 
 #ifdef __cplusplus

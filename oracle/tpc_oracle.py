@@ -102,6 +102,8 @@ def _load():
         L.orcGetRefit.restype = None
         L.orcRefitPoints.argtypes = [ctypes.POINTER(Geometry), ctypes.POINTER(Params), ci, vp, vp, vp, ci, vp, vp]
         L.orcRefitPoints.restype = ci
+        L.orcSearch.argtypes = [ctypes.POINTER(Geometry), ctypes.POINTER(Params), ci, vp, vp, vp, ci, vp, vp, ci, ci]
+        L.orcSearch.restype = ci
         L.orcPropagate.argtypes = [vp, vp, dbl, dbl, dbl, ci]
         L.orcPropagate.restype = ci
         L.orcUpdate.argtypes = [vp, vp, vp, dbl, dbl, dbl, dbl, ci]
@@ -276,6 +278,21 @@ def update(state, cov, chi2, ym, zm, err2_y=0.01, err2_z=0.01, fp64=True):
     ok = _load().orcUpdate(s.ctypes.data, c.ctypes.data, x2.ctypes.data, float(ym), float(zm), float(err2_y),
                            float(err2_z), int(fp64))
     return bool(ok), s, c, float(x2[0])
+
+
+def search(rows, y, z, row, state, cov, row_x, params: Params | None = None, fp64=False, brute=False, bz_tesla=0.5):
+    """One O4 Search among the given clusters of one sector (ascending rows).  Returns the picked index or -1."""
+    p = params if params is not None else default_params()
+    row_x = np.ascontiguousarray(row_x, np.float32)
+    g = Geometry(1, len(row_x), row_x.ctypes.data, None, bz_tesla, float(np.tan(np.radians(10.0))), -250.0, 250.0)
+    rows = np.ascontiguousarray(rows, np.int32)
+    yy, zz = np.ascontiguousarray(y, np.float32), np.ascontiguousarray(z, np.float32)
+    s, c = np.array(state, np.float64), np.array(cov, np.float64)
+    rc = _load().orcSearch(ctypes.byref(g), ctypes.byref(p), len(rows), _ptr(rows), _ptr(yy), _ptr(zz), int(row),
+                           s.ctypes.data, c.ctypes.data, int(fp64), int(brute))
+    if rc == -2:
+        raise ValueError("orcSearch: bad arguments")
+    return int(rc)
 
 
 def refit_points(rows, y, z, row_x, bz_tesla=0.5, params: Params | None = None, fp64=True):
