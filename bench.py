@@ -32,16 +32,25 @@ WORKLOADS = {0: "config0 single sector, 200 primaries", 1: "config1 central Pb-P
 
 
 ALU_SMS = 148
-# ncu counts of one launch on the bench workload (config 4, seed 5), from the committed capture profiles/r1m_full_capture.md
-NCU_R1 = {(4, "a4_constructor"): {"kernel": "trackletConstructor", "warp_inst": 2.2849e10, "dram_bytes": 13136154000},
-          (4, "a2_neighbours"): {"kernel": "neighbourFinder", "warp_inst": 1.1833e10, "dram_bytes": 1605503999}}
+# ncu figures of ONE launch of the hot kernels on the bench workload, keyed by (config, generator seed): DRAM bytes
+# (dram__bytes_read.sum + dram__bytes_write.sum) and warp instructions (smsp__inst_executed.sum) of the committed
+# `ncu --set full` capture named in "file".  They are cited constants (a number taken under a profiler is never a bench
+# value); every other configuration or seed reports "traffic": null.
+NCU_CAPTURE = {
+    (4, 5): {"file": "profiles/r1m_full_capture.md",
+             "a4_constructor": {"kernel": "trackletConstructor", "warp_inst": 2.2849e10, "dram_bytes": 13136154000},
+             "a2_neighbours": {"kernel": "neighbourFinder", "warp_inst": 1.1833e10, "dram_bytes": 1605503999}},
+}
+STAGE_KERNEL = {"a1_grid": "gridCount+gridScatter", "a2_neighbours": "neighbourFinder", "a3_cleaner_start": "cleanLinks",
+                "a4_constructor": "trackletConstructor", "a5_selector": "selectClaim+selectCount+selectEmit"}
 
-
-# O4 operations per hit of the accepted tracklets on config 4 (oracle/count_o4_ops.py, sectors 0 / 7 / 20 agree to 0.5 %):
-# Propagate, Update, Search, clusters inside the roads; and the fp32 operations of each as DESIGN.md section 3 writes them
-# (adds, multiplies, divisions, square roots each counted once; R0: nothing is fused): DESIGN.md section 8.
-O4_OPS_PER_HIT = {4: (1.515, 1.443, 1.020, 1.444)}
+# fp32 operations of one Propagate, Update, Search and of one cluster inside a road, and of one window candidate and one
+# (u, d) pair of the neighbour finder, as DESIGN.md section 3 writes them (adds, multiplies, divisions, square roots each
+# counted once; R0: nothing is fused): DESIGN.md section 8.  HOW OFTEN each runs per unit comes from the oracle's own
+# counters on this run's cpu_baseline sample (orcGetO4Counts / orcGetO2Counts), not from a stored table.
 O4_FLOPS = (176, 100, 6, 5)
+O2_FLOPS = (4, 5)            # slopes of a window candidate (2 subtractions, 2 products); Dev of a pair (2, 2, 1)
+SURVEY_BYTES_PER_CLUSTER = 140   # the fixed accounting with H = N
 
 
 def _peaks():
@@ -168,6 +177,31 @@ def aggregate(units: float, ms: float, device, world: int):
     return float(u.item()), float(t.item())
 
 
+def _oracle_counts(ores):
+    """Per-unit operation counts of the oracle's own counters on the cpu_baseline sample: O4 per hit of the accepted
+    tracklets (Propagate, Update, Search, clusters inside the roads), O2 per cluster (window candidates, pairs)."""
+    H0 = int(ores.tl_nhits[ores.tl_status == 2].sum())
+    n0 = int(ores.n_clusters)
+    o4 = [float(v) / max(H0, 1) for v in ores.o4_ops]
+    o2 = [float(ores.o2_ops[1] + ores.o2_ops[2]) / max(n0, 1), float(ores.o2_ops[3]) / max(n0, 1)]
+    return o4, o2
+
+
+def run_dry(args, rank, world):
+    """--dry-run: the N > 1 plumbing without a GPU (gloo): every rank contributes made-up figures through the same
+    aggregate(); rank 0 prints one line.  Used by tests/test_multirank_gloo.py to cover the spawner."""
+    import torch
+    import torch.distributed as dist
+    if world > 1:
+        dist.init_process_group("gloo")
+    units, ms = aggregate(1000.0 * (rank + 1), 10.0 * (rank + 1), torch.device("cpu"), world)
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps({"metric": METRIC, "dry_run": True, "n_gpus": world, "units": units, "ms": ms}), flush=True)
+
+
 def run_ours(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
@@ -179,7 +213,8 @@ def run_ours(args, rank, world, local_rank):
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     # every rank tracks its own time frame (replicas: independent data per GPU)
-    ev = datagen.generate(datagen.config(args.config, seed=args.config + 1 + 100 * rank), name=f"config{args.config}")
+    seed = args.config + 1 + 100 * rank
+    ev = datagen.generate(datagen.config(args.config, seed=seed), name=f"config{args.config}")
     N = ev.n_clusters
     trk = tpc.TpcTracker.from_event(ev, device=local_rank)
     off, y, z = trk.upload(ev)
@@ -189,41 +224,58 @@ def run_ours(args, rank, world, local_rank):
     capT = int(st0.n_start_hits * 1.05) + 1024
     capK = int(st0.n_tracks * 1.05) + 1024
     capC = int(st0.n_track_clusters * 1.05) + 1024
-    trk.set_profiling(True)
     stream = torch.cuda.current_stream()
+    dev = torch.device("cuda", local_rank)
 
     def step():
         trk.run(off, y, z, cap_tracklets=capT, cap_tracks=capK, cap_track_clusters=capC, sync=False)
 
-    for _ in range(max(args.warmup, 3)):
+    trk.set_profiling(False)
+    W = max(args.warmup, 3)
+    for _ in range(W):
         step()
     st = trk.status()
     assert st.status == 0
+    # ---- the timed region: exactly K steps back to back on one stream, no host synchronisation inside; one CUDA event
+    #      between consecutive steps gives the per-step times (median and min) -------------------------
+    K = args.steps
     sampler = ClockSampler(local_rank) if rank == 0 else None
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    evs = [torch.cuda.Event(enable_timing=True) for _ in range(K + 1)]
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
     t0 = time.time()
-    stage = np.zeros(8)
-    e0.record(stream)
-    for _ in range(args.steps):
+    evs[0].record(stream)
+    for i in range(K):
         step()
-        s = trk.status()                            # waits for the step; per-stage CUDA-event times of this step
-        stage += np.array(list(s.stage_ms))
-    e1.record(stream)
+        evs[i + 1].record(stream)
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
     t1 = time.time()
-    ms_total = e0.elapsed_time(e1)
-    total_clusters, ms_max = aggregate(float(N), ms_total, torch.device("cuda", local_rank), world)
-    ms_step = ms_max / args.steps
+    st = trk.status()
+    assert st.status == 0
+    per = np.array([evs[i].elapsed_time(evs[i + 1]) for i in range(K)])
+    ms_total = evs[0].elapsed_time(evs[K])
+    total_clusters, ms_total_max = aggregate(float(N), ms_total, dev, world)
+    _, ms_median = aggregate(float(N), float(np.median(per)), dev, world)
+    _, ms_min = aggregate(float(N), float(per.min()), dev, world)
+    ms_mean = ms_total_max / K
+    ms_step = ms_median                              # `value` stands on the median step (max over ranks)
     value = total_clusters / (ms_step * 1e-3)
     clocks = sampler.stop(t0, t1) if sampler else None
-    stage /= args.steps
 
-    # ---- the NEXT-2 row (a6 refit of the selected tracks), timed apart: it is not part of the a1..a5 step ----------
+    # ---- per-stage CUDA-event times: a separate instrumented run (the library records an event between the stages) ---
+    trk.set_profiling(True)
+    stage = np.zeros(8)
+    n_inst = 3
+    for _ in range(n_inst):
+        step()
+        s = trk.status()
+        stage += np.array(list(s.stage_ms))
+    stage /= n_inst
+
+    # ---- the NEXT rows (a6 refit, a7 merger, a10 legs, a8 flags, a9 codes), timed apart: not part of the a1..a5 step ----
     refit_ms = merge_ms = flags_ms = pack_ms = legs_ms = None
     n_links = n_legs = 0
     flag_frac = {}
@@ -246,6 +298,7 @@ def run_ours(args, rank, world, local_rank):
                      for name, bit in (("attached", 1), ("adjacent", 2), ("protected", 4), ("removed_A", 8), ("removed_B", 16))}
         n_links = int((trk._out["trk_mg_next"][:int(s.n_tracks)] >= 0).sum().item())
         n_legs = int((trk._out["trk_leg_partner"][:int(s.n_tracks)] >= 0).sum().item()) // 2
+    trk.set_profiling(False)
 
     # ---- end to end through the host-buffer ABI call (pinned host memory; copies inside the timed region) ----
     hy = torch.from_numpy(ev.y).pin_memory()
@@ -262,6 +315,7 @@ def run_ours(args, rank, world, local_rank):
     for w in range(2):
         sth, outh = trk.collect_host(w)                # warm-up of both slots (their pools are allocated here)
         assert sth.status == 0
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     if world > 1:
         dist.barrier()
     torch.cuda.synchronize()
@@ -278,78 +332,28 @@ def run_ours(args, rank, world, local_rank):
     wall_e2e = (time.perf_counter() - t_e2e) * 1e3 / e2e_steps
     # the slots run on the library's own streams: the host clock around submit ... collect is the measure (the events on
     # torch's stream only bracket it); max over ranks as for `value`
-    _, ms_e2e = aggregate(float(N), max(wall_e2e, e0.elapsed_time(e1) / e2e_steps), torch.device("cuda", local_rank), world)
+    _, ms_e2e = aggregate(float(N), max(wall_e2e, e0.elapsed_time(e1) / e2e_steps), dev, world)
     e2e_value = total_clusters / (ms_e2e * 1e-3)
-    nt, nc = int(sth.n_tracks), int(sth.n_track_clusters)
     h2d = 4 * (len(ev.row_offset)) + 8 * N
     # tpcSubmitHost copies back up to the capacities (the counts are not known on the host at submit time)
     d2h = capK * (5 * 4 + 4 + 20 + 60 + 4) + 4 * (capK + 1) + 4 * capC + 8 * 11
 
     if rank != 0:
         return
-    # ---- roofline of the dominant kernel (algorithmic bytes per stage) -------------------
-    peak, peak_src = _peaks()
-    H = int(st.n_tracklet_hits)
-    nT = int(st.n_tracklets)
-    alg = {"a1_grid": 24 * N, "a2_neighbours": 20 * N, "a3_cleaner_start": 24 * N, "a4_constructor": 40 * H + 100 * nT,
-           "a5_selector": 32 * H}
-    names = list(alg)
-    stages = {}
-    for i, k in enumerate(names):
-        ms = float(stage[i])
-        stages[k] = {"ms": round(ms, 4), "alg_bytes": int(alg[k]),
-                     "gbs": round(alg[k] / (ms * 1e-3) / 1e9, 1) if ms > 0 else None}
-    dom = max(names, key=lambda k: stages[k]["ms"])
-    dom_ms = stages[dom]["ms"]
-    total_alg = sum(alg.values())
-    whole = {"alg_bytes": int(total_alg), "gbs": round(total_alg / (ms_step * 1e-3) / 1e9, 1),
-             "frac_of_hbm_peak": round(total_alg / (ms_step * 1e-3) / 1e9 / peak, 5), "hbm_peak_gbs": peak,
-             "peak_source": peak_src}
-    share = round(dom_ms / max(float(stage[6]), 1e-9), 4)
-    ncu = NCU_R1.get((args.config, dom))
-    if ncu is not None:
-        # The dominant kernels are bound by instruction issue, not by HBM (profiles/r1m_full_capture.md):
-        # achieved = warp instructions of one launch (ncu smsp__inst_executed.sum of the committed capture of this
-        # workload) / the live CUDA-event time of the stage; peak = SMs x 4 schedulers x 1 instruction/clock x max SM clock.
-        sm_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
-        issue_peak = ALU_SMS * 4 * sm_mhz * 1e6 / 1e9
-        issued = ncu["warp_inst"] / (dom_ms * 1e-3) / 1e9
-        issue = {"achieved": round(issued, 2), "peak": round(issue_peak, 1), "unit": "Gwarp-inst/s",
-                 "frac": round(issued / issue_peak, 5), "counts_from": "profiles/r1m_full_capture.md",
-                 "peak_source": f"{ALU_SMS} SMs x 4 schedulers x {sm_mhz:.0f} MHz"}
-        common = {"traffic": ncu["dram_bytes"], "alg_bytes": int(alg[dom]),
-                  "alg_gbs": round(alg[dom] / (dom_ms * 1e-3) / 1e9, 1),
-                  "alg_frac_of_hbm_peak": round(alg[dom] / (dom_ms * 1e-3) / 1e9 / peak, 5),
-                  "issue": issue, "whole_path": whole, "share_of_step": share}
-        per_hit = O4_OPS_PER_HIT.get(args.config) if dom == "a4_constructor" else None
-        if per_hit is not None:
-            # algorithmic fp32 operations of one launch = tracklet hits x (O4 operations per hit x operations each), against
-            # the non-fused fp32 peak: SMs x 128 lanes x 1 operation / clock (R0 forbids the FMA that doubles it)
-            flops = H * sum(a * b for a, b in zip(per_hit, O4_FLOPS))
-            alu_peak = ALU_SMS * 128 * sm_mhz * 1e6 / 1e12
-            achieved = flops / (dom_ms * 1e-3) / 1e12
-            roofline = {"bound": "alu", "kernel": ncu["kernel"], "achieved": round(achieved, 3), "peak": round(alu_peak, 2),
-                        "unit": "TFLOP/s", "frac": round(achieved / alu_peak, 5), "alg_flops": int(flops),
-                        "flops_per_tracklet_hit": round(flops / max(H, 1), 1),
-                        "peak_source": f"{ALU_SMS} SMs x 128 fp32 lanes x {sm_mhz:.0f} MHz, no FMA (B200_PROFILING.md unit "
-                                       "counts and clocks; DESIGN.md section 8)", **common}
-        else:
-            roofline = {"bound": "alu", "kernel": ncu["kernel"], "achieved": issue["achieved"], "peak": issue["peak"],
-                        "unit": issue["unit"], "frac": issue["frac"], "peak_source": issue["peak_source"], **common}
-    else:
-        achieved = alg[dom] / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0
-        roofline = {"bound": "hbm", "kernel": dom, "achieved": round(achieved, 2), "peak": peak, "unit": "GB/s",
-                    "frac": round(achieved / peak, 5), "traffic": None, "peak_source": peak_src, "whole_path": whole,
-                    "share_of_step": share}
-    # ---- CPU baseline: the oracle on one sector of this event (rank 0, N = 1 only) ----------------------------
+    # ---- CPU baseline: the oracle on one sector of this event (rank 0, N = 1 only); its operation counters give the
+    #      per-unit algorithmic operation counts of the roofline below ------------------------------------------------
     cpu = None
+    o4_per_hit = o2_per_cluster = None
     if world == 1 and not args.no_cpu_baseline:
         sample = _sector_sample(ev, 1) if ev.n_sectors > 1 and N > 2e6 else ev
         dt, ores = _time_oracle(sample)
+        o4_per_hit, o2_per_cluster = _oracle_counts(ores)
         cpu = {"value": sample.n_clusters / dt, "unit": UNIT, "cores": 1, "kind": "oracle",
                "sample": (f"sector 0 of the event ({sample.n_clusters} clusters, 1/{ev.n_sectors} of the step), {dt:.1f} s"
                           if sample is not ev else f"whole event ({N} clusters), {dt:.2f} s"),
-               "host_cores_available": os.cpu_count()}
+               "host_cores_available": os.cpu_count(),
+               "o4_ops_per_tracklet_hit": [round(v, 4) for v in o4_per_hit],
+               "o2_candidates_and_pairs_per_cluster": [round(v, 3) for v in o2_per_cluster]}
         # the same oracle on several sectors at once, one thread per sector (ctypes releases the GIL): what the host's
         # cores do together; `cpu_baseline` above stays the single-core figure of the contract
         if ev.n_sectors > 1 and N > 2e6 and (os.cpu_count() or 1) > 1:
@@ -369,17 +373,86 @@ def run_ours(args, rank, world, local_rank):
             dtm = time.perf_counter() - t0m
             cpu["multicore"] = {"value": sum(s.n_clusters for s in samples) / dtm, "unit": UNIT, "cores": ncore,
                                 "sample": f"sectors 0..{ncore - 1} of the event, one oracle thread each, {dtm:.1f} s"}
-    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
-            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+
+    # ---- roofline of the dominant kernel ---------------------------------------------------
+    peak, peak_src = _peaks()
+    H = int(st.n_tracklet_hits)
+    nT = int(st.n_tracklets)
+    alg = {"a1_grid": 24 * N, "a2_neighbours": 20 * N, "a3_cleaner_start": 24 * N, "a4_constructor": 40 * H + 100 * nT,
+           "a5_selector": 32 * H}
+    names = list(alg)
+    stages = {}
+    for i, k in enumerate(names):
+        ms = float(stage[i])
+        stages[k] = {"ms": round(ms, 4), "alg_bytes": int(alg[k]),
+                     "gbs": round(alg[k] / (ms * 1e-3) / 1e9, 1) if ms > 0 else None,
+                     "frac_of_hbm_peak": round(alg[k] / (ms * 1e-3) / 1e9 / peak, 4) if ms > 0 else None}
+    dom = max(names, key=lambda k: stages[k]["ms"])
+    dom_ms = stages[dom]["ms"]
+    total_alg = sum(alg.values())
+    survey_alg = SURVEY_BYTES_PER_CLUSTER * N
+    whole = {"alg_bytes": int(total_alg), "gbs": round(total_alg / (ms_step * 1e-3) / 1e9, 1),
+             "frac_of_hbm_peak": round(total_alg / (ms_step * 1e-3) / 1e9 / peak, 5),
+             "survey_fixed_accounting": {"bytes_per_cluster": SURVEY_BYTES_PER_CLUSTER, "alg_bytes": int(survey_alg),
+                                         "frac_of_hbm_peak": round(survey_alg / (ms_step * 1e-3) / 1e9 / peak, 5)},
+             "target_frac": 0.40, "hbm_peak_gbs": peak, "peak_source": peak_src}
+    share = round(dom_ms / max(float(stage[6]), 1e-9), 4)
+    cap = NCU_CAPTURE.get((args.config, seed))
+    ncu = cap.get(dom) if cap else None
+    sm_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0
+    alu_peak = ALU_SMS * 128 * sm_mhz * 1e6 / 1e12
+    hbm = {"alg_bytes": int(alg[dom]), "alg_gbs": round(alg[dom] / (dom_ms * 1e-3) / 1e9, 1),
+           "alg_frac_of_hbm_peak": round(alg[dom] / (dom_ms * 1e-3) / 1e9 / peak, 5), "hbm_peak_gbs": peak}
+    # algorithmic fp32 operations of one launch of the dominant kernel, when it is one of the two arithmetic stages and
+    # the oracle leg of this run counted the operations per unit
+    flops = per_unit = None
+    if dom == "a4_constructor" and o4_per_hit is not None:
+        per_unit = sum(a * b for a, b in zip(o4_per_hit, O4_FLOPS))
+        flops = H * per_unit
+        unit_name = "flops_per_tracklet_hit"
+    elif dom == "a2_neighbours" and o2_per_cluster is not None:
+        per_unit = sum(a * b for a, b in zip(o2_per_cluster, O2_FLOPS))
+        flops = N * per_unit
+        unit_name = "flops_per_cluster"
+    if dom in ("a4_constructor", "a2_neighbours"):
+        # These two stages are bound by instruction issue, not by HBM (DRAM at 1-6 % of peak in the
+        # committed captures): "bound": "alu", achieved = algorithmic fp32 operations / live CUDA-event time of the stage,
+        # peak = SMs x 128 fp32 lanes x 1 operation / clock (R0 forbids the FMA that would double it).
+        roofline = {"bound": "alu", "kernel": STAGE_KERNEL[dom], "unit": "TFLOP/s", "peak": round(alu_peak, 2),
+                    "peak_source": f"{ALU_SMS} SMs x 128 fp32 lanes x {sm_mhz:.0f} MHz, no FMA (B200_PROFILING.md unit counts "
+                                   "and clocks; DESIGN.md section 8)"}
+        if flops is not None:
+            achieved = flops / (dom_ms * 1e-3) / 1e12
+            roofline.update({"achieved": round(achieved, 3), "frac": round(achieved / alu_peak, 5), "alg_flops": int(flops),
+                             unit_name: round(per_unit, 1), "counts_from": "this run's cpu_baseline oracle leg"})
+        else:
+            roofline.update({"achieved": None, "frac": None, "alg_flops": None,
+                             "counts_from": "unavailable: the cpu_baseline oracle leg did not run (N > 1 or --no-cpu-baseline)"})
+    else:
+        achieved = alg[dom] / (dom_ms * 1e-3) / 1e9 if dom_ms > 0 else 0.0
+        roofline = {"bound": "hbm", "kernel": STAGE_KERNEL[dom], "achieved": round(achieved, 2), "peak": peak, "unit": "GB/s",
+                    "frac": round(achieved / peak, 5), "peak_source": peak_src}
+    roofline.update({"traffic": ncu["dram_bytes"] if ncu else None, "traffic_from": cap["file"] if ncu else None,
+                     "hbm_view": hbm, "whole_path": whole, "share_of_step": share, "launch_ms": round(dom_ms, 4)})
+    if ncu:
+        issue_peak = ALU_SMS * 4 * sm_mhz * 1e6 / 1e9
+        issued = ncu["warp_inst"] / (dom_ms * 1e-3) / 1e9
+        roofline["issue"] = {"achieved": round(issued, 2), "peak": round(issue_peak, 1), "unit": "Gwarp-inst/s",
+                             "frac": round(issued / issue_peak, 5), "counts_from": cap["file"],
+                             "peak_source": f"{ALU_SMS} SMs x 4 schedulers x {sm_mhz:.0f} MHz"}
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
+            "ms_per_step": ms_step, "ms_per_step_min": ms_min, "ms_per_step_mean": ms_mean,
+            "timing": "K steps back to back on one stream, one CUDA event between steps; value on the median step, max over ranks",
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic",
-            "config": {"workload": WORKLOADS[args.config], "n_clusters_per_gpu": N, "n_sectors": ev.n_sectors,
+            "config": {"workload": WORKLOADS[args.config], "seed": seed, "n_clusters_per_gpu": N, "n_sectors": ev.n_sectors,
                        "n_rows": ev.n_rows, "cache": "inputs_larger_than_L2" if 8 * N > 126e6 else "working set may fit L2",
                        "parallelism": f"replicas x{world}", "tracks_per_step": int(st.n_tracks),
                        "tracklets_per_step": nT, "start_hits_per_step": int(st.n_start_hits), "tracklet_hits": H},
             "tracks_per_s": float(st.n_tracks) * world / (ms_step * 1e-3),
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": ms_e2e, "steps": e2e_steps, "how": "tpcSubmitHost/tpcCollectHost, 2 slots, pinned host buffers"},
-            "gpu_launches": int(st.kernel_launches) * args.steps,
+            "gpu_launches": int(st.kernel_launches) * K,
             "clocks": clocks, "roofline": roofline, "stages": stages, "cpu_baseline": cpu}
     if refit_ms is not None:
         ncl = int(st.n_track_clusters)
@@ -402,6 +475,19 @@ def run_ours(args, rank, world, local_rank):
     print(json.dumps(line), flush=True)
 
 
+def _spawn(args, argv):
+    """`python bench.py --gpus N` without a launcher: start N ranks of this same command under torch.distributed.run
+    (one process per GPU, rendezvous on 127.0.0.1) and pass their exit code on."""
+    import socket
+    s = socket.socket()
+    s.bind(("127.0.0.1", 0))
+    port = s.getsockname()[1]
+    s.close()
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}", "--master-addr",
+           "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + argv
+    return subprocess.call(cmd)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -410,13 +496,24 @@ def main():
     ap.add_argument("--config", type=int, default=4, choices=sorted(WORKLOADS))
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--no-refit", action="store_true", help="skip the separate timing of the a6 refit (NEXT-2)")
+    ap.add_argument("--no-refit", action="store_true", help="skip the separate timing of the NEXT rows (a6..a10)")
+    ap.add_argument("--dry-run", action="store_true", help="N > 1 plumbing only (gloo, no GPU work): for the tests")
     args = ap.parse_args()
+    if args.gpus < 1 or args.steps < 1:
+        ap.error("--gpus and --steps must be >= 1")
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1 and args.impl == "ours":
+        sys.exit(_spawn(args, sys.argv[1:]))
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if world != args.gpus and args.impl == "ours":
+        print(f"bench.py: --gpus {args.gpus} but the launcher started {world} rank(s)", file=sys.stderr)
+        sys.exit(2)
     if args.impl == "reference":
         run_reference(args, rank)
+        return
+    if args.dry_run:
+        run_dry(args, rank, world)
         return
     run_ours(args, rank, world, local_rank)
     if world > 1:

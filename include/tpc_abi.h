@@ -39,7 +39,8 @@ enum {
   TPC_ERR_CAPACITY = -4,            /* an output capacity was exceeded: outputs truncated, nothing written out of
                                        bounds, required sizes are in tpcRunStatus */
   TPC_ERR_CUDA = -5,                /* a CUDA runtime call failed (tpcErrorString gives the last message) */
-  TPC_ERR_NONFINITE_INPUT = -6      /* validate_input was set and a cluster coordinate is NaN/Inf (R25) */
+  TPC_ERR_NONFINITE_INPUT = -6,     /* validate_input was set and a cluster coordinate is NaN/Inf (R25) */
+  TPC_ERR_OUT_OF_MEMORY = -7        /* host allocation of the handle failed */
 };
 
 typedef struct tpcHandle tpcHandle;
@@ -177,7 +178,8 @@ typedef struct {
   int64_t n_tracks;             /* required cap_tracks */
   int64_t n_track_clusters;     /* required cap_track_clusters */
   int64_t n_cells;              /* grid cells over all (sector,row) */
-  float stage_ms[8];            /* per-stage device times of the last run when profiling is on (else 0):
+  float stage_ms[8];            /* per-stage device times of the last tpcRun / tpcRunHost when profiling is on (else 0;
+                                   always 0 from tpcCollectHost: the stage events belong to the handle, not to a slot):
                                    0 grid, 1 neighbour finder, 2 cleaner+start hits, 3 constructor, 4 selector,
                                    5 optional refit, merger and exports, 6 total, 7 refit alone */
   float merge_ms;               /* the O7 merger alone (profiling on, merger requested) */

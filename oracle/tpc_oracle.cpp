@@ -247,6 +247,7 @@ struct orcResult {
   std::vector<int32_t> rf_status;
   std::vector<double> rf_x_in, rf_par_in, rf_cov_in, rf_chi2, rf_x_out, rf_par_out, rf_cov_out;
   int64_t o4_ops[4] = {0, 0, 0, 0};   // Propagates, Updates, Searches, clusters inside the roads (O4)
+  int64_t o2_ops[4] = {0, 0, 0, 0};   // clusters with a row pair, up candidates, down candidates, (u, d) pairs (O2)
   // O7 merger (NEXT-1)
   std::vector<int32_t> mg_next, mg_prev, mg_head;
   std::vector<double> mg_chi2;
@@ -384,6 +385,8 @@ struct Tracker {
       U.clear(); D.clear(); tyu.clear(); tzu.clear(); tyd.clear(); tzd.clear();
       forWindow(s * R + ru, Y[h], Z[h], wyu, wzu, [&](int32_t u) { U.push_back(u); });
       forWindow(s * R + rd, Y[h], Z[h], wyd, wzd, [&](int32_t d) { D.push_back(d); });
+      res.o2_ops[0] += 1; res.o2_ops[1] += (int64_t)U.size(); res.o2_ops[2] += (int64_t)D.size();
+      res.o2_ops[3] += (int64_t)U.size() * (int64_t)D.size();          // plain counters: no arithmetic depends on them
       if (U.empty() || D.empty()) continue;
       for (int32_t u : U) { tyu.push_back((Y[u] - Y[h]) * iu); tzu.push_back((Z[u] - Z[h]) * iu); }
       for (int32_t d : D) { tyd.push_back((Y[h] - Y[d]) * id); tzd.push_back((Z[h] - Z[d]) * id); }
@@ -831,6 +834,7 @@ void orcGetLinks(const orcResult* r, int32_t* ur, int32_t* dr, int32_t* u, int32
   copyOut(ur, r->up_raw); copyOut(dr, r->dn_raw); copyOut(u, r->up); copyOut(d, r->dn);
 }
 void orcGetO4Counts(const orcResult* r, int64_t* four) { for (int i = 0; i < 4; ++i) four[i] = r->o4_ops[i]; }
+void orcGetO2Counts(const orcResult* r, int64_t* four) { for (int i = 0; i < 4; ++i) four[i] = r->o2_ops[i]; }
 void orcGetStartHits(const orcResult* r, uint32_t* sh) { copyOut(sh, r->start_hits); }
 void orcGetRefit(const orcResult* r, int32_t* status, double* x_in, double* par_in, double* cov_in, double* chi2,
                  double* x_out, double* par_out, double* cov_out) {

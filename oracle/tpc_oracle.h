@@ -77,6 +77,9 @@ void orcGetStartHits(const orcResult*, uint32_t* start_hits);
 /* How often O4 ran Propagate, Update, Search, and how many clusters its Searches found inside their roads (four counts):
  * the algorithmic operation count of the measurement. */
 void orcGetO4Counts(const orcResult*, int64_t* four);
+/* The same for O2: clusters that have both a row above and a row below, their up candidates, their down candidates and
+ * the (u, d) pairs the definition evaluates (sum of nU * nD). */
+void orcGetO2Counts(const orcResult*, int64_t* four);
 /* O4: one entry per start hit (tracklet id = rank).  status: 0 discarded in the chain fit,
  * 1 built but rejected (nhits < min_tracklet_hits or no snapshot), 2 accepted.
  * rowhit [n_start*n_rows] global indices / -1; x [n_start]; par [n_start*5]; cov [n_start*15]. */

@@ -73,6 +73,8 @@ def _load():
         L.orcGetLinks.argtypes = [vp] * 5
         L.orcGetO4Counts.argtypes = [vp] * 2
         L.orcGetO4Counts.restype = None
+        L.orcGetO2Counts.argtypes = [vp] * 2
+        L.orcGetO2Counts.restype = None
         L.orcGetStartHits.argtypes = [vp] * 2
         L.orcGetTracklets.argtypes = [vp] * 10
         L.orcGetTracks.argtypes = [vp] * 12
@@ -173,6 +175,7 @@ class OracleResult:
     cf_res_z: np.ndarray | None = None
     cf_res_code: np.ndarray | None = None   # O11: the residuals as 16-bit integers (y16 | z16 << 16), pos_bits of the call
     o4_ops: np.ndarray | None = None        # O4: Propagates, Updates, Searches, clusters inside the roads (counters only)
+    o2_ops: np.ndarray | None = None        # O2: clusters with a row pair, up candidates, down candidates, pairs (counters only)
 
     @property
     def n_tracks(self) -> int:
@@ -231,13 +234,16 @@ def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool 
         ops = np.zeros(4, np.int64)
         L.orcGetO4Counts(h, _ptr(ops))
         rf["o4_ops"] = ops
+        ops2 = np.zeros(4, np.int64)
+        L.orcGetO2Counts(h, _ptr(ops2))
+        rf["o2_ops"] = ops2
         refit = refit or merge or flags or legs
         if refit:
             rst = np.zeros(nt, np.int32)
             rxi, rchi, rxo = np.zeros(nt), np.zeros(nt), np.zeros(nt)
             rpi, rpo, rci, rco = np.zeros((nt, 5)), np.zeros((nt, 5)), np.zeros((nt, 15)), np.zeros((nt, 15))
             L.orcGetRefit(h, _ptr(rst), _ptr(rxi), _ptr(rpi), _ptr(rci), _ptr(rchi), _ptr(rxo), _ptr(rpo), _ptr(rco))
-            rf = dict(rf_status=rst, rf_x_in=rxi, rf_par_in=rpi, rf_cov_in=rci, rf_chi2=rchi, rf_x_out=rxo, rf_par_out=rpo,
+            rf.update(rf_status=rst, rf_x_in=rxi, rf_par_in=rpi, rf_cov_in=rci, rf_chi2=rchi, rf_x_out=rxo, rf_par_out=rpo,
                       rf_cov_out=rco)
         if merge:
             mn, mp, mh = (np.full(nt, -1, np.int32) for _ in range(3))

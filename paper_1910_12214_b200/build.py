@@ -52,5 +52,15 @@ def build_cuda(force: bool = False, verbose: bool = False, defines=(), out: str 
     return LIB
 
 
+def emit_ptx(out: str) -> str:
+    """The PTX of every kernel under the product's own arithmetic flags (for tests/test_build_flags.py: R0 is a property
+    of the generated code, not only of a command line)."""
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    flags = [f for f in NVCC_FLAGS if f not in ("-shared", "-Xcompiler", "-fPIC", "-lineinfo")]
+    flags[flags.index("-gencode") + 1] = "arch=compute_100a,code=compute_100a"
+    subprocess.check_call([nvcc] + flags + ["-ptx", os.path.join(CSRC, "tpc_api.cu"), "-o", out])
+    return out
+
+
 if __name__ == "__main__":
     print(build_cuda(force=True, verbose=True))

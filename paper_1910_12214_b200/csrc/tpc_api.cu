@@ -238,7 +238,7 @@ int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cud
   if (p->pos_bits < 0 || p->pos_bits > 15) return TPC_ERR_INVALID_ARG;
   if (p->leg_max_sectors < 0 || p->leg_max_sectors > LEG_MAX_SECTORS || p->leg_max_row_diff < 0) return TPC_ERR_INVALID_ARG;
   tpcHandle* h = new (std::nothrow) tpcHandle();
-  if (!h) return TPC_ERR_INVALID_ARG;
+  if (!h) return TPC_ERR_OUT_OF_MEMORY;
   h->device = cuda_device;
   h->params = *p;
   DevParams& P = h->P;
@@ -303,11 +303,11 @@ int tpcDestroy(tpcHandle* h) {
   if (h->h_cnt) cudaFreeHost(h->h_cnt);
   if (h->ev_done) cudaEventDestroy(h->ev_done);
   for (int i = 0; i < 17; ++i) if (h->ev_stage[i]) cudaEventDestroy(h->ev_stage[i]);
-  if (h->cur_slot != 0) {}   // the active state is freed below; the parked slots here
+  // the active state is freed below; the parked slots here, whatever part of them was initialised
   for (int k = 0; k < 3; ++k) {
-    if (k == h->cur_slot || !h->slots[k].init) continue;
+    if (k == h->cur_slot) continue;
     tpcHandle::Slot& S = h->slots[k];
-    cudaFree(S.d_cnt); if (S.h_cnt) cudaFreeHost(S.h_cnt); if (S.ev_done) cudaEventDestroy(S.ev_done);
+    if (S.d_cnt) cudaFree(S.d_cnt); if (S.h_cnt) cudaFreeHost(S.h_cnt); if (S.ev_done) cudaEventDestroy(S.ev_done);
     for (int i = 0; i < 16; ++i) if (S.pool[i]) cudaFree(S.pool[i]);
   }
   for (int k = 1; k < 3; ++k) {
@@ -645,6 +645,7 @@ const char* tpcErrorString(int code) {
     case TPC_ERR_CAPACITY: return "output capacity exceeded (outputs truncated; see tpcRunStatus for required sizes)";
     case TPC_ERR_CUDA: return "CUDA runtime error";
     case TPC_ERR_NONFINITE_INPUT: return "non-finite cluster coordinate";
+    case TPC_ERR_OUT_OF_MEMORY: return "out of host memory";
     default: return "unknown error";
   }
 }
@@ -864,6 +865,10 @@ extern "C" int tpcCollectHost(tpcHandle* h, int slot, tpcRunStatus* status) {
   rc = tpcGetRunStatus(h, status);            // waits for the slot's last event: run and copies are complete
   S.submitted = false;
   if (rc == TPC_OK) {
+    // the per-stage events belong to the handle, not to the slot: with two events in flight they may be the other
+    // slot's.  Per-stage times are valid for tpcRun / tpcRunHost only.
+    memset(status->stage_ms, 0, sizeof(status->stage_ms));
+    status->merge_ms = status->flags_ms = status->pack_ms = status->legs_ms = 0.0f;
     float ms = 0;
     if (cudaEventElapsedTime(&ms, S.ev_begin, S.ev_kernels) == cudaSuccess) status->submit_ms[0] = ms;
     if (cudaEventElapsedTime(&ms, S.ev_begin, h->ev_done) == cudaSuccess) status->submit_ms[1] = ms;

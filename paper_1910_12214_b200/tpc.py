@@ -21,6 +21,7 @@ TPC_ERR_WORKSPACE_TOO_SMALL = -3
 TPC_ERR_CAPACITY = -4
 TPC_ERR_CUDA = -5
 TPC_ERR_NONFINITE_INPUT = -6
+TPC_ERR_OUT_OF_MEMORY = -7
 
 
 class tpcGeometry(ctypes.Structure):

@@ -65,3 +65,27 @@ def test_reference_arm_runs_on_rank_zero_only(tmp_path):
     import json
     line = json.loads(out.stdout.strip().splitlines()[-1])
     assert line["impl"] == "reference" and line["value"] > 0 and line["cpu_baseline"]["kind"] == "oracle"
+
+
+def test_bench_spawns_its_own_ranks_when_no_launcher_did():
+    """`python bench.py --gpus 2` without WORLD_SIZE starts two ranks itself (torch.distributed.run on 127.0.0.1); with
+    --dry-run they rendezvous over gloo, each contributes its own figures through bench.aggregate(), and rank 0 alone
+    prints the one line: units summed over ranks (1000 + 2000), time = max over ranks (20 ms), n_gpus = the world used."""
+    import json
+    import subprocess
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--dry-run"], capture_output=True,
+                         text=True, env=env, timeout=300)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    line = json.loads(lines[0])
+    assert line["n_gpus"] == 2 and line["units"] == 3000.0 and line["ms"] == 20.0
+
+
+def test_bench_refuses_a_world_that_differs_from_gpus():
+    import subprocess
+    env = dict(os.environ, RANK="0", WORLD_SIZE="1", LOCAL_RANK="0")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "8", "--dry-run"], capture_output=True,
+                         text=True, env=env, timeout=120)
+    assert out.returncode == 2 and "--gpus 8" in out.stderr

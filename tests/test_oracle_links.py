@@ -272,3 +272,21 @@ def test_non_finite_input_is_rejected():
     ev = _event({10: [(float("nan"), 0.0)]})
     with pytest.raises(ValueError):
         orc.run(ev)
+
+
+def test_o2_operation_counters_on_a_hand_case():
+    """The O2 counters behind bench.py's operation count of the neighbour finder (no arithmetic depends on them): three
+    collinear clusters on rows 10, 11, 12 plus one far-away cluster on row 11.  Every cluster has a row above and below (4);
+    up candidates: the cluster of row 10 sees 1 (the far one is outside its window), that of row 11 sees 1, the far one 0,
+    row 12 none: 2; down candidates likewise 2; pairs: 1 * 0 + 1 * 1 + 0 * 0 + 0 * 1 = 1."""
+    from paper_1910_12214_b200.datagen import default_row_x
+    X = default_row_x()
+    counts = np.zeros(152, np.int64)
+    counts[10], counts[11], counts[12] = 1, 2, 1
+    off = np.concatenate([[0], np.cumsum(counts)])
+    y = [0.0, 0.3 * (X[11] - X[10]), 40.0, 0.3 * (X[12] - X[10])]
+    z = [5.0, 5.0, -100.0, 5.0]
+    res = orc.run(datagen.event_from_arrays(off, y, z, 1, 152))
+    assert res.o2_ops.tolist() == [4, 2, 2, 1]
+    assert res.link_up_raw.tolist() == [-1, 3, -1, -1] and res.link_dn_raw.tolist() == [-1, 0, -1, -1]
+    assert res.link_up.tolist() == [-1] * 4            # the end clusters have no pair, so nothing is reciprocal
