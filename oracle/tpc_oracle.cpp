@@ -254,6 +254,9 @@ struct orcResult {
   // O10 looper legs (rest of NEXT-1)
   std::vector<int32_t> lg_partner;
   std::vector<double> lg_chi2;
+  // O12 merged tracks (NEXT-1 / NEXT-3): merged-track id and leg rank per track, cluster lists per merged track
+  std::vector<int32_t> mt_id, mt_rank;
+  std::vector<uint32_t> mt_cl_offset, mt_cl_index;
   // O8 cluster flags (NEXT-3)
   std::vector<uint8_t> cf_flags;
   std::vector<int32_t> cf_owner;
@@ -594,6 +597,55 @@ struct Tracker {
     }
   }
 
+  // ---- O12 merged tracks and leg labels (O12; readings R46..R48) ------
+  // A leg = an O7 chain head, next(head), ...; a merged track = one leg, or two legs whose LAST tracks are O10 partners
+  // (the two sides of an outer turn).  Of two legs the primary ("first") is the one whose innermost kept
+  // cluster has the smaller |z| (R48); ties -> the smaller head index.  Cluster list of a merged track: the primary leg
+  // from its inner end outwards, then the secondary leg from the turn inwards -- the order along the particle's path.
+  void mergedAll() {
+    const int64_t nt = (int64_t)res.tr_id.size();
+    res.mt_id.assign(nt, -1); res.mt_rank.assign(nt, 0);
+    const bool haveLegs = (int64_t)res.lg_partner.size() == nt;
+    auto tailOf = [&](int64_t k) { for (int64_t g = 0; res.mg_next[k] >= 0 && g < nt; ++g) k = res.mg_next[k]; return k; };
+    auto innerAbsZ = [&](int64_t h) { return std::fabs(Z[res.tr_cl_index[res.tr_cl_offset[h]]]); };
+    std::vector<int32_t> otherHead(nt, -1);
+    for (int64_t h = 0; h < nt; ++h) {
+      if (res.mg_head[h] != (int32_t)h) continue;          // heads only: one pass per leg
+      const int64_t tl = tailOf(h);
+      const int32_t p = haveLegs ? res.lg_partner[tl] : -1;
+      const int32_t other = (p >= 0 && res.mg_next[p] < 0) ? res.mg_head[p] : -1;     // the partner must end its own leg
+      otherHead[h] = other;
+      int32_t rank = 0, id = (int32_t)h;
+      if (other >= 0) {
+        const Real za = innerAbsZ(h), zb = innerAbsZ(other);
+        const bool primary = za < zb || (za == zb && (int32_t)h < other);
+        rank = primary ? 0 : 1;
+        id = (int32_t)h < other ? (int32_t)h : other;
+      }
+      for (int64_t k = h; k >= 0; k = res.mg_next[k]) { res.mt_id[k] = id; res.mt_rank[k] = rank; }
+    }
+    res.mt_cl_offset.assign(1, 0);
+    res.mt_cl_index.clear();
+    std::vector<int64_t> chain;
+    for (int64_t k = 0; k < nt; ++k) {
+      if (res.mt_id[k] == (int32_t)k && res.mg_head[k] == (int32_t)k) {   // k represents its merged track
+        int64_t first = k, second = otherHead[k];
+        if (second >= 0 && res.mt_rank[k] == 1) { first = second; second = k; }
+        for (int64_t a = first; a >= 0; a = res.mg_next[a])
+          for (uint32_t i = res.tr_cl_offset[a]; i < res.tr_cl_offset[a + 1]; ++i) res.mt_cl_index.push_back(res.tr_cl_index[i]);
+        if (second >= 0) {
+          chain.clear();
+          for (int64_t a = second; a >= 0; a = res.mg_next[a]) chain.push_back(a);
+          for (size_t c = chain.size(); c-- > 0;) {
+            const int64_t a = chain[c];
+            for (uint32_t i = res.tr_cl_offset[a + 1]; i-- > res.tr_cl_offset[a];) res.mt_cl_index.push_back(res.tr_cl_index[i]);
+          }
+        }
+      }
+      res.mt_cl_offset.push_back((uint32_t)res.mt_cl_index.size());
+    }
+  }
+
   // ---- O8 cluster flags (O8; readings R34..R37) ---------------------------
   void flagAll() {
     const int64_t nt = (int64_t)res.tr_id.size();
@@ -603,7 +655,8 @@ struct Tracker {
     const Real msp = (Real)P.max_sinphi, tube2 = (Real)P.tube_radius * (Real)P.tube_radius;
     const Real sin70 = (Real)0.9396926207859084, qmax = (Real)P.inv_pt_protect;
     std::vector<Real> ownerQ(N, 0);
-    std::vector<uint8_t> ownerBad(N, 0);         // owner is low or steep at the cluster's row
+    std::vector<uint8_t> protAny(N, 0);          // some track that is neither low, steep nor a secondary leg has it in its tube
+    const bool haveRanks = (int64_t)res.mt_rank.size() == nt;      // leg labels of O12 (else R37: every track is primary)
     for (int64_t k = 0; k < nt; ++k) {
       if (!res.rf_status[k]) continue;
       State<Real> st{};
@@ -612,6 +665,7 @@ struct Tracker {
       for (int i = 0; i < 15; ++i) st.C[i] = (Real)res.rf_cov_in[k * 15 + i];
       const Real aq = std::fabs(st.q);
       const bool low = !(aq < qmax);
+      const bool secondary = haveRanks && res.mt_rank[k] == 1;     // only the primary, first leg protects
       const int sec = res.tr_sector[k];
       const uint32_t* cl = res.tr_cl_index.data() + res.tr_cl_offset[k];
       const int ncl = (int)(res.tr_cl_offset[k + 1] - res.tr_cl_offset[k]);
@@ -619,7 +673,7 @@ struct Tracker {
       for (int r = res.tr_first[k]; r <= res.tr_last[k]; ++r) {
         if (dead(r)) continue;
         if (r > res.tr_first[k] && !propagate(st, X[r], bf, msp)) break;
-        const bool bad = low || !(std::fabs(st.s) < sin70);
+        const bool bad = low || secondary || !(std::fabs(st.s) < sin70);
         while (ic < ncl && rowOf[cl[ic]] < r) ++ic;
         const int32_t own = (ic < ncl && rowOf[cl[ic]] == r) ? (int32_t)cl[ic] : -1;     // the attached cluster of this row
         if (own >= 0) { res.cf_res_y[own] = (double)(Y[own] - st.y); res.cf_res_z[own] = (double)(Z[own] - st.z); }   // R39
@@ -627,8 +681,9 @@ struct Tracker {
           const Real dy = Y[c] - st.y, dz = Z[c] - st.z;
           const Real d2 = dy * dy + dz * dz;
           if (!(d2 <= tube2) && (int32_t)c != own) continue;
+          if (!bad) protAny[c] = 1;                         // R36b: every good track protects what is in its tube
           if (res.cf_owner[c] < 0 || aq < ownerQ[c]) {      // ties: the lower track index (loop order)
-            res.cf_owner[c] = (int32_t)k; ownerQ[c] = aq; ownerBad[c] = bad ? 1 : 0;
+            res.cf_owner[c] = (int32_t)k; ownerQ[c] = aq;
           }
         }
       }
@@ -637,7 +692,7 @@ struct Tracker {
       for (uint32_t i = res.tr_cl_offset[k]; i < res.tr_cl_offset[k + 1]; ++i) res.cf_flags[res.tr_cl_index[i]] |= 1;
     for (int64_t c = 0; c < N; ++c) {
       uint8_t f = res.cf_flags[c];
-      const bool has = res.cf_owner[c] >= 0, prot = has && !ownerBad[c];
+      const bool has = res.cf_owner[c] >= 0, prot = has && protAny[c];
       if (has) f |= 2;
       if (prot) f |= 4;
       if (has && !prot) f |= 8;
@@ -811,12 +866,13 @@ int orcRun(const orcGeometry* g, const orcParams* p, int64_t n, const uint32_t* 
   orcResult* r = new orcResult();
   r->n = n; r->n_sectors = g->n_sectors; r->n_rows = g->n_rows;
   r->fp64 = (flags & ORC_FP64) != 0; r->brute = (flags & ORC_BRUTE_FORCE) != 0;
-  const bool mg = (flags & ORC_MERGE) != 0;
+  const bool md = (flags & ORC_MERGED) != 0;
+  const bool mg = md || (flags & ORC_MERGE) != 0;
   const bool fg = (flags & ORC_FLAGS) != 0;
-  const bool lg = (flags & ORC_LEGS) != 0;
+  const bool lg = md || (flags & ORC_LEGS) != 0;
   const bool rf = mg || fg || lg || (flags & ORC_REFIT) != 0;
-  if (r->fp64) { Tracker<double> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); if (rf) T.refitAll(); if (mg) T.mergeAll(); if (lg) T.legAll(); if (fg) T.flagAll(); }
-  else { Tracker<float> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); if (rf) T.refitAll(); if (mg) T.mergeAll(); if (lg) T.legAll(); if (fg) T.flagAll(); }
+  if (r->fp64) { Tracker<double> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); if (rf) T.refitAll(); if (mg) T.mergeAll(); if (lg) T.legAll(); if (md) T.mergedAll(); if (fg) T.flagAll(); }
+  else { Tracker<float> T(*g, *p, n, off, y, z, r->brute, *r); T.run(); if (rf) T.refitAll(); if (mg) T.mergeAll(); if (lg) T.legAll(); if (md) T.mergedAll(); if (fg) T.flagAll(); }
   *out = r;
   return ORC_OK;
 }
@@ -845,6 +901,9 @@ void orcGetRefit(const orcResult* r, int32_t* status, double* x_in, double* par_
 void orcGetClusterFlags(const orcResult* r, uint8_t* flags, int32_t* owner) { copyOut(flags, r->cf_flags); copyOut(owner, r->cf_owner); }
 void orcGetResiduals(const orcResult* r, double* ry, double* rz) { copyOut(ry, r->cf_res_y); copyOut(rz, r->cf_res_z); }
 void orcGetLegs(const orcResult* r, int32_t* partner, double* chi2) { copyOut(partner, r->lg_partner); copyOut(chi2, r->lg_chi2); }
+void orcGetMerged(const orcResult* r, int32_t* id, int32_t* rank, uint32_t* cl_offset, uint32_t* cl_index) {
+  copyOut(id, r->mt_id); copyOut(rank, r->mt_rank); copyOut(cl_offset, r->mt_cl_offset); copyOut(cl_index, r->mt_cl_index);
+}
 void orcGetMerge(const orcResult* r, int32_t* next, int32_t* prev, int32_t* head, double* chi2) {
   copyOut(next, r->mg_next); copyOut(prev, r->mg_prev); copyOut(head, r->mg_head); copyOut(chi2, r->mg_chi2);
 }

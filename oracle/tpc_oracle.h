@@ -52,7 +52,8 @@ typedef struct orcResult orcResult;
 
 enum { ORC_OK = 0, ORC_ERR_INVALID_ARG = -1, ORC_ERR_UNSORTED_OFFSETS = -2 };
 enum { ORC_BRUTE_FORCE = 1, ORC_FP64 = 2, ORC_REFIT = 4, ORC_MERGE = 8 /* implies ORC_REFIT */,
-       ORC_FLAGS = 16 /* implies ORC_REFIT */, ORC_LEGS = 32 /* implies ORC_REFIT */ };
+       ORC_FLAGS = 16 /* implies ORC_REFIT */, ORC_LEGS = 32 /* implies ORC_REFIT */,
+       ORC_MERGED = 64 /* implies ORC_MERGE and ORC_LEGS */ };
 
 void orcDefaultParams(orcParams* p);
 
@@ -107,7 +108,8 @@ int orcRefitPoints(const orcGeometry* g, const orcParams* p, int n, const int32_
  * to next (0 if none).  Pins: tests/test_oracle_merge.py. */
 void orcGetMerge(const orcResult*, int32_t* next, int32_t* prev, int32_t* head, double* chi2);
 /* O8 (NEXT-3 of SURVEY.md 8(f), DESIGN.md section 3 "O8"): per-cluster flags, only with ORC_FLAGS.
- * flags [n_clusters] bit mask 1 attached, 2 adjacent, 4 protected, 8 removed by strategy A, 16 removed by strategy B;
+ * flags [n_clusters] bit mask 1 attached, 2 adjacent, 4 protected (some track with pT > 50 MeV/c, |phi| < 70 degrees on that
+ * row and not a secondary leg has the cluster in its tube), 8 removed by strategy A, 16 removed by strategy B;
  * owner [n_clusters] track index of the highest-momentum track with the cluster in its tube, -1 none. */
 void orcGetClusterFlags(const orcResult*, uint8_t* flags, int32_t* owner);
 /* track-model residuals (O8, R39) of the clusters attached to refitted tracks, 0 elsewhere;
@@ -135,6 +137,14 @@ int orcMatch(const orcParams* p, double bz_tesla, const double* a_state, const d
  * only with ORC_LEGS.  partner [n_tracks] = the track whose outer end is the other side of this track's outer turn
  * (-1 none; partner[partner[k]] == k), chi2 [n_tracks] of that pair (0 if none).  Pins: tests/test_oracle_legs.py. */
 void orcGetLegs(const orcResult*, int32_t* partner, double* chi2);
+/* O12 (rest of NEXT-1 and what NEXT-3 needs of it; DESIGN.md section 3 "O12", readings R46..R48; "only the
+ * primary, first leg is protected", L86, L92 "merging of track segments and legs of the same track"): merged tracks, only
+ * with ORC_MERGED.  id [n_tracks] = the merged track of every track (the smallest head index of its one or two legs),
+ * rank [n_tracks] 0 = on the primary (first) leg, 1 = on the secondary leg; cl_offset [n_tracks + 1], cl_index
+ * [n_track_clusters]: cluster list of the merged track in the order along the particle's path, stored at the index of the
+ * track that names it (empty ranges elsewhere).  With ORC_FLAGS | ORC_MERGED the cluster flags treat secondary legs as
+ * not protecting and their clusters as removable by strategy A (L86).  Pins: tests/test_oracle_merged.py. */
+void orcGetMerged(const orcResult*, int32_t* id, int32_t* rank, uint32_t* cl_offset, uint32_t* cl_index);
 /* Pieces of O10 for the pins.  orcMirror: the state seen from the frame turned by 180 degrees and walked backwards.
  * orcLegMatch: chi2 of two outer states a, b (b's sector d sectors after a's); returns 1 and *chi2 when admissible. */
 void orcMirror(double* state, double* cov);

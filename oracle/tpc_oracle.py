@@ -23,6 +23,7 @@ REFIT = 4
 MERGE = 8
 FLAGS = 16
 LEGS = 32
+MERGED = 64
 
 
 def build(force: bool = False) -> str:
@@ -96,6 +97,8 @@ def _load():
         L.orcMatch.restype = ci
         L.orcGetLegs.argtypes = [vp] * 3
         L.orcGetLegs.restype = None
+        L.orcGetMerged.argtypes = [vp] * 5
+        L.orcGetMerged.restype = None
         L.orcMirror.argtypes = [vp, vp]
         L.orcMirror.restype = None
         L.orcLegMatch.argtypes = [ctypes.POINTER(Params), dbl, vp, vp, ci, vp, vp, ci, vp]
@@ -168,6 +171,11 @@ class OracleResult:
     # O10 looper legs (only with legs=True): the track on the other side of the outer turn, chi2 of the pair
     lg_partner: np.ndarray | None = None
     lg_chi2: np.ndarray | None = None
+    # O12 merged tracks (only with merged=True): merged-track id and leg rank per track, cluster lists along the path
+    mt_id: np.ndarray | None = None
+    mt_rank: np.ndarray | None = None
+    mt_cl_offset: np.ndarray | None = None
+    mt_cl_index: np.ndarray | None = None
     # O8 cluster flags (only with flags=True): bit mask per cluster and the owning track
     cf_flags: np.ndarray | None = None
     cf_owner: np.ndarray | None = None
@@ -188,7 +196,7 @@ def _ptr(a):
 
 def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool = False,
         stages_only: bool = False, refit: bool = False, merge: bool = False, flags: bool = False,
-        legs: bool = False, pos_bits: int = 6) -> OracleResult:
+        legs: bool = False, pos_bits: int = 6, merged: bool = False) -> OracleResult:
     """Run O1..O5 on an Event-like object (fields n_sectors, n_rows, row_x, row_dead, bz_tesla,
     tan_half_sector, z_min, z_max, row_offset, y, z; numpy arrays)."""
     L = _load()
@@ -203,7 +211,7 @@ def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool 
     n = int(y.shape[0])
     h = ctypes.c_void_p()
     rc = L.orcRun(ctypes.byref(g), ctypes.byref(p), n, off.ctypes.data, _ptr(y), _ptr(z),
-                  (BRUTE_FORCE if brute_force else 0) | (FP64 if fp64 else 0) | (REFIT if refit else 0) | (MERGE if merge else 0) | (FLAGS if flags else 0) | (LEGS if legs else 0),
+                  (BRUTE_FORCE if brute_force else 0) | (FP64 if fp64 else 0) | (REFIT if refit else 0) | (MERGE if merge else 0) | (FLAGS if flags else 0) | (LEGS if legs else 0) | (MERGED if merged else 0),
                   ctypes.byref(h))
     if rc != 0:
         raise ValueError(f"orcRun failed with {rc}")
@@ -237,6 +245,8 @@ def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool 
         ops2 = np.zeros(4, np.int64)
         L.orcGetO2Counts(h, _ptr(ops2))
         rf["o2_ops"] = ops2
+        merge = merge or merged
+        legs = legs or merged
         refit = refit or merge or flags or legs
         if refit:
             rst = np.zeros(nt, np.int32)
@@ -254,6 +264,11 @@ def run(ev, params: Params | None = None, brute_force: bool = False, fp64: bool 
             lp, lc = np.full(nt, -1, np.int32), np.zeros(nt)
             L.orcGetLegs(h, _ptr(lp), _ptr(lc))
             rf.update(lg_partner=lp, lg_chi2=lc)
+        if merged:
+            mi, mr = np.full(nt, -1, np.int32), np.zeros(nt, np.int32)
+            mo, mx = np.zeros(nt + 1, np.uint32), np.zeros(ntc, np.uint32)
+            L.orcGetMerged(h, _ptr(mi), _ptr(mr), _ptr(mo), _ptr(mx))
+            rf.update(mt_id=mi, mt_rank=mr, mt_cl_offset=mo, mt_cl_index=mx)
         if flags:
             cf, co = np.zeros(n, np.uint8), np.full(n, -1, np.int32)
             L.orcGetClusterFlags(h, _ptr(cf), _ptr(co))

@@ -45,6 +45,8 @@ struct Workspace {
   unsigned long long* tiles64;
   uint32_t *start_orig, *start_pos;
   SeedRec* work_list;        // long seeds, in the order the constructor takes them
+  TurnRec* turn_list;        // [capT] constructUp -> constructDown<0>
+  uint4* down_list;          // [capT][DOWNREC_WORDS / 4] constructDown<0> -> constructDown<1>
   TrackletStore tl;
   unsigned long long *tsel, *tscan;
   int32_t *kept_first, *kept_last;
@@ -85,7 +87,7 @@ struct tpcHandle {
   //   // 0..6 stage boundaries, 7/8 around the optional refit, 9/10 merger, 11/12 flags
   int profiling = 0;
   int launches = 0;
-  int tc_grid = 148;               // persistent grid of the tracklet constructor: SMs x resident blocks
+  int tc_grid[3] = {148, 148, 148};   // persistent grids of the three constructor passes: SMs x resident blocks
   bool pending = false;
   int64_t last_n = 0;
   double cells_per_bucket_bound = 0;   // sum over buckets of the n-independent part of the cell bound
@@ -153,6 +155,8 @@ Workspace layout(const tpcHandle* h, int64_t N, int64_t capT, char* base) {
   w.start_orig = (uint32_t*)take(4 * (size_t)Tn);
   w.start_pos = (uint32_t*)take(4 * (size_t)Tn);
   w.work_list = (SeedRec*)take(sizeof(SeedRec) * (size_t)Tn);
+  w.turn_list = (TurnRec*)take(sizeof(TurnRec) * (size_t)Tn);
+  w.down_list = (uint4*)take(4 * (size_t)DOWNREC_WORDS * (size_t)Tn);
   w.tl.capT = capT;
   w.tl.n_rows = R;
   w.tl.status = (int32_t*)take(4 * (size_t)Tn);
@@ -284,11 +288,14 @@ int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cud
        cudaMemcpy(h->d_dead, dead.data(), R, cudaMemcpyHostToDevice) == cudaSuccess;
   if (!ok) { tpcDestroy(h); return TPC_ERR_CUDA; }
   {
-    int sms = 148, per_sm = 1;
+    int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, cuda_device);
-    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, trackletConstructor, TC_THREADS, 0) != cudaSuccess || per_sm < 1)
-      per_sm = 1;
-    h->tc_grid = sms * per_sm;
+    const void* pass[3] = {(const void*)constructUp, (const void*)constructDown<0>, (const void*)constructDown<1>};
+    for (int i = 0; i < 3; ++i) {
+      int per_sm = 1;
+      if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pass[i], TC_THREADS, 0) != cudaSuccess || per_sm < 1) per_sm = 1;
+      h->tc_grid[i] = sms * per_sm;
+    }
   }
   memset(h->h_cnt, 0, 8 * (CNT_COUNT + 1));
   *out = h;
@@ -418,11 +425,15 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   stage(3);
   // ---- a4 tracklet constructor --------------------------------------------------------------------
   if (N > 0 && capT > 0) {
-    const unsigned grid = (unsigned)std::min<int64_t>(ceilDiv(capT, TC_THREADS), h->tc_grid);
+    const int64_t blocks = ceilDiv(capT, TC_THREADS);
     seedPrepare<<<(unsigned)ceilDiv(capT, 128), 128, 0, st>>>(in->row_offset, P, T, w.syz, w.cup, w.start_pos, w.work_list,
                                                               w.tl, cnt); ++L;
-    trackletConstructor<<<grid, TC_THREADS, 0, st>>>(P, T, w.desc, w.cell_start, w.syz, w.s2o, w.cup, w.work_list,
-                                                     w.tl, cnt); ++L;
+    constructUp<<<(unsigned)std::min<int64_t>(blocks, h->tc_grid[0]), TC_THREADS, 0, st>>>(
+        P, T, w.desc, w.cell_start, w.syz, w.s2o, w.cup, w.work_list, w.turn_list, w.tl, cnt); ++L;
+    constructDown<0><<<(unsigned)std::min<int64_t>(blocks, h->tc_grid[1]), TC_THREADS, 0, st>>>(
+        P, T, w.desc, w.cell_start, w.syz, w.s2o, w.turn_list, w.down_list, w.tl, cnt); ++L;
+    constructDown<1><<<(unsigned)std::min<int64_t>(blocks, h->tc_grid[2]), TC_THREADS, 0, st>>>(
+        P, T, w.desc, w.cell_start, w.syz, w.s2o, w.turn_list, w.down_list, w.tl, cnt); ++L;
   }
   stage(4);
   // optional per-stage export of the tracklets: before the selector, which compacts the row-hit slices in place

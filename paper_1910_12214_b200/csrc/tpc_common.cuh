@@ -40,10 +40,12 @@ enum Counter {
   CNT_N_TRACKS = 4,     // tracks found (may exceed cap_tracks)
   CNT_N_TRK_CL = 5,     // track clusters (may exceed cap)
   CNT_N_CELLS = 6,
-  CNT_WORK = 7,         // dynamic work counter of the constructor
+  CNT_WORK = 7,         // dynamic work counter of the constructor's up pass
   CNT_N_LONG = 8,       // seeds whose link chain is long enough to survive the chain fit (the constructor's work list)
   CNT_INF = 9,          // a count larger than any array: "scan everything" for the device-counted scan kernels
-  CNT_COUNT = 10
+  CNT_WORK2 = 10,       // work counters of the two down-pass kernels of the constructor
+  CNT_WORK3 = 11,
+  CNT_COUNT = 12
 };
 
 // Tracklet SoA in the workspace (capT = capacity in tracklets).

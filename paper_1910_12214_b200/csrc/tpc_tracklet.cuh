@@ -199,58 +199,105 @@ __global__ void __launch_bounds__(128) seedPrepare(const uint32_t* __restrict__ 
   out.status[t] = 0; out.nhits[t] = nhits; out.first_row[t] = -1; out.last_row[t] = -1;
 }
 
-// Persistent warps; every lane owns one seed at a time and fetches the next one from a global counter as soon
-// as its seed is finished ("lane refill"), so a warp stays full although seeds need between 1 and ~300 steps.
-// The three passes of O4 (chain fit, up extrapolation, down pass) are folded into ONE step body
-//     Propagate -> candidate (link | known hit | Search) -> Update -> bookkeeping
-// driven by a per-lane phase, so that all lanes execute the expensive Kalman arithmetic together.  Loads are
-// software-pipelined around the arithmetic: the hit of a step (link or known row hit) is fetched one step
-// ahead, its coordinates and the row's grid descriptor are requested before Propagate, the cell ranges of a
-// search from inside Propagate.  The order of floating-point operations of a seed is exactly the sequential
-// algorithm's.
-#ifdef TC_MAXNREG
-__global__ void __maxnreg__(TC_MAXNREG) trackletConstructor(
-#else
-__global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor(
-#endif
-    DevParams P, RowTables T, const GridDesc* __restrict__ desc, const uint32_t* __restrict__ cell_start,
-    const float2* __restrict__ syz, const uint32_t* __restrict__ s2o, const int32_t* __restrict__ cup,
-    const SeedRec* __restrict__ work_list, TrackletStore out, int64_t* __restrict__ cnt) {
-  __shared__ float sx[MAX_ROWS];
-  __shared__ int16_t sup[MAX_ROWS];          // up_row (R2)
-  __shared__ int16_t snu[MAX_ROWS];          // next live row above (n_rows if none)
-  __shared__ int16_t snd[MAX_ROWS];          // next live row below (-1 if none)
-  __shared__ float snap[22][TC_THREADS];     // state after the last Update of the down pass (O4 step 5)
-  // per-lane bookkeeping that is read once per step or less lives in shared memory (volatile: re-read where used):
-  // in registers it pushed the kernel over 96 and the spilled bucket base sat on the path to every grid load
-  __shared__ volatile uint32_t s_t[TC_THREADS];       // tracklet id
-  __shared__ volatile int s_bsec[TC_THREADS];         // first bucket of the seed's sector
-  __shared__ volatile int16_t s_rtop[TC_THREADS];     // top row of the down pass
-  __shared__ volatile int16_t s_rc[TC_THREADS];       // chain fit: row of the last Propagate
-  if (cnt[CNT_ERROR] != 0) return;
-  const int R = P.n_rows;
-  const int tid = threadIdx.x;
-  for (int i = tid; i < R; i += blockDim.x) {
-    sx[i] = T.row_x[i]; sup[i] = T.up_row[i];
+// ---- the three passes of O4 as three persistent kernels -------------------------------------------------------------
+// Every lane owns one seed at a time and fetches the next one from a global counter as soon as its seed is finished
+// ("lane refill"), so a warp stays full although seeds need between 1 and ~150 steps per pass.  A step is
+//     Propagate -> candidate (link | known hit | Search) -> Update -> bookkeeping.
+// The passes run as SEPARATE kernels so that the lanes of a warp do the same kind of step:
+//   constructUp        chain fit (links) and up extrapolation (a Search per row)          -> TurnRec  (32 bytes per seed)
+//   constructDown<0>   down pass over the span [r0, top]: the hits are known, Searches only on the rare gap rows
+//                                                                                         -> DownRec (112 bytes per seed)
+//   constructDown<1>   down pass below r0: a Search per row, miss counting                 -> the tracklet
+// In one kernel (round 1) the Search code ran whenever any lane of the warp wanted it, at 19.6 of 32 lanes, and the
+// phase bookkeeping at 12.3 lanes.  The hand-off records cost 0.3 GB of writes and reads per event, the time of 0.1 ms.
+// The order of the floating-point operations of a seed is exactly the sequential algorithm's; the turn (O4 step 4) keeps
+// only the parameters, so a TurnRec carries five floats.
+// Loads are software-pipelined around the arithmetic: the hit of a step (link or known row hit) is fetched one step
+// ahead, its coordinates and the row's grid descriptor are requested before Propagate, the cell ranges of a search from
+// inside Propagate.
+
+constexpr uint32_t REC_NONE = 0xFFFFFFFFu;
+
+struct TurnRec {           // state of a seed at the turn (O4 step 4)
+  uint32_t t;              // tracklet id; REC_NONE = the seed ended in the chain fit
+  int32_t last_c;          // the hit on the top row
+  float y, z, s, tt, q;    // parameters at plane row_x[rx]
+  uint32_t rows;           // r0 | top row << 8 | rx << 16
+};
+static_assert(sizeof(TurnRec) == 32, "TurnRec is two 16-byte words");
+
+// state of a seed after the Update on its start row r0, going down: t, rows (r0 | top << 8), nhits, pad, then
+// y z s t q, c00..c44, chi2 (21 floats) and 3 floats of padding: seven 16-byte words
+constexpr int DOWNREC_WORDS = 28;
+
+struct RowSmem {
+  float sx[MAX_ROWS];
+  int16_t sup[MAX_ROWS];          // up_row (R2)
+  int16_t snu[MAX_ROWS];          // next live row above (n_rows if none)
+  int16_t snd[MAX_ROWS];          // next live row below (-1 if none)
+};
+
+__device__ __forceinline__ void rowSmemFill(RowSmem& rs, const RowTables& T, int R) {
+  for (int i = threadIdx.x; i < R; i += blockDim.x) {
+    rs.sx[i] = T.row_x[i]; rs.sup[i] = T.up_row[i];
     int u = i + 1, d = i - 1;
     while (u < R && T.dead[u]) ++u;
     while (d >= 0 && T.dead[d]) --d;
-    snu[i] = (int16_t)u; snd[i] = (int16_t)d;
+    rs.snu[i] = (int16_t)u; rs.snd[i] = (int16_t)d;
   }
   __syncthreads();
-  const int64_t nW = cnt[CNT_N_LONG];            // seeds on the work list (seedPrepare)
+}
+
+#define TC_SNAP_STORE(snap, tid, S)                                                                                   \
+  do {                                                                                                                \
+    snap[0][tid] = S.x; snap[1][tid] = S.y; snap[2][tid] = S.z; snap[3][tid] = S.s; snap[4][tid] = S.t;               \
+    snap[5][tid] = S.q; snap[6][tid] = S.chi2; snap[7][tid] = S.c00; snap[8][tid] = S.c10; snap[9][tid] = S.c11;      \
+    snap[10][tid] = S.c20; snap[11][tid] = S.c21; snap[12][tid] = S.c22; snap[13][tid] = S.c30;                       \
+    snap[14][tid] = S.c31; snap[15][tid] = S.c32; snap[16][tid] = S.c33; snap[17][tid] = S.c40;                       \
+    snap[18][tid] = S.c41; snap[19][tid] = S.c42; snap[20][tid] = S.c43; snap[21][tid] = S.c44;                       \
+  } while (0)
+
+// O4 step 6: the tracklet is the last snapshot of the down pass (state at the innermost attached row)
+__device__ __forceinline__ void writeTracklet(const TrackletStore& out, const DevParams& P, uint32_t t, int nhits,
+                                              int snap_row, int rtop, float (*snap)[TC_THREADS], int tid) {
+  if (snap_row < 0) {
+    out.status[t] = 1; out.nhits[t] = 0; out.first_row[t] = -1; out.last_row[t] = -1;
+    return;
+  }
   const int64_t capT = out.capT;
+  out.status[t] = nhits >= P.min_tracklet_hits ? 2 : 1;
+  out.nhits[t] = nhits; out.first_row[t] = snap_row; out.last_row[t] = rtop;
+  out.x[t] = snap[0][tid]; out.chi2[t] = snap[6][tid];
+#pragma unroll
+  for (int i = 0; i < 5; ++i) out.par[i * capT + t] = snap[1 + i][tid];
+#pragma unroll
+  for (int i = 0; i < 15; ++i) out.cov[i * capT + t] = snap[7 + i][tid];
+}
+
+// ---- pass 1: chain fit (O4 step 2) and up extrapolation (step 3) ---------------------------------------------------
+__global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) constructUp(
+    DevParams P, RowTables T, const GridDesc* __restrict__ desc, const uint32_t* __restrict__ cell_start,
+    const float2* __restrict__ syz, const uint32_t* __restrict__ s2o, const int32_t* __restrict__ cup,
+    const SeedRec* __restrict__ work_list, TurnRec* __restrict__ turn_list, TrackletStore out, int64_t* __restrict__ cnt) {
+  __shared__ RowSmem rs;
+  // per-lane bookkeeping that is read once per step or less lives in shared memory (volatile: re-read where used):
+  // in registers it pushed the kernel over its budget and the spilled bucket base sat on the path to every grid load
+  __shared__ volatile uint32_t s_t[TC_THREADS];       // tracklet id
+  __shared__ volatile uint32_t s_j[TC_THREADS];       // index of the seed in the work list
+  __shared__ volatile int s_bsec[TC_THREADS];         // first bucket of the seed's sector
+  __shared__ volatile int16_t s_rc[TC_THREADS];       // row of the last Propagate
+  if (cnt[CNT_ERROR] != 0) return;
+  const int R = P.n_rows;
+  const int tid = threadIdx.x;
+  rowSmemFill(rs, T, R);
+  const int64_t nW = cnt[CNT_N_LONG];            // seeds on the work list (seedPrepare)
   unsigned long long* work = (unsigned long long*)(cnt + CNT_WORK);
 
   KFState S;
-  int phase = -1;                 // -1 wants a seed, -2 no seeds left, 0 chain fit, 1 up extrapolation, 2 down pass
+  int phase = -1;                 // -1 wants a seed, -2 no seeds left, 0 chain fit, 1 up extrapolation
   int32_t* rowhit = nullptr;      // this tracklet's [n_rows] slice
-  int r0 = 0, rn = 0, lastw = 0, nhits = 0, miss = 0, snap_row = -1;
-  int32_t c_cur = -1;             // hit of the coming step if known (link / row hit), else -1 = search
-  // down pass: row hit of the step after, loaded one step ahead.  Kept as (raw value, valid) and merged with -1 only
-  // when it becomes c_cur: a select right behind the load would wait for the load and undo the pipelining.
-  int32_t nx_raw = -1;
-  bool nx_ok = false;
+  int r0 = 0, rn = 0, lastw = 0, nhits = 0, miss = 0;
+  int32_t c_cur = -1;             // hit of the coming step if known (link), else -1 = search
   int32_t last_c = -1;            // last recorded hit (the hit on row lastw)
 
   for (;;) {
@@ -262,23 +309,23 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
         const uint4* rp = reinterpret_cast<const uint4*>(work_list + j);
         const uint4 a = __ldg(rp), b = __ldg(rp + 1);
         const uint32_t t = a.x;
-        s_t[tid] = t;
+        s_t[tid] = t; s_j[tid] = (uint32_t)j;
         const uint32_t h0 = a.y;
         c_cur = (int32_t)a.z;
         r0 = (int)(a.w & 0xffu);
         s_bsec[tid] = (int)(a.w >> 8) - r0;
         rowhit = out.rowhit + (int64_t)t * R;
-        rn = sup[r0];
+        rn = rs.sup[r0];
         const float y0 = __uint_as_float(b.x), z0 = __uint_as_float(b.y);
-        S.x = sx[r0]; S.y = y0; S.z = z0;
-        const float dx = sx[rn] - sx[r0], dy = __uint_as_float(b.z) - y0, dz = __uint_as_float(b.w) - z0;
+        S.x = rs.sx[r0]; S.y = y0; S.z = z0;
+        const float dx = rs.sx[rn] - rs.sx[r0], dy = __uint_as_float(b.z) - y0, dz = __uint_as_float(b.w) - z0;
         const float L = sqrtf(dx * dx + dy * dy);
         S.s = dy / L; S.t = dz / L; S.q = 0.0f;
         kfSetDiag(S, P.err2_y, P.err2_z, P);
         S.chi2 = 0.0f;
         rowhit[r0] = (int32_t)h0;
         last_c = (int32_t)h0;
-        nhits = 1; s_rc[tid] = (int16_t)r0; lastw = r0; miss = 0; snap_row = -1;
+        nhits = 1; s_rc[tid] = (int16_t)r0; lastw = r0; miss = 0;
         phase = 0;
       }
     }
@@ -287,22 +334,21 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
     // ---- one step: early loads -> Propagate (search loads issued inside) -> candidate -> Update ----
     const bool act = phase >= 0;
     float ym = 0.0f, zm = 0.0f;
-    float2 mk = make_float2(0.0f, 0.0f);         // coordinates of the known hit: consumed only at the Update
+    float2 mk = make_float2(0.0f, 0.0f);         // coordinates of the link: consumed only at the Update
     int32_t hnext = -1;
     // the grid descriptor of the row is loaded by every lane (a conditional struct assignment would make the compiler
     // wait for the load right here, to merge it with the "not loaded" value)
     const GridDesc G = desc[act ? s_bsec[tid] + rn : 0];
     if (act && c_cur >= 0) {
       mk = __ldg(syz + c_cur);
-      if (phase == 0) hnext = __ldg(cup + c_cur);
+      hnext = __ldg(cup + c_cur);
     }
     SearchPre sp;
     const bool want_search = act && c_cur < 0;
-    const bool okp = act && kfPropagate(S, sx[act ? rn : 0], P, [&](float y1, float z1, float c00, float c11) {
+    const bool okp = act && kfPropagate(S, rs.sx[act ? rn : 0], P, [&](float y1, float z1, float c00, float c11) {
       if (want_search) searchBegin(sp, y1, z1, c00, c11, G, cell_start, P);
     });
     int32_t c = c_cur;
-    const bool known = okp && c >= 0 && phase == 2;
     if (okp && c < 0) c = searchFinish(sp, syz, s2o, ym, zm);
     if (c_cur >= 0) { ym = mk.x; zm = mk.y; }
     bool oku = false;
@@ -313,87 +359,198 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) trackletConstructor
     bool end_phase = !okp || (c >= 0 && !oku);       // Propagate or Update refused: the pass ends here
     bool turn = false;
     const int rb = rn;                               // the row of this step
-    if (okp && !known) rowhit[rb] = oku ? c : -1;    // rows beyond the final first/last row are never read
+    if (okp) { rowhit[rb] = oku ? c : -1; s_rc[tid] = (int16_t)rb; }    // rows beyond the final first/last row are never read
     if (phase == 0) {
-      if (okp) s_rc[tid] = (int16_t)rb;
       if (oku) {
         lastw = rb; last_c = c; ++nhits;
         c_cur = hnext;
-        rn = sup[rb];
+        rn = rs.sup[rb];
         if (hnext == -1) end_phase = true;
       }
       if (end_phase) {
         if (nhits < P.min_chain_hits) {
           const uint32_t t = s_t[tid];
           out.status[t] = 0; out.nhits[t] = nhits; out.first_row[t] = -1; out.last_row[t] = -1;
+          turn_list[s_j[tid]].t = REC_NONE;
           phase = -1;
         } else {
           phase = 1; miss = 0; c_cur = -1;
-          rn = snu[s_rc[tid]];
+          rn = rs.snu[s_rc[tid]];
           if (rn >= R) turn = true;
         }
       }
-    } else if (phase == 1) {
+    } else {
       if (oku) {
         lastw = rb; last_c = c; ++nhits; miss = 0;
       } else if (!end_phase) {
         if (++miss > P.max_row_gap) end_phase = true;
       }
       if (!end_phase) {
-        rn = snu[rb];
+        rn = rs.snu[rb];
         if (rn >= R) end_phase = true;
       }
       if (end_phase) turn = true;
-    } else {
-      if (!end_phase) {
-        if (oku) {
-          ++nhits; snap_row = rb;
-          snap[0][tid] = S.x; snap[1][tid] = S.y; snap[2][tid] = S.z; snap[3][tid] = S.s; snap[4][tid] = S.t;
-          snap[5][tid] = S.q; snap[6][tid] = S.chi2; snap[7][tid] = S.c00; snap[8][tid] = S.c10; snap[9][tid] = S.c11;
-          snap[10][tid] = S.c20; snap[11][tid] = S.c21; snap[12][tid] = S.c22; snap[13][tid] = S.c30;
-          snap[14][tid] = S.c31; snap[15][tid] = S.c32; snap[16][tid] = S.c33; snap[17][tid] = S.c40;
-          snap[18][tid] = S.c41; snap[19][tid] = S.c42; snap[20][tid] = S.c43; snap[21][tid] = S.c44;
-          if (rb < r0) miss = 0;
-        } else if (rb < r0) {
-          if (++miss > P.max_row_gap) end_phase = true;
-        }
-      }
-      if (!end_phase) {
-        rn = snd[rb];
-        if (rn < 0) end_phase = true;
-      }
-      if (!end_phase) {           // pipeline: this step's hit was loaded a step ago; request the one after
-        c_cur = nx_ok ? nx_raw : -1;
-        const int r2 = snd[rn];
-        nx_ok = r2 >= r0;
-        if (nx_ok) nx_raw = rowhit[r2];
-      } else {                    // O4 step 6: output = last snapshot
-        const uint32_t t = s_t[tid];
-        if (snap_row < 0) {
-          out.status[t] = 1; out.nhits[t] = 0; out.first_row[t] = -1; out.last_row[t] = -1;
-        } else {
-          out.status[t] = nhits >= P.min_tracklet_hits ? 2 : 1;
-          out.nhits[t] = nhits; out.first_row[t] = snap_row; out.last_row[t] = s_rtop[tid];
-          out.x[t] = snap[0][tid]; out.chi2[t] = snap[6][tid];
-#pragma unroll
-          for (int i = 0; i < 5; ++i) out.par[i * capT + t] = snap[1 + i][tid];
-#pragma unroll
-          for (int i = 0; i < 15; ++i) out.cov[i * capT + t] = snap[7 + i][tid];
-        }
-        phase = -1;
-      }
     }
-    if (turn) {                   // O4 step 4: diffuse covariance, parameters kept (R17); down pass starts at rtop
-      kfSetDiag(S, P.turn_var_scale * P.err2_y, P.turn_var_scale * P.err2_z, P);
-      S.chi2 = 0.0f;
-      s_rtop[tid] = (int16_t)lastw; rn = lastw;
-      phase = 2; miss = 0; nhits = 0; snap_row = -1;
-      c_cur = last_c;             // the hit on row rtop
-      const int r2 = snd[rn];
-      nx_ok = r2 >= r0;
-      if (nx_ok) nx_raw = rowhit[r2];
+    if (turn) {                   // O4 step 4 happens in the next kernel: hand the parameters over
+      uint4* q = reinterpret_cast<uint4*>(turn_list + s_j[tid]);
+      q[0] = make_uint4(s_t[tid], (uint32_t)last_c, __float_as_uint(S.y), __float_as_uint(S.z));
+      q[1] = make_uint4(__float_as_uint(S.s), __float_as_uint(S.t), __float_as_uint(S.q),
+                        (uint32_t)r0 | ((uint32_t)lastw << 8) | ((uint32_t)(uint16_t)s_rc[tid] << 16));
+      phase = -1;
     } else if (phase >= 0) {      // dead rows stepped over (R23) hold no hit
       const int lo = min(rb, rn), hi = max(rb, rn);
+      if (hi - lo > 1)
+        for (int g = lo + 1; g < hi; ++g) rowhit[g] = -1;
+    }
+  }
+}
+
+// ---- passes 2 and 3: the down pass (O4 steps 4-6), over the span (EXT = 0) and below the start row (EXT = 1) -----------
+template <int EXT>
+__global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) constructDown(
+    DevParams P, RowTables T, const GridDesc* __restrict__ desc, const uint32_t* __restrict__ cell_start,
+    const float2* __restrict__ syz, const uint32_t* __restrict__ s2o, const TurnRec* __restrict__ turn_list,
+    uint4* __restrict__ down_list, TrackletStore out, int64_t* __restrict__ cnt) {
+  __shared__ RowSmem rs;
+  __shared__ float snap[22][TC_THREADS];     // state after the last Update (O4 step 5)
+  __shared__ volatile uint32_t s_t[TC_THREADS];
+  __shared__ volatile uint32_t s_j[TC_THREADS];
+  __shared__ volatile int s_bsec[TC_THREADS];
+  __shared__ volatile int16_t s_rtop[TC_THREADS];
+  if (cnt[CNT_ERROR] != 0) return;
+  const int R = P.n_rows;
+  const int tid = threadIdx.x;
+  rowSmemFill(rs, T, R);
+  const int64_t nW = cnt[CNT_N_LONG];
+  unsigned long long* work = (unsigned long long*)(cnt + (EXT ? CNT_WORK3 : CNT_WORK2));
+
+  KFState S;
+  int phase = -1;                 // -1 wants a seed, -2 no seeds left, 2 down pass
+  int32_t* rowhit = nullptr;
+  int r0 = 0, rn = 0, nhits = 0, miss = 0, snap_row = -1;
+  int32_t c_cur = -1;             // hit of the coming step if known (row hit), else -1 = search
+  // row hit of the step after, loaded one step ahead.  Kept as (raw value, valid) and merged with -1 only when it
+  // becomes c_cur: a select right behind the load would wait for the load and undo the pipelining.
+  int32_t nx_raw = -1;
+  bool nx_ok = false;
+
+  for (;;) {
+    while (phase == -1) {         // ---- fetch the next seed that is still alive ----
+      const int64_t j = (int64_t)atomicAdd(work, 1ull);
+      if (j >= nW) { phase = -2; break; }
+      if (!EXT) {
+        const uint4* rp = reinterpret_cast<const uint4*>(turn_list + j);
+        const uint4 a = __ldg(rp), b = __ldg(rp + 1);
+        if (a.x == REC_NONE) { down_list[j * (DOWNREC_WORDS / 4)].x = REC_NONE; continue; }
+        const uint32_t t = a.x;
+        s_t[tid] = t; s_j[tid] = (uint32_t)j;
+        r0 = (int)(b.w & 0xffu);
+        const int rtop = (int)((b.w >> 8) & 0xffu), rx = (int)(b.w >> 16);
+        s_rtop[tid] = (int16_t)rtop;
+        s_bsec[tid] = out.sector[t] * R;
+        rowhit = out.rowhit + (int64_t)t * R;
+        // O4 step 4: diffuse covariance, parameters kept (R17); the down pass starts at the top row
+        S.x = rs.sx[rx]; S.y = __uint_as_float(a.z); S.z = __uint_as_float(a.w);
+        S.s = __uint_as_float(b.x); S.t = __uint_as_float(b.y); S.q = __uint_as_float(b.z);
+        kfSetDiag(S, P.turn_var_scale * P.err2_y, P.turn_var_scale * P.err2_z, P);
+        S.chi2 = 0.0f;
+        rn = rtop; miss = 0; nhits = 0; snap_row = -1;
+        c_cur = (int32_t)a.y;       // the hit on the top row
+        const int r2 = rs.snd[rn];
+        nx_ok = r2 >= r0;
+        if (nx_ok) nx_raw = rowhit[r2];
+        phase = 2;
+      } else {
+        const uint4* rp = down_list + j * (DOWNREC_WORDS / 4);
+        const uint4 a = rp[0];
+        if (a.x == REC_NONE) continue;
+        const uint4 b = rp[1], c4 = rp[2], d = rp[3], e = rp[4], f = rp[5], g = rp[6];
+        const uint32_t t = a.x;
+        s_t[tid] = t; s_j[tid] = (uint32_t)j;
+        r0 = (int)(a.y & 0xffu);
+        s_rtop[tid] = (int16_t)((a.y >> 8) & 0xffu);
+        nhits = (int)a.z;
+        s_bsec[tid] = out.sector[t] * R;
+        rowhit = out.rowhit + (int64_t)t * R;
+        S.x = rs.sx[r0];
+        S.y = __uint_as_float(b.x); S.z = __uint_as_float(b.y); S.s = __uint_as_float(b.z); S.t = __uint_as_float(b.w);
+        S.q = __uint_as_float(c4.x); S.c00 = __uint_as_float(c4.y); S.c10 = __uint_as_float(c4.z); S.c11 = __uint_as_float(c4.w);
+        S.c20 = __uint_as_float(d.x); S.c21 = __uint_as_float(d.y); S.c22 = __uint_as_float(d.z); S.c30 = __uint_as_float(d.w);
+        S.c31 = __uint_as_float(e.x); S.c32 = __uint_as_float(e.y); S.c33 = __uint_as_float(e.z); S.c40 = __uint_as_float(e.w);
+        S.c41 = __uint_as_float(f.x); S.c42 = __uint_as_float(f.y); S.c43 = __uint_as_float(f.z); S.c44 = __uint_as_float(f.w);
+        S.chi2 = __uint_as_float(g.x);
+        TC_SNAP_STORE(snap, tid, S);        // the state after the Update on r0 is the snapshot so far
+        snap_row = r0; miss = 0; c_cur = -1;
+        rn = rs.snd[r0];                    // >= 0: the span pass finishes seeds with nothing below r0 itself
+        for (int g = rn + 1; g < r0; ++g) rowhit[g] = -1;     // dead rows stepped over (R23) hold no hit
+        phase = 2;
+      }
+    }
+    if (__all_sync(0xffffffffu, phase == -2)) break;
+
+    // ---- one step ----
+    const bool act = phase >= 0;
+    float ym = 0.0f, zm = 0.0f;
+    float2 mk = make_float2(0.0f, 0.0f);
+    const GridDesc G = desc[act ? s_bsec[tid] + rn : 0];
+    if (!EXT && act && c_cur >= 0) mk = __ldg(syz + c_cur);
+    SearchPre sp;
+    const bool want_search = act && (EXT || c_cur < 0);
+    const bool okp = act && kfPropagate(S, rs.sx[act ? rn : 0], P, [&](float y1, float z1, float c00, float c11) {
+      if (want_search) searchBegin(sp, y1, z1, c00, c11, G, cell_start, P);
+    });
+    int32_t c = EXT ? -1 : c_cur;
+    const bool known = !EXT && okp && c >= 0;
+    if (okp && c < 0) c = searchFinish(sp, syz, s2o, ym, zm);
+    if (!EXT && c_cur >= 0) { ym = mk.x; zm = mk.y; }
+    bool oku = false;
+    if (okp && c >= 0) oku = kfUpdate(S, ym, zm, P);
+    if (!act) continue;
+
+    // ---- bookkeeping ----
+    bool end_phase = !okp || (c >= 0 && !oku);       // Propagate or Update refused: the pass ends here
+    const int rb = rn;
+    if (okp && !known) rowhit[rb] = oku ? c : -1;
+    if (!end_phase) {
+      if (oku) {
+        ++nhits; snap_row = rb;
+        TC_SNAP_STORE(snap, tid, S);
+        if (EXT) miss = 0;
+      } else if (EXT) {
+        if (++miss > P.max_row_gap) end_phase = true;
+      }
+    }
+    bool handoff = false;
+    if (!end_phase) {
+      if (!EXT && rb == r0) {        // the span is done: S is the state after the Update on r0 (h0 is always known)
+        if (rs.snd[rb] < 0) end_phase = true; else handoff = true;
+      } else {
+        rn = rs.snd[rb];
+        if (rn < 0) end_phase = true;
+      }
+    }
+    if (handoff) {
+      uint4* q = down_list + (int64_t)s_j[tid] * (DOWNREC_WORDS / 4);
+      q[0] = make_uint4(s_t[tid], (uint32_t)r0 | ((uint32_t)(uint16_t)s_rtop[tid] << 8), (uint32_t)nhits, 0u);
+      q[1] = make_uint4(__float_as_uint(S.y), __float_as_uint(S.z), __float_as_uint(S.s), __float_as_uint(S.t));
+      q[2] = make_uint4(__float_as_uint(S.q), __float_as_uint(S.c00), __float_as_uint(S.c10), __float_as_uint(S.c11));
+      q[3] = make_uint4(__float_as_uint(S.c20), __float_as_uint(S.c21), __float_as_uint(S.c22), __float_as_uint(S.c30));
+      q[4] = make_uint4(__float_as_uint(S.c31), __float_as_uint(S.c32), __float_as_uint(S.c33), __float_as_uint(S.c40));
+      q[5] = make_uint4(__float_as_uint(S.c41), __float_as_uint(S.c42), __float_as_uint(S.c43), __float_as_uint(S.c44));
+      q[6] = make_uint4(__float_as_uint(S.chi2), 0u, 0u, 0u);
+      phase = -1;
+    } else if (end_phase) {         // O4 step 6: output = last snapshot
+      writeTracklet(out, P, s_t[tid], nhits, snap_row, s_rtop[tid], snap, tid);
+      if (!EXT) down_list[(int64_t)s_j[tid] * (DOWNREC_WORDS / 4)].x = REC_NONE;
+      phase = -1;
+    } else {
+      if (!EXT) {                   // pipeline: this step's hit was loaded a step ago; request the one after
+        c_cur = nx_ok ? nx_raw : -1;
+        const int r2 = rs.snd[rn];
+        nx_ok = r2 >= r0;
+        if (nx_ok) nx_raw = rowhit[r2];
+      }
+      const int lo = rn, hi = rb;   // dead rows stepped over (R23) hold no hit
       if (hi - lo > 1)
         for (int g = lo + 1; g < hi; ++g) rowhit[g] = -1;
     }

@@ -85,14 +85,15 @@ def test_ambiguity_goes_to_the_higher_momentum_track_and_low_momentum_tracks_do_
     assert np.all(res.cf_flags[m] == ADJ | PROT)                     # still owned by the 6 GeV/c track
 
 
-def _flags_numpy(ev, res, p):
-    """O8 restated: walk every refitted track with the pinned single Propagate step (binary32), tubes by numpy."""
+def _flags_numpy(ev, res, p, rank=None):
+    """O8 restated: walk every refitted track with the pinned single Propagate step (binary32), tubes by numpy.
+    rank: leg rank per track (1 = secondary leg: it does not protect), None = every track is a primary leg."""
     n = ev.n_clusters
     off = ev.row_offset.astype(np.int64)
     rowof = np.repeat(np.arange(ev.n_rows * ev.n_sectors), np.diff(off)) % ev.n_rows
     owner = np.full(n, -1, np.int64)
     oq = np.zeros(n, np.float32)
-    bad = np.zeros(n, bool)
+    good_any = np.zeros(n, bool)                 # R36b: some good track has the cluster in its tube
     res_y, res_z = np.zeros(n), np.zeros(n)
     sin70 = np.float32(0.9396926207859084)
     tube2 = np.float32(p.tube_radius) * np.float32(p.tube_radius)
@@ -123,14 +124,15 @@ def _flags_numpy(ev, res, p):
             for c in own:
                 res_y[c] = float(y32[c] - np.float32(st[1]))
                 res_z[c] = float(z32[c] - np.float32(st[2]))
-            b = low or not (np.float32(abs(st[3])) < sin70)
+            b = low or not (np.float32(abs(st[3])) < sin70) or (rank is not None and rank[k] == 1)
             for c in np.nonzero(inside)[0] + lo:
+                good_any[c] |= not b
                 if owner[c] < 0 or aq < oq[c]:
-                    owner[c], oq[c], bad[c] = k, aq, b
+                    owner[c], oq[c] = k, aq
     f = np.zeros(n, np.uint8)
     f[res.trk_cl_index] |= ATT
     has = owner >= 0
-    prot = has & ~bad
+    prot = has & good_any
     f[has] |= ADJ
     f[prot] |= PROT
     f[has & ~prot] |= RMA
@@ -149,6 +151,55 @@ def test_flags_equal_the_numpy_restatement(idx, scale, dead):
     assert np.array_equal(ry, res.cf_res_y) and np.array_equal(rz, res.cf_res_z)
     if idx == 2:
         assert ((res.cf_flags & RMA) != 0).sum() > 10            # steep looper segments are exercised
+        # with the leg labels of O12: secondary legs do not protect and are removable by strategy A (L86)
+        res = orc.run(ev, p, flags=True, merged=True)
+        assert (res.mt_rank == 1).sum() > 5
+        f2, owner2, _, _ = _flags_numpy(ev, res, p, rank=res.mt_rank)
+        assert np.array_equal(owner2, res.cf_owner) and np.array_equal(owner2, owner)      # ownership does not look at legs
+        assert np.array_equal(f2, res.cf_flags)
+        assert ((f2 & RMA) != 0).sum() > ((f & RMA) != 0).sum() + 100
+
+
+def test_every_good_track_protects_the_clusters_in_its_tube_even_when_a_steep_track_owns_them():
+    """R36b ("All clusters adjacent to the primary leg of a track with pT > 50 MeV/c and |phi| < 70 degrees
+    are protected"; L88: strategy A "only rejects clusters that have been positively identified as not useful").  Two exact
+    circles in one sector: G with pT = 70 MeV/c at moderate angles, and S with pT = 120 MeV/c whose sin(phi) passes
+    sin(70 degrees) = 0.94 between rows 43 and 44 (0.5 + 0.012491 / cm * 1.0596 cm * (row - 10): 0.937, 0.950).  G is laid 0.5 cm
+    beside S on row 45.  By hand: S has the higher momentum, so it owns the clusters of both tracks that lie in its tube on row 45; it is steep there, so it protects nothing -- but G is a good
+    track and those clusters are in G's own tube: they stay protected (flags attached | adjacent | protected, owner = S).
+    Under the round-1 reading (protection only through the owner) they were removed by strategies A and B."""
+    b_field = 0.00299792458 * BZ
+
+    def circle(pt, s10, y10, z10, t, rows, y_at=None):
+        k = (1.0 / pt) * b_field
+        s_of = lambda r: s10 + k * (ROW_X[r] - ROW_X[10])
+        c10 = math.sqrt(1 - s10 * s10)
+        ys = {r: y10 + (c10 - math.sqrt(1 - s_of(r) ** 2)) / k for r in rows}
+        zs = {r: z10 + t * (math.asin(s_of(r)) - math.asin(s10)) / k for r in rows}
+        return s_of, ys, zs
+
+    rows_s = list(range(10, 47))
+    sS, yS, zS = circle(0.12, 0.50, 0.0, 30.0, 0.3, rows_s)
+    assert sS(43) < 0.9397 < sS(44) and sS(46) < 0.98                       # steep from row 44 on, inside max_sinphi
+    rows_g = list(range(10, 60))
+    sG, yG0, zG0 = circle(0.07, -0.45, 0.0, 0.0, 0.25, rows_g)
+    dy, dz = yS[45] + 0.4 - yG0[45], zS[45] + 0.3 - zG0[45]                 # shift G so that it passes 0.5 cm from S on row 45
+    pts = [(r, yS[r], zS[r]) for r in rows_s] + [(r, yG0[r] + dy, zG0[r] + dz) for r in rows_g]
+    ev, where = _event(pts)
+    res = orc.run(ev, flags=True)
+    assert res.n_tracks == 2
+    pt = 1.0 / np.abs(res.rf_par_in[:, 4])
+    kS, kG = int(np.argmax(pt)), int(np.argmin(pt))
+    assert pt[kS] == pytest.approx(0.12, rel=0.05) and pt[kG] == pytest.approx(0.07, rel=0.05)
+    g45 = where[len(rows_s) + (45 - 10)]
+    s45 = where[45 - 10]
+    assert res.cf_owner[g45] == kS and res.cf_owner[s45] == kS             # the higher-momentum track owns both
+    assert res.cf_flags[g45] == ATT | ADJ | PROT                           # ... but G protects what is in its tube
+    assert res.cf_flags[s45] == ATT | ADJ | PROT                           # S's own cluster lies 0.5 cm from G as well
+    far = where[46 - 10]                                                   # S on row 46: steep, and G is > 1.5 cm away by then
+    g_at_46 = np.hypot(yS[46] - (yG0[46] + dy), zS[46] - (zG0[46] + dz))
+    assert g_at_46 > 1.6
+    assert res.cf_flags[far] == ATT | ADJ | RMA | RMB and res.cf_owner[far] == kS
 
 
 def test_flag_invariants_and_what_the_strategies_remove():
