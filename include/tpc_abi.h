@@ -165,6 +165,15 @@ typedef struct {
   uint32_t* cl_pos_code;        /* [n_clusters] code of the absolute (y, z) of every cluster; NULL = not computed */
   uint32_t* cl_res_code;        /* [n_clusters] code of the track-model residuals (0 where there is none); needs cl_flags and
                                    cl_owner (and with them the refit outputs); NULL = not computed */
+  /* optional O12 merged tracks and leg labels (DESIGN.md section 3 "O12", R46..R48); all four or
+   * none; need the merger and the leg-pair outputs.  When they are given together with cl_flags, the cluster flags treat
+   * secondary legs as not protecting and their clusters as removable by strategy A (L86). */
+  int32_t* trk_mt_id;           /* [cap_tracks] the merged track of every track: the smallest head index of its one or two legs */
+  int32_t* trk_mt_rank;         /* [cap_tracks] 0 = on the primary (first) leg of its merged track, 1 = on the secondary leg */
+  uint32_t* mt_cl_offset;       /* [cap_tracks + 1] cluster list of the merged track named by track k: [off[k], off[k+1]);
+                                   empty for tracks that name none */
+  uint32_t* mt_cl_index;        /* [cap_track_clusters] clusters in the order along the particle's path: the primary leg from
+                                   its inner end outwards, then the secondary leg from the turn inwards */
 } tpcTracks;
 
 /* Filled by tpcGetRunStatus after the stream has drained. */
@@ -186,6 +195,7 @@ typedef struct {
   float pack_ms;                /* the O9 charge code and the O11 position code alone (profiling on, cl_qcode / cl_pos_code requested) */
   float flags_ms;               /* the O8 cluster flags alone (profiling on, flags requested) */
   float legs_ms;                /* the O10 leg pairs alone (profiling on, legs requested) */
+  float merged_ms;              /* the O12 merged tracks alone (profiling on, merged tracks requested) */
   float submit_ms[2];           /* tpcCollectHost only: device time of the slot from its first copy in to the end of its
                                    kernels [0] and to the end of its copies out [1] (includes waiting for the other slot) */
 } tpcRunStatus;
@@ -231,6 +241,12 @@ int tpcCollectHost(tpcHandle* h, int slot, tpcRunStatus* status);
 
 const char* tpcErrorString(int code);
 const char* tpcLastCudaError(const tpcHandle* h);
+
+/* Diagnostic: the Kalman update divides six numerators by one denominator with a shared reciprocal (csrc/tpc_kalman.cuh,
+ * `divShared`), which must be bit-identical to the IEEE division the formula sheet writes (R0).  This call runs
+ * both forms on the device for n_threads x 48 operand pairs drawn over the whole domain of the shared form (seeded,
+ * edge values included) and reports how many were tested and how many bit patterns differ (must be 0).  Synchronous. */
+int tpcSelfTestDivision(tpcHandle* h, int64_t n_threads, uint64_t seed, int64_t* n_tested, int64_t* n_mismatches);
 
 #ifdef __cplusplus
 }

@@ -22,6 +22,7 @@
 #include "tpc_merge.cuh"
 #include "tpc_legs.cuh"
 #include "tpc_flags.cuh"
+#include "tpc_merged.cuh"
 
 using namespace tpc;
 
@@ -62,6 +63,8 @@ struct Workspace {
   float* mg_chi_b;
   unsigned long long* mg_key_a;
   unsigned long long* fl_key;      // [N] bids of the cluster flags
+  uint32_t* fl_prot;               // [ceil(N / 32)] protection bits of the cluster flags
+  uint32_t* mt_tiles;              // tile sums of the merged-track offsets scan
   uint32_t *lg_start, *lg_fill, *lg_list;   // leg pairs: leg ends bucketed by (sector, sign, last row, dip bin)
   float4* lg_rec;                           // [capT] dip, curvature and their variances of the leg ends, in list order
   uint32_t *lg_maxv, *lg_tiles;             // largest dip variance per (sector, sign, row); tile sums of the bucket scan
@@ -83,7 +86,7 @@ struct tpcHandle {
   int64_t* d_cnt = nullptr;        // CNT_COUNT counters + 1 slot for the packed selector total
   int64_t* h_cnt = nullptr;        // pinned copy
   cudaEvent_t ev_done = nullptr;
-  cudaEvent_t ev_stage[17] = {};   // ... 13/14 around the charge code, 15/16 leg pairs
+  cudaEvent_t ev_stage[19] = {};   // ... 13/14 around the charge code, 15/16 leg pairs, 17/18 merged tracks
   //   // 0..6 stage boundaries, 7/8 around the optional refit, 9/10 merger, 11/12 flags
   int profiling = 0;
   int launches = 0;
@@ -193,6 +196,8 @@ Workspace layout(const tpcHandle* h, int64_t N, int64_t capT, char* base) {
   w.mg_chi_b = (float*)take(4 * (size_t)Tn);
   w.mg_key_a = (unsigned long long*)take(8 * (size_t)Tn);
   w.fl_key = (unsigned long long*)take(8 * (size_t)Nn);
+  w.fl_prot = (uint32_t*)take(4 * (size_t)ceilDiv(Nn, 32));
+  w.mt_tiles = (uint32_t*)take(4 * (size_t)(ceilDiv(Tn + 1, SCAN_TILE) + 2));
   const size_t lgb = (int64_t)nb * 2 * LEG_BINS < (1ll << 31) ? (size_t)nb * 2 * LEG_BINS + 1 : 1;   // else: leg pairs refused
   w.lg_start = (uint32_t*)take(4 * lgb);
   w.lg_fill = (uint32_t*)take(4 * lgb);
@@ -281,7 +286,7 @@ int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cud
             cudaMalloc(&h->d_cnt, 8 * (CNT_COUNT + 1)) == cudaSuccess &&
             cudaMallocHost(&h->h_cnt, 8 * (CNT_COUNT + 1)) == cudaSuccess &&
             cudaEventCreate(&h->ev_done) == cudaSuccess;
-  for (int i = 0; ok && i < 17; ++i) ok = cudaEventCreate(&h->ev_stage[i]) == cudaSuccess;
+  for (int i = 0; ok && i < 19; ++i) ok = cudaEventCreate(&h->ev_stage[i]) == cudaSuccess;
   ok = ok && cudaMemcpy(h->d_row_x, g->row_x, 4 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
        cudaMemcpy(h->d_up, up.data(), 2 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
        cudaMemcpy(h->d_dn, dn.data(), 2 * R, cudaMemcpyHostToDevice) == cudaSuccess &&
@@ -309,7 +314,7 @@ int tpcDestroy(tpcHandle* h) {
   cudaFree(h->d_row_x); cudaFree(h->d_up); cudaFree(h->d_dn); cudaFree(h->d_dead); cudaFree(h->d_cnt);
   if (h->h_cnt) cudaFreeHost(h->h_cnt);
   if (h->ev_done) cudaEventDestroy(h->ev_done);
-  for (int i = 0; i < 17; ++i) if (h->ev_stage[i]) cudaEventDestroy(h->ev_stage[i]);
+  for (int i = 0; i < 19; ++i) if (h->ev_stage[i]) cudaEventDestroy(h->ev_stage[i]);
   // the active state is freed below; the parked slots here, whatever part of them was initialised
   for (int k = 0; k < 3; ++k) {
     if (k == h->cur_slot) continue;
@@ -370,6 +375,9 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   if ((n_fl != 0 && n_fl != 2) || (n_fl == 2 && n_rf != 8)) return TPC_ERR_INVALID_ARG;   // so do the cluster flags
   if ((out->cl_res_y != nullptr) != (out->cl_res_z != nullptr) || (out->cl_res_y && n_fl != 2)) return TPC_ERR_INVALID_ARG;
   if (out->cl_res_code && n_fl != 2) return TPC_ERR_INVALID_ARG;                         // the residual code rides on the flag pass
+  const int n_mt = (out->trk_mt_id != nullptr) + (out->trk_mt_rank != nullptr) + (out->mt_cl_offset != nullptr) +
+                   (out->mt_cl_index != nullptr);
+  if ((n_mt != 0 && n_mt != 4) || (n_mt == 4 && (n_mg != 4 || n_lg != 2))) return TPC_ERR_INVALID_ARG;   // chains and leg pairs
   if (!workspace || ((uintptr_t)workspace % ALIGN) != 0) return TPC_ERR_INVALID_ARG;
   const Workspace w = layout(h, N, capT, (char*)workspace);
   if (workspace_bytes < w.bytes) return TPC_ERR_WORKSPACE_TOO_SMALL;
@@ -560,10 +568,27 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
     legLink<<<gK, 256, 0, st>>>(li, lo, w.lg_best, w.lg_chi, cnt); ++L;
   }
   stage(16);
+  // ---- a11 optional merged tracks and leg labels (O12) ------------------------------------------------
+  stage(17);
+  if (n_mt == 4 && N > 0 && out->cap_tracks > 0) {
+    const int64_t nk = std::min<int64_t>(out->cap_tracks, capT);
+    const MergedIn mi{out->cap_tracks, out->trk_mg_next, out->trk_mg_head, out->trk_leg_partner, out->trk_cl_offset,
+                      out->trk_cl_index, in->z};
+    const MergedOut mo{out->trk_mt_id, out->trk_mt_rank, out->mt_cl_offset, out->mt_cl_index};
+    mergedLabel<<<(unsigned)ceilDiv(nk + 1, 256), 256, 0, st>>>(mi, mo, cnt); ++L;
+    // exclusive scan of the lengths in place: n_tracks entries and the closing one (the scan writes out[n] itself)
+    const unsigned tiles = (unsigned)ceilDiv(nk + 1, SCAN_TILE);
+    scanTileSums<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(out->mt_cl_offset, cnt + CNT_N_TRACKS, nk, w.mt_tiles); ++L;
+    scanTileOffsets<uint32_t><<<1, 1024, 0, st>>>(w.mt_tiles, cnt + CNT_N_TRACKS, nk, nullptr); ++L;
+    scanApply<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(out->mt_cl_offset, out->mt_cl_offset, cnt + CNT_N_TRACKS, nk, w.mt_tiles); ++L;
+    mergedFill<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(mi, mo, out->cap_track_clusters, cnt); ++L;
+  }
+  stage(18);
   // ---- a8 optional per-cluster flags (O8) ------------------------------------------------------------
   stage(11);
   if (n_fl == 2 && N > 0) {
     TPC_CUDA(h, cudaMemsetAsync(w.fl_key, 0xFF, 8 * (size_t)N, st)); ++L;
+    TPC_CUDA(h, cudaMemsetAsync(w.fl_prot, 0, 4 * (size_t)ceilDiv(N, 32), st)); ++L;
     TPC_CUDA(h, cudaMemsetAsync(out->cl_flags, 0, (size_t)N, st)); ++L;
     if (out->cl_res_code) { TPC_CUDA(h, cudaMemsetAsync(out->cl_res_code, 0, 4 * (size_t)N, st)); ++L; }
     if (out->cl_res_y) {
@@ -583,13 +608,13 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
                                                                                                        out->cl_flags, cnt); ++L;
       flagBid<<<(unsigned)ceilDiv(nk * FLAG_GROUP, 128), 128, 0, st>>>(fi, in->row_offset, P, T, h->params.tube_radius,
                                                           h->params.inv_pt_protect, w.desc, w.cell_start, w.syz, w.s2o,
-                                                          w.fl_key, walk_yz, cnt); ++L;
+                                                          w.fl_key, w.fl_prot, n_mt == 4 ? out->trk_mt_rank : nullptr, walk_yz, cnt); ++L;
       if (walk_yz) {
         flagResiduals<<<(unsigned)ceilDiv(n_ent, 256), 256, 0, st>>>(out->trk_cl_index, walk_yz, in->y, in->z, out->cl_res_y,
                                                                     out->cl_res_z, out->cl_res_code, h->params.pos_bits, cnt); ++L;
       }
     }
-    flagFinish<<<gN256, 256, 0, st>>>(N, w.fl_key, out->cl_flags, out->cl_owner, cnt); ++L;
+    flagFinish<<<gN256, 256, 0, st>>>(N, w.fl_key, w.fl_prot, out->cl_flags, out->cl_owner, cnt); ++L;
   }
   stage(12);
   // ---- a9 optional dynamic-precision charge code (O9) ------------------------------------------------
@@ -643,6 +668,7 @@ int tpcGetRunStatus(tpcHandle* h, tpcRunStatus* out) {
     if (cudaEventElapsedTime(&ms, h->ev_stage[11], h->ev_stage[12]) == cudaSuccess) out->flags_ms = ms;
     if (cudaEventElapsedTime(&ms, h->ev_stage[13], h->ev_stage[14]) == cudaSuccess) out->pack_ms = ms;
     if (cudaEventElapsedTime(&ms, h->ev_stage[15], h->ev_stage[16]) == cudaSuccess) out->legs_ms = ms;
+    if (cudaEventElapsedTime(&ms, h->ev_stage[17], h->ev_stage[18]) == cudaSuccess) out->merged_ms = ms;
   }
   return TPC_OK;
 }
@@ -662,6 +688,24 @@ const char* tpcErrorString(int code) {
 }
 
 const char* tpcLastCudaError(const tpcHandle* h) { return h ? h->cuda_msg : ""; }
+
+int tpcSelfTestDivision(tpcHandle* h, int64_t n_threads, uint64_t seed, int64_t* n_tested, int64_t* n_mismatches) {
+  if (!h || n_threads < 1 || n_threads > (1ll << 34) || !n_tested || !n_mismatches) return TPC_ERR_INVALID_ARG;
+  TPC_CUDA(h, cudaSetDevice(h->device));
+  unsigned long long* d = nullptr;
+  TPC_CUDA(h, cudaMalloc(&d, 16));
+  cudaError_t e = cudaMemset(d, 0, 16);
+  if (e == cudaSuccess) {
+    divisionSelfTest<<<(unsigned)ceilDiv(n_threads, 256), 256>>>((uint64_t)n_threads, seed, d, d + 1);
+    e = cudaGetLastError();
+  }
+  unsigned long long r[2] = {0, 0};
+  if (e == cudaSuccess) e = cudaMemcpy(r, d, 16, cudaMemcpyDeviceToHost);
+  cudaFree(d);
+  if (e != cudaSuccess) return cudaFail(h, e, "tpcSelfTestDivision");
+  *n_mismatches = (int64_t)r[0]; *n_tested = (int64_t)r[1];
+  return TPC_OK;
+}
 
 }  // extern "C"
 
@@ -688,7 +732,8 @@ extern "C" int tpcRunHost(tpcHandle* h, int64_t N, const uint32_t* row_offset, c
       oh->tl_first_row || oh->tl_last_row || oh->tl_rowhit || oh->tl_x || oh->tl_par || oh->tl_cov || oh->tl_chi2 ||
       oh->trk_rf_status || oh->trk_rf_x_in || oh->trk_rf_par_in || oh->trk_rf_cov_in || oh->trk_rf_chi2 || oh->trk_rf_x_out ||
       oh->trk_rf_par_out || oh->trk_rf_cov_out || oh->trk_mg_next || oh->trk_mg_prev || oh->trk_mg_head || oh->trk_mg_chi2 ||
-      oh->trk_leg_partner || oh->trk_leg_chi2 || oh->cl_flags || oh->cl_owner || oh->cl_qcode || oh->cl_res_y || oh->cl_res_z || oh->cl_pos_code || oh->cl_res_code)
+      oh->trk_leg_partner || oh->trk_leg_chi2 || oh->cl_flags || oh->cl_owner || oh->cl_qcode || oh->cl_res_y || oh->cl_res_z || oh->cl_pos_code || oh->cl_res_code ||
+      oh->trk_mt_id || oh->trk_mt_rank || oh->mt_cl_offset || oh->mt_cl_index)
     return TPC_ERR_INVALID_ARG;
   if (!oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0) return TPC_ERR_INVALID_ARG;
   TPC_CUDA(h, cudaSetDevice(h->device));
@@ -798,7 +843,7 @@ extern "C" int tpcSubmitHost(tpcHandle* h, int slot, int64_t N, const uint32_t* 
     return TPC_ERR_INVALID_ARG;
   if (oh->link_up_raw || oh->link_dn_raw || oh->link_up || oh->link_dn || oh->start_hits || oh->tl_status || oh->tl_nhits ||
       oh->tl_first_row || oh->tl_last_row || oh->tl_rowhit || oh->tl_x || oh->tl_par || oh->tl_cov || oh->tl_chi2 ||
-      oh->trk_rf_status || oh->trk_mg_next || oh->trk_leg_partner || oh->trk_leg_chi2 || oh->cl_flags || oh->cl_owner || oh->cl_qcode || oh->cl_res_y || oh->cl_res_z || oh->cl_pos_code || oh->cl_res_code || !oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0)
+      oh->trk_rf_status || oh->trk_mg_next || oh->trk_leg_partner || oh->trk_leg_chi2 || oh->cl_flags || oh->cl_owner || oh->cl_qcode || oh->cl_res_y || oh->cl_res_z || oh->cl_pos_code || oh->cl_res_code || oh->trk_mt_id || oh->trk_mt_rank || oh->mt_cl_offset || oh->mt_cl_index || !oh->trk_cl_offset || oh->cap_tracks < 0 || oh->cap_track_clusters < 0)
     return TPC_ERR_INVALID_ARG;
   TPC_CUDA(h, cudaSetDevice(h->device));
   int rc;
@@ -879,7 +924,7 @@ extern "C" int tpcCollectHost(tpcHandle* h, int slot, tpcRunStatus* status) {
     // the per-stage events belong to the handle, not to the slot: with two events in flight they may be the other
     // slot's.  Per-stage times are valid for tpcRun / tpcRunHost only.
     memset(status->stage_ms, 0, sizeof(status->stage_ms));
-    status->merge_ms = status->flags_ms = status->pack_ms = status->legs_ms = 0.0f;
+    status->merge_ms = status->flags_ms = status->pack_ms = status->legs_ms = status->merged_ms = 0.0f;
     float ms = 0;
     if (cudaEventElapsedTime(&ms, S.ev_begin, S.ev_kernels) == cudaSuccess) status->submit_ms[0] = ms;
     if (cudaEventElapsedTime(&ms, S.ev_begin, h->ev_done) == cudaSuccess) status->submit_ms[1] = ms;

@@ -5,10 +5,12 @@
 // A group of FLAG_GROUP lanes per refitted track walks its rows (every lane of the group carries the same state: the
 // Propagate is redundant but uniform, the candidates of a tube are shared out among the lanes).  The track walks its rows from the inner state by Propagate alone and bids for every cluster in
 // its tube (found through the a1 grid: cells of the box around the tube, exact circle predicate) and for its own
-// attached cluster of the row.  The bid is a 64-bit key  |q/pT| bits : track id : bad  taken with atomicMin, so the
-// owner is the track of minimal (|q/pT|, id) and the key carries whether that track is low-pT or steep at the
-// cluster's row (a track meets a cluster on one row only, so the last bit never decides).  A last pass per cluster
-// decodes the key into the flag byte.  Keys and flags are indexed by the ORIGINAL cluster index.
+// attached cluster of the row.  The bid is a 64-bit key  |q/pT| bits : track id  taken with atomicMin, so the owner is
+// the track of minimal (|q/pT|, id) -- the highest momentum (R36).  Protection does not go through the owner (R36b): every
+// track that is neither low-pT, nor steep on that row, nor a secondary leg (O12 rank 1, when the leg labels are given)
+// sets the cluster's bit in a protection bit mask (atomicOr), so a good track protects what lies in its tube even when
+// a steep or low track of higher momentum owns it.  A last pass per cluster decodes key and bit into
+// the flag byte.  Keys, bits and flags are indexed by the ORIGINAL cluster index.
 #pragma once
 #include "tpc_kalman.cuh"
 #include "tpc_select.cuh"
@@ -40,6 +42,7 @@ __global__ void __launch_bounds__(128) flagBid(FlagIn in, const uint32_t* __rest
                                                float tube, float inv_pt_protect, const GridDesc* __restrict__ desc,
                                                const uint32_t* __restrict__ cell_start, const float2* __restrict__ syz,
                                                const uint32_t* __restrict__ s2o, unsigned long long* __restrict__ key,
+                                               uint32_t* __restrict__ prot_bits, const int32_t* __restrict__ leg_rank,
                                                float2* __restrict__ walk_yz, const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
   const int64_t k = ((int64_t)blockIdx.x * blockDim.x + threadIdx.x) / FLAG_GROUP;
@@ -56,10 +59,10 @@ __global__ void __launch_bounds__(128) flagBid(FlagIn in, const uint32_t* __rest
   S.c32 = in.cov_in[8 * cap + k]; S.c33 = in.cov_in[9 * cap + k]; S.c40 = in.cov_in[10 * cap + k]; S.c41 = in.cov_in[11 * cap + k];
   S.c42 = in.cov_in[12 * cap + k]; S.c43 = in.cov_in[13 * cap + k]; S.c44 = in.cov_in[14 * cap + k];
   const float aq = fabsf(S.q);
-  const bool low = !(aq < inv_pt_protect);
+  const bool low = !(aq < inv_pt_protect) || (leg_rank != nullptr && leg_rank[k] == 1);      // or a secondary leg (L83, L86)
   const float sin70 = (float)0.9396926207859084;
   const float tube2 = tube * tube;
-  const unsigned long long khi = ((unsigned long long)__float_as_uint(aq) << 32) | ((unsigned long long)(uint32_t)k << 1);
+  const unsigned long long bid = ((unsigned long long)__float_as_uint(aq) << 32) | (unsigned long long)(uint32_t)k;
   const int sec = in.sector[k], f = in.first_row[k], l = in.last_row[k];
   const int bsec = sec * R;
   const uint32_t* cl = in.cl_index + in.cl_offset[k];
@@ -68,13 +71,14 @@ __global__ void __launch_bounds__(128) flagBid(FlagIn in, const uint32_t* __rest
   for (int r = f; r <= l; ++r) {
     if (T.dead[r]) continue;
     if (r > f && !kfPropagate(S, T.row_x[r], P, [](float, float, float, float) {})) break;
-    const unsigned long long bid = khi | (unsigned long long)((low || !(fabsf(S.s) < sin70)) ? 1u : 0u);
+    const bool good = !low && fabsf(S.s) < sin70;
     // the attached cluster of this row (R35): the list is in ascending row, rows follow from row_offset (R26)
     const uint32_t b_lo = __ldg(off + bsec + r), b_hi = __ldg(off + bsec + r + 1);
     while (ic < ncl && cl[ic] < b_lo) ++ic;
     if (sub == 0 && ic < ncl && cl[ic] < b_hi) {
       const uint32_t own = cl[ic];
       atomicMin(key + own, bid);
+      if (good) atomicOr(prot_bits + (own >> 5), 1u << (own & 31u));
       // for the track-model residuals (R39): the walking state at the attached cluster, in the order of the track's
       // cluster list (consecutive writes); flagResiduals turns them into residuals in one pass over all lists
       if (walk_yz) walk_yz[in.cl_offset[k] + ic] = make_float2(S.y, S.z);
@@ -94,7 +98,11 @@ __global__ void __launch_bounds__(128) flagBid(FlagIn in, const uint32_t* __rest
         const float2 c = __ldg(syz + i);
         const float dy = c.x - yc, dz = c.y - zc;
         const float d2 = dy * dy + dz * dz;
-        if (d2 <= tube2) atomicMin(key + __ldg(s2o + i), bid);
+        if (d2 <= tube2) {
+          const uint32_t o = __ldg(s2o + i);
+          atomicMin(key + o, bid);
+          if (good) atomicOr(prot_bits + (o >> 5), 1u << (o & 31u));
+        }
       }
     }
   }
@@ -130,21 +138,21 @@ __global__ void __launch_bounds__(256) flagResiduals(const uint32_t* __restrict_
 
 // thread per cluster: key -> flag byte and owner
 __global__ void __launch_bounds__(256) flagFinish(int64_t N, const unsigned long long* __restrict__ key,
-                                                  uint8_t* __restrict__ flags, int32_t* __restrict__ owner,
-                                                  const int64_t* __restrict__ cnt) {
+                                                  const uint32_t* __restrict__ prot_bits, uint8_t* __restrict__ flags,
+                                                  int32_t* __restrict__ owner, const int64_t* __restrict__ cnt) {
   if (cnt[CNT_ERROR] != 0) return;
   const int64_t c = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= N) return;
   const unsigned long long kk = key[c];
   const bool has = kk != ~0ull;
-  const bool prot = has && (kk & 1ull) == 0ull;
+  const bool prot = has && ((prot_bits[c >> 5] >> (c & 31)) & 1u) != 0u;
   uint8_t fl = flags[c] & 1;
   if (has) fl |= 2;
   if (prot) fl |= 4;
   if (has && !prot) fl |= 8;
   if (!prot) fl |= 16;
   flags[c] = fl;
-  owner[c] = has ? (int32_t)((kk >> 1) & 0x7fffffffull) : -1;
+  owner[c] = has ? (int32_t)(kk & 0x7fffffffull) : -1;
 }
 
 // a9 (part of NEXT-4; DESIGN.md section 3 "O9"): dynamic-precision 16-bit code of the cluster charges.

@@ -17,6 +17,15 @@ constexpr int TC_THREADS = TC_THREADS_;
 #ifndef TC_MIN_BLOCKS
 #define TC_MIN_BLOCKS 5
 #endif
+#ifndef TC_MB_UP
+#define TC_MB_UP TC_MIN_BLOCKS          // resident CTAs per SM the three passes are compiled for (register budget)
+#endif
+#ifndef TC_MB_SPAN
+#define TC_MB_SPAN TC_MIN_BLOCKS
+#endif
+#ifndef TC_MB_EXT
+#define TC_MB_EXT TC_MIN_BLOCKS
+#endif
 constexpr int MAX_ROWS = 256;
 #ifndef TC_HEADS
 #define TC_HEADS 6                  // candidates per cell row loaded and evaluated without a loop
@@ -275,7 +284,7 @@ __device__ __forceinline__ void writeTracklet(const TrackletStore& out, const De
 }
 
 // ---- pass 1: chain fit (O4 step 2) and up extrapolation (step 3) ---------------------------------------------------
-__global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) constructUp(
+__global__ void __launch_bounds__(TC_THREADS, TC_MB_UP) constructUp(
     DevParams P, RowTables T, const GridDesc* __restrict__ desc, const uint32_t* __restrict__ cell_start,
     const float2* __restrict__ syz, const uint32_t* __restrict__ s2o, const int32_t* __restrict__ cup,
     const SeedRec* __restrict__ work_list, TurnRec* __restrict__ turn_list, TrackletStore out, int64_t* __restrict__ cnt) {
@@ -407,7 +416,7 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) constructUp(
 
 // ---- passes 2 and 3: the down pass (O4 steps 4-6), over the span (EXT = 0) and below the start row (EXT = 1) -----------
 template <int EXT>
-__global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) constructDown(
+__global__ void __launch_bounds__(TC_THREADS, EXT ? TC_MB_EXT : TC_MB_SPAN) constructDown(
     DevParams P, RowTables T, const GridDesc* __restrict__ desc, const uint32_t* __restrict__ cell_start,
     const float2* __restrict__ syz, const uint32_t* __restrict__ s2o, const TurnRec* __restrict__ turn_list,
     uint4* __restrict__ down_list, TrackletStore out, int64_t* __restrict__ cnt) {
@@ -495,6 +504,10 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MIN_BLOCKS) constructDown(
     const GridDesc G = desc[act ? s_bsec[tid] + rn : 0];
     if (!EXT && act && c_cur >= 0) mk = __ldg(syz + c_cur);
     SearchPre sp;
+    // span pass: 4 % of the steps are gap rows (the up pass found nothing there) and need a Search; 1.5 lanes of a warp at
+    // a time, so the whole warp issues the search code on nearly every step.  A lean out-of-line search with plain loops
+    // was tried (4.8e9 instead of 5.9e9 warp instructions) and is slower (a4 26.5 ms against 25.7 ms): its dependent
+    // loads cost the other lanes four memory latencies where the prefetching form below costs one.
     const bool want_search = act && (EXT || c_cur < 0);
     const bool okp = act && kfPropagate(S, rs.sx[act ? rn : 0], P, [&](float y1, float z1, float c00, float c11) {
       if (want_search) searchBegin(sp, y1, z1, c00, c11, G, cell_start, P);

@@ -59,22 +59,24 @@ _LEG_PTRS = ("trk_leg_partner", "trk_leg_chi2")
 _FLAG_PTRS = ("cl_flags", "cl_owner", "cl_res_y", "cl_res_z")
 _PACK_PTRS = ("cl_qcode",)
 _POS_PTRS = ("cl_pos_code", "cl_res_code")
+_MERGED_PTRS = ("trk_mt_id", "trk_mt_rank", "mt_cl_offset", "mt_cl_index")
 
 
 class tpcTracks(ctypes.Structure):
     _fields_ = [("cap_tracks", c_int64), ("cap_track_clusters", c_int64)] + \
-               [(n, c_void_p) for n in _TRK_PTRS + _STAGE_PTRS + _REFIT_PTRS + _MERGE_PTRS + _LEG_PTRS + _FLAG_PTRS + _PACK_PTRS + _POS_PTRS]
+               [(n, c_void_p) for n in _TRK_PTRS + _STAGE_PTRS + _REFIT_PTRS + _MERGE_PTRS + _LEG_PTRS + _FLAG_PTRS + _PACK_PTRS + _POS_PTRS + _MERGED_PTRS]
 
 
 class tpcRunStatus(ctypes.Structure):
     _fields_ = [("status", c_int32), ("kernel_launches", c_int32), ("n_clusters", c_int64), ("n_start_hits", c_int64),
                 ("n_tracklets", c_int64), ("n_tracklet_hits", c_int64), ("n_tracks", c_int64),
-                ("n_track_clusters", c_int64), ("n_cells", c_int64), ("stage_ms", c_float * 8), ("merge_ms", c_float), ("pack_ms", c_float), ("flags_ms", c_float), ("legs_ms", c_float),
+                ("n_track_clusters", c_int64), ("n_cells", c_int64), ("stage_ms", c_float * 8), ("merge_ms", c_float), ("pack_ms", c_float), ("flags_ms", c_float), ("legs_ms", c_float), ("merged_ms", c_float),
                 ("submit_ms", c_float * 2)]
 
 
 ABI_SYMBOLS = ("tpcDefaultParams", "tpcCreate", "tpcDestroy", "tpcWorkspaceBytes", "tpcRun", "tpcGetRunStatus",
-               "tpcSetProfiling", "tpcRunHost", "tpcSubmitHost", "tpcCollectHost", "tpcErrorString", "tpcLastCudaError")
+               "tpcSetProfiling", "tpcRunHost", "tpcSubmitHost", "tpcCollectHost", "tpcErrorString", "tpcLastCudaError",
+               "tpcSelfTestDivision")
 
 _lib = None
 
@@ -111,6 +113,8 @@ def load_library(build_if_stale: bool = True) -> ctypes.CDLL:
     L.tpcErrorString.restype = c_char_p
     L.tpcLastCudaError.argtypes = [vp]
     L.tpcLastCudaError.restype = c_char_p
+    L.tpcSelfTestDivision.argtypes = [vp, c_int64, ctypes.c_uint64, POINTER(c_int64), POINTER(c_int64)]
+    L.tpcSelfTestDivision.restype = c_int
     _lib = L
     return L
 
@@ -170,6 +174,16 @@ def tpcGetRunStatus(handle) -> tpcRunStatus:
 
 def tpcSetProfiling(handle, on: bool) -> None:
     load_library().tpcSetProfiling(handle, int(on))
+
+
+def tpcSelfTestDivision(handle, n_threads: int, seed: int = 1):
+    """(operand pairs tested, bit patterns that differ between the shared-reciprocal division and the IEEE one)."""
+    L = load_library()
+    nt, nm = c_int64(), c_int64()
+    rc = L.tpcSelfTestDivision(handle, int(n_threads), int(seed), byref(nt), byref(nm))
+    if rc != TPC_OK:
+        raise TpcError(rc, "tpcSelfTestDivision", L.tpcLastCudaError(handle).decode())
+    return nt.value, nm.value
 
 
 # ---- convenience wrapper: allocation of device tensors with torch, nothing else ---------------------------
@@ -240,7 +254,8 @@ class TpcTracker:
         z = t.from_numpy(np.ascontiguousarray(ev.z, np.float32)).to(self.device)
         return off, y, z
 
-    def _ensure(self, n, capT, capK, capC, stages, refit=False, merge=False, flags=False, pack=False, legs=False, pos=False):
+    def _ensure(self, n, capT, capK, capC, stages, refit=False, merge=False, flags=False, pack=False, legs=False, pos=False,
+                merged=False):
         t = self.torch
         need = tpcWorkspaceBytes(self.handle, n, capT)
         if self._ws is None or self._ws.numel() < need:
@@ -277,6 +292,9 @@ class TpcTracker:
                 spec.update({"cl_res_code": ((max(n, 1),), i32)})
         if legs:
             spec.update({"trk_leg_partner": ((capK,), i32), "trk_leg_chi2": ((capK,), f32)})
+        if merged:
+            spec.update({"trk_mt_id": ((capK,), i32), "trk_mt_rank": ((capK,), i32), "mt_cl_offset": ((capK + 1,), i32),
+                         "mt_cl_index": ((max(capC, 1),), i32)})
         for k, (shape, dt) in spec.items():
             cur = self._out.get(k)
             if cur is None or tuple(cur.shape) != shape:
@@ -288,17 +306,19 @@ class TpcTracker:
     def run(self, row_offset, y, z, cap_tracklets: int | None = None, cap_tracks: int | None = None,
             cap_track_clusters: int | None = None, stages: bool = False, stream=None, sync: bool = True,
             grow: bool = True, refit: bool = False, merge: bool = False, flags: bool = False, q=None,
-            legs: bool = False, pos: bool = False):
+            legs: bool = False, pos: bool = False, merged: bool = False):
         """One tpcRun on device tensors (q: optional device tensor of charges -> cl_qcode, the O9 charge code).  Returns a TrackResult (after synchronising) or None when sync=False."""
         t = self.torch
         n = int(y.shape[0])
+        merge = merge or merged                   # the merged tracks are built from the merger's chains and the leg pairs
+        legs = legs or merged
         refit = refit or merge or flags or legs   # the merger, the leg pairs and the cluster flags work on the refitted states
         capT = int(cap_tracklets) if cap_tracklets is not None else max(4096, n // 8)
         capK = int(cap_tracks) if cap_tracks is not None else capT
         capC = int(cap_track_clusters) if cap_track_clusters is not None else max(n, 1)
         attempts = 3 if grow else 0     # a too-small cap_tracklets hides the true track counts: up to 3 rounds
         while True:
-            self._ensure(n, capT, capK, capC, stages, refit, merge, flags, q is not None, legs, pos)
+            self._ensure(n, capT, capK, capC, stages, refit, merge, flags, q is not None, legs, pos, merged)
             cl = tpcClusters(n, row_offset.data_ptr(), None, y.data_ptr() if n else None, z.data_ptr() if n else None,
                              q.data_ptr() if (q is not None and n) else None)
             tr = tpcTracks()
@@ -335,6 +355,9 @@ class TpcTracker:
         if legs:
             for k in _LEG_PTRS:
                 trk[k] = o[k][:nt]
+        if merged:
+            trk["trk_mt_id"], trk["trk_mt_rank"] = o["trk_mt_id"][:nt], o["trk_mt_rank"][:nt]
+            trk["mt_cl_offset"], trk["mt_cl_index"] = o["mt_cl_offset"][:nt + 1], o["mt_cl_index"][:nc]
         if flags:
             for k in _FLAG_PTRS:
                 trk[k] = o[k][:n]

@@ -269,3 +269,19 @@ def test_submit_collect_pipeline_matches_run_host():
     st, out = trk.collect_host(1)
     assert st.status == 0
     trk.close()
+
+
+def test_shared_denominator_division_is_bit_identical_to_the_ieee_division():
+    """R0 for the one place where the kernels do not write `a / S`: the Kalman update's six quotients by one reciprocal
+    (csrc/tpc_kalman.cuh).  2^26 threads x 48 operand pairs over the whole domain of the shared form, zeros of both signs,
+    exact quotients, the edge of the domain and overflowing quotients included: no bit pattern may differ."""
+    from paper_1910_12214_b200 import tpc
+    ev = datagen.make_event(0, scale=0.05)
+    trk = tpc.TpcTracker.from_event(ev)
+    tested = 0
+    for seed in (1, 2, 3):
+        n, bad = tpc.tpcSelfTestDivision(trk.handle, 1 << 26, seed)
+        assert bad == 0, (seed, bad, n)
+        tested += n
+    trk.close()
+    assert tested == 3 * 48 * (1 << 26)
