@@ -653,6 +653,7 @@ struct Tracker {
     res.cf_res_y.assign(N, 0); res.cf_res_z.assign(N, 0);
     const Real bf = (Real)(0.00299792458 * (double)g.bz_tesla);
     const Real msp = (Real)P.max_sinphi, tube2 = (Real)P.tube_radius * (Real)P.tube_radius;
+    const bool dyn = P.tube_chi2_max > 0.0f;       // R49: the chi2 criterion of PAPER.md L108 / L114 on top of the fixed tube
     const Real sin70 = (Real)0.9396926207859084, qmax = (Real)P.inv_pt_protect;
     std::vector<Real> ownerQ(N, 0);
     std::vector<uint8_t> protAny(N, 0);          // some track that is neither low, steep nor a secondary leg has it in its tube
@@ -680,7 +681,12 @@ struct Tracker {
         for (uint32_t c = off[sec * R + r]; c < off[sec * R + r + 1]; ++c) {
           const Real dy = Y[c] - st.y, dz = Z[c] - st.z;
           const Real d2 = dy * dy + dz * dz;
-          if (!(d2 <= tube2) && (int32_t)c != own) continue;
+          bool in = d2 <= tube2;
+          if (in && dyn) {                                  // distance in units of the track's own uncertainty on this row
+            const Real x2 = (dy * dy) / (st.C[0] + (Real)P.err2_y) + (dz * dz) / (st.C[2] + (Real)P.err2_z);
+            in = x2 <= (Real)P.tube_chi2_max;
+          }
+          if (!in && (int32_t)c != own) continue;
           if (!bad) protAny[c] = 1;                         // R36b: every good track protects what is in its tube
           if (res.cf_owner[c] < 0 || aq < ownerQ[c]) {      // ties: the lower track index (loop order)
             res.cf_owner[c] = (int32_t)k; ownerQ[c] = aq;
@@ -851,6 +857,7 @@ void orcDefaultParams(orcParams* p) {
   p->tube_radius = 1.5f; p->inv_pt_protect = 20.0f;
   p->leg_min_sinphi = 0.5f; p->leg_chi2_max = 50.0f; p->leg_max_sectors = 4; p->leg_max_row_diff = 12;
   p->leg_max_centre_dist = 10.0f;
+  p->tube_chi2_max = 0.0f;
 }
 
 int orcRun(const orcGeometry* g, const orcParams* p, int64_t n, const uint32_t* off, const float* y, const float* z,

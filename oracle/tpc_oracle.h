@@ -46,6 +46,7 @@ typedef struct {
   float leg_min_sinphi, leg_chi2_max;           /* O10: 0.5, 50 */
   int32_t leg_max_sectors, leg_max_row_diff;    /* O10: 4, 12 */
   float leg_max_centre_dist;                    /* O10: 10 cm */
+  float tube_chi2_max;                          /* O8, R49: 0 = fixed tube only; > 0: also dy^2/(C00+err2_y) + dz^2/(C11+err2_z) <= this */
 } orcParams;
 
 typedef struct orcResult orcResult;

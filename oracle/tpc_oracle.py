@@ -49,7 +49,7 @@ class Params(ctypes.Structure):
                 ("merge_back_rows", ctypes.c_int32), ("merge_chi2_max", ctypes.c_float), ("tube_radius", ctypes.c_float),
                 ("inv_pt_protect", ctypes.c_float),
                 ("leg_min_sinphi", ctypes.c_float), ("leg_chi2_max", ctypes.c_float), ("leg_max_sectors", ctypes.c_int32),
-                ("leg_max_row_diff", ctypes.c_int32), ("leg_max_centre_dist", ctypes.c_float)]
+                ("leg_max_row_diff", ctypes.c_int32), ("leg_max_centre_dist", ctypes.c_float), ("tube_chi2_max", ctypes.c_float)]
 
 
 _lib = None

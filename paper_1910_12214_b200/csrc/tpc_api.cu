@@ -90,6 +90,7 @@ struct tpcHandle {
   //   // 0..6 stage boundaries, 7/8 around the optional refit, 9/10 merger, 11/12 flags
   int profiling = 0;
   int launches = 0;
+  int gb_smem_cells = 24 * 1024;      // cells of a bucket whose histogram gridBuild keeps in shared memory (96 KB: two CTAs per SM)
   int tc_grid[3] = {148, 148, 148};   // persistent grids of the three constructor passes: SMs x resident blocks
   bool pending = false;
   int64_t last_n = 0;
@@ -302,6 +303,10 @@ int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cud
       h->tc_grid[i] = sms * per_sm;
     }
   }
+  if (cudaFuncSetAttribute(gridBuild, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * h->gb_smem_cells) != cudaSuccess) {
+    cudaGetLastError();
+    h->gb_smem_cells = 10 * 1024;     // 40 KB needs no opt-in
+  }
   memset(h->h_cnt, 0, 8 * (CNT_COUNT + 1));
   *out = h;
   return TPC_OK;
@@ -398,15 +403,9 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   // ---- a1 grid ----------------------------------------------------------------------------------
   gridSetup<<<1, 1024, 0, st>>>(in->row_offset, N, P, h->d_row_x, w.desc, w.chunk_base, NF_THREADS, cnt, cc); ++L;
   if (N > 0) {
-    TPC_CUDA(h, cudaMemsetAsync(w.cell_start, 0, 4 * (size_t)(cc + 1), st)); ++L;
-    gridCount<<<gN256, 256, 0, st>>>(in->row_offset, in->y, in->z, N, nb, w.desc, w.cell_start, w.rank, cnt,
-                                     h->params.validate_input); ++L;
-    const unsigned tiles = (unsigned)ceilDiv(cc, SCAN_TILE);
-    scanTileSums<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.cell_start, cnt + CNT_N_CELLS, cc, w.tiles32); ++L;
-    scanTileOffsets<uint32_t><<<1, 1024, 0, st>>>(w.tiles32, cnt + CNT_N_CELLS, cc, nullptr); ++L;
-    scanApply<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.cell_start, w.cell_start, cnt + CNT_N_CELLS, cc, w.tiles32); ++L;
-    gridScatter<<<gN256, 256, 0, st>>>(in->row_offset, in->y, in->z, N, nb, w.desc, w.cell_start, w.rank, w.syz, w.s2o,
-                                       cnt); ++L;
+    gridBuild<<<(unsigned)nb, GB_THREADS, 4 * (size_t)h->gb_smem_cells, st>>>(in->row_offset, in->y, in->z, nb, w.desc, w.cell_start,
+                                                                              w.rank, w.syz, w.s2o, cnt, h->params.validate_input,
+                                                                              (uint32_t)h->gb_smem_cells); ++L;
   }
   stage(1);
   // ---- a2 neighbour finder ------------------------------------------------------------------------

@@ -119,6 +119,10 @@ def _flags_numpy(ev, res, p, rank=None):
             dy = y32[lo:hi] - np.float32(st[1])
             dz = z32[lo:hi] - np.float32(st[2])
             inside = (dy * dy + dz * dz) <= tube2
+            if p.tube_chi2_max > 0:                      # R49
+                c32 = cov.astype(np.float32)
+                x2 = (dy * dy) / (c32[0] + np.float32(p.err2_y)) + (dz * dz) / (c32[2] + np.float32(p.err2_z))
+                inside &= x2 <= np.float32(p.tube_chi2_max)
             own = cl[rowof[cl] == r]
             inside[own - lo] = True
             for c in own:
@@ -236,3 +240,52 @@ def test_residuals_have_the_least_squares_variance():
     assert np.mean(ry ** 2) == pytest.approx(np.mean(ey), rel=0.05)
     assert np.mean(rz ** 2) == pytest.approx(np.mean(ez), rel=0.05)
     assert abs(np.mean(ry)) < 0.005 and abs(np.mean(rz)) < 0.005
+
+
+def test_chi2_tube_on_a_hand_built_track():
+    """R49 ("replacing the fixed tube of 1.5 cm radius by a dynamic criterion taking into account the chi2").
+    The straight-ish 20 GeV/c track of the first test with extra clusters on row 40.  The walking state there comes from the
+    inner state (row 10) by Propagate alone, so its variances are those of the fit carried 30 rows: the test takes them from
+    the pinned single Propagate step, builds the ellipse chi2 = dy^2 / (C00 + 0.01) + dz^2 / (C11 + 0.01) = 25 by hand and puts
+    clusters 3 % inside and 3 % outside it on both axes and on the diagonal: inside -> adjacent and protected, outside ->
+    untouched -- although every one of them lies well inside the fixed 1.5 cm tube, which alone would take them all."""
+    rows = list(range(10, 70))
+    tr = _helix_points(20.0, 1, 0.1, 0.3, -3.0, 20.0, rows)
+    pts = [(r, p[1], p[2]) for r, p in zip(rows, tr)]
+    ev, where = _event(pts)
+    base = orc.run(ev, flags=True)
+    st, cov = np.concatenate([[base.rf_x_in[0]], base.rf_par_in[0]]), base.rf_cov_in[0].copy()
+    for r in range(11, 41):
+        ok, st, cov = orc.propagate(st, cov, ROW_X[r], BZ, 0.98, fp64=False)
+        assert ok
+    ay, az = math.sqrt(25.0 * (cov[0] + 0.01)), math.sqrt(25.0 * (cov[2] + 0.01))     # half axes of the chi2 = 25 ellipse
+    assert 0.5 < ay < 1.0 and 0.5 < az < 1.0                                          # far inside the 1.5 cm tube
+    y40, z40 = st[1], st[2]
+    d = math.sqrt(0.5)
+    extra = [(40, y40 + 0.97 * ay, z40), (40, y40 + 1.03 * ay, z40), (40, y40, z40 - 0.97 * az), (40, y40, z40 - 1.03 * az),
+             (40, y40 - 0.97 * d * ay, z40 + 0.97 * d * az), (40, y40 - 1.03 * d * ay, z40 + 1.03 * d * az)]
+    ev, where = _event(pts + extra)
+    p = orc.default_params()
+    p.tube_chi2_max = 25.0
+    res = orc.run(ev, p, flags=True)
+    assert res.n_tracks == 1 and res.trk_ncl[0] == len(rows)
+    e = where[len(rows):]
+    assert [int(res.cf_flags[i]) for i in e] == [ADJ | PROT, RMB, ADJ | PROT, RMB, ADJ | PROT, RMB]
+    assert np.all(res.cf_flags[where[:len(rows)]] == ATT | ADJ | PROT)                # the attached clusters always count (R35)
+    res = orc.run(ev, flags=True)                                                      # fixed tube: all six are inside
+    assert np.all(res.cf_flags[e] == ADJ | PROT)
+
+
+def test_chi2_tube_equals_the_numpy_restatement_and_only_shrinks_the_tubes():
+    ev = datagen.make_event(2, scale=0.03)
+    p = orc.default_params()
+    fixed = orc.run(ev, p, flags=True, merged=True)
+    p.tube_chi2_max = 25.0
+    res = orc.run(ev, p, flags=True, merged=True)
+    f, owner, ry, rz = _flags_numpy(ev, res, p, rank=res.mt_rank)
+    assert np.array_equal(owner, res.cf_owner) and np.array_equal(f, res.cf_flags)
+    adj_f, adj_d = (fixed.cf_flags & ADJ) != 0, (res.cf_flags & ADJ) != 0
+    assert not np.any(adj_d & ~adj_f) and adj_d.sum() < adj_f.sum()                  # a subset of the fixed tube
+    assert np.array_equal((fixed.cf_flags & ATT) != 0, (res.cf_flags & ATT) != 0)
+    noise = ev.truth_track < 0
+    assert ((res.cf_flags & PROT) != 0)[noise].mean() < ((fixed.cf_flags & PROT) != 0)[noise].mean()     # fewer fake-protected
