@@ -51,6 +51,7 @@ STAGE_KERNEL = {"a1_grid": "gridCount+gridScatter", "a2_neighbours": "neighbourF
 O4_FLOPS = (176, 100, 6, 5)
 O2_FLOPS = (4, 5)            # slopes of a window candidate (2 subtractions, 2 products); Dev of a pair (2, 2, 1)
 SURVEY_BYTES_PER_CLUSTER = 140   # the fixed accounting with H = N
+TUBE_CHI2_MAX = 25.0             # the chi2 tube of the second flags run (R49)
 
 
 def _peaks():
@@ -276,15 +277,16 @@ def run_ours(args, rank, world, local_rank):
     stage /= n_inst
 
     # ---- the NEXT rows (a6 refit, a7 merger, a10 legs, a8 flags, a9 codes), timed apart: not part of the a1..a5 step ----
-    refit_ms = merge_ms = flags_ms = pack_ms = legs_ms = None
-    n_links = n_legs = 0
+    refit_ms = merge_ms = flags_ms = pack_ms = legs_ms = merged_ms = None
+    n_links = n_legs = n_two_leg = 0
     flag_frac = {}
+    flag_names = (("attached", 1), ("adjacent", 2), ("protected", 4), ("removed_A", 8), ("removed_B", 16))
     if not args.no_refit:
-        acc = accm = accf = accp = accl = 0.0
+        acc = accm = accf = accp = accl = accd = 0.0
         dq = torch.from_numpy(ev.q).to(y.device)
         for i in range(4):
             trk.run(off, y, z, cap_tracklets=capT, cap_tracks=capK, cap_track_clusters=capC, sync=False, merge=True, flags=True, q=dq,
-                    legs=True, pos=True)
+                    legs=True, pos=True, merged=True)
             s = trk.status()
             if i > 0:
                 acc += float(s.stage_ms[7])
@@ -292,10 +294,11 @@ def run_ours(args, rank, world, local_rank):
                 accf += float(s.flags_ms)
                 accp += float(s.pack_ms)
                 accl += float(s.legs_ms)
-        refit_ms, merge_ms, flags_ms, pack_ms, legs_ms = acc / 3, accm / 3, accf / 3, accp / 3, accl / 3
+                accd += float(s.merged_ms)
+        refit_ms, merge_ms, flags_ms, pack_ms, legs_ms, merged_ms = acc / 3, accm / 3, accf / 3, accp / 3, accl / 3, accd / 3
         fl = trk._out["cl_flags"][:N]
-        flag_frac = {name: round(float(((fl & bit) != 0).float().mean().item()), 4)
-                     for name, bit in (("attached", 1), ("adjacent", 2), ("protected", 4), ("removed_A", 8), ("removed_B", 16))}
+        flag_frac = {name: round(float(((fl & bit) != 0).float().mean().item()), 4) for name, bit in flag_names}
+        n_two_leg = int((trk._out["trk_mt_rank"][:int(s.n_tracks)] == 1).sum().item())
         n_links = int((trk._out["trk_mg_next"][:int(s.n_tracks)] >= 0).sum().item())
         n_legs = int((trk._out["trk_leg_partner"][:int(s.n_tracks)] >= 0).sum().item()) // 2
     trk.set_profiling(False)
@@ -338,6 +341,22 @@ def run_ours(args, rank, world, local_rank):
     # tpcSubmitHost copies back up to the capacities (the counts are not known on the host at submit time)
     d2h = capK * (5 * 4 + 4 + 20 + 60 + 4) + 4 * (capK + 1) + 4 * capC + 8 * 11
 
+    # ---- the flags once more with the chi2 criterion of PAPER.md L108 / L114 on top of the fixed tube (R49): a second
+    #      tracker, because the criterion is a creation-time parameter ------------------------------------------------
+    flag_frac_chi2, flags_chi2_ms = {}, None
+    if not args.no_refit and rank == 0:
+        trk.close()
+        p2 = tpc.tpcDefaultParams()
+        p2.tube_chi2_max = TUBE_CHI2_MAX
+        trk2 = tpc.TpcTracker.from_event(ev, params=p2, device=local_rank)
+        trk2.set_profiling(True)
+        for i in range(2):
+            trk2.run(off, y, z, cap_tracklets=capT, cap_tracks=capK, cap_track_clusters=capC, sync=False, flags=True, merged=True)
+            s2 = trk2.status()
+        flags_chi2_ms = float(s2.flags_ms)
+        fl = trk2._out["cl_flags"][:N]
+        flag_frac_chi2 = {name: round(float(((fl & bit) != 0).float().mean().item()), 4) for name, bit in flag_names}
+        trk2.close()
     if rank != 0:
         return
     # ---- CPU baseline: the oracle on one sector of this event (rank 0, N = 1 only); its operation counters give the
@@ -464,14 +483,19 @@ def run_ours(args, rank, world, local_rank):
                               "links": n_links}
         line["next_legs"] = {"what": "a10 pairs of looper legs (rest of NEXT-1), not part of `value`", "ms": round(legs_ms, 4),
                              "pairs": n_legs}
+        line["next_merged"] = {"what": "a11 merged tracks and leg labels (O12; rest of NEXT-1, input of NEXT-3), not part of `value`",
+                               "ms": round(merged_ms, 4), "tracks_on_secondary_legs": n_two_leg}
         pb = 6 * N + 12 * N       # charge: 4 B in, 2 B out; positions: 8 B in, 4 B out
         line["next_pack"] = {"what": "a9 dynamic-precision charge code and 16-bit position code (NEXT-4), two streaming "
                                      "kernels, not part of `value`",
                              "ms": round(pack_ms, 4), "alg_bytes": pb, "bound": "hbm",
                              "gbs": round(pb / (pack_ms * 1e-3) / 1e9, 1) if pack_ms > 0 else None,
                              "frac_of_hbm_peak": round(pb / (pack_ms * 1e-3) / 1e9 / peak, 4) if pack_ms > 0 else None}
-        line["next_flags"] = {"what": "a8 cluster flags and rejection strategies A / B (NEXT-3), not part of `value`",
-                              "ms": round(flags_ms, 4), "fractions_of_clusters": flag_frac}
+        line["next_flags"] = {"what": "a8 cluster flags and rejection strategies A / B (NEXT-3) with the leg labels of a11 (secondary "
+                                      "legs do not protect and are removable by strategy A), not part of `value`",
+                              "ms": round(flags_ms, 4), "fractions_of_clusters": flag_frac,
+                              "chi2_tube": {"tube_chi2_max": TUBE_CHI2_MAX, "ms": round(flags_chi2_ms, 4) if flags_chi2_ms else None,
+                                            "fractions_of_clusters": flag_frac_chi2}}
     print(json.dumps(line), flush=True)
 
 

@@ -87,6 +87,8 @@ typedef struct {
   int32_t leg_max_row_diff;     /* 12         O10: and their last rows at most this many rows */
   float leg_max_centre_dist;    /* 10         O10: and the centres of their circles at most this far apart, cm */
   int32_t pos_bits;             /* 6          O11: positions and residuals are stored in units of 2^-pos_bits cm (0..15) */
+  float tube_chi2_max;          /* 0          O8, R49: 0 = the fixed tube alone; > 0: a cluster of the tube must
+                                              also have dy^2/(C00+err2_y) + dz^2/(C11+err2_z) <= this (walking state's variances) */
 } tpcParams;
 
 /* Input clusters: CSR by (sector,row), fp32 SoA (single-precision cluster properties). */

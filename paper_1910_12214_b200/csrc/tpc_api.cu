@@ -229,7 +229,7 @@ int tpcDefaultParams(tpcParams* p) {
   p->merge_max_row_gap = 40; p->merge_back_rows = 5; p->merge_chi2_max = 50.0f;
   p->tube_radius = 1.5f; p->inv_pt_protect = 20.0f; p->charge_trunc_bits = 4;
   p->leg_min_sinphi = 0.5f; p->leg_chi2_max = 50.0f; p->leg_max_sectors = 4; p->leg_max_row_diff = 12;
-  p->leg_max_centre_dist = 10.0f; p->pos_bits = 6;
+  p->leg_max_centre_dist = 10.0f; p->pos_bits = 6; p->tube_chi2_max = 0.0f;
   return TPC_OK;
 }
 
@@ -244,6 +244,7 @@ int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cud
   if (!(p->cell_min > 0) || !(p->cell_max >= p->cell_min) || !(p->clusters_per_cell > 0)) return TPC_ERR_INVALID_ARG;
   if (p->min_chain_hits < 2 || p->max_row_gap < 0) return TPC_ERR_INVALID_ARG;
   if (p->merge_max_row_gap < 0 || p->merge_back_rows < 0) return TPC_ERR_INVALID_ARG;
+  if (!(p->tube_chi2_max >= 0)) return TPC_ERR_INVALID_ARG;
   if (!(p->tube_radius >= 0) || p->charge_trunc_bits < 0 || p->charge_trunc_bits > 14) return TPC_ERR_INVALID_ARG;
   if (p->pos_bits < 0 || p->pos_bits > 15) return TPC_ERR_INVALID_ARG;
   if (p->leg_max_sectors < 0 || p->leg_max_sectors > LEG_MAX_SECTORS || p->leg_max_row_diff < 0) return TPC_ERR_INVALID_ARG;
@@ -605,9 +606,16 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
       if (walk_yz) { TPC_CUDA(h, cudaMemsetAsync(walk_yz, 0xFF, 8 * (size_t)n_ent, st)); ++L; }
       flagAttach<<<(unsigned)ceilDiv(std::min<int64_t>(out->cap_track_clusters, N), 256), 256, 0, st>>>(out->trk_cl_index,
                                                                                                        out->cl_flags, cnt); ++L;
-      flagBid<<<(unsigned)ceilDiv(nk * FLAG_GROUP, 128), 128, 0, st>>>(fi, in->row_offset, P, T, h->params.tube_radius,
-                                                          h->params.inv_pt_protect, w.desc, w.cell_start, w.syz, w.s2o,
-                                                          w.fl_key, w.fl_prot, n_mt == 4 ? out->trk_mt_rank : nullptr, walk_yz, cnt); ++L;
+      const unsigned gB = (unsigned)ceilDiv(nk * FLAG_GROUP, 128);
+      const int32_t* rk = n_mt == 4 ? out->trk_mt_rank : nullptr;
+      if (h->params.tube_chi2_max > 0.0f)
+        flagBid<1><<<gB, 128, 0, st>>>(fi, in->row_offset, P, T, h->params.tube_radius, h->params.tube_chi2_max,
+                                       h->params.inv_pt_protect, w.desc, w.cell_start, w.syz, w.s2o, w.fl_key, w.fl_prot, rk,
+                                       walk_yz, cnt);
+      else
+        flagBid<0><<<gB, 128, 0, st>>>(fi, in->row_offset, P, T, h->params.tube_radius, 0.0f, h->params.inv_pt_protect, w.desc,
+                                       w.cell_start, w.syz, w.s2o, w.fl_key, w.fl_prot, rk, walk_yz, cnt);
+      ++L;
       if (walk_yz) {
         flagResiduals<<<(unsigned)ceilDiv(n_ent, 256), 256, 0, st>>>(out->trk_cl_index, walk_yz, in->y, in->z, out->cl_res_y,
                                                                     out->cl_res_z, out->cl_res_code, h->params.pos_bits, cnt); ++L;

@@ -38,8 +38,11 @@ __global__ void __launch_bounds__(256) flagAttach(const uint32_t* __restrict__ c
 #endif
 constexpr int FLAG_GROUP = FLAG_GROUP_;      // lanes per track
 
+// CHI2 = 1: the chi2 criterion of R49 on top of the fixed tube (the walk then carries its covariance; with CHI2 = 0 the
+// compiler drops the covariance transport, which no result depends on)
+template <int CHI2>
 __global__ void __launch_bounds__(128) flagBid(FlagIn in, const uint32_t* __restrict__ off, DevParams P, RowTables T,
-                                               float tube, float inv_pt_protect, const GridDesc* __restrict__ desc,
+                                               float tube, float chi2_max, float inv_pt_protect, const GridDesc* __restrict__ desc,
                                                const uint32_t* __restrict__ cell_start, const float2* __restrict__ syz,
                                                const uint32_t* __restrict__ s2o, unsigned long long* __restrict__ key,
                                                uint32_t* __restrict__ prot_bits, const int32_t* __restrict__ leg_rank,
@@ -98,7 +101,12 @@ __global__ void __launch_bounds__(128) flagBid(FlagIn in, const uint32_t* __rest
         const float2 c = __ldg(syz + i);
         const float dy = c.x - yc, dz = c.y - zc;
         const float d2 = dy * dy + dz * dz;
-        if (d2 <= tube2) {
+        bool inside = d2 <= tube2;
+        if (CHI2 && inside) {
+          const float x2 = (dy * dy) / (S.c00 + P.err2_y) + (dz * dz) / (S.c11 + P.err2_z);
+          inside = x2 <= chi2_max;
+        }
+        if (inside) {
           const uint32_t o = __ldg(s2o + i);
           atomicMin(key + o, bid);
           if (good) atomicOr(prot_bits + (o >> 5), 1u << (o & 31u));

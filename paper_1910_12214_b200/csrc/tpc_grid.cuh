@@ -79,6 +79,10 @@ __global__ void __launch_bounds__(1024) gridSetup(const uint32_t* __restrict__ o
 // array (more than `smem_cells`) runs the same passes with its slice of the global table as the histogram and the
 // arrival ranks kept in `rank`.
 constexpr int GB_THREADS = 1024;
+#ifndef GB_UNROLL_
+#define GB_UNROLL_ 4
+#endif
+constexpr int GB_UNROLL = GB_UNROLL_;
 
 __global__ void __launch_bounds__(GB_THREADS) gridBuild(const uint32_t* __restrict__ off, const float* __restrict__ y,
                                                         const float* __restrict__ z, int nb, const GridDesc* __restrict__ desc,
@@ -100,12 +104,25 @@ __global__ void __launch_bounds__(GB_THREADS) gridBuild(const uint32_t* __restri
   __syncthreads();
   const uint32_t lo = g.lo, hi = g.lo + g.n;
   bool bad = false;
-  for (uint32_t i = lo + tid; i < hi; i += GB_THREADS) {
-    const float yy = y[i], zz = z[i];
-    bad = bad || !(finitef(yy) && finitef(zz));
-    const int cell = cellCoord(zz, g.z0, g.inv_e, g.nz) * g.ny + cellCoord(yy, g.y0, g.inv_e, g.ny);
-    const uint32_t r = atomicAdd(hist + cell, 1u);
-    if (!in_smem) rank[i] = r;
+  // four clusters per thread and trip: eight independent loads in flight before the first atomic (two CTAs of 1024
+  // threads per SM then keep 64 KB on the way, what the HBM latency asks for)
+  for (uint32_t i0 = lo + tid; i0 < hi; i0 += GB_UNROLL * GB_THREADS) {
+    float yy[GB_UNROLL], zz[GB_UNROLL];
+#pragma unroll
+    for (int u = 0; u < GB_UNROLL; ++u) {
+      const uint32_t i = i0 + u * GB_THREADS;
+      yy[u] = i < hi ? y[i] : 0.0f; zz[u] = i < hi ? z[i] : 0.0f;
+    }
+#pragma unroll
+    for (int u = 0; u < GB_UNROLL; ++u) {
+      const uint32_t i = i0 + u * GB_THREADS;
+      if (i < hi) {
+        bad = bad || !(finitef(yy[u]) && finitef(zz[u]));
+        const int cell = cellCoord(zz[u], g.z0, g.inv_e, g.nz) * g.ny + cellCoord(yy[u], g.y0, g.inv_e, g.ny);
+        const uint32_t r = atomicAdd(hist + cell, 1u);
+        if (!in_smem) rank[i] = r;
+      }
+    }
   }
   if (validate && bad) cnt[CNT_ERROR] = -6;
   __syncthreads();
@@ -120,12 +137,23 @@ __global__ void __launch_bounds__(GB_THREADS) gridBuild(const uint32_t* __restri
   __syncthreads();
   if (in_smem)
     for (uint32_t c = tid; c < nc; c += GB_THREADS) table[c] = hist[c];
-  for (uint32_t i = lo + tid; i < hi; i += GB_THREADS) {
-    const float yy = y[i], zz = z[i];
-    const int cell = cellCoord(zz, g.z0, g.inv_e, g.nz) * g.ny + cellCoord(yy, g.y0, g.inv_e, g.ny);
-    const uint32_t pos = in_smem ? atomicAdd(hist + cell, 1u) : hist[cell] + rank[i];
-    syz[pos] = make_float2(yy, zz);
-    s2o[pos] = i;
+  for (uint32_t i0 = lo + tid; i0 < hi; i0 += GB_UNROLL * GB_THREADS) {
+    float yy[GB_UNROLL], zz[GB_UNROLL];
+#pragma unroll
+    for (int u = 0; u < GB_UNROLL; ++u) {
+      const uint32_t i = i0 + u * GB_THREADS;
+      yy[u] = i < hi ? y[i] : 0.0f; zz[u] = i < hi ? z[i] : 0.0f;
+    }
+#pragma unroll
+    for (int u = 0; u < GB_UNROLL; ++u) {
+      const uint32_t i = i0 + u * GB_THREADS;
+      if (i < hi) {
+        const int cell = cellCoord(zz[u], g.z0, g.inv_e, g.nz) * g.ny + cellCoord(yy[u], g.y0, g.inv_e, g.ny);
+        const uint32_t pos = in_smem ? atomicAdd(hist + cell, 1u) : hist[cell] + rank[i];
+        syz[pos] = make_float2(yy[u], zz[u]);
+        s2o[pos] = i;
+      }
+    }
   }
 }
 

@@ -40,7 +40,7 @@ class tpcParams(ctypes.Structure):
                 ("merge_back_rows", c_int32), ("merge_chi2_max", c_float), ("tube_radius", c_float),
                 ("inv_pt_protect", c_float), ("charge_trunc_bits", c_int32), ("leg_min_sinphi", c_float),
                 ("leg_chi2_max", c_float), ("leg_max_sectors", c_int32), ("leg_max_row_diff", c_int32),
-                ("leg_max_centre_dist", c_float), ("pos_bits", c_int32)]
+                ("leg_max_centre_dist", c_float), ("pos_bits", c_int32), ("tube_chi2_max", c_float)]
 
 
 class tpcClusters(ctypes.Structure):

@@ -49,6 +49,8 @@ def test_flags_parity_dead_rows_lattice_ties_and_other_cuts():
     _both(ev2, tube_radius=1.25)
     _both(ev, tube_radius=3.0, inv_pt_protect=2.0, clusters_per_cell=0.3)
     _both(ev, tube_radius=0.0)
+    _both(ev, tube_chi2_max=25.0)                       # R49: the chi2 criterion on top of the fixed tube
+    _both(ev2, tube_chi2_max=9.0, tube_radius=2.0)
 
 
 def test_flags_on_an_event_without_tracks():

@@ -55,6 +55,7 @@ def test_merged_tracks_parity_dead_rows_and_other_cuts():
     _both(ev)
     _both(ev, leg_chi2_max=400.0, leg_max_centre_dist=30.0, merge_chi2_max=200.0, merge_max_row_gap=80)
     _both(ev, flags=False)
+    _both(ev, tube_chi2_max=25.0)                       # chi2 tube together with the leg labels
 
 
 def test_merged_outputs_need_the_merger_and_the_leg_pairs():
