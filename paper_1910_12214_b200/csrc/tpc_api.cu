@@ -48,6 +48,7 @@ struct Workspace {
   SeedRec* work_list;        // long seeds, in the order the constructor takes them
   TurnRec* turn_list;        // [capT] constructUp -> constructDown<0>
   uint4* down_list;          // [capT][DOWNREC_WORDS / 4] constructDown<0> -> constructDown<1>
+  uint32_t* gap_idx;         // [capT] work-list indices of the seeds with a gap row in their span
   TrackletStore tl;
   unsigned long long *tsel, *tscan;
   int32_t *kept_first, *kept_last;
@@ -91,7 +92,7 @@ struct tpcHandle {
   int profiling = 0;
   int launches = 0;
   int gb_smem_cells = 24 * 1024;      // cells of a bucket whose histogram gridBuild keeps in shared memory (96 KB: two CTAs per SM)
-  int tc_grid[3] = {148, 148, 148};   // persistent grids of the three constructor passes: SMs x resident blocks
+  int tc_grid[4] = {148, 148, 148, 148};   // persistent grids of the constructor passes: SMs x resident blocks
   bool pending = false;
   int64_t last_n = 0;
   double cells_per_bucket_bound = 0;   // sum over buckets of the n-independent part of the cell bound
@@ -161,6 +162,7 @@ Workspace layout(const tpcHandle* h, int64_t N, int64_t capT, char* base) {
   w.work_list = (SeedRec*)take(sizeof(SeedRec) * (size_t)Tn);
   w.turn_list = (TurnRec*)take(sizeof(TurnRec) * (size_t)Tn);
   w.down_list = (uint4*)take(4 * (size_t)DOWNREC_WORDS * (size_t)Tn);
+  w.gap_idx = (uint32_t*)take(4 * (size_t)Tn);
   w.tl.capT = capT;
   w.tl.n_rows = R;
   w.tl.status = (int32_t*)take(4 * (size_t)Tn);
@@ -297,8 +299,9 @@ int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cud
   {
     int sms = 148;
     cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, cuda_device);
-    const void* pass[3] = {(const void*)constructUp, (const void*)constructDown<0>, (const void*)constructDown<1>};
-    for (int i = 0; i < 3; ++i) {
+    const void* pass[4] = {(const void*)constructUp, (const void*)constructDown<0, 0>, (const void*)constructDown<1, 0>,
+                           (const void*)constructDown<0, 1>};
+    for (int i = 0; i < 4; ++i) {
       int per_sm = 1;
       if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, pass[i], TC_THREADS, 0) != cudaSuccess || per_sm < 1) per_sm = 1;
       h->tc_grid[i] = sms * per_sm;
@@ -438,10 +441,13 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
                                                               w.tl, cnt); ++L;
     constructUp<<<(unsigned)std::min<int64_t>(blocks, h->tc_grid[0]), TC_THREADS, 0, st>>>(
         P, T, w.desc, w.cell_start, w.syz, w.s2o, w.cup, w.work_list, w.turn_list, w.tl, cnt); ++L;
-    constructDown<0><<<(unsigned)std::min<int64_t>(blocks, h->tc_grid[1]), TC_THREADS, 0, st>>>(
-        P, T, w.desc, w.cell_start, w.syz, w.s2o, w.turn_list, w.down_list, w.tl, cnt); ++L;
-    constructDown<1><<<(unsigned)std::min<int64_t>(blocks, h->tc_grid[2]), TC_THREADS, 0, st>>>(
-        P, T, w.desc, w.cell_start, w.syz, w.s2o, w.turn_list, w.down_list, w.tl, cnt); ++L;
+    gapListBuild<<<(unsigned)ceilDiv(capT, 1024), 1024, 0, st>>>(w.turn_list, w.gap_idx, cnt); ++L;
+    constructDown<0, 0><<<(unsigned)std::min<int64_t>(blocks, h->tc_grid[1]), TC_THREADS, 0, st>>>(
+        P, T, w.desc, w.cell_start, w.syz, w.s2o, w.turn_list, w.gap_idx, w.down_list, w.tl, cnt); ++L;
+    constructDown<0, 1><<<(unsigned)std::min<int64_t>(blocks, h->tc_grid[3]), TC_THREADS, 0, st>>>(
+        P, T, w.desc, w.cell_start, w.syz, w.s2o, w.turn_list, w.gap_idx, w.down_list, w.tl, cnt); ++L;
+    constructDown<1, 0><<<(unsigned)std::min<int64_t>(blocks, h->tc_grid[2]), TC_THREADS, 0, st>>>(
+        P, T, w.desc, w.cell_start, w.syz, w.s2o, w.turn_list, w.gap_idx, w.down_list, w.tl, cnt); ++L;
   }
   stage(4);
   // optional per-stage export of the tracklets: before the selector, which compacts the row-hit slices in place

@@ -45,7 +45,9 @@ enum Counter {
   CNT_INF = 9,          // a count larger than any array: "scan everything" for the device-counted scan kernels
   CNT_WORK2 = 10,       // work counters of the two down-pass kernels of the constructor
   CNT_WORK3 = 11,
-  CNT_COUNT = 12
+  CNT_WORK4 = 12,
+  CNT_N_GAP = 13,       // seeds whose span has a gap row (the gap instance of the span pass)
+  CNT_COUNT = 14
 };
 
 // Tracklet SoA in the workspace (capT = capacity in tracklets).

@@ -289,15 +289,22 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
     __syncthreads();
     // ---- per-cluster reduction over its own items, full key (Dev, orig u, orig d) ----
     if (now) {
+      // branch-free: the minimum over the cluster's own u's; an exact tie with the running minimum, between two u's or
+      // inside the D loop of the winning u, only raises `tied` (the cluster is then redone by neighbourSlow, R6)
+      float bst = __int_as_float(0x7f800000);
+      int ba = 0;
+      uint32_t bcode = 0;
       for (int a = 0; a < nU; ++a) {
         const float dev = it_dev[base * NF_UB + a];
-        if (!have || dev <= best) {
-          const uint32_t dcode = it_d[base * NF_UB + a];
-          tied = tied || (dcode & 0x8000u) != 0u;
-          const uint32_t u = kU0 + ul[a * NF_THREADS + tid], d = kD0 + (dcode & 0x7fffu);
-          if (pairBetter(have, dev, best, u, d, bu, bd, s2o)) { have = true; best = dev; bu = u; bd = d; }
-        }
+        const uint32_t dcode = it_d[base * NF_UB + a];
+        tied = tied || dev == bst || (dev < bst && (dcode & 0x8000u) != 0u);
+        const bool better = dev < bst;
+        ba = better ? a : ba;
+        bcode = better ? dcode : bcode;
+        bst = better ? dev : bst;
       }
+      have = true; best = bst;                      // nU >= 1 here, and every dev is finite
+      bu = kU0 + ul[ba * NF_THREADS + tid]; bd = kD0 + (bcode & 0x7fffu);
       pending = false;
     }
     __syncthreads();                                // the item arrays are rewritten in the next round

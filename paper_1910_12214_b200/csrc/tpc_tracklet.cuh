@@ -231,8 +231,9 @@ struct TurnRec {           // state of a seed at the turn (O4 step 4)
   uint32_t t;              // tracklet id; REC_NONE = the seed ended in the chain fit
   int32_t last_c;          // the hit on the top row
   float y, z, s, tt, q;    // parameters at plane row_x[rx]
-  uint32_t rows;           // r0 | top row << 8 | rx << 16
+  uint32_t rows;           // r0 | top row << 8 | rx << 16 | TURN_HAS_GAP
 };
+constexpr uint32_t TURN_HAS_GAP = 1u << 24;     // some live row inside (r0, top) has no hit: the span pass searches there
 static_assert(sizeof(TurnRec) == 32, "TurnRec is two 16-byte words");
 
 // state of a seed after the Update on its start row r0, going down: t, rows (r0 | top << 8), nhits, pad, then
@@ -308,6 +309,9 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MB_UP) constructUp(
   int r0 = 0, rn = 0, lastw = 0, nhits = 0, miss = 0;
   int32_t c_cur = -1;             // hit of the coming step if known (link), else -1 = search
   int32_t last_c = -1;            // last recorded hit (the hit on row lastw)
+  // a live row without a hit (a miss, or a refused Update) that a later hit closes in is a gap row of the span: the span
+  // pass must search there.  Seeds without one go to the search-free span kernel.
+  bool open_miss = false, has_gap = false;
 
   for (;;) {
     if (phase == -1) {            // ---- fetch and initialise the next seed (O4 step 1) ----
@@ -335,6 +339,7 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MB_UP) constructUp(
         rowhit[r0] = (int32_t)h0;
         last_c = (int32_t)h0;
         nhits = 1; s_rc[tid] = (int16_t)r0; lastw = r0; miss = 0;
+        open_miss = false; has_gap = false;
         phase = 0;
       }
     }
@@ -369,6 +374,7 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MB_UP) constructUp(
     bool turn = false;
     const int rb = rn;                               // the row of this step
     if (okp) { rowhit[rb] = oku ? c : -1; s_rc[tid] = (int16_t)rb; }    // rows beyond the final first/last row are never read
+    if (okp) { has_gap = has_gap || (oku && open_miss); open_miss = open_miss || !oku; }
     if (phase == 0) {
       if (oku) {
         lastw = rb; last_c = c; ++nhits;
@@ -404,7 +410,8 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MB_UP) constructUp(
       uint4* q = reinterpret_cast<uint4*>(turn_list + s_j[tid]);
       q[0] = make_uint4(s_t[tid], (uint32_t)last_c, __float_as_uint(S.y), __float_as_uint(S.z));
       q[1] = make_uint4(__float_as_uint(S.s), __float_as_uint(S.t), __float_as_uint(S.q),
-                        (uint32_t)r0 | ((uint32_t)lastw << 8) | ((uint32_t)(uint16_t)s_rc[tid] << 16));
+                        (uint32_t)r0 | ((uint32_t)lastw << 8) | (((uint32_t)(uint16_t)s_rc[tid] & 0xffu) << 16) |
+                            (has_gap ? TURN_HAS_GAP : 0u));
       phase = -1;
     } else if (phase >= 0) {      // dead rows stepped over (R23) hold no hit
       const int lo = min(rb, rn), hi = max(rb, rn);
@@ -414,12 +421,36 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MB_UP) constructUp(
   }
 }
 
+// The seeds whose span has a gap row, as a dense list of work-list indices in ascending order inside every block of 1024
+// (the blocks append their runs with one atomic each): the gap instance of the span pass takes its seeds from it.
+// The order matters: seeds that are neighbours in the work list are neighbours in the detector, and the passes live on
+// the L2 hits of their grid and cluster gathers (a list in completion order cost the last pass 24 GB of DRAM reads
+// instead of 9 GB).
+__global__ void __launch_bounds__(1024) gapListBuild(const TurnRec* __restrict__ turn_list, uint32_t* __restrict__ gap_idx,
+                                                     int64_t* __restrict__ cnt) {
+  __shared__ uint32_t sm[33];
+  __shared__ uint32_t s_base;
+  if (cnt[CNT_ERROR] != 0) return;
+  const int64_t nW = cnt[CNT_N_LONG];
+  const int64_t j = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if ((int64_t)blockIdx.x * blockDim.x >= nW) return;
+  const bool gap = j < nW && turn_list[j].t != REC_NONE && (turn_list[j].rows & TURN_HAS_GAP) != 0u;
+  uint32_t total;
+  const uint32_t pre = blockExclusiveScan(gap ? 1u : 0u, sm, &total);
+  if (threadIdx.x == 0) s_base = total ? (uint32_t)atomicAdd((unsigned long long*)(cnt + CNT_N_GAP), (unsigned long long)total) : 0u;
+  __syncthreads();
+  if (gap) gap_idx[s_base + pre] = (uint32_t)j;
+}
+
 // ---- passes 2 and 3: the down pass (O4 steps 4-6), over the span (EXT = 0) and below the start row (EXT = 1) -----------
-template <int EXT>
+// GAP (span pass only): 1 = the seeds whose span has gap rows (taken from gap_idx), with the Search code; 0 = the others
+// (the whole list, skipping the seeds of the other kind), without it.  In one kernel the whole warp issued the search code
+// on nearly every step for the 1.5 lanes that stood on a gap row: 20 % of the span pass's instructions.
+template <int EXT, int GAP>
 __global__ void __launch_bounds__(TC_THREADS, EXT ? TC_MB_EXT : TC_MB_SPAN) constructDown(
     DevParams P, RowTables T, const GridDesc* __restrict__ desc, const uint32_t* __restrict__ cell_start,
     const float2* __restrict__ syz, const uint32_t* __restrict__ s2o, const TurnRec* __restrict__ turn_list,
-    uint4* __restrict__ down_list, TrackletStore out, int64_t* __restrict__ cnt) {
+    const uint32_t* __restrict__ gap_idx, uint4* __restrict__ down_list, TrackletStore out, int64_t* __restrict__ cnt) {
   __shared__ RowSmem rs;
   __shared__ float snap[22][TC_THREADS];     // state after the last Update (O4 step 5)
   __shared__ volatile uint32_t s_t[TC_THREADS];
@@ -430,8 +461,8 @@ __global__ void __launch_bounds__(TC_THREADS, EXT ? TC_MB_EXT : TC_MB_SPAN) cons
   const int R = P.n_rows;
   const int tid = threadIdx.x;
   rowSmemFill(rs, T, R);
-  const int64_t nW = cnt[CNT_N_LONG];
-  unsigned long long* work = (unsigned long long*)(cnt + (EXT ? CNT_WORK3 : CNT_WORK2));
+  const int64_t nW = cnt[(!EXT && GAP) ? CNT_N_GAP : CNT_N_LONG];
+  unsigned long long* work = (unsigned long long*)(cnt + (EXT ? CNT_WORK3 : GAP ? CNT_WORK4 : CNT_WORK2));
 
   KFState S;
   int phase = -1;                 // -1 wants a seed, -2 no seeds left, 2 down pass
@@ -445,16 +476,20 @@ __global__ void __launch_bounds__(TC_THREADS, EXT ? TC_MB_EXT : TC_MB_SPAN) cons
 
   for (;;) {
     while (phase == -1) {         // ---- fetch the next seed that is still alive ----
-      const int64_t j = (int64_t)atomicAdd(work, 1ull);
+      int64_t j = (int64_t)atomicAdd(work, 1ull);
       if (j >= nW) { phase = -2; break; }
       if (!EXT) {
+        if (GAP) j = (int64_t)__ldg(gap_idx + j);
         const uint4* rp = reinterpret_cast<const uint4*>(turn_list + j);
         const uint4 a = __ldg(rp), b = __ldg(rp + 1);
-        if (a.x == REC_NONE) { down_list[j * (DOWNREC_WORDS / 4)].x = REC_NONE; continue; }
+        if (!GAP) {
+          if (a.x == REC_NONE) { down_list[j * (DOWNREC_WORDS / 4)].x = REC_NONE; continue; }
+          if ((b.w & TURN_HAS_GAP) != 0u) continue;                     // the gap instance's seed
+        }
         const uint32_t t = a.x;
         s_t[tid] = t; s_j[tid] = (uint32_t)j;
         r0 = (int)(b.w & 0xffu);
-        const int rtop = (int)((b.w >> 8) & 0xffu), rx = (int)(b.w >> 16);
+        const int rtop = (int)((b.w >> 8) & 0xffu), rx = (int)((b.w >> 16) & 0xffu);
         s_rtop[tid] = (int16_t)rtop;
         s_bsec[tid] = out.sector[t] * R;
         rowhit = out.rowhit + (int64_t)t * R;
@@ -501,20 +536,23 @@ __global__ void __launch_bounds__(TC_THREADS, EXT ? TC_MB_EXT : TC_MB_SPAN) cons
     const bool act = phase >= 0;
     float ym = 0.0f, zm = 0.0f;
     float2 mk = make_float2(0.0f, 0.0f);
-    const GridDesc G = desc[act ? s_bsec[tid] + rn : 0];
+    constexpr bool SEARCH = EXT || GAP;
+    const GridDesc G = desc[(SEARCH && act) ? s_bsec[tid] + rn : 0];
     if (!EXT && act && c_cur >= 0) mk = __ldg(syz + c_cur);
     SearchPre sp;
-    // span pass: 4 % of the steps are gap rows (the up pass found nothing there) and need a Search; 1.5 lanes of a warp at
-    // a time, so the whole warp issues the search code on nearly every step.  A lean out-of-line search with plain loops
-    // was tried (4.8e9 instead of 5.9e9 warp instructions) and is slower (a4 26.5 ms against 25.7 ms): its dependent
-    // loads cost the other lanes four memory latencies where the prefetching form below costs one.
-    const bool want_search = act && (EXT || c_cur < 0);
+    // (A lean out-of-line search with plain loops for the gap rows was tried instead of the two span instances: fewer
+    // instructions but slower, its dependent loads cost the other lanes four memory latencies where the prefetching form costs one.)
+    const bool want_search = SEARCH && act && (EXT || c_cur < 0);
     const bool okp = act && kfPropagate(S, rs.sx[act ? rn : 0], P, [&](float y1, float z1, float c00, float c11) {
-      if (want_search) searchBegin(sp, y1, z1, c00, c11, G, cell_start, P);
+      if (SEARCH && want_search) searchBegin(sp, y1, z1, c00, c11, G, cell_start, P);
     });
     int32_t c = EXT ? -1 : c_cur;
     const bool known = !EXT && okp && c >= 0;
-    if (okp && c < 0) c = searchFinish(sp, syz, s2o, ym, zm);
+    if (SEARCH) {
+      if (okp && c < 0) c = searchFinish(sp, syz, s2o, ym, zm);
+    } else if (okp && c < 0) {
+      cnt[CNT_ERROR] = -9;          // cannot happen: constructUp flags every seed with a gap row in its span
+    }
     if (!EXT && c_cur >= 0) { ym = mk.x; zm = mk.y; }
     bool oku = false;
     if (okp && c >= 0) oku = kfUpdate(S, ym, zm, P);
