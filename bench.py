@@ -37,12 +37,15 @@ ALU_SMS = 148
 # `ncu --set full` capture named in "file".  They are cited constants (a number taken under a profiler is never a bench
 # value); every other configuration or seed reports "traffic": null.
 NCU_CAPTURE = {
-    (4, 5): {"file": "profiles/r1m_full_capture.md",
-             "a4_constructor": {"kernel": "trackletConstructor", "warp_inst": 2.2849e10, "dram_bytes": 13136154000},
-             "a2_neighbours": {"kernel": "neighbourFinder", "warp_inst": 1.1833e10, "dram_bytes": 1605503999}},
+    (4, 5): {"file": "profiles/r2a_full_capture.md",
+             "a4_constructor": {"kernel": "constructUp + constructDown<0,0> + constructDown<0,1> + constructDown<1,0>",
+                                "warp_inst": 1.8740e10, "dram_bytes": 22006616000},
+             "a2_neighbours": {"kernel": "neighbourFinder", "warp_inst": 1.1509e10, "dram_bytes": 1605245000}},
 }
-STAGE_KERNEL = {"a1_grid": "gridCount+gridScatter", "a2_neighbours": "neighbourFinder", "a3_cleaner_start": "cleanLinks",
-                "a4_constructor": "trackletConstructor", "a5_selector": "selectClaim+selectCount+selectEmit"}
+STAGE_KERNEL = {"a1_grid": "gridBuild", "a2_neighbours": "neighbourFinder", "a3_cleaner_start": "cleanLinks",
+                "a4_constructor": "constructUp + constructDown<0,0> + constructDown<0,1> + constructDown<1,0> (the passes of the "
+                                  "tracklet constructor: one step body, launched back to back)",
+                "a5_selector": "selectClaim+selectCount+selectEmit"}
 
 # fp32 operations of one Propagate, Update, Search and of one cluster inside a road, and of one window candidate and one
 # (u, d) pair of the neighbour finder, as DESIGN.md section 3 writes them (adds, multiplies, divisions, square roots each
@@ -459,6 +462,36 @@ def run_ours(args, rank, world, local_rank):
         roofline["issue"] = {"achieved": round(issued, 2), "peak": round(issue_peak, 1), "unit": "Gwarp-inst/s",
                              "frac": round(issued / issue_peak, 5), "counts_from": cap["file"],
                              "peak_source": f"{ALU_SMS} SMs x 4 schedulers x {sm_mhz:.0f} MHz"}
+    # the other arithmetic stage, in the same terms (a2 when the constructor dominates, and the other way round)
+    other = "a2_neighbours" if dom == "a4_constructor" else "a4_constructor" if dom == "a2_neighbours" else None
+    roofline_second = None
+    if other is not None:
+        o_ms = stages[other]["ms"]
+        o_ncu = cap.get(other) if cap else None
+        if other == "a2_neighbours" and o2_per_cluster is not None:
+            o_unit = sum(a * b for a, b in zip(o2_per_cluster, O2_FLOPS))
+            o_flops, o_name = N * o_unit, "flops_per_cluster"
+        elif other == "a4_constructor" and o4_per_hit is not None:
+            o_unit = sum(a * b for a, b in zip(o4_per_hit, O4_FLOPS))
+            o_flops, o_name = H * o_unit, "flops_per_tracklet_hit"
+        else:
+            o_flops = None
+        roofline_second = {"bound": "alu", "kernel": STAGE_KERNEL[other], "unit": "TFLOP/s", "peak": round(alu_peak, 2),
+                           "launch_ms": round(o_ms, 4), "share_of_step": round(o_ms / max(float(stage[6]), 1e-9), 4),
+                           "traffic": o_ncu["dram_bytes"] if o_ncu else None, "traffic_from": cap["file"] if o_ncu else None,
+                           "alg_bytes": int(alg[other]),
+                           "alg_frac_of_hbm_peak": round(alg[other] / (o_ms * 1e-3) / 1e9 / peak, 5) if o_ms > 0 else None}
+        if o_flops is not None and o_ms > 0:
+            o_ach = o_flops / (o_ms * 1e-3) / 1e12
+            roofline_second.update({"achieved": round(o_ach, 3), "frac": round(o_ach / alu_peak, 5), "alg_flops": int(o_flops),
+                                    o_name: round(o_unit, 1), "counts_from": "this run's cpu_baseline oracle leg"})
+        else:
+            roofline_second.update({"achieved": None, "frac": None, "alg_flops": None})
+        if o_ncu and o_ms > 0:
+            o_iss = o_ncu["warp_inst"] / (o_ms * 1e-3) / 1e9
+            roofline_second["issue"] = {"achieved": round(o_iss, 2), "peak": round(ALU_SMS * 4 * sm_mhz * 1e6 / 1e9, 1),
+                                        "unit": "Gwarp-inst/s", "frac": round(o_iss / (ALU_SMS * 4 * sm_mhz * 1e6 / 1e9), 5),
+                                        "counts_from": cap["file"]}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
             "ms_per_step": ms_step, "ms_per_step_min": ms_min, "ms_per_step_mean": ms_mean,
             "timing": "K steps back to back on one stream, one CUDA event between steps; value on the median step, max over ranks",
@@ -472,7 +505,7 @@ def run_ours(args, rank, world, local_rank):
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
                     "ms_per_step": ms_e2e, "steps": e2e_steps, "how": "tpcSubmitHost/tpcCollectHost, 2 slots, pinned host buffers"},
             "gpu_launches": int(st.kernel_launches) * K,
-            "clocks": clocks, "roofline": roofline, "stages": stages, "cpu_baseline": cpu}
+            "clocks": clocks, "roofline": roofline, "roofline_second": roofline_second, "stages": stages, "cpu_baseline": cpu}
     if refit_ms is not None:
         ncl = int(st.n_track_clusters)
         rb = 2 * 12 * ncl + 2 * 88 * int(st.n_tracks)       # per pass: index 4 + y,z 8 per cluster; two 88-byte states out
