@@ -123,6 +123,13 @@ int cudaFail(tpcHandle* h, cudaError_t e, const char* what) {
   if (h) snprintf(h->cuda_msg, sizeof(h->cuda_msg), "%s: %s", what, cudaGetErrorString(e));
   return TPC_ERR_CUDA;
 }
+// after every kernel launch of tpcRun: count it, and name the kernel if the launch itself was refused
+#define TPC_LAUNCHED(name)                                                     \
+  do {                                                                         \
+    ++L;                                                                       \
+    const cudaError_t e_ = cudaPeekAtLastError();                              \
+    if (e_ != cudaSuccess) { cudaGetLastError(); return cudaFail(h, e_, "launch of " name); } \
+  } while (0)
 #define TPC_CUDA(h, call)                                   \
   do {                                                      \
     cudaError_t e_ = (call);                                \
@@ -405,20 +412,20 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   stage(0);
   TPC_CUDA(h, cudaMemsetAsync(cnt, 0, 8 * (CNT_COUNT + 1), st)); ++L;
   // ---- a1 grid ----------------------------------------------------------------------------------
-  gridSetup<<<1, 1024, 0, st>>>(in->row_offset, N, P, h->d_row_x, w.desc, w.chunk_base, NF_THREADS, cnt, cc); ++L;
+  gridSetup<<<1, 1024, 0, st>>>(in->row_offset, N, P, h->d_row_x, w.desc, w.chunk_base, NF_THREADS, cnt, cc); TPC_LAUNCHED("gridSetup");
   if (N > 0) {
     gridBuild<<<(unsigned)nb, GB_THREADS, 4 * (size_t)h->gb_smem_cells, st>>>(in->row_offset, in->y, in->z, nb, w.desc, w.cell_start,
                                                                               w.rank, w.syz, w.s2o, cnt, h->params.validate_input,
-                                                                              (uint32_t)h->gb_smem_cells); ++L;
+                                                                              (uint32_t)h->gb_smem_cells); TPC_LAUNCHED("gridBuild");
   }
   stage(1);
   // ---- a2 neighbour finder ------------------------------------------------------------------------
   if (N > 0) {
     // one CTA per chunk of NF_THREADS clusters of one bucket; the exact CTA count is on the device (chunk_base[nb])
     const int64_t max_chunks = ceilDiv(N, NF_THREADS) + nb;
-    chunkFill<<<(unsigned)ceilDiv(max_chunks, 256), 256, 0, st>>>(w.chunk_base, nb, max_chunks, w.chunk_bucket, cnt); ++L;
+    chunkFill<<<(unsigned)ceilDiv(max_chunks, 256), 256, 0, st>>>(w.chunk_base, nb, max_chunks, w.chunk_bucket, cnt); TPC_LAUNCHED("chunkFill");
     neighbourFinder<<<(unsigned)max_chunks, NF_THREADS, 0, st>>>(w.chunk_base, w.chunk_bucket, P, T, w.desc, w.cell_start,
-                                                                                    w.syz, w.s2o, w.lup, w.ldn, cnt); ++L;
+                                                                                    w.syz, w.s2o, w.lup, w.ldn, cnt); TPC_LAUNCHED("neighbourFinder");
   }
   stage(2);
   // ---- a3 cleaner + start hits --------------------------------------------------------------------
@@ -426,28 +433,28 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   uint32_t* cpTile = w.tiles32 + ceilDiv(cc + 1, SCAN_TILE) + 1;
   if (N > 0) {
     TPC_CUDA(h, cudaMemsetAsync(w.spos_by_orig, 0xFF, 4 * (size_t)N, st)); ++L;
-    cleanLinks<<<gN256, 256, 0, st>>>(N, w.lup, w.ldn, w.s2o, w.cup, w.cdn, w.spos_by_orig, cnt); ++L;
-    startCount<<<(unsigned)cpTiles, CP_THREADS, 0, st>>>(N, w.spos_by_orig, cpTile); ++L;
+    cleanLinks<<<gN256, 256, 0, st>>>(N, w.lup, w.ldn, w.s2o, w.cup, w.cdn, w.spos_by_orig, cnt); TPC_LAUNCHED("cleanLinks");
+    startCount<<<(unsigned)cpTiles, CP_THREADS, 0, st>>>(N, w.spos_by_orig, cpTile); TPC_LAUNCHED("startCount");
   }
-  scanArrayInPlace<uint32_t><<<1, 1024, 0, st>>>(cpTile, cpTiles, cnt + CNT_N_START); ++L;
+  scanArrayInPlace<uint32_t><<<1, 1024, 0, st>>>(cpTile, cpTiles, cnt + CNT_N_START); TPC_LAUNCHED("scanArrayInPlace<uint32_t>");
   if (N > 0 && capT > 0) {
-    startWrite<<<(unsigned)cpTiles, CP_THREADS, 0, st>>>(N, w.spos_by_orig, cpTile, capT, w.start_orig, w.start_pos); ++L;
+    startWrite<<<(unsigned)cpTiles, CP_THREADS, 0, st>>>(N, w.spos_by_orig, cpTile, capT, w.start_orig, w.start_pos); TPC_LAUNCHED("startWrite");
   }
   stage(3);
   // ---- a4 tracklet constructor --------------------------------------------------------------------
   if (N > 0 && capT > 0) {
     const int64_t blocks = ceilDiv(capT, TC_THREADS);
     seedPrepare<<<(unsigned)ceilDiv(capT, 128), 128, 0, st>>>(in->row_offset, P, T, w.syz, w.cup, w.start_pos, w.work_list,
-                                                              w.tl, cnt); ++L;
+                                                              w.tl, cnt); TPC_LAUNCHED("seedPrepare");
     constructUp<<<(unsigned)std::min<int64_t>(blocks, h->tc_grid[0]), TC_THREADS, 0, st>>>(
-        P, T, w.desc, w.cell_start, w.syz, w.s2o, w.cup, w.work_list, w.turn_list, w.tl, cnt); ++L;
-    gapListBuild<<<(unsigned)ceilDiv(capT, 1024), 1024, 0, st>>>(w.turn_list, w.gap_idx, cnt); ++L;
+        P, T, w.desc, w.cell_start, w.syz, w.s2o, w.cup, w.work_list, w.turn_list, w.tl, cnt); TPC_LAUNCHED("constructUp");
+    gapListBuild<<<(unsigned)ceilDiv(capT, 1024), 1024, 0, st>>>(w.turn_list, w.gap_idx, cnt); TPC_LAUNCHED("gapListBuild");
     constructDown<0, 0><<<(unsigned)std::min<int64_t>(blocks, h->tc_grid[1]), TC_THREADS, 0, st>>>(
-        P, T, w.desc, w.cell_start, w.syz, w.s2o, w.turn_list, w.gap_idx, w.down_list, w.tl, cnt); ++L;
+        P, T, w.desc, w.cell_start, w.syz, w.s2o, w.turn_list, w.gap_idx, w.down_list, w.tl, cnt); TPC_LAUNCHED("constructDown<0, 0>");
     constructDown<0, 1><<<(unsigned)std::min<int64_t>(blocks, h->tc_grid[3]), TC_THREADS, 0, st>>>(
-        P, T, w.desc, w.cell_start, w.syz, w.s2o, w.turn_list, w.gap_idx, w.down_list, w.tl, cnt); ++L;
+        P, T, w.desc, w.cell_start, w.syz, w.s2o, w.turn_list, w.gap_idx, w.down_list, w.tl, cnt); TPC_LAUNCHED("constructDown<0, 1>");
     constructDown<1, 0><<<(unsigned)std::min<int64_t>(blocks, h->tc_grid[2]), TC_THREADS, 0, st>>>(
-        P, T, w.desc, w.cell_start, w.syz, w.s2o, w.turn_list, w.gap_idx, w.down_list, w.tl, cnt); ++L;
+        P, T, w.desc, w.cell_start, w.syz, w.s2o, w.turn_list, w.gap_idx, w.down_list, w.tl, cnt); TPC_LAUNCHED("constructDown<1, 0>");
   }
   stage(4);
   // optional per-stage export of the tracklets: before the selector, which compacts the row-hit slices in place
@@ -455,7 +462,7 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
                             out->tl_rowhit || out->tl_x || out->tl_par || out->tl_cov || out->tl_chi2)) {
     const TrackletOut xo{out->start_hits, out->tl_status, out->tl_nhits, out->tl_first_row, out->tl_last_row,
                          out->tl_rowhit, out->tl_x, out->tl_par, out->tl_cov, out->tl_chi2};
-    exportTracklets<<<(unsigned)ceilDiv(capT, 128), 128, 0, st>>>(w.tl, w.start_orig, w.s2o, P.n_rows, xo, cnt); ++L;
+    exportTracklets<<<(unsigned)ceilDiv(capT, 128), 128, 0, st>>>(w.tl, w.start_orig, w.s2o, P.n_rows, xo, cnt); TPC_LAUNCHED("exportTracklets");
   }
   // ---- a5 selector ----------------------------------------------------------------------------------
   const TrackOut to{out->cap_tracks, out->cap_track_clusters, out->trk_tracklet, out->trk_sector, out->trk_first_row,
@@ -465,21 +472,21 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   if (N > 0 && capT > 0) {
     const unsigned gT = (unsigned)ceilDiv(capT, 128);
     TPC_CUDA(h, cudaMemsetAsync(w.owner_key, 0, 8 * (size_t)N, st)); ++L;
-    selectClaim<<<gT, 128, 0, st>>>(w.tl, w.owner_key, wide, cnt); ++L;
+    selectClaim<<<gT, 128, 0, st>>>(w.tl, w.owner_key, wide, cnt); TPC_LAUNCHED("selectClaim");
     if (wide) {
       TPC_CUDA(h, cudaMemsetAsync(w.owner_id, 0xFF, 4 * (size_t)N, st)); ++L;
-      selectClaimId<<<gT, 128, 0, st>>>(w.tl, w.owner_key, w.owner_id, cnt); ++L;
+      selectClaimId<<<gT, 128, 0, st>>>(w.tl, w.owner_key, w.owner_id, cnt); TPC_LAUNCHED("selectClaimId");
     }
     selectCount<<<gT, 128, 0, st>>>(w.tl, w.owner_key, w.owner_id, wide, P.min_track_hits, w.tsel, w.kept_first,
-                                    w.kept_last, cnt); ++L;
+                                    w.kept_last, cnt); TPC_LAUNCHED("selectCount");
     const unsigned tiles = (unsigned)ceilDiv(capT, SCAN_TILE);
-    scanTileSums<unsigned long long><<<tiles, SCAN_THREADS, 0, st>>>(w.tsel, cnt + CNT_N_START, capT, w.tiles64); ++L;
-    scanTileOffsets<unsigned long long><<<1, 1024, 0, st>>>(w.tiles64, cnt + CNT_N_START, capT, sel_total); ++L;
-    scanApply<unsigned long long><<<tiles, SCAN_THREADS, 0, st>>>(w.tsel, w.tscan, cnt + CNT_N_START, capT, w.tiles64); ++L;
+    scanTileSums<unsigned long long><<<tiles, SCAN_THREADS, 0, st>>>(w.tsel, cnt + CNT_N_START, capT, w.tiles64); TPC_LAUNCHED("scanTileSums<unsigned long long>");
+    scanTileOffsets<unsigned long long><<<1, 1024, 0, st>>>(w.tiles64, cnt + CNT_N_START, capT, sel_total); TPC_LAUNCHED("scanTileOffsets<unsigned long long>");
+    scanApply<unsigned long long><<<tiles, SCAN_THREADS, 0, st>>>(w.tsel, w.tscan, cnt + CNT_N_START, capT, w.tiles64); TPC_LAUNCHED("scanApply<unsigned long long>");
     selectEmit<<<gT, 128, 0, st>>>(w.tl, w.owner_key, w.owner_id, wide, w.tsel, w.tscan, w.kept_first, w.kept_last,
-                                   w.s2o, to, cnt); ++L;
+                                   w.s2o, to, cnt); TPC_LAUNCHED("selectEmit");
   }
-  finalize<<<1, 32, 0, st>>>(sel_total, to, capT, cnt); ++L;
+  finalize<<<1, 32, 0, st>>>(sel_total, to, capT, cnt); TPC_LAUNCHED("finalize");
   stage(5);
   // ---- a6 optional refit of the selected tracks (O6) ------------------------------------------------
   stage(7);
@@ -490,10 +497,10 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
     const size_t rfb = (size_t)(nk / RF_CHUNK + 1) * RF_BINS + 1;
     TPC_CUDA(h, cudaMemsetAsync(w.rf_hist, 0, 4 * rfb, st)); ++L;
     TPC_CUDA(h, cudaMemsetAsync(w.rf_fill, 0, 4 * rfb, st)); ++L;
-    refitCount<<<(unsigned)ceilDiv(nk, 256), 256, 0, st>>>(to, w.rf_hist, cnt); ++L;
-    scanArrayInPlace<uint32_t><<<1, 1024, 0, st>>>(w.rf_hist, (int64_t)rfb, nullptr); ++L;
-    refitFill<<<(unsigned)ceilDiv(nk, 256), 256, 0, st>>>(to, w.rf_hist, w.rf_fill, w.rf_order, cnt); ++L;
-    refitTracks<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(in->row_offset, w.rf_order, in->y, in->z, P, T, to, rf, cnt); ++L;
+    refitCount<<<(unsigned)ceilDiv(nk, 256), 256, 0, st>>>(to, w.rf_hist, cnt); TPC_LAUNCHED("refitCount");
+    scanArrayInPlace<uint32_t><<<1, 1024, 0, st>>>(w.rf_hist, (int64_t)rfb, nullptr); TPC_LAUNCHED("scanArrayInPlace<uint32_t>");
+    refitFill<<<(unsigned)ceilDiv(nk, 256), 256, 0, st>>>(to, w.rf_hist, w.rf_fill, w.rf_order, cnt); TPC_LAUNCHED("refitFill");
+    refitTracks<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(in->row_offset, w.rf_order, in->y, in->z, P, T, to, rf, cnt); TPC_LAUNCHED("refitTracks");
   }
   stage(8);
   // ---- a7 optional links between track segments (O7) -------------------------------------------------
@@ -513,22 +520,22 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
     TPC_CUDA(h, cudaMemsetAsync(w.mg_ostart, 0, 4 * mgb, st)); ++L;
     TPC_CUDA(h, cudaMemsetAsync(w.mg_ofill, 0, 4 * mgb, st)); ++L;
     TPC_CUDA(h, cudaMemsetAsync(w.mg_maxv, 0, 4 * (size_t)nb, st)); ++L;
-    mergeCount<<<gK, 256, 0, st>>>(mi, mo, P, T, w.mg_start, w.mg_ostart, w.mg_maxv, w.mg_best_b, w.mg_key_a, cnt); ++L;
+    mergeCount<<<gK, 256, 0, st>>>(mi, mo, P, T, w.mg_start, w.mg_ostart, w.mg_maxv, w.mg_best_b, w.mg_key_a, cnt); TPC_LAUNCHED("mergeCount");
     {   // exclusive scan of the bucket counts; the closing sentinel lands on the last (spare) entry
       const int64_t nscan = (int64_t)mgb - 1;
       const unsigned tiles = (unsigned)ceilDiv(nscan, SCAN_TILE);
-      scanTileSums<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.mg_start, cnt + CNT_INF, nscan, w.mg_tiles); ++L;
-      scanTileOffsets<uint32_t><<<1, 1024, 0, st>>>(w.mg_tiles, cnt + CNT_INF, nscan, nullptr); ++L;
-      scanApply<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.mg_start, w.mg_start, cnt + CNT_INF, nscan, w.mg_tiles); ++L;
-      scanTileSums<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.mg_ostart, cnt + CNT_INF, nscan, w.mg_tiles); ++L;
-      scanTileOffsets<uint32_t><<<1, 1024, 0, st>>>(w.mg_tiles, cnt + CNT_INF, nscan, nullptr); ++L;
-      scanApply<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.mg_ostart, w.mg_ostart, cnt + CNT_INF, nscan, w.mg_tiles); ++L;
+      scanTileSums<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.mg_start, cnt + CNT_INF, nscan, w.mg_tiles); TPC_LAUNCHED("scanTileSums<uint32_t>");
+      scanTileOffsets<uint32_t><<<1, 1024, 0, st>>>(w.mg_tiles, cnt + CNT_INF, nscan, nullptr); TPC_LAUNCHED("scanTileOffsets<uint32_t>");
+      scanApply<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.mg_start, w.mg_start, cnt + CNT_INF, nscan, w.mg_tiles); TPC_LAUNCHED("scanApply<uint32_t>");
+      scanTileSums<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.mg_ostart, cnt + CNT_INF, nscan, w.mg_tiles); TPC_LAUNCHED("scanTileSums<uint32_t>");
+      scanTileOffsets<uint32_t><<<1, 1024, 0, st>>>(w.mg_tiles, cnt + CNT_INF, nscan, nullptr); TPC_LAUNCHED("scanTileOffsets<uint32_t>");
+      scanApply<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.mg_ostart, w.mg_ostart, cnt + CNT_INF, nscan, w.mg_tiles); TPC_LAUNCHED("scanApply<uint32_t>");
     }
-    mergeFill<<<gK, 256, 0, st>>>(mi, P, T, w.mg_start, w.mg_fill, w.mg_list, w.mg_rec, w.mg_ostart, w.mg_ofill, w.mg_order, cnt); ++L;
+    mergeFill<<<gK, 256, 0, st>>>(mi, P, T, w.mg_start, w.mg_fill, w.mg_list, w.mg_rec, w.mg_ostart, w.mg_ofill, w.mg_order, cnt); TPC_LAUNCHED("mergeFill");
     mergeMatch<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(mi, P, T, mp, w.mg_start, w.mg_maxv, w.mg_list, w.mg_rec, w.mg_ostart, w.mg_order, w.mg_best_b,
-                                                         w.mg_chi_b, w.mg_key_a, cnt); ++L;
-    mergeLink<<<gK, 256, 0, st>>>(mi, mo, w.mg_best_b, w.mg_chi_b, w.mg_key_a, cnt); ++L;
-    mergeHead<<<gK, 256, 0, st>>>(mi, mo, cnt); ++L;
+                                                         w.mg_chi_b, w.mg_key_a, cnt); TPC_LAUNCHED("mergeMatch");
+    mergeLink<<<gK, 256, 0, st>>>(mi, mo, w.mg_best_b, w.mg_chi_b, w.mg_key_a, cnt); TPC_LAUNCHED("mergeLink");
+    mergeHead<<<gK, 256, 0, st>>>(mi, mo, cnt); TPC_LAUNCHED("mergeHead");
   }
   stage(10);
   // ---- a10 optional pairs of looper legs (O10) -------------------------------------------------------
@@ -560,18 +567,18 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
     TPC_CUDA(h, cudaMemsetAsync(w.lg_start, 0, 4 * lgb, st)); ++L;
     TPC_CUDA(h, cudaMemsetAsync(w.lg_fill, 0, 4 * lgb, st)); ++L;
     TPC_CUDA(h, cudaMemsetAsync(w.lg_maxv, 0, 4 * (size_t)nb * 2, st)); ++L;
-    legCount<<<gK, 256, 0, st>>>(li, lo, P, lp, w.lg_start, w.lg_maxv, w.lg_best, cnt); ++L;
+    legCount<<<gK, 256, 0, st>>>(li, lo, P, lp, w.lg_start, w.lg_maxv, w.lg_best, cnt); TPC_LAUNCHED("legCount");
     {   // exclusive scan of the bucket counts; the closing sentinel lands on the last (spare) entry
       const int64_t nscan = (int64_t)lgb - 1;
       const unsigned tiles = (unsigned)ceilDiv(nscan, SCAN_TILE);
-      scanTileSums<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.lg_start, cnt + CNT_INF, nscan, w.lg_tiles); ++L;
-      scanTileOffsets<uint32_t><<<1, 1024, 0, st>>>(w.lg_tiles, cnt + CNT_INF, nscan, nullptr); ++L;
-      scanApply<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.lg_start, w.lg_start, cnt + CNT_INF, nscan, w.lg_tiles); ++L;
+      scanTileSums<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.lg_start, cnt + CNT_INF, nscan, w.lg_tiles); TPC_LAUNCHED("scanTileSums<uint32_t>");
+      scanTileOffsets<uint32_t><<<1, 1024, 0, st>>>(w.lg_tiles, cnt + CNT_INF, nscan, nullptr); TPC_LAUNCHED("scanTileOffsets<uint32_t>");
+      scanApply<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(w.lg_start, w.lg_start, cnt + CNT_INF, nscan, w.lg_tiles); TPC_LAUNCHED("scanApply<uint32_t>");
     }
-    legFill<<<gK, 256, 0, st>>>(li, P, lp, w.lg_start, w.lg_fill, w.lg_list, w.lg_rec, cnt); ++L;
+    legFill<<<gK, 256, 0, st>>>(li, P, lp, w.lg_start, w.lg_fill, w.lg_list, w.lg_rec, cnt); TPC_LAUNCHED("legFill");
     legMatch<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(li, P, lp, w.lg_start, w.lg_maxv, w.lg_list, w.lg_rec, w.lg_best,
-                                                         w.lg_chi, cnt); ++L;
-    legLink<<<gK, 256, 0, st>>>(li, lo, w.lg_best, w.lg_chi, cnt); ++L;
+                                                         w.lg_chi, cnt); TPC_LAUNCHED("legMatch");
+    legLink<<<gK, 256, 0, st>>>(li, lo, w.lg_best, w.lg_chi, cnt); TPC_LAUNCHED("legLink");
   }
   stage(16);
   // ---- a11 optional merged tracks and leg labels (O12) ------------------------------------------------
@@ -581,13 +588,13 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
     const MergedIn mi{out->cap_tracks, out->trk_mg_next, out->trk_mg_head, out->trk_leg_partner, out->trk_cl_offset,
                       out->trk_cl_index, in->z};
     const MergedOut mo{out->trk_mt_id, out->trk_mt_rank, out->mt_cl_offset, out->mt_cl_index};
-    mergedLabel<<<(unsigned)ceilDiv(nk + 1, 256), 256, 0, st>>>(mi, mo, cnt); ++L;
+    mergedLabel<<<(unsigned)ceilDiv(nk + 1, 256), 256, 0, st>>>(mi, mo, cnt); TPC_LAUNCHED("mergedLabel");
     // exclusive scan of the lengths in place: n_tracks entries and the closing one (the scan writes out[n] itself)
     const unsigned tiles = (unsigned)ceilDiv(nk + 1, SCAN_TILE);
-    scanTileSums<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(out->mt_cl_offset, cnt + CNT_N_TRACKS, nk, w.mt_tiles); ++L;
-    scanTileOffsets<uint32_t><<<1, 1024, 0, st>>>(w.mt_tiles, cnt + CNT_N_TRACKS, nk, nullptr); ++L;
-    scanApply<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(out->mt_cl_offset, out->mt_cl_offset, cnt + CNT_N_TRACKS, nk, w.mt_tiles); ++L;
-    mergedFill<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(mi, mo, out->cap_track_clusters, cnt); ++L;
+    scanTileSums<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(out->mt_cl_offset, cnt + CNT_N_TRACKS, nk, w.mt_tiles); TPC_LAUNCHED("scanTileSums<uint32_t>");
+    scanTileOffsets<uint32_t><<<1, 1024, 0, st>>>(w.mt_tiles, cnt + CNT_N_TRACKS, nk, nullptr); TPC_LAUNCHED("scanTileOffsets<uint32_t>");
+    scanApply<uint32_t><<<tiles, SCAN_THREADS, 0, st>>>(out->mt_cl_offset, out->mt_cl_offset, cnt + CNT_N_TRACKS, nk, w.mt_tiles); TPC_LAUNCHED("scanApply<uint32_t>");
+    mergedFill<<<(unsigned)ceilDiv(nk, 128), 128, 0, st>>>(mi, mo, out->cap_track_clusters, cnt); TPC_LAUNCHED("mergedFill");
   }
   stage(18);
   // ---- a8 optional per-cluster flags (O8) ------------------------------------------------------------
@@ -611,7 +618,7 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
       const int64_t n_ent = std::min<int64_t>(out->cap_track_clusters, N);
       if (walk_yz) { TPC_CUDA(h, cudaMemsetAsync(walk_yz, 0xFF, 8 * (size_t)n_ent, st)); ++L; }
       flagAttach<<<(unsigned)ceilDiv(std::min<int64_t>(out->cap_track_clusters, N), 256), 256, 0, st>>>(out->trk_cl_index,
-                                                                                                       out->cl_flags, cnt); ++L;
+                                                                                                       out->cl_flags, cnt); TPC_LAUNCHED("flagAttach");
       const unsigned gB = (unsigned)ceilDiv(nk * FLAG_GROUP, 128);
       const int32_t* rk = n_mt == 4 ? out->trk_mt_rank : nullptr;
       if (h->params.tube_chi2_max > 0.0f)
@@ -621,28 +628,28 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
       else
         flagBid<0><<<gB, 128, 0, st>>>(fi, in->row_offset, P, T, h->params.tube_radius, 0.0f, h->params.inv_pt_protect, w.desc,
                                        w.cell_start, w.syz, w.s2o, w.fl_key, w.fl_prot, rk, walk_yz, cnt);
-      ++L;
+      TPC_LAUNCHED("flagBid");
       if (walk_yz) {
         flagResiduals<<<(unsigned)ceilDiv(n_ent, 256), 256, 0, st>>>(out->trk_cl_index, walk_yz, in->y, in->z, out->cl_res_y,
-                                                                    out->cl_res_z, out->cl_res_code, h->params.pos_bits, cnt); ++L;
+                                                                    out->cl_res_z, out->cl_res_code, h->params.pos_bits, cnt); TPC_LAUNCHED("flagResiduals");
       }
     }
-    flagFinish<<<gN256, 256, 0, st>>>(N, w.fl_key, w.fl_prot, out->cl_flags, out->cl_owner, cnt); ++L;
+    flagFinish<<<gN256, 256, 0, st>>>(N, w.fl_key, w.fl_prot, out->cl_flags, out->cl_owner, cnt); TPC_LAUNCHED("flagFinish");
   }
   stage(12);
   // ---- a9 optional dynamic-precision charge code (O9) ------------------------------------------------
   stage(13);
   if (out->cl_qcode && N > 0) {
-    packCharge<<<(unsigned)ceilDiv(ceilDiv(N, 8), 256), 256, 0, st>>>(N, in->q, h->params.charge_trunc_bits, out->cl_qcode); ++L;
+    packCharge<<<(unsigned)ceilDiv(ceilDiv(N, 8), 256), 256, 0, st>>>(N, in->q, h->params.charge_trunc_bits, out->cl_qcode); TPC_LAUNCHED("packCharge");
   }
   if (out->cl_pos_code && N > 0) {    // O11 of the absolute positions
-    packPositions<<<(unsigned)ceilDiv(ceilDiv(N, 4), 256), 256, 0, st>>>(N, in->y, in->z, h->params.pos_bits, out->cl_pos_code); ++L;
+    packPositions<<<(unsigned)ceilDiv(ceilDiv(N, 4), 256), 256, 0, st>>>(N, in->y, in->z, h->params.pos_bits, out->cl_pos_code); TPC_LAUNCHED("packPositions");
   }
   stage(14);
   // ---- optional per-stage exports -----------------------------------------------------------------
   if (N > 0 && (out->link_up_raw || out->link_dn_raw || out->link_up || out->link_dn)) {
     exportLinks<<<gN256, 256, 0, st>>>(N, w.s2o, w.lup, w.ldn, w.cup, w.cdn, out->link_up_raw, out->link_dn_raw,
-                                       out->link_up, out->link_dn, cnt); ++L;
+                                       out->link_up, out->link_dn, cnt); TPC_LAUNCHED("exportLinks");
   }
   stage(6);
   TPC_CUDA(h, cudaGetLastError());

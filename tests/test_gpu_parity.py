@@ -285,3 +285,27 @@ def test_shared_denominator_division_is_bit_identical_to_the_ieee_division():
         tested += n
     trk.close()
     assert tested == 3 * 48 * (1 << 26)
+
+
+def test_parity_on_the_hand_built_events_of_the_control_rule_pins():
+    """The hand-built events of tests/test_oracle_search.py (gaps of max_row_gap and one more, dead rows inside a gap, gaps
+    inside the span, two candidates in a road, chains and tracklets around the length thresholds, four crossing lines that
+    share single clusters, a Propagate refused in the down pass and in the up pass): the oracle's answers there are worked
+    out by hand, and the CUDA path must give the same, bit for bit -- these are the cases that drive the gap instance of the
+    span pass, the rows-below-the-snapshot rule and the single-pass ownership of the selector."""
+    from tests import test_oracle_search as S
+    cases = [(S._gap_event(4), {}), (S._gap_event(5), {}), (S._gap_event(5), {"max_row_gap": 5}), (S._gap_event(5, dead=(43,)), {}),
+             (S._crossing_event(10)[0], {}), (S._crossing_event(9)[0], {}),
+             (S._circle_event(0.502), {"max_sinphi": 0.5}), (S._circle_event(0.502), {"max_sinphi": 0.51}),
+             (S._circle_event(0.502), {"max_sinphi": 0.53}), (S._circle_event(0.30, k=0.015, r_hi=45), {"max_sinphi": 0.5})]
+    b = S.Builder()
+    b.line(list(range(10, 31)) + list(range(34, 51)) + list(range(54, 71)), y0=2.0, z0=-30.0, ty=-0.25, tz=0.4)
+    cases.append((b.event(), {}))
+    for n in (4, 5, 9, 10, 11):
+        b = S.Builder()
+        b.line(list(range(10, 10 + n)), y0=1.0, z0=5.0, ty=0.1, tz=0.5)
+        cases.append((b.event(), {}))
+        cases.append((b.event(), {"min_chain_hits": 4, "min_tracklet_hits": 5, "min_track_hits": 5}))
+    for ev, par in cases:
+        rep, res, o = _run_both(ev, **par)
+        assert rep["exact"] and rep["tl_exact"], (par, rep)
