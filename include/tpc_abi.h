@@ -236,7 +236,10 @@ int tpcRunHost(tpcHandle* h, int64_t n_clusters, const uint32_t* row_offset, con
  * buffers (inputs and the arrays of `out_host`, pinned for real overlap) must stay valid and untouched until the
  * collect.  The counts are not known at submit time: up to min(capacity of the handle's device buffers, capacity of
  * out_host) entries are copied back and tpcRunStatus says how many are valid.  status TPC_ERR_CAPACITY = a capacity
- * was too small (first events of a stream): run that event again with tpcRunHost, which grows the buffers. */
+ * was too small (first events of a stream): run that event again with tpcRunHost, which grows the buffers.  The device
+ * pools of a slot grow with cudaFree / cudaMalloc, which synchronise the device: a submit that has to grow its pools (the
+ * first events of a stream, or an event larger than any before) waits for the other slot's event; steady state allocates
+ * nothing. */
 int tpcSubmitHost(tpcHandle* h, int slot, int64_t n_clusters, const uint32_t* row_offset, const float* y, const float* z,
                   const tpcTracks* out_host);
 int tpcCollectHost(tpcHandle* h, int slot, tpcRunStatus* status);
