@@ -135,8 +135,10 @@ __global__ void __launch_bounds__(GB_THREADS) gridBuild(const uint32_t* __restri
   uint32_t pre = lo + blockExclusiveScan(sum, sm, &total);        // global sorted position of the run's first cluster
   for (uint32_t c = c0; c < c1; ++c) { const uint32_t v = hist[c]; hist[c] = pre; pre += v; }
   __syncthreads();
-  if (in_smem)
+  if (in_smem) {
     for (uint32_t c = tid; c < nc; c += GB_THREADS) table[c] = hist[c];
+    __syncthreads();      // the cursors below overwrite the starts: every start must be copied out first
+  }
   for (uint32_t i0 = lo + tid; i0 < hi; i0 += GB_UNROLL * GB_THREADS) {
     float yy[GB_UNROLL], zz[GB_UNROLL];
 #pragma unroll

@@ -152,7 +152,7 @@ struct SeedRec {
   uint32_t t, h0;        // tracklet id, sorted position of the start hit
   int32_t h1;            // first link
   uint32_t b0r0;         // bucket << 8 | row of the start hit
-  float y0, z0, y1, z1;  // coordinates of h0 and h1
+  float y0, z0, s0, t0;  // O4 step 1: coordinates of h0, and sin phi and dz/ds of the first link (computed by seedPrepare)
 };
 
 // One thread per start hit, before the constructor: bucket of the seed, length of its link chain.  Chains shorter
@@ -178,9 +178,12 @@ __global__ void __launch_bounds__(128) seedPrepare(const uint32_t* __restrict__ 
     const unsigned long long j = atomicAdd((unsigned long long*)(cnt + CNT_N_LONG), 1ull);
     const int32_t h1 = cup[h0];
     const float2 a = syz[h0], c = syz[h1];
+    // O4 step 1 here, at full lanes, instead of at the 5 lanes of the constructor's seed fetch
+    const float dx = T.row_x[T.up_row[r0]] - T.row_x[r0], dy = c.x - a.x, dz = c.y - a.y;
+    const float L = sqrtf(dx * dx + dy * dy);
     uint4* q = reinterpret_cast<uint4*>(work + j);
     q[0] = make_uint4((uint32_t)t, h0, (uint32_t)h1, ((uint32_t)b0 << 8) | (uint32_t)r0);
-    q[1] = make_uint4(__float_as_uint(a.x), __float_as_uint(a.y), __float_as_uint(c.x), __float_as_uint(c.y));
+    q[1] = make_uint4(__float_as_uint(a.x), __float_as_uint(a.y), __float_as_uint(dy / L), __float_as_uint(dz / L));
     return;
   }
   // short chain: O4 steps 1-2 on its len-1 links; the result is always status 0, nhits = hits fitted
@@ -331,9 +334,7 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MB_UP) constructUp(
         rn = rs.sup[r0];
         const float y0 = __uint_as_float(b.x), z0 = __uint_as_float(b.y);
         S.x = rs.sx[r0]; S.y = y0; S.z = z0;
-        const float dx = rs.sx[rn] - rs.sx[r0], dy = __uint_as_float(b.z) - y0, dz = __uint_as_float(b.w) - z0;
-        const float L = sqrtf(dx * dx + dy * dy);
-        S.s = dy / L; S.t = dz / L; S.q = 0.0f;
+        S.s = __uint_as_float(b.z); S.t = __uint_as_float(b.w); S.q = 0.0f;
         kfSetDiag(S, P.err2_y, P.err2_z, P);
         S.chi2 = 0.0f;
         rowhit[r0] = (int32_t)h0;
