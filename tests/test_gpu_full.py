@@ -238,3 +238,29 @@ def test_full_size_leg_pairs_sampled_against_the_oracle_pair_function():
             assert lp[k] == -1 and lc[k] == 0
     assert n_pairs >= 150
     print("config 4: leg ends", len(ends), "paired", len(linked), "legs_ms", res.status.legs_ms)
+
+
+def test_full_size_optional_stages_are_deterministic():
+    """Config 3 at full size with every optional stage on (refit, merger, leg pairs, merged tracks, flags, residual and
+    position codes), twice: identical bytes.  The bids of the flags and the merger go through atomics; their outcome must not
+    depend on the order in which they arrive."""
+    import hashlib
+    from paper_1910_12214_b200 import tpc
+    ev = datagen.make_event(3)
+    trk = tpc.TpcTracker.from_event(ev)
+    off, y, z = trk.upload(ev)
+    st = trk.run(off, y, z).status
+    caps = dict(cap_tracklets=int(st.n_start_hits * 1.05) + 1024, cap_tracks=int(st.n_tracks * 1.05) + 1024,
+                cap_track_clusters=int(st.n_track_clusters * 1.05) + 1024)
+    digests = []
+    for _ in range(2):
+        res = trk.run(off, y, z, merged=True, flags=True, pos=True, **caps)
+        assert res.status.status == 0
+        hsh = hashlib.sha256()
+        for k in ("trk_cl_index", "trk_rf_par_in", "trk_rf_cov_out", "trk_mg_next", "trk_mg_chi2", "trk_leg_partner", "trk_leg_chi2",
+                  "trk_mt_id", "trk_mt_rank", "mt_cl_offset", "mt_cl_index", "cl_flags", "cl_owner", "cl_res_y", "cl_res_code",
+                  "cl_pos_code"):
+            hsh.update(res.trk[k].contiguous().cpu().numpy().tobytes())
+        digests.append(hsh.hexdigest())
+    trk.close()
+    assert digests[0] == digests[1]
