@@ -309,3 +309,18 @@ def test_parity_on_the_hand_built_events_of_the_control_rule_pins():
     for ev, par in cases:
         rep, res, o = _run_both(ev, **par)
         assert rep["exact"] and rep["tl_exact"], (par, rep)
+
+
+def test_parity_when_a_bucket_has_more_cells_than_the_shared_histogram_holds():
+    """a1 `gridBuild` keeps the cell histogram of a bucket in shared memory up to 24 576 cells; with `clusters_per_cell` =
+    0.003 the ~117 clusters of a config-0 bucket get ~39 000 cells, and the same passes run on the bucket's slice of the
+    global cell table with the arrival ranks in `rank`.  The grid never decides a result (R3): everything stays bit-exact."""
+    ev = datagen.make_event(0)
+    trk = _tracker(ev, clusters_per_cell=0.003)
+    off, y, z = trk.upload(ev)
+    res = trk.run(off, y, z, stages=True)
+    assert res.status.status == 0
+    assert res.status.n_cells > 24576 * 100                  # most of the 152 buckets are above the shared-memory limit
+    rep = compare(res.numpy(), orc.run(ev), ev.n_rows)
+    trk.close()
+    assert rep["exact"] and rep["tl_exact"]
