@@ -278,6 +278,8 @@ int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cud
   std::vector<int16_t> up(R, -1), dn(R, -1);
   std::vector<uint8_t> dead(R, 0);
   for (int r = 0; r < R; ++r) dead[r] = (g->row_dead && g->row_dead[r]) ? 1 : 0;
+  P.any_dead = 0;
+  for (int r = 0; r < R; ++r) P.any_dead |= dead[r];
   for (int r = 0; r < R; ++r) {
     if (dead[r]) continue;
     for (int k = 1; k <= 2; ++k) if (r + k < R && !dead[r + k]) { up[r] = (int16_t)(r + k); break; }

@@ -29,6 +29,7 @@ struct DevParams {
   float tan_half_sector, z_min, z_max;
   int32_t n_rows, n_sectors, n_buckets;
   int32_t max_cells_per_bucket;
+  int32_t any_dead;             // 1 if some row is dead (then the constructor fills the rows it steps over with -1)
 };
 
 // Device status / counter block (int64 slots), copied to pinned host memory at the end of a run.

@@ -414,7 +414,7 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MB_UP) constructUp(
                         (uint32_t)r0 | ((uint32_t)lastw << 8) | (((uint32_t)(uint16_t)s_rc[tid] & 0xffu) << 16) |
                             (has_gap ? TURN_HAS_GAP : 0u));
       phase = -1;
-    } else if (phase >= 0) {      // dead rows stepped over (R23) hold no hit
+    } else if (phase >= 0 && P.any_dead) {      // dead rows stepped over (R23) hold no hit
       const int lo = min(rb, rn), hi = max(rb, rn);
       if (hi - lo > 1)
         for (int g = lo + 1; g < hi; ++g) rowhit[g] = -1;
@@ -451,7 +451,8 @@ template <int EXT, int GAP>
 __global__ void __launch_bounds__(TC_THREADS, EXT ? TC_MB_EXT : TC_MB_SPAN) constructDown(
     DevParams P, RowTables T, const GridDesc* __restrict__ desc, const uint32_t* __restrict__ cell_start,
     const float2* __restrict__ syz, const uint32_t* __restrict__ s2o, const TurnRec* __restrict__ turn_list,
-    const uint32_t* __restrict__ gap_idx, uint4* __restrict__ down_list, TrackletStore out, int64_t* __restrict__ cnt) {
+    const uint32_t* gap_idx, uint4* __restrict__ down_list, TrackletStore out, int64_t* __restrict__ cnt) {
+  uint32_t* gap_idx_out = const_cast<uint32_t*>(gap_idx);       // written by the search-free instance only (refused seeds)
   __shared__ RowSmem rs;
   __shared__ float snap[22][TC_THREADS];     // state after the last Update (O4 step 5)
   __shared__ volatile uint32_t s_t[TC_THREADS];
@@ -480,7 +481,7 @@ __global__ void __launch_bounds__(TC_THREADS, EXT ? TC_MB_EXT : TC_MB_SPAN) cons
       int64_t j = (int64_t)atomicAdd(work, 1ull);
       if (j >= nW) { phase = -2; break; }
       if (!EXT) {
-        if (GAP) j = (int64_t)__ldg(gap_idx + j);
+        if (GAP) j = (int64_t)gap_idx[j];
         const uint4* rp = reinterpret_cast<const uint4*>(turn_list + j);
         const uint4 a = __ldg(rp), b = __ldg(rp + 1);
         if (!GAP) {
@@ -527,7 +528,7 @@ __global__ void __launch_bounds__(TC_THREADS, EXT ? TC_MB_EXT : TC_MB_SPAN) cons
         TC_SNAP_STORE(snap, tid, S);        // the state after the Update on r0 is the snapshot so far
         snap_row = r0; miss = 0; c_cur = -1;
         rn = rs.snd[r0];                    // >= 0: the span pass finishes seeds with nothing below r0 itself
-        for (int g = rn + 1; g < r0; ++g) rowhit[g] = -1;     // dead rows stepped over (R23) hold no hit
+        if (P.any_dead) for (int g = rn + 1; g < r0; ++g) rowhit[g] = -1;     // dead rows stepped over (R23) hold no hit
         phase = 2;
       }
     }
@@ -561,12 +562,16 @@ __global__ void __launch_bounds__(TC_THREADS, EXT ? TC_MB_EXT : TC_MB_SPAN) cons
 
     // ---- bookkeeping ----
     bool end_phase = !okp || (c >= 0 && !oku);       // Propagate or Update refused: the pass ends here
+    const bool refused = end_phase;
     const int rb = rn;
     if (okp && !known) rowhit[rb] = oku ? c : -1;
     if (!end_phase) {
       if (oku) {
         ++nhits; snap_row = rb;
-        TC_SNAP_STORE(snap, tid, S);
+        // the search-free span instance keeps no snapshot: every step of it ends in an Update, so the live state IS the
+        // snapshot; a seed whose Propagate or Update is refused there (rare) is handed to the gap instance, which redoes
+        // its span from the TurnRec with snapshots (the span pass writes no row hit of a seed without gap rows)
+        if (SEARCH) TC_SNAP_STORE(snap, tid, S);
         if (EXT) miss = 0;
       } else if (EXT) {
         if (++miss > P.max_row_gap) end_phase = true;
@@ -592,8 +597,13 @@ __global__ void __launch_bounds__(TC_THREADS, EXT ? TC_MB_EXT : TC_MB_SPAN) cons
       q[6] = make_uint4(__float_as_uint(S.chi2), 0u, 0u, 0u);
       phase = -1;
     } else if (end_phase) {         // O4 step 6: output = last snapshot
-      writeTracklet(out, P, s_t[tid], nhits, snap_row, s_rtop[tid], snap, tid);
-      if (!EXT) down_list[(int64_t)s_j[tid] * (DOWNREC_WORDS / 4)].x = REC_NONE;
+      if (!SEARCH && refused) {
+        gap_idx_out[atomicAdd((unsigned long long*)(cnt + CNT_N_GAP), 1ull)] = s_j[tid];
+      } else {
+        if (!SEARCH) TC_SNAP_STORE(snap, tid, S);     // ended on the Update of r0 with nothing below it
+        writeTracklet(out, P, s_t[tid], nhits, snap_row, s_rtop[tid], snap, tid);
+        if (!EXT) down_list[(int64_t)s_j[tid] * (DOWNREC_WORDS / 4)].x = REC_NONE;
+      }
       phase = -1;
     } else {
       if (!EXT) {                   // pipeline: this step's hit was loaded a step ago; request the one after
@@ -603,7 +613,7 @@ __global__ void __launch_bounds__(TC_THREADS, EXT ? TC_MB_EXT : TC_MB_SPAN) cons
         if (nx_ok) nx_raw = rowhit[r2];
       }
       const int lo = rn, hi = rb;   // dead rows stepped over (R23) hold no hit
-      if (hi - lo > 1)
+      if (P.any_dead && hi - lo > 1)
         for (int g = lo + 1; g < hi; ++g) rowhit[g] = -1;
     }
   }
