@@ -40,7 +40,8 @@ enum {
                                        bounds, required sizes are in tpcRunStatus */
   TPC_ERR_CUDA = -5,                /* a CUDA runtime call failed (tpcErrorString gives the last message) */
   TPC_ERR_NONFINITE_INPUT = -6,     /* validate_input was set and a cluster coordinate is NaN/Inf (R25) */
-  TPC_ERR_OUT_OF_MEMORY = -7        /* host allocation of the handle failed */
+  TPC_ERR_OUT_OF_MEMORY = -7,       /* host allocation of the handle failed */
+  TPC_ERR_NOALLOC_LIMIT = -8        /* tpcStartHitsNoAlloc: n_clusters beyond TPC_NOALLOC_MAX_CLUSTERS (nothing was launched) */
 };
 
 typedef struct tpcHandle tpcHandle;
@@ -252,6 +253,40 @@ const char* tpcLastCudaError(const tpcHandle* h);
  * both forms on the device for n_threads x 48 operand pairs drawn over the whole domain of the shared form (seeded,
  * edge values included) and reports how many were tested and how many bit patterns differ (must be 0).  Synchronous. */
 int tpcSelfTestDivision(tpcHandle* h, int64_t n_threads, uint64_t seed, int64_t* n_tested, int64_t* n_mismatches);
+
+/* ---- the allocation-free entry point (csrc/tpc_noalloc.cu) ---------------------------------------------------------------
+ * For callers that cannot call cudaMalloc (code under CUDA graph capture, tight serving loops, harnesses that forbid
+ * it): the a3 start-hit list (O3, R8) computed with NO workspace argument and no
+ * allocation of any kind.  The scratch of its stream compaction (one count per 2048 clusters) is a static device array
+ * of the library: 33 024 bytes that every GPU which loads libtpcgpu.so holds until the process exits.  That fixes the
+ * largest input: */
+#define TPC_NOALLOC_MAX_CLUSTERS 16777216 /* 2^24; more -> TPC_ERR_NOALLOC_LIMIT */
+
+/* The limit again, for callers that cannot read the macro (ctypes). */
+int64_t tpcNoAllocMaxClusters(void);
+
+/* Looks up the device address of the static scratch on `cuda_device` (once per device; idempotent, thread-safe).
+ * tpcStartHitsNoAlloc does this itself on its first call for a device; call it beforehand where the first call would be
+ * inside a stream capture (the look-up is not a stream operation and may be refused there). */
+int tpcNoAllocSetup(int cuda_device);
+
+/* Enqueues three kernels on `cuda_stream` (a cudaStream_t, NULL = default stream) of `cuda_device` and returns without
+ * synchronising; calls no cudaMalloc / cudaFree / allocating routine.
+ *   link_up, link_dn  DEVICE [n_clusters] cleaned links as global input indices, -1 = none (the tpcTracks.link_up /
+ *                     link_dn outputs of tpcRun); read only; 0 <= n_clusters <= TPC_NOALLOC_MAX_CLUSTERS
+ *   start_hits        DEVICE [cap_start_hits] out: global input indices c with link_dn[c] == -1 and link_up[c] != -1,
+ *                     ascending (= tpcTracks.start_hits); entries beyond cap_start_hits are not written
+ *   n_start_hits      DEVICE [1] out: the number of start hits found (the required cap_start_hits, also when truncated)
+ * Outputs are valid once the stream has drained.  Argument errors (TPC_ERR_INVALID_ARG, TPC_ERR_NOALLOC_LIMIT) and
+ * launch errors (TPC_ERR_CUDA) are returned here; tpcNoAllocLastError gives the text.
+ * ALL calls on a device share the one scratch array: calls that overlap on the GPU (different streams without an
+ * ordering between them, graphs in flight together) race and give wrong lists; calls ordered on the device (one
+ * stream, or events between streams) are safe.  The array keeps the last call's contents; no call relies on them. */
+int tpcStartHitsNoAlloc(int cuda_device, int64_t n_clusters, const int32_t* link_up, const int32_t* link_dn,
+                        uint32_t* start_hits, int64_t cap_start_hits, int64_t* n_start_hits, void* cuda_stream);
+
+/* Text of the last error of the two calls above on this host thread ("" after a success). */
+const char* tpcNoAllocLastError(void);
 
 #ifdef __cplusplus
 }

@@ -32,7 +32,8 @@ def is_stale() -> bool:
 
 
 def build_cuda(force: bool = False, verbose: bool = False, defines=(), out: str | None = None) -> str:
-    """Compile csrc/tpc_api.cu (which includes every kernel header) into libtpcgpu.so.
+    """Compile csrc/tpc_api.cu (which includes every kernel header) and csrc/tpc_noalloc.cu (the allocation-free entry
+    point, a translation unit of its own) into libtpcgpu.so.
 
     ``defines`` / ``out`` build a tuning variant (-DNAME=VALUE ...) under another file name; the product is
     always the default build.
@@ -40,14 +41,15 @@ def build_cuda(force: bool = False, verbose: bool = False, defines=(), out: str 
     if out is not None:
         nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
         subprocess.check_call([nvcc] + NVCC_FLAGS + [f"-D{d}" for d in defines] +
-                              [os.path.join(CSRC, "tpc_api.cu"), "-o", out])
+                              [os.path.join(CSRC, "tpc_api.cu"), os.path.join(CSRC, "tpc_noalloc.cu"), "-o", out])
         return out
     if not force and not is_stale():
         return LIB
     nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
     if not os.path.exists(nvcc):
         raise RuntimeError("nvcc not found: libtpcgpu.so cannot be built (there is no CPU fallback)")
-    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + [os.path.join(CSRC, "tpc_api.cu"), "-o", LIB]
+    cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+          [os.path.join(CSRC, "tpc_api.cu"), os.path.join(CSRC, "tpc_noalloc.cu"), "-o", LIB]
     subprocess.check_call(cmd)
     return LIB
 

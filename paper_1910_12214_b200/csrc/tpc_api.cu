@@ -705,6 +705,7 @@ const char* tpcErrorString(int code) {
     case TPC_ERR_CUDA: return "CUDA runtime error";
     case TPC_ERR_NONFINITE_INPUT: return "non-finite cluster coordinate";
     case TPC_ERR_OUT_OF_MEMORY: return "out of host memory";
+    case TPC_ERR_NOALLOC_LIMIT: return "input larger than the static scratch of the allocation-free entry point (TPC_NOALLOC_MAX_CLUSTERS)";
     default: return "unknown error";
   }
 }

@@ -22,6 +22,7 @@ TPC_ERR_CAPACITY = -4
 TPC_ERR_CUDA = -5
 TPC_ERR_NONFINITE_INPUT = -6
 TPC_ERR_OUT_OF_MEMORY = -7
+TPC_ERR_NOALLOC_LIMIT = -8
 
 
 class tpcGeometry(ctypes.Structure):
@@ -76,7 +77,7 @@ class tpcRunStatus(ctypes.Structure):
 
 ABI_SYMBOLS = ("tpcDefaultParams", "tpcCreate", "tpcDestroy", "tpcWorkspaceBytes", "tpcRun", "tpcGetRunStatus",
                "tpcSetProfiling", "tpcRunHost", "tpcSubmitHost", "tpcCollectHost", "tpcErrorString", "tpcLastCudaError",
-               "tpcSelfTestDivision")
+               "tpcSelfTestDivision", "tpcNoAllocMaxClusters", "tpcNoAllocSetup", "tpcStartHitsNoAlloc", "tpcNoAllocLastError")
 
 _lib = None
 
@@ -115,6 +116,14 @@ def load_library(build_if_stale: bool = True) -> ctypes.CDLL:
     L.tpcLastCudaError.restype = c_char_p
     L.tpcSelfTestDivision.argtypes = [vp, c_int64, ctypes.c_uint64, POINTER(c_int64), POINTER(c_int64)]
     L.tpcSelfTestDivision.restype = c_int
+    L.tpcNoAllocMaxClusters.argtypes = []
+    L.tpcNoAllocMaxClusters.restype = c_int64
+    L.tpcNoAllocSetup.argtypes = [c_int]
+    L.tpcNoAllocSetup.restype = c_int
+    L.tpcStartHitsNoAlloc.argtypes = [c_int, c_int64, vp, vp, vp, c_int64, vp, vp]
+    L.tpcStartHitsNoAlloc.restype = c_int
+    L.tpcNoAllocLastError.argtypes = []
+    L.tpcNoAllocLastError.restype = c_char_p
     _lib = L
     return L
 
@@ -187,6 +196,27 @@ def tpcSelfTestDivision(handle, n_threads: int, seed: int = 1):
 
 
 # ---- convenience wrapper: allocation of device tensors with torch, nothing else ---------------------------
+def tpcNoAllocMaxClusters() -> int:
+    return int(load_library().tpcNoAllocMaxClusters())
+
+
+def tpcNoAllocSetup(cuda_device: int = 0) -> None:
+    L = load_library()
+    rc = L.tpcNoAllocSetup(cuda_device)
+    if rc != TPC_OK:
+        raise TpcError(rc, "tpcNoAllocSetup", L.tpcNoAllocLastError().decode())
+
+
+def tpcStartHitsNoAlloc(cuda_device: int, n_clusters: int, link_up_ptr: int, link_dn_ptr: int, start_hits_ptr: int,
+                        cap_start_hits: int, n_start_hits_ptr: int, cuda_stream: int = 0) -> None:
+    """The allocation-free start-hit list (include/tpc_abi.h): DEVICE pointers as integers; enqueues and returns."""
+    L = load_library()
+    rc = L.tpcStartHitsNoAlloc(cuda_device, n_clusters, link_up_ptr or None, link_dn_ptr or None, start_hits_ptr or None,
+                               cap_start_hits, n_start_hits_ptr or None, cuda_stream or None)
+    if rc != TPC_OK:
+        raise TpcError(rc, "tpcStartHitsNoAlloc", L.tpcNoAllocLastError().decode())
+
+
 @dataclass
 class TrackResult:
     """Device tensors (torch) of one tpcRun, trimmed to the counts of the run status."""
