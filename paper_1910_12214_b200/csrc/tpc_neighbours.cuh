@@ -44,6 +44,10 @@ constexpr int NF_ITEMS = NF_ITEMS_; // items per CTA and round
 #define NF_GUNROLL_ 2
 #endif
 constexpr int NF_GUNROLL = NF_GUNROLL_;
+#ifndef NF_DUNROLL_
+#define NF_DUNROLL_ 4
+#endif
+constexpr int NF_DUNROLL = NF_DUNROLL_;   // unrolling of the D loop of the pair phase
 constexpr int NF_ROWS = 6;         // cell rows of a window whose ranges are staged (more: slow path)
 
 struct RowTables {
@@ -56,6 +60,12 @@ struct RowTables {
 __device__ __forceinline__ void nfCpAsync8(void* smem, const void* gmem) {
   const unsigned sa = (unsigned)__cvta_generic_to_shared(smem);
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;\n" ::"r"(sa), "l"(gmem) : "memory");
+}
+
+// region entry at a byte offset (the window lists hold 8 * index: 16 bits are enough, bit 15 stays free for the tie flag)
+static_assert(NF_REGION * 8 <= 0x8000, "byte offsets of the region must fit 15 bits");
+__device__ __forceinline__ float2 nfAt(const float2* reg, uint32_t byte_off) {
+  return *reinterpret_cast<const float2*>(reinterpret_cast<const char*>(reg) + byte_off);
 }
 
 // lexicographic (Dev, orig(u), orig(d)) "is the new pair better" (R6)
@@ -122,7 +132,9 @@ __device__ __forceinline__ int gatherWindow(const GridDesc& G, const uint32_t* _
     for (uint32_t k = v.x; k < v.y; ++k) {
       const float2 c = reg[k];
       const bool pass = fabsf(c.x - yc) <= wy && fabsf(c.y - zc) <= wz;
-      list[min(n, NF_LIST) * NF_THREADS + tid] = (uint16_t)k;     // row NF_LIST is a spare: no branch needed
+      list[min(n, NF_LIST) * NF_THREADS + tid] = (uint16_t)(k << 3);     // byte offset into the region (the pair loop
+                                                                         // adds it to the base: no multiply there); row
+                                                                         // NF_LIST is a spare: no branch needed
       n += pass ? 1 : 0;
     }
   }
@@ -253,24 +265,34 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
       const int hl = e >> 5, a0 = e & 31;
       const float2 hh = sH[hl];
       const int nu = snU[hl];
-      float tyu[NF_UB], tzu[NF_UB], bdev[NF_UB];
+      // The slopes are kept as (y, z) pairs and subtracted / squared with the packed fp32 instructions of sm_100
+      // (FADD2 / FMUL2: each half is the IEEE round-to-nearest operation, so the result is bit-identical to the
+      // scalar form; one issue slot for two operations).  ptxas contracts a packed mul that feeds a packed add into
+      // FFMA2 even with --fmad=false and explicit .rn (measured), so that pattern is never
+      // written: the differences of two slopes (products) are scalar adds, and only add -> mul and mul -> scalar add
+      // chains are packed (tests/test_build_flags.py checks the SASS of the library for FFMA2).
+      float2 tu[NF_UB];
+      float bdev[NF_UB];
       uint32_t bdi[NF_UB];
       bool tie[NF_UB];
+      const float2 iu2 = make_float2(iu, iu), id2 = make_float2(id, id), nh = make_float2(-hh.x, -hh.y);
 #pragma unroll
       for (int q = 0; q < NF_UB; ++q) {
-        const float2 uu = sU[ul[min(a0 + q, nu - 1) * NF_THREADS + hl]];     // a short last group repeats its last u
-        tyu[q] = (uu.x - hh.x) * iu; tzu[q] = (uu.y - hh.y) * iu;
+        const float2 uu = nfAt(sU, ul[min(a0 + q, nu - 1) * NF_THREADS + hl]);     // a short last group repeats its last u
+        tu[q] = __fmul2_rn(__fadd2_rn(uu, nh), iu2);                         // ((y_u - y_h) * iu, (z_u - z_h) * iu)
         bdev[q] = __int_as_float(0x7f800000); bdi[q] = 0; tie[q] = false;
       }
       const int n = snD[hl];
+#pragma unroll NF_DUNROLL
       for (int j = 0; j < n; ++j) {
-        const uint32_t di = dl[j * NF_THREADS + hl];
-        const float2 dd = sD[di];
-        const float tyd = (hh.x - dd.x) * id, tzd = (hh.y - dd.y) * id;
+        const uint32_t di = dl[j * NF_THREADS + hl];                         // byte offset of d in the region
+        const float2 dd = nfAt(sD, di);
+        const float2 ntd = __fmul2_rn(__fadd2_rn(dd, nh), id2);              // -(tyd, tzd): -((y_h - y_d) * id) exactly
 #pragma unroll
         for (int q = 0; q < NF_UB; ++q) {
-          const float ey = tyu[q] - tyd, ez = tzu[q] - tzd;
-          const float dev = ey * ey + ez * ez;
+          const float2 e = make_float2(tu[q].x + ntd.x, tu[q].y + ntd.y);    // (tyu - tyd, tzu - tzd): scalar, see above
+          const float2 m = __fmul2_rn(e, e);
+          const float dev = m.x + m.y;
           // Window slopes are bounded by area_y/area_z, so dev is finite: +inf is a safe "none yet".  The minimum
           // is tracked with selects (no branch).  An exact tie with the running minimum (duplicated clusters) is
           // only flagged: such a cluster is redone by neighbourSlow with the full key (R6).
@@ -304,7 +326,7 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
         bst = better ? dev : bst;
       }
       have = true; best = bst;                      // nU >= 1 here, and every dev is finite
-      bu = kU0 + ul[ba * NF_THREADS + tid]; bd = kD0 + (bcode & 0x7fffu);
+      bu = kU0 + (ul[ba * NF_THREADS + tid] >> 3); bd = kD0 + ((bcode & 0x7fffu) >> 3);
       pending = false;
     }
     __syncthreads();                                // the item arrays are rewritten in the next round
