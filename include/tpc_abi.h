@@ -48,7 +48,7 @@ typedef struct tpcHandle tpcHandle;
 
 /* Detector description (R1, R2).  All pointers HOST, copied by tpcCreate. */
 typedef struct {
-  int32_t n_sectors;            /* 36 (config 0: 1) */
+  int32_t n_sectors;            /* 36 (config 0: 1); 1 <= n_sectors <= 64 */
   int32_t n_rows;               /* 152; 3 <= n_rows <= 255 */
   const float* row_x;           /* [n_rows] local x of the pad-row planes, cm, strictly increasing */
   const float* row_pitch;       /* [n_rows] pad pitch, cm; carried only (may be NULL) */

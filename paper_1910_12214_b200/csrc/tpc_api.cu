@@ -246,7 +246,7 @@ int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cud
   if (!out || !g || !p || !g->row_x) return TPC_ERR_INVALID_ARG;
   *out = nullptr;
   const int R = g->n_rows, S = g->n_sectors;
-  if (R < 3 || R >= MAX_ROWS || S < 1 || (int64_t)R * S > (1 << 24)) return TPC_ERR_INVALID_ARG;
+  if (R < 3 || R >= MAX_ROWS || S < 1 || S > 64) return TPC_ERR_INVALID_ARG;      // the hand-off records of the constructor carry the sector in 6 bits
   for (int r = 1; r < R; ++r)
     if (!(g->row_x[r] > g->row_x[r - 1])) return TPC_ERR_INVALID_ARG;
   if (!(g->z_max > g->z_min) || !(g->tan_half_sector > 0) || !(g->row_x[0] > 0)) return TPC_ERR_INVALID_ARG;

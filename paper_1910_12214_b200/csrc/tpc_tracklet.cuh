@@ -151,7 +151,7 @@ __device__ __forceinline__ int32_t searchFinish(const SearchPre& sp, const float
 struct SeedRec {
   uint32_t t, h0;        // tracklet id, sorted position of the start hit
   int32_t h1;            // first link
-  uint32_t b0r0;         // bucket << 8 | row of the start hit
+  uint32_t b0r0;         // sector << 22 | bucket << 8 | row of the start hit
   float y0, z0, s0, t0;  // O4 step 1: coordinates of h0, and sin phi and dz/ds of the first link (computed by seedPrepare)
 };
 
@@ -182,7 +182,7 @@ __global__ void __launch_bounds__(128) seedPrepare(const uint32_t* __restrict__ 
     const float dx = T.row_x[T.up_row[r0]] - T.row_x[r0], dy = c.x - a.x, dz = c.y - a.y;
     const float L = sqrtf(dx * dx + dy * dy);
     uint4* q = reinterpret_cast<uint4*>(work + j);
-    q[0] = make_uint4((uint32_t)t, h0, (uint32_t)h1, ((uint32_t)b0 << 8) | (uint32_t)r0);
+    q[0] = make_uint4((uint32_t)t, h0, (uint32_t)h1, ((uint32_t)(b0 / R) << 22) | ((uint32_t)b0 << 8) | (uint32_t)r0);
     q[1] = make_uint4(__float_as_uint(a.x), __float_as_uint(a.y), __float_as_uint(dy / L), __float_as_uint(dz / L));
     return;
   }
@@ -234,9 +234,10 @@ struct TurnRec {           // state of a seed at the turn (O4 step 4)
   uint32_t t;              // tracklet id; REC_NONE = the seed ended in the chain fit
   int32_t last_c;          // the hit on the top row
   float y, z, s, tt, q;    // parameters at plane row_x[rx]
-  uint32_t rows;           // r0 | top row << 8 | rx << 16 | TURN_HAS_GAP
+  uint32_t rows;           // r0 | top row << 8 | rx << 16 | TURN_HAS_GAP | sector << 25
 };
 constexpr uint32_t TURN_HAS_GAP = 1u << 24;     // some live row inside (r0, top) has no hit: the span pass searches there
+constexpr int TURN_SECTOR_SHIFT = 25;           // the sector rides along (< 64): no load of out.sector in the span pass
 static_assert(sizeof(TurnRec) == 32, "TurnRec is two 16-byte words");
 
 // state of a seed after the Update on its start row r0, going down: t, rows (r0 | top << 8), nhits, pad, then
@@ -287,6 +288,53 @@ __device__ __forceinline__ void writeTracklet(const TrackletStore& out, const De
   for (int i = 0; i < 15; ++i) out.cov[i * capT + t] = snap[7 + i][tid];
 }
 
+// Work distribution of the persistent passes.  A lane that has finished its seed needs the next index of the pass's list.
+// Drawn per lane from a global counter, that is an atomic round trip to the L2, then the load of the record, then -- in
+// the down passes, before the records carried the sector -- the load of the tracklet's sector: dependent memory latencies
+// during which the other lanes of the warp stand still (11 % of the stall samples of the passes, profiles/r2d).  With
+// drawIndex a warp draws TC_CHUNK consecutive indices with ONE atomic, keeps the chunk in shared memory and hands its
+// indices out to the lanes that ask (in lane order, by ballot); the records of the chunk are requested into the L2 when
+// the chunk is drawn.  Used by the search-free span instance only (see constructDown).
+#ifndef TC_CHUNK_
+#define TC_CHUNK_ 32
+#endif
+constexpr uint32_t TC_CHUNK = TC_CHUNK_;
+
+__device__ __forceinline__ void prefetchL2(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
+
+// Warp-synchronous (all 32 lanes call it together).  Lanes with `want` get the next indices of the warp's chunk in lane
+// order; returns true and the index in j for those served.  A lane that wants and is not served (the chunk ran out
+// in front of it) asks again: the next call draws a new chunk.  The indices may lie beyond the end of the list (the
+// caller checks); `rec` / `rec_bytes` / `n_rec` describe the record array to prefetch (rec may be NULL).
+__device__ __forceinline__ bool drawIndex(bool want, unsigned long long* __restrict__ work, volatile uint32_t* w_next,
+                                          volatile uint32_t* w_end, const void* rec, uint32_t rec_bytes, int64_t n_rec,
+                                          uint32_t& j) {
+  const unsigned need = __ballot_sync(0xffffffffu, want);
+  const uint32_t lane = threadIdx.x & 31u;
+  uint32_t nxt = *w_next, end = *w_end;
+  if (nxt == end) {                    // uniform over the warp: the chunk is used up (or none drawn yet)
+    uint32_t base = 0;
+    if (lane == 0) base = (uint32_t)atomicAdd(work, (unsigned long long)TC_CHUNK);
+    base = __shfl_sync(0xffffffffu, base, 0);
+    nxt = base; end = base + TC_CHUNK;
+    if (lane == 0) *w_end = end;
+    if (rec) {
+      const int64_t last = min((int64_t)end, n_rec);
+      const char* a = reinterpret_cast<const char*>(rec) + (int64_t)base * rec_bytes;
+      const char* e = reinterpret_cast<const char*>(rec) + last * rec_bytes;
+      for (const char* q = a + lane * 128; q < e; q += 32 * 128) prefetchL2(q);
+    }
+  }
+  const uint32_t avail = end - nxt;
+  const uint32_t rank = __popc(need & ((1u << lane) - 1u));
+  const uint32_t take = min((uint32_t)__popc(need), avail);
+  __syncwarp();                        // every lane has read w_next
+  if (lane == 0) *w_next = nxt + take;
+  __syncwarp();
+  j = nxt + rank;
+  return want && rank < avail;
+}
+
 // ---- pass 1: chain fit (O4 step 2) and up extrapolation (step 3) ---------------------------------------------------
 __global__ void __launch_bounds__(TC_THREADS, TC_MB_UP) constructUp(
     DevParams P, RowTables T, const GridDesc* __restrict__ desc, const uint32_t* __restrict__ cell_start,
@@ -299,6 +347,7 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MB_UP) constructUp(
   __shared__ volatile uint32_t s_j[TC_THREADS];       // index of the seed in the work list
   __shared__ volatile int s_bsec[TC_THREADS];         // first bucket of the seed's sector
   __shared__ volatile int16_t s_rc[TC_THREADS];       // row of the last Propagate
+  __shared__ volatile uint8_t s_sec[TC_THREADS];      // sector of the seed
   if (cnt[CNT_ERROR] != 0) return;
   const int R = P.n_rows;
   const int tid = threadIdx.x;
@@ -329,7 +378,8 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MB_UP) constructUp(
         const uint32_t h0 = a.y;
         c_cur = (int32_t)a.z;
         r0 = (int)(a.w & 0xffu);
-        s_bsec[tid] = (int)(a.w >> 8) - r0;
+        s_bsec[tid] = (int)((a.w >> 8) & 0x3fffu) - r0;
+        s_sec[tid] = (uint8_t)(a.w >> 22);
         rowhit = out.rowhit + (int64_t)t * R;
         rn = rs.sup[r0];
         const float y0 = __uint_as_float(b.x), z0 = __uint_as_float(b.y);
@@ -412,7 +462,7 @@ __global__ void __launch_bounds__(TC_THREADS, TC_MB_UP) constructUp(
       q[0] = make_uint4(s_t[tid], (uint32_t)last_c, __float_as_uint(S.y), __float_as_uint(S.z));
       q[1] = make_uint4(__float_as_uint(S.s), __float_as_uint(S.t), __float_as_uint(S.q),
                         (uint32_t)r0 | ((uint32_t)lastw << 8) | (((uint32_t)(uint16_t)s_rc[tid] & 0xffu) << 16) |
-                            (has_gap ? TURN_HAS_GAP : 0u));
+                            (has_gap ? TURN_HAS_GAP : 0u) | ((uint32_t)s_sec[tid] << TURN_SECTOR_SHIFT));
       phase = -1;
     } else if (phase >= 0 && P.any_dead) {      // dead rows stepped over (R23) hold no hit
       const int lo = min(rb, rn), hi = max(rb, rn);
@@ -459,9 +509,11 @@ __global__ void __launch_bounds__(TC_THREADS, EXT ? TC_MB_EXT : TC_MB_SPAN) cons
   __shared__ volatile uint32_t s_j[TC_THREADS];
   __shared__ volatile int s_bsec[TC_THREADS];
   __shared__ volatile int16_t s_rtop[TC_THREADS];
+  __shared__ volatile uint32_t s_wn[TC_THREADS / 32], s_we[TC_THREADS / 32];      // the warp's chunk of work indices
   if (cnt[CNT_ERROR] != 0) return;
   const int R = P.n_rows;
   const int tid = threadIdx.x;
+  if ((tid & 31) == 0) { s_wn[tid >> 5] = 0; s_we[tid >> 5] = 0; }
   rowSmemFill(rs, T, R);
   const int64_t nW = cnt[(!EXT && GAP) ? CNT_N_GAP : CNT_N_LONG];
   unsigned long long* work = (unsigned long long*)(cnt + (EXT ? CNT_WORK3 : GAP ? CNT_WORK4 : CNT_WORK2));
@@ -477,9 +529,21 @@ __global__ void __launch_bounds__(TC_THREADS, EXT ? TC_MB_EXT : TC_MB_SPAN) cons
   bool nx_ok = false;
 
   for (;;) {
-    while (phase == -1) {         // ---- fetch the next seed that is still alive ----
-      int64_t j = (int64_t)atomicAdd(work, 1ull);
-      if (j >= nW) { phase = -2; break; }
+    // The search-free span instance draws its indices a chunk per warp (see drawIndex); the instances that search keep
+    // the one global counter: with chunks their seeds in flight spread over more rows of the detector and the gathers of
+    // the searches miss the L2 (measured with chunks of 64: L2 hit rate of the pass below r0 67 -> 46 %, DRAM reads
+    // 9.4 -> 27 GB, 10.7 -> 13.0 ms; the up pass 7.8 -> 8.8 ms; even chunks of 4 cost 6 %).
+    constexpr bool CHUNKED = !EXT && !GAP;
+    while (CHUNKED ? __any_sync(0xffffffffu, phase == -1) : phase == -1) {         // ---- fetch the next seed that is still alive ----
+      int64_t j;
+      if (CHUNKED) {
+        uint32_t jw;
+        if (!drawIndex(phase == -1, work, &s_wn[tid >> 5], &s_we[tid >> 5], turn_list, (uint32_t)sizeof(TurnRec), nW, jw)) continue;
+        j = (int64_t)jw;
+      } else {
+        j = (int64_t)atomicAdd(work, 1ull);
+      }
+      if (j >= nW) { phase = -2; if (CHUNKED) continue; else break; }
       if (!EXT) {
         if (GAP) j = (int64_t)gap_idx[j];
         const uint4* rp = reinterpret_cast<const uint4*>(turn_list + j);
@@ -493,7 +557,7 @@ __global__ void __launch_bounds__(TC_THREADS, EXT ? TC_MB_EXT : TC_MB_SPAN) cons
         r0 = (int)(b.w & 0xffu);
         const int rtop = (int)((b.w >> 8) & 0xffu), rx = (int)((b.w >> 16) & 0xffu);
         s_rtop[tid] = (int16_t)rtop;
-        s_bsec[tid] = out.sector[t] * R;
+        s_bsec[tid] = (int)(b.w >> TURN_SECTOR_SHIFT) * R;
         rowhit = out.rowhit + (int64_t)t * R;
         // O4 step 4: diffuse covariance, parameters kept (R17); the down pass starts at the top row
         S.x = rs.sx[rx]; S.y = __uint_as_float(a.z); S.z = __uint_as_float(a.w);
@@ -516,6 +580,7 @@ __global__ void __launch_bounds__(TC_THREADS, EXT ? TC_MB_EXT : TC_MB_SPAN) cons
         r0 = (int)(a.y & 0xffu);
         s_rtop[tid] = (int16_t)((a.y >> 8) & 0xffu);
         nhits = (int)a.z;
+        // (measured: with the sector carried in the DownRec instead of this load, the pass takes 11.3 ms instead of 10.7 ms)
         s_bsec[tid] = out.sector[t] * R;
         rowhit = out.rowhit + (int64_t)t * R;
         S.x = rs.sx[r0];
