@@ -36,6 +36,7 @@ struct Workspace {
   GridDesc* desc;
   uint32_t* chunk_base;      // [nb+1] first neighbour-finder CTA of every bucket
   uint32_t* chunk_bucket;    // [ceil(N/128)+nb] bucket of every neighbour-finder CTA
+  uint4* chunk_reg;          // [ceil(N/128)+nb][2] per neighbour-finder CTA: candidate ranges (kD0, kD1, kU0, kU1); (first cluster, bucket end, bucket, -)
   uint32_t* cell_start;
   uint32_t* rank;            // aliases spos_by_orig (a1 only)
   float2* syz;
@@ -152,6 +153,7 @@ Workspace layout(const tpcHandle* h, int64_t N, int64_t capT, char* base) {
   w.desc = (GridDesc*)take(sizeof(GridDesc) * nb);
   w.chunk_base = (uint32_t*)take(4 * (size_t)(nb + 1));
   w.chunk_bucket = (uint32_t*)take(4 * (size_t)(ceilDiv(Nn, NF_THREADS) + nb));
+  w.chunk_reg = (uint4*)take(32 * (size_t)(ceilDiv(Nn, NF_THREADS) + nb));
   w.cell_start = (uint32_t*)take(4 * (size_t)(cc + 1));
   w.spos_by_orig = (int32_t*)take(4 * (size_t)Nn);
   w.rank = (uint32_t*)w.spos_by_orig;
@@ -426,7 +428,9 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
     // one CTA per chunk of NF_THREADS clusters of one bucket; the exact CTA count is on the device (chunk_base[nb])
     const int64_t max_chunks = ceilDiv(N, NF_THREADS) + nb;
     chunkFill<<<(unsigned)ceilDiv(max_chunks, 256), 256, 0, st>>>(w.chunk_base, nb, max_chunks, w.chunk_bucket, cnt); TPC_LAUNCHED("chunkFill");
-    neighbourFinder<<<(unsigned)max_chunks, NF_THREADS, 0, st>>>(w.chunk_base, w.chunk_bucket, P, T, w.desc, w.cell_start,
+    chunkRegions<<<(unsigned)ceilDiv(max_chunks * 32, 256), 256, 0, st>>>(w.chunk_base, w.chunk_bucket, P, T, w.desc, w.cell_start,
+                                                                          w.syz, w.chunk_reg, cnt); TPC_LAUNCHED("chunkRegions");
+    neighbourFinder<<<(unsigned)max_chunks, NF_THREADS, 0, st>>>(w.chunk_base, w.chunk_bucket, w.chunk_reg, P, T, w.desc, w.cell_start,
                                                                                     w.syz, w.s2o, w.lup, w.ldn, cnt); TPC_LAUNCHED("neighbourFinder");
   }
   stage(2);

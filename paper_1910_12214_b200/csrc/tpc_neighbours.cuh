@@ -156,8 +156,67 @@ __global__ void __launch_bounds__(256) chunkFill(const uint32_t* __restrict__ ch
   chunk_bucket[c] = (uint32_t)lo;
 }
 
+// One warp per neighbour-finder CTA (chunk of NF_THREADS consecutive sorted clusters of one bucket), after chunkFill: the
+// z extent of the chunk and from it the two CONTIGUOUS candidate ranges of the sorted array, [kD0, kD1) on the row below and
+// [kU0, kU1) on the row above (all zero when the row has no row pair).  Inside neighbourFinder this was a block reduction
+// and four dependent cell-table loads in front of the staging copies: three memory latencies per CTA before its first
+// useful instruction (16 % of the kernel's stall samples sat in that prologue, profiles/r2e).  Here it is throughput
+// work, and the CTA starts with two 16-byte loads: the ranges, and (first cluster, end of the bucket, bucket).
+__global__ void __launch_bounds__(256) chunkRegions(const uint32_t* __restrict__ chunk_base,
+                                                    const uint32_t* __restrict__ chunk_bucket, DevParams P, RowTables T,
+                                                    const GridDesc* __restrict__ desc,
+                                                    const uint32_t* __restrict__ cell_start,
+                                                    const float2* __restrict__ syz, uint4* __restrict__ chunk_reg,
+                                                    const int64_t* __restrict__ cnt) {
+  if (cnt[CNT_ERROR] != 0) return;
+  const int nb = P.n_buckets;
+  const uint32_t c = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;      // warp = chunk
+  const int lane = threadIdx.x & 31;
+  if (c >= __ldg(chunk_base + nb)) return;
+  const int b = (int)__ldg(chunk_bucket + c);
+  const GridDesc Gh = desc[b];
+  const int r = b % P.n_rows;
+  const int ru = T.up_row[r], rd = T.dn_row[r];
+  const uint32_t p0 = Gh.lo + (c - __ldg(chunk_base + b)) * NF_THREADS, pend = Gh.lo + Gh.n;
+  if (lane == 0) chunk_reg[2 * c + 1] = make_uint4(p0, pend, (uint32_t)b, 0u);
+  if (ru < 0 || rd < 0) {
+    if (lane == 0) chunk_reg[2 * c] = make_uint4(0u, 0u, 0u, 0u);
+    return;
+  }
+  // the descriptors of the two neighbour rows are requested together with the clusters (one memory latency, not two)
+  const GridDesc Gu = desc[b - r + ru], Gd = desc[b - r + rd];
+  float zlo = 3.0e38f, zhi = -3.0e38f;
+#pragma unroll
+  for (int k = 0; k < NF_THREADS / 32; ++k) {
+    const uint32_t p = p0 + k * 32 + lane;
+    if (p < pend) { const float z = syz[p].y; zlo = fminf(zlo, z); zhi = fmaxf(zhi, z); }
+  }
+  for (int d = 16; d > 0; d >>= 1) {
+    zlo = fminf(zlo, __shfl_xor_sync(0xffffffffu, zlo, d));
+    zhi = fmaxf(zhi, __shfl_xor_sync(0xffffffffu, zhi, d));
+  }
+  if (lane != 0) return;
+  const float xr = T.row_x[r];
+  const float dxu = T.row_x[ru] - xr, dxd = xr - T.row_x[rd];
+  const float wzu = P.area_z * dxu, wzd = P.area_z * dxd;
+  uint32_t kD0 = 0, kD1 = 0, kU0 = 0, kU1 = 0;
+  const float s = 1e-5f * (fmaxf(fabsf(zlo), fabsf(zhi)) + wzu + wzd) + 1e-6f;
+  if (Gd.n) {
+    const int a = cellCoord((zlo - wzd) - s, Gd.z0, Gd.inv_e, Gd.nz), e = cellCoord((zhi + wzd) + s, Gd.z0, Gd.inv_e, Gd.nz);
+    kD0 = __ldg(cell_start + Gd.cell_base + a * Gd.ny);
+    kD1 = __ldg(cell_start + Gd.cell_base + (e + 1) * Gd.ny);
+  }
+  if (Gu.n) {
+    const int a = cellCoord((zlo - wzu) - s, Gu.z0, Gu.inv_e, Gu.nz), e = cellCoord((zhi + wzu) + s, Gu.z0, Gu.inv_e, Gu.nz);
+    kU0 = __ldg(cell_start + Gu.cell_base + a * Gu.ny);
+    kU1 = __ldg(cell_start + Gu.cell_base + (e + 1) * Gu.ny);
+  }
+  chunk_reg[2 * c] = make_uint4(kD0, kD1, kU0, kU1);
+}
+
 __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __restrict__ chunk_base,
-                                                              const uint32_t* __restrict__ chunk_bucket, DevParams P, RowTables T,
+                                                              const uint32_t* __restrict__ chunk_bucket,
+                                                              const uint4* __restrict__ chunk_reg, DevParams P, RowTables T,
                                                               const GridDesc* __restrict__ desc,
                                                               const uint32_t* __restrict__ cell_start,
                                                               const float2* __restrict__ syz,
@@ -170,17 +229,16 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
   __shared__ uint8_t snD[NF_THREADS], snU[NF_THREADS];
   ushort2* srow = reinterpret_cast<ushort2*>(it_dev);   // cell-row ranges: only live while the lists are built
   static_assert(sizeof(float) * NF_ITEMS * NF_UB >= sizeof(ushort2) * NF_ROWS * NF_THREADS, "srow aliases it_dev");
-  __shared__ float red[2][NF_THREADS / 32];
   __shared__ uint32_t sscan[33];
   __shared__ uint32_t sm_T;
   if (cnt[CNT_ERROR] != 0) return;
   const int tid = threadIdx.x;
   const int nb = P.n_buckets;
   if (blockIdx.x >= __ldg(chunk_base + nb)) return;
-  const int b = (int)__ldg(chunk_bucket + blockIdx.x);
-  const GridDesc Gh = desc[b];
-  const uint32_t p = Gh.lo + (blockIdx.x - __ldg(chunk_base + b)) * NF_THREADS + tid;
-  const bool valid = p < Gh.lo + Gh.n;
+  const uint4 kr = __ldg(chunk_reg + 2 * blockIdx.x), kq = __ldg(chunk_reg + 2 * blockIdx.x + 1);
+  const int b = (int)kq.z;
+  const uint32_t p = kq.x + tid;
+  const bool valid = p < kq.y;
   const int r = b % P.n_rows;
   const int ru = T.up_row[r], rd = T.dn_row[r];
   if (ru < 0 || rd < 0) {   // no row pair (first / last rows, dead rows): no links (uniform branch)
@@ -195,31 +253,8 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
   const GridDesc Gu = desc[b - r + ru], Gd = desc[b - r + rd];
   const float2 h = valid ? syz[p] : make_float2(0.0f, 0.0f);
 
-  // ---- z extent of the chunk -> contiguous candidate regions ----
-  float zlo = valid ? h.y : 3.0e38f, zhi = valid ? h.y : -3.0e38f;
-  for (int d = 16; d > 0; d >>= 1) {
-    zlo = fminf(zlo, __shfl_xor_sync(0xffffffffu, zlo, d));
-    zhi = fmaxf(zhi, __shfl_xor_sync(0xffffffffu, zhi, d));
-  }
-  if ((tid & 31) == 0) { red[0][tid >> 5] = zlo; red[1][tid >> 5] = zhi; }
-  __syncthreads();
-  zlo = red[0][0]; zhi = red[1][0];
-#pragma unroll
-  for (int w = 1; w < NF_THREADS / 32; ++w) { zlo = fminf(zlo, red[0][w]); zhi = fmaxf(zhi, red[1][w]); }
-  uint32_t kD0 = 0, kD1 = 0, kU0 = 0, kU1 = 0;
-  {
-    const float s = 1e-5f * (fmaxf(fabsf(zlo), fabsf(zhi)) + wzu + wzd) + 1e-6f;
-    if (Gd.n) {
-      const int a = cellCoord((zlo - wzd) - s, Gd.z0, Gd.inv_e, Gd.nz), e = cellCoord((zhi + wzd) + s, Gd.z0, Gd.inv_e, Gd.nz);
-      kD0 = __ldg(cell_start + Gd.cell_base + a * Gd.ny);
-      kD1 = __ldg(cell_start + Gd.cell_base + (e + 1) * Gd.ny);
-    }
-    if (Gu.n) {
-      const int a = cellCoord((zlo - wzu) - s, Gu.z0, Gu.inv_e, Gu.nz), e = cellCoord((zhi + wzu) + s, Gu.z0, Gu.inv_e, Gu.nz);
-      kU0 = __ldg(cell_start + Gu.cell_base + a * Gu.ny);
-      kU1 = __ldg(cell_start + Gu.cell_base + (e + 1) * Gu.ny);
-    }
-  }
+  // ---- the contiguous candidate regions of the chunk: computed by chunkRegions ----
+  const uint32_t kD0 = kr.x, kD1 = kr.y, kU0 = kr.z, kU1 = kr.w;
   if (kD1 - kD0 > NF_REGION || kU1 - kU0 > NF_REGION) {     // regions too large for shared memory (uniform branch)
     if (valid) neighbourSlow(p, h, Gu, Gd, cell_start, syz, s2o, iu, id, wyu, wzu, wyd, wzd, P.link_dev2_max, lup, ldn);
     return;
