@@ -32,11 +32,11 @@ constexpr int NF_REGION = NF_REGION_;     // staged candidates per side
 #define NF_LIST_ 32
 #endif
 #ifndef NF_ITEMS_
-#define NF_ITEMS_ 640
+#define NF_ITEMS_ 512
 #endif
 constexpr int NF_LIST = NF_LIST_;  // window candidates kept per thread and side (<= 32: packed item code)
 #ifndef NF_UB_
-#define NF_UB_ 2
+#define NF_UB_ 4
 #endif
 constexpr int NF_UB = NF_UB_;          // u's per item (register blocking of the pair loop)
 constexpr int NF_ITEMS = NF_ITEMS_; // items per CTA and round
@@ -45,7 +45,7 @@ constexpr int NF_ITEMS = NF_ITEMS_; // items per CTA and round
 #endif
 constexpr int NF_GUNROLL = NF_GUNROLL_;
 #ifndef NF_DUNROLL_
-#define NF_DUNROLL_ 4
+#define NF_DUNROLL_ 2
 #endif
 constexpr int NF_DUNROLL = NF_DUNROLL_;   // unrolling of the D loop of the pair phase
 constexpr int NF_ROWS = 6;         // cell rows of a window whose ranges are staged (more: slow path)
@@ -106,7 +106,8 @@ __device__ __noinline__ void neighbourSlow(uint32_t p, float2 h, const GridDesc&
 // NF_LIST + 1 when the window spans more than NF_ROWS cell rows (the caller then takes the slow path).
 __device__ __forceinline__ int gatherWindow(const GridDesc& G, const uint32_t* __restrict__ cell_start, const float2* reg,
                                             uint32_t k0, float yc, float zc, float wy, float wz, uint16_t* list,
-                                            ushort2* rows, int tid) {
+                                            ushort2* rows, int tid) {      // rows: the warp's own [NF_ROWS][32] slice
+  const int lane = tid & 31;
   if (G.n == 0) return 0;
   const float sy = 1e-5f * (fabsf(yc) + wy) + 1e-6f;
   const float sz = 1e-5f * (fabsf(zc) + wz) + 1e-6f;
@@ -123,22 +124,29 @@ __device__ __forceinline__ int gatherWindow(const GridDesc& G, const uint32_t* _
     const uint32_t* c = cs + (r < nr ? r : 0) * G.ny;
     ra[r] = __ldg(c); rb[r] = __ldg(c + span);
   }
+  // the ranges are kept as BYTE offsets into the region (8 bytes per cluster; at most 8 * NF_REGION: 16 bits)
 #pragma unroll
-  for (int r = 0; r < NF_ROWS; ++r) rows[r * NF_THREADS + tid] = make_ushort2((uint16_t)(ra[r] - k0), (uint16_t)(rb[r] - k0));
-  int n = 0;
+  for (int r = 0; r < NF_ROWS; ++r) rows[r * 32 + lane] = make_ushort2((uint16_t)((ra[r] - k0) << 3), (uint16_t)((rb[r] - k0) << 3));
+  // The loop body is eight instructions per candidate: one shared load, one packed subtraction (FADD2: each half is the
+  // IEEE c - centre, as c + (-centre)), two compares, the store of the byte offset to the slot the cursor points at (clamped
+  // to the spare row NF_LIST: no branch), the cursor advanced by one row when the candidate passes.  The cursor is a
+  // shared-memory ADDRESS (not a count times a stride plus a base: that was seven more instructions, r2e), the count comes
+  // out of it at the end.
+  const uint32_t l0 = (uint32_t)__cvta_generic_to_shared(list + tid);
+  const uint32_t lmax = l0 + NF_LIST * NF_THREADS * (uint32_t)sizeof(uint16_t);
+  uint32_t la = l0;
+  const float2 nc = make_float2(-yc, -zc);
   for (int r = 0; r < nr; ++r) {
-    const ushort2 v = rows[r * NF_THREADS + tid];
+    const ushort2 v = rows[r * 32 + lane];
 #pragma unroll NF_GUNROLL
-    for (uint32_t k = v.x; k < v.y; ++k) {
-      const float2 c = reg[k];
-      const bool pass = fabsf(c.x - yc) <= wy && fabsf(c.y - zc) <= wz;
-      list[min(n, NF_LIST) * NF_THREADS + tid] = (uint16_t)(k << 3);     // byte offset into the region (the pair loop
-                                                                         // adds it to the base: no multiply there); row
-                                                                         // NF_LIST is a spare: no branch needed
-      n += pass ? 1 : 0;
+    for (uint32_t k8 = v.x; k8 < v.y; k8 += 8) {
+      const float2 d = __fadd2_rn(nfAt(reg, k8), nc);
+      const bool pass = (fabsf(d.x) <= wy) & (fabsf(d.y) <= wz);
+      asm volatile("st.shared.u16 [%0], %1;" ::"r"(min(la, lmax)), "h"((uint16_t)k8) : "memory");
+      if (pass) la += NF_THREADS * (uint32_t)sizeof(uint16_t);
     }
   }
-  return n;
+  return (int)((la - l0) / (NF_THREADS * (uint32_t)sizeof(uint16_t)));
 }
 
 // thread per neighbour-finder CTA: its bucket (largest b with chunk_base[b] <= cta), so that the CTAs themselves start
@@ -224,15 +232,19 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
                                                               int32_t* __restrict__ ldn, const int64_t* __restrict__ cnt) {
   __shared__ float2 sD[NF_REGION], sU[NF_REGION], sH[NF_THREADS];
   __shared__ uint16_t dl[(NF_LIST + 1) * NF_THREADS], ul[(NF_LIST + 1) * NF_THREADS];
-  __shared__ uint16_t it[NF_ITEMS], it_d[NF_ITEMS * NF_UB];
+  __shared__ uint16_t it[NF_ITEMS];
   __shared__ float it_dev[NF_ITEMS * NF_UB];
   __shared__ uint8_t snD[NF_THREADS], snU[NF_THREADS];
-  ushort2* srow = reinterpret_cast<ushort2*>(it_dev);   // cell-row ranges: only live while the lists are built
-  static_assert(sizeof(float) * NF_ITEMS * NF_UB >= sizeof(ushort2) * NF_ROWS * NF_THREADS, "srow aliases it_dev");
-  __shared__ uint32_t sscan[33];
-  __shared__ uint32_t sm_T;
+  // From the staging barrier on every warp works for itself: its 32 clusters, their lists, its own slice of the item
+  // arrays (NF_WITEMS items), warp scans and __syncwarp -- no block barrier in the rounds (three per round and a block scan
+  // before: a tenth of the kernel's stall samples, profiles/r2e).
+  constexpr int NF_WITEMS = NF_ITEMS / (NF_THREADS / 32);
+  static_assert(NF_WITEMS >= 32 / NF_UB + 1, "a cluster's items must fit a warp's slice");
+  static_assert(sizeof(float) * NF_WITEMS * NF_UB >= sizeof(ushort2) * NF_ROWS * 32, "srow aliases the warp's slice of it_dev");
   if (cnt[CNT_ERROR] != 0) return;
   const int tid = threadIdx.x;
+  const int lane = tid & 31, wbase = (tid >> 5) * NF_WITEMS;
+  ushort2* srow = reinterpret_cast<ushort2*>(it_dev + wbase * NF_UB);   // cell-row ranges: only live while the lists are built
   const int nb = P.n_buckets;
   if (blockIdx.x >= __ldg(chunk_base + nb)) return;
   const uint4 kr = __ldg(chunk_reg + 2 * blockIdx.x), kq = __ldg(chunk_reg + 2 * blockIdx.x + 1);
@@ -279,23 +291,22 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
   bool have = false, tied = false;
   float best = 0.0f;
   uint32_t bu = 0, bd = 0;
-  // The item list holds NF_ITEMS (h,u) items; CTAs with more run the pair phase in several rounds.
+  // A warp's item list holds NF_WITEMS (h,u) items; warps with more run the pair phase in several rounds.
+  __syncwarp();                                     // the lists and counts of the warp's clusters are written
   for (;;) {
-    uint32_t total;
     const uint32_t mine = pending ? (uint32_t)((nU + NF_UB - 1) / NF_UB) : 0u;     // items: groups of NF_UB u's
-    if (tid == 0) sm_T = 0;
-    const uint32_t base = blockExclusiveScan(mine, sscan, &total);
-    if (total == 0) break;                          // uniform
-    const bool now = pending && base + mine <= NF_ITEMS;
-    if (now) {
-      for (uint32_t a = 0; a < mine; ++a) it[base + a] = (uint16_t)(tid * 32 + a * NF_UB);
-      atomicMax(&sm_T, base + mine);
-    }
-    __syncthreads();
-    const uint32_t Tn = sm_T;                       // end of the last thread that fitted this round
+    const uint32_t inc = warpInclusiveScan(mine);
+    if (__shfl_sync(0xffffffffu, inc, 31) == 0) break;      // uniform over the warp
+    const uint32_t base = inc - mine;
+    const bool now = pending && base + mine <= NF_WITEMS;   // the clusters that fit are a prefix: no holes in the list
+    if (now)
+      for (uint32_t a = 0; a < mine; ++a) it[wbase + base + a] = (uint16_t)(tid * 32 + a * NF_UB);
+    const uint32_t Tn = __reduce_max_sync(0xffffffffu, now ? base + mine : 0u);    // end of the last cluster that fitted
+    __syncwarp();
     // ---- pair phase: one item = (h, NF_UB consecutive u's of its list); loop over the D list of h.
     //      The down slopes are computed once per d and used for all u's of the item (register blocking).
-    for (uint32_t i = tid; i < Tn; i += NF_THREADS) {
+    for (uint32_t iw = lane; iw < Tn; iw += 32) {
+      const uint32_t i = wbase + iw;
       const uint32_t e = it[i];
       const int hl = e >> 5, a0 = e & 31;
       const float2 hh = sH[hl];
@@ -306,16 +317,18 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
       // FFMA2 even with --fmad=false and explicit .rn (measured), so that pattern is never
       // written: the differences of two slopes (products) are scalar adds, and only add -> mul and mul -> scalar add
       // chains are packed (tests/test_build_flags.py checks the SASS of the library for FFMA2).
+      // The pair loop keeps only the MINIMUM of Dev over the D list of every (h, u) (one FMNMX per pair; the running
+      // argmin and the tie flag were four instructions per pair, 93 pairs per cluster).  Which d it was is found
+      // afterwards, by the cluster's own thread, for the winning u alone: the same arithmetic once more over its D list,
+      // looking for the value (a second d with it = an exact tie, redone by neighbourSlow with the full key, R6).
       float2 tu[NF_UB];
       float bdev[NF_UB];
-      uint32_t bdi[NF_UB];
-      bool tie[NF_UB];
       const float2 iu2 = make_float2(iu, iu), id2 = make_float2(id, id), nh = make_float2(-hh.x, -hh.y);
 #pragma unroll
       for (int q = 0; q < NF_UB; ++q) {
         const float2 uu = nfAt(sU, ul[min(a0 + q, nu - 1) * NF_THREADS + hl]);     // a short last group repeats its last u
         tu[q] = __fmul2_rn(__fadd2_rn(uu, nh), iu2);                         // ((y_u - y_h) * iu, (z_u - z_h) * iu)
-        bdev[q] = __int_as_float(0x7f800000); bdi[q] = 0; tie[q] = false;
+        bdev[q] = __int_as_float(0x7f800000);
       }
       const int n = snD[hl];
 #pragma unroll NF_DUNROLL
@@ -328,43 +341,49 @@ __global__ void __launch_bounds__(NF_THREADS) neighbourFinder(const uint32_t* __
           const float2 e = make_float2(tu[q].x + ntd.x, tu[q].y + ntd.y);    // (tyu - tyd, tzu - tzd): scalar, see above
           const float2 m = __fmul2_rn(e, e);
           const float dev = m.x + m.y;
-          // Window slopes are bounded by area_y/area_z, so dev is finite: +inf is a safe "none yet".  The minimum
-          // is tracked with selects (no branch).  An exact tie with the running minimum (duplicated clusters) is
-          // only flagged: such a cluster is redone by neighbourSlow with the full key (R6).
-          tie[q] = tie[q] || dev == bdev[q];
-          const bool better = dev < bdev[q];
-          bdi[q] = better ? di : bdi[q];
-          bdev[q] = better ? dev : bdev[q];
+          // Window slopes are bounded by area_y/area_z, so dev is finite: +inf is a safe "none yet".
+          bdev[q] = fminf(bdev[q], dev);
         }
       }
 #pragma unroll
-      for (int q = 0; q < NF_UB; ++q) {
-        it_dev[i * NF_UB + q] = bdev[q];
-        it_d[i * NF_UB + q] = (uint16_t)(bdi[q] | (tie[q] ? 0x8000u : 0u));
-      }
+      for (int q = 0; q < NF_UB; ++q) it_dev[i * NF_UB + q] = bdev[q];
     }
-    __syncthreads();
+    __syncwarp();
     // ---- per-cluster reduction over its own items, full key (Dev, orig u, orig d) ----
     if (now) {
-      // branch-free: the minimum over the cluster's own u's; an exact tie with the running minimum, between two u's or
-      // inside the D loop of the winning u, only raises `tied` (the cluster is then redone by neighbourSlow, R6)
+      // branch-free: the minimum over the cluster's own u's; an exact tie between two u's only raises `tied` (the
+      // cluster is then redone by neighbourSlow, R6)
       float bst = __int_as_float(0x7f800000);
       int ba = 0;
-      uint32_t bcode = 0;
       for (int a = 0; a < nU; ++a) {
-        const float dev = it_dev[base * NF_UB + a];
-        const uint32_t dcode = it_d[base * NF_UB + a];
-        tied = tied || dev == bst || (dev < bst && (dcode & 0x8000u) != 0u);
+        const float dev = it_dev[(wbase + base) * NF_UB + a];
+        tied = tied || dev == bst;
         const bool better = dev < bst;
         ba = better ? a : ba;
-        bcode = better ? dcode : bcode;
         bst = better ? dev : bst;
       }
+      // the d of the winning u: Dev of (u*, d) recomputed with the pair loop's own operations, bit for bit
+      const uint32_t ucode = ul[ba * NF_THREADS + tid];
+      uint32_t bcode = 0, hits = 0;
+      {
+        const float2 iu2 = make_float2(iu, iu), id2 = make_float2(id, id), nh = make_float2(-h.x, -h.y);
+        const float2 tu = __fmul2_rn(__fadd2_rn(nfAt(sU, ucode), nh), iu2);
+        for (int j = nD - 1; j >= 0; --j) {           // downwards: the last match kept is the first of the list
+          const uint32_t di = dl[j * NF_THREADS + tid];
+          const float2 ntd = __fmul2_rn(__fadd2_rn(nfAt(sD, di), nh), id2);
+          const float2 e = make_float2(tu.x + ntd.x, tu.y + ntd.y);
+          const float2 m = __fmul2_rn(e, e);
+          const bool eq = m.x + m.y == bst;
+          bcode = eq ? di : bcode;
+          hits += eq ? 1u : 0u;
+        }
+      }
+      tied = tied || hits != 1u;                    // two d's at the minimum: a tie; none cannot happen (then: slow path)
       have = true; best = bst;                      // nU >= 1 here, and every dev is finite
-      bu = kU0 + (ul[ba * NF_THREADS + tid] >> 3); bd = kD0 + ((bcode & 0x7fffu) >> 3);
+      bu = kU0 + (ucode >> 3); bd = kD0 + (bcode >> 3);
       pending = false;
     }
-    __syncthreads();                                // the item arrays are rewritten in the next round
+    __syncwarp();                                   // the item arrays are rewritten in the next round
   }
   if (!valid) return;
   if (slow || tied) {
