@@ -141,9 +141,12 @@ __device__ __forceinline__ int gatherWindow(const GridDesc& G, const uint32_t* _
 #pragma unroll NF_GUNROLL
     for (uint32_t k8 = v.x; k8 < v.y; k8 += 8) {
       const float2 d = __fadd2_rn(nfAt(reg, k8), nc);
-      const bool pass = (fabsf(d.x) <= wy) & (fabsf(d.y) <= wz);
       asm volatile("st.shared.u16 [%0], %1;" ::"r"(min(la, lmax)), "h"((uint16_t)k8) : "memory");
-      if (pass) la += NF_THREADS * (uint32_t)sizeof(uint16_t);
+      // pass = |dy| <= wy && |dz| <= wz (false for NaN); the cursor moves on under that predicate: three instructions
+      asm("{\n\t.reg .pred p;\n\t.reg .f32 a, b;\n\tabs.f32 a, %1;\n\tabs.f32 b, %2;\n\tsetp.le.f32 p, a, %3;\n\t"
+          "setp.le.and.f32 p, b, %4, p;\n\t@p add.u32 %0, %0, %5;\n\t}"
+          : "+r"(la)
+          : "f"(d.x), "f"(d.y), "f"(wy), "f"(wz), "n"(NF_THREADS * (int)sizeof(uint16_t)));
     }
   }
   return (int)((la - l0) / (NF_THREADS * (uint32_t)sizeof(uint16_t)));
