@@ -58,8 +58,8 @@ def test_default_params_are_table_p():
 
 def test_error_strings_and_argument_checks_without_a_device():
     lib = tpc.load_library()
-    for code in (0, -1, -2, -3, -4, -5, -6):
-        assert len(lib.tpcErrorString(code)) > 1
+    for code in (0, -1, -2, -3, -4, -5, -6, -7, -8):
+        assert len(lib.tpcErrorString(code)) > 1 and lib.tpcErrorString(code) != lib.tpcErrorString(-99)
     assert lib.tpcDefaultParams(None) == tpc.TPC_ERR_INVALID_ARG
     h = ctypes.c_void_p()
     p = tpc.tpcDefaultParams()
@@ -68,6 +68,15 @@ def test_error_strings_and_argument_checks_without_a_device():
     assert lib.tpcCreate(ctypes.byref(h), None, ctypes.byref(p), 0) == tpc.TPC_ERR_INVALID_ARG
     bad = tpc.tpcGeometry(36, 2, row_x.ctypes.data, None, None, 0.5, 0.176, -250.0, 250.0)      # n_rows < 3
     assert lib.tpcCreate(ctypes.byref(h), ctypes.byref(bad), ctypes.byref(p), 0) == tpc.TPC_ERR_INVALID_ARG
+    bad = tpc.tpcGeometry(65, 152, row_x.ctypes.data, None, None, 0.5, 0.176, -250.0, 250.0)    # n_sectors > 64 (header)
+    assert lib.tpcCreate(ctypes.byref(h), ctypes.byref(bad), ctypes.byref(p), 0) == tpc.TPC_ERR_INVALID_ARG
+    # the allocation-free entry point checks its arguments before it touches the device
+    assert lib.tpcNoAllocMaxClusters() == 1 << 24
+    assert lib.tpcStartHitsNoAlloc(0, (1 << 24) + 1, 8, 8, 8, 1, 8, None) == tpc.TPC_ERR_NOALLOC_LIMIT
+    assert b"TPC_NOALLOC_MAX_CLUSTERS" in lib.tpcNoAllocLastError()
+    assert lib.tpcStartHitsNoAlloc(0, 10, None, 8, 8, 1, 8, None) == tpc.TPC_ERR_INVALID_ARG
+    assert lib.tpcStartHitsNoAlloc(0, -1, 8, 8, 8, 1, 8, None) == tpc.TPC_ERR_INVALID_ARG
+    assert lib.tpcNoAllocSetup(-1) == tpc.TPC_ERR_INVALID_ARG
     rev = row_x[::-1].copy()                                                                     # not increasing
     bad = tpc.tpcGeometry(36, 152, rev.ctypes.data, None, None, 0.5, 0.176, -250.0, 250.0)
     assert lib.tpcCreate(ctypes.byref(h), ctypes.byref(bad), ctypes.byref(p), 0) == tpc.TPC_ERR_INVALID_ARG
