@@ -58,8 +58,12 @@ _lib = None
 def _load():
     global _lib
     if _lib is None:
-        build()
-        L = ctypes.CDLL(_LIB)
+        # TPC_ORACLE_LIB: another build of the same source (tests/test_oracle_sanitized.py loads one made with
+        # -fsanitize=address,undefined); the arithmetic flags of that build are the test's business
+        override = os.environ.get("TPC_ORACLE_LIB")
+        if not override:
+            build()
+        L = ctypes.CDLL(override or _LIB)
         vp, i64, dbl, ci = ctypes.c_void_p, ctypes.c_int64, ctypes.c_double, ctypes.c_int
         L.orcDefaultParams.argtypes = [ctypes.POINTER(Params)]
         L.orcDefaultParams.restype = None
