@@ -92,7 +92,8 @@ struct tpcHandle {
   //   // 0..6 stage boundaries, 7/8 around the optional refit, 9/10 merger, 11/12 flags
   int profiling = 0;
   int launches = 0;
-  int gb_smem_cells = 24 * 1024;      // cells of a bucket whose histogram gridBuild keeps in shared memory (96 KB: two CTAs per SM)
+  int gb_smem_cells = 24 * 1024;      // cells of a bucket whose histogram gridBuild keeps in shared memory (96 KB)
+  int gb_smem_bytes = 220 * 1024;     // dynamic shared memory of gridBuild: the histogram and, behind it, the stage of the scatter
   int tc_grid[4] = {148, 148, 148, 148};   // persistent grids of the constructor passes: SMs x resident blocks
   bool pending = false;
   int64_t last_n = 0;
@@ -318,9 +319,14 @@ int tpcCreate(tpcHandle** out, const tpcGeometry* g, const tpcParams* p, int cud
       h->tc_grid[i] = sms * per_sm;
     }
   }
-  if (cudaFuncSetAttribute(gridBuild, cudaFuncAttributeMaxDynamicSharedMemorySize, 4 * h->gb_smem_cells) != cudaSuccess) {
+  if (cudaFuncSetAttribute(gridBuild, cudaFuncAttributeMaxDynamicSharedMemorySize, h->gb_smem_bytes) != cudaSuccess) {
     cudaGetLastError();
-    h->gb_smem_cells = 10 * 1024;     // 40 KB needs no opt-in
+    h->gb_smem_bytes = 4 * h->gb_smem_cells;      // the histogram alone: direct scatter
+    if (cudaFuncSetAttribute(gridBuild, cudaFuncAttributeMaxDynamicSharedMemorySize, h->gb_smem_bytes) != cudaSuccess) {
+      cudaGetLastError();
+      h->gb_smem_cells = 10 * 1024;     // 40 KB needs no opt-in
+      h->gb_smem_bytes = 4 * h->gb_smem_cells;
+    }
   }
   memset(h->h_cnt, 0, 8 * (CNT_COUNT + 1));
   *out = h;
@@ -418,9 +424,9 @@ int tpcRun(tpcHandle* h, const tpcClusters* in, tpcTracks* out, int64_t cap_trac
   // ---- a1 grid ----------------------------------------------------------------------------------
   gridSetup<<<1, 1024, 0, st>>>(in->row_offset, N, P, h->d_row_x, w.desc, w.chunk_base, NF_THREADS, cnt, cc); TPC_LAUNCHED("gridSetup");
   if (N > 0) {
-    gridBuild<<<(unsigned)nb, GB_THREADS, 4 * (size_t)h->gb_smem_cells, st>>>(in->row_offset, in->y, in->z, nb, w.desc, w.cell_start,
-                                                                              w.rank, w.syz, w.s2o, cnt, h->params.validate_input,
-                                                                              (uint32_t)h->gb_smem_cells); TPC_LAUNCHED("gridBuild");
+    gridBuild<<<(unsigned)nb, GB_THREADS, (size_t)h->gb_smem_bytes, st>>>(in->row_offset, in->y, in->z, nb, w.desc, w.cell_start,
+                                                                          w.rank, w.syz, w.s2o, cnt, h->params.validate_input,
+                                                                          (uint32_t)h->gb_smem_cells, (uint32_t)h->gb_smem_bytes); TPC_LAUNCHED("gridBuild");
   }
   stage(1);
   // ---- a2 neighbour finder ------------------------------------------------------------------------
