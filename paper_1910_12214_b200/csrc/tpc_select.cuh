@@ -153,37 +153,42 @@ __global__ void __launch_bounds__(128) selectEmit(TrackletStore tl, const unsign
   if (cnt[CNT_ERROR] != 0) return;
   const int64_t nT = min(cnt[CNT_N_START], tl.capT);
   const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= nT) return;
-  const unsigned long long sel = tsel[t];
-  if (!(sel & 1ull)) return;
-  const unsigned long long sc = tscan[t];
-  const int64_t k = (int64_t)(sc & 0xffffffffull);
-  const int64_t off = (int64_t)(sc >> 32);
-  if (k >= o.cap_tracks) return;
-  const int64_t capT = tl.capT, capK = o.cap_tracks;
-  o.tracklet[k] = (int32_t)t; o.sector[k] = tl.sector[t];
-  o.first_row[k] = kept_first[t]; o.last_row[k] = kept_last[t]; o.ncl[k] = (int32_t)(sel >> 32);
-  o.x[k] = tl.x[t]; o.chi2[k] = tl.chi2[t];
-#pragma unroll
-  for (int i = 0; i < 5; ++i) o.par[i * capK + k] = tl.par[i * capT + t];
-#pragma unroll
-  for (int i = 0; i < 15; ++i) o.cov[i * capK + k] = tl.cov[i * capT + t];
-  o.cl_offset[k] = (uint32_t)off;
-  const int kept = (int)(sel >> 32);
-  const int32_t* row = tl.rowhit + t * tl.n_rows + tl.first_row[t];      // compacted by selectCount
-  const int nk = (int)max((int64_t)0, min((int64_t)kept, o.cap_cl - off));      // entries that fit the output
-  int i = 0;
-  for (; i + 8 <= nk; i += 8) {       // eight independent row -> index gathers in flight
-    int32_t c[8];
-    uint32_t g[8];
-#pragma unroll
-    for (int q = 0; q < 8; ++q) c[q] = row[i + q];
-#pragma unroll
-    for (int q = 0; q < 8; ++q) g[q] = s2o[c[q]];
-#pragma unroll
-    for (int q = 0; q < 8; ++q) o.cl_index[off + i + q] = g[q];
+  const unsigned long long sel = t < nT ? tsel[t] : 0ull;
+  unsigned long long sc = 0ull;
+  bool track = (sel & 1ull) != 0ull;
+  if (track) {
+    sc = tscan[t];
+    if ((int64_t)(sc & 0xffffffffull) >= o.cap_tracks) track = false;
   }
-  for (; i < nk; ++i) o.cl_index[off + i] = s2o[row[i]];
+  const int64_t off = (int64_t)(sc >> 32);
+  const int kept = (int)(sel >> 32);
+  if (track) {        // the per-track values: one lane each (the ranks of a warp's tracks are consecutive)
+    const int64_t k = (int64_t)(sc & 0xffffffffull);
+    const int64_t capT = tl.capT, capK = o.cap_tracks;
+    o.tracklet[k] = (int32_t)t; o.sector[k] = tl.sector[t];
+    o.first_row[k] = kept_first[t]; o.last_row[k] = kept_last[t]; o.ncl[k] = kept;
+    o.x[k] = tl.x[t]; o.chi2[k] = tl.chi2[t];
+#pragma unroll
+    for (int i = 0; i < 5; ++i) o.par[i * capK + k] = tl.par[i * capT + t];
+#pragma unroll
+    for (int i = 0; i < 15; ++i) o.cov[i * capK + k] = tl.cov[i * capT + t];
+    o.cl_offset[k] = (uint32_t)off;
+  }
+  // The cluster lists: the WARP copies the list of each of its tracks together (about one tracklet in twelve is a track:
+  // with a thread per track three lanes of a warp were at work, each on its own run of 4-byte loads and stores).  Lane i
+  // takes entry i, i + 32, ...: the compacted row hits are read and the indices written as whole lines.
+  const int lane = threadIdx.x & 31;
+  const int32_t* row = track ? tl.rowhit + t * tl.n_rows + tl.first_row[t] : nullptr;      // compacted by selectCount
+  const int nk = track ? (int)max((int64_t)0, min((int64_t)kept, o.cap_cl - off)) : 0;     // entries that fit the output
+  unsigned todo = __ballot_sync(0xffffffffu, nk > 0);
+  while (todo) {
+    const int src = __ffs(todo) - 1;
+    todo &= todo - 1;
+    const int32_t* r = reinterpret_cast<const int32_t*>(__shfl_sync(0xffffffffu, (unsigned long long)(uintptr_t)row, src));
+    const int n = __shfl_sync(0xffffffffu, nk, src);
+    const int64_t o0 = __shfl_sync(0xffffffffu, (long long)off, src);
+    for (int i = lane; i < n; i += 32) o.cl_index[o0 + i] = s2o[r[i]];
+  }
 }
 
 // one thread: totals, closing CSR offset, capacity status.
