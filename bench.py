@@ -37,10 +37,10 @@ ALU_SMS = 148
 # `ncu --set full` capture named in "file".  They are cited constants (a number taken under a profiler is never a bench
 # value); every other configuration or seed reports "traffic": null.
 NCU_CAPTURE = {
-    (4, 5): {"file": "profiles/r2g_full_capture.md",
+    (4, 5): {"file": "profiles/r2h_full_capture.md",
              "a4_constructor": {"kernel": "constructUp + constructDown<0,0> + constructDown<0,1> + constructDown<1,0>",
-                                "warp_inst": 1.8539e10, "dram_bytes": 22041956000},
-             "a2_neighbours": {"kernel": "neighbourFinder", "warp_inst": 8.491e9, "dram_bytes": 1624440000}},
+                                "warp_inst": 1.8536e10, "dram_bytes": 22244717000},
+             "a2_neighbours": {"kernel": "neighbourFinder", "warp_inst": 8.491e9, "dram_bytes": 1624126000}},
 }
 STAGE_KERNEL = {"a1_grid": "gridBuild", "a2_neighbours": "neighbourFinder", "a3_cleaner_start": "cleanLinks",
                 "a4_constructor": "constructUp + constructDown<0,0> + constructDown<0,1> + constructDown<1,0> (the passes of the "
